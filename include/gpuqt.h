@@ -1,0 +1,163 @@
+/*
+ * gpuqt.h — C-ABI boundary of the B200-native GPUQT hot path (arXiv 1705.01387).
+ *
+ * One opaque handle owns a tight-binding Hamiltonian in sliced-ELL form on ONE GPU plus the state
+ * vectors of a batch of random-phase vectors.  Every arithmetic step of the path (SpMV, Chebyshev
+ * recurrences, commutator recursion, velocity apply, inner products, moment finalisation, Jackson
+ * damping and energy transform) runs in hand-written sm_100a CUDA kernels; the host side only
+ * validates, lays out memory, computes the N_p Bessel coefficients of one time step, and launches.
+ * There is no CPU fallback: without a CUDA device every compute call returns GPUQT_ERR_CUDA.
+ *
+ * Citations are PAPER.md:<line> (= /root/reference/PAPER.md at build time, the text of the paper)
+ * plus the equation.  Readings of silent points are marked [A#] and listed in DESIGN.md.
+ *
+ * Conventions
+ *   N        number of orbitals (sites);  K_max  max neighbours per row
+ *   batch    number of random vectors B processed together (B in {1, 2, 4, 8})
+ *   dE       energy scale "energy_max", H~ = H / dE  (PAPER.md:160 Eq. 19, :329)
+ *   hbar = 1
+ *   complex vectors cross the ABI as interleaved doubles (re, im):  [batch][N][2]
+ *   "host"   pointer to host memory (pageable or pinned);  "device" pointer to device memory
+ *
+ * Ownership: the caller owns every array it passes and the device workspace; gpuqt_create copies
+ * the host inputs and keeps no host pointer.  Results are written to caller-allocated buffers and
+ * are complete when the call returns (the call synchronises the stream).  gpuqt_destroy frees only
+ * the handle.
+ *
+ * Errors: every call returns a gpuqt_status (0 = ok, < 0 = error); nothing throws or aborts across
+ * the ABI; the handle stays valid after an error; gpuqt_last_error gives text.
+ *
+ * Threading: a handle is not thread-safe; all work is issued on the stream given at create.
+ */
+#ifndef GPUQT_H
+#define GPUQT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gpuqt_handle gpuqt_handle;
+
+typedef enum {
+    GPUQT_OK = 0,
+    GPUQT_ERR_ARG = -1,            /* null/negative/unsupported argument                          */
+    GPUQT_ERR_INDEX = -2,          /* neighbour count or index out of range  [A11]                */
+    GPUQT_ERR_NOT_HERMITIAN = -3,  /* H_nm != conj(H_mn) bit-exactly  [A10]                       */
+    GPUQT_ERR_SCALE = -4,          /* Gershgorin bound of H exceeds dE  [A9]        */
+    GPUQT_ERR_ENERGY = -5,         /* |E / dE| >= 1 in the transform  [A15]         */
+    GPUQT_ERR_STATE = -6,          /* call order / mode not enabled at create                     */
+    GPUQT_ERR_CUDA = -7,           /* CUDA runtime error or no device                             */
+    GPUQT_ERR_NOMEM = -8,          /* workspace too small or host allocation failed               */
+    GPUQT_ERR_POSITION = -9        /* |X_n - X_m| == box/2 on a non-zero hop: ambiguous image [A6]*/
+} gpuqt_status;
+
+/* modes (bit mask) — which branches gpuqt_evolve advances */
+#define GPUQT_MODE_VAC 1   /* a = U(t)^dagger phi, b = U(t)^dagger V phi       (Eq. 29)  [A1]     */
+#define GPUQT_MODE_MSD 2   /* psi = U(t) phi and chi = [X, U(t)] phi            (Eq. 30)  [A3]     */
+#define GPUQT_MODE_PSI 4   /* psi = U(t) phi alone (implied by MSD; plain time evolution)         */
+
+/* state selectors for gpuqt_get_state */
+#define GPUQT_STATE_PSI 0
+#define GPUQT_STATE_CHI 1
+#define GPUQT_STATE_VAC_A 2
+#define GPUQT_STATE_VAC_B 3
+
+/* kernel classes for gpuqt_kernel_stats */
+#define GPUQT_KERNEL_KPM_DOUBLING 0  /* fused SpMV + recurrence + 2 dots (DOS, MSD moments)       */
+#define GPUQT_KERNEL_KPM_LEFT 1      /* fused SpMV + recurrence + <phi_L|.> (VAC moments)         */
+#define GPUQT_KERNEL_EVOLVE 2        /* fused SpMV + recurrence + Bessel-weighted accumulate      */
+#define GPUQT_KERNEL_EVOLVE_MSD 3    /* the same for (psi, chi) with the [X,H~] walk fused in     */
+#define GPUQT_KERNEL_VELOCITY 4      /* V apply                                                   */
+#define GPUQT_KERNEL_CLASSES 5
+
+#define GPUQT_MAX_MOMENTS 16384
+
+/* Bytes of device workspace gpuqt_create needs for this problem (0 on invalid arguments).
+ * nnz_slots = number of sliced-ELL entries; pass 0 to use the upper bound ceil32(N) * K_max.    */
+size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes);
+
+/* Host-only validation of the four input data sets: argument sanity, index range
+ * [A11], bit-exact Hermiticity [A10], Gershgorin bound max_m(|U_m| + sum_k |H_mk|) <= dE [A9],
+ * unambiguous minimum image [A6].  Uses no GPU.  Same checks gpuqt_create runs.                  */
+int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index,
+                   const double* hop_re, const double* hop_im, const double* onsite,
+                   const double* x, double box_length, double energy_scale);
+
+/* Build the model on the GPU.
+ *   nbr_count  host [N]          number of neighbours of site m
+ *   nbr_index  host [N*K_max]    row-major, 0-based; slots >= count ignored  PAPER.md:244 [A11]
+ *   hop_re     host [N*K_max] or NULL => every hopping is -1
+ *   hop_im     host [N*K_max] or NULL => real-hopping variant
+ *   onsite     host [N] or NULL => 0
+ *   x          host [N]          transport-direction coordinate X_m          PAPER.md:271, Eq. 33
+ *   box_length length of the periodic box along x (<= 0: open boundary) and
+ *   volume     Omega, the two numbers of line 1 of position.in
+ *   energy_scale dE
+ *   batch      B in {1,2,4,8};  modes: GPUQT_MODE_* mask
+ *   workspace  device memory of at least gpuqt_workspace_bytes(...) bytes, 256-byte aligned,
+ *              owned by the caller and alive until gpuqt_destroy
+ *   cuda_stream a cudaStream_t (NULL = default stream)
+ * Storage: slices of 32 rows, column-major inside a slice, int32 columns, SoA fp64 hoppings
+ * (imaginary plane absent in the real variant); padding entries are (own row, 0.0).             */
+int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nbr_count,
+                 const int32_t* nbr_index, const double* hop_re, const double* hop_im,
+                 const double* onsite, const double* x, double box_length, double volume,
+                 double energy_scale, int32_t batch, int modes, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream);
+
+/* Load B random vectors (Eq. 13; generated by the caller [A7]) and reset time to 0:
+ * psi = phi, chi = 0, a = phi, b = V phi (Eq. 34).  phi: [batch][N][2].                          */
+int gpuqt_set_state(gpuqt_handle* h, const double* phi_host);
+int gpuqt_set_state_device(gpuqt_handle* h, const double* phi_device);
+
+/* C_n^DOS = <psi|T_n(H~)|psi>, n < n_moments (Eq. 28) at the current psi (= phi when
+ * called before any gpuqt_evolve).  out: host [batch][n_moments].  2 <= n_moments <= MAX.        */
+int gpuqt_dos_moments(gpuqt_handle* h, int32_t n_moments, double* out_host);
+
+/* One Chebyshev time step of N_p = order terms (Eq. 17-24) for every enabled
+ * branch:  psi <- U(dt) psi;  chi <- U(dt) chi + [X,U(dt)] psi  [A3];  a <- U(-dt) a,
+ * b <- U(-dt) b  [A1].  dt may differ from call to call and may be negative.
+ * order >= 1.                                                                                     */
+int gpuqt_evolve(gpuqt_handle* h, double dt, int32_t order);
+
+/* C_n^VAC(t) = Re <V a|T_n(H~)|b> (Eq. 29) at the current time; does not advance it.
+ * out: host [batch][n_moments].                                                                   */
+int gpuqt_vac(gpuqt_handle* h, int32_t n_moments, double* out_host);
+
+/* C_n^MSD(t) = <chi|T_n(H~)|chi> (Eq. 30) at the current time.                      */
+int gpuqt_msd(gpuqt_handle* h, int32_t n_moments, double* out_host);
+
+/* out[s][j] = 2 / (pi Omega dE sqrt(1 - E~_j^2)) sum_n g_n (2 - delta_n0) T_n(E~_j) C_n[s] with the
+ * Jackson damping g_n (PAPER.md:184-188 Eq. 25-27, :203 Eq. 31).  moments: host [n_sets][n_moments];
+ * energies: host [n_energies]; out: host [n_sets][n_energies].                                    */
+int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_moments,
+                        int32_t n_sets, const double* energies_host, int32_t n_energies,
+                        double* out_host);
+
+/* Copy a state back: host [batch][N][2].                                                          */
+int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host);
+
+/* Decode the device sliced-ELL table back to canonical padded row-major [N*K_max] arrays
+ * (padding = (own row, 0)); dx = minimum-image X_n - X_m as the kernels compute it [A6].
+ * Any output pointer may be NULL.  Used for the bit-exact indexing check.                         */
+int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, double* dx);
+
+/* The N_p Bessel coefficients of one step, host only:
+ * c_m = (2 - delta_0m) (-i sgn dt)^m J_m(dE |dt|), m < order   (Eq. 17).            */
+int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im);
+
+/* Accumulated device time (CUDA events on the handle's stream around each run of launches) and
+ * number of launches of one kernel class since the last reset.                                    */
+int gpuqt_kernel_stats(gpuqt_handle* h, int kernel_class, double* ms, int64_t* launches);
+int gpuqt_reset_stats(gpuqt_handle* h);
+
+const char* gpuqt_last_error(const gpuqt_handle* h);
+void gpuqt_destroy(gpuqt_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPUQT_H */

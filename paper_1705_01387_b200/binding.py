@@ -1,0 +1,213 @@
+"""Thin Python binding of the C-ABI in include/gpuqt.h (argument marshalling only).
+
+The functions below carry the same names as the C entry points; `GpuQT` is a small convenience
+object around one handle.  PyTorch is used for device memory (the workspace), pinned host buffers
+and the CUDA stream; every step of the path runs in libgpuqt.so's kernels.  There is no fallback:
+if the library is missing or no CUDA device is present the calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgpuqt.so")
+
+MODE_VAC, MODE_MSD, MODE_PSI = 1, 2, 4
+STATE_PSI, STATE_CHI, STATE_VAC_A, STATE_VAC_B = 0, 1, 2, 3
+KERNEL_KPM_DOUBLING, KERNEL_KPM_LEFT, KERNEL_EVOLVE, KERNEL_EVOLVE_MSD, KERNEL_VELOCITY = range(5)
+MAX_MOMENTS = 16384
+
+STATUS = {0: "GPUQT_OK", -1: "GPUQT_ERR_ARG", -2: "GPUQT_ERR_INDEX", -3: "GPUQT_ERR_NOT_HERMITIAN",
+          -4: "GPUQT_ERR_SCALE", -5: "GPUQT_ERR_ENERGY", -6: "GPUQT_ERR_STATE", -7: "GPUQT_ERR_CUDA",
+          -8: "GPUQT_ERR_NOMEM", -9: "GPUQT_ERR_POSITION"}
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+_model_args = [C.c_int64, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp, C.c_double]
+
+_SIGNATURES = {
+    "gpuqt_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int32, C.c_int, C.c_int32, C.c_int]),
+    "gpuqt_validate": (C.c_int, _model_args + [C.c_double]),
+    "gpuqt_create": (C.c_int, [C.POINTER(C.c_void_p)] + _model_args + [C.c_double, C.c_double, C.c_int32, C.c_int,
+                                                                       C.c_void_p, C.c_size_t, C.c_void_p]),
+    "gpuqt_set_state": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "gpuqt_set_state_device": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "gpuqt_dos_moments": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
+    "gpuqt_evolve": (C.c_int, [C.c_void_p, C.c_double, C.c_int32]),
+    "gpuqt_vac": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
+    "gpuqt_msd": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
+    "gpuqt_kpm_transform": (C.c_int, [C.c_void_p, _dp, C.c_int32, C.c_int32, _dp, C.c_int32, _dp]),
+    "gpuqt_get_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "gpuqt_get_table": (C.c_int, [C.c_void_p, _ip, _dp, _dp, _dp]),
+    "gpuqt_bessel_coeffs": (C.c_int, [C.c_double, C.c_double, C.c_int32, _dp, _dp]),
+    "gpuqt_kernel_stats": (C.c_int, [C.c_void_p, C.c_int, _dp, C.POINTER(C.c_int64)]),
+    "gpuqt_reset_stats": (C.c_int, [C.c_void_p]),
+    "gpuqt_last_error": (C.c_char_p, [C.c_void_p]),
+    "gpuqt_destroy": (None, [C.c_void_p]),
+}
+
+_lib = None
+
+
+def load():
+    """Load libgpuqt.so (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1705_01387_b200.build` "
+                               "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def __getattr__(name):          # gpuqt_* entry points under their C names
+    if name in _SIGNATURES:
+        return getattr(load(), name)
+    raise AttributeError(name)
+
+
+class GpuqtError(RuntimeError):
+    def __init__(self, status, what, detail=""):
+        self.status = status
+        super().__init__(f"{what}: {STATUS.get(status, status)} {detail}".strip())
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _i(a):
+    return None if a is None else a.ctypes.data_as(_ip)
+
+
+def _model_tuple(model):
+    return (C.c_int64(model.N), C.c_int32(model.K), _i(model.nbr_count), _i(model.nbr_index),
+            _d(model.hop_re), _d(model.hop_im), _d(model.onsite), _d(model.x), C.c_double(model.box_length))
+
+
+def validate(model) -> int:
+    """gpuqt_validate on a TBModel-like object; returns the status code (host only, no GPU)."""
+    return load().gpuqt_validate(*_model_tuple(model), C.c_double(model.energy_scale))
+
+
+def bessel_coeffs(dE, dt, order):
+    cr, ci = np.empty(order), np.empty(order)
+    rc = load().gpuqt_bessel_coeffs(dE, dt, order, _d(cr), _d(ci))
+    if rc:
+        raise GpuqtError(rc, "gpuqt_bessel_coeffs")
+    return cr + 1j * ci
+
+
+class GpuQT:
+    """One gpuqt_handle on the current CUDA device; workspace and stream come from torch."""
+
+    def __init__(self, model, batch=1, modes=MODE_VAC | MODE_MSD, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("gpuqt needs a CUDA device (no CPU fallback)")
+        lib = load()
+        self._torch = torch
+        self.N, self.K, self.batch, self.modes = model.N, model.K, batch, modes
+        nbytes = lib.gpuqt_workspace_bytes(model.N, model.K, int(model.hop_im is not None), batch, modes)
+        if nbytes == 0:
+            raise GpuqtError(-1, "gpuqt_workspace_bytes")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self._h = C.c_void_p()
+        rc = lib.gpuqt_create(C.byref(self._h), *_model_tuple(model), C.c_double(model.volume),
+                              C.c_double(model.energy_scale), C.c_int32(batch), C.c_int(modes),
+                              C.c_void_p(self.workspace.data_ptr()), C.c_size_t(nbytes),
+                              C.c_void_p(self.stream.cuda_stream))
+        if rc:
+            self._h = C.c_void_p()
+            raise GpuqtError(rc, "gpuqt_create")
+
+    def _ck(self, rc, what):
+        if rc:
+            raise GpuqtError(rc, what, (load().gpuqt_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load().gpuqt_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- state
+    def set_state(self, phi):
+        """phi: host [batch][N][2] float64 — numpy array or (pinned) CPU torch tensor."""
+        if isinstance(phi, np.ndarray):
+            phi = np.ascontiguousarray(phi, np.float64)
+            assert phi.shape == (self.batch, self.N, 2)
+            self._ck(load().gpuqt_set_state(self._h, C.c_void_p(phi.ctypes.data)), "gpuqt_set_state")
+        else:
+            assert phi.device.type == "cpu" and phi.is_contiguous() and phi.dtype == self._torch.float64
+            assert tuple(phi.shape) == (self.batch, self.N, 2)
+            self._ck(load().gpuqt_set_state(self._h, C.c_void_p(phi.data_ptr())), "gpuqt_set_state")
+
+    def set_state_device(self, phi):
+        assert phi.is_cuda and phi.is_contiguous() and phi.dtype == self._torch.float64
+        assert tuple(phi.shape) == (self.batch, self.N, 2)
+        self._ck(load().gpuqt_set_state_device(self._h, C.c_void_p(phi.data_ptr())), "gpuqt_set_state_device")
+
+    def get_state(self, which):
+        out = np.empty((self.batch, self.N, 2), np.float64)
+        self._ck(load().gpuqt_get_state(self._h, which, C.c_void_p(out.ctypes.data)), "gpuqt_get_state")
+        return out
+
+    def get_table(self):
+        nk = self.N * self.K
+        col = np.empty(nk, np.int32)
+        re, im, dx = (np.empty(nk, np.float64) for _ in range(3))
+        self._ck(load().gpuqt_get_table(self._h, _i(col), _d(re), _d(im), _d(dx)), "gpuqt_get_table")
+        return col, re, im, dx
+
+    # ---- the path
+    def _moments(self, fn, what, n, out=None):
+        if out is None:
+            out = np.empty((self.batch, n), np.float64)
+            ptr = out.ctypes.data
+        else:                                   # pinned torch tensor
+            ptr = out.data_ptr()
+        self._ck(fn(self._h, C.c_int32(n), C.c_void_p(ptr)), what)
+        return out
+
+    def dos_moments(self, n, out=None):
+        return self._moments(load().gpuqt_dos_moments, "gpuqt_dos_moments", n, out)
+
+    def msd(self, n, out=None):
+        return self._moments(load().gpuqt_msd, "gpuqt_msd", n, out)
+
+    def vac(self, n, out=None):
+        return self._moments(load().gpuqt_vac, "gpuqt_vac", n, out)
+
+    def evolve(self, dt, order):
+        self._ck(load().gpuqt_evolve(self._h, C.c_double(dt), C.c_int32(order)), "gpuqt_evolve")
+
+    def kpm_transform(self, moments, energies):
+        moments = np.ascontiguousarray(moments, np.float64)
+        energies = np.ascontiguousarray(energies, np.float64)
+        m2 = moments.reshape(-1, moments.shape[-1])
+        out = np.empty((m2.shape[0], energies.size), np.float64)
+        self._ck(load().gpuqt_kpm_transform(self._h, _d(m2), C.c_int32(m2.shape[1]), C.c_int32(m2.shape[0]),
+                                            _d(energies), C.c_int32(energies.size), _d(out)), "gpuqt_kpm_transform")
+        return out
+
+    # ---- timing
+    def kernel_stats(self, cls):
+        ms, n = C.c_double(), C.c_int64()
+        self._ck(load().gpuqt_kernel_stats(self._h, cls, C.byref(ms), C.byref(n)), "gpuqt_kernel_stats")
+        return ms.value, n.value
+
+    def reset_stats(self):
+        self._ck(load().gpuqt_reset_stats(self._h), "gpuqt_reset_stats")

@@ -1,0 +1,664 @@
+// C-ABI of the B200-native GPUQT hot path (include/gpuqt.h): host logic + kernel launches.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <string>
+#include <vector>
+
+#include "../../include/gpuqt.h"
+#include "host_util.h"
+#include "kernels.cuh"
+
+using namespace gpuqt;
+
+namespace {
+
+constexpr int kMaxGrid = 4096;
+constexpr int kPartialDoubles = 32;   // Q*B <= 24
+
+struct PendingStat {
+    int cls;
+    cudaEvent_t start, stop;
+    int64_t launches;
+};
+
+}  // namespace
+
+struct gpuqt_handle {
+    int64_t N = 0;
+    int32_t K = 0, B = 0;
+    int modes = 0, cplx = 0, kt = 0;
+    double dE = 0, box = 0, volume = 0;
+    cudaStream_t stream = nullptr;
+    int n_sm = 0;
+    Mat mat{};
+    size_t vec_elems = 0;   // N * B double2
+    // vectors (device, inside the caller's workspace)
+    double2 *psi = nullptr, *chi = nullptr, *va = nullptr, *vb = nullptr, *phiL = nullptr;
+    double2 *out0 = nullptr, *out1 = nullptr, *ring[3] = {nullptr, nullptr, nullptr},
+            *ringe[3] = {nullptr, nullptr, nullptr};
+    double *partials = nullptr, *dots = nullptr, *moments = nullptr;
+    unsigned int* ticket = nullptr;
+    int grid[4] = {0, 0, 0, 0};
+    int grid_aux = 0;
+    bool state_set = false;
+    std::string err;
+    double stat_ms[GPUQT_KERNEL_CLASSES] = {0};
+    int64_t stat_launches[GPUQT_KERNEL_CLASSES] = {0};
+    std::vector<PendingStat> pending;
+    std::vector<cudaEvent_t> free_events;
+};
+
+namespace {
+
+int fail(gpuqt_handle* h, int code, const std::string& msg) {
+    if (h) h->err = msg;
+    return code;
+}
+int cuda_fail(gpuqt_handle* h, cudaError_t e, const char* what) {
+    return fail(h, GPUQT_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);     \
+    } while (0)
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+int n_vectors(int modes) {
+    int n = 2 + 3;                                  // psi, out0, ring[3]
+    if (modes & GPUQT_MODE_MSD) n += 2 + 3;         // chi, out1, ringe[3]
+    if (modes & GPUQT_MODE_VAC) n += 3;             // a, b, phi_L
+    return n;
+}
+
+struct Layout {
+    size_t col, hre, him, onsite, x, slice_ptr, vectors, partials, dots, moments, ticket, total;
+};
+
+Layout make_layout(int64_t N, int32_t K, int cplx, int32_t B, int modes, size_t entries) {
+    Layout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        size_t o = off;
+        off = align_up(off + bytes);
+        return o;
+    };
+    const size_t n_slices = (size_t)((N + 31) / 32);
+    L.col = take(entries * sizeof(int32_t));
+    L.hre = take(entries * sizeof(double));
+    L.him = take(cplx ? entries * sizeof(double) : 0);
+    L.onsite = take((size_t)N * sizeof(double));
+    L.x = take((size_t)N * sizeof(double));
+    L.slice_ptr = take((n_slices + 1) * sizeof(long long));
+    L.vectors = take((size_t)n_vectors(modes) * align_up((size_t)N * B * sizeof(double2)));
+    L.partials = take((size_t)kMaxGrid * kPartialDoubles * sizeof(double));
+    L.dots = take((size_t)GPUQT_MAX_MOMENTS * 3 * 8 * sizeof(double));
+    L.moments = take((size_t)GPUQT_MAX_MOMENTS * 8 * sizeof(double));
+    L.ticket = take(256);
+    L.total = off;
+    return L;
+}
+
+bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
+
+// ---------------------------------------------------------------- kernel dispatch
+template <int MODE, int BB, int KK>
+void* step_fn(bool cplx) {
+    return cplx ? (void*)cheb_step_kernel<BB, KK, true, MODE> : (void*)cheb_step_kernel<BB, KK, false, MODE>;
+}
+template <int MODE, int BB>
+void* step_fn_k(int kt, bool cplx) {
+    switch (kt) {
+    case 3: return step_fn<MODE, BB, 3>(cplx);
+    case 4: return step_fn<MODE, BB, 4>(cplx);
+    case 6: return step_fn<MODE, BB, 6>(cplx);
+    default: return step_fn<MODE, BB, 0>(cplx);
+    }
+}
+template <int MODE>
+void* step_fn_b(int B, int kt, bool cplx) {
+    switch (B) {
+    case 1: return step_fn_k<MODE, 1>(kt, cplx);
+    case 2: return step_fn_k<MODE, 2>(kt, cplx);
+    case 4: return step_fn_k<MODE, 4>(kt, cplx);
+    default: return step_fn_k<MODE, 8>(kt, cplx);
+    }
+}
+void* step_kernel(const gpuqt_handle* h, int mode) {
+    switch (mode) {
+    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->cplx);
+    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->cplx);
+    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->cplx);
+    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->cplx);
+    }
+}
+
+template <int BB, int KK>
+void* vel_fn(bool cplx) {
+    return cplx ? (void*)velocity_kernel<BB, KK, true> : (void*)velocity_kernel<BB, KK, false>;
+}
+template <int BB>
+void* vel_fn_k(int kt, bool cplx) {
+    switch (kt) {
+    case 3: return vel_fn<BB, 3>(cplx);
+    case 4: return vel_fn<BB, 4>(cplx);
+    case 6: return vel_fn<BB, 6>(cplx);
+    default: return vel_fn<BB, 0>(cplx);
+    }
+}
+void* velocity_fn(const gpuqt_handle* h) {
+    switch (h->B) {
+    case 1: return vel_fn_k<1>(h->kt, h->cplx);
+    case 2: return vel_fn_k<2>(h->kt, h->cplx);
+    case 4: return vel_fn_k<4>(h->kt, h->cplx);
+    default: return vel_fn_k<8>(h->kt, h->cplx);
+    }
+}
+void* dot_fn(int B) {
+    switch (B) {
+    case 1: return (void*)dot_kernel<1>;
+    case 2: return (void*)dot_kernel<2>;
+    case 4: return (void*)dot_kernel<4>;
+    default: return (void*)dot_kernel<8>;
+    }
+}
+
+int grid_for(gpuqt_handle* h, void* fn) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kThreads, 0) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    const long long rows = kThreads / h->B;
+    const long long chunks = (h->N + rows - 1) / rows;
+    long long g = (long long)per_sm * h->n_sm;
+    if (g > chunks) g = chunks;
+    if (g > kMaxGrid) g = kMaxGrid;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
+    void* fn = step_kernel(h, mode);
+    if (!h->grid[mode]) h->grid[mode] = grid_for(h, fn);
+    a.partials = h->partials;
+    a.ticket = h->ticket;
+    void* args[] = {(void*)&h->mat, (void*)&a};
+    return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, 0, h->stream);
+}
+
+cudaError_t launch_velocity(gpuqt_handle* h, const double2* in, double2* out) {
+    void* fn = velocity_fn(h);
+    if (!h->grid_aux) h->grid_aux = grid_for(h, fn);
+    void* args[] = {(void*)&h->mat, (void*)&in, (void*)&out};
+    return cudaLaunchKernel(fn, dim3(h->grid_aux), dim3(kThreads), args, 0, h->stream);
+}
+
+cudaError_t launch_dot(gpuqt_handle* h, const double2* l, const double2* r, double* result) {
+    void* fn = dot_fn(h->B);
+    if (!h->grid_aux) h->grid_aux = grid_for(h, velocity_fn(h));
+    long long N = h->N;
+    void* args[] = {(void*)&N, (void*)&l, (void*)&r, (void*)&h->partials, (void*)&h->ticket, (void*)&result};
+    return cudaLaunchKernel(fn, dim3(h->grid_aux), dim3(kThreads), args, 0, h->stream);
+}
+
+// ---------------------------------------------------------------- timing statistics
+cudaEvent_t get_event(gpuqt_handle* h) {
+    if (!h->free_events.empty()) {
+        cudaEvent_t e = h->free_events.back();
+        h->free_events.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+struct StatScope {
+    gpuqt_handle* h;
+    PendingStat p;
+    StatScope(gpuqt_handle* hh, int cls) : h(hh) {
+        p.cls = cls;
+        p.launches = 0;
+        p.start = get_event(h);
+        p.stop = get_event(h);
+        cudaEventRecord(p.start, h->stream);
+    }
+    void count(int64_t n = 1) { p.launches += n; }
+    ~StatScope() {
+        cudaEventRecord(p.stop, h->stream);
+        h->pending.push_back(p);
+    }
+};
+void flush_stats(gpuqt_handle* h) {
+    for (auto& p : h->pending) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(p.stop) == cudaSuccess && cudaEventElapsedTime(&ms, p.start, p.stop) == cudaSuccess) {
+            h->stat_ms[p.cls] += ms;
+            h->stat_launches[p.cls] += p.launches;
+        }
+        h->free_events.push_back(p.start);
+        h->free_events.push_back(p.stop);
+    }
+    h->pending.clear();
+}
+
+// ---------------------------------------------------------------- building blocks
+// out_vec <- sum_{m<order} c_m T_m(H~) in_vec   (Eq. 17, 21, 23), one fused kernel per term.
+// `in` is left untouched; `out` must differ from in and from the ring buffers.
+int evolve_one(gpuqt_handle* h, const double2* in, double2* out, const std::vector<double>& cr,
+               const std::vector<double>& ci, int order) {
+    if (order == 1) {   // U ~ c_0: out = c_0 in  -> run the first-term kernel with c_1 = 0
+        StepArgs a{};
+        a.in = in; a.out = h->ring[0]; a.acc = out;
+        a.c0r = cr[0]; a.c0i = ci[0]; a.cr = 0; a.ci = 0; a.first = 1; a.store = 0;
+        StatScope s(h, GPUQT_KERNEL_EVOLVE);
+        CU(launch_step(h, kModeEvolve, a));
+        s.count();
+        return GPUQT_OK;
+    }
+    StatScope s(h, GPUQT_KERNEL_EVOLVE);
+    const double2* tm1 = in;        // T_{m-1}
+    const double2* tm2 = nullptr;   // T_{m-2}
+    for (int m = 1; m < order; ++m) {
+        StepArgs a{};
+        double2* tnew = h->ring[(m - 1) % 3];
+        a.in = tm1; a.prev = tm2; a.out = tnew; a.acc = out;
+        a.cr = cr[m]; a.ci = ci[m]; a.c0r = cr[0]; a.c0i = ci[0];
+        a.first = (m == 1); a.store = (m + 1 < order);
+        CU(launch_step(h, kModeEvolve, a));
+        s.count();
+        tm2 = tm1;
+        tm1 = tnew;
+    }
+    return GPUQT_OK;
+}
+
+// (psi, chi) <- (U psi, U chi + [X,U] psi) with the fused e-recursion
+//   a_m = T_m psi, e_m = T_m chi + [X,T_m] psi:  e_m = 2 H~ e_{m-1} - e_{m-2} + 2 [X,H~] a_{m-1}
+int evolve_msd_pair(gpuqt_handle* h, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
+    StatScope s(h, GPUQT_KERNEL_EVOLVE_MSD);
+    const double2 *am1 = h->psi, *am2 = nullptr, *em1 = h->chi, *em2 = nullptr;
+    const int terms = order < 2 ? 2 : order;
+    for (int m = 1; m < terms; ++m) {
+        StepArgs a{};
+        double2* anew = h->ring[(m - 1) % 3];
+        double2* enew = h->ringe[(m - 1) % 3];
+        a.in = am1; a.prev = am2; a.out = anew;
+        a.in_e = em1; a.prev_e = em2; a.out_e = enew;
+        a.acc = h->out0; a.acc_e = h->out1;
+        if (order < 2) { a.cr = 0; a.ci = 0; } else { a.cr = cr[m]; a.ci = ci[m]; }
+        a.c0r = cr[0]; a.c0i = ci[0];
+        a.first = (m == 1); a.store = (m + 1 < terms);
+        CU(launch_step(h, kModeEvolveMsd, a));
+        s.count();
+        am2 = am1; am1 = anew;
+        em2 = em1; em1 = enew;
+    }
+    std::swap(h->psi, h->out0);
+    std::swap(h->chi, h->out1);
+    return GPUQT_OK;
+}
+
+// moments with the doubling identity: C_n = <v|T_n|v>, n < n_moments  -> h->moments [B][n]
+int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
+    const int n_steps = n_moments / 2;   // step j gives C_{2j+1}, C_{2j+2}
+    {
+        StatScope s(h, GPUQT_KERNEL_KPM_DOUBLING);
+        const double2 *tm1 = v, *tm2 = nullptr;
+        for (int j = 0; j < n_steps; ++j) {
+            StepArgs a{};
+            double2* tnew = h->ring[j % 3];
+            a.in = tm1; a.prev = tm2; a.out = tnew;
+            a.first = (j == 0); a.store = (j + 1 < n_steps);
+            a.result = h->dots + (size_t)j * 3 * h->B;
+            CU(launch_step(h, kModeDoubling, a));
+            s.count();
+            tm2 = tm1; tm1 = tnew;
+        }
+    }
+    const int total = h->B * n_moments;
+    finalize_doubling<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, n_steps, h->dots, h->moments);
+    CU(cudaGetLastError());
+    return GPUQT_OK;
+}
+
+// C_n = <l|T_n|r>  -> h->moments [B][n] (real part)
+int moments_left(gpuqt_handle* h, const double2* l, const double2* r, int n_moments) {
+    CU(launch_dot(h, l, r, h->dots));
+    {
+        StatScope s(h, GPUQT_KERNEL_KPM_LEFT);
+        const double2 *tm1 = r, *tm2 = nullptr;
+        for (int n = 1; n < n_moments; ++n) {
+            StepArgs a{};
+            double2* tnew = h->ring[(n - 1) % 3];
+            a.in = tm1; a.prev = tm2; a.out = tnew; a.phiL = l;
+            a.first = (n == 1); a.store = (n + 1 < n_moments);
+            a.result = h->dots + (size_t)n * 2 * h->B;
+            CU(launch_step(h, kModeLeft, a));
+            s.count();
+            tm2 = tm1; tm1 = tnew;
+        }
+    }
+    const int total = h->B * n_moments;
+    finalize_left<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, h->dots, h->moments);
+    CU(cudaGetLastError());
+    return GPUQT_OK;
+}
+
+int copy_moments_out(gpuqt_handle* h, int n_moments, double* out_host) {
+    CU(cudaMemcpyAsync(out_host, h->moments, (size_t)h->B * n_moments * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    flush_stats(h);
+    return GPUQT_OK;
+}
+
+int finish_set_state(gpuqt_handle* h) {
+    // ring[0] holds phi in [batch][N] order
+    const long long total = (long long)h->vec_elems;
+    const int blocks = (int)((total + 255) / 256);
+    to_device_layout<<<blocks, 256, 0, h->stream>>>(h->N, h->B, h->ring[0], h->psi);
+    CU(cudaGetLastError());
+    if (h->modes & GPUQT_MODE_MSD) {
+        zero_vec<<<blocks, 256, 0, h->stream>>>(total, h->chi);
+        CU(cudaGetLastError());
+    }
+    if (h->modes & GPUQT_MODE_VAC) {
+        CU(cudaMemcpyAsync(h->va, h->psi, h->vec_elems * sizeof(double2), cudaMemcpyDeviceToDevice, h->stream));
+        StatScope s(h, GPUQT_KERNEL_VELOCITY);
+        CU(launch_velocity(h, h->psi, h->vb));
+        s.count();
+    }
+    h->state_set = true;
+    return GPUQT_OK;
+}
+
+}  // namespace
+
+// =================================================================== C ABI
+extern "C" {
+
+size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes) {
+    if (N <= 0 || K_max <= 0 || !batch_ok(batch)) return 0;
+    const size_t entries = (size_t)((N + 31) / 32) * 32 * (size_t)K_max;
+    return make_layout(N, K_max, is_complex ? 1 : 0, batch, modes, entries).total;
+}
+
+int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index,
+                   const double* hop_re, const double* hop_im, const double* onsite,
+                   const double* x, double box_length, double energy_scale) {
+    std::string msg;
+    return validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
+}
+
+int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im) {
+    if (!(energy_scale > 0.0) || order < 1 || !c_re || !c_im) return GPUQT_ERR_ARG;
+    std::vector<double> cr, ci;
+    bessel_coeffs(energy_scale, dt, order, cr, ci);
+    for (int m = 0; m < order; ++m) {
+        c_re[m] = cr[(size_t)m];
+        c_im[m] = ci[(size_t)m];
+    }
+    return GPUQT_OK;
+}
+
+int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nbr_count,
+                 const int32_t* nbr_index, const double* hop_re, const double* hop_im,
+                 const double* onsite, const double* x, double box_length, double volume,
+                 double energy_scale, int32_t batch, int modes, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return GPUQT_ERR_ARG;
+    *out = nullptr;
+    if (!batch_ok(batch) || !workspace || !(volume > 0.0) || (modes & ~7)) return GPUQT_ERR_ARG;
+    std::string msg;
+    int rc = validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
+    if (rc != GPUQT_OK) {
+        fprintf(stderr, "gpuqt_create: %s\n", msg.c_str());
+        return rc;
+    }
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return GPUQT_ERR_ARG;
+    if (modes & GPUQT_MODE_MSD) modes |= GPUQT_MODE_PSI;
+    gpuqt_handle* h = new (std::nothrow) gpuqt_handle();
+    if (!h) return GPUQT_ERR_NOMEM;
+    h->N = N; h->K = K_max; h->B = batch; h->modes = modes; h->cplx = hop_im ? 1 : 0;
+    h->dE = energy_scale; h->box = box_length; h->volume = volume;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->vec_elems = (size_t)N * batch;
+
+    SellHost sell;
+    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, sell);
+    const size_t entries = sell.col.size();
+    const Layout L = make_layout(N, K_max, h->cplx, batch, modes, entries);
+    if (L.total > workspace_bytes) {
+        delete h;
+        return GPUQT_ERR_NOMEM;
+    }
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (ce != cudaSuccess) {
+        fprintf(stderr, "gpuqt_create: no usable CUDA device: %s\n", cudaGetErrorString(ce));
+        delete h;
+        return GPUQT_ERR_CUDA;
+    }
+    char* base = (char*)workspace;
+    int32_t* d_col = (int32_t*)(base + L.col);
+    double* d_hre = (double*)(base + L.hre);
+    double* d_him = h->cplx ? (double*)(base + L.him) : nullptr;
+    double* d_on = (double*)(base + L.onsite);
+    double* d_x = (double*)(base + L.x);
+    long long* d_sp = (long long*)(base + L.slice_ptr);
+    std::vector<double> on_host((size_t)N, 0.0);
+    if (onsite) memcpy(on_host.data(), onsite, (size_t)N * sizeof(double));
+    auto up = [&](void* d, const void* s, size_t bytes) {
+        return bytes ? cudaMemcpyAsync(d, s, bytes, cudaMemcpyHostToDevice, h->stream) : cudaSuccess;
+    };
+    ce = up(d_col, sell.col.data(), entries * sizeof(int32_t));
+    if (ce == cudaSuccess) ce = up(d_hre, sell.hre.data(), entries * sizeof(double));
+    if (ce == cudaSuccess && h->cplx) ce = up(d_him, sell.him.data(), entries * sizeof(double));
+    if (ce == cudaSuccess) ce = up(d_on, on_host.data(), (size_t)N * sizeof(double));
+    if (ce == cudaSuccess) ce = up(d_x, x, (size_t)N * sizeof(double));
+    if (ce == cudaSuccess) ce = up(d_sp, sell.slice_ptr.data(), sell.slice_ptr.size() * sizeof(long long));
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(base + L.ticket, 0, 256, h->stream);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+    if (ce != cudaSuccess) {
+        fprintf(stderr, "gpuqt_create: upload failed: %s\n", cudaGetErrorString(ce));
+        delete h;
+        return GPUQT_ERR_CUDA;
+    }
+    h->mat.col = d_col; h->mat.hre = d_hre; h->mat.him = d_him; h->mat.onsite = d_on; h->mat.x = d_x;
+    h->mat.slice_ptr = d_sp; h->mat.N = N; h->mat.K = K_max; h->mat.uniform = sell.uniform;
+    h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
+    h->kt = (sell.uniform && (K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
+
+    const size_t vstride = align_up((size_t)N * batch * sizeof(double2));
+    char* v = base + L.vectors;
+    auto nextv = [&]() {
+        double2* p = (double2*)v;
+        v += vstride;
+        return p;
+    };
+    h->psi = nextv(); h->out0 = nextv();
+    for (int i = 0; i < 3; ++i) h->ring[i] = nextv();
+    if (modes & GPUQT_MODE_MSD) {
+        h->chi = nextv(); h->out1 = nextv();
+        for (int i = 0; i < 3; ++i) h->ringe[i] = nextv();
+    }
+    if (modes & GPUQT_MODE_VAC) {
+        h->va = nextv(); h->vb = nextv(); h->phiL = nextv();
+    }
+    h->partials = (double*)(base + L.partials);
+    h->dots = (double*)(base + L.dots);
+    h->moments = (double*)(base + L.moments);
+    h->ticket = (unsigned int*)(base + L.ticket);
+    *out = h;
+    return GPUQT_OK;
+}
+
+int gpuqt_set_state(gpuqt_handle* h, const double* phi_host) {
+    if (!h || !phi_host) return fail(h, GPUQT_ERR_ARG, "null argument");
+    CU(cudaMemcpyAsync(h->ring[0], phi_host, h->vec_elems * sizeof(double2), cudaMemcpyHostToDevice, h->stream));
+    return finish_set_state(h);
+}
+
+int gpuqt_set_state_device(gpuqt_handle* h, const double* phi_device) {
+    if (!h || !phi_device) return fail(h, GPUQT_ERR_ARG, "null argument");
+    CU(cudaMemcpyAsync(h->ring[0], phi_device, h->vec_elems * sizeof(double2), cudaMemcpyDeviceToDevice, h->stream));
+    return finish_set_state(h);
+}
+
+int gpuqt_dos_moments(gpuqt_handle* h, int32_t n_moments, double* out_host) {
+    if (!h || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return fail(h, GPUQT_ERR_ARG, "bad n_moments or null output");
+    if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
+    int rc = moments_doubling(h, h->psi, n_moments);
+    if (rc) return rc;
+    return copy_moments_out(h, n_moments, out_host);
+}
+
+int gpuqt_msd(gpuqt_handle* h, int32_t n_moments, double* out_host) {
+    if (!h || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return fail(h, GPUQT_ERR_ARG, "bad n_moments or null output");
+    if (!(h->modes & GPUQT_MODE_MSD)) return fail(h, GPUQT_ERR_STATE, "handle was created without GPUQT_MODE_MSD");
+    if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
+    int rc = moments_doubling(h, h->chi, n_moments);
+    if (rc) return rc;
+    return copy_moments_out(h, n_moments, out_host);
+}
+
+int gpuqt_vac(gpuqt_handle* h, int32_t n_moments, double* out_host) {
+    if (!h || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return fail(h, GPUQT_ERR_ARG, "bad n_moments or null output");
+    if (!(h->modes & GPUQT_MODE_VAC)) return fail(h, GPUQT_ERR_STATE, "handle was created without GPUQT_MODE_VAC");
+    if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
+    {
+        StatScope s(h, GPUQT_KERNEL_VELOCITY);
+        CU(launch_velocity(h, h->va, h->phiL));   // phi_L = V a
+        s.count();
+    }
+    int rc = moments_left(h, h->phiL, h->vb, n_moments);
+    if (rc) return rc;
+    return copy_moments_out(h, n_moments, out_host);
+}
+
+int gpuqt_evolve(gpuqt_handle* h, double dt, int32_t order) {
+    if (!h || order < 1 || !std::isfinite(dt)) return fail(h, GPUQT_ERR_ARG, "bad dt or order");
+    if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
+    std::vector<double> cr, ci;
+    int rc;
+    if (h->modes & (GPUQT_MODE_MSD | GPUQT_MODE_PSI)) {
+        bessel_coeffs(h->dE, dt, order, cr, ci);
+        if (h->modes & GPUQT_MODE_MSD) {
+            rc = evolve_msd_pair(h, cr, ci, order);
+            if (rc) return rc;
+        } else {
+            rc = evolve_one(h, h->psi, h->out0, cr, ci, order);
+            if (rc) return rc;
+            std::swap(h->psi, h->out0);
+        }
+    }
+    if (h->modes & GPUQT_MODE_VAC) {
+        bessel_coeffs(h->dE, -dt, order, cr, ci);   // both VAC branches step with U(-dt)  [A1]
+        rc = evolve_one(h, h->va, h->out0, cr, ci, order);
+        if (rc) return rc;
+        std::swap(h->va, h->out0);
+        rc = evolve_one(h, h->vb, h->out0, cr, ci, order);
+        if (rc) return rc;
+        std::swap(h->vb, h->out0);
+    }
+    return GPUQT_OK;
+}
+
+int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_moments,
+                        int32_t n_sets, const double* energies_host, int32_t n_energies,
+                        double* out_host) {
+    if (!h || !moments_host || !energies_host || !out_host || n_moments < 1 || n_sets < 1 || n_energies < 1)
+        return fail(h, GPUQT_ERR_ARG, "null or non-positive argument");
+    for (int j = 0; j < n_energies; ++j)
+        if (!(std::fabs(energies_host[j] / h->dE) < 1.0))
+            return fail(h, GPUQT_ERR_ENERGY, "energy point outside (-energy_scale, energy_scale)");
+    const size_t bm = (size_t)n_sets * n_moments * sizeof(double), be = (size_t)n_energies * sizeof(double),
+                 bo = (size_t)n_sets * n_energies * sizeof(double), bg = (size_t)n_moments * sizeof(double);
+    double* scratch = nullptr;
+    const size_t om = 0, oe = align_up(bm), oo = oe + align_up(be), og = oo + align_up(bo), tot = og + align_up(bg);
+    CU(cudaMallocAsync((void**)&scratch, tot, h->stream));
+    char* s = (char*)scratch;
+    cudaError_t e = cudaMemcpyAsync(s + om, moments_host, bm, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s + oe, energies_host, be, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+        jackson_kernel<<<(n_moments + 255) / 256, 256, 0, h->stream>>>(n_moments, (double*)(s + og));
+        const int total = n_sets * n_energies;
+        transform_kernel<<<(total + 127) / 128, 128, 0, h->stream>>>(n_moments, n_sets, n_energies, (double*)(s + og),
+                                                                     (double*)(s + om), (double*)(s + oe), 1.0 / h->dE,
+                                                                     h->volume, (double*)(s + oo));
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, s + oo, bo, cudaMemcpyDeviceToHost, h->stream);
+    cudaFreeAsync(scratch, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "kpm_transform");
+    flush_stats(h);
+    return GPUQT_OK;
+}
+
+int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host) {
+    if (!h || !out_host) return fail(h, GPUQT_ERR_ARG, "null argument");
+    const double2* src = which == GPUQT_STATE_PSI ? h->psi : which == GPUQT_STATE_CHI ? h->chi
+                       : which == GPUQT_STATE_VAC_A ? h->va : which == GPUQT_STATE_VAC_B ? h->vb : nullptr;
+    if (!src) return fail(h, GPUQT_ERR_STATE, "state not available in this mode");
+    const long long total = (long long)h->vec_elems;
+    from_device_layout<<<(int)((total + 255) / 256), 256, 0, h->stream>>>(h->N, h->B, src, h->ring[0]);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out_host, h->ring[0], h->vec_elems * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    flush_stats(h);
+    return GPUQT_OK;
+}
+
+int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, double* dx) {
+    if (!h) return GPUQT_ERR_ARG;
+    const size_t nk = (size_t)h->N * h->K;
+    // scratch: the ring buffers are free between calls (3 * N*B*16 bytes >= N*K*28 is not
+    // guaranteed), so use a stream-ordered allocation
+    char* scratch = nullptr;
+    const size_t oc = 0, orr = align_up(nk * 4), oi = orr + align_up(nk * 8), od = oi + align_up(nk * 8), tot = od + align_up(nk * 8);
+    CU(cudaMallocAsync((void**)&scratch, tot, h->stream));
+    decode_table<<<(int)((nk + 255) / 256), 256, 0, h->stream>>>(h->mat, (int32_t*)(scratch + oc), (double*)(scratch + orr),
+                                                                 (double*)(scratch + oi), (double*)(scratch + od));
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && col) e = cudaMemcpyAsync(col, scratch + oc, nk * 4, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && re) e = cudaMemcpyAsync(re, scratch + orr, nk * 8, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && im) e = cudaMemcpyAsync(im, scratch + oi, nk * 8, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && dx) e = cudaMemcpyAsync(dx, scratch + od, nk * 8, cudaMemcpyDeviceToHost, h->stream);
+    cudaFreeAsync(scratch, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "get_table");
+    return GPUQT_OK;
+}
+
+int gpuqt_kernel_stats(gpuqt_handle* h, int kernel_class, double* ms, int64_t* launches) {
+    if (!h || kernel_class < 0 || kernel_class >= GPUQT_KERNEL_CLASSES) return GPUQT_ERR_ARG;
+    flush_stats(h);
+    if (ms) *ms = h->stat_ms[kernel_class];
+    if (launches) *launches = h->stat_launches[kernel_class];
+    return GPUQT_OK;
+}
+
+int gpuqt_reset_stats(gpuqt_handle* h) {
+    if (!h) return GPUQT_ERR_ARG;
+    flush_stats(h);
+    for (int i = 0; i < GPUQT_KERNEL_CLASSES; ++i) {
+        h->stat_ms[i] = 0;
+        h->stat_launches[i] = 0;
+    }
+    return GPUQT_OK;
+}
+
+const char* gpuqt_last_error(const gpuqt_handle* h) { return h ? h->err.c_str() : "null handle"; }
+
+void gpuqt_destroy(gpuqt_handle* h) {
+    if (!h) return;
+    cudaStreamSynchronize(h->stream);
+    flush_stats(h);
+    for (auto e : h->free_events) cudaEventDestroy(e);
+    delete h;
+}
+
+}  // extern "C"

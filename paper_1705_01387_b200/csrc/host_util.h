@@ -1,0 +1,181 @@
+// Host-side pieces of the GPUQT library that need no GPU: input validation, the sliced-ELL
+// builder and the Bessel coefficient table (a9).  Product code; shares nothing
+// with oracle/.
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/gpuqt.h"
+
+namespace gpuqt {
+
+inline double host_min_image(double d, double box) {
+    if (box > 0.0) {
+        if (d > 0.5 * box) d -= box;
+        else if (d < -0.5 * box) d += box;
+    }
+    return d;
+}
+
+// Validation of the paper's four data sets.  Returns a gpuqt_status and a message.
+inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
+                           const double* hre, const double* him, const double* onsite,
+                           const double* x, double box, double dE, std::string& msg) {
+    if (N <= 0 || K <= 0 || !cnt || !idx || !x || !(dE > 0.0) || N > 0x7fffffffLL) {
+        msg = "invalid argument (N, K_max, energy_scale must be positive; nbr_count, nbr_index, x required; N < 2^31)";
+        return GPUQT_ERR_ARG;
+    }
+    if (him && !hre) {
+        msg = "hop_im given without hop_re";
+        return GPUQT_ERR_ARG;
+    }
+    // index range [A11]
+    for (int64_t m = 0; m < N; ++m) {
+        const int32_t c = cnt[m];
+        if (c < 0 || c > K) {
+            msg = "neighbour count out of range at site " + std::to_string(m);
+            return GPUQT_ERR_INDEX;
+        }
+        for (int32_t k = 0; k < c; ++k) {
+            const int32_t n = idx[(size_t)m * K + k];
+            if (n < 0 || n >= N) {
+                msg = "neighbour index out of range at site " + std::to_string(m);
+                return GPUQT_ERR_INDEX;
+            }
+        }
+    }
+    auto H = [&](int64_t m, int32_t k, double& re, double& im) {
+        re = hre ? hre[(size_t)m * K + k] : -1.0;
+        im = him ? him[(size_t)m * K + k] : 0.0;
+    };
+    // Hermiticity, bit-exact [A10]: the number of entries (m -> n, h) in row m equals the number
+    // of entries (n -> m, conj h) in row n.  Gershgorin bound [A9].  Ambiguous image [A6].
+    for (int64_t m = 0; m < N; ++m) {
+        double g = onsite ? std::fabs(onsite[m]) : 0.0;
+        for (int32_t k = 0; k < cnt[m]; ++k) {
+            const int32_t n = idx[(size_t)m * K + k];
+            double re, im;
+            H(m, k, re, im);
+            g += std::hypot(re, im);
+            if (re == 0.0 && im == 0.0) continue;
+            int here = 0, there = 0;
+            for (int32_t j = 0; j < cnt[m]; ++j) {
+                double r2, i2;
+                H(m, j, r2, i2);
+                if (idx[(size_t)m * K + j] == n && r2 == re && i2 == im) ++here;
+            }
+            for (int32_t j = 0; j < cnt[n]; ++j) {
+                double r2, i2;
+                H(n, j, r2, i2);
+                if (idx[(size_t)n * K + j] == (int32_t)m && r2 == re && i2 == -im) ++there;
+            }
+            if (here != there) {
+                msg = "H is not Hermitian: entry (" + std::to_string(m) + "," + std::to_string(n) + ") has no conjugate partner";
+                return GPUQT_ERR_NOT_HERMITIAN;
+            }
+            if (box > 0.0 && std::fabs(x[n] - x[m]) == 0.5 * box) {
+                msg = "ambiguous minimum image: |X_n - X_m| == box_length/2 for hop (" + std::to_string(m) + "," + std::to_string(n) + ")";
+                return GPUQT_ERR_POSITION;
+            }
+        }
+        if (g > dE) {
+            msg = "Gershgorin bound " + std::to_string(g) + " at site " + std::to_string(m) + " exceeds energy_scale " + std::to_string(dE);
+            return GPUQT_ERR_SCALE;
+        }
+    }
+    return GPUQT_OK;
+}
+
+// Sliced-ELL table on the host: slices of 32 rows, column-major inside a slice.
+struct SellHost {
+    int64_t n_slices = 0;
+    int uniform = 1;                    // every slice has width K_max
+    std::vector<long long> slice_ptr;   // [n_slices + 1] entry offsets
+    std::vector<int32_t> col;
+    std::vector<double> hre, him;
+};
+
+inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
+                       const double* hre, const double* him, SellHost& s) {
+    s.n_slices = (N + 31) / 32;
+    s.slice_ptr.assign((size_t)s.n_slices + 1, 0);
+    s.uniform = 1;
+    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+        int w = 0;
+        for (int64_t m = sl * 32; m < std::min<int64_t>(N, sl * 32 + 32); ++m) w = std::max(w, cnt[m]);
+        if (w != K) s.uniform = 0;
+        s.slice_ptr[(size_t)sl + 1] = s.slice_ptr[(size_t)sl] + (long long)w * 32;
+    }
+    const size_t total = (size_t)s.slice_ptr[(size_t)s.n_slices];
+    s.col.assign(total, 0);
+    s.hre.assign(total, 0.0);
+    if (him) s.him.assign(total, 0.0);
+    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+        const long long base = s.slice_ptr[(size_t)sl];
+        const int w = (int)((s.slice_ptr[(size_t)sl + 1] - base) / 32);
+        for (int lane = 0; lane < 32; ++lane) {
+            const int64_t m = sl * 32 + lane;
+            for (int k = 0; k < w; ++k) {
+                const size_t e = (size_t)base + (size_t)k * 32 + lane;
+                if (m < N && k < cnt[m]) {
+                    s.col[e] = idx[(size_t)m * K + k];
+                    s.hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
+                    if (him) s.him[e] = him[(size_t)m * K + k];
+                } else {
+                    s.col[e] = (int32_t)(m < N ? m : N - 1);               // padding: own row, hop 0
+                }
+            }
+        }
+    }
+}
+
+// J_m(x), m < n, by Miller's backward recurrence normalised with J_0 + 2 sum_k J_2k = 1.
+// (Deliberately a different routine from the oracle's libm jn().)
+inline void bessel_j_table(double x, int n, std::vector<double>& J) {
+    J.assign((size_t)n, 0.0);
+    if (n <= 0) return;
+    x = std::fabs(x);
+    if (x == 0.0) {
+        J[0] = 1.0;
+        return;
+    }
+    const int top = std::max(n, (int)std::ceil(x));
+    int M = top + 40 + (int)std::ceil(4.0 * std::sqrt((double)top));
+    M += (M & 1);   // even
+    std::vector<long double> f((size_t)M + 2, 0.0L);
+    f[(size_t)M] = 1e-300L;
+    const long double xl = (long double)x;
+    for (int k = M; k >= 1; --k) {
+        f[(size_t)k - 1] = (2.0L * k / xl) * f[(size_t)k] - f[(size_t)k + 1];
+        if (fabsl(f[(size_t)k - 1]) > 1e+3000L) {
+            for (int j = k - 1; j <= M; ++j) f[(size_t)j] *= 1e-3000L;
+        }
+    }
+    long double norm = f[0];
+    for (int k = 2; k <= M; k += 2) norm += 2.0L * f[(size_t)k];
+    for (int k = 0; k < n; ++k) J[(size_t)k] = (double)(f[(size_t)k] / norm);
+}
+
+// c_m = (2 - delta_0m) (-i sgn dt)^m J_m(dE |dt|)   PAPER.md:154 Eq. 17, :162 Eq. 20 [A8]
+inline void bessel_coeffs(double dE, double dt, int order, std::vector<double>& cr, std::vector<double>& ci) {
+    std::vector<double> J;
+    bessel_j_table(dE * std::fabs(dt), order, J);
+    cr.assign((size_t)order, 0.0);
+    ci.assign((size_t)order, 0.0);
+    const double sg = dt < 0 ? -1.0 : 1.0;
+    for (int m = 0; m < order; ++m) {
+        const double j = (m == 0 ? 1.0 : 2.0) * J[(size_t)m];
+        switch (m & 3) {
+        case 0: cr[(size_t)m] = j; break;
+        case 1: ci[(size_t)m] = -sg * j; break;
+        case 2: cr[(size_t)m] = -j; break;
+        default: ci[(size_t)m] = sg * j; break;
+        }
+    }
+}
+
+}  // namespace gpuqt

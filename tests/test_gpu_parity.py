@@ -1,0 +1,202 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Sizes span several 256-thread tiles, several 32-row slices and a ragged tail.
+
+Tolerances, written here:
+  tables / indices / dx : bit-exact
+  moments               : max_n |C_gpu - C_cpu| / (||phi_L|| ||phi_R||) <= 1e-10
+  vectors               : max_i |d psi_i| / max_i |psi_i|             <= 1e-10
+  transform             : max |d| / max |out|                          <= 1e-10
+"""
+import numpy as np
+import pytest
+
+from workloads import lattices as L
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gq():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1705_01387_b200 as g
+    return g
+
+
+def vec_err(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+def norms(v):
+    """[B][N][2] -> per-vector 2-norm"""
+    return np.sqrt(np.sum(v * v, axis=(1, 2)))
+
+
+def small_models():
+    return [
+        ("square_k4", L.square(70, 37, W=2.0, seed=3)),                         # N = 2590, KT = 4 path
+        ("cubic_k6", L.cubic(13, W=16.5, seed=4, energy_scale=16.0)),           # N = 2197, KT = 6 path
+        ("graphene_k3", L.graphene(29, 17, W=1.0, seed=5)),                     # N = 1972, KT = 3 path
+        ("graphene_vac", L.graphene(31, 19, vacancy_fraction=0.03, vacancy_seed=9)),  # ragged rows
+        ("square_open", L.square(41, 23, W=1.0, seed=6, periodic=False)),       # generic width path
+        ("peierls_cplx", L.square_peierls(45, 31, flux_quanta=3, W=1.5, seed=7)),  # complex hoppings
+        ("chain_k2", L.chain(3001, W=1.0, seed=8)),                             # generic K = 2
+    ]
+
+
+@pytest.mark.parametrize("name,model", small_models(), ids=[n for n, _ in small_models()])
+def test_table_bit_exact(gq, oracle_mod, name, model):
+    o = oracle_mod.Oracle(model)
+    g = gq.GpuQT(model, batch=1, modes=0)
+    for a, b in zip(g.get_table(), o.get_table()):
+        assert a.tobytes() == b.tobytes()
+    g.close()
+
+
+@pytest.mark.parametrize("batch", [1, 2, 4, 8])
+@pytest.mark.parametrize("name,model", small_models(), ids=[n for n, _ in small_models()])
+def test_dos_moments(gq, oracle_mod, name, model, batch):
+    phi = L.random_phase_vectors(model.N, batch, config=50)
+    o = oracle_mod.Oracle(model, batch=batch)
+    o.set_state(phi)
+    g = gq.GpuQT(model, batch=batch, modes=0)
+    g.set_state(phi)
+    for nm in (64, 33):                                     # even and odd moment counts
+        ref = o.dos_moments(nm)
+        got = g.dos_moments(nm)
+        assert np.max(np.abs(got - ref)) / model.N <= TOL
+    assert np.max(np.abs(g.get_state(gq.STATE_PSI) - phi)) == 0.0
+    g.close()
+
+
+@pytest.mark.parametrize("batch", [1, 4])
+@pytest.mark.parametrize("name,model", small_models(), ids=[n for n, _ in small_models()])
+def test_time_stepping_all_branches(gq, oracle_mod, name, model, batch):
+    """psi, chi (fused e-recursion vs the oracle's separate U chi + [X,U] psi), a, b after
+    non-uniform steps; VAC = measure-then-evolve, MSD = evolve-then-measure [A4]."""
+    phi = L.random_phase_vectors(model.N, batch, config=51)
+    modes = gq.MODE_VAC | gq.MODE_MSD
+    o = oracle_mod.Oracle(model, batch=batch, modes=modes)
+    g = gq.GpuQT(model, batch=batch, modes=modes)
+    o.set_state(phi)
+    g.set_state(phi)
+    nm = 24
+    assert vec_err(g.get_state(gq.STATE_VAC_B), o.get_state(oracle_mod.VAC_B)) <= TOL   # V phi
+    dE = model.energy_scale
+    for dt in (0.4, 1.0, 0.15):
+        order = int(dE * dt) + 30
+        vac_ref, vac_got = o.vac(nm), g.vac(nm)
+        va = o.get_state(oracle_mod.VAC_A)
+        vb = o.get_state(oracle_mod.VAC_B)
+        scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(batch)])
+        assert np.max(np.abs(vac_got - vac_ref) / scale[:, None]) <= TOL
+        o.evolve(dt, order)
+        g.evolve(dt, order)
+        for which_g, which_o in ((gq.STATE_PSI, oracle_mod.PSI), (gq.STATE_CHI, oracle_mod.CHI),
+                                 (gq.STATE_VAC_A, oracle_mod.VAC_A), (gq.STATE_VAC_B, oracle_mod.VAC_B)):
+            assert vec_err(g.get_state(which_g), o.get_state(which_o)) <= TOL
+        chi = o.get_state(oracle_mod.CHI)
+        msd_ref, msd_got = o.msd(nm), g.msd(nm)
+        assert np.max(np.abs(msd_got - msd_ref) / (norms(chi) ** 2)[:, None]) <= TOL
+    g.close()
+
+
+def test_negative_dt_and_order_one(gq, oracle_mod):
+    model = L.square(33, 21, W=2.0, seed=12)
+    phi = L.random_phase_vectors(model.N, 2, config=52)
+    o = oracle_mod.Oracle(model, batch=2, modes=oracle_mod.MODE_MSD)
+    g = gq.GpuQT(model, batch=2, modes=gq.MODE_MSD)
+    o.set_state(phi)
+    g.set_state(phi)
+    for dt, order in ((-0.7, 40), (0.3, 1), (0.2, 2), (0.9, 3)):
+        o.evolve(dt, order)
+        g.evolve(dt, order)
+        assert vec_err(g.get_state(gq.STATE_PSI), o.get_state(oracle_mod.PSI)) <= TOL
+        assert vec_err(g.get_state(gq.STATE_CHI), o.get_state(oracle_mod.CHI)) <= TOL
+    g.close()
+
+
+def test_psi_only_mode(gq, oracle_mod):
+    model = L.graphene(20, 11, W=1.0, seed=2)
+    phi = L.random_phase_vectors(model.N, 1, config=53)
+    o = oracle_mod.Oracle(model, batch=1, modes=0)
+    g = gq.GpuQT(model, batch=1, modes=gq.MODE_PSI)
+    o.set_state(phi)
+    g.set_state(phi)
+    o.evolve(1.3, 50)
+    g.evolve(1.3, 50)
+    assert vec_err(g.get_state(gq.STATE_PSI), o.get_state(oracle_mod.PSI)) <= TOL
+    # unitarity: the norm is preserved to rounding
+    assert abs(np.linalg.norm(g.get_state(gq.STATE_PSI)) - np.sqrt(model.N)) < 1e-9
+    g.close()
+
+
+def test_transform(gq, oracle_mod):
+    model = L.square(40, 30, W=2.0, seed=1)
+    phi = L.random_phase_vectors(model.N, 4, config=54)
+    o = oracle_mod.Oracle(model, batch=4)
+    g = gq.GpuQT(model, batch=4, modes=0)
+    o.set_state(phi)
+    g.set_state(phi)
+    for nm in (1000, 257):
+        C = o.dos_moments(nm)
+        E = np.linspace(-0.98 * model.energy_scale, 0.98 * model.energy_scale, 601)
+        ref = o.kpm_transform(C, E)
+        got = g.kpm_transform(C, E)
+        assert np.max(np.abs(got - ref)) / np.max(np.abs(ref)) <= TOL
+    with pytest.raises(gq.GpuqtError) as ei:
+        g.kpm_transform(C, np.array([model.energy_scale]))
+    assert ei.value.status == -5
+    g.close()
+
+
+def test_errors_and_call_order(gq):
+    model = L.square(10, 10, W=1.0, seed=1)
+    g = gq.GpuQT(model, batch=1, modes=gq.MODE_MSD)
+    with pytest.raises(gq.GpuqtError) as ei:
+        g.dos_moments(16)                                   # before set_state
+    assert ei.value.status == -6
+    g.set_state(L.random_phase_vectors(model.N, 1, config=55))
+    with pytest.raises(gq.GpuqtError) as ei:
+        g.vac(16)                                           # VAC mode not enabled
+    assert ei.value.status == -6
+    with pytest.raises(gq.GpuqtError) as ei:
+        g.msd(1)
+    assert ei.value.status == -1
+    with pytest.raises(gq.GpuqtError):
+        gq.GpuQT(model, batch=3)                            # unsupported batch
+    g.close()
+
+
+def test_run_to_run_determinism(gq):
+    """Fixed-order reductions: two runs give bit-identical moments."""
+    model = L.cubic(24, W=16.5, seed=4, energy_scale=16.0)
+    phi = L.random_phase_vectors(model.N, 4, config=56)
+    outs = []
+    for _ in range(2):
+        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD)
+        g.set_state(phi)
+        g.evolve(1.0, 44)
+        outs.append((g.dos_moments(100).copy(), g.msd(100).copy()))
+        g.close()
+    assert outs[0][0].tobytes() == outs[1][0].tobytes()
+    assert outs[0][1].tobytes() == outs[1][1].tobytes()
+
+
+def test_empty_rows_and_tiny_sizes(gq, oracle_mod):
+    """Degenerate inputs: N smaller than one slice, sites with no neighbours at all."""
+    for model in (L.chain(5, W=0.5, seed=1), L.square(3, 3, periodic=False),
+                  L.graphene(4, 3, vacancy_fraction=0.3, vacancy_seed=2)):
+        phi = L.random_phase_vectors(model.N, 2, config=57)
+        o = oracle_mod.Oracle(model, batch=2)
+        g = gq.GpuQT(model, batch=2)
+        o.set_state(phi)
+        g.set_state(phi)
+        o.evolve(0.5, 30)
+        g.evolve(0.5, 30)
+        assert vec_err(g.get_state(gq.STATE_CHI), o.get_state(oracle_mod.CHI)) <= TOL
+        assert np.max(np.abs(g.dos_moments(10) - o.dos_moments(10))) / model.N <= TOL
+        g.close()

@@ -289,6 +289,15 @@ def _gaussian_potential(xy, Lx, Ly, centres, eps, xi):
     nbx = max(1, int(np.floor(Lx / rc)))
     nby = max(1, int(np.floor(Ly / rc)))
     bx, by = Lx / nbx, Ly / nby
+    if nbx < 3 or nby < 3:          # the 3x3 stencil would alias: small sheet, all pairs directly
+        U = np.zeros(N, dtype=np.float64)
+        for k in range(len(centres)):
+            dxy = xy - xy[centres[k]]
+            dxy[:, 0] -= Lx * np.round(dxy[:, 0] / Lx)
+            dxy[:, 1] -= Ly * np.round(dxy[:, 1] / Ly)
+            r2 = dxy[:, 0] ** 2 + dxy[:, 1] ** 2
+            U += np.where(r2 <= rc * rc, eps[k] * np.exp(-r2 / (2.0 * xi * xi)), 0.0)
+        return U
     cell = (np.minimum((xy[:, 0] / bx).astype(np.int64), nbx - 1)
             + nbx * np.minimum((xy[:, 1] / by).astype(np.int64), nby - 1))
     order = np.argsort(cell, kind="stable")
