@@ -104,6 +104,16 @@ def bessel_coeffs(dE, dt, order):
     return cr + 1j * ci
 
 
+def choose_order(dE, dt, tol=1e-15):
+    """Smallest N_p with |J_m(dE |dt|)| < tol for every m >= N_p (tail rule [A5]), from the
+    library's own coefficient table."""
+    x = dE * abs(dt)
+    n = int(x) + 80 + int(4 * np.sqrt(x + 1))
+    J = np.abs(bessel_coeffs(dE, dt, n)) / np.where(np.arange(n) == 0, 1.0, 2.0)
+    big = np.nonzero(J >= tol)[0]
+    return int(big[-1]) + 1 if big.size else 1
+
+
 class GpuQT:
     """One gpuqt_handle on the current CUDA device; workspace and stream come from torch."""
 

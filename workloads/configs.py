@@ -1,0 +1,73 @@
+"""The five BASELINE.json configs as seeded synthetic workloads.
+
+Only input construction and the schedule parameters live here (no method arithmetic)."""
+from dataclasses import dataclass
+from typing import Callable
+
+from . import lattices as L
+from . import rng
+
+
+@dataclass
+class Workload:
+    key: str
+    description: str
+    build: Callable[[], "L.TBModel"]
+    batch: int
+    n_moments: int          # N_m ("KPM order")
+    dt: float
+    n_steps: int
+    order: int              # N_p Chebyshev terms per step
+    path: str               # "vac" or "msd"
+    config_id: int
+
+    def phases(self, model, first_vector=0):
+        return L.random_phase_vectors(model.N, self.batch, self.config_id, first_vector)
+
+
+def _c1():
+    return L.graphene(24, 24, hop=-2.7, W=1.0, seed=rng.stream_seed(1, 0), energy_scale=10.0)
+
+
+def _c2():
+    return L.square(1000, 1000, W=2.0, seed=rng.stream_seed(2, 0), energy_scale=5.1)
+
+
+def _c3():
+    return L.graphene(707, 707, hop=-2.7, vacancy_fraction=0.01, vacancy_seed=rng.stream_seed(3, 1),
+                      energy_scale=10.0)
+
+
+def _c4():
+    return L.cubic(160, W=16.5, seed=rng.stream_seed(4, 0), energy_scale=16.0)
+
+
+def _c5():
+    return L.graphene_peierls_correlated(2828, 1414, config=5)
+
+
+WORKLOADS = {
+    "c1": Workload("c1", "graphene 24x24 four-atom cells (2304 orbitals), W=1 eV Anderson, dE=10 eV, "
+                   "N_m=256, VAC 10 steps dt=1, N_p=64, B=1", _c1, 1, 256, 1.0, 10, 64, "vac", 1),
+    "c2": Workload("c2", "square 1000x1000 (1e6 orbitals), W=2, dE=5.1, N_m=3000, VAC 20 steps dt=2, "
+                   "N_p=40, B=1", _c2, 1, 3000, 2.0, 20, 40, "vac", 2),
+    "c3": Workload("c3", "graphene 707x707 four-atom cells with 1% vacancies (1979403 orbitals), dE=10 eV, "
+                   "N_m=2000, MSD 50 steps dt=2, N_p=50, B=1", _c3, 1, 2000, 2.0, 50, 50, "msd", 3),
+    "c4": Workload("c4", "simple-cubic Anderson 160^3 (4.096e6 orbitals), W=16.5, dE=16, N_m=1000, "
+                   "MSD 40 steps dt=1, N_p=44, B=4", _c4, 4, 1000, 1.0, 40, 44, "msd", 4),
+    "c5": Workload("c5", "graphene 2828x1414 four-atom cells (15995168 orbitals), Peierls flux 1e-4/hexagon, "
+                   "Gaussian-correlated potential, N_m=3000, VAC 30 steps dt=1, N_p=34..38 (tail rule), B=8",
+                   _c5, 8, 3000, 1.0, 30, 0, "vac", 5),
+}
+
+
+def small_variant(key: str):
+    """Reduced-size lattices of the same family, for parity cases the oracle finishes in seconds."""
+    return {
+        "c1": lambda: _c1(),
+        "c2": lambda: L.square(120, 90, W=2.0, seed=rng.stream_seed(2, 0), energy_scale=5.1),
+        "c3": lambda: L.graphene(40, 36, hop=-2.7, vacancy_fraction=0.01, vacancy_seed=rng.stream_seed(3, 1),
+                                 energy_scale=10.0),
+        "c4": lambda: L.cubic(20, W=16.5, seed=rng.stream_seed(4, 0), energy_scale=16.0),
+        "c5": lambda: L.graphene_peierls_correlated(60, 32, config=5),
+    }[key]()
