@@ -29,6 +29,11 @@ struct gpuqt_handle {
     int64_t N = 0;
     int32_t K = 0, B = 0;
     int modes = 0, cplx = 0, kt = 0;
+    int max_blocks_per_sm = 0;          // GPUQT_BLOCKS_PER_SM (tuning override), 0 = occupancy limit
+    int run = kWarps;                   // GPUQT_RUN: consecutive slices per CTA run (multiple of kWarps)
+    int alternate = 1;                  // GPUQT_ALTERNATE: sweep direction alternates between launches
+    size_t step_smem = 0;               // dynamic shared memory of the staged step kernels
+    std::vector<void*> smem_set;        // kernels whose dynamic-smem attribute has been raised
     double dE = 0, box = 0, volume = 0;
     cudaStream_t stream = nullptr;
     int n_sm = 0;
@@ -42,6 +47,7 @@ struct gpuqt_handle {
     unsigned int* ticket = nullptr;
     int grid[4] = {0, 0, 0, 0};
     int grid_aux = 0;
+    int sweep = 0;                      // direction of the next step launch (reset per building block)
     bool state_set = false;
     std::string err;
     double stat_ms[GPUQT_KERNEL_CLASSES] = {0};
@@ -75,10 +81,10 @@ int n_vectors(int modes) {
 }
 
 struct Layout {
-    size_t col, hre, him, onsite, x, slice_ptr, vectors, partials, dots, moments, ticket, total;
+    size_t rec, slice_off, x, vectors, partials, dots, moments, ticket, total;
 };
 
-Layout make_layout(int64_t N, int32_t K, int cplx, int32_t B, int modes, size_t entries) {
+Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
     Layout L{};
     size_t off = 0;
     auto take = [&](size_t bytes) {
@@ -87,12 +93,9 @@ Layout make_layout(int64_t N, int32_t K, int cplx, int32_t B, int modes, size_t 
         return o;
     };
     const size_t n_slices = (size_t)((N + 31) / 32);
-    L.col = take(entries * sizeof(int32_t));
-    L.hre = take(entries * sizeof(double));
-    L.him = take(cplx ? entries * sizeof(double) : 0);
-    L.onsite = take((size_t)N * sizeof(double));
+    L.rec = take(rec_bytes);
+    L.slice_off = take((n_slices + 1) * sizeof(long long));
     L.x = take((size_t)N * sizeof(double));
-    L.slice_ptr = take((n_slices + 1) * sizeof(long long));
     L.vectors = take((size_t)n_vectors(modes) * align_up((size_t)N * B * sizeof(double2)));
     L.partials = take((size_t)kMaxGrid * kPartialDoubles * sizeof(double));
     L.dots = take((size_t)GPUQT_MAX_MOMENTS * 3 * 8 * sizeof(double));
@@ -100,6 +103,17 @@ Layout make_layout(int64_t N, int32_t K, int cplx, int32_t B, int modes, size_t 
     L.ticket = take(256);
     L.total = off;
     return L;
+}
+
+// shared memory of one step-kernel CTA: mbarriers, then kWarps * stages record buffers
+size_t step_smem_bytes(int stages, int stage_bytes) {
+    return 128 * (((size_t)kWarps * kMaxStages * 8 + 127) / 128) + (size_t)kWarps * stages * stage_bytes;
+}
+constexpr size_t kSmemBudget = 200 * 1024;   // leaves room for the static reduction buffers
+
+int env_int(const char* name, int dflt) {
+    const char* v = getenv(name);
+    return (v && *v) ? atoi(v) : dflt;
 }
 
 bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
@@ -112,6 +126,7 @@ void* step_fn(bool cplx) {
 template <int MODE, int BB>
 void* step_fn_k(int kt, bool cplx) {
     switch (kt) {
+    case 2: return step_fn<MODE, BB, 2>(cplx);
     case 3: return step_fn<MODE, BB, 3>(cplx);
     case 4: return step_fn<MODE, BB, 4>(cplx);
     case 6: return step_fn<MODE, BB, 6>(cplx);
@@ -136,25 +151,12 @@ void* step_kernel(const gpuqt_handle* h, int mode) {
     }
 }
 
-template <int BB, int KK>
-void* vel_fn(bool cplx) {
-    return cplx ? (void*)velocity_kernel<BB, KK, true> : (void*)velocity_kernel<BB, KK, false>;
-}
-template <int BB>
-void* vel_fn_k(int kt, bool cplx) {
-    switch (kt) {
-    case 3: return vel_fn<BB, 3>(cplx);
-    case 4: return vel_fn<BB, 4>(cplx);
-    case 6: return vel_fn<BB, 6>(cplx);
-    default: return vel_fn<BB, 0>(cplx);
-    }
-}
 void* velocity_fn(const gpuqt_handle* h) {
     switch (h->B) {
-    case 1: return vel_fn_k<1>(h->kt, h->cplx);
-    case 2: return vel_fn_k<2>(h->kt, h->cplx);
-    case 4: return vel_fn_k<4>(h->kt, h->cplx);
-    default: return vel_fn_k<8>(h->kt, h->cplx);
+    case 1: return (void*)velocity_kernel<1>;
+    case 2: return (void*)velocity_kernel<2>;
+    case 4: return (void*)velocity_kernel<4>;
+    default: return (void*)velocity_kernel<8>;
     }
 }
 void* dot_fn(int B) {
@@ -166,14 +168,13 @@ void* dot_fn(int B) {
     }
 }
 
-int grid_for(gpuqt_handle* h, void* fn) {
+int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items) {
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kThreads, 0) != cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kThreads, smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
-    const long long rows = kThreads / h->B;
-    const long long chunks = (h->N + rows - 1) / rows;
+    if (h->max_blocks_per_sm > 0 && per_sm > h->max_blocks_per_sm) per_sm = h->max_blocks_per_sm;
     long long g = (long long)per_sm * h->n_sm;
-    if (g > chunks) g = chunks;
+    if (g > work_items) g = work_items;
     if (g > kMaxGrid) g = kMaxGrid;
     if (g < 1) g = 1;
     return (int)g;
@@ -181,23 +182,32 @@ int grid_for(gpuqt_handle* h, void* fn) {
 
 cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
     void* fn = step_kernel(h, mode);
-    if (!h->grid[mode]) h->grid[mode] = grid_for(h, fn);
+    if (!h->grid[mode]) {
+        if (h->step_smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->step_smem);
+            if (e != cudaSuccess) return e;
+        }
+        h->grid[mode] = grid_for(h, fn, h->step_smem, (h->mat.n_slices + h->run - 1) / h->run);
+    }
     a.partials = h->partials;
     a.ticket = h->ticket;
+    a.reverse = h->alternate ? (h->sweep & 1) : 0;
+    a.run = h->run;
+    h->sweep ^= 1;
     void* args[] = {(void*)&h->mat, (void*)&a};
-    return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, 0, h->stream);
+    return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, h->step_smem, h->stream);
 }
 
 cudaError_t launch_velocity(gpuqt_handle* h, const double2* in, double2* out) {
     void* fn = velocity_fn(h);
-    if (!h->grid_aux) h->grid_aux = grid_for(h, fn);
+    if (!h->grid_aux) h->grid_aux = grid_for(h, fn, 0, (h->N * h->B + kThreads - 1) / kThreads);
     void* args[] = {(void*)&h->mat, (void*)&in, (void*)&out};
     return cudaLaunchKernel(fn, dim3(h->grid_aux), dim3(kThreads), args, 0, h->stream);
 }
 
 cudaError_t launch_dot(gpuqt_handle* h, const double2* l, const double2* r, double* result) {
     void* fn = dot_fn(h->B);
-    if (!h->grid_aux) h->grid_aux = grid_for(h, velocity_fn(h));
+    if (!h->grid_aux) h->grid_aux = grid_for(h, velocity_fn(h), 0, (h->N * h->B + kThreads - 1) / kThreads);
     long long N = h->N;
     void* args[] = {(void*)&N, (void*)&l, (void*)&r, (void*)&h->partials, (void*)&h->ticket, (void*)&result};
     return cudaLaunchKernel(fn, dim3(h->grid_aux), dim3(kThreads), args, 0, h->stream);
@@ -380,8 +390,9 @@ extern "C" {
 
 size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes) {
     if (N <= 0 || K_max <= 0 || !batch_ok(batch)) return 0;
-    const size_t entries = (size_t)((N + 31) / 32) * 32 * (size_t)K_max;
-    return make_layout(N, K_max, is_complex ? 1 : 0, batch, modes, entries).total;
+    // upper bound: every slice record padded to K_max
+    const size_t rec = (size_t)((N + 31) / 32) * (size_t)record_bytes(K_max, is_complex ? 1 : 0);
+    return make_layout(N, batch, modes, rec).total;
 }
 
 int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index,
@@ -425,10 +436,17 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->stream = (cudaStream_t)cuda_stream;
     h->vec_elems = (size_t)N * batch;
 
+    const int stage_bytes = (int)record_bytes(K_max, h->cplx);
+    if (step_smem_bytes(1, stage_bytes) > kSmemBudget) {
+        fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "
+                        "shared memory\n", K_max, stage_bytes);
+        delete h;
+        return GPUQT_ERR_ARG;
+    }
     SellHost sell;
-    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, sell);
-    const size_t entries = sell.col.size();
-    const Layout L = make_layout(N, K_max, h->cplx, batch, modes, entries);
+    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, sell);
+    const size_t rec_bytes = sell.rec.size();
+    const Layout L = make_layout(N, batch, modes, rec_bytes);
     if (L.total > workspace_bytes) {
         delete h;
         return GPUQT_ERR_NOMEM;
@@ -442,23 +460,15 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
         return GPUQT_ERR_CUDA;
     }
     char* base = (char*)workspace;
-    int32_t* d_col = (int32_t*)(base + L.col);
-    double* d_hre = (double*)(base + L.hre);
-    double* d_him = h->cplx ? (double*)(base + L.him) : nullptr;
-    double* d_on = (double*)(base + L.onsite);
+    unsigned char* d_rec = (unsigned char*)(base + L.rec);
     double* d_x = (double*)(base + L.x);
-    long long* d_sp = (long long*)(base + L.slice_ptr);
-    std::vector<double> on_host((size_t)N, 0.0);
-    if (onsite) memcpy(on_host.data(), onsite, (size_t)N * sizeof(double));
+    long long* d_sp = (long long*)(base + L.slice_off);
     auto up = [&](void* d, const void* s, size_t bytes) {
         return bytes ? cudaMemcpyAsync(d, s, bytes, cudaMemcpyHostToDevice, h->stream) : cudaSuccess;
     };
-    ce = up(d_col, sell.col.data(), entries * sizeof(int32_t));
-    if (ce == cudaSuccess) ce = up(d_hre, sell.hre.data(), entries * sizeof(double));
-    if (ce == cudaSuccess && h->cplx) ce = up(d_him, sell.him.data(), entries * sizeof(double));
-    if (ce == cudaSuccess) ce = up(d_on, on_host.data(), (size_t)N * sizeof(double));
+    ce = up(d_rec, sell.rec.data(), rec_bytes);
     if (ce == cudaSuccess) ce = up(d_x, x, (size_t)N * sizeof(double));
-    if (ce == cudaSuccess) ce = up(d_sp, sell.slice_ptr.data(), sell.slice_ptr.size() * sizeof(long long));
+    if (ce == cudaSuccess) ce = up(d_sp, sell.slice_off.data(), sell.slice_off.size() * sizeof(long long));
     if (ce == cudaSuccess) ce = cudaMemsetAsync(base + L.ticket, 0, 256, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
     if (ce != cudaSuccess) {
@@ -466,10 +476,22 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
         delete h;
         return GPUQT_ERR_CUDA;
     }
-    h->mat.col = d_col; h->mat.hre = d_hre; h->mat.him = d_him; h->mat.onsite = d_on; h->mat.x = d_x;
-    h->mat.slice_ptr = d_sp; h->mat.N = N; h->mat.K = K_max; h->mat.uniform = sell.uniform;
+    h->mat.rec = d_rec; h->mat.slice_off = d_sp; h->mat.x = d_x;
+    h->mat.N = N; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
+    h->mat.cplx = h->cplx; h->mat.stage_bytes = stage_bytes;
     h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
-    h->kt = (sell.uniform && (K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
+    h->kt = (sell.uniform && (K_max == 2 || K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
+    // Shared-memory stages per warp: one sub-step of a slice takes about one memory latency and a
+    // slice has `batch` sub-steps, so small batches need a deeper prefetch.  Tuning overrides:
+    // GPUQT_STAGES, GPUQT_BLOCKS_PER_SM, GPUQT_ALTERNATE.
+    int stages = env_int("GPUQT_STAGES", batch == 1 ? 4 : batch == 2 ? 3 : 2);
+    stages = std::max(1, std::min(stages, kMaxStages));
+    while (stages > 1 && step_smem_bytes(stages, stage_bytes) > kSmemBudget) --stages;
+    h->mat.stages = stages;
+    h->step_smem = step_smem_bytes(stages, stage_bytes);
+    h->max_blocks_per_sm = env_int("GPUQT_BLOCKS_PER_SM", 0);
+    h->alternate = env_int("GPUQT_ALTERNATE", 1);
+    h->run = std::max(1, env_int("GPUQT_RUN", 48) / kWarps) * kWarps;
 
     const size_t vstride = align_up((size_t)N * batch * sizeof(double2));
     char* v = base + L.vectors;
@@ -508,6 +530,7 @@ int gpuqt_set_state_device(gpuqt_handle* h, const double* phi_device) {
 }
 
 int gpuqt_dos_moments(gpuqt_handle* h, int32_t n_moments, double* out_host) {
+    if (h) h->sweep = 0;
     if (!h || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return fail(h, GPUQT_ERR_ARG, "bad n_moments or null output");
     if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
     int rc = moments_doubling(h, h->psi, n_moments);
@@ -516,6 +539,7 @@ int gpuqt_dos_moments(gpuqt_handle* h, int32_t n_moments, double* out_host) {
 }
 
 int gpuqt_msd(gpuqt_handle* h, int32_t n_moments, double* out_host) {
+    if (h) h->sweep = 0;
     if (!h || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return fail(h, GPUQT_ERR_ARG, "bad n_moments or null output");
     if (!(h->modes & GPUQT_MODE_MSD)) return fail(h, GPUQT_ERR_STATE, "handle was created without GPUQT_MODE_MSD");
     if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
@@ -525,6 +549,7 @@ int gpuqt_msd(gpuqt_handle* h, int32_t n_moments, double* out_host) {
 }
 
 int gpuqt_vac(gpuqt_handle* h, int32_t n_moments, double* out_host) {
+    if (h) h->sweep = 0;
     if (!h || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return fail(h, GPUQT_ERR_ARG, "bad n_moments or null output");
     if (!(h->modes & GPUQT_MODE_VAC)) return fail(h, GPUQT_ERR_STATE, "handle was created without GPUQT_MODE_VAC");
     if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
@@ -539,6 +564,7 @@ int gpuqt_vac(gpuqt_handle* h, int32_t n_moments, double* out_host) {
 }
 
 int gpuqt_evolve(gpuqt_handle* h, double dt, int32_t order) {
+    if (h) h->sweep = 0;
     if (!h || order < 1 || !std::isfinite(dt)) return fail(h, GPUQT_ERR_ARG, "bad dt or order");
     if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
     std::vector<double> cr, ci;

@@ -90,43 +90,58 @@ inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32
     return GPUQT_OK;
 }
 
-// Sliced-ELL table on the host: slices of 32 rows, column-major inside a slice.
+// Packed sliced-ELL table on the host (layout: kernels.cuh).  A slice is 32 rows; its record is
+//   double hre[w][32] | double him[w][32] (complex) | double onsite[32] | int32 col[w][32]
+// with w the largest neighbour count in the slice.  If padding every record to K_max costs less
+// than 1/16 extra bytes the table is stored uniform (w = K_max everywhere), which lets the
+// kernels compute record offsets arithmetically and unroll the neighbour walk.
 struct SellHost {
     int64_t n_slices = 0;
-    int uniform = 1;                    // every slice has width K_max
-    std::vector<long long> slice_ptr;   // [n_slices + 1] entry offsets
-    std::vector<int32_t> col;
-    std::vector<double> hre, him;
+    int uniform = 1;                    // every record has width K_max
+    std::vector<long long> slice_off;   // [n_slices + 1] byte offsets of the records
+    std::vector<unsigned char> rec;
 };
 
+inline long long host_record_bytes(int w, int cplx) { return 32LL * (8LL * w * (1 + cplx) + 8 + 4LL * w); }
+
 inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
-                       const double* hre, const double* him, SellHost& s) {
+                       const double* hre, const double* him, const double* onsite, SellHost& s) {
+    const int cplx = him ? 1 : 0;
     s.n_slices = (N + 31) / 32;
-    s.slice_ptr.assign((size_t)s.n_slices + 1, 0);
-    s.uniform = 1;
+    std::vector<int> width((size_t)s.n_slices, 0);
+    long long ragged = 0;
     for (int64_t sl = 0; sl < s.n_slices; ++sl) {
         int w = 0;
         for (int64_t m = sl * 32; m < std::min<int64_t>(N, sl * 32 + 32); ++m) w = std::max(w, cnt[m]);
-        if (w != K) s.uniform = 0;
-        s.slice_ptr[(size_t)sl + 1] = s.slice_ptr[(size_t)sl] + (long long)w * 32;
+        width[(size_t)sl] = w;
+        ragged += host_record_bytes(w, cplx);
     }
-    const size_t total = (size_t)s.slice_ptr[(size_t)s.n_slices];
-    s.col.assign(total, 0);
-    s.hre.assign(total, 0.0);
-    if (him) s.him.assign(total, 0.0);
+    const long long padded = (long long)s.n_slices * host_record_bytes(K, cplx);
+    s.uniform = (padded <= ragged + ragged / 16) ? 1 : 0;
+    s.slice_off.assign((size_t)s.n_slices + 1, 0);
     for (int64_t sl = 0; sl < s.n_slices; ++sl) {
-        const long long base = s.slice_ptr[(size_t)sl];
-        const int w = (int)((s.slice_ptr[(size_t)sl + 1] - base) / 32);
+        if (s.uniform) width[(size_t)sl] = K;
+        s.slice_off[(size_t)sl + 1] = s.slice_off[(size_t)sl] + host_record_bytes(width[(size_t)sl], cplx);
+    }
+    s.rec.assign((size_t)s.slice_off[(size_t)s.n_slices], 0);
+    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+        const int w = width[(size_t)sl];
+        unsigned char* base = s.rec.data() + s.slice_off[(size_t)sl];
+        double* r_hre = reinterpret_cast<double*>(base);
+        double* r_him = r_hre + (size_t)w * 32;
+        double* r_on = r_hre + (size_t)w * 32 * (1 + cplx);
+        int32_t* r_col = reinterpret_cast<int32_t*>(r_on + 32);
         for (int lane = 0; lane < 32; ++lane) {
             const int64_t m = sl * 32 + lane;
+            r_on[lane] = (m < N && onsite) ? onsite[m] : 0.0;
             for (int k = 0; k < w; ++k) {
-                const size_t e = (size_t)base + (size_t)k * 32 + lane;
+                const size_t e = (size_t)k * 32 + lane;
                 if (m < N && k < cnt[m]) {
-                    s.col[e] = idx[(size_t)m * K + k];
-                    s.hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
-                    if (him) s.him[e] = him[(size_t)m * K + k];
+                    r_col[e] = idx[(size_t)m * K + k];
+                    r_hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
+                    if (cplx) r_him[e] = him[(size_t)m * K + k];
                 } else {
-                    s.col[e] = (int32_t)(m < N ? m : N - 1);               // padding: own row, hop 0
+                    r_col[e] = (int32_t)(m < N ? m : N - 1);                   // padding: own row, hop 0
                 }
             }
         }

@@ -4,32 +4,67 @@
 // Layout
 //   vectors   complex fp64 [N][B] as double2: the B vectors of a row are contiguous (16*B bytes),
 //             so one neighbour index serves one 16*B-byte gather (B = 8: one 128-byte line).
-//   matrix    sliced ELL, slices of 32 rows, column-major inside a slice:
-//             entry(row, k) = slice_ptr[row / 32] + k * 32 + row % 32
-//             int32 col[], fp64 hre[], fp64 him[] (complex variant only), padding = (own row, 0).
-//   thread    one thread per (row, b): tid -> row = tid / B, b = tid % B.  Own-row vector
-//             loads/stores of a warp are one contiguous 512-byte segment.
+//   matrix    packed sliced ELL.  A slice is 32 consecutive rows; slice s of width w is ONE
+//             contiguous record, column-major inside the record:
+//                 double hre[w][32] | double him[w][32] (complex variant only) |
+//                 double onsite[32] | int32 col[w][32]
+//             record bytes = 32 * (8 w (1 + cplx) + 8 + 4 w), a multiple of 128.  Records are
+//             stored back to back; slice_off[s] is the byte offset of record s.  Padding entries
+//             are (a valid row, hop 0.0).  One record = one 1-D TMA bulk copy.
+//   warp      the unit of work is (warp, slice): a warp double/triple-buffers the records of its
+//             slices in shared memory with cp.async.bulk + mbarrier (no CTA-wide barrier in the
+//             loop), and walks the slice in B sub-steps of 32/B rows: lane -> (row = lane / B,
+//             b = lane % B).  Own-row vector loads/stores of a warp are one contiguous 512-byte
+//             segment; index/hopping reads come from shared memory, so all gathers of a sub-step
+//             are issued back to back.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#ifndef GPUQT_THREADS
+#define GPUQT_THREADS 256
+#endif
+#ifndef GPUQT_U_KPM        // sub-steps of a slice processed together (independent gathers in flight)
+#define GPUQT_U_KPM 2
+#endif
+#ifndef GPUQT_U_EVOLVE
+#define GPUQT_U_EVOLVE 2
+#endif
+#ifndef GPUQT_U_MSD
+#define GPUQT_U_MSD 1
+#endif
+
+#ifndef GPUQT_MINB
+#define GPUQT_MINB 4
+#endif
+#ifndef GPUQT_MINB_MSD
+#define GPUQT_MINB_MSD 2
+#endif
+
 namespace gpuqt {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = GPUQT_THREADS;
+constexpr int kWarps = kThreads / 32;
 constexpr int kSlice = 32;
+constexpr int kMaxStages = 4;
+
+__host__ __device__ __forceinline__ long long record_bytes(int w, int cplx) {
+    return 32LL * (8LL * w * (1 + cplx) + 8 + 4LL * w);
+}
 
 struct Mat {
-    const int32_t* __restrict__ col;
-    const double* __restrict__ hre;
-    const double* __restrict__ him;       // null in the real variant
-    const double* __restrict__ onsite;    // [N]
-    const double* __restrict__ x;         // [N]
-    const long long* __restrict__ slice_ptr;  // [n_slices + 1], entry offsets (multiples of 32)
+    const unsigned char* __restrict__ rec;      // packed slice records
+    const long long* __restrict__ slice_off;    // [n_slices + 1] byte offsets (ragged variant)
+    const double* __restrict__ x;               // [N]
     long long N;
-    int K;                                // K_max
-    int uniform;                          // every slice has width K
+    long long n_slices;
+    int K;                                      // K_max
+    int uniform;                                // every record has width K
+    int cplx;
+    int stages;                                 // shared-memory stages per warp
+    int stage_bytes;                            // record_bytes(K, cplx)
     double inv_dE;
-    double box;                           // <= 0: open boundary
+    double box;                                 // <= 0: open boundary
 };
 
 enum Mode : int {
@@ -53,14 +88,56 @@ struct StepArgs {
     double c0r, c0i;                     // c_0, used when first (acc = c_0 T_0 + c_1 T_1)
     int first;                           // T_1 = H~ T_0 (no factor 2, no prev)
     int store;                           // write T_m (0 on the last term of an evolve)
+    int reverse;                         // sweep the slices from the top (L2 reuse between launches)
+    int run;                             // consecutive slices one CTA walks before jumping (multiple of kWarps)
     double* partials;                    // [grid][Q*B]
     unsigned int* ticket;
     double* result;                      // [Q][B] reduced dots of this launch
 };
 
-__device__ __forceinline__ double2 ldcs2(const double2* p) {
-    return __ldcs(p);
+// ------------------------------------------------------------------ PTX helpers (TMA / mbarrier)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
 }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+// 1-D bulk copy global -> shared through the TMA unit; completion is signalled on `bar`.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar,
+                                         uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::
+            "r"(smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+
+__device__ __forceinline__ double2 ldcs2(const double2* p) { return __ldcs(p); }
 
 // minimum-image X_n - X_m  [A6]; pure add/sub so it is bit-identical to the oracle's
 __device__ __forceinline__ double min_image(double d, double box) {
@@ -77,7 +154,6 @@ __device__ __forceinline__ double min_image(double d, double box) {
 template <int B, int Q>
 __device__ __forceinline__ void block_reduce_and_finish(double (&v)[Q], double* partials,
                                                         unsigned int* ticket, double* result) {
-    constexpr int kWarps = kThreads / 32;
     __shared__ double s_part[kWarps][Q * B];
     __shared__ double s_tree[kThreads];
     __shared__ int s_last;
@@ -124,143 +200,326 @@ __device__ __forceinline__ void block_reduce_and_finish(double (&v)[Q], double* 
     if (tid == 0) *ticket = 0u;
 }
 
-// One Chebyshev recurrence step fused with what consumes it.
-template <int B, int KT, bool CPLX, int MODE>
-__global__ void __launch_bounds__(kThreads) cheb_step_kernel(const Mat m, const StepArgs a) {
-    constexpr int Q = (MODE == kModeDoubling) ? 3 : 2;
-    constexpr int kRows = kThreads / B;
-    const int tid = threadIdx.x;
-    const int b = tid % B;
-    const int rl = tid / B;
-    double red[Q];
-#pragma unroll
-    for (int q = 0; q < Q; ++q) red[q] = 0.0;
-    const long long n_chunks = (m.N + kRows - 1) / kRows;
-    const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
+template <int MODE>
+struct ModeTraits {
+    static constexpr int Q = (MODE == kModeDoubling) ? 3 : 2;
+    static constexpr int kMinBlocks = (MODE == kModeEvolveMsd) ? GPUQT_MINB_MSD : GPUQT_MINB;   // register cap
+    static constexpr int U = (MODE == kModeEvolveMsd) ? GPUQT_U_MSD
+                             : (MODE == kModeEvolve)  ? GPUQT_U_EVOLVE
+                                                      : GPUQT_U_KPM;
+};
 
-    for (long long chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
-        const long long row = chunk * kRows + rl;
-        if (row >= m.N) continue;
-        const size_t vi = (size_t)row * B + b;
-        long long e0;
-        int w;
-        if (KT > 0) {
-            e0 = (row >> 5) * (long long)(KT * kSlice) + (row & 31);
-            w = KT;
-        } else {
-            const long long s0 = m.slice_ptr[row >> 5], s1 = m.slice_ptr[(row >> 5) + 1];
-            e0 = s0 + (row & 31);
-            w = (int)((s1 - s0) >> 5);
-        }
-        const double2 self = a.in[vi];
-        const double u = __ldcs(&m.onsite[row]);
-        double sr = u * self.x, si = u * self.y;
-        double er = 0.0, ei = 0.0;     // H~ e_{m-1}
-        double xr = 0.0, xi = 0.0;     // [X,H] a_{m-1}
-        double2 self_e = make_double2(0.0, 0.0);
-        double xm = 0.0;
-        if (MODE == kModeEvolveMsd) {
-            self_e = a.in_e[vi];
-            er = u * self_e.x;
-            ei = u * self_e.y;
-            xm = m.x[row];
-        }
-        auto body = [&](int k) {
-            const long long e = e0 + (long long)k * kSlice;
-            const int c = __ldcs(&m.col[e]);
-            const double hr = __ldcs(&m.hre[e]);
-            double hi = 0.0;
-            if (CPLX) hi = __ldcs(&m.him[e]);
-            const double2 v = a.in[(size_t)c * B + b];
-            sr = fma(hr, v.x, sr);
-            si = fma(hr, v.y, si);
-            if (CPLX) {
-                sr = fma(-hi, v.y, sr);
-                si = fma(hi, v.x, si);
-            }
-            if (MODE == kModeEvolveMsd) {
-                const double2 ve = a.in_e[(size_t)c * B + b];
-                er = fma(hr, ve.x, er);
-                ei = fma(hr, ve.y, ei);
-                if (CPLX) {
-                    er = fma(-hi, ve.y, er);
-                    ei = fma(hi, ve.x, ei);
-                }
-                // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
-                const double ndx = -min_image(m.x[c] - xm, m.box);
-                const double wr = ndx * hr;
-                xr = fma(wr, v.x, xr);
-                xi = fma(wr, v.y, xi);
-                if (CPLX) {
-                    const double wi = ndx * hi;
-                    xr = fma(-wi, v.y, xr);
-                    xi = fma(wi, v.x, xi);
-                }
-            }
-        };
-        if (KT > 0) {
+// U sub-steps (U * 32/B rows) of one slice whose record sits in shared memory at `stage`.
+template <int B, int KT, bool CPLX, int MODE, int U>
+__device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
+                                          long long slice, int j0, int lane, double scale,
+                                          double (&red)[ModeTraits<MODE>::Q]) {
+    constexpr int RS = 32 / B;
+    constexpr int KU = KT > 0 ? KT : 1;
+    const int rl = lane / B, b = lane % B;
+    const double* s_hre = reinterpret_cast<const double*>(stage);
+    const double* s_him = s_hre + (size_t)w * 32;
+    const double* s_on = s_hre + (size_t)w * 32 * (CPLX ? 2 : 1);
+    const int* s_col = reinterpret_cast<const int*>(s_on + 32);
+
+    int r[U];
+    bool ok[U];
+    size_t vi[U];
+    double2 self[U], self_e[U], prev[U], prev_e[U], other[U], other_e[U];
+    double sr[U], si[U], er[U], ei[U], xr[U], xi[U], xm[U];
 #pragma unroll
-            for (int k = 0; k < KT; ++k) body(k);
-        } else {
-            for (int k = 0; k < w; ++k) body(k);
+    for (int u = 0; u < U; ++u) {
+        r[u] = (j0 + u) * RS + rl;
+        long long row = slice * 32 + r[u];
+        ok[u] = row < m.N;
+        if (!ok[u]) row = m.N - 1;
+        vi[u] = (size_t)row * B + b;
+        self[u] = a.in[vi[u]];
+        if (MODE == kModeEvolveMsd) {
+            self_e[u] = a.in_e[vi[u]];
+            xm[u] = m.x[row];
         }
-        double2 t;   // T_m
-        t.x = scale * sr;
-        t.y = scale * si;
+        // streamed own-row operands: issued with the gathers so one memory round trip covers all
+        prev[u] = prev_e[u] = other[u] = other_e[u] = make_double2(0.0, 0.0);
         if (!a.first) {
-            const double2 p = ldcs2(&a.prev[vi]);
-            t.x -= p.x;
-            t.y -= p.y;
+            prev[u] = ldcs2(&a.prev[vi[u]]);
+            if (MODE == kModeEvolveMsd) prev_e[u] = ldcs2(&a.prev_e[vi[u]]);
+            if (MODE == kModeEvolve || MODE == kModeEvolveMsd) other[u] = ldcs2(&a.acc[vi[u]]);
+            if (MODE == kModeEvolveMsd) other_e[u] = ldcs2(&a.acc_e[vi[u]]);
         }
-        if (a.store) a.out[vi] = t;
+        if (MODE == kModeLeft) other[u] = ldcs2(&a.phiL[vi[u]]);
+    }
+    if (KT > 0) {
+        // all gathers of the U rows first (independent loads in flight), then the arithmetic
+        double2 v[U][KU], ve[U][KU];
+        double xn[U][KU];
+#pragma unroll
+        for (int k = 0; k < KU; ++k) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int c = s_col[k * 32 + r[u]];
+                v[u][k] = a.in[(size_t)c * B + b];
+                if (MODE == kModeEvolveMsd) {
+                    ve[u][k] = a.in_e[(size_t)c * B + b];
+                    xn[u][k] = m.x[c];
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const double on = s_on[r[u]];
+            sr[u] = on * self[u].x;
+            si[u] = on * self[u].y;
+            er[u] = ei[u] = xr[u] = xi[u] = 0.0;
+            if (MODE == kModeEvolveMsd) {
+                er[u] = on * self_e[u].x;
+                ei[u] = on * self_e[u].y;
+            }
+#pragma unroll
+            for (int k = 0; k < KU; ++k) {
+                const double hr = s_hre[k * 32 + r[u]];
+                double hi = 0.0;
+                if (CPLX) hi = s_him[k * 32 + r[u]];
+                sr[u] = fma(hr, v[u][k].x, sr[u]);
+                si[u] = fma(hr, v[u][k].y, si[u]);
+                if (CPLX) {
+                    sr[u] = fma(-hi, v[u][k].y, sr[u]);
+                    si[u] = fma(hi, v[u][k].x, si[u]);
+                }
+                if (MODE == kModeEvolveMsd) {
+                    er[u] = fma(hr, ve[u][k].x, er[u]);
+                    ei[u] = fma(hr, ve[u][k].y, ei[u]);
+                    if (CPLX) {
+                        er[u] = fma(-hi, ve[u][k].y, er[u]);
+                        ei[u] = fma(hi, ve[u][k].x, ei[u]);
+                    }
+                    // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
+                    const double ndx = -min_image(xn[u][k] - xm[u], m.box);
+                    const double wr = ndx * hr;
+                    xr[u] = fma(wr, v[u][k].x, xr[u]);
+                    xi[u] = fma(wr, v[u][k].y, xi[u]);
+                    if (CPLX) {
+                        const double wi = ndx * hi;
+                        xr[u] = fma(-wi, v[u][k].y, xr[u]);
+                        xi[u] = fma(wi, v[u][k].x, xi[u]);
+                    }
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const double on = s_on[r[u]];
+            sr[u] = on * self[u].x;
+            si[u] = on * self[u].y;
+            er[u] = ei[u] = xr[u] = xi[u] = 0.0;
+            if (MODE == kModeEvolveMsd) {
+                er[u] = on * self_e[u].x;
+                ei[u] = on * self_e[u].y;
+            }
+        }
+        for (int k = 0; k < w; ++k) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int c = s_col[k * 32 + r[u]];
+                const double hr = s_hre[k * 32 + r[u]];
+                double hi = 0.0;
+                if (CPLX) hi = s_him[k * 32 + r[u]];
+                const double2 vv = a.in[(size_t)c * B + b];
+                sr[u] = fma(hr, vv.x, sr[u]);
+                si[u] = fma(hr, vv.y, si[u]);
+                if (CPLX) {
+                    sr[u] = fma(-hi, vv.y, sr[u]);
+                    si[u] = fma(hi, vv.x, si[u]);
+                }
+                if (MODE == kModeEvolveMsd) {
+                    const double2 vve = a.in_e[(size_t)c * B + b];
+                    er[u] = fma(hr, vve.x, er[u]);
+                    ei[u] = fma(hr, vve.y, ei[u]);
+                    if (CPLX) {
+                        er[u] = fma(-hi, vve.y, er[u]);
+                        ei[u] = fma(hi, vve.x, ei[u]);
+                    }
+                    const double ndx = -min_image(m.x[c] - xm[u], m.box);
+                    const double wr = ndx * hr;
+                    xr[u] = fma(wr, vv.x, xr[u]);
+                    xi[u] = fma(wr, vv.y, xi[u]);
+                    if (CPLX) {
+                        const double wi = ndx * hi;
+                        xr[u] = fma(-wi, vv.y, xr[u]);
+                        xi[u] = fma(wi, vv.x, xi[u]);
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        double2 t;   // T_m
+        t.x = scale * sr[u];
+        t.y = scale * si[u];
+        t.x -= prev[u].x;
+        t.y -= prev[u].y;
+        if (a.store && ok[u]) a.out[vi[u]] = t;
         if (MODE == kModeDoubling) {
-            red[0] += t.x * t.x + t.y * t.y;
-            red[1] += t.x * self.x + t.y * self.y;
-            red[2] += self.x * self.x + self.y * self.y;
+            if (ok[u]) {
+                red[0] += t.x * t.x + t.y * t.y;
+                red[1] += t.x * self[u].x + t.y * self[u].y;
+                red[2] += self[u].x * self[u].x + self[u].y * self[u].y;
+            }
         } else if (MODE == kModeLeft) {
-            const double2 l = ldcs2(&a.phiL[vi]);
-            red[0] += l.x * t.x + l.y * t.y;       // conj(l) * t
-            red[1] += l.x * t.y - l.y * t.x;
+            const double2 l = other[u];
+            if (ok[u]) {
+                red[0] += l.x * t.x + l.y * t.y;       // conj(l) * t
+                red[1] += l.x * t.y - l.y * t.x;
+            }
         } else {
             double2 acc;
             if (a.first) {
-                acc.x = a.c0r * self.x - a.c0i * self.y;
-                acc.y = a.c0r * self.y + a.c0i * self.x;
+                acc.x = a.c0r * self[u].x - a.c0i * self[u].y;
+                acc.y = a.c0r * self[u].y + a.c0i * self[u].x;
             } else {
-                acc = a.acc[vi];
+                acc = other[u];
             }
             acc.x += a.cr * t.x - a.ci * t.y;
             acc.y += a.cr * t.y + a.ci * t.x;
-            a.acc[vi] = acc;
+            if (ok[u]) a.acc[vi[u]] = acc;
             if (MODE == kModeEvolveMsd) {
                 double2 te;
-                te.x = scale * (er + xr);
-                te.y = scale * (ei + xi);
-                if (!a.first) {
-                    const double2 p = ldcs2(&a.prev_e[vi]);
-                    te.x -= p.x;
-                    te.y -= p.y;
-                }
-                if (a.store) a.out_e[vi] = te;
+                te.x = scale * (er[u] + xr[u]);
+                te.y = scale * (ei[u] + xi[u]);
+                te.x -= prev_e[u].x;
+                te.y -= prev_e[u].y;
+                if (a.store && ok[u]) a.out_e[vi[u]] = te;
                 double2 ae;
                 if (a.first) {
-                    ae.x = a.c0r * self_e.x - a.c0i * self_e.y;
-                    ae.y = a.c0r * self_e.y + a.c0i * self_e.x;
+                    ae.x = a.c0r * self_e[u].x - a.c0i * self_e[u].y;
+                    ae.y = a.c0r * self_e[u].y + a.c0i * self_e[u].x;
                 } else {
-                    ae = a.acc_e[vi];
+                    ae = other_e[u];
                 }
                 ae.x += a.cr * te.x - a.ci * te.y;
                 ae.y += a.cr * te.y + a.ci * te.x;
-                a.acc_e[vi] = ae;
+                if (ok[u]) a.acc_e[vi[u]] = ae;
             }
         }
+    }
+}
+
+// One Chebyshev recurrence step fused with what consumes it.  Persistent warps: global warp g
+// takes slices g, g + W, g + 2W, ... (W = warps in the grid), so neighbouring warps stream
+// neighbouring slices and the gathered rows stay hot in L1/L2.
+template <int B, int KT, bool CPLX, int MODE>
+__global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
+    constexpr int Q = ModeTraits<MODE>::Q;
+    constexpr int U = ModeTraits<MODE>::U < B ? ModeTraits<MODE>::U : B;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int stages = m.stages;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + warp * kMaxStages;
+    unsigned char* wstage = smem + 128 * ((kWarps * kMaxStages * 8 + 127) / 128) + (size_t)warp * stages * m.stage_bytes;
+
+    double red[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) red[q] = 0.0;
+    const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
+
+    // Work split: the slices are cut into runs of a.run consecutive slices; CTA c walks runs
+    // c, c + G, c + 2G, ...; inside a run warp w takes slices w, w + kWarps, ...  A CTA therefore
+    // streams a contiguous band of rows, so gathers to nearby rows (the +-x, +-y neighbours of a
+    // lattice) are served by the SM's L1 instead of L2.
+    const int per = a.run / kWarps;
+    const long long n_runs = (m.n_slices + a.run - 1) / a.run;
+    const long long G = gridDim.x;
+    const long long my_runs = blockIdx.x < n_runs ? (n_runs - blockIdx.x + G - 1) / G : 0;
+    long long n_my = 0;
+    if (my_runs > 0) {
+        const long long last = blockIdx.x + (my_runs - 1) * G;
+        const long long rem = m.n_slices - last * a.run;          // slices in my last run (may be partial)
+        const long long in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
+        n_my = (my_runs - 1) * per + in_last;
+    }
+    uint64_t policy = 0;
+    if (lane == 0) {
+        for (int s = 0; s < stages; ++s) mbar_init(&bars[s], 1);
+        fence_mbar_init();
+        policy = policy_evict_first();
+    }
+    __syncwarp();
+
+    auto slice_of = [&](long long i) {
+        const long long s = (blockIdx.x + (i / per) * G) * a.run + warp + (long long)kWarps * (i % per);
+        return a.reverse ? m.n_slices - 1 - s : s;
+    };
+    auto issue = [&](long long i) {   // lane 0 only
+        const long long s = slice_of(i);
+        long long off, bytes;
+        if (KT > 0) {
+            bytes = record_bytes(KT, CPLX ? 1 : 0);
+            off = s * bytes;
+        } else {
+            off = m.slice_off[s];
+            bytes = m.slice_off[s + 1] - off;
+        }
+        const int st = (int)(i % stages);
+        mbar_expect_tx(&bars[st], (uint32_t)bytes);
+        bulk_g2s(wstage + (size_t)st * m.stage_bytes, m.rec + off, (uint32_t)bytes, &bars[st], policy);
+    };
+
+    if (lane == 0) {
+        for (long long i = 0; i < stages - 1 && i < n_my; ++i) issue(i);
+    }
+    for (long long i = 0; i < n_my; ++i) {
+        // stage (i - 1) % stages was consumed by the whole warp in the previous iteration
+        if (lane == 0 && i + stages - 1 < n_my) issue(i + stages - 1);
+        const int st = (int)(i % stages);
+        mbar_wait(&bars[st], (uint32_t)((i / stages) & 1));
+        const unsigned char* stage = wstage + (size_t)st * m.stage_bytes;
+        const long long slice = slice_of(i);
+        int w = KT;
+        if (KT == 0) {
+            const long long bytes = m.slice_off[slice + 1] - m.slice_off[slice];
+            w = (int)((bytes / 32 - 8) / (CPLX ? 20 : 12));
+        }
+#pragma unroll 1
+        for (int j0 = 0; j0 < B; j0 += U)
+            walk_rows<B, KT, CPLX, MODE, U>(m, a, stage, w, slice, j0, lane, scale, red);
+        __syncwarp();
     }
     if (MODE == kModeDoubling || MODE == kModeLeft)
         block_reduce_and_finish<B, Q>(red, a.partials, a.ticket, a.result);
 }
 
-// out = V in,  V_mn = i (X_n - X_m) H_mn  (Eq. 34) — not scaled by 1/dE, no on-site
-template <int B, int KT, bool CPLX>
+// Address of entry (row, k) pieces inside the packed records (plain global reads; used by the
+// rarely-run kernels below).
+struct RecView {
+    const double* hre;
+    const double* him;
+    const double* on;
+    const int* col;
+    int w;
+};
+__device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
+    long long off, bytes;
+    if (m.uniform) {
+        bytes = record_bytes(m.K, m.cplx);
+        off = slice * bytes;
+    } else {
+        off = m.slice_off[slice];
+        bytes = m.slice_off[slice + 1] - off;
+    }
+    RecView v;
+    v.w = (int)((bytes / 32 - 8) / (m.cplx ? 20 : 12));
+    v.hre = reinterpret_cast<const double*>(m.rec + off);
+    v.him = v.hre + (size_t)v.w * 32;
+    v.on = v.hre + (size_t)v.w * 32 * (m.cplx ? 2 : 1);
+    v.col = reinterpret_cast<const int*>(v.on + 32);
+    return v;
+}
+
+// out = V in,  V_mn = i (X_n - X_m) H_mn  (Eq. 34) — not scaled by 1/dE, no on-site.
+// Runs once per VAC measurement (1 of N_m walks), so it reads the records straight from global.
+template <int B>
 __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const double2* __restrict__ in,
                                                             double2* __restrict__ out) {
     constexpr int kRows = kThreads / B;
@@ -269,37 +528,22 @@ __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const d
     for (long long chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
         const long long row = chunk * kRows + rl;
         if (row >= m.N) continue;
-        long long e0;
-        int w;
-        if (KT > 0) {
-            e0 = (row >> 5) * (long long)(KT * kSlice) + (row & 31);
-            w = KT;
-        } else {
-            const long long s0 = m.slice_ptr[row >> 5], s1 = m.slice_ptr[(row >> 5) + 1];
-            e0 = s0 + (row & 31);
-            w = (int)((s1 - s0) >> 5);
-        }
+        const RecView rv = record_view(m, row >> 5);
+        const int r = (int)(row & 31);
         const double xm = m.x[row];
         double sr = 0.0, si = 0.0;
-        auto body = [&](int k) {
-            const long long e = e0 + (long long)k * kSlice;
-            const int c = __ldcs(&m.col[e]);
+        for (int k = 0; k < rv.w; ++k) {
+            const int c = rv.col[k * 32 + r];
             const double dx = min_image(m.x[c] - xm, m.box);
-            const double wr = dx * __ldcs(&m.hre[e]);
+            const double wr = dx * rv.hre[k * 32 + r];
             const double2 v = in[(size_t)c * B + b];
             sr = fma(wr, v.x, sr);
             si = fma(wr, v.y, si);
-            if (CPLX) {
-                const double wi = dx * __ldcs(&m.him[e]);
+            if (m.cplx) {
+                const double wi = dx * rv.him[k * 32 + r];
                 sr = fma(-wi, v.y, sr);
                 si = fma(wi, v.x, si);
             }
-        };
-        if (KT > 0) {
-#pragma unroll
-            for (int k = 0; k < KT; ++k) body(k);
-        } else {
-            for (int k = 0; k < w; ++k) body(k);
         }
         out[(size_t)row * B + b] = make_double2(-si, sr);   // multiply by i
     }
@@ -400,22 +644,21 @@ __global__ void transform_kernel(int n_moments, int n_sets, int n_energies, cons
     out[i] = pref * sum;
 }
 
-// Decode the sliced-ELL table back to canonical padded row-major arrays (bit-exact check)
+// Decode the packed records back to canonical padded row-major arrays (bit-exact check)
 __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __restrict__ re,
                              double* __restrict__ im, double* __restrict__ dx) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.N * m.K) return;
     const long long row = i / m.K;
     const int k = (int)(i % m.K);
-    const long long s0 = m.slice_ptr[row >> 5], s1 = m.slice_ptr[(row >> 5) + 1];
-    const int w = (int)((s1 - s0) >> 5);
+    const RecView rv = record_view(m, row >> 5);
+    const int r = (int)(row & 31);
     int c = (int)row;
     double hr = 0.0, hi = 0.0, d = 0.0;
-    if (k < w) {
-        const long long e = s0 + (long long)k * kSlice + (row & 31);
-        c = m.col[e];
-        hr = m.hre[e];
-        if (m.him) hi = m.him[e];
+    if (k < rv.w) {
+        c = rv.col[k * 32 + r];
+        hr = rv.hre[k * 32 + r];
+        if (m.cplx) hi = rv.him[k * 32 + r];
         d = min_image(m.x[c] - m.x[row], m.box);
     }
     if (col) col[i] = c;
