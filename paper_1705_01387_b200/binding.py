@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgpuqt.so")
+LIB_PATH = os.environ.get("GPUQT_LIB") or os.path.join(_HERE, "libgpuqt.so")
 
 MODE_VAC, MODE_MSD, MODE_PSI = 1, 2, 4
 STATE_PSI, STATE_CHI, STATE_VAC_A, STATE_VAC_B = 0, 1, 2, 3

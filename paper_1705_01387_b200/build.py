@@ -5,7 +5,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libgpuqt.so")
+LIB = os.environ.get("GPUQT_LIB") or os.path.join(HERE, "libgpuqt.so")
 SOURCES = [os.path.join(CSRC, "gpuqt.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "host_util.h")] + [
     os.path.join(os.path.dirname(HERE), "include", "gpuqt.h")]
@@ -23,7 +23,8 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+        extra = os.environ.get("GPUQT_NVCC_EXTRA", "").split()      # e.g. -DGPUQT_U_KPM=4 (kernel tuning macros)
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
         subprocess.check_call(cmd)
     return LIB
 

@@ -32,7 +32,11 @@ struct gpuqt_handle {
     int max_blocks_per_sm = 0;          // GPUQT_BLOCKS_PER_SM (tuning override), 0 = occupancy limit
     int run = kWarps;                   // GPUQT_RUN: consecutive slices per CTA run (multiple of kWarps)
     int alternate = 1;                  // GPUQT_ALTERNATE: sweep direction alternates between launches
-    size_t step_smem = 0;               // dynamic shared memory of the staged step kernels
+    int rec_bytes = 0;                  // bytes of one (widest) slice record
+    int want_stages = 2;                // requested pipeline depth per warp
+    int mode_stages[4] = {0, 0, 0, 0};  // per step-kernel mode: stages, bytes per stage, dynamic smem
+    int mode_stage_bytes[4] = {0, 0, 0, 0};
+    size_t mode_smem[4] = {0, 0, 0, 0};
     std::vector<void*> smem_set;        // kernels whose dynamic-smem attribute has been raised
     double dE = 0, box = 0, volume = 0;
     cudaStream_t stream = nullptr;
@@ -109,7 +113,8 @@ Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
 size_t step_smem_bytes(int stages, int stage_bytes) {
     return 128 * (((size_t)kWarps * kMaxStages * 8 + 127) / 128) + (size_t)kWarps * stages * stage_bytes;
 }
-constexpr size_t kSmemBudget = 200 * 1024;   // leaves room for the static reduction buffers
+constexpr size_t kSmemBudget = 200 * 1024;   // per CTA; leaves room for the static reduction buffers
+constexpr size_t kSmemPerSm = 227 * 1024;
 
 int env_int(const char* name, int dflt) {
     const char* v = getenv(name);
@@ -180,22 +185,40 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items) {
     return (int)g;
 }
 
+// bytes of one stage of a step kernel: the record plus the staged own rows of T_{m-1}, T_{m-2}
+// (and e_{m-1}, e_{m-2} for the (a, e) pair)
+int mode_stage_bytes_for(const gpuqt_handle* h, int mode) {
+    const int streams = (mode == kModeEvolveMsd) ? 4 : 2;
+    return h->rec_bytes + streams * 32 * h->B * (int)sizeof(double2);
+}
+
 cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
     void* fn = step_kernel(h, mode);
     if (!h->grid[mode]) {
-        if (h->step_smem > 48 * 1024) {
-            cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->step_smem);
+        const int sb = mode_stage_bytes_for(h, mode);
+        int stages = h->want_stages;
+        while (stages > 1 && step_smem_bytes(stages, sb) > kSmemBudget) --stages;
+        // prefer two resident CTAs per SM over a deeper pipeline
+        while (stages > 2 && 2 * (step_smem_bytes(stages, sb) + 4096) > kSmemPerSm) --stages;
+        h->mode_stages[mode] = stages;
+        h->mode_stage_bytes[mode] = sb;
+        h->mode_smem[mode] = step_smem_bytes(stages, sb);
+        if (h->mode_smem[mode] > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->mode_smem[mode]);
             if (e != cudaSuccess) return e;
         }
-        h->grid[mode] = grid_for(h, fn, h->step_smem, (h->mat.n_slices + h->run - 1) / h->run);
+        h->grid[mode] = grid_for(h, fn, h->mode_smem[mode], (h->mat.n_slices + h->run - 1) / h->run);
     }
+    a.stages = h->mode_stages[mode];
+    a.stage_bytes = h->mode_stage_bytes[mode];
+    a.rec_bytes = h->rec_bytes;
     a.partials = h->partials;
     a.ticket = h->ticket;
     a.reverse = h->alternate ? (h->sweep & 1) : 0;
     a.run = h->run;
     h->sweep ^= 1;
     void* args[] = {(void*)&h->mat, (void*)&a};
-    return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, h->step_smem, h->stream);
+    return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, h->mode_smem[mode], h->stream);
 }
 
 cudaError_t launch_velocity(gpuqt_handle* h, const double2* in, double2* out) {
@@ -437,7 +460,8 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->vec_elems = (size_t)N * batch;
 
     const int stage_bytes = (int)record_bytes(K_max, h->cplx);
-    if (step_smem_bytes(1, stage_bytes) > kSmemBudget) {
+    h->rec_bytes = stage_bytes;
+    if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd)) > kSmemBudget) {
         fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "
                         "shared memory\n", K_max, stage_bytes);
         delete h;
@@ -478,7 +502,7 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     }
     h->mat.rec = d_rec; h->mat.slice_off = d_sp; h->mat.x = d_x;
     h->mat.N = N; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
-    h->mat.cplx = h->cplx; h->mat.stage_bytes = stage_bytes;
+    h->mat.cplx = h->cplx;
     h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
     h->kt = (sell.uniform && (K_max == 2 || K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
     // Shared-memory stages per warp: one sub-step of a slice takes about one memory latency and a
@@ -486,12 +510,10 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     // GPUQT_STAGES, GPUQT_BLOCKS_PER_SM, GPUQT_ALTERNATE.
     int stages = env_int("GPUQT_STAGES", batch == 1 ? 4 : batch == 2 ? 3 : 2);
     stages = std::max(1, std::min(stages, kMaxStages));
-    while (stages > 1 && step_smem_bytes(stages, stage_bytes) > kSmemBudget) --stages;
-    h->mat.stages = stages;
-    h->step_smem = step_smem_bytes(stages, stage_bytes);
+    h->want_stages = stages;
     h->max_blocks_per_sm = env_int("GPUQT_BLOCKS_PER_SM", 0);
     h->alternate = env_int("GPUQT_ALTERNATE", 1);
-    h->run = std::max(1, env_int("GPUQT_RUN", 48) / kWarps) * kWarps;
+    h->run = std::max(1, env_int("GPUQT_RUN", 16) / kWarps) * kWarps;
 
     const size_t vstride = align_up((size_t)N * batch * sizeof(double2));
     char* v = base + L.vectors;

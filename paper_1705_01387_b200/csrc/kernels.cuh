@@ -11,12 +11,16 @@
 //             record bytes = 32 * (8 w (1 + cplx) + 8 + 4 w), a multiple of 128.  Records are
 //             stored back to back; slice_off[s] is the byte offset of record s.  Padding entries
 //             are (a valid row, hop 0.0).  One record = one 1-D TMA bulk copy.
-//   warp      the unit of work is (warp, slice): a warp double/triple-buffers the records of its
-//             slices in shared memory with cp.async.bulk + mbarrier (no CTA-wide barrier in the
-//             loop), and walks the slice in B sub-steps of 32/B rows: lane -> (row = lane / B,
-//             b = lane % B).  Own-row vector loads/stores of a warp are one contiguous 512-byte
-//             segment; index/hopping reads come from shared memory, so all gathers of a sub-step
-//             are issued back to back.
+//   warp      the unit of work is (warp, slice).  A stage of a warp's shared-memory pipeline holds
+//             everything the slice streams from HBM exactly once: the packed record, the slice's
+//             own rows of T_{m-1} (and e_{m-1}) and of T_{m-2} (and e_{m-2}) -- each one 1-D TMA
+//             bulk copy (cp.async.bulk + mbarrier, no CTA-wide barrier in the loop), issued one or
+//             more slices ahead, so the DRAM streams never sit on a warp's scoreboard.  The warp
+//             walks the slice in B sub-steps of 32/B rows: lane -> (row = lane / B, b = lane % B).
+//             Neighbours inside the slice are read from the staged rows in shared memory; the
+//             others are gathered from global memory (L1/L2 hits along the sweep front), all
+//             gathers of a sub-step group issued back to back.  Stores of a warp are one
+//             contiguous 512-byte segment.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -35,10 +39,21 @@
 #endif
 
 #ifndef GPUQT_MINB
-#define GPUQT_MINB 4
+#define GPUQT_MINB 2
 #endif
 #ifndef GPUQT_MINB_MSD
 #define GPUQT_MINB_MSD 2
+#endif
+
+// L2 policy experiments
+#ifndef GPUQT_GATHER_POLICY   // 0: plain ld.global, 1: L2::evict_last
+#define GPUQT_GATHER_POLICY 1
+#endif
+#ifndef GPUQT_IN_POLICY       // own rows of T_{m-1} by TMA: 0 no hint, 1 evict_last
+#define GPUQT_IN_POLICY 0
+#endif
+#ifndef GPUQT_ST_POLICY       // stores of T_m / acc: 0 plain, 1 st.global.cs (evict-first)
+#define GPUQT_ST_POLICY 0
 #endif
 
 namespace gpuqt {
@@ -61,8 +76,6 @@ struct Mat {
     int K;                                      // K_max
     int uniform;                                // every record has width K
     int cplx;
-    int stages;                                 // shared-memory stages per warp
-    int stage_bytes;                            // record_bytes(K, cplx)
     double inv_dE;
     double box;                                 // <= 0: open boundary
 };
@@ -90,6 +103,9 @@ struct StepArgs {
     int store;                           // write T_m (0 on the last term of an evolve)
     int reverse;                         // sweep the slices from the top (L2 reuse between launches)
     int run;                             // consecutive slices one CTA walks before jumping (multiple of kWarps)
+    int stages;                          // shared-memory stages per warp (<= kMaxStages)
+    int stage_bytes;                     // bytes of one stage: record + staged vector rows
+    int rec_bytes;                       // bytes reserved for the record inside a stage
     double* partials;                    // [grid][Q*B]
     unsigned int* ticket;
     double* result;                      // [Q][B] reduced dots of this launch
@@ -137,6 +153,26 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
         : "memory");
 }
 
+__device__ __forceinline__ void bulk_g2s_nohint(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_vec(double2* p, double2 v) {
+#if GPUQT_ST_POLICY == 1
+    __stcs(p, v);
+#else
+    *p = v;
+#endif
+}
 __device__ __forceinline__ double2 ldcs2(const double2* p) { return __ldcs(p); }
 
 // minimum-image X_n - X_m  [A6]; pure add/sub so it is bit-identical to the oracle's
@@ -209,7 +245,29 @@ struct ModeTraits {
                                                       : GPUQT_U_KPM;
 };
 
-// U sub-steps (U * 32/B rows) of one slice whose record sits in shared memory at `stage`.
+// Number of vector streams staged per slice: own rows of T_{m-1}, T_{m-2} (x2 for the (a, e) pair).
+template <int MODE>
+struct StagedStreams {
+    static constexpr int value = (MODE == kModeEvolveMsd) ? 4 : 2;
+};
+
+// Gather of T_{m-1}[c]: rows of the current slice come from the staged copy in shared memory.
+template <int B>
+__device__ __forceinline__ double2 gather(const double2* __restrict__ g, const double2* s_own, int c, int row0, int b) {
+    const unsigned d = (unsigned)(c - row0);
+    if (d < 32u) return s_own[d * B + b];
+#if GPUQT_GATHER_POLICY == 1
+    double2 v;
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(g + (size_t)c * B + b), "l"(pol));
+    return v;
+#else
+    return g[(size_t)c * B + b];
+#endif
+}
+
+// U sub-steps (U * 32/B rows) of one slice whose record and own rows sit in shared memory at `stage`.
 template <int B, int KT, bool CPLX, int MODE, int U>
 __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
                                           long long slice, int j0, int lane, double scale,
@@ -221,6 +279,12 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
     const double* s_him = s_hre + (size_t)w * 32;
     const double* s_on = s_hre + (size_t)w * 32 * (CPLX ? 2 : 1);
     const int* s_col = reinterpret_cast<const int*>(s_on + 32);
+    // staged vector rows: [in | (in_e) | prev | (prev_e)], each 32 * B double2
+    const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
+    const double2* s_in_e = s_in + 32 * B;
+    const double2* s_prev = s_in + (MODE == kModeEvolveMsd ? 2 : 1) * 32 * B;
+    const double2* s_prev_e = s_prev + 32 * B;
+    const int row0 = (int)(slice * 32);
 
     int r[U];
     bool ok[U];
@@ -234,20 +298,25 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
         ok[u] = row < m.N;
         if (!ok[u]) row = m.N - 1;
         vi[u] = (size_t)row * B + b;
-        self[u] = a.in[vi[u]];
-        if (MODE == kModeEvolveMsd) {
-            self_e[u] = a.in_e[vi[u]];
-            xm[u] = m.x[row];
-        }
-        // streamed own-row operands: issued with the gathers so one memory round trip covers all
-        prev[u] = prev_e[u] = other[u] = other_e[u] = make_double2(0.0, 0.0);
+        // streamed read-modify-write operands: issued first, consumed last
+        other[u] = other_e[u] = make_double2(0.0, 0.0);
         if (!a.first) {
-            prev[u] = ldcs2(&a.prev[vi[u]]);
-            if (MODE == kModeEvolveMsd) prev_e[u] = ldcs2(&a.prev_e[vi[u]]);
             if (MODE == kModeEvolve || MODE == kModeEvolveMsd) other[u] = ldcs2(&a.acc[vi[u]]);
             if (MODE == kModeEvolveMsd) other_e[u] = ldcs2(&a.acc_e[vi[u]]);
         }
         if (MODE == kModeLeft) other[u] = ldcs2(&a.phiL[vi[u]]);
+        if (MODE == kModeEvolveMsd) xm[u] = m.x[row];
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const int si_ = r[u] * B + b;
+        self[u] = ok[u] ? s_in[si_] : make_double2(0.0, 0.0);
+        self_e[u] = prev[u] = prev_e[u] = make_double2(0.0, 0.0);
+        if (MODE == kModeEvolveMsd) self_e[u] = ok[u] ? s_in_e[si_] : make_double2(0.0, 0.0);
+        if (!a.first) {
+            if (ok[u]) prev[u] = s_prev[si_];
+            if (MODE == kModeEvolveMsd && ok[u]) prev_e[u] = s_prev_e[si_];
+        }
     }
     if (KT > 0) {
         // all gathers of the U rows first (independent loads in flight), then the arithmetic
@@ -258,9 +327,9 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int c = s_col[k * 32 + r[u]];
-                v[u][k] = a.in[(size_t)c * B + b];
+                v[u][k] = gather<B>(a.in, s_in, c, row0, b);
                 if (MODE == kModeEvolveMsd) {
-                    ve[u][k] = a.in_e[(size_t)c * B + b];
+                    ve[u][k] = gather<B>(a.in_e, s_in_e, c, row0, b);
                     xn[u][k] = m.x[c];
                 }
             }
@@ -325,7 +394,7 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
                 const double hr = s_hre[k * 32 + r[u]];
                 double hi = 0.0;
                 if (CPLX) hi = s_him[k * 32 + r[u]];
-                const double2 vv = a.in[(size_t)c * B + b];
+                const double2 vv = gather<B>(a.in, s_in, c, row0, b);
                 sr[u] = fma(hr, vv.x, sr[u]);
                 si[u] = fma(hr, vv.y, si[u]);
                 if (CPLX) {
@@ -333,7 +402,7 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
                     si[u] = fma(hi, vv.x, si[u]);
                 }
                 if (MODE == kModeEvolveMsd) {
-                    const double2 vve = a.in_e[(size_t)c * B + b];
+                    const double2 vve = gather<B>(a.in_e, s_in_e, c, row0, b);
                     er[u] = fma(hr, vve.x, er[u]);
                     ei[u] = fma(hr, vve.y, ei[u]);
                     if (CPLX) {
@@ -360,7 +429,7 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
         t.y = scale * si[u];
         t.x -= prev[u].x;
         t.y -= prev[u].y;
-        if (a.store && ok[u]) a.out[vi[u]] = t;
+        if (a.store && ok[u]) st_vec(&a.out[vi[u]], t);
         if (MODE == kModeDoubling) {
             if (ok[u]) {
                 red[0] += t.x * t.x + t.y * t.y;
@@ -383,14 +452,14 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
             }
             acc.x += a.cr * t.x - a.ci * t.y;
             acc.y += a.cr * t.y + a.ci * t.x;
-            if (ok[u]) a.acc[vi[u]] = acc;
+            if (ok[u]) st_vec(&a.acc[vi[u]], acc);
             if (MODE == kModeEvolveMsd) {
                 double2 te;
                 te.x = scale * (er[u] + xr[u]);
                 te.y = scale * (ei[u] + xi[u]);
                 te.x -= prev_e[u].x;
                 te.y -= prev_e[u].y;
-                if (a.store && ok[u]) a.out_e[vi[u]] = te;
+                if (a.store && ok[u]) st_vec(&a.out_e[vi[u]], te);
                 double2 ae;
                 if (a.first) {
                     ae.x = a.c0r * self_e[u].x - a.c0i * self_e[u].y;
@@ -400,7 +469,7 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
                 }
                 ae.x += a.cr * te.x - a.ci * te.y;
                 ae.y += a.cr * te.y + a.ci * te.x;
-                if (ok[u]) a.acc_e[vi[u]] = ae;
+                if (ok[u]) st_vec(&a.acc_e[vi[u]], ae);
             }
         }
     }
@@ -415,9 +484,10 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     constexpr int U = ModeTraits<MODE>::U < B ? ModeTraits<MODE>::U : B;
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int stages = m.stages;
+    const int stages = a.stages;
+    const int stage_bytes = a.stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + warp * kMaxStages;
-    unsigned char* wstage = smem + 128 * ((kWarps * kMaxStages * 8 + 127) / 128) + (size_t)warp * stages * m.stage_bytes;
+    unsigned char* wstage = smem + 128 * ((kWarps * kMaxStages * 8 + 127) / 128) + (size_t)warp * stages * stage_bytes;
 
     double red[Q];
 #pragma unroll
@@ -439,19 +509,21 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         const long long in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
         n_my = (my_runs - 1) * per + in_last;
     }
-    uint64_t policy = 0;
+    uint64_t policy = 0, policy_last = 0;
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(&bars[s], 1);
         fence_mbar_init();
         policy = policy_evict_first();
+        policy_last = policy_evict_last();
     }
+    (void)policy_last;
     __syncwarp();
 
     auto slice_of = [&](long long i) {
         const long long s = (blockIdx.x + (i / per) * G) * a.run + warp + (long long)kWarps * (i % per);
         return a.reverse ? m.n_slices - 1 - s : s;
     };
-    auto issue = [&](long long i) {   // lane 0 only
+    auto issue = [&](long long i) {   // lane 0 only: every HBM stream of slice i -> one stage, one mbarrier
         const long long s = slice_of(i);
         long long off, bytes;
         if (KT > 0) {
@@ -461,9 +533,27 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
             off = m.slice_off[s];
             bytes = m.slice_off[s + 1] - off;
         }
+        const long long rows = (m.N - s * 32) < 32 ? (m.N - s * 32) : 32;
+        const uint32_t vbytes = (uint32_t)(rows * B * sizeof(double2));
+        constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
+        const uint32_t total = (uint32_t)bytes + vbytes * (a.first ? kPair : 2 * kPair);
         const int st = (int)(i % stages);
-        mbar_expect_tx(&bars[st], (uint32_t)bytes);
-        bulk_g2s(wstage + (size_t)st * m.stage_bytes, m.rec + off, (uint32_t)bytes, &bars[st], policy);
+        unsigned char* dst = wstage + (size_t)st * stage_bytes;
+        unsigned char* vdst = dst + a.rec_bytes;
+        const size_t voff = (size_t)s * 32 * B;
+        mbar_expect_tx(&bars[st], total);
+        bulk_g2s(dst, m.rec + off, (uint32_t)bytes, &bars[st], policy);
+#if GPUQT_IN_POLICY == 1
+        bulk_g2s(vdst, a.in + voff, vbytes, &bars[st], policy_last);
+        if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 512 * B, a.in_e + voff, vbytes, &bars[st], policy_last);
+#else
+        bulk_g2s_nohint(vdst, a.in + voff, vbytes, &bars[st]);
+        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, a.in_e + voff, vbytes, &bars[st]);
+#endif
+        if (!a.first) {
+            bulk_g2s(vdst + kPair * 512 * B, a.prev + voff, vbytes, &bars[st], policy);
+            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, a.prev_e + voff, vbytes, &bars[st], policy);
+        }
     };
 
     if (lane == 0) {
@@ -474,7 +564,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         if (lane == 0 && i + stages - 1 < n_my) issue(i + stages - 1);
         const int st = (int)(i % stages);
         mbar_wait(&bars[st], (uint32_t)((i / stages) & 1));
-        const unsigned char* stage = wstage + (size_t)st * m.stage_bytes;
+        const unsigned char* stage = wstage + (size_t)st * stage_bytes;
         const long long slice = slice_of(i);
         int w = KT;
         if (KT == 0) {
