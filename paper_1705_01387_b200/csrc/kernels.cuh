@@ -29,10 +29,10 @@
 #define GPUQT_THREADS 256
 #endif
 #ifndef GPUQT_U_KPM        // sub-steps of a slice processed together (independent gathers in flight)
-#define GPUQT_U_KPM 2
+#define GPUQT_U_KPM 1
 #endif
 #ifndef GPUQT_U_EVOLVE
-#define GPUQT_U_EVOLVE 2
+#define GPUQT_U_EVOLVE 1
 #endif
 #ifndef GPUQT_U_MSD
 #define GPUQT_U_MSD 1
@@ -42,7 +42,7 @@
 #define GPUQT_MINB 2
 #endif
 #ifndef GPUQT_MINB_MSD
-#define GPUQT_MINB_MSD 2
+#define GPUQT_MINB_MSD 1
 #endif
 
 // L2 policy experiments
@@ -51,6 +51,9 @@
 #endif
 #ifndef GPUQT_IN_POLICY       // own rows of T_{m-1} by TMA: 0 no hint, 1 evict_last
 #define GPUQT_IN_POLICY 0
+#endif
+#ifndef GPUQT_PREFETCH_FAR    // 1: L2-prefetch the out-of-slice neighbours of the NEXT staged slice
+#define GPUQT_PREFETCH_FAR 0
 #endif
 #ifndef GPUQT_ST_POLICY       // stores of T_m / acc: 0 plain, 1 st.global.cs (evict-first)
 #define GPUQT_ST_POLICY 0
@@ -138,6 +141,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "r"(parity)
         : "memory");
 }
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n"
+        "}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
@@ -184,24 +203,28 @@ __device__ __forceinline__ double min_image(double d, double box) {
     return d;
 }
 
-// Deterministic reduction of Q*B per-thread values: warp shuffle over lanes with equal b ->
-// shared memory over warps -> per-block partial -> the last block to finish sums the per-block
-// partials in a fixed order (no floating-point atomics, run-to-run identical).
-template <int B, int Q>
-__device__ __forceinline__ void block_reduce_and_finish(double (&v)[Q], double* partials,
+// Deterministic reduction of Q*B values per CTA.  A lane holds v[q * V + j] for vector
+// b = (lane % (B / V)) * V + j.  Warp shuffle over lanes with equal b -> shared memory over warps ->
+// per-block partial -> the last block to finish sums the per-block partials in a fixed order (no
+// floating-point atomics, run-to-run identical).  result[q * B + b].
+template <int B, int Q, int V = 1>
+__device__ __forceinline__ void block_reduce_and_finish(double (&v)[Q * V], double* partials,
                                                         unsigned int* ticket, double* result) {
+    constexpr int LPR = B / V;   // lanes per row
     __shared__ double s_part[kWarps][Q * B];
     __shared__ double s_tree[kThreads];
     __shared__ int s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 #pragma unroll
-    for (int q = 0; q < Q; ++q) {
+    for (int q = 0; q < Q * V; ++q) {
 #pragma unroll
-        for (int off = 16; off >= B; off >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], off);
+        for (int off = 16; off >= LPR; off >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], off);
     }
-    if (lane < B) {
+    if (lane < LPR) {
 #pragma unroll
-        for (int q = 0; q < Q; ++q) s_part[warp][q * B + lane] = v[q];
+        for (int q = 0; q < Q; ++q)
+#pragma unroll
+            for (int j = 0; j < V; ++j) s_part[warp][q * B + lane * V + j] = v[q * V + j];
     }
     __syncthreads();
     if (tid < Q * B) {
@@ -251,30 +274,142 @@ struct StagedStreams {
     static constexpr int value = (MODE == kModeEvolveMsd) ? 4 : 2;
 };
 
-// Gather of T_{m-1}[c]: rows of the current slice come from the staged copy in shared memory.
+// A lane owns V consecutive vectors of a row (V = 2 when B >= 2: one 256-bit access per operand).
 template <int B>
-__device__ __forceinline__ double2 gather(const double2* __restrict__ g, const double2* s_own, int c, int row0, int b) {
-    const unsigned d = (unsigned)(c - row0);
-    if (d < 32u) return s_own[d * B + b];
-#if GPUQT_GATHER_POLICY == 1
-    double2 v;
-    uint64_t pol;
-    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(g + (size_t)c * B + b), "l"(pol));
+struct LaneShape {
+    static constexpr int V = B >= 2 ? 2 : 1;
+    static constexpr int LPR = B / V;        // lanes per row
+    static constexpr int RS = 32 / LPR;      // rows per round
+    static constexpr int ROUNDS = LPR;       // rounds per slice
+};
+
+template <int V>
+struct CV {   // V complex numbers
+    double re[V], im[V];
+};
+template <int V>
+__device__ __forceinline__ CV<V> cv_zero() {
+    CV<V> z;
+#pragma unroll
+    for (int j = 0; j < V; ++j) z.re[j] = z.im[j] = 0.0;
+    return z;
+}
+// shared memory, V consecutive double2
+template <int V>
+__device__ __forceinline__ CV<V> cv_lds(const double2* p) {
+    CV<V> v;
+#pragma unroll
+    for (int j = 0; j < V; ++j) {
+        const double2 t = p[j];
+        v.re[j] = t.x;
+        v.im[j] = t.y;
+    }
     return v;
+}
+// global memory, read once (evict-first)
+template <int V>
+__device__ __forceinline__ CV<V> cv_ld_stream(const double2* p);
+template <>
+__device__ __forceinline__ CV<1> cv_ld_stream<1>(const double2* p) {
+    const double2 t = __ldcs(p);
+    CV<1> v;
+    v.re[0] = t.x;
+    v.im[0] = t.y;
+    return v;
+}
+template <>
+__device__ __forceinline__ CV<2> cv_ld_stream<2>(const double2* p) {
+    CV<2> v;
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];"
+                 : "=d"(v.re[0]), "=d"(v.im[0]), "=d"(v.re[1]), "=d"(v.im[1])
+                 : "l"(p));
+    return v;
+}
+template <int V>
+__device__ __forceinline__ void cv_st(double2* p, const CV<V>& v);
+template <>
+__device__ __forceinline__ void cv_st<1>(double2* p, const CV<1>& v) {
+    st_vec(p, make_double2(v.re[0], v.im[0]));
+}
+template <>
+__device__ __forceinline__ void cv_st<2>(double2* p, const CV<2>& v) {
+#if GPUQT_ST_POLICY == 1
+    asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v.re[0]), "d"(v.im[0]), "d"(v.re[1]), "d"(v.im[1])
+                 : "memory");
 #else
-    return g[(size_t)c * B + b];
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v.re[0]), "d"(v.im[0]), "d"(v.re[1]), "d"(v.im[1])
+                 : "memory");
 #endif
 }
+// Gather of V consecutive vectors of row c of T_{m-1}: rows of the current slice come from the
+// staged copy in shared memory (s_own = shared-window address of the slice's row 0), the others
+// from global memory with an L2 evict_last hint (they are re-read by the neighbouring slices).
+// Both loads are predicated, so there is no branch.
+template <int V>
+__device__ __forceinline__ CV<V> cv_gather(const double2* g, uint32_t s_own, int c, int row0, int B, int l);
+template <>
+__device__ __forceinline__ CV<1> cv_gather<1>(const double2* g, uint32_t s_own, int c, int row0, int B, int l) {
+    const unsigned d = (unsigned)(c - row0);
+    const uint32_t sa = s_own + (d * B + l) * 16u;
+    const double2* ga = g + (size_t)c * B + l;
+    CV<1> v;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.lt.u32 p, %4, 32;\n"
+        "@p ld.shared.v2.f64 {%0, %1}, [%2];\n"
+        "@!p ld.global.v2.f64 {%0, %1}, [%3];\n"
+        "}"
+        : "=d"(v.re[0]), "=d"(v.im[0])
+        : "r"(sa), "l"(ga), "r"(d));
+    return v;
+}
+template <>
+__device__ __forceinline__ CV<2> cv_gather<2>(const double2* g, uint32_t s_own, int c, int row0, int B, int l) {
+    const unsigned d = (unsigned)(c - row0);
+    const uint32_t sa = s_own + (d * B + l * 2) * 16u;
+    const double2* ga = g + (size_t)c * B + l * 2;
+    CV<2> v;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.lt.u32 p, %6, 32;\n"
+        "@p ld.shared.v2.f64 {%0, %1}, [%4];\n"
+        "@p ld.shared.v2.f64 {%2, %3}, [%4+16];\n"
+#if GPUQT_GATHER_POLICY == 1
+        "@!p ld.global.L2::evict_last.v4.f64 {%0, %1, %2, %3}, [%5];\n"
+#else
+        "@!p ld.global.v4.f64 {%0, %1, %2, %3}, [%5];\n"
+#endif
+        "}"
+        : "=d"(v.re[0]), "=d"(v.im[0]), "=d"(v.re[1]), "=d"(v.im[1])
+        : "r"(sa), "l"(ga), "r"(d));
+    return v;
+}
 
-// U sub-steps (U * 32/B rows) of one slice whose record and own rows sit in shared memory at `stage`.
+// acc += h * v for V vectors; h = (hr, hi)
+template <int V, bool CPLX>
+__device__ __forceinline__ void cv_fma(CV<V>& acc, double hr, double hi, const CV<V>& v) {
+#pragma unroll
+    for (int j = 0; j < V; ++j) {
+        acc.re[j] = fma(hr, v.re[j], acc.re[j]);
+        acc.im[j] = fma(hr, v.im[j], acc.im[j]);
+        if (CPLX) {
+            acc.re[j] = fma(-hi, v.im[j], acc.re[j]);
+            acc.im[j] = fma(hi, v.re[j], acc.im[j]);
+        }
+    }
+}
+
+// U rounds (U * RS rows) of one slice whose record and own rows sit in shared memory at `stage`.
 template <int B, int KT, bool CPLX, int MODE, int U>
 __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
                                           long long slice, int j0, int lane, double scale,
-                                          double (&red)[ModeTraits<MODE>::Q]) {
-    constexpr int RS = 32 / B;
+                                          double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V]) {
+    constexpr int V = LaneShape<B>::V, LPR = LaneShape<B>::LPR, RS = LaneShape<B>::RS;
     constexpr int KU = KT > 0 ? KT : 1;
-    const int rl = lane / B, b = lane % B;
+    constexpr bool MSD = (MODE == kModeEvolveMsd);
+    const int rl = lane / LPR, l = lane % LPR;
     const double* s_hre = reinterpret_cast<const double*>(stage);
     const double* s_him = s_hre + (size_t)w * 32;
     const double* s_on = s_hre + (size_t)w * 32 * (CPLX ? 2 : 1);
@@ -282,54 +417,53 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
     // staged vector rows: [in | (in_e) | prev | (prev_e)], each 32 * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
     const double2* s_in_e = s_in + 32 * B;
-    const double2* s_prev = s_in + (MODE == kModeEvolveMsd ? 2 : 1) * 32 * B;
+    const double2* s_prev = s_in + (MSD ? 2 : 1) * 32 * B;
     const double2* s_prev_e = s_prev + 32 * B;
+    const uint32_t sa_in = smem_u32(s_in), sa_in_e = smem_u32(s_in_e);
     const int row0 = (int)(slice * 32);
 
     int r[U];
     bool ok[U];
     size_t vi[U];
-    double2 self[U], self_e[U], prev[U], prev_e[U], other[U], other_e[U];
-    double sr[U], si[U], er[U], ei[U], xr[U], xi[U], xm[U];
+    CV<V> other[U], other_e[U];
+    double xm[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         r[u] = (j0 + u) * RS + rl;
         long long row = slice * 32 + r[u];
         ok[u] = row < m.N;
         if (!ok[u]) row = m.N - 1;
-        vi[u] = (size_t)row * B + b;
+        vi[u] = (size_t)row * B + l * V;
         // streamed read-modify-write operands: issued first, consumed last
-        other[u] = other_e[u] = make_double2(0.0, 0.0);
+        other[u] = other_e[u] = cv_zero<V>();
         if (!a.first) {
-            if (MODE == kModeEvolve || MODE == kModeEvolveMsd) other[u] = ldcs2(&a.acc[vi[u]]);
-            if (MODE == kModeEvolveMsd) other_e[u] = ldcs2(&a.acc_e[vi[u]]);
+            if (MODE == kModeEvolve || MSD) other[u] = cv_ld_stream<V>(&a.acc[vi[u]]);
+            if (MSD) other_e[u] = cv_ld_stream<V>(&a.acc_e[vi[u]]);
         }
-        if (MODE == kModeLeft) other[u] = ldcs2(&a.phiL[vi[u]]);
-        if (MODE == kModeEvolveMsd) xm[u] = m.x[row];
+        if (MODE == kModeLeft) other[u] = cv_ld_stream<V>(&a.phiL[vi[u]]);
+        if (MSD) xm[u] = m.x[row];
     }
+
+    CV<V> sum[U], sum_e[U], sum_x[U];   // H T_{m-1}, H e_{m-1}, [X,H] T_{m-1}  (unscaled)
+    CV<V> self[U], self_e[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-        const int si_ = r[u] * B + b;
-        self[u] = ok[u] ? s_in[si_] : make_double2(0.0, 0.0);
-        self_e[u] = prev[u] = prev_e[u] = make_double2(0.0, 0.0);
-        if (MODE == kModeEvolveMsd) self_e[u] = ok[u] ? s_in_e[si_] : make_double2(0.0, 0.0);
-        if (!a.first) {
-            if (ok[u]) prev[u] = s_prev[si_];
-            if (MODE == kModeEvolveMsd && ok[u]) prev_e[u] = s_prev_e[si_];
-        }
+        const int si_ = r[u] * B + l * V;
+        self[u] = ok[u] ? cv_lds<V>(s_in + si_) : cv_zero<V>();
+        self_e[u] = (MSD && ok[u]) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
     }
     if (KT > 0) {
         // all gathers of the U rows first (independent loads in flight), then the arithmetic
-        double2 v[U][KU], ve[U][KU];
-        double xn[U][KU];
+        CV<V> v[U][KU], ve[U][MSD ? KU : 1];
+        double xn[U][MSD ? KU : 1];
 #pragma unroll
         for (int k = 0; k < KU; ++k) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int c = s_col[k * 32 + r[u]];
-                v[u][k] = gather<B>(a.in, s_in, c, row0, b);
-                if (MODE == kModeEvolveMsd) {
-                    ve[u][k] = gather<B>(a.in_e, s_in_e, c, row0, b);
+                v[u][k] = cv_gather<V>(a.in, sa_in, c, row0, B, l);
+                if (MSD) {
+                    ve[u][k] = cv_gather<V>(a.in_e, sa_in_e, c, row0, B, l);
                     xn[u][k] = m.x[c];
                 }
             }
@@ -337,41 +471,20 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const double on = s_on[r[u]];
-            sr[u] = on * self[u].x;
-            si[u] = on * self[u].y;
-            er[u] = ei[u] = xr[u] = xi[u] = 0.0;
-            if (MODE == kModeEvolveMsd) {
-                er[u] = on * self_e[u].x;
-                ei[u] = on * self_e[u].y;
-            }
+            sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
+            cv_fma<V, false>(sum[u], on, 0.0, self[u]);
+            if (MSD) cv_fma<V, false>(sum_e[u], on, 0.0, self_e[u]);
 #pragma unroll
             for (int k = 0; k < KU; ++k) {
                 const double hr = s_hre[k * 32 + r[u]];
                 double hi = 0.0;
                 if (CPLX) hi = s_him[k * 32 + r[u]];
-                sr[u] = fma(hr, v[u][k].x, sr[u]);
-                si[u] = fma(hr, v[u][k].y, si[u]);
-                if (CPLX) {
-                    sr[u] = fma(-hi, v[u][k].y, sr[u]);
-                    si[u] = fma(hi, v[u][k].x, si[u]);
-                }
-                if (MODE == kModeEvolveMsd) {
-                    er[u] = fma(hr, ve[u][k].x, er[u]);
-                    ei[u] = fma(hr, ve[u][k].y, ei[u]);
-                    if (CPLX) {
-                        er[u] = fma(-hi, ve[u][k].y, er[u]);
-                        ei[u] = fma(hi, ve[u][k].x, ei[u]);
-                    }
+                cv_fma<V, CPLX>(sum[u], hr, hi, v[u][k]);
+                if (MSD) {
+                    cv_fma<V, CPLX>(sum_e[u], hr, hi, ve[u][k]);
                     // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
                     const double ndx = -min_image(xn[u][k] - xm[u], m.box);
-                    const double wr = ndx * hr;
-                    xr[u] = fma(wr, v[u][k].x, xr[u]);
-                    xi[u] = fma(wr, v[u][k].y, xi[u]);
-                    if (CPLX) {
-                        const double wi = ndx * hi;
-                        xr[u] = fma(-wi, v[u][k].y, xr[u]);
-                        xi[u] = fma(wi, v[u][k].x, xi[u]);
-                    }
+                    cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, v[u][k]);
                 }
             }
         }
@@ -379,13 +492,9 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const double on = s_on[r[u]];
-            sr[u] = on * self[u].x;
-            si[u] = on * self[u].y;
-            er[u] = ei[u] = xr[u] = xi[u] = 0.0;
-            if (MODE == kModeEvolveMsd) {
-                er[u] = on * self_e[u].x;
-                ei[u] = on * self_e[u].y;
-            }
+            sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
+            cv_fma<V, false>(sum[u], on, 0.0, self[u]);
+            if (MSD) cv_fma<V, false>(sum_e[u], on, 0.0, self_e[u]);
         }
         for (int k = 0; k < w; ++k) {
 #pragma unroll
@@ -394,82 +503,72 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
                 const double hr = s_hre[k * 32 + r[u]];
                 double hi = 0.0;
                 if (CPLX) hi = s_him[k * 32 + r[u]];
-                const double2 vv = gather<B>(a.in, s_in, c, row0, b);
-                sr[u] = fma(hr, vv.x, sr[u]);
-                si[u] = fma(hr, vv.y, si[u]);
-                if (CPLX) {
-                    sr[u] = fma(-hi, vv.y, sr[u]);
-                    si[u] = fma(hi, vv.x, si[u]);
-                }
-                if (MODE == kModeEvolveMsd) {
-                    const double2 vve = gather<B>(a.in_e, s_in_e, c, row0, b);
-                    er[u] = fma(hr, vve.x, er[u]);
-                    ei[u] = fma(hr, vve.y, ei[u]);
-                    if (CPLX) {
-                        er[u] = fma(-hi, vve.y, er[u]);
-                        ei[u] = fma(hi, vve.x, ei[u]);
-                    }
+                const CV<V> vv = cv_gather<V>(a.in, sa_in, c, row0, B, l);
+                cv_fma<V, CPLX>(sum[u], hr, hi, vv);
+                if (MSD) {
+                    const CV<V> vve = cv_gather<V>(a.in_e, sa_in_e, c, row0, B, l);
+                    cv_fma<V, CPLX>(sum_e[u], hr, hi, vve);
                     const double ndx = -min_image(m.x[c] - xm[u], m.box);
-                    const double wr = ndx * hr;
-                    xr[u] = fma(wr, vv.x, xr[u]);
-                    xi[u] = fma(wr, vv.y, xi[u]);
-                    if (CPLX) {
-                        const double wi = ndx * hi;
-                        xr[u] = fma(-wi, vv.y, xr[u]);
-                        xi[u] = fma(wi, vv.x, xi[u]);
-                    }
+                    cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, vv);
                 }
             }
         }
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-        double2 t;   // T_m
-        t.x = scale * sr[u];
-        t.y = scale * si[u];
-        t.x -= prev[u].x;
-        t.y -= prev[u].y;
-        if (a.store && ok[u]) st_vec(&a.out[vi[u]], t);
-        if (MODE == kModeDoubling) {
-            if (ok[u]) {
-                red[0] += t.x * t.x + t.y * t.y;
-                red[1] += t.x * self[u].x + t.y * self[u].y;
-                red[2] += self[u].x * self[u].x + self[u].y * self[u].y;
-            }
-        } else if (MODE == kModeLeft) {
-            const double2 l = other[u];
-            if (ok[u]) {
-                red[0] += l.x * t.x + l.y * t.y;       // conj(l) * t
-                red[1] += l.x * t.y - l.y * t.x;
-            }
-        } else {
-            double2 acc;
-            if (a.first) {
-                acc.x = a.c0r * self[u].x - a.c0i * self[u].y;
-                acc.y = a.c0r * self[u].y + a.c0i * self[u].x;
-            } else {
-                acc = other[u];
-            }
-            acc.x += a.cr * t.x - a.ci * t.y;
-            acc.y += a.cr * t.y + a.ci * t.x;
-            if (ok[u]) st_vec(&a.acc[vi[u]], acc);
-            if (MODE == kModeEvolveMsd) {
-                double2 te;
-                te.x = scale * (er[u] + xr[u]);
-                te.y = scale * (ei[u] + xi[u]);
-                te.x -= prev_e[u].x;
-                te.y -= prev_e[u].y;
-                if (a.store && ok[u]) st_vec(&a.out_e[vi[u]], te);
-                double2 ae;
-                if (a.first) {
-                    ae.x = a.c0r * self_e[u].x - a.c0i * self_e[u].y;
-                    ae.y = a.c0r * self_e[u].y + a.c0i * self_e[u].x;
-                } else {
-                    ae = other_e[u];
+        const int si_ = r[u] * B + l * V;
+        CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
+        if (!a.first && ok[u]) {
+            prev = cv_lds<V>(s_prev + si_);
+            if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
+        }
+        CV<V> t, te, acc, ae;   // T_m, e_m, and the accumulators
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+            t.re[j] = scale * sum[u].re[j] - prev.re[j];
+            t.im[j] = scale * sum[u].im[j] - prev.im[j];
+            if (MODE == kModeDoubling) {
+                if (ok[u]) {
+                    red[0 * V + j] += t.re[j] * t.re[j] + t.im[j] * t.im[j];
+                    red[1 * V + j] += t.re[j] * self[u].re[j] + t.im[j] * self[u].im[j];
+                    red[2 * V + j] += self[u].re[j] * self[u].re[j] + self[u].im[j] * self[u].im[j];
                 }
-                ae.x += a.cr * te.x - a.ci * te.y;
-                ae.y += a.cr * te.y + a.ci * te.x;
-                if (ok[u]) st_vec(&a.acc_e[vi[u]], ae);
+            } else if (MODE == kModeLeft) {
+                if (ok[u]) {   // conj(l) * t
+                    red[0 * V + j] += other[u].re[j] * t.re[j] + other[u].im[j] * t.im[j];
+                    red[1 * V + j] += other[u].re[j] * t.im[j] - other[u].im[j] * t.re[j];
+                }
+            } else {
+                if (a.first) {
+                    acc.re[j] = a.c0r * self[u].re[j] - a.c0i * self[u].im[j];
+                    acc.im[j] = a.c0r * self[u].im[j] + a.c0i * self[u].re[j];
+                } else {
+                    acc.re[j] = other[u].re[j];
+                    acc.im[j] = other[u].im[j];
+                }
+                acc.re[j] += a.cr * t.re[j] - a.ci * t.im[j];
+                acc.im[j] += a.cr * t.im[j] + a.ci * t.re[j];
+                if (MSD) {
+                    te.re[j] = scale * (sum_e[u].re[j] + sum_x[u].re[j]) - prev_e.re[j];
+                    te.im[j] = scale * (sum_e[u].im[j] + sum_x[u].im[j]) - prev_e.im[j];
+                    if (a.first) {
+                        ae.re[j] = a.c0r * self_e[u].re[j] - a.c0i * self_e[u].im[j];
+                        ae.im[j] = a.c0r * self_e[u].im[j] + a.c0i * self_e[u].re[j];
+                    } else {
+                        ae.re[j] = other_e[u].re[j];
+                        ae.im[j] = other_e[u].im[j];
+                    }
+                    ae.re[j] += a.cr * te.re[j] - a.ci * te.im[j];
+                    ae.im[j] += a.cr * te.im[j] + a.ci * te.re[j];
+                }
+            }
+        }
+        if (ok[u]) {
+            if (a.store) cv_st<V>(&a.out[vi[u]], t);
+            if (MODE == kModeEvolve || MSD) cv_st<V>(&a.acc[vi[u]], acc);
+            if (MSD) {
+                if (a.store) cv_st<V>(&a.out_e[vi[u]], te);
+                cv_st<V>(&a.acc_e[vi[u]], ae);
             }
         }
     }
@@ -481,7 +580,8 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
 template <int B, int KT, bool CPLX, int MODE>
 __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
     constexpr int Q = ModeTraits<MODE>::Q;
-    constexpr int U = ModeTraits<MODE>::U < B ? ModeTraits<MODE>::U : B;
+    constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
+    constexpr int U = ModeTraits<MODE>::U < ROUNDS ? ModeTraits<MODE>::U : ROUNDS;
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int stages = a.stages;
@@ -489,9 +589,9 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + warp * kMaxStages;
     unsigned char* wstage = smem + 128 * ((kWarps * kMaxStages * 8 + 127) / 128) + (size_t)warp * stages * stage_bytes;
 
-    double red[Q];
+    double red[Q * V];
 #pragma unroll
-    for (int q = 0; q < Q; ++q) red[q] = 0.0;
+    for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
     const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
 
     // Work split: the slices are cut into runs of a.run consecutive slices; CTA c walks runs
@@ -572,12 +672,35 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
             w = (int)((bytes / 32 - 8) / (CPLX ? 20 : 12));
         }
 #pragma unroll 1
-        for (int j0 = 0; j0 < B; j0 += U)
+        for (int j0 = 0; j0 < ROUNDS; j0 += U) {
             walk_rows<B, KT, CPLX, MODE, U>(m, a, stage, w, slice, j0, lane, scale, red);
+#if GPUQT_PREFETCH_FAR
+            // Once per slice: if the next slice's record has landed, pull its out-of-slice
+            // neighbours (the rows no TMA stream brings in) towards L2 a whole slice ahead.
+            if (j0 == 0 && i + 1 < n_my) {
+                const int st1 = (int)((i + 1) % stages);
+                if (mbar_test(&bars[st1], (uint32_t)(((i + 1) / stages) & 1))) {
+                    const long long s1 = slice_of(i + 1);
+                    int w1 = KT;
+                    if (KT == 0) w1 = (int)(((m.slice_off[s1 + 1] - m.slice_off[s1]) / 32 - 8) / (CPLX ? 20 : 12));
+                    const unsigned char* nxt = wstage + (size_t)st1 * stage_bytes;
+                    const int* col1 = reinterpret_cast<const int*>(nxt + (size_t)w1 * 256 * (CPLX ? 2 : 1) + 256);
+                    const int row1 = (int)(s1 * 32);
+                    for (int k = 0; k < w1; ++k) {
+                        const int c = col1[k * 32 + lane];
+                        if ((unsigned)(c - row1) >= 32u) {
+                            prefetch_l2(a.in + (size_t)c * B);
+                            if (MODE == kModeEvolveMsd) prefetch_l2(a.in_e + (size_t)c * B);
+                        }
+                    }
+                }
+            }
+#endif
+        }
         __syncwarp();
     }
     if (MODE == kModeDoubling || MODE == kModeLeft)
-        block_reduce_and_finish<B, Q>(red, a.partials, a.ticket, a.result);
+        block_reduce_and_finish<B, Q, V>(red, a.partials, a.ticket, a.result);
 }
 
 // Address of entry (row, k) pieces inside the packed records (plain global reads; used by the
