@@ -160,9 +160,8 @@ def run_ours(args, w):
     import paper_1705_01387_b200 as gq
     from paper_1705_01387_b200 import binding
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1705_01387_b200 import replicas
+    rank, local, world = replicas.world()
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
@@ -174,7 +173,7 @@ def run_ours(args, w):
     with torch.cuda.stream(stream):
         g = gq.GpuQT(model, batch=w.batch, modes=modes, stream=stream)
         # replicas over random vectors: rank r owns vectors [r*B, (r+1)*B)
-        phi_host = torch.from_numpy(w.phases(model, first_vector=rank * w.batch)).pin_memory()
+        phi_host = torch.from_numpy(w.phases(model, first_vector=replicas.first_vector(rank, w.batch))).pin_memory()
         phi_dev = phi_host.to("cuda", non_blocking=True)
         mom_host = torch.empty((w.batch, w.n_moments), dtype=torch.float64).pin_memory()
         energies = energies_for(model)
@@ -209,11 +208,7 @@ def run_ours(args, w):
             ev1.record(stream)
             barrier()
             ms = ev0.elapsed_time(ev1)
-            if world > 1:
-                t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ms = float(t.item())
-            return ms, out
+            return replicas.max_over_ranks(ms, device="cuda"), out
 
         sampler = ClockSampler(local)
         sampler.start()
