@@ -200,3 +200,46 @@ def test_empty_rows_and_tiny_sizes(gq, oracle_mod):
         assert vec_err(g.get_state(gq.STATE_CHI), o.get_state(oracle_mod.CHI)) <= TOL
         assert np.max(np.abs(g.dos_moments(10) - o.dos_moments(10))) / model.N <= TOL
         g.close()
+
+
+@pytest.mark.parametrize("key", ["c1", "c2", "c3", "c4", "c5"])
+def test_config_families_small(gq, oracle_mod, key):
+    """The five BASELINE.json families at sizes the oracle finishes in seconds, with each config's
+    own batch, path, dt and N_p: every time step's moments (all N_m' = 96) and final vectors."""
+    from paper_1705_01387_b200 import binding
+    from workloads import configs
+    w = configs.WORKLOADS[key]
+    model = configs.small_variant(key)
+    order = w.order or binding.choose_order(model.energy_scale, w.dt)
+    nm, steps, B = 96, 3, w.batch
+    phi = w.phases(model)
+    mg = gq.MODE_MSD if w.path == "msd" else gq.MODE_VAC
+    mo = oracle_mod.MODE_MSD if w.path == "msd" else oracle_mod.MODE_VAC
+    g, o = gq.GpuQT(model, batch=B, modes=mg), oracle_mod.Oracle(model, batch=B, modes=mo)
+    for a, b in zip(g.get_table(), o.get_table()):
+        assert a.tobytes() == b.tobytes()
+    g.set_state(phi)
+    o.set_state(phi)
+    assert np.max(np.abs(g.dos_moments(nm) - o.dos_moments(nm))) / model.N <= TOL
+    for _ in range(steps):
+        if w.path == "vac":
+            va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+            scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(B)])
+            assert np.max(np.abs(g.vac(nm) - o.vac(nm)) / scale[:, None]) <= TOL
+            g.evolve(w.dt, order)
+            o.evolve(w.dt, order)
+        else:
+            g.evolve(w.dt, order)
+            o.evolve(w.dt, order)
+            chi = o.get_state(oracle_mod.CHI)
+            assert np.max(np.abs(g.msd(nm) - o.msd(nm)) / (norms(chi) ** 2)[:, None]) <= TOL
+    pairs = (((gq.STATE_PSI, oracle_mod.PSI), (gq.STATE_CHI, oracle_mod.CHI)) if w.path == "msd" else
+             ((gq.STATE_VAC_A, oracle_mod.VAC_A), (gq.STATE_VAC_B, oracle_mod.VAC_B)))
+    for sg, so in pairs:
+        assert vec_err(g.get_state(sg), o.get_state(so)) <= TOL
+    # energy transform of this run's moments on the paper's 601-point grid (a8)
+    C = o.dos_moments(nm)
+    E = np.linspace(-0.98 * model.energy_scale, 0.98 * model.energy_scale, 601)
+    ref = o.kpm_transform(C, E)
+    assert np.max(np.abs(g.kpm_transform(C, E) - ref)) / np.max(np.abs(ref)) <= TOL
+    g.close()
