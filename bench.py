@@ -234,6 +234,11 @@ def run_ours(args, w):
             per_row_launch = (model.K * (4 + (16 if cplx else 8)) + 8 + 8) + w.batch * 2 * 80
         else:
             per_row_launch = bpo * w.batch
+        # bytes the stored layout really holds per row (constant-hopping records carry no hop array)
+        hop_const = model.hop_im is None and (model.hop_re is None or np.unique(
+            model.hop_re.reshape(model.N, model.K)[np.arange(model.K)[None, :] < model.nbr_count[:, None]]).size <= 1)
+        hop_const = hop_const and os.environ.get("GPUQT_HOP_CONST", "1") != "0"
+        stored_row_launch = per_row_launch - (8 * model.K if hop_const else 0)
         dom_ms, dom_n = stats[dom]
         achieved = per_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9
         peak, peak_src = load_peak()
@@ -266,6 +271,8 @@ def run_ours(args, w):
                              "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                              "frac_of_nominal_8000": achieved / 8000.0,
                              "bytes_per_launch": per_row_launch * model.N,
+                             "stored_bytes_per_launch": stored_row_launch * model.N,
+                             "stored_gbs": stored_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9,
                              "avg_launch_us": dom_ms * 1e3 / max(dom_n, 1), "launches": dom_n,
                              "share_of_step": dom_ms / ms,
                              "per_class_ms": {names[c]: stats[c][0] for c in names}},

@@ -28,7 +28,7 @@ struct PendingStat {
 struct gpuqt_handle {
     int64_t N = 0;
     int32_t K = 0, B = 0;
-    int modes = 0, cplx = 0, kt = 0;
+    int modes = 0, cplx = 0, kt = 0, hop = 0;
     int max_blocks_per_sm = 0;          // GPUQT_BLOCKS_PER_SM (tuning override), 0 = occupancy limit
     int run = kWarps;                   // GPUQT_RUN: consecutive slices per CTA run (multiple of kWarps)
     int alternate = 1;                  // GPUQT_ALTERNATE: sweep direction alternates between launches
@@ -125,13 +125,14 @@ bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
 
 // ---------------------------------------------------------------- kernel dispatch
 template <int MODE, int BB, int KK>
-void* step_fn(bool cplx) {
-    return cplx ? (void*)cheb_step_kernel<BB, KK, true, MODE> : (void*)cheb_step_kernel<BB, KK, false, MODE>;
+void* step_fn(int hop) {
+    return hop == kHopComplex ? (void*)cheb_step_kernel<BB, KK, kHopComplex, MODE>
+           : hop == kHopConst ? (void*)cheb_step_kernel<BB, KK, kHopConst, MODE>
+                              : (void*)cheb_step_kernel<BB, KK, kHopReal, MODE>;
 }
 template <int MODE, int BB>
-void* step_fn_k(int kt, bool cplx) {
+void* step_fn_k(int kt, int cplx) {
     switch (kt) {
-    case 2: return step_fn<MODE, BB, 2>(cplx);
     case 3: return step_fn<MODE, BB, 3>(cplx);
     case 4: return step_fn<MODE, BB, 4>(cplx);
     case 6: return step_fn<MODE, BB, 6>(cplx);
@@ -139,7 +140,7 @@ void* step_fn_k(int kt, bool cplx) {
     }
 }
 template <int MODE>
-void* step_fn_b(int B, int kt, bool cplx) {
+void* step_fn_b(int B, int kt, int cplx) {
     switch (B) {
     case 1: return step_fn_k<MODE, 1>(kt, cplx);
     case 2: return step_fn_k<MODE, 2>(kt, cplx);
@@ -149,10 +150,10 @@ void* step_fn_b(int B, int kt, bool cplx) {
 }
 void* step_kernel(const gpuqt_handle* h, int mode) {
     switch (mode) {
-    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->cplx);
-    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->cplx);
-    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->cplx);
-    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->cplx);
+    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->hop);
+    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->hop);
+    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->hop);
+    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->hop);
     }
 }
 
@@ -414,7 +415,7 @@ extern "C" {
 size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes) {
     if (N <= 0 || K_max <= 0 || !batch_ok(batch)) return 0;
     // upper bound: every slice record padded to K_max
-    const size_t rec = (size_t)((N + 31) / 32) * (size_t)record_bytes(K_max, is_complex ? 1 : 0);
+    const size_t rec = (size_t)((N + 31) / 32) * (size_t)record_bytes(K_max, is_complex ? 2 : 1);
     return make_layout(N, batch, modes, rec).total;
 }
 
@@ -459,7 +460,10 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->stream = (cudaStream_t)cuda_stream;
     h->vec_elems = (size_t)N * batch;
 
-    const int stage_bytes = (int)record_bytes(K_max, h->cplx);
+    SellHost sell;
+    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, env_int("GPUQT_HOP_CONST", 1) != 0, sell);
+    h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : kHopConst;
+    const int stage_bytes = (int)record_bytes(K_max, sell.nd);
     h->rec_bytes = stage_bytes;
     if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd)) > kSmemBudget) {
         fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "
@@ -467,8 +471,6 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
         delete h;
         return GPUQT_ERR_ARG;
     }
-    SellHost sell;
-    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, sell);
     const size_t rec_bytes = sell.rec.size();
     const Layout L = make_layout(N, batch, modes, rec_bytes);
     if (L.total > workspace_bytes) {
@@ -502,9 +504,9 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     }
     h->mat.rec = d_rec; h->mat.slice_off = d_sp; h->mat.x = d_x;
     h->mat.N = N; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
-    h->mat.cplx = h->cplx;
+    h->mat.cplx = h->cplx; h->mat.hop = h->hop; h->mat.hop_const = sell.hop_const;
     h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
-    h->kt = (sell.uniform && (K_max == 2 || K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
+    h->kt = (sell.uniform && (K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
     // Shared-memory stages per warp: one sub-step of a slice takes about one memory latency and a
     // slice has `batch` sub-steps, so small batches need a deeper prefetch.  Tuning overrides:
     // GPUQT_STAGES, GPUQT_BLOCKS_PER_SM, GPUQT_ALTERNATE.

@@ -91,22 +91,52 @@ inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32
 }
 
 // Packed sliced-ELL table on the host (layout: kernels.cuh).  A slice is 32 rows; its record is
-//   double hre[w][32] | double him[w][32] (complex) | double onsite[32] | int32 col[w][32]
-// with w the largest neighbour count in the slice.  If padding every record to K_max costs less
+//   double hre[w][32] (nd >= 1) | double him[w][32] (nd == 2) | double onsite[32] | int32 col[w][32]
+// with w the largest neighbour count in the slice and nd the doubles stored per entry: 2 complex,
+// 1 real, 0 when every listed hopping is the same real number (hop_const; the paper's default
+// "all hoppings -1", and every clean-lattice model) -- then padding is col = -1.  If padding every record to K_max costs less
 // than 1/16 extra bytes the table is stored uniform (w = K_max everywhere), which lets the
 // kernels compute record offsets arithmetically and unroll the neighbour walk.
 struct SellHost {
     int64_t n_slices = 0;
     int uniform = 1;                    // every record has width K_max
+    int nd = 1;                         // doubles per entry: 0 constant hopping, 1 real, 2 complex
+    double hop_const = 0.0;
     std::vector<long long> slice_off;   // [n_slices + 1] byte offsets of the records
     std::vector<unsigned char> rec;
 };
 
-inline long long host_record_bytes(int w, int cplx) { return 32LL * (8LL * w * (1 + cplx) + 8 + 4LL * w); }
+inline long long host_record_bytes(int w, int nd) { return 32LL * (8LL * w * nd + 8 + 4LL * w); }
+
+// true (and the value) if hop_im is absent and all listed hoppings carry the same bit pattern
+inline bool constant_hopping(int64_t N, int32_t K, const int32_t* cnt, const double* hre, const double* him,
+                             double& value) {
+    if (him) return false;
+    if (!hre) {
+        value = -1.0;
+        return true;
+    }
+    bool have = false;
+    for (int64_t m = 0; m < N; ++m)
+        for (int32_t k = 0; k < cnt[m]; ++k) {
+            const double h = hre[(size_t)m * K + k];
+            if (!have) {
+                value = h;
+                have = true;
+            } else if (std::memcmp(&h, &value, sizeof(double)) != 0) {
+                return false;
+            }
+        }
+    if (!have) value = 0.0;
+    return true;
+}
 
 inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
-                       const double* hre, const double* him, const double* onsite, SellHost& s) {
-    const int cplx = him ? 1 : 0;
+                       const double* hre, const double* him, const double* onsite, bool allow_const,
+                       SellHost& s) {
+    s.nd = him ? 2 : 1;
+    if (allow_const && constant_hopping(N, K, cnt, hre, him, s.hop_const)) s.nd = 0;
+    const int cplx = s.nd;   // doubles per entry
     s.n_slices = (N + 31) / 32;
     std::vector<int> width((size_t)s.n_slices, 0);
     long long ragged = 0;
@@ -129,7 +159,7 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
         unsigned char* base = s.rec.data() + s.slice_off[(size_t)sl];
         double* r_hre = reinterpret_cast<double*>(base);
         double* r_him = r_hre + (size_t)w * 32;
-        double* r_on = r_hre + (size_t)w * 32 * (1 + cplx);
+        double* r_on = r_hre + (size_t)w * 32 * s.nd;
         int32_t* r_col = reinterpret_cast<int32_t*>(r_on + 32);
         for (int lane = 0; lane < 32; ++lane) {
             const int64_t m = sl * 32 + lane;
@@ -138,8 +168,10 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
                 const size_t e = (size_t)k * 32 + lane;
                 if (m < N && k < cnt[m]) {
                     r_col[e] = idx[(size_t)m * K + k];
-                    r_hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
-                    if (cplx) r_him[e] = him[(size_t)m * K + k];
+                    if (s.nd >= 1) r_hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
+                    if (s.nd == 2) r_him[e] = him[(size_t)m * K + k];
+                } else if (s.nd == 0) {
+                    r_col[e] = -1;                                             // padding: no entry
                 } else {
                     r_col[e] = (int32_t)(m < N ? m : N - 1);                   // padding: own row, hop 0
                 }

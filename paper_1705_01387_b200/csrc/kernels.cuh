@@ -6,11 +6,13 @@
 //             so one neighbour index serves one 16*B-byte gather (B = 8: one 128-byte line).
 //   matrix    packed sliced ELL.  A slice is 32 consecutive rows; slice s of width w is ONE
 //             contiguous record, column-major inside the record:
-//                 double hre[w][32] | double him[w][32] (complex variant only) |
+//                 double hre[w][32] (per-entry variants) | double him[w][32] (complex variant) |
 //                 double onsite[32] | int32 col[w][32]
-//             record bytes = 32 * (8 w (1 + cplx) + 8 + 4 w), a multiple of 128.  Records are
-//             stored back to back; slice_off[s] is the byte offset of record s.  Padding entries
-//             are (a valid row, hop 0.0).  One record = one 1-D TMA bulk copy.
+//             record bytes = 32 * (8 w nd + 8 + 4 w), nd = doubles per entry (0, 1, 2), a multiple
+//             of 128.  Records are stored back to back; slice_off[s] is the byte offset of record
+//             s.  Padding entries are (own row, hop 0.0); in the constant-hopping variant (nd = 0:
+//             every stored hopping is the same real number, kept in Mat::hop_const) padding is
+//             col = -1.  One record = one 1-D TMA bulk copy.
 //   warp      the unit of work is (warp, slice).  A stage of a warp's shared-memory pipeline holds
 //             everything the slice streams from HBM exactly once: the packed record, the slice's
 //             own rows of T_{m-1} (and e_{m-1}) and of T_{m-2} (and e_{m-2}) -- each one 1-D TMA
@@ -52,9 +54,6 @@
 #ifndef GPUQT_IN_POLICY       // own rows of T_{m-1} by TMA: 0 no hint, 1 evict_last
 #define GPUQT_IN_POLICY 0
 #endif
-#ifndef GPUQT_PREFETCH_FAR    // 1: L2-prefetch the out-of-slice neighbours of the NEXT staged slice
-#define GPUQT_PREFETCH_FAR 0
-#endif
 #ifndef GPUQT_ST_POLICY       // stores of T_m / acc: 0 plain, 1 st.global.cs (evict-first)
 #define GPUQT_ST_POLICY 0
 #endif
@@ -66,9 +65,15 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kSlice = 32;
 constexpr int kMaxStages = 4;
 
-__host__ __device__ __forceinline__ long long record_bytes(int w, int cplx) {
-    return 32LL * (8LL * w * (1 + cplx) + 8 + 4LL * w);
+// nd = doubles stored per entry: 0 constant real hopping, 1 real, 2 complex
+__host__ __device__ __forceinline__ long long record_bytes(int w, int nd) {
+    return 32LL * (8LL * w * nd + 8 + 4LL * w);
 }
+__host__ __device__ __forceinline__ int record_width(long long bytes, int nd) {
+    return (int)((bytes / 32 - 8) / (4 + 8 * nd));
+}
+enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2 };
+__host__ __device__ constexpr int hop_doubles(int hop) { return hop == kHopConst ? 0 : hop == kHopComplex ? 2 : 1; }
 
 struct Mat {
     const unsigned char* __restrict__ rec;      // packed slice records
@@ -79,6 +84,8 @@ struct Mat {
     int K;                                      // K_max
     int uniform;                                // every record has width K
     int cplx;
+    int hop;                                    // Hop variant of the records
+    double hop_const;                           // kHopConst: the one hopping value
     double inv_dE;
     double box;                                 // <= 0: open boundary
 };
@@ -402,17 +409,18 @@ __device__ __forceinline__ void cv_fma(CV<V>& acc, double hr, double hi, const C
 }
 
 // U rounds (U * RS rows) of one slice whose record and own rows sit in shared memory at `stage`.
-template <int B, int KT, bool CPLX, int MODE, int U>
+template <int B, int KT, int HOP, int MODE, int U>
 __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
                                           long long slice, int j0, int lane, double scale,
                                           double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V]) {
     constexpr int V = LaneShape<B>::V, LPR = LaneShape<B>::LPR, RS = LaneShape<B>::RS;
     constexpr int KU = KT > 0 ? KT : 1;
     constexpr bool MSD = (MODE == kModeEvolveMsd);
+    constexpr bool CPLX = (HOP == kHopComplex), CONST = (HOP == kHopConst);
     const int rl = lane / LPR, l = lane % LPR;
     const double* s_hre = reinterpret_cast<const double*>(stage);
     const double* s_him = s_hre + (size_t)w * 32;
-    const double* s_on = s_hre + (size_t)w * 32 * (CPLX ? 2 : 1);
+    const double* s_on = s_hre + (size_t)w * 32 * hop_doubles(HOP);
     const int* s_col = reinterpret_cast<const int*>(s_on + 32);
     // staged vector rows: [in | (in_e) | prev | (prev_e)], each 32 * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
@@ -456,11 +464,16 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
         // all gathers of the U rows first (independent loads in flight), then the arithmetic
         CV<V> v[U][KU], ve[U][MSD ? KU : 1];
         double xn[U][MSD ? KU : 1];
+        double hc[U][CONST ? KU : 1];
 #pragma unroll
         for (int k = 0; k < KU; ++k) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int c = s_col[k * 32 + r[u]];
+                int c = s_col[k * 32 + r[u]];
+                if (CONST) {   // padding is col = -1: own row with weight 0
+                    hc[u][k] = c >= 0 ? m.hop_const : 0.0;
+                    c = c >= 0 ? c : row0 + (ok[u] ? r[u] : 0);
+                }
                 v[u][k] = cv_gather<V>(a.in, sa_in, c, row0, B, l);
                 if (MSD) {
                     ve[u][k] = cv_gather<V>(a.in_e, sa_in_e, c, row0, B, l);
@@ -476,7 +489,7 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
             if (MSD) cv_fma<V, false>(sum_e[u], on, 0.0, self_e[u]);
 #pragma unroll
             for (int k = 0; k < KU; ++k) {
-                const double hr = s_hre[k * 32 + r[u]];
+                const double hr = CONST ? hc[u][k] : s_hre[k * 32 + r[u]];
                 double hi = 0.0;
                 if (CPLX) hi = s_him[k * 32 + r[u]];
                 cv_fma<V, CPLX>(sum[u], hr, hi, v[u][k]);
@@ -499,9 +512,14 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
         for (int k = 0; k < w; ++k) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int c = s_col[k * 32 + r[u]];
-                const double hr = s_hre[k * 32 + r[u]];
-                double hi = 0.0;
+                int c = s_col[k * 32 + r[u]];
+                double hr, hi = 0.0;
+                if (CONST) {
+                    hr = c >= 0 ? m.hop_const : 0.0;
+                    c = c >= 0 ? c : row0 + (ok[u] ? r[u] : 0);
+                } else {
+                    hr = s_hre[k * 32 + r[u]];
+                }
                 if (CPLX) hi = s_him[k * 32 + r[u]];
                 const CV<V> vv = cv_gather<V>(a.in, sa_in, c, row0, B, l);
                 cv_fma<V, CPLX>(sum[u], hr, hi, vv);
@@ -577,7 +595,7 @@ __device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const
 // One Chebyshev recurrence step fused with what consumes it.  Persistent warps: global warp g
 // takes slices g, g + W, g + 2W, ... (W = warps in the grid), so neighbouring warps stream
 // neighbouring slices and the gathered rows stay hot in L1/L2.
-template <int B, int KT, bool CPLX, int MODE>
+template <int B, int KT, int HOP, int MODE>
 __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
     constexpr int Q = ModeTraits<MODE>::Q;
     constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
@@ -627,7 +645,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         const long long s = slice_of(i);
         long long off, bytes;
         if (KT > 0) {
-            bytes = record_bytes(KT, CPLX ? 1 : 0);
+            bytes = record_bytes(KT, hop_doubles(HOP));
             off = s * bytes;
         } else {
             off = m.slice_off[s];
@@ -668,34 +686,11 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         const long long slice = slice_of(i);
         int w = KT;
         if (KT == 0) {
-            const long long bytes = m.slice_off[slice + 1] - m.slice_off[slice];
-            w = (int)((bytes / 32 - 8) / (CPLX ? 20 : 12));
+            w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
         }
 #pragma unroll 1
         for (int j0 = 0; j0 < ROUNDS; j0 += U) {
-            walk_rows<B, KT, CPLX, MODE, U>(m, a, stage, w, slice, j0, lane, scale, red);
-#if GPUQT_PREFETCH_FAR
-            // Once per slice: if the next slice's record has landed, pull its out-of-slice
-            // neighbours (the rows no TMA stream brings in) towards L2 a whole slice ahead.
-            if (j0 == 0 && i + 1 < n_my) {
-                const int st1 = (int)((i + 1) % stages);
-                if (mbar_test(&bars[st1], (uint32_t)(((i + 1) / stages) & 1))) {
-                    const long long s1 = slice_of(i + 1);
-                    int w1 = KT;
-                    if (KT == 0) w1 = (int)(((m.slice_off[s1 + 1] - m.slice_off[s1]) / 32 - 8) / (CPLX ? 20 : 12));
-                    const unsigned char* nxt = wstage + (size_t)st1 * stage_bytes;
-                    const int* col1 = reinterpret_cast<const int*>(nxt + (size_t)w1 * 256 * (CPLX ? 2 : 1) + 256);
-                    const int row1 = (int)(s1 * 32);
-                    for (int k = 0; k < w1; ++k) {
-                        const int c = col1[k * 32 + lane];
-                        if ((unsigned)(c - row1) >= 32u) {
-                            prefetch_l2(a.in + (size_t)c * B);
-                            if (MODE == kModeEvolveMsd) prefetch_l2(a.in_e + (size_t)c * B);
-                        }
-                    }
-                }
-            }
-#endif
+            walk_rows<B, KT, HOP, MODE, U>(m, a, stage, w, slice, j0, lane, scale, red);
         }
         __syncwarp();
     }
@@ -714,18 +709,19 @@ struct RecView {
 };
 __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
     long long off, bytes;
+    const int nd = hop_doubles(m.hop);
     if (m.uniform) {
-        bytes = record_bytes(m.K, m.cplx);
+        bytes = record_bytes(m.K, nd);
         off = slice * bytes;
     } else {
         off = m.slice_off[slice];
         bytes = m.slice_off[slice + 1] - off;
     }
     RecView v;
-    v.w = (int)((bytes / 32 - 8) / (m.cplx ? 20 : 12));
+    v.w = record_width(bytes, nd);
     v.hre = reinterpret_cast<const double*>(m.rec + off);
     v.him = v.hre + (size_t)v.w * 32;
-    v.on = v.hre + (size_t)v.w * 32 * (m.cplx ? 2 : 1);
+    v.on = v.hre + (size_t)v.w * 32 * nd;
     v.col = reinterpret_cast<const int*>(v.on + 32);
     return v;
 }
@@ -746,9 +742,16 @@ __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const d
         const double xm = m.x[row];
         double sr = 0.0, si = 0.0;
         for (int k = 0; k < rv.w; ++k) {
-            const int c = rv.col[k * 32 + r];
+            int c = rv.col[k * 32 + r];
+            double hr;
+            if (m.hop == kHopConst) {
+                hr = c >= 0 ? m.hop_const : 0.0;
+                c = c >= 0 ? c : (int)row;
+            } else {
+                hr = rv.hre[k * 32 + r];
+            }
             const double dx = min_image(m.x[c] - xm, m.box);
-            const double wr = dx * rv.hre[k * 32 + r];
+            const double wr = dx * hr;
             const double2 v = in[(size_t)c * B + b];
             sr = fma(wr, v.x, sr);
             si = fma(wr, v.y, si);
@@ -870,7 +873,12 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
     double hr = 0.0, hi = 0.0, d = 0.0;
     if (k < rv.w) {
         c = rv.col[k * 32 + r];
-        hr = rv.hre[k * 32 + r];
+        if (m.hop == kHopConst) {
+            hr = c >= 0 ? m.hop_const : 0.0;
+            c = c >= 0 ? c : (int)row;
+        } else {
+            hr = rv.hre[k * 32 + r];
+        }
         if (m.cplx) hi = rv.him[k * 32 + r];
         d = min_image(m.x[c] - m.x[row], m.box);
     }

@@ -44,6 +44,11 @@ def small_models():
         ("square_open", L.square(41, 23, W=1.0, seed=6, periodic=False)),       # generic width path
         ("peierls_cplx", L.square_peierls(45, 31, flux_quanta=3, W=1.5, seed=7)),  # complex hoppings
         ("chain_k2", L.chain(3001, W=1.0, seed=8)),                             # generic K = 2
+        # per-entry real hoppings (every model above without Peierls phases has ONE hopping value
+        # and is stored in the constant-hopping record variant)
+        ("square_bonddis", L.with_bond_disorder(L.square(52, 33, W=1.0, seed=13), 0.5, 21)),
+        ("graphene_vac_bonddis", L.with_bond_disorder(L.graphene(23, 17, vacancy_fraction=0.05, vacancy_seed=4), 0.3, 22)),
+        ("cubic_bonddis", L.with_bond_disorder(L.cubic(11, W=8.0, seed=14, energy_scale=11.0), 0.2, 23)),
     ]
 
 
@@ -243,3 +248,28 @@ def test_config_families_small(gq, oracle_mod, key):
     ref = o.kpm_transform(C, E)
     assert np.max(np.abs(g.kpm_transform(C, E) - ref)) / np.max(np.abs(ref)) <= TOL
     g.close()
+
+
+def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod, monkeypatch):
+    """The constant-hopping record variant (no hop array, padding col = -1) and the per-entry
+    variant (GPUQT_HOP_CONST=0) of the same model decode to the same table and give moments and
+    vectors within rounding of the oracle."""
+    model = L.graphene(31, 19, W=0.5, seed=3, vacancy_fraction=0.2, vacancy_seed=9)   # many padded rows
+    phi = L.random_phase_vectors(model.N, 4, config=58)
+    o = oracle_mod.Oracle(model, batch=4, modes=oracle_mod.MODE_MSD | oracle_mod.MODE_VAC)
+    o.set_state(phi)
+    ref_tab = o.get_table()
+    ref_dos, ref_vac = o.dos_moments(40), o.vac(40)
+    o.evolve(0.8, 45)
+    ref_chi = o.get_state(oracle_mod.CHI)
+    for flag in ("1", "0"):
+        monkeypatch.setenv("GPUQT_HOP_CONST", flag)
+        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC)
+        for a, b in zip(g.get_table(), ref_tab):
+            assert a.tobytes() == b.tobytes()
+        g.set_state(phi)
+        assert np.max(np.abs(g.dos_moments(40) - ref_dos)) / model.N <= TOL
+        assert np.max(np.abs(g.vac(40) - ref_vac)) / np.max(np.abs(ref_vac[:, 0])) <= TOL
+        g.evolve(0.8, 45)
+        assert vec_err(g.get_state(gq.STATE_CHI), ref_chi) <= TOL
+        g.close()

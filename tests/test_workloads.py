@@ -119,3 +119,15 @@ def test_random_phase_vectors():
     assert np.allclose(np.sum(v * v, axis=2), 1.0, atol=1e-15)
     assert not np.array_equal(v[0], v[1])
     assert np.array_equal(v[1], L.random_phase_vectors(1000, 1, config=4, first_vector=1)[0])
+
+
+def test_bond_disorder_is_hermitian_and_not_constant():
+    from paper_1705_01387_b200 import binding
+    base = L.graphene(7, 5, vacancy_fraction=0.1, vacancy_seed=2)
+    m = L.with_bond_disorder(base, 0.4, 7)
+    assert binding.validate(m) == 0                                   # bit-exact Hermiticity, Gershgorin
+    h = m.hop_re.reshape(m.N, m.K)
+    valid = np.arange(m.K)[None, :] < m.nbr_count[:, None]
+    assert np.unique(h[valid]).size > 10
+    assert np.all(np.abs(h[valid] / -2.7 - 1.0) <= 0.2 + 1e-12)
+    assert np.all(h[~valid] == 0.0)

@@ -66,6 +66,31 @@ def random_phase_vectors(N: int, batch: int, config: int, first_vector: int = 0)
     return out
 
 
+def with_bond_disorder(model: TBModel, delta: float, seed: int) -> TBModel:
+    """Real, bond-dependent hoppings h_mn = h0 * (1 + delta * (u_mn - 1/2)), u_mn = u_nm a counter-based
+    uniform of the unordered pair (min, max) -- symmetric bit for bit, so H stays Hermitian.  Exercises
+    the per-entry real-hopping storage (the paper's hopping.in with distinct values)."""
+    assert model.hop_im is None
+    N, K = model.N, model.K
+    idx = model.nbr_index.reshape(N, K).astype(np.int64)
+    rows = np.repeat(np.arange(N, dtype=np.int64)[:, None], K, axis=1)
+    valid = np.arange(K)[None, :] < model.nbr_count[:, None]
+    lo, hi = np.minimum(rows, idx), np.maximum(rows, idx)
+    pair = np.where(valid, lo * N + hi, 0).reshape(-1)
+    with np.errstate(over="ignore"):
+        z = np.uint64(seed & 0xFFFFFFFFFFFFFFFF) + rng._GAMMA * (pair.astype(np.uint64) + np.uint64(1))
+        z = (z ^ (z >> np.uint64(30))) * rng._M1
+        z = (z ^ (z >> np.uint64(27))) * rng._M2
+        z = z ^ (z >> np.uint64(31))
+    u = (z >> np.uint64(11)).astype(np.float64) * (2.0 ** -53)
+    h0 = model.hop_re if model.hop_re is not None else np.full(N * K, -1.0)
+    hre = np.where(valid.reshape(-1), h0 * (1.0 + delta * (u - 0.5)), 0.0)
+    return TBModel(name=model.name + "_bonddis", N=N, K=K, nbr_count=model.nbr_count, nbr_index=model.nbr_index,
+                   hop_re=np.ascontiguousarray(hre), hop_im=None, onsite=model.onsite, x=model.x,
+                   box_length=model.box_length, volume=model.volume,
+                   energy_scale=model.energy_scale * (1.0 + abs(delta) / 2.0), meta=dict(model.meta))
+
+
 # --------------------------------------------------------------------------- hypercubic lattices
 def chain(L: int, W: float = 0.0, seed: int = 0, periodic: bool = True, hop: float = -1.0,
           energy_scale: Optional[float] = None, explicit_hop: bool = False) -> TBModel:
