@@ -99,8 +99,9 @@ Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
     const size_t n_slices = (size_t)((N + 31) / 32);
     L.rec = take(rec_bytes);
     L.slice_off = take((n_slices + 1) * sizeof(long long));
-    L.x = take((size_t)N * sizeof(double));
-    L.vectors = take((size_t)n_vectors(modes) * align_up((size_t)N * B * sizeof(double2)));
+    L.x = take((size_t)(N + 1) * sizeof(double));
+    // every vector buffer has N + 1 rows; row N stays zero for ever (nothing writes it)
+    L.vectors = take((size_t)n_vectors(modes) * align_up((size_t)(N + 1) * B * sizeof(double2)));
     L.partials = take((size_t)kMaxGrid * kPartialDoubles * sizeof(double));
     L.dots = take((size_t)GPUQT_MAX_MOMENTS * 3 * 8 * sizeof(double));
     L.moments = take((size_t)GPUQT_MAX_MOMENTS * 8 * sizeof(double));
@@ -494,6 +495,10 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     };
     ce = up(d_rec, sell.rec.data(), rec_bytes);
     if (ce == cudaSuccess) ce = up(d_x, x, (size_t)N * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(d_x + N, 0, sizeof(double), h->stream);
+    if (ce == cudaSuccess)
+        ce = cudaMemsetAsync(base + L.vectors, 0, (size_t)n_vectors(modes) * align_up((size_t)(N + 1) * batch * sizeof(double2)),
+                             h->stream);
     if (ce == cudaSuccess) ce = up(d_sp, sell.slice_off.data(), sell.slice_off.size() * sizeof(long long));
     if (ce == cudaSuccess) ce = cudaMemsetAsync(base + L.ticket, 0, 256, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
@@ -517,7 +522,7 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->alternate = env_int("GPUQT_ALTERNATE", 1);
     h->run = std::max(1, env_int("GPUQT_RUN", 16) / kWarps) * kWarps;
 
-    const size_t vstride = align_up((size_t)N * batch * sizeof(double2));
+    const size_t vstride = align_up((size_t)(N + 1) * batch * sizeof(double2));
     char* v = base + L.vectors;
     auto nextv = [&]() {
         double2* p = (double2*)v;

@@ -94,7 +94,8 @@ inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32
 //   double hre[w][32] (nd >= 1) | double him[w][32] (nd == 2) | double onsite[32] | int32 col[w][32]
 // with w the largest neighbour count in the slice and nd the doubles stored per entry: 2 complex,
 // 1 real, 0 when every listed hopping is the same real number (hop_const; the paper's default
-// "all hoppings -1", and every clean-lattice model) -- then padding is col = -1.  If padding every record to K_max costs less
+// "all hoppings -1", and every clean-lattice model) -- then padding is col = N, the
+// all-zero row every device vector carries.  If padding every record to K_max costs less
 // than 1/16 extra bytes the table is stored uniform (w = K_max everywhere), which lets the
 // kernels compute record offsets arithmetically and unroll the neighbour walk.
 struct SellHost {
@@ -171,7 +172,7 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
                     if (s.nd >= 1) r_hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
                     if (s.nd == 2) r_him[e] = him[(size_t)m * K + k];
                 } else if (s.nd == 0) {
-                    r_col[e] = -1;                                             // padding: no entry
+                    r_col[e] = (int32_t)N;                                     // padding: the zero row
                 } else {
                     r_col[e] = (int32_t)(m < N ? m : N - 1);                   // padding: own row, hop 0
                 }

@@ -12,7 +12,8 @@
 //             of 128.  Records are stored back to back; slice_off[s] is the byte offset of record
 //             s.  Padding entries are (own row, hop 0.0); in the constant-hopping variant (nd = 0:
 //             every stored hopping is the same real number, kept in Mat::hop_const) padding is
-//             col = -1.  One record = one 1-D TMA bulk copy.
+//             col = N: every vector buffer carries an all-zero row N (and x[N] = 0), so the walk
+//             needs no guard.  One record = one 1-D TMA bulk copy.
 //   warp      the unit of work is (warp, slice).  A stage of a warp's shared-memory pipeline holds
 //             everything the slice streams from HBM exactly once: the packed record, the slice's
 //             own rows of T_{m-1} (and e_{m-1}) and of T_{m-2} (and e_{m-2}) -- each one 1-D TMA
@@ -29,15 +30,6 @@
 
 #ifndef GPUQT_THREADS
 #define GPUQT_THREADS 256
-#endif
-#ifndef GPUQT_U_KPM        // sub-steps of a slice processed together (independent gathers in flight)
-#define GPUQT_U_KPM 1
-#endif
-#ifndef GPUQT_U_EVOLVE
-#define GPUQT_U_EVOLVE 1
-#endif
-#ifndef GPUQT_U_MSD
-#define GPUQT_U_MSD 1
 #endif
 
 #ifndef GPUQT_MINB
@@ -78,7 +70,7 @@ __host__ __device__ constexpr int hop_doubles(int hop) { return hop == kHopConst
 struct Mat {
     const unsigned char* __restrict__ rec;      // packed slice records
     const long long* __restrict__ slice_off;    // [n_slices + 1] byte offsets (ragged variant)
-    const double* __restrict__ x;               // [N]
+    const double* __restrict__ x;               // [N + 1], x[N] = 0
     long long N;
     long long n_slices;
     int K;                                      // K_max
@@ -270,9 +262,6 @@ template <int MODE>
 struct ModeTraits {
     static constexpr int Q = (MODE == kModeDoubling) ? 3 : 2;
     static constexpr int kMinBlocks = (MODE == kModeEvolveMsd) ? GPUQT_MINB_MSD : GPUQT_MINB;   // register cap
-    static constexpr int U = (MODE == kModeEvolveMsd) ? GPUQT_U_MSD
-                             : (MODE == kModeEvolve)  ? GPUQT_U_EVOLVE
-                                                      : GPUQT_U_KPM;
 };
 
 // Number of vector streams staged per slice: own rows of T_{m-1}, T_{m-2} (x2 for the (a, e) pair).
@@ -349,16 +338,18 @@ __device__ __forceinline__ void cv_st<2>(double2* p, const CV<2>& v) {
 #endif
 }
 // Gather of V consecutive vectors of row c of T_{m-1}: rows of the current slice come from the
-// staged copy in shared memory (s_own = shared-window address of the slice's row 0), the others
-// from global memory with an L2 evict_last hint (they are re-read by the neighbouring slices).
-// Both loads are predicated, so there is no branch.
+// staged copy in shared memory, the others from global memory with an L2 evict_last hint (they are
+// re-read by the neighbouring slices).  Both loads are predicated, so there is no branch.
+//   g_l  = byte address of (row 0, the lane's first vector) in global memory
+//   s_l  = shared-window address of the same element of the slice's staged rows, minus row0 * RB
+//   RB   = bytes of one row (16 B)
 template <int V>
-__device__ __forceinline__ CV<V> cv_gather(const double2* g, uint32_t s_own, int c, int row0, int B, int l);
+__device__ __forceinline__ CV<V> cv_gather(const char* g_l, uint32_t s_l, int c, int row0, int RB);
 template <>
-__device__ __forceinline__ CV<1> cv_gather<1>(const double2* g, uint32_t s_own, int c, int row0, int B, int l) {
+__device__ __forceinline__ CV<1> cv_gather<1>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
-    const uint32_t sa = s_own + (d * B + l) * 16u;
-    const double2* ga = g + (size_t)c * B + l;
+    const uint32_t sa = s_l + (uint32_t)(c * RB);
+    const char* ga = g_l + (long long)c * RB;
     CV<1> v;
     asm volatile(
         "{\n"
@@ -372,10 +363,10 @@ __device__ __forceinline__ CV<1> cv_gather<1>(const double2* g, uint32_t s_own, 
     return v;
 }
 template <>
-__device__ __forceinline__ CV<2> cv_gather<2>(const double2* g, uint32_t s_own, int c, int row0, int B, int l) {
+__device__ __forceinline__ CV<2> cv_gather<2>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
-    const uint32_t sa = s_own + (d * B + l * 2) * 16u;
-    const double2* ga = g + (size_t)c * B + l * 2;
+    const uint32_t sa = s_l + (uint32_t)(c * RB);
+    const char* ga = g_l + (long long)c * RB;
     CV<2> v;
     asm volatile(
         "{\n"
@@ -408,200 +399,178 @@ __device__ __forceinline__ void cv_fma(CV<V>& acc, double hr, double hi, const C
     }
 }
 
-// U rounds (U * RS rows) of one slice whose record and own rows sit in shared memory at `stage`.
-template <int B, int KT, int HOP, int MODE, int U>
-__device__ __forceinline__ void walk_rows(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
-                                          long long slice, int j0, int lane, double scale,
-                                          double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V]) {
+template <int V>
+__device__ __forceinline__ void cv_add(CV<V>& acc, const CV<V>& v) {
+#pragma unroll
+    for (int j = 0; j < V; ++j) {
+        acc.re[j] += v.re[j];
+        acc.im[j] += v.im[j];
+    }
+}
+
+// One round (RS rows) of one slice whose record and own rows sit in shared memory at `stage`.
+// Rows past the end of the table (last slice only) are computed like the others on zero inputs
+// (their staged self / prev are replaced by 0 and their entries are padding), so the dot products
+// need no guard; only their stores are predicated off.
+template <int B, int KT, int HOP, int MODE>
+__device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
+                                           int row0, int rows_valid, int j, int lane, double scale,
+                                           double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V]) {
     constexpr int V = LaneShape<B>::V, LPR = LaneShape<B>::LPR, RS = LaneShape<B>::RS;
     constexpr int KU = KT > 0 ? KT : 1;
+    constexpr int RB = B * 16;   // bytes of one row of a vector set
     constexpr bool MSD = (MODE == kModeEvolveMsd);
     constexpr bool CPLX = (HOP == kHopComplex), CONST = (HOP == kHopConst);
     const int rl = lane / LPR, l = lane % LPR;
     const double* s_hre = reinterpret_cast<const double*>(stage);
-    const double* s_him = s_hre + (size_t)w * 32;
-    const double* s_on = s_hre + (size_t)w * 32 * hop_doubles(HOP);
+    const double* s_him = s_hre + w * 32;
+    const double* s_on = s_hre + w * 32 * hop_doubles(HOP);
     const int* s_col = reinterpret_cast<const int*>(s_on + 32);
     // staged vector rows: [in | (in_e) | prev | (prev_e)], each 32 * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
     const double2* s_in_e = s_in + 32 * B;
     const double2* s_prev = s_in + (MSD ? 2 : 1) * 32 * B;
     const double2* s_prev_e = s_prev + 32 * B;
-    const uint32_t sa_in = smem_u32(s_in), sa_in_e = smem_u32(s_in_e);
-    const int row0 = (int)(slice * 32);
+    // lane-relative bases of the gathers (see cv_gather)
+    const uint32_t sl_in = smem_u32(s_in + l * V) - (uint32_t)(row0 * RB);
+    const uint32_t sl_in_e = smem_u32(s_in_e + l * V) - (uint32_t)(row0 * RB);
+    const char* gl_in = reinterpret_cast<const char*>(a.in + l * V);
+    const char* gl_in_e = reinterpret_cast<const char*>(a.in_e + l * V);
 
-    int r[U];
-    bool ok[U];
-    size_t vi[U];
-    CV<V> other[U], other_e[U];
-    double xm[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        r[u] = (j0 + u) * RS + rl;
-        long long row = slice * 32 + r[u];
-        ok[u] = row < m.N;
-        if (!ok[u]) row = m.N - 1;
-        vi[u] = (size_t)row * B + l * V;
-        // streamed read-modify-write operands: issued first, consumed last
-        other[u] = other_e[u] = cv_zero<V>();
-        if (!a.first) {
-            if (MODE == kModeEvolve || MSD) other[u] = cv_ld_stream<V>(&a.acc[vi[u]]);
-            if (MSD) other_e[u] = cv_ld_stream<V>(&a.acc_e[vi[u]]);
-        }
-        if (MODE == kModeLeft) other[u] = cv_ld_stream<V>(&a.phiL[vi[u]]);
-        if (MSD) xm[u] = m.x[row];
-    }
+    const int r = j * RS + rl;
+    const bool ok = r < rows_valid;
+    const int si_ = r * B + l * V;                                     // element inside the staged rows
+    const size_t vi = (size_t)(row0 + (ok ? r : 0)) * B + l * V;       // element in global memory
 
-    CV<V> sum[U], sum_e[U], sum_x[U];   // H T_{m-1}, H e_{m-1}, [X,H] T_{m-1}  (unscaled)
-    CV<V> self[U], self_e[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const int si_ = r[u] * B + l * V;
-        self[u] = ok[u] ? cv_lds<V>(s_in + si_) : cv_zero<V>();
-        self_e[u] = (MSD && ok[u]) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
+    // streamed read-modify-write operands: issued first, consumed last
+    CV<V> other = cv_zero<V>(), other_e = cv_zero<V>();
+    if (!a.first) {
+        if (MODE == kModeEvolve || MSD) other = cv_ld_stream<V>(&a.acc[vi]);
+        if (MSD) other_e = cv_ld_stream<V>(&a.acc_e[vi]);
     }
+    if (MODE == kModeLeft) other = cv_ld_stream<V>(&a.phiL[vi]);
+    double xm = 0.0;
+    if (MSD) xm = m.x[row0 + (ok ? r : 0)];
+
+    const CV<V> self = ok ? cv_lds<V>(s_in + si_) : cv_zero<V>();
+    const CV<V> self_e = (MSD && ok) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
+    const double on = s_on[r];
+
+    CV<V> sum = cv_zero<V>(), sum_e = cv_zero<V>(), sum_x = cv_zero<V>();   // H T, H e, [X,H] T (unscaled)
     if (KT > 0) {
-        // all gathers of the U rows first (independent loads in flight), then the arithmetic
-        CV<V> v[U][KU], ve[U][MSD ? KU : 1];
-        double xn[U][MSD ? KU : 1];
-        double hc[U][CONST ? KU : 1];
+        // all gathers of the row first (independent loads in flight), then the arithmetic
+        CV<V> v[KU], ve[MSD ? KU : 1];
+        double xn[MSD ? KU : 1];
 #pragma unroll
         for (int k = 0; k < KU; ++k) {
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                int c = s_col[k * 32 + r[u]];
-                if (CONST) {   // padding is col = -1: own row with weight 0
-                    hc[u][k] = c >= 0 ? m.hop_const : 0.0;
-                    c = c >= 0 ? c : row0 + (ok[u] ? r[u] : 0);
-                }
-                v[u][k] = cv_gather<V>(a.in, sa_in, c, row0, B, l);
-                if (MSD) {
-                    ve[u][k] = cv_gather<V>(a.in_e, sa_in_e, c, row0, B, l);
-                    xn[u][k] = m.x[c];
-                }
+            const int c = s_col[k * 32 + r];
+            v[k] = cv_gather<V>(gl_in, sl_in, c, row0, RB);
+            if (MSD) {
+                ve[k] = cv_gather<V>(gl_in_e, sl_in_e, c, row0, RB);
+                xn[k] = m.x[c];
             }
         }
 #pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const double on = s_on[r[u]];
-            sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
-            cv_fma<V, false>(sum[u], on, 0.0, self[u]);
-            if (MSD) cv_fma<V, false>(sum_e[u], on, 0.0, self_e[u]);
-#pragma unroll
-            for (int k = 0; k < KU; ++k) {
-                const double hr = CONST ? hc[u][k] : s_hre[k * 32 + r[u]];
-                double hi = 0.0;
-                if (CPLX) hi = s_him[k * 32 + r[u]];
-                cv_fma<V, CPLX>(sum[u], hr, hi, v[u][k]);
-                if (MSD) {
-                    cv_fma<V, CPLX>(sum_e[u], hr, hi, ve[u][k]);
-                    // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
-                    const double ndx = -min_image(xn[u][k] - xm[u], m.box);
-                    cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, v[u][k]);
-                }
+        for (int k = 0; k < KU; ++k) {
+            double hr = 1.0, hi = 0.0;                                  // CONST: the factor is applied once below
+            if (!CONST) hr = s_hre[k * 32 + r];
+            if (CPLX) hi = s_him[k * 32 + r];
+            if (CONST) cv_add<V>(sum, v[k]);
+            else cv_fma<V, CPLX>(sum, hr, hi, v[k]);
+            if (MSD) {
+                if (CONST) cv_add<V>(sum_e, ve[k]);
+                else cv_fma<V, CPLX>(sum_e, hr, hi, ve[k]);
+                // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
+                const double ndx = -min_image(xn[k] - xm, m.box);
+                cv_fma<V, CPLX>(sum_x, ndx * hr, ndx * hi, v[k]);
             }
         }
     } else {
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const double on = s_on[r[u]];
-            sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
-            cv_fma<V, false>(sum[u], on, 0.0, self[u]);
-            if (MSD) cv_fma<V, false>(sum_e[u], on, 0.0, self_e[u]);
-        }
         for (int k = 0; k < w; ++k) {
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                int c = s_col[k * 32 + r[u]];
-                double hr, hi = 0.0;
-                if (CONST) {
-                    hr = c >= 0 ? m.hop_const : 0.0;
-                    c = c >= 0 ? c : row0 + (ok[u] ? r[u] : 0);
-                } else {
-                    hr = s_hre[k * 32 + r[u]];
-                }
-                if (CPLX) hi = s_him[k * 32 + r[u]];
-                const CV<V> vv = cv_gather<V>(a.in, sa_in, c, row0, B, l);
-                cv_fma<V, CPLX>(sum[u], hr, hi, vv);
-                if (MSD) {
-                    const CV<V> vve = cv_gather<V>(a.in_e, sa_in_e, c, row0, B, l);
-                    cv_fma<V, CPLX>(sum_e[u], hr, hi, vve);
-                    const double ndx = -min_image(m.x[c] - xm[u], m.box);
-                    cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, vv);
-                }
+            const int c = s_col[k * 32 + r];
+            double hr = 1.0, hi = 0.0;
+            if (!CONST) hr = s_hre[k * 32 + r];
+            if (CPLX) hi = s_him[k * 32 + r];
+            const CV<V> vv = cv_gather<V>(gl_in, sl_in, c, row0, RB);
+            if (CONST) cv_add<V>(sum, vv);
+            else cv_fma<V, CPLX>(sum, hr, hi, vv);
+            if (MSD) {
+                const CV<V> vve = cv_gather<V>(gl_in_e, sl_in_e, c, row0, RB);
+                if (CONST) cv_add<V>(sum_e, vve);
+                else cv_fma<V, CPLX>(sum_e, hr, hi, vve);
+                const double ndx = -min_image(m.x[c] - xm, m.box);
+                cv_fma<V, CPLX>(sum_x, ndx * hr, ndx * hi, vv);
             }
         }
     }
+    CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
+    if (!a.first && ok) {
+        prev = cv_lds<V>(s_prev + si_);
+        if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
+    }
+    const double hs = CONST ? scale * m.hop_const : scale;              // scale of the neighbour sums
+    const double os = scale * on;                                       // scale of the on-site term
+    CV<V> t, te, acc, ae;   // T_m, e_m, and the accumulators
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const int si_ = r[u] * B + l * V;
-        CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
-        if (!a.first && ok[u]) {
-            prev = cv_lds<V>(s_prev + si_);
-            if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
-        }
-        CV<V> t, te, acc, ae;   // T_m, e_m, and the accumulators
-#pragma unroll
-        for (int j = 0; j < V; ++j) {
-            t.re[j] = scale * sum[u].re[j] - prev.re[j];
-            t.im[j] = scale * sum[u].im[j] - prev.im[j];
-            if (MODE == kModeDoubling) {
-                if (ok[u]) {
-                    red[0 * V + j] += t.re[j] * t.re[j] + t.im[j] * t.im[j];
-                    red[1 * V + j] += t.re[j] * self[u].re[j] + t.im[j] * self[u].im[j];
-                    red[2 * V + j] += self[u].re[j] * self[u].re[j] + self[u].im[j] * self[u].im[j];
-                }
-            } else if (MODE == kModeLeft) {
-                if (ok[u]) {   // conj(l) * t
-                    red[0 * V + j] += other[u].re[j] * t.re[j] + other[u].im[j] * t.im[j];
-                    red[1 * V + j] += other[u].re[j] * t.im[j] - other[u].im[j] * t.re[j];
-                }
+    for (int q = 0; q < V; ++q) {
+        t.re[q] = fma(hs, sum.re[q], fma(os, self.re[q], -prev.re[q]));
+        t.im[q] = fma(hs, sum.im[q], fma(os, self.im[q], -prev.im[q]));
+        if (MODE == kModeDoubling) {
+            red[0 * V + q] += t.re[q] * t.re[q] + t.im[q] * t.im[q];
+            red[1 * V + q] += t.re[q] * self.re[q] + t.im[q] * self.im[q];
+            red[2 * V + q] += self.re[q] * self.re[q] + self.im[q] * self.im[q];
+        } else if (MODE == kModeLeft) {   // conj(l) * t
+            red[0 * V + q] += other.re[q] * t.re[q] + other.im[q] * t.im[q];
+            red[1 * V + q] += other.re[q] * t.im[q] - other.im[q] * t.re[q];
+        } else {
+            if (a.first) {
+                acc.re[q] = a.c0r * self.re[q] - a.c0i * self.im[q];
+                acc.im[q] = a.c0r * self.im[q] + a.c0i * self.re[q];
             } else {
+                acc.re[q] = other.re[q];
+                acc.im[q] = other.im[q];
+            }
+            acc.re[q] += a.cr * t.re[q] - a.ci * t.im[q];
+            acc.im[q] += a.cr * t.im[q] + a.ci * t.re[q];
+            if (MSD) {
+                te.re[q] = fma(hs, sum_e.re[q] + sum_x.re[q], fma(os, self_e.re[q], -prev_e.re[q]));
+                te.im[q] = fma(hs, sum_e.im[q] + sum_x.im[q], fma(os, self_e.im[q], -prev_e.im[q]));
                 if (a.first) {
-                    acc.re[j] = a.c0r * self[u].re[j] - a.c0i * self[u].im[j];
-                    acc.im[j] = a.c0r * self[u].im[j] + a.c0i * self[u].re[j];
+                    ae.re[q] = a.c0r * self_e.re[q] - a.c0i * self_e.im[q];
+                    ae.im[q] = a.c0r * self_e.im[q] + a.c0i * self_e.re[q];
                 } else {
-                    acc.re[j] = other[u].re[j];
-                    acc.im[j] = other[u].im[j];
+                    ae.re[q] = other_e.re[q];
+                    ae.im[q] = other_e.im[q];
                 }
-                acc.re[j] += a.cr * t.re[j] - a.ci * t.im[j];
-                acc.im[j] += a.cr * t.im[j] + a.ci * t.re[j];
-                if (MSD) {
-                    te.re[j] = scale * (sum_e[u].re[j] + sum_x[u].re[j]) - prev_e.re[j];
-                    te.im[j] = scale * (sum_e[u].im[j] + sum_x[u].im[j]) - prev_e.im[j];
-                    if (a.first) {
-                        ae.re[j] = a.c0r * self_e[u].re[j] - a.c0i * self_e[u].im[j];
-                        ae.im[j] = a.c0r * self_e[u].im[j] + a.c0i * self_e[u].re[j];
-                    } else {
-                        ae.re[j] = other_e[u].re[j];
-                        ae.im[j] = other_e[u].im[j];
-                    }
-                    ae.re[j] += a.cr * te.re[j] - a.ci * te.im[j];
-                    ae.im[j] += a.cr * te.im[j] + a.ci * te.re[j];
-                }
+                ae.re[q] += a.cr * te.re[q] - a.ci * te.im[q];
+                ae.im[q] += a.cr * te.im[q] + a.ci * te.re[q];
             }
         }
-        if (ok[u]) {
-            if (a.store) cv_st<V>(&a.out[vi[u]], t);
-            if (MODE == kModeEvolve || MSD) cv_st<V>(&a.acc[vi[u]], acc);
-            if (MSD) {
-                if (a.store) cv_st<V>(&a.out_e[vi[u]], te);
-                cv_st<V>(&a.acc_e[vi[u]], ae);
-            }
+    }
+    if (ok) {
+        if (a.store) cv_st<V>(&a.out[vi], t);
+        if (MODE == kModeEvolve || MSD) cv_st<V>(&a.acc[vi], acc);
+        if (MSD) {
+            if (a.store) cv_st<V>(&a.out_e[vi], te);
+            cv_st<V>(&a.acc_e[vi], ae);
         }
     }
 }
 
-// One Chebyshev recurrence step fused with what consumes it.  Persistent warps: global warp g
-// takes slices g, g + W, g + 2W, ... (W = warps in the grid), so neighbouring warps stream
-// neighbouring slices and the gathered rows stay hot in L1/L2.
+// One Chebyshev recurrence step fused with what consumes it.  Persistent CTAs: the slices are cut
+// into runs of a.run consecutive slices; CTA c walks runs c, c + G, c + 2G, ...; inside a run warp w
+// takes slices w, w + kWarps, ...  A CTA therefore streams a contiguous band of rows and the grid
+// sweeps the vector as a tight front, so gathers to nearby rows (the +-x, +-y, +-z neighbours of a
+// lattice) are served by L1/L2.  All loop indices are kept incrementally (no divisions in the loop).
 template <int B, int KT, int HOP, int MODE>
 __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
     constexpr int Q = ModeTraits<MODE>::Q;
     constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
-    constexpr int U = ModeTraits<MODE>::U < ROUNDS ? ModeTraits<MODE>::U : ROUNDS;
+    constexpr int RB = B * 16;
+    constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
     extern __shared__ __align__(128) unsigned char smem[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
     const int stages = a.stages;
     const int stage_bytes = a.stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + warp * kMaxStages;
@@ -612,86 +581,99 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
     const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
 
-    // Work split: the slices are cut into runs of a.run consecutive slices; CTA c walks runs
-    // c, c + G, c + 2G, ...; inside a run warp w takes slices w, w + kWarps, ...  A CTA therefore
-    // streams a contiguous band of rows, so gathers to nearby rows (the +-x, +-y neighbours of a
-    // lattice) are served by the SM's L1 instead of L2.
+    const int N = (int)m.N, n_slices = (int)m.n_slices;
     const int per = a.run / kWarps;
-    const long long n_runs = (m.n_slices + a.run - 1) / a.run;
-    const long long G = gridDim.x;
-    const long long my_runs = blockIdx.x < n_runs ? (n_runs - blockIdx.x + G - 1) / G : 0;
-    long long n_my = 0;
+    const int n_runs = (n_slices + a.run - 1) / a.run;
+    const int G = gridDim.x;
+    const int my_runs = (int)blockIdx.x < n_runs ? (n_runs - (int)blockIdx.x + G - 1) / G : 0;
+    int n_my = 0;
     if (my_runs > 0) {
-        const long long last = blockIdx.x + (my_runs - 1) * G;
-        const long long rem = m.n_slices - last * a.run;          // slices in my last run (may be partial)
-        const long long in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
+        const int last = blockIdx.x + (my_runs - 1) * G;
+        const int rem = n_slices - last * a.run;          // slices in my last run (may be partial)
+        const int in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
         n_my = (my_runs - 1) * per + in_last;
     }
-    uint64_t policy = 0, policy_last = 0;
+    uint64_t policy = 0;
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(&bars[s], 1);
         fence_mbar_init();
         policy = policy_evict_first();
-        policy_last = policy_evict_last();
     }
-    (void)policy_last;
     __syncwarp();
 
-    auto slice_of = [&](long long i) {
-        const long long s = (blockIdx.x + (i / per) * G) * a.run + warp + (long long)kWarps * (i % per);
-        return a.reverse ? m.n_slices - 1 - s : s;
+    // position of a pipeline cursor: slice (forward order), index inside the run, stage, phase
+    struct Cursor {
+        int s, k, st;
+        uint32_t ph;
     };
-    auto issue = [&](long long i) {   // lane 0 only: every HBM stream of slice i -> one stage, one mbarrier
-        const long long s = slice_of(i);
-        long long off, bytes;
+    const int jump = G * a.run - (per - 1) * kWarps;     // last slice of a run -> first slice of my next run
+    auto advance = [&](Cursor& c) {
+        if (++c.k == per) {
+            c.k = 0;
+            c.s += jump;
+        } else {
+            c.s += kWarps;
+        }
+        if (++c.st == stages) {
+            c.st = 0;
+            c.ph ^= 1u;
+        }
+    };
+    auto issue = [&](const Cursor& c) {   // lane 0 only: every HBM stream of the slice -> one stage, one mbarrier
+        const int s = a.reverse ? n_slices - 1 - c.s : c.s;
+        long long off;
+        uint32_t bytes;
         if (KT > 0) {
-            bytes = record_bytes(KT, hop_doubles(HOP));
-            off = s * bytes;
+            bytes = (uint32_t)record_bytes(KT, hop_doubles(HOP));
+            off = (long long)s * bytes;
         } else {
             off = m.slice_off[s];
-            bytes = m.slice_off[s + 1] - off;
+            bytes = (uint32_t)(m.slice_off[s + 1] - off);
         }
-        const long long rows = (m.N - s * 32) < 32 ? (m.N - s * 32) : 32;
-        const uint32_t vbytes = (uint32_t)(rows * B * sizeof(double2));
-        constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
-        const uint32_t total = (uint32_t)bytes + vbytes * (a.first ? kPair : 2 * kPair);
-        const int st = (int)(i % stages);
-        unsigned char* dst = wstage + (size_t)st * stage_bytes;
+        const int left = N - s * 32;
+        const uint32_t vbytes = (uint32_t)((left < 32 ? left : 32) * RB);
+        // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
+        // constant-hopping padding entries point at it)
+        const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
+        const uint32_t total = bytes + vbytes_in * kPair + (a.first ? 0u : vbytes * kPair);
+        unsigned char* dst = wstage + c.st * stage_bytes;
         unsigned char* vdst = dst + a.rec_bytes;
         const size_t voff = (size_t)s * 32 * B;
-        mbar_expect_tx(&bars[st], total);
-        bulk_g2s(dst, m.rec + off, (uint32_t)bytes, &bars[st], policy);
-#if GPUQT_IN_POLICY == 1
-        bulk_g2s(vdst, a.in + voff, vbytes, &bars[st], policy_last);
-        if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 512 * B, a.in_e + voff, vbytes, &bars[st], policy_last);
-#else
-        bulk_g2s_nohint(vdst, a.in + voff, vbytes, &bars[st]);
-        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, a.in_e + voff, vbytes, &bars[st]);
-#endif
+        mbar_expect_tx(&bars[c.st], total);
+        bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
+        bulk_g2s_nohint(vdst, a.in + voff, vbytes_in, &bars[c.st]);
+        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, a.in_e + voff, vbytes_in, &bars[c.st]);
         if (!a.first) {
-            bulk_g2s(vdst + kPair * 512 * B, a.prev + voff, vbytes, &bars[st], policy);
-            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, a.prev_e + voff, vbytes, &bars[st], policy);
+            bulk_g2s(vdst + kPair * 512 * B, a.prev + voff, vbytes, &bars[c.st], policy);
+            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, a.prev_e + voff, vbytes, &bars[c.st], policy);
         }
     };
 
+    Cursor prod{(int)blockIdx.x * a.run + warp, 0, 0, 0u}, cons = prod;
+    int issued = 0;
     if (lane == 0) {
-        for (long long i = 0; i < stages - 1 && i < n_my; ++i) issue(i);
+        for (; issued < stages - 1 && issued < n_my; ++issued) {
+            issue(prod);
+            advance(prod);
+        }
     }
-    for (long long i = 0; i < n_my; ++i) {
-        // stage (i - 1) % stages was consumed by the whole warp in the previous iteration
-        if (lane == 0 && i + stages - 1 < n_my) issue(i + stages - 1);
-        const int st = (int)(i % stages);
-        mbar_wait(&bars[st], (uint32_t)((i / stages) & 1));
-        const unsigned char* stage = wstage + (size_t)st * stage_bytes;
-        const long long slice = slice_of(i);
+    for (int i = 0; i < n_my; ++i) {
+        // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
+        if (lane == 0 && issued < n_my) {
+            issue(prod);
+            advance(prod);
+            ++issued;
+        }
+        mbar_wait(&bars[cons.st], cons.ph);
+        const unsigned char* stage = wstage + cons.st * stage_bytes;
+        const int slice = a.reverse ? n_slices - 1 - cons.s : cons.s;
         int w = KT;
-        if (KT == 0) {
-            w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
-        }
+        if (KT == 0) w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
+        const int row0 = slice * 32;
+        const int rows_valid = N - row0;          // >= 32 except in the last slice
 #pragma unroll 1
-        for (int j0 = 0; j0 < ROUNDS; j0 += U) {
-            walk_rows<B, KT, HOP, MODE, U>(m, a, stage, w, slice, j0, lane, scale, red);
-        }
+        for (int j = 0; j < ROUNDS; ++j) walk_round<B, KT, HOP, MODE>(m, a, stage, w, row0, rows_valid, j, lane, scale, red);
+        advance(cons);
         __syncwarp();
     }
     if (MODE == kModeDoubling || MODE == kModeLeft)
@@ -742,14 +724,8 @@ __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const d
         const double xm = m.x[row];
         double sr = 0.0, si = 0.0;
         for (int k = 0; k < rv.w; ++k) {
-            int c = rv.col[k * 32 + r];
-            double hr;
-            if (m.hop == kHopConst) {
-                hr = c >= 0 ? m.hop_const : 0.0;
-                c = c >= 0 ? c : (int)row;
-            } else {
-                hr = rv.hre[k * 32 + r];
-            }
+            const int c = rv.col[k * 32 + r];               // constant-hopping padding: the zero row N
+            const double hr = (m.hop == kHopConst) ? m.hop_const : rv.hre[k * 32 + r];
             const double dx = min_image(m.x[c] - xm, m.box);
             const double wr = dx * hr;
             const double2 v = in[(size_t)c * B + b];
@@ -874,8 +850,8 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
     if (k < rv.w) {
         c = rv.col[k * 32 + r];
         if (m.hop == kHopConst) {
-            hr = c >= 0 ? m.hop_const : 0.0;
-            c = c >= 0 ? c : (int)row;
+            hr = c < m.N ? m.hop_const : 0.0;
+            c = c < m.N ? c : (int)row;
         } else {
             hr = rv.hre[k * 32 + r];
         }
