@@ -211,10 +211,12 @@ def run_ours(args, w):
             return replicas.max_over_ranks(ms, device="cuda"), out
 
         sampler = ClockSampler(local)
-        sampler.start()
+        if not args.no_clock_sampler:
+            sampler.start()
         ms, out = timed(False)
         clocks = sampler.stop()
-        stats = {c: g.kernel_stats(c) for c in range(5)}
+        stats = {c: (g.kernel_stats(c)[0], g.kernel_steps(c)) for c in range(5)}       # (ms, recurrence steps)
+        n_launches = sum(g.kernel_stats(c)[1] for c in range(5))
         ms_e2e, _ = timed(True)
 
     ev_w, mom_w = walks_per_step(w, order)
@@ -249,7 +251,7 @@ def run_ours(args, w):
                 traffic = json.load(open(tp)).get(f"{w.key}:{names[dom]}")
             except Exception:
                 traffic = None
-        launches = sum(stats[c][1] for c in range(5)) + args.steps * 3      # + finalize, jackson, transform
+        launches = n_launches + args.steps * 3      # + finalize, jackson, transform
         line = {"metric": "orbital-SpMV/s in Chebyshev evolution + KPM moments", "value": value,
                 "unit": "orbital-SpMV/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -274,6 +276,9 @@ def run_ours(args, w):
                              "stored_bytes_per_launch": stored_row_launch * model.N,
                              "stored_gbs": stored_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9,
                              "avg_launch_us": dom_ms * 1e3 / max(dom_n, 1), "launches": dom_n,
+                             "note": "per recurrence step: a launch of the step kernel performs two consecutive "
+                                     "steps (fused through L2) except the first / an odd last one; bytes and time "
+                                     "are both per step, so achieved = algorithmic bytes of a launch / its duration",
                              "share_of_step": dom_ms / ms,
                              "per_class_ms": {names[c]: stats[c][0] for c in names}},
                 }
@@ -295,6 +300,7 @@ def main():
     ap.add_argument("--config", default="c4", choices=sorted(configs.WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-clock-sampler", action="store_true", help="diagnostic: do not poll nvidia-smi during the timed region")
     args = ap.parse_args()
     w = configs.WORKLOADS[args.config]
     if args.impl == "reference":

@@ -149,9 +149,24 @@ int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, doubl
  * c_m = (2 - delta_0m) (-i sgn dt)^m J_m(dE |dt|), m < order   (Eq. 17).            */
 int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im);
 
+/* Host only: the work list of a launch that performs two consecutive recurrence steps (DESIGN.md 6,
+ * "two steps per launch").  nbr_ptr/nbr_slices: CSR over the 32-row slices of the slices each one
+ * gathers from (itself included); the table is cut into runs of `run` slices, CTA c of `grid` takes
+ * items c, c + grid, ...  items[2t] = run | step << 30 (run = 2^30 - 1: no-op), items[2t+1] = -1;
+ * a second-step item of run R may start when the first step of the runs
+ * dep_list[dep_ptr[R] .. dep_ptr[R+1]) is complete; `slack` = items by which it trails them in the
+ * list.  items / dep_ptr+dep_list may be NULL to query the sizes.  Exposed so that the schedule's
+ * invariants can be tested without a GPU.                                                         */
+int gpuqt_fused_schedule(int32_t n_slices, int32_t run, int32_t grid, int reverse, int32_t slack,
+                         const int32_t* nbr_ptr, const int32_t* nbr_slices, int32_t* items, int32_t capacity,
+                         int32_t* n_items, int32_t* dep_ptr, int32_t* dep_list, int32_t dep_capacity, int32_t* n_dep);
+
 /* Accumulated device time (CUDA events on the handle's stream around each run of launches) and
  * number of launches of one kernel class since the last reset.                                    */
 int gpuqt_kernel_stats(gpuqt_handle* h, int kernel_class, double* ms, int64_t* launches);
+/* Number of recurrence steps (Eq. 21/23 applications) those launches performed: a launch of the
+ * step kernels performs one step, or two consecutive steps fused through L2.        */
+int gpuqt_kernel_steps(gpuqt_handle* h, int kernel_class, int64_t* steps);
 int gpuqt_reset_stats(gpuqt_handle* h);
 
 const char* gpuqt_last_error(const gpuqt_handle* h);

@@ -42,6 +42,9 @@ _SIGNATURES = {
     "gpuqt_get_table": (C.c_int, [C.c_void_p, _ip, _dp, _dp, _dp]),
     "gpuqt_bessel_coeffs": (C.c_int, [C.c_double, C.c_double, C.c_int32, _dp, _dp]),
     "gpuqt_kernel_stats": (C.c_int, [C.c_void_p, C.c_int, _dp, C.POINTER(C.c_int64)]),
+    "gpuqt_fused_schedule": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.c_int, C.c_int32, _ip, _ip, _ip, C.c_int32, _ip,
+                                       _ip, _ip, C.c_int32, _ip]),
+    "gpuqt_kernel_steps": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "gpuqt_reset_stats": (C.c_int, [C.c_void_p]),
     "gpuqt_last_error": (C.c_char_p, [C.c_void_p]),
     "gpuqt_destroy": (None, [C.c_void_p]),
@@ -112,6 +115,27 @@ def choose_order(dE, dt, tol=1e-15):
     J = np.abs(bessel_coeffs(dE, dt, n)) / np.where(np.arange(n) == 0, 1.0, 2.0)
     big = np.nonzero(J >= tol)[0]
     return int(big[-1]) + 1 if big.size else 1
+
+
+def fused_schedule(nbr_ptr, nbr_slices, run, grid, reverse=0, slack=None):
+    """gpuqt_fused_schedule (host only) -> (items int32 [n_items][2], dep_ptr, dep_list)."""
+    nbr_ptr = np.ascontiguousarray(nbr_ptr, np.int32)
+    nbr_slices = np.ascontiguousarray(nbr_slices, np.int32)
+    n_slices = nbr_ptr.size - 1
+    slack = grid if slack is None else slack
+    n, nd = C.c_int32(), C.c_int32()
+    fn = load().gpuqt_fused_schedule
+    rc = fn(n_slices, run, grid, reverse, slack, _i(nbr_ptr), _i(nbr_slices), None, 0, C.byref(n), None, None, 0, C.byref(nd))
+    if rc:
+        raise GpuqtError(rc, "gpuqt_fused_schedule")
+    items = np.empty((n.value, 2), np.int32)
+    dep_ptr = np.empty((n_slices + run - 1) // run + 1, np.int32)
+    dep_list = np.empty(max(nd.value, 1), np.int32)
+    rc = fn(n_slices, run, grid, reverse, slack, _i(nbr_ptr), _i(nbr_slices), _i(items), n.value, C.byref(n),
+            _i(dep_ptr), _i(dep_list), nd.value, C.byref(nd))
+    if rc:
+        raise GpuqtError(rc, "gpuqt_fused_schedule")
+    return items, dep_ptr, dep_list[:nd.value]
 
 
 class GpuQT:
@@ -218,6 +242,11 @@ class GpuQT:
         ms, n = C.c_double(), C.c_int64()
         self._ck(load().gpuqt_kernel_stats(self._h, cls, C.byref(ms), C.byref(n)), "gpuqt_kernel_stats")
         return ms.value, n.value
+
+    def kernel_steps(self, cls):
+        n = C.c_int64()
+        self._ck(load().gpuqt_kernel_steps(self._h, cls, C.byref(n)), "gpuqt_kernel_steps")
+        return n.value
 
     def reset_stats(self):
         self._ck(load().gpuqt_reset_stats(self._h), "gpuqt_reset_stats")

@@ -15,12 +15,13 @@ using namespace gpuqt;
 namespace {
 
 constexpr int kMaxGrid = 4096;
-constexpr int kPartialDoubles = 32;   // Q*B <= 24
+constexpr int kPartialDoubles = 64;   // n_steps*Q*B <= 48
+constexpr int kRing = 4;              // recurrence ring: a fused pair reads two slots and writes two
 
 struct PendingStat {
     int cls;
     cudaEvent_t start, stop;
-    int64_t launches;
+    int64_t launches, steps;
 };
 
 }  // namespace
@@ -45,8 +46,22 @@ struct gpuqt_handle {
     size_t vec_elems = 0;   // N * B double2
     // vectors (device, inside the caller's workspace)
     double2 *psi = nullptr, *chi = nullptr, *va = nullptr, *vb = nullptr, *phiL = nullptr;
-    double2 *out0 = nullptr, *out1 = nullptr, *ring[3] = {nullptr, nullptr, nullptr},
-            *ringe[3] = {nullptr, nullptr, nullptr};
+    double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr, nullptr},
+            *ringe[kRing] = {nullptr, nullptr, nullptr, nullptr};
+    // fused pairs of steps: dependency structure of the table and the cached work lists
+    int fuse = 1, lag = 2;              // GPUQT_FUSE, GPUQT_LAG (slack of the second step in half rounds)
+    std::vector<int> nbr_ptr, nbr_slices;
+    struct DevSchedule {
+        int G, reverse, n_items, n_runs;
+        int2* items;
+        int *dep_ptr, *dep_list;
+        unsigned int* run_done;
+    };
+    std::vector<DevSchedule> schedules;
+    // library-owned scratch for the small transform / table-decode calls: grown on demand, kept
+    // (stream-ordered pool allocations can trim at every synchronisation and stall the step)
+    char* scratch = nullptr;
+    size_t scratch_bytes = 0;
     double *partials = nullptr, *dots = nullptr, *moments = nullptr;
     unsigned int* ticket = nullptr;
     int grid[4] = {0, 0, 0, 0};
@@ -56,6 +71,7 @@ struct gpuqt_handle {
     std::string err;
     double stat_ms[GPUQT_KERNEL_CLASSES] = {0};
     int64_t stat_launches[GPUQT_KERNEL_CLASSES] = {0};
+    int64_t stat_steps[GPUQT_KERNEL_CLASSES] = {0};     // recurrence steps (a fused launch does two)
     std::vector<PendingStat> pending;
     std::vector<cudaEvent_t> free_events;
 };
@@ -78,8 +94,8 @@ int cuda_fail(gpuqt_handle* h, cudaError_t e, const char* what) {
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 int n_vectors(int modes) {
-    int n = 2 + 3;                                  // psi, out0, ring[3]
-    if (modes & GPUQT_MODE_MSD) n += 2 + 3;         // chi, out1, ringe[3]
+    int n = 2 + kRing;                              // psi, out0, ring
+    if (modes & GPUQT_MODE_MSD) n += 2 + kRing;     // chi, out1, ringe
     if (modes & GPUQT_MODE_VAC) n += 3;             // a, b, phi_L
     return n;
 }
@@ -190,7 +206,7 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items) {
 // bytes of one stage of a step kernel: the record plus the staged own rows of T_{m-1}, T_{m-2}
 // (and e_{m-1}, e_{m-2} for the (a, e) pair)
 int mode_stage_bytes_for(const gpuqt_handle* h, int mode) {
-    const int streams = (mode == kModeEvolveMsd) ? 4 : 2;
+    const int streams = ((mode == kModeEvolveMsd) ? 4 : 2) / (GPUQT_PREV_DIRECT ? 2 : 1);
     return h->rec_bytes + streams * 32 * h->B * (int)sizeof(double2);
 }
 
@@ -210,6 +226,46 @@ cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
             if (e != cudaSuccess) return e;
         }
         h->grid[mode] = grid_for(h, fn, h->mode_smem[mode], (h->mat.n_slices + h->run - 1) / h->run);
+    }
+    a.sched = nullptr;
+    a.n_items = 0;
+    a.run_done = nullptr;
+    a.dep_ptr = nullptr;
+    a.dep_list = nullptr;
+    if (a.n_steps == 2) {
+        const int reverse = h->alternate ? (h->sweep & 1) : 0;
+        const gpuqt_handle::DevSchedule* ds = nullptr;
+        for (const auto& d : h->schedules)
+            if (d.G == h->grid[mode] && d.reverse == reverse) ds = &d;
+        if (!ds) {
+            FusedSchedule fs;
+            build_fused_schedule((int)h->mat.n_slices, h->run, h->grid[mode], reverse, std::max(1, h->lag * h->grid[mode] / 2),
+                                 kNoRun, h->nbr_ptr, h->nbr_slices, fs);
+            gpuqt_handle::DevSchedule d{};
+            d.G = h->grid[mode];
+            d.reverse = reverse;
+            d.n_items = (int)(fs.items.size() / 2);
+            d.n_runs = (int)fs.dep_ptr.size() - 1;
+            auto up = [&](void** dst, const std::vector<int>& v) {
+                cudaError_t e = cudaMalloc(dst, std::max<size_t>(v.size(), 1) * sizeof(int));
+                if (e == cudaSuccess && !v.empty()) e = cudaMemcpy(*dst, v.data(), v.size() * sizeof(int), cudaMemcpyHostToDevice);
+                return e;
+            };
+            cudaError_t e = up((void**)&d.items, fs.items);
+            if (e == cudaSuccess) e = up((void**)&d.dep_ptr, fs.dep_ptr);
+            if (e == cudaSuccess) e = up((void**)&d.dep_list, fs.dep_list);
+            if (e == cudaSuccess) e = cudaMalloc((void**)&d.run_done, (size_t)d.n_runs * sizeof(unsigned int));
+            if (e != cudaSuccess) return e;
+            h->schedules.push_back(d);
+            ds = &h->schedules.back();
+        }
+        cudaError_t e = cudaMemsetAsync(ds->run_done, 0, (size_t)ds->n_runs * sizeof(unsigned int), h->stream);
+        if (e != cudaSuccess) return e;
+        a.sched = ds->items;
+        a.n_items = ds->n_items;
+        a.run_done = ds->run_done;
+        a.dep_ptr = ds->dep_ptr;
+        a.dep_list = ds->dep_list;
     }
     a.stages = h->mode_stages[mode];
     a.stage_bytes = h->mode_stage_bytes[mode];
@@ -238,6 +294,19 @@ cudaError_t launch_dot(gpuqt_handle* h, const double2* l, const double2* r, doub
     return cudaLaunchKernel(fn, dim3(h->grid_aux), dim3(kThreads), args, 0, h->stream);
 }
 
+cudaError_t ensure_scratch(gpuqt_handle* h, size_t bytes) {
+    if (bytes <= h->scratch_bytes) return cudaSuccess;
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return e;
+    if (h->scratch) cudaFree(h->scratch);
+    h->scratch = nullptr;
+    h->scratch_bytes = 0;
+    const size_t want = bytes + bytes / 2;
+    e = cudaMalloc((void**)&h->scratch, want);
+    if (e == cudaSuccess) h->scratch_bytes = want;
+    return e;
+}
+
 // ---------------------------------------------------------------- timing statistics
 cudaEvent_t get_event(gpuqt_handle* h) {
     if (!h->free_events.empty()) {
@@ -255,11 +324,15 @@ struct StatScope {
     StatScope(gpuqt_handle* hh, int cls) : h(hh) {
         p.cls = cls;
         p.launches = 0;
+        p.steps = 0;
         p.start = get_event(h);
         p.stop = get_event(h);
         cudaEventRecord(p.start, h->stream);
     }
-    void count(int64_t n = 1) { p.launches += n; }
+    void count(int64_t n = 1, int64_t steps = 1) {
+        p.launches += n;
+        p.steps += steps;
+    }
     ~StatScope() {
         cudaEventRecord(p.stop, h->stream);
         h->pending.push_back(p);
@@ -271,6 +344,7 @@ void flush_stats(gpuqt_handle* h) {
         if (cudaEventSynchronize(p.stop) == cudaSuccess && cudaEventElapsedTime(&ms, p.start, p.stop) == cudaSuccess) {
             h->stat_ms[p.cls] += ms;
             h->stat_launches[p.cls] += p.launches;
+            h->stat_steps[p.cls] += p.steps;
         }
         h->free_events.push_back(p.start);
         h->free_events.push_back(p.stop);
@@ -279,57 +353,70 @@ void flush_stats(gpuqt_handle* h) {
 }
 
 // ---------------------------------------------------------------- building blocks
-// out_vec <- sum_{m<order} c_m T_m(H~) in_vec   (Eq. 17, 21, 23), one fused kernel per term.
-// `in` is left untouched; `out` must differ from in and from the ring buffers.
-int evolve_one(gpuqt_handle* h, const double2* in, double2* out, const std::vector<double>& cr,
-               const std::vector<double>& ci, int order) {
-    if (order == 1) {   // U ~ c_0: out = c_0 in  -> run the first-term kernel with c_1 = 0
-        StepArgs a{};
-        a.in = in; a.out = h->ring[0]; a.acc = out;
-        a.c0r = cr[0]; a.c0i = ci[0]; a.cr = 0; a.ci = 0; a.first = 1; a.store = 0;
-        StatScope s(h, GPUQT_KERNEL_EVOLVE);
-        CU(launch_step(h, kModeEvolve, a));
-        s.count();
-        return GPUQT_OK;
-    }
-    StatScope s(h, GPUQT_KERNEL_EVOLVE);
-    const double2* tm1 = in;        // T_{m-1}
-    const double2* tm2 = nullptr;   // T_{m-2}
-    for (int m = 1; m < order; ++m) {
-        StepArgs a{};
-        double2* tnew = h->ring[(m - 1) % 3];
-        a.in = tm1; a.prev = tm2; a.out = tnew; a.acc = out;
-        a.cr = cr[m]; a.ci = ci[m]; a.c0r = cr[0]; a.c0i = ci[0];
-        a.first = (m == 1); a.store = (m + 1 < order);
-        CU(launch_step(h, kModeEvolve, a));
-        s.count();
-        tm2 = tm1;
-        tm1 = tnew;
+// Driver of one three-term recurrence: terms m = 1 .. terms-1, T_m from T_{m-1}, T_{m-2} (and the
+// e-chain of the MSD pair).  Term 1 is a single-step launch (no T_{-1}, factor 1); after it two
+// consecutive terms share one launch when fusing is on (kernels.cuh, cheb_step_kernel).
+// fill(io, m) sets the per-term fields (coefficient, dot destination, store flag).
+template <class Fill>
+int run_recurrence(gpuqt_handle* h, int mode, int cls, int terms, const double2* t0, const double2* e0,
+                   const StepArgs& base, Fill fill) {
+    StatScope s(h, cls);
+    const double2 *tm1 = t0, *tm2 = nullptr, *em1 = e0, *em2 = nullptr;
+    int slot = 0, m = 1;
+    while (m < terms) {
+        StepArgs a = base;
+        a.first = (m == 1);
+        a.n_steps = (h->fuse && m >= 2 && m + 1 < terms) ? 2 : 1;
+        for (int k = 0; k < a.n_steps; ++k) {
+            StepIO& io = a.io[k];
+            double2* tnew = h->ring[slot];
+            io.in = tm1; io.prev = tm2; io.out = tnew;
+            tm2 = tm1; tm1 = tnew;
+            if (e0) {
+                double2* enew = h->ringe[slot];
+                io.in_e = em1; io.prev_e = em2; io.out_e = enew;
+                em2 = em1; em1 = enew;
+            }
+            slot = (slot + 1) % kRing;
+            io.store = 1;
+            fill(io, m + k);
+        }
+        CU(launch_step(h, mode, a));
+        s.count(1, a.n_steps);
+        m += a.n_steps;
     }
     return GPUQT_OK;
+}
+
+// out_vec <- sum_{m<order} c_m T_m(H~) in_vec   (Eq. 17, 21, 23), recurrence and accumulation in
+// one kernel.  `in` is left untouched; `out` must differ from in and from the ring buffers.
+int evolve_one(gpuqt_handle* h, const double2* in, double2* out, const std::vector<double>& cr,
+               const std::vector<double>& ci, int order) {
+    StepArgs base{};
+    base.acc = out;
+    base.c0r = cr[0]; base.c0i = ci[0];
+    const int terms = order < 2 ? 2 : order;   // order 1: U ~ c_0 -> the first-term kernel with c_1 = 0
+    return run_recurrence(h, kModeEvolve, GPUQT_KERNEL_EVOLVE, terms, in, nullptr, base, [&](StepIO& io, int m) {
+        io.cr = order < 2 ? 0.0 : cr[(size_t)m];
+        io.ci = order < 2 ? 0.0 : ci[(size_t)m];
+        io.store = (m + 1 < terms);
+    });
 }
 
 // (psi, chi) <- (U psi, U chi + [X,U] psi) with the fused e-recursion
 //   a_m = T_m psi, e_m = T_m chi + [X,T_m] psi:  e_m = 2 H~ e_{m-1} - e_{m-2} + 2 [X,H~] a_{m-1}
 int evolve_msd_pair(gpuqt_handle* h, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
-    StatScope s(h, GPUQT_KERNEL_EVOLVE_MSD);
-    const double2 *am1 = h->psi, *am2 = nullptr, *em1 = h->chi, *em2 = nullptr;
+    StepArgs base{};
+    base.acc = h->out0; base.acc_e = h->out1;
+    base.c0r = cr[0]; base.c0i = ci[0];
     const int terms = order < 2 ? 2 : order;
-    for (int m = 1; m < terms; ++m) {
-        StepArgs a{};
-        double2* anew = h->ring[(m - 1) % 3];
-        double2* enew = h->ringe[(m - 1) % 3];
-        a.in = am1; a.prev = am2; a.out = anew;
-        a.in_e = em1; a.prev_e = em2; a.out_e = enew;
-        a.acc = h->out0; a.acc_e = h->out1;
-        if (order < 2) { a.cr = 0; a.ci = 0; } else { a.cr = cr[m]; a.ci = ci[m]; }
-        a.c0r = cr[0]; a.c0i = ci[0];
-        a.first = (m == 1); a.store = (m + 1 < terms);
-        CU(launch_step(h, kModeEvolveMsd, a));
-        s.count();
-        am2 = am1; am1 = anew;
-        em2 = em1; em1 = enew;
-    }
+    int rc = run_recurrence(h, kModeEvolveMsd, GPUQT_KERNEL_EVOLVE_MSD, terms, h->psi, h->chi, base,
+                            [&](StepIO& io, int m) {
+                                io.cr = order < 2 ? 0.0 : cr[(size_t)m];
+                                io.ci = order < 2 ? 0.0 : ci[(size_t)m];
+                                io.store = (m + 1 < terms);
+                            });
+    if (rc) return rc;
     std::swap(h->psi, h->out0);
     std::swap(h->chi, h->out1);
     return GPUQT_OK;
@@ -338,20 +425,13 @@ int evolve_msd_pair(gpuqt_handle* h, const std::vector<double>& cr, const std::v
 // moments with the doubling identity: C_n = <v|T_n|v>, n < n_moments  -> h->moments [B][n]
 int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
     const int n_steps = n_moments / 2;   // step j gives C_{2j+1}, C_{2j+2}
-    {
-        StatScope s(h, GPUQT_KERNEL_KPM_DOUBLING);
-        const double2 *tm1 = v, *tm2 = nullptr;
-        for (int j = 0; j < n_steps; ++j) {
-            StepArgs a{};
-            double2* tnew = h->ring[j % 3];
-            a.in = tm1; a.prev = tm2; a.out = tnew;
-            a.first = (j == 0); a.store = (j + 1 < n_steps);
-            a.result = h->dots + (size_t)j * 3 * h->B;
-            CU(launch_step(h, kModeDoubling, a));
-            s.count();
-            tm2 = tm1; tm1 = tnew;
-        }
-    }
+    StepArgs base{};
+    int rc = run_recurrence(h, kModeDoubling, GPUQT_KERNEL_KPM_DOUBLING, n_steps + 1, v, nullptr, base,
+                            [&](StepIO& io, int m) {
+                                io.store = (m < n_steps);
+                                io.result = h->dots + (size_t)(m - 1) * 3 * h->B;
+                            });
+    if (rc) return rc;
     const int total = h->B * n_moments;
     finalize_doubling<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, n_steps, h->dots, h->moments);
     CU(cudaGetLastError());
@@ -361,20 +441,13 @@ int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
 // C_n = <l|T_n|r>  -> h->moments [B][n] (real part)
 int moments_left(gpuqt_handle* h, const double2* l, const double2* r, int n_moments) {
     CU(launch_dot(h, l, r, h->dots));
-    {
-        StatScope s(h, GPUQT_KERNEL_KPM_LEFT);
-        const double2 *tm1 = r, *tm2 = nullptr;
-        for (int n = 1; n < n_moments; ++n) {
-            StepArgs a{};
-            double2* tnew = h->ring[(n - 1) % 3];
-            a.in = tm1; a.prev = tm2; a.out = tnew; a.phiL = l;
-            a.first = (n == 1); a.store = (n + 1 < n_moments);
-            a.result = h->dots + (size_t)n * 2 * h->B;
-            CU(launch_step(h, kModeLeft, a));
-            s.count();
-            tm2 = tm1; tm1 = tnew;
-        }
-    }
+    StepArgs base{};
+    base.phiL = l;
+    int rc = run_recurrence(h, kModeLeft, GPUQT_KERNEL_KPM_LEFT, n_moments, r, nullptr, base, [&](StepIO& io, int n) {
+        io.store = (n + 1 < n_moments);
+        io.result = h->dots + (size_t)n * 2 * h->B;
+    });
+    if (rc) return rc;
     const int total = h->B * n_moments;
     finalize_left<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, h->dots, h->moments);
     CU(cudaGetLastError());
@@ -425,6 +498,27 @@ int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int
                    const double* x, double box_length, double energy_scale) {
     std::string msg;
     return validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
+}
+
+int gpuqt_fused_schedule(int32_t n_slices, int32_t run, int32_t grid, int reverse, int32_t slack,
+                         const int32_t* nbr_ptr, const int32_t* nbr_slices, int32_t* items, int32_t capacity,
+                         int32_t* n_items, int32_t* dep_ptr, int32_t* dep_list, int32_t dep_capacity, int32_t* n_dep) {
+    if (n_slices < 1 || run < 1 || grid < 1 || slack < 1 || !nbr_ptr || !nbr_slices || !n_items || !n_dep) return GPUQT_ERR_ARG;
+    std::vector<int> np(nbr_ptr, nbr_ptr + n_slices + 1), ns(nbr_slices, nbr_slices + nbr_ptr[n_slices]);
+    FusedSchedule fs;
+    build_fused_schedule(n_slices, run, grid, reverse, slack, kNoRun, np, ns, fs);
+    *n_items = (int32_t)(fs.items.size() / 2);
+    *n_dep = (int32_t)fs.dep_list.size();
+    if (items) {
+        if (*n_items > capacity) return GPUQT_ERR_NOMEM;
+        for (size_t i = 0; i < fs.items.size(); ++i) items[i] = fs.items[i];
+    }
+    if (dep_ptr && dep_list) {
+        if (*n_dep > dep_capacity) return GPUQT_ERR_NOMEM;
+        for (size_t i = 0; i < fs.dep_ptr.size(); ++i) dep_ptr[i] = fs.dep_ptr[i];
+        for (size_t i = 0; i < fs.dep_list.size(); ++i) dep_list[i] = fs.dep_list[i];
+    }
+    return GPUQT_OK;
 }
 
 int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im) {
@@ -521,6 +615,13 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->max_blocks_per_sm = env_int("GPUQT_BLOCKS_PER_SM", 0);
     h->alternate = env_int("GPUQT_ALTERNATE", 1);
     h->run = std::max(1, env_int("GPUQT_RUN", 16) / kWarps) * kWarps;
+    h->fuse = env_int("GPUQT_FUSE", 0);
+    h->lag = std::max(1, env_int("GPUQT_LAG", 2));
+    h->nbr_ptr.swap(sell.nbr_ptr);
+    h->nbr_slices.swap(sell.nbr_slices);
+    // without locality in the table (a slice gathering from very many others) a second step cannot
+    // trail the first through L2: single-step launches only
+    if (h->nbr_slices.size() > (size_t)24 * (size_t)sell.n_slices) h->fuse = 0;
 
     const size_t vstride = align_up((size_t)(N + 1) * batch * sizeof(double2));
     char* v = base + L.vectors;
@@ -530,10 +631,10 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
         return p;
     };
     h->psi = nextv(); h->out0 = nextv();
-    for (int i = 0; i < 3; ++i) h->ring[i] = nextv();
+    for (int i = 0; i < kRing; ++i) h->ring[i] = nextv();
     if (modes & GPUQT_MODE_MSD) {
         h->chi = nextv(); h->out1 = nextv();
-        for (int i = 0; i < 3; ++i) h->ringe[i] = nextv();
+        for (int i = 0; i < kRing; ++i) h->ringe[i] = nextv();
     }
     if (modes & GPUQT_MODE_VAC) {
         h->va = nextv(); h->vb = nextv(); h->phiL = nextv();
@@ -631,10 +732,9 @@ int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_m
             return fail(h, GPUQT_ERR_ENERGY, "energy point outside (-energy_scale, energy_scale)");
     const size_t bm = (size_t)n_sets * n_moments * sizeof(double), be = (size_t)n_energies * sizeof(double),
                  bo = (size_t)n_sets * n_energies * sizeof(double), bg = (size_t)n_moments * sizeof(double);
-    double* scratch = nullptr;
     const size_t om = 0, oe = align_up(bm), oo = oe + align_up(be), og = oo + align_up(bo), tot = og + align_up(bg);
-    CU(cudaMallocAsync((void**)&scratch, tot, h->stream));
-    char* s = (char*)scratch;
+    CU(ensure_scratch(h, tot));
+    char* s = h->scratch;
     cudaError_t e = cudaMemcpyAsync(s + om, moments_host, bm, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(s + oe, energies_host, be, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) {
@@ -646,7 +746,6 @@ int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_m
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, s + oo, bo, cudaMemcpyDeviceToHost, h->stream);
-    cudaFreeAsync(scratch, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "kpm_transform");
     flush_stats(h);
@@ -672,9 +771,9 @@ int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, doubl
     const size_t nk = (size_t)h->N * h->K;
     // scratch: the ring buffers are free between calls (3 * N*B*16 bytes >= N*K*28 is not
     // guaranteed), so use a stream-ordered allocation
-    char* scratch = nullptr;
     const size_t oc = 0, orr = align_up(nk * 4), oi = orr + align_up(nk * 8), od = oi + align_up(nk * 8), tot = od + align_up(nk * 8);
-    CU(cudaMallocAsync((void**)&scratch, tot, h->stream));
+    CU(ensure_scratch(h, tot));
+    char* scratch = h->scratch;
     decode_table<<<(int)((nk + 255) / 256), 256, 0, h->stream>>>(h->mat, (int32_t*)(scratch + oc), (double*)(scratch + orr),
                                                                  (double*)(scratch + oi), (double*)(scratch + od));
     cudaError_t e = cudaGetLastError();
@@ -682,7 +781,6 @@ int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, doubl
     if (e == cudaSuccess && re) e = cudaMemcpyAsync(re, scratch + orr, nk * 8, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && im) e = cudaMemcpyAsync(im, scratch + oi, nk * 8, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && dx) e = cudaMemcpyAsync(dx, scratch + od, nk * 8, cudaMemcpyDeviceToHost, h->stream);
-    cudaFreeAsync(scratch, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "get_table");
     return GPUQT_OK;
@@ -696,12 +794,20 @@ int gpuqt_kernel_stats(gpuqt_handle* h, int kernel_class, double* ms, int64_t* l
     return GPUQT_OK;
 }
 
+int gpuqt_kernel_steps(gpuqt_handle* h, int kernel_class, int64_t* steps) {
+    if (!h || !steps || kernel_class < 0 || kernel_class >= GPUQT_KERNEL_CLASSES) return GPUQT_ERR_ARG;
+    flush_stats(h);
+    *steps = h->stat_steps[kernel_class];
+    return GPUQT_OK;
+}
+
 int gpuqt_reset_stats(gpuqt_handle* h) {
     if (!h) return GPUQT_ERR_ARG;
     flush_stats(h);
     for (int i = 0; i < GPUQT_KERNEL_CLASSES; ++i) {
         h->stat_ms[i] = 0;
         h->stat_launches[i] = 0;
+        h->stat_steps[i] = 0;
     }
     return GPUQT_OK;
 }
@@ -713,6 +819,13 @@ void gpuqt_destroy(gpuqt_handle* h) {
     cudaStreamSynchronize(h->stream);
     flush_stats(h);
     for (auto e : h->free_events) cudaEventDestroy(e);
+    if (h->scratch) cudaFree(h->scratch);
+    for (auto& d : h->schedules) {
+        cudaFree(d.items);
+        cudaFree(d.dep_ptr);
+        cudaFree(d.dep_list);
+        cudaFree(d.run_done);
+    }
     delete h;
 }
 

@@ -103,6 +103,7 @@ struct SellHost {
     int uniform = 1;                    // every record has width K_max
     int nd = 1;                         // doubles per entry: 0 constant hopping, 1 real, 2 complex
     double hop_const = 0.0;
+    std::vector<int> nbr_ptr, nbr_slices;   // CSR over slices: the slices a slice gathers from (sorted, itself included)
     std::vector<long long> slice_off;   // [n_slices + 1] byte offsets of the records
     std::vector<unsigned char> rec;
 };
@@ -155,6 +156,19 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
         s.slice_off[(size_t)sl + 1] = s.slice_off[(size_t)sl] + host_record_bytes(width[(size_t)sl], cplx);
     }
     s.rec.assign((size_t)s.slice_off[(size_t)s.n_slices], 0);
+    s.nbr_ptr.assign((size_t)s.n_slices + 1, 0);
+    s.nbr_slices.clear();
+    std::vector<int> tmp;
+    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+        tmp.clear();
+        tmp.push_back((int)sl);
+        for (int64_t m = sl * 32; m < std::min<int64_t>(N, sl * 32 + 32); ++m)
+            for (int32_t k = 0; k < cnt[m]; ++k) tmp.push_back(idx[(size_t)m * K + k] >> 5);
+        std::sort(tmp.begin(), tmp.end());
+        tmp.erase(std::unique(tmp.begin(), tmp.end()), tmp.end());
+        s.nbr_slices.insert(s.nbr_slices.end(), tmp.begin(), tmp.end());
+        s.nbr_ptr[(size_t)sl + 1] = (int)s.nbr_slices.size();
+    }
     for (int64_t sl = 0; sl < s.n_slices; ++sl) {
         const int w = width[(size_t)sl];
         unsigned char* base = s.rec.data() + s.slice_off[(size_t)sl];
@@ -178,6 +192,77 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
                 }
             }
         }
+    }
+}
+
+// Work list of a launch that performs two consecutive recurrence steps (kernels.cuh,
+// cheb_step_kernel).  Items are (step, run); CTA c of G takes items c, c + G, ...  First-step items
+// come in sweep order.  The second step of run R gathers T_m from a few runs dep(R) (from the
+// table's sparsity); it is emitted once the first-step item of the farthest of them lies at least
+// `slack` items back, so that when a CTA reaches it those runs are normally finished and their
+// T_m, T_{m-1} and matrix records are still in L2.  Steps alternate along the list with the
+// parity flipped every 4 G items, so every CTA (and SM) gets both kinds of work, four items of a
+// kind in a row.  Runs whose
+// dependency wraps around the end of the table (periodic boundaries) follow after the first
+// sweep; no-op items pad while nothing is eligible.
+//   items[2t] = run | step << 30 (run = no_run: no-op), items[2t+1] = -1 (reserved)
+//   dep_ptr / dep_list: CSR over runs of the first-step runs a second-step item waits for
+struct FusedSchedule {
+    std::vector<int> items;
+    std::vector<int> dep_ptr, dep_list;
+};
+inline void build_fused_schedule(int n_slices, int run, int G, int reverse, int slack, int no_run,
+                                 const std::vector<int>& nbr_ptr, const std::vector<int>& nbr_slices,
+                                 FusedSchedule& out) {
+    const int n_runs = (n_slices + run - 1) / run;
+    std::vector<int> far((size_t)n_runs, 0), tmp;
+    out.dep_ptr.assign((size_t)n_runs + 1, 0);
+    out.dep_list.clear();
+    for (int R = 0; R < n_runs; ++R) {
+        tmp.clear();
+        for (int vs = R * run; vs < std::min(n_slices, (R + 1) * run); ++vs) {
+            const int s = reverse ? n_slices - 1 - vs : vs;
+            for (int i = nbr_ptr[(size_t)s]; i < nbr_ptr[(size_t)s + 1]; ++i) {
+                const int ns = nbr_slices[(size_t)i];
+                tmp.push_back((reverse ? n_slices - 1 - ns : ns) / run);
+            }
+        }
+        std::sort(tmp.begin(), tmp.end());
+        tmp.erase(std::unique(tmp.begin(), tmp.end()), tmp.end());
+        far[(size_t)R] = tmp.back();
+        out.dep_list.insert(out.dep_list.end(), tmp.begin(), tmp.end());
+        out.dep_ptr[(size_t)R + 1] = (int)out.dep_list.size();
+    }
+    std::vector<int> order((size_t)n_runs);
+    for (int R = 0; R < n_runs; ++R) order[(size_t)R] = R;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return far[(size_t)a] < far[(size_t)b]; });
+    std::vector<int> pos1((size_t)n_runs, -1);
+    out.items.clear();
+    auto n_items = [&]() { return (int)(out.items.size() / 2); };
+    auto emit = [&](int x) {
+        out.items.push_back(x);
+        out.items.push_back(-1);
+    };
+    int i2 = 0, R1 = 0;
+    auto try_second = [&]() {
+        if (i2 >= n_runs) return false;
+        const int R2 = order[(size_t)i2];
+        const int d = pos1[(size_t)far[(size_t)R2]];
+        if (d < 0 || d + slack > n_items()) return false;
+        emit(R2 | (1 << 30));
+        ++i2;
+        return true;
+    };
+    while (R1 < n_runs || i2 < n_runs) {
+        const int t = n_items();
+        const bool want_second = (((t % G) + (t / (4 * G))) & 1) != 0;   // a CTA switches step every 4 items
+        if (want_second && try_second()) continue;
+        if (R1 < n_runs) {
+            pos1[(size_t)R1] = t;
+            emit(R1++);
+            continue;
+        }
+        if (!try_second()) emit(no_run);
     }
 }
 

@@ -40,6 +40,9 @@
 #endif
 
 // L2 policy experiments
+#ifndef GPUQT_PREV_DIRECT     // experiment: 1 = T_{m-2} own rows by a streaming 256-bit global load instead of TMA staging
+#define GPUQT_PREV_DIRECT 0
+#endif
 #ifndef GPUQT_GATHER_POLICY   // 0: plain ld.global, 1: L2::evict_last
 #define GPUQT_GATHER_POLICY 1
 #endif
@@ -89,29 +92,46 @@ enum Mode : int {
     kModeEvolveMsd = 3,  // (a, e) pair with the [X,H~] weights in the same walk     (Eq. 18, 22)
 };
 
+// Operands of one recurrence step.  A launch performs one step, or two consecutive steps fused
+// through L2 (see cheb_step_kernel): io[0] is T_m = 2 H~ T_{m-1} - T_{m-2}, io[1] is T_{m+1}.
+struct StepIO {
+    const double2* in;       // T_{m-1}: gathered and own row
+    const double2* prev;     // T_{m-2}: own row (unused when first)
+    double2* out;            // T_m (unused when !store)
+    const double2* in_e;     // MSD pair: e_{m-1}
+    const double2* prev_e;   //           e_{m-2}
+    double2* out_e;          //           e_m
+    double cr, ci;           // c_m
+    double* result;          // [Q][B] reduced dots of this step
+    int store;               // write T_m (0 on the last term of an evolve)
+    int pad_;
+};
+
 struct StepArgs {
-    const double2* __restrict__ in;      // T_{m-1}: gathered and own row
-    const double2* __restrict__ prev;    // T_{m-2}: own row (unused when first)
-    double2* __restrict__ out;           // T_m (unused when !store)
-    const double2* __restrict__ in_e;    // MSD pair: e_{m-1}
-    const double2* __restrict__ prev_e;  //           e_{m-2}
-    double2* __restrict__ out_e;         //           e_m
+    StepIO io[2];
     double2* __restrict__ acc;           // evolve: sum_m c_m T_m
     double2* __restrict__ acc_e;         // evolve MSD: sum_m c_m e_m
     const double2* __restrict__ phiL;    // kModeLeft
-    double cr, ci;                       // c_m
     double c0r, c0i;                     // c_0, used when first (acc = c_0 T_0 + c_1 T_1)
-    int first;                           // T_1 = H~ T_0 (no factor 2, no prev)
-    int store;                           // write T_m (0 on the last term of an evolve)
+    int first;                           // T_1 = H~ T_0 (no factor 2, no prev); single-step launches only
+    int n_steps;                         // 1, or 2 (fused pair, scheduled by `sched`)
     int reverse;                         // sweep the slices from the top (L2 reuse between launches)
     int run;                             // consecutive slices one CTA walks before jumping (multiple of kWarps)
     int stages;                          // shared-memory stages per warp (<= kMaxStages)
     int stage_bytes;                     // bytes of one stage: record + staged vector rows
     int rec_bytes;                       // bytes reserved for the record inside a stage
-    double* partials;                    // [grid][Q*B]
+    double* partials;                    // [grid][n_steps*Q*B]
     unsigned int* ticket;
-    double* result;                      // [Q][B] reduced dots of this launch
+    // fused pair: item t (taken by CTA t % G) = {run | step << 30 (run = kNoRun: nothing to do), -1};
+    // a second-step item of run R waits until run_done[r] == kWarps for r in dep_list[dep_ptr[R] ..
+    // dep_ptr[R+1]) (the first-step runs it gathers T_m from)
+    const int2* sched;
+    int n_items;
+    unsigned int* run_done;              // [runs] warps that have finished the first step of the run
+    const int* dep_ptr;
+    const int* dep_list;
 };
+constexpr int kNoRun = (1 << 30) - 1;
 
 // ------------------------------------------------------------------ PTX helpers (TMA / mbarrier)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -190,6 +210,9 @@ __device__ __forceinline__ void st_vec(double2* p, double2 v) {
 #else
     *p = v;
 #endif
+}
+__device__ __forceinline__ void red_release_gpu_inc(unsigned int* p) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
 }
 __device__ __forceinline__ double2 ldcs2(const double2* p) { return __ldcs(p); }
 
@@ -413,9 +436,10 @@ __device__ __forceinline__ void cv_add(CV<V>& acc, const CV<V>& v) {
 // (their staged self / prev are replaced by 0 and their entries are padding), so the dot products
 // need no guard; only their stores are predicated off.
 template <int B, int KT, int HOP, int MODE>
-__device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, const unsigned char* stage, int w,
+__device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, const StepIO& io, const unsigned char* stage, int w,
                                            int row0, int rows_valid, int j, int lane, double scale,
-                                           double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V]) {
+                                           double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V],
+                                           unsigned int* signal) {
     constexpr int V = LaneShape<B>::V, LPR = LaneShape<B>::LPR, RS = LaneShape<B>::RS;
     constexpr int KU = KT > 0 ? KT : 1;
     constexpr int RB = B * 16;   // bytes of one row of a vector set
@@ -434,8 +458,8 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     // lane-relative bases of the gathers (see cv_gather)
     const uint32_t sl_in = smem_u32(s_in + l * V) - (uint32_t)(row0 * RB);
     const uint32_t sl_in_e = smem_u32(s_in_e + l * V) - (uint32_t)(row0 * RB);
-    const char* gl_in = reinterpret_cast<const char*>(a.in + l * V);
-    const char* gl_in_e = reinterpret_cast<const char*>(a.in_e + l * V);
+    const char* gl_in = reinterpret_cast<const char*>(io.in + l * V);
+    const char* gl_in_e = reinterpret_cast<const char*>(io.in_e + l * V);
 
     const int r = j * RS + rl;
     const bool ok = r < rows_valid;
@@ -451,6 +475,13 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     if (MODE == kModeLeft) other = cv_ld_stream<V>(&a.phiL[vi]);
     double xm = 0.0;
     if (MSD) xm = m.x[row0 + (ok ? r : 0)];
+#if GPUQT_PREV_DIRECT
+    CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
+    if (!a.first) {
+        prev = cv_ld_stream<V>(&io.prev[vi]);
+        if (MSD) prev_e = cv_ld_stream<V>(&io.prev_e[vi]);
+    }
+#endif
 
     const CV<V> self = ok ? cv_lds<V>(s_in + si_) : cv_zero<V>();
     const CV<V> self_e = (MSD && ok) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
@@ -470,6 +501,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
                 xn[k] = m.x[c];
             }
         }
+        if (signal && lane == 0) red_release_gpu_inc(signal);           // see cheb_step_kernel, `pending`
 #pragma unroll
         for (int k = 0; k < KU; ++k) {
             double hr = 1.0, hi = 0.0;                                  // CONST: the factor is applied once below
@@ -486,6 +518,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
             }
         }
     } else {
+        if (signal && lane == 0) red_release_gpu_inc(signal);
         for (int k = 0; k < w; ++k) {
             const int c = s_col[k * 32 + r];
             double hr = 1.0, hi = 0.0;
@@ -503,11 +536,13 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
             }
         }
     }
+#if !GPUQT_PREV_DIRECT
     CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
     if (!a.first && ok) {
         prev = cv_lds<V>(s_prev + si_);
         if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
     }
+#endif
     const double hs = CONST ? scale * m.hop_const : scale;              // scale of the neighbour sums
     const double os = scale * on;                                       // scale of the on-site term
     CV<V> t, te, acc, ae;   // T_m, e_m, and the accumulators
@@ -530,8 +565,8 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
                 acc.re[q] = other.re[q];
                 acc.im[q] = other.im[q];
             }
-            acc.re[q] += a.cr * t.re[q] - a.ci * t.im[q];
-            acc.im[q] += a.cr * t.im[q] + a.ci * t.re[q];
+            acc.re[q] += io.cr * t.re[q] - io.ci * t.im[q];
+            acc.im[q] += io.cr * t.im[q] + io.ci * t.re[q];
             if (MSD) {
                 te.re[q] = fma(hs, sum_e.re[q] + sum_x.re[q], fma(os, self_e.re[q], -prev_e.re[q]));
                 te.im[q] = fma(hs, sum_e.im[q] + sum_x.im[q], fma(os, self_e.im[q], -prev_e.im[q]));
@@ -542,57 +577,138 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
                     ae.re[q] = other_e.re[q];
                     ae.im[q] = other_e.im[q];
                 }
-                ae.re[q] += a.cr * te.re[q] - a.ci * te.im[q];
-                ae.im[q] += a.cr * te.im[q] + a.ci * te.re[q];
+                ae.re[q] += io.cr * te.re[q] - io.ci * te.im[q];
+                ae.im[q] += io.cr * te.im[q] + io.ci * te.re[q];
             }
         }
     }
     if (ok) {
-        if (a.store) cv_st<V>(&a.out[vi], t);
+        if (io.store) cv_st<V>(&io.out[vi], t);
         if (MODE == kModeEvolve || MSD) cv_st<V>(&a.acc[vi], acc);
         if (MSD) {
-            if (a.store) cv_st<V>(&a.out_e[vi], te);
+            if (io.store) cv_st<V>(&io.out_e[vi], te);
             cv_st<V>(&a.acc_e[vi], ae);
         }
     }
 }
 
-// One Chebyshev recurrence step fused with what consumes it.  Persistent CTAs: the slices are cut
-// into runs of a.run consecutive slices; CTA c walks runs c, c + G, c + 2G, ...; inside a run warp w
-// takes slices w, w + kWarps, ...  A CTA therefore streams a contiguous band of rows and the grid
-// sweeps the vector as a tight front, so gathers to nearby rows (the +-x, +-y, +-z neighbours of a
-// lattice) are served by L1/L2.  All loop indices are kept incrementally (no divisions in the loop).
+// Dots of one warp: shuffle over lanes that hold the same vectors, then lanes < LPR add into the
+// warp's shared-memory row dst[q * B + b]; the register accumulators restart from zero.
+template <int B, int Q, int V>
+__device__ __forceinline__ void warp_flush(double (&v)[Q * V], double* dst, int lane) {
+    constexpr int LPR = B / V;
+#pragma unroll
+    for (int q = 0; q < Q * V; ++q) {
+#pragma unroll
+        for (int off = 16; off >= LPR; off >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], off);
+    }
+    if (lane < LPR) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q)
+#pragma unroll
+            for (int j = 0; j < V; ++j) dst[q * B + lane * V + j] += v[q * V + j];
+    }
+#pragma unroll
+    for (int q = 0; q < Q * V; ++q) v[q] = 0.0;
+    __syncwarp();
+}
+
+// Deterministic CTA / grid stage of the reduction: s_part[warp][P] -> per-block partial -> the last
+// block to finish sums the per-block partials in a fixed order (no floating-point atomics).
+// Value p < P0 goes to r0[p], the others to r1[p - P0] (second step of a fused pair).
+__device__ __forceinline__ void block_finish(const double* s_part, int P, int P0, double* partials,
+                                             unsigned int* ticket, double* r0, double* r1) {
+    __shared__ double s_tree[kThreads];
+    __shared__ int s_last;
+    const int tid = threadIdx.x;
+    __syncthreads();
+    if (tid < P) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) s += s_part[w * P + tid];
+        partials[(size_t)blockIdx.x * P + tid] = s;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        unsigned int t = atomicAdd(ticket, 1u);
+        s_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // fixed-shape sum over blocks: thread t handles value (t % P), blocks strand, strand + S, ...
+    const int S = kThreads / P;              // strands per value
+    const int pv = tid % P, strand = tid / P;
+    double s = 0.0;
+    if (strand < S)
+        for (unsigned int g = strand; g < gridDim.x; g += S) s += __ldcg(&partials[(size_t)g * P + pv]);
+    s_tree[tid] = (strand < S) ? s : 0.0;
+    __syncthreads();
+    if (tid < P) {
+        double tot = 0.0;
+        for (int j = 0; j < S; ++j) tot += s_tree[j * P + tid];
+        if (tid < P0) r0[tid] = tot;
+        else r1[tid - P0] = tot;
+    }
+    if (tid == 0) *ticket = 0u;
+}
+
+__device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+
+// One Chebyshev recurrence step fused with what consumes it -- or TWO consecutive steps in one
+// launch (a.n_steps == 2), the second trailing the first by a few sweep rounds so that it finds
+// T_m, T_{m-1} and the matrix records in L2: per pair of steps DRAM then sees T_{m-1}, T_{m-2} read
+// and T_m, T_{m+1} written once each and the matrix once, instead of 6 vector passes and 2 matrix
+// passes.
+//
+// Persistent CTAs.  The slices are cut into runs of a.run consecutive slices; the work list is a
+// sequence of items = (step, run); CTA c takes items c, c + G, c + 2G, ...; inside a run warp w takes
+// slices w, w + kWarps, ...  Single-step launches use the arithmetic list item t = run t.  Fused
+// launches read the list from a.sched (built on the host from the table's sparsity, host_util.h):
+// first-step items in sweep order, each second-step item a fixed slack behind the first-step items
+// it depends on.  A warp that finishes its slices of a first-step item releases run_done[run]; a
+// warp about to start a second-step item checks (all lanes, relaxed loads + one acquire fence) that
+// the runs it gathers from are complete.  A warp only blocks on that when it has nothing in flight,
+// and an item depends only on earlier items of the list, so the scheme cannot deadlock as long as
+// all CTAs are co-resident (the grid is sized by occupancy).
+// All loop indices are kept incrementally (no divisions in the loop).
 template <int B, int KT, int HOP, int MODE>
 __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
     constexpr int Q = ModeTraits<MODE>::Q;
     constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
-    constexpr int RB = B * 16;
+    constexpr int RB = B * 16, QB = Q * B;
     constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
+    constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
     extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ double s_part[DOTS ? kWarps * 2 * QB : 1];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
     const int stages = a.stages;
     const int stage_bytes = a.stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + warp * kMaxStages;
     unsigned char* wstage = smem + 128 * ((kWarps * kMaxStages * 8 + 127) / 128) + (size_t)warp * stages * stage_bytes;
+    const int P = a.n_steps * QB;                 // dot values per block
+    double* my_part = s_part + warp * P;
 
     double red[Q * V];
 #pragma unroll
     for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
+    if (DOTS) {
+        for (int i = lane; i < P; i += 32) my_part[i] = 0.0;
+    }
     const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
 
     const int N = (int)m.N, n_slices = (int)m.n_slices;
-    const int per = a.run / kWarps;
     const int n_runs = (n_slices + a.run - 1) / a.run;
     const int G = gridDim.x;
-    const int my_runs = (int)blockIdx.x < n_runs ? (n_runs - (int)blockIdx.x + G - 1) / G : 0;
-    int n_my = 0;
-    if (my_runs > 0) {
-        const int last = blockIdx.x + (my_runs - 1) * G;
-        const int rem = n_slices - last * a.run;          // slices in my last run (may be partial)
-        const int in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
-        n_my = (my_runs - 1) * per + in_last;
-    }
+    const bool fused = a.sched != nullptr;
+    const int n_total = fused ? a.n_items : n_runs;
     uint64_t policy = 0;
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(&bars[s], 1);
@@ -601,25 +717,51 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     }
     __syncwarp();
 
-    // position of a pipeline cursor: slice (forward order), index inside the run, stage, phase
+    // a pipeline cursor: item (t, run, step, wait, cnt = slices of this warp in the run), slice
+    // index k inside the item, virtual slice s, shared-memory stage and phase
     struct Cursor {
-        int s, k, st;
+        int t, run, step, cnt, k, s, st;
         uint32_t ph;
     };
-    const int jump = G * a.run - (per - 1) * kWarps;     // last slice of a run -> first slice of my next run
-    auto advance = [&](Cursor& c) {
-        if (++c.k == per) {
-            c.k = 0;
-            c.s += jump;
-        } else {
-            c.s += kWarps;
+    auto load_item = [&](Cursor& c) {
+        c.step = 0;
+        c.run = kNoRun;
+        if (c.t < n_total) {
+            if (fused) {
+                const int2 e = a.sched[c.t];
+                c.run = e.x & kNoRun;
+                c.step = (e.x >> 30) & 1;
+            } else {
+                c.run = c.t;
+            }
         }
+        c.cnt = 0;
+        if (c.run != kNoRun) {
+            int left = n_slices - c.run * a.run;
+            left = left < a.run ? left : a.run;
+            c.cnt = warp < left ? (left - warp + kWarps - 1) / kWarps : 0;
+        }
+        c.k = 0;
+        c.s = c.run * a.run + warp;
+    };
+    auto next_stage = [&](Cursor& c) {
         if (++c.st == stages) {
             c.st = 0;
             c.ph ^= 1u;
         }
     };
+    auto deps_done = [&](int run) {   // whole warp: have all first-step runs this run gathers from finished?
+        const int b = a.dep_ptr[run], e = a.dep_ptr[run + 1];
+        bool ok = true;
+#pragma unroll 1
+        for (int i0 = b; i0 < e; i0 += 32) {      // every lane acquires (lanes past the end re-read the last entry)
+            const int i = i0 + lane < e ? i0 + lane : e - 1;
+            ok = ok && (ld_acquire_gpu(a.run_done + a.dep_list[i]) >= (unsigned int)kWarps);
+        }
+        return __all_sync(0xffffffffu, ok) != 0;
+    };
     auto issue = [&](const Cursor& c) {   // lane 0 only: every HBM stream of the slice -> one stage, one mbarrier
+        const StepIO& io = a.io[c.step];
         const int s = a.reverse ? n_slices - 1 - c.s : c.s;
         long long off;
         uint32_t bytes;
@@ -635,34 +777,73 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
         // constant-hopping padding entries point at it)
         const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-        const uint32_t total = bytes + vbytes_in * kPair + (a.first ? 0u : vbytes * kPair);
+        const uint32_t total = bytes + vbytes_in * kPair + ((a.first || GPUQT_PREV_DIRECT) ? 0u : vbytes * kPair);
         unsigned char* dst = wstage + c.st * stage_bytes;
         unsigned char* vdst = dst + a.rec_bytes;
         const size_t voff = (size_t)s * 32 * B;
         mbar_expect_tx(&bars[c.st], total);
-        bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
-        bulk_g2s_nohint(vdst, a.in + voff, vbytes_in, &bars[c.st]);
-        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, a.in_e + voff, vbytes_in, &bars[c.st]);
-        if (!a.first) {
-            bulk_g2s(vdst + kPair * 512 * B, a.prev + voff, vbytes, &bars[c.st], policy);
-            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, a.prev_e + voff, vbytes, &bars[c.st], policy);
+        // the first step of a fused pair leaves the record in L2 for the second one
+        if (fused && c.step == 0) bulk_g2s_nohint(dst, m.rec + off, bytes, &bars[c.st]);
+        else bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
+        bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[c.st]);
+        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &bars[c.st]);
+        if (!a.first && !GPUQT_PREV_DIRECT) {
+            bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &bars[c.st], policy);
+            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &bars[c.st], policy);
         }
     };
 
-    Cursor prod{(int)blockIdx.x * a.run + warp, 0, 0, 0u}, cons = prod;
-    int issued = 0;
-    if (lane == 0) {
-        for (; issued < stages - 1 && issued < n_my; ++issued) {
-            issue(prod);
-            advance(prod);
-        }
+    // Both cursors are advanced by all lanes (warp-uniform control flow); only the TMA issue itself
+    // is lane 0's.  Items in which this warp has no slice are skipped (first-step ones are signalled).
+    Cursor prod{}, cons{};
+    prod.t = blockIdx.x;
+    load_item(prod);
+    while (prod.cnt == 0 && prod.t < n_total) {
+        prod.t += G;
+        load_item(prod);
     }
-    for (int i = 0; i < n_my; ++i) {
-        // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
-        if (lane == 0 && issued < n_my) {
-            issue(prod);
-            advance(prod);
-            ++issued;
+    cons.t = blockIdx.x;
+    load_item(cons);
+    while (cons.cnt == 0 && cons.t < n_total) {
+        if (fused && cons.step == 0 && cons.run != kNoRun && lane == 0) red_release_gpu_inc(a.run_done + cons.run);
+        cons.t += G;
+        load_item(cons);
+    }
+    int inflight = 0;          // slices issued and not yet consumed
+    bool dep_ok = false;       // the producer's item has passed its dependency check
+    int red_step = cons.step;  // step whose dots the register accumulators hold
+    // A finished first-step item is published (release on run_done) one slice later, from inside the
+    // next slice's walk right after its gathers have been issued: the fence then overlaps with the
+    // gather latency instead of stalling the warp on the write acknowledgements.
+    unsigned int* pending = nullptr;
+
+    while (cons.t < n_total) {
+        while (prod.t < n_total && inflight < stages) {
+            if (fused && prod.step == 1 && !dep_ok) {
+                if (!deps_done(prod.run)) {
+                    if (inflight > 0) break;                     // keep consuming; retry later
+                    if (pending && lane == 0) red_release_gpu_inc(pending);   // nothing of mine may stay unpublished
+                    pending = nullptr;
+                    do __nanosleep(200);
+                    while (!deps_done(prod.run));
+                }
+                // The rows were stored through the generic proxy by other SMs, fenced and released at
+                // gpu scope (they are in L2), and acquired above; the TMA reads that follow are issued
+                // behind that acquire by control dependency and go to L2.  (A reader-side
+                // fence.proxy.async compiles to a full MEMBAR.GPU per item and is not needed here.)
+                dep_ok = true;
+            }
+            if (lane == 0) issue(prod);
+            ++inflight;
+            next_stage(prod);
+            prod.s += kWarps;
+            if (++prod.k == prod.cnt) {
+                dep_ok = false;
+                do {
+                    prod.t += G;
+                    load_item(prod);
+                } while (prod.cnt == 0 && prod.t < n_total);
+            }
         }
         mbar_wait(&bars[cons.st], cons.ph);
         const unsigned char* stage = wstage + cons.st * stage_bytes;
@@ -671,13 +852,36 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         if (KT == 0) w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
         const int row0 = slice * 32;
         const int rows_valid = N - row0;          // >= 32 except in the last slice
+        const StepIO& io = a.io[cons.step];
 #pragma unroll 1
-        for (int j = 0; j < ROUNDS; ++j) walk_round<B, KT, HOP, MODE>(m, a, stage, w, row0, rows_valid, j, lane, scale, red);
-        advance(cons);
+        for (int j = 0; j < ROUNDS; ++j) {
+            walk_round<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, scale, red, pending);
+            pending = nullptr;
+        }
         __syncwarp();
+        --inflight;
+        next_stage(cons);
+        cons.s += kWarps;
+        if (++cons.k == cons.cnt) {
+            // item finished: publish the T_m rows of a first-step item, move to my next item
+            if (fused && cons.step == 0) pending = a.run_done + cons.run;
+            do {
+                cons.t += G;
+                load_item(cons);
+                if (fused && cons.cnt == 0 && cons.step == 0 && cons.run != kNoRun && lane == 0)
+                    red_release_gpu_inc(a.run_done + cons.run);
+            } while (cons.cnt == 0 && cons.t < n_total);
+            if (DOTS && cons.t < n_total && cons.step != red_step) {
+                warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
+                red_step = cons.step;
+            }
+        }
     }
-    if (MODE == kModeDoubling || MODE == kModeLeft)
-        block_reduce_and_finish<B, Q, V>(red, a.partials, a.ticket, a.result);
+    if (pending && lane == 0) red_release_gpu_inc(pending);
+    if (DOTS) {
+        warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
+        block_finish(s_part, P, QB, a.partials, a.ticket, a.io[0].result, a.io[1].result);
+    }
 }
 
 // Address of entry (row, k) pieces inside the packed records (plain global reads; used by the

@@ -273,3 +273,39 @@ def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod, monkeypatch)
         g.evolve(0.8, 45)
         assert vec_err(g.get_state(gq.STATE_CHI), ref_chi) <= TOL
         g.close()
+
+
+@pytest.mark.parametrize("env", [{"GPUQT_FUSE": "0"}, {"GPUQT_FUSE": "1", "GPUQT_RUN": "8", "GPUQT_LAG": "1"},
+                                 {"GPUQT_FUSE": "1", "GPUQT_BLOCKS_PER_SM": "1", "GPUQT_STAGES": "4"},
+                                 {"GPUQT_FUSE": "1", "GPUQT_ALTERNATE": "0", "GPUQT_RUN": "32", "GPUQT_LAG": "3"}],
+                         ids=["unfused", "fused_run8_lag1", "fused_1cta_4stages", "fused_noalt_run32"])
+def test_two_steps_per_launch(gq, oracle_mod, monkeypatch, env):
+    """Launches that perform two recurrence steps (second step trailing the first through L2, ordered
+    by the round counters) against single-step launches and the oracle, on lattices large enough
+    for many runs per CTA, every mode, odd and even term counts, periodic wrap-around dependencies."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    for model, B in ((L.cubic(40, W=16.5, seed=4, energy_scale=16.0), 4),                    # 64000 rows, K = 6
+                     (L.graphene(150, 101, vacancy_fraction=0.02, vacancy_seed=9), 1),       # ragged, B = 1
+                     (L.square_peierls(240, 130, flux_quanta=5, W=1.5, seed=7), 8)):         # complex, B = 8
+        phi = L.random_phase_vectors(model.N, B, config=59)
+        modes = gq.MODE_VAC | gq.MODE_MSD
+        o = oracle_mod.Oracle(model, batch=B, modes=modes)
+        g = gq.GpuQT(model, batch=B, modes=modes)
+        o.set_state(phi)
+        g.set_state(phi)
+        for nm in (37, 64):
+            assert np.max(np.abs(g.dos_moments(nm) - o.dos_moments(nm))) / model.N <= TOL
+        for dt, order in ((0.7, 24), (0.35, 17)):
+            va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+            scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(B)])
+            assert np.max(np.abs(g.vac(33) - o.vac(33)) / scale[:, None]) <= TOL
+            o.evolve(dt, order)
+            g.evolve(dt, order)
+            for sg, so in ((gq.STATE_PSI, oracle_mod.PSI), (gq.STATE_CHI, oracle_mod.CHI),
+                           (gq.STATE_VAC_A, oracle_mod.VAC_A), (gq.STATE_VAC_B, oracle_mod.VAC_B)):
+                assert vec_err(g.get_state(sg), o.get_state(so)) <= TOL
+            chi = o.get_state(oracle_mod.CHI)
+            assert np.max(np.abs(g.msd(30) - o.msd(30)) / (norms(chi) ** 2)[:, None]) <= TOL
+        g.close()
+        o.close()
