@@ -98,12 +98,19 @@ def load_peak():
 
 
 # ------------------------------------------------------------------------------------ oracle legs
+def sample_moments(w, model):
+    """Moments of the oracle's bounded sample: ~5e8 row-walks/s on 16 cores, aim at <= 1e10 row-walks."""
+    return int(min(w.n_moments, max(16, (1e10 / model.N) // 2 * 2)))
+
+
+
 def oracle_sample(w, model, order, seconds_hint=15.0):
     """Bounded sample of the workload's step on the CPU oracle: 1 vector, full N, the full evolve
-    step, and a 16-moment set.  Returns (task-normalised orbital-SpMV, executed SpMV rows, seconds,
-    cores, description)."""
+    step, and a moment set sized for about 10-30 s of CPU work (the whole N_m when that fits).
+    Returns (task-normalised orbital-SpMV, executed SpMV rows, seconds, cores, description)."""
     from oracle import oracle
-    nm_s = 16
+    # ~5e8 row-walks/s on 16 cores: aim at <= 1e10 row-walks in the moment set
+    nm_s = sample_moments(w, model)
     o = oracle.Oracle(model, batch=1, modes=oracle.MODE_MSD if w.path == "msd" else oracle.MODE_VAC)
     phi = w.phases(model)[:1]
     o.set_state(phi)
@@ -145,7 +152,7 @@ def run_reference(args, w):
             "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.key, "description": w.description, "N": model.N, "K": model.K,
-                       "batch": 1, "n_moments_sampled": 16, "order": order},
+                       "batch": 1, "n_moments_sampled": sample_moments(w, model), "order": order},
             "cpu_baseline": {"value": value, "unit": "orbital-SpMV/s", "cores": cores, "kind": "oracle", "sample": desc,
                              "executed_value": executed * len(times) / total},
             "e2e": {"value": value, "unit": "orbital-SpMV/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},

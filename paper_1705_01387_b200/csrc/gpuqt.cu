@@ -35,9 +35,10 @@ struct gpuqt_handle {
     int alternate = 1;                  // GPUQT_ALTERNATE: sweep direction alternates between launches
     int rec_bytes = 0;                  // bytes of one (widest) slice record
     int want_stages = 2;                // requested pipeline depth per warp
-    int mode_stages[4] = {0, 0, 0, 0};  // per step-kernel mode: stages, bytes per stage, dynamic smem
-    int mode_stage_bytes[4] = {0, 0, 0, 0};
-    size_t mode_smem[4] = {0, 0, 0, 0};
+    // per launch configuration [mode + 4 * pair]: stages, bytes per stage, dynamic smem
+    int mode_stages[8] = {0};
+    int mode_stage_bytes[8] = {0};
+    size_t mode_smem[8] = {0};
     std::vector<void*> smem_set;        // kernels whose dynamic-smem attribute has been raised
     double dE = 0, box = 0, volume = 0;
     cudaStream_t stream = nullptr;
@@ -64,7 +65,7 @@ struct gpuqt_handle {
     size_t scratch_bytes = 0;
     double *partials = nullptr, *dots = nullptr, *moments = nullptr;
     unsigned int* ticket = nullptr;
-    int grid[4] = {0, 0, 0, 0};
+    int grid[8] = {0};                  // [mode + 4 * pair]
     int grid_aux = 0;
     int sweep = 0;                      // direction of the next step launch (reset per building block)
     bool state_set = false;
@@ -127,8 +128,8 @@ Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
 }
 
 // shared memory of one step-kernel CTA: mbarriers, then kWarps * stages record buffers
-size_t step_smem_bytes(int stages, int stage_bytes) {
-    return 128 * (((size_t)kWarps * kMaxStages * 8 + 127) / 128) + (size_t)kWarps * stages * stage_bytes;
+size_t step_smem_bytes(int stages, int stage_bytes, bool pair = false) {
+    return 128 * (((pair ? 2 : 1) * (size_t)kWarps * kMaxStages * 8 + 127) / 128) + (size_t)kWarps * stages * stage_bytes;
 }
 constexpr size_t kSmemBudget = 200 * 1024;   // per CTA; leaves room for the static reduction buffers
 constexpr size_t kSmemPerSm = 227 * 1024;
@@ -142,35 +143,39 @@ bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
 
 // ---------------------------------------------------------------- kernel dispatch
 template <int MODE, int BB, int KK>
-void* step_fn(int hop) {
+void* step_fn(int hop, bool pair) {
+    if (pair)
+        return hop == kHopComplex ? (void*)cheb_pair_kernel<BB, KK, kHopComplex, MODE>
+               : hop == kHopConst ? (void*)cheb_pair_kernel<BB, KK, kHopConst, MODE>
+                                  : (void*)cheb_pair_kernel<BB, KK, kHopReal, MODE>;
     return hop == kHopComplex ? (void*)cheb_step_kernel<BB, KK, kHopComplex, MODE>
            : hop == kHopConst ? (void*)cheb_step_kernel<BB, KK, kHopConst, MODE>
                               : (void*)cheb_step_kernel<BB, KK, kHopReal, MODE>;
 }
 template <int MODE, int BB>
-void* step_fn_k(int kt, int cplx) {
+void* step_fn_k(int kt, int hop, bool pair) {
     switch (kt) {
-    case 3: return step_fn<MODE, BB, 3>(cplx);
-    case 4: return step_fn<MODE, BB, 4>(cplx);
-    case 6: return step_fn<MODE, BB, 6>(cplx);
-    default: return step_fn<MODE, BB, 0>(cplx);
+    case 3: return step_fn<MODE, BB, 3>(hop, pair);
+    case 4: return step_fn<MODE, BB, 4>(hop, pair);
+    case 6: return step_fn<MODE, BB, 6>(hop, pair);
+    default: return step_fn<MODE, BB, 0>(hop, pair);
     }
 }
 template <int MODE>
-void* step_fn_b(int B, int kt, int cplx) {
+void* step_fn_b(int B, int kt, int hop, bool pair) {
     switch (B) {
-    case 1: return step_fn_k<MODE, 1>(kt, cplx);
-    case 2: return step_fn_k<MODE, 2>(kt, cplx);
-    case 4: return step_fn_k<MODE, 4>(kt, cplx);
-    default: return step_fn_k<MODE, 8>(kt, cplx);
+    case 1: return step_fn_k<MODE, 1>(kt, hop, pair);
+    case 2: return step_fn_k<MODE, 2>(kt, hop, pair);
+    case 4: return step_fn_k<MODE, 4>(kt, hop, pair);
+    default: return step_fn_k<MODE, 8>(kt, hop, pair);
     }
 }
-void* step_kernel(const gpuqt_handle* h, int mode) {
+void* step_kernel(const gpuqt_handle* h, int mode, bool pair) {
     switch (mode) {
-    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->hop);
-    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->hop);
-    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->hop);
-    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->hop);
+    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->hop, pair);
+    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->hop, pair);
+    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->hop, pair);
+    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->hop, pair);
     }
 }
 
@@ -191,9 +196,9 @@ void* dot_fn(int B) {
     }
 }
 
-int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items) {
+int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items, int threads = kThreads) {
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kThreads, smem) != cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
     if (h->max_blocks_per_sm > 0 && per_sm > h->max_blocks_per_sm) per_sm = h->max_blocks_per_sm;
     long long g = (long long)per_sm * h->n_sm;
@@ -205,27 +210,30 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items) {
 
 // bytes of one stage of a step kernel: the record plus the staged own rows of T_{m-1}, T_{m-2}
 // (and e_{m-1}, e_{m-2} for the (a, e) pair)
-int mode_stage_bytes_for(const gpuqt_handle* h, int mode) {
-    const int streams = ((mode == kModeEvolveMsd) ? 4 : 2) / (GPUQT_PREV_DIRECT ? 2 : 1);
-    return h->rec_bytes + streams * 32 * h->B * (int)sizeof(double2);
+int mode_stage_bytes_for(const gpuqt_handle* h, int mode, bool pair = false) {
+    const int streams = (mode == kModeEvolveMsd) ? 4 : 2;
+    return h->rec_bytes + streams * 32 * h->B * (int)sizeof(double2) + (pair ? kHdrBytes : 0);
 }
 
 cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
-    void* fn = step_kernel(h, mode);
-    if (!h->grid[mode]) {
-        const int sb = mode_stage_bytes_for(h, mode);
+    const bool pair = a.n_steps == 2;
+    const int cfg = mode + (pair ? 4 : 0);
+    const int threads = pair ? kThreads + 32 : kThreads;     // the pair kernel has a producer warp
+    void* fn = step_kernel(h, mode, pair);
+    if (!h->grid[cfg]) {
+        const int sb = mode_stage_bytes_for(h, mode, pair);
         int stages = h->want_stages;
-        while (stages > 1 && step_smem_bytes(stages, sb) > kSmemBudget) --stages;
+        while (stages > 1 && step_smem_bytes(stages, sb, pair) > kSmemBudget) --stages;
         // prefer two resident CTAs per SM over a deeper pipeline
-        while (stages > 2 && 2 * (step_smem_bytes(stages, sb) + 4096) > kSmemPerSm) --stages;
-        h->mode_stages[mode] = stages;
-        h->mode_stage_bytes[mode] = sb;
-        h->mode_smem[mode] = step_smem_bytes(stages, sb);
-        if (h->mode_smem[mode] > 48 * 1024) {
-            cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->mode_smem[mode]);
+        while (stages > 2 && 2 * (step_smem_bytes(stages, sb, pair) + 4096) > kSmemPerSm) --stages;
+        h->mode_stages[cfg] = stages;
+        h->mode_stage_bytes[cfg] = sb;
+        h->mode_smem[cfg] = step_smem_bytes(stages, sb, pair);
+        if (h->mode_smem[cfg] > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->mode_smem[cfg]);
             if (e != cudaSuccess) return e;
         }
-        h->grid[mode] = grid_for(h, fn, h->mode_smem[mode], (h->mat.n_slices + h->run - 1) / h->run);
+        h->grid[cfg] = grid_for(h, fn, h->mode_smem[cfg], (h->mat.n_slices + h->run - 1) / h->run, threads);
     }
     a.sched = nullptr;
     a.n_items = 0;
@@ -236,13 +244,13 @@ cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
         const int reverse = h->alternate ? (h->sweep & 1) : 0;
         const gpuqt_handle::DevSchedule* ds = nullptr;
         for (const auto& d : h->schedules)
-            if (d.G == h->grid[mode] && d.reverse == reverse) ds = &d;
+            if (d.G == h->grid[cfg] && d.reverse == reverse) ds = &d;
         if (!ds) {
             FusedSchedule fs;
-            build_fused_schedule((int)h->mat.n_slices, h->run, h->grid[mode], reverse, std::max(1, h->lag * h->grid[mode] / 2),
+            build_fused_schedule((int)h->mat.n_slices, h->run, h->grid[cfg], reverse, std::max(1, h->lag * h->grid[cfg] / 2),
                                  kNoRun, h->nbr_ptr, h->nbr_slices, fs);
             gpuqt_handle::DevSchedule d{};
-            d.G = h->grid[mode];
+            d.G = h->grid[cfg];
             d.reverse = reverse;
             d.n_items = (int)(fs.items.size() / 2);
             d.n_runs = (int)fs.dep_ptr.size() - 1;
@@ -267,8 +275,8 @@ cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
         a.dep_ptr = ds->dep_ptr;
         a.dep_list = ds->dep_list;
     }
-    a.stages = h->mode_stages[mode];
-    a.stage_bytes = h->mode_stage_bytes[mode];
+    a.stages = h->mode_stages[cfg];
+    a.stage_bytes = h->mode_stage_bytes[cfg];
     a.rec_bytes = h->rec_bytes;
     a.partials = h->partials;
     a.ticket = h->ticket;
@@ -276,7 +284,7 @@ cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
     a.run = h->run;
     h->sweep ^= 1;
     void* args[] = {(void*)&h->mat, (void*)&a};
-    return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, h->mode_smem[mode], h->stream);
+    return cudaLaunchKernel(fn, dim3(h->grid[cfg]), dim3(threads), args, h->mode_smem[cfg], h->stream);
 }
 
 cudaError_t launch_velocity(gpuqt_handle* h, const double2* in, double2* out) {
@@ -560,7 +568,7 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : kHopConst;
     const int stage_bytes = (int)record_bytes(K_max, sell.nd);
     h->rec_bytes = stage_bytes;
-    if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd)) > kSmemBudget) {
+    if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd, true), true) > kSmemBudget) {
         fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "
                         "shared memory\n", K_max, stage_bytes);
         delete h;
@@ -615,6 +623,8 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->max_blocks_per_sm = env_int("GPUQT_BLOCKS_PER_SM", 0);
     h->alternate = env_int("GPUQT_ALTERNATE", 1);
     h->run = std::max(1, env_int("GPUQT_RUN", 16) / kWarps) * kWarps;
+    // two steps per launch (cheb_pair_kernel) are opt-in: they cut the DRAM bytes of a step pair by a
+    // third but are time-neutral at best on B200 so far
     h->fuse = env_int("GPUQT_FUSE", 0);
     h->lag = std::max(1, env_int("GPUQT_LAG", 2));
     h->nbr_ptr.swap(sell.nbr_ptr);

@@ -14,16 +14,17 @@
 //             every stored hopping is the same real number, kept in Mat::hop_const) padding is
 //             col = N: every vector buffer carries an all-zero row N (and x[N] = 0), so the walk
 //             needs no guard.  One record = one 1-D TMA bulk copy.
-//   warp      the unit of work is (warp, slice).  A stage of a warp's shared-memory pipeline holds
-//             everything the slice streams from HBM exactly once: the packed record, the slice's
-//             own rows of T_{m-1} (and e_{m-1}) and of T_{m-2} (and e_{m-2}) -- each one 1-D TMA
-//             bulk copy (cp.async.bulk + mbarrier, no CTA-wide barrier in the loop), issued one or
-//             more slices ahead, so the DRAM streams never sit on a warp's scoreboard.  The warp
-//             walks the slice in B sub-steps of 32/B rows: lane -> (row = lane / B, b = lane % B).
-//             Neighbours inside the slice are read from the staged rows in shared memory; the
-//             others are gathered from global memory (L1/L2 hits along the sweep front), all
-//             gathers of a sub-step group issued back to back.  Stores of a warp are one
-//             contiguous 512-byte segment.
+//   warp      the unit of work is (consumer warp, slice).  A stage of a warp's shared-memory pipeline
+//             holds everything the slice streams from HBM exactly once: the packed record, the
+//             slice's own rows of T_{m-1} (and e_{m-1}) and of T_{m-2} (and e_{m-2}) -- each one
+//             1-D TMA bulk copy (cp.async.bulk + mbarrier) issued by the CTA's producer warp one or
+//             more slices ahead, so the DRAM streams never sit on a consumer's scoreboard and there
+//             is no CTA-wide barrier in the loop.  A consumer walks the slice in rounds of 32/LPR
+//             rows; a lane owns V = 2 consecutive vectors of a row (256-bit accesses) and LPR = B/V
+//             lanes share a row.  Neighbours inside the slice are read from the staged rows in
+//             shared memory; the others are gathered from global memory (L2 hits along the sweep
+//             front), all gathers of a round issued back to back.  Stores of a warp are one
+//             contiguous segment.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -40,9 +41,6 @@
 #endif
 
 // L2 policy experiments
-#ifndef GPUQT_PREV_DIRECT     // experiment: 1 = T_{m-2} own rows by a streaming 256-bit global load instead of TMA staging
-#define GPUQT_PREV_DIRECT 0
-#endif
 #ifndef GPUQT_GATHER_POLICY   // 0: plain ld.global, 1: L2::evict_last
 #define GPUQT_GATHER_POLICY 1
 #endif
@@ -159,6 +157,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "}" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
     uint32_t ok;
@@ -475,13 +476,6 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     if (MODE == kModeLeft) other = cv_ld_stream<V>(&a.phiL[vi]);
     double xm = 0.0;
     if (MSD) xm = m.x[row0 + (ok ? r : 0)];
-#if GPUQT_PREV_DIRECT
-    CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
-    if (!a.first) {
-        prev = cv_ld_stream<V>(&io.prev[vi]);
-        if (MSD) prev_e = cv_ld_stream<V>(&io.prev_e[vi]);
-    }
-#endif
 
     const CV<V> self = ok ? cv_lds<V>(s_in + si_) : cv_zero<V>();
     const CV<V> self_e = (MSD && ok) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
@@ -536,13 +530,11 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
             }
         }
     }
-#if !GPUQT_PREV_DIRECT
     CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
     if (!a.first && ok) {
         prev = cv_lds<V>(s_prev + si_);
         if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
     }
-#endif
     const double hs = CONST ? scale * m.hop_const : scale;              // scale of the neighbour sums
     const double os = scale * on;                                       // scale of the on-site term
     CV<V> t, te, acc, ae;   // T_m, e_m, and the accumulators
@@ -618,7 +610,7 @@ __device__ __forceinline__ void warp_flush(double (&v)[Q * V], double* dst, int 
 // Value p < P0 goes to r0[p], the others to r1[p - P0] (second step of a fused pair).
 __device__ __forceinline__ void block_finish(const double* s_part, int P, int P0, double* partials,
                                              unsigned int* ticket, double* r0, double* r1) {
-    __shared__ double s_tree[kThreads];
+    __shared__ double s_tree[kThreads + 32];   // the step kernel calls this with its producer warp as well
     __shared__ int s_last;
     const int tid = threadIdx.x;
     __syncthreads();
@@ -661,54 +653,49 @@ __device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
 }
 
 
-// One Chebyshev recurrence step fused with what consumes it -- or TWO consecutive steps in one
-// launch (a.n_steps == 2), the second trailing the first by a few sweep rounds so that it finds
-// T_m, T_{m-1} and the matrix records in L2: per pair of steps DRAM then sees T_{m-1}, T_{m-2} read
-// and T_m, T_{m+1} written once each and the matrix once, instead of 6 vector passes and 2 matrix
-// passes.
-//
-// Persistent CTAs.  The slices are cut into runs of a.run consecutive slices; the work list is a
-// sequence of items = (step, run); CTA c takes items c, c + G, c + 2G, ...; inside a run warp w takes
-// slices w, w + kWarps, ...  Single-step launches use the arithmetic list item t = run t.  Fused
-// launches read the list from a.sched (built on the host from the table's sparsity, host_util.h):
-// first-step items in sweep order, each second-step item a fixed slack behind the first-step items
-// it depends on.  A warp that finishes its slices of a first-step item releases run_done[run]; a
-// warp about to start a second-step item checks (all lanes, relaxed loads + one acquire fence) that
-// the runs it gathers from are complete.  A warp only blocks on that when it has nothing in flight,
-// and an item depends only on earlier items of the list, so the scheme cannot deadlock as long as
-// all CTAs are co-resident (the grid is sized by occupancy).
-// All loop indices are kept incrementally (no divisions in the loop).
+// One Chebyshev recurrence step fused with what consumes it (single-step launches; the default).
+// Every warp issues its own TMA copies (lane 0) one or more slices ahead.  Persistent CTAs: the slices are cut
+// into runs of a.run consecutive slices; CTA c walks runs c, c + G, c + 2G, ...; inside a run warp w
+// takes slices w, w + kWarps, ...  A CTA therefore streams a contiguous band of rows and the grid
+// sweeps the vector as a tight front, so gathers to nearby rows (the +-x, +-y, +-z neighbours of a
+// lattice) are served by L1/L2.  All loop indices are kept incrementally (no divisions in the loop).
 template <int B, int KT, int HOP, int MODE>
 __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
     constexpr int Q = ModeTraits<MODE>::Q;
     constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
     constexpr int RB = B * 16, QB = Q * B;
-    constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
     constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
+    __shared__ double s_part[DOTS ? kWarps * QB : 1];
+    const StepIO& io = a.io[0];
+    constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ double s_part[DOTS ? kWarps * 2 * QB : 1];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
     const int stages = a.stages;
     const int stage_bytes = a.stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + warp * kMaxStages;
     unsigned char* wstage = smem + 128 * ((kWarps * kMaxStages * 8 + 127) / 128) + (size_t)warp * stages * stage_bytes;
-    const int P = a.n_steps * QB;                 // dot values per block
-    double* my_part = s_part + warp * P;
 
     double red[Q * V];
 #pragma unroll
     for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
     if (DOTS) {
-        for (int i = lane; i < P; i += 32) my_part[i] = 0.0;
+        for (int i = lane; i < QB; i += 32) s_part[warp * QB + i] = 0.0;
     }
     const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
 
     const int N = (int)m.N, n_slices = (int)m.n_slices;
+    const int per = a.run / kWarps;
     const int n_runs = (n_slices + a.run - 1) / a.run;
     const int G = gridDim.x;
-    const bool fused = a.sched != nullptr;
-    const int n_total = fused ? a.n_items : n_runs;
+    const int my_runs = (int)blockIdx.x < n_runs ? (n_runs - (int)blockIdx.x + G - 1) / G : 0;
+    int n_my = 0;
+    if (my_runs > 0) {
+        const int last = blockIdx.x + (my_runs - 1) * G;
+        const int rem = n_slices - last * a.run;          // slices in my last run (may be partial)
+        const int in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
+        n_my = (my_runs - 1) * per + in_last;
+    }
     uint64_t policy = 0;
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(&bars[s], 1);
@@ -717,51 +704,25 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     }
     __syncwarp();
 
-    // a pipeline cursor: item (t, run, step, wait, cnt = slices of this warp in the run), slice
-    // index k inside the item, virtual slice s, shared-memory stage and phase
+    // position of a pipeline cursor: slice (forward order), index inside the run, stage, phase
     struct Cursor {
-        int t, run, step, cnt, k, s, st;
+        int s, k, st;
         uint32_t ph;
     };
-    auto load_item = [&](Cursor& c) {
-        c.step = 0;
-        c.run = kNoRun;
-        if (c.t < n_total) {
-            if (fused) {
-                const int2 e = a.sched[c.t];
-                c.run = e.x & kNoRun;
-                c.step = (e.x >> 30) & 1;
-            } else {
-                c.run = c.t;
-            }
+    const int jump = G * a.run - (per - 1) * kWarps;     // last slice of a run -> first slice of my next run
+    auto advance = [&](Cursor& c) {
+        if (++c.k == per) {
+            c.k = 0;
+            c.s += jump;
+        } else {
+            c.s += kWarps;
         }
-        c.cnt = 0;
-        if (c.run != kNoRun) {
-            int left = n_slices - c.run * a.run;
-            left = left < a.run ? left : a.run;
-            c.cnt = warp < left ? (left - warp + kWarps - 1) / kWarps : 0;
-        }
-        c.k = 0;
-        c.s = c.run * a.run + warp;
-    };
-    auto next_stage = [&](Cursor& c) {
         if (++c.st == stages) {
             c.st = 0;
             c.ph ^= 1u;
         }
     };
-    auto deps_done = [&](int run) {   // whole warp: have all first-step runs this run gathers from finished?
-        const int b = a.dep_ptr[run], e = a.dep_ptr[run + 1];
-        bool ok = true;
-#pragma unroll 1
-        for (int i0 = b; i0 < e; i0 += 32) {      // every lane acquires (lanes past the end re-read the last entry)
-            const int i = i0 + lane < e ? i0 + lane : e - 1;
-            ok = ok && (ld_acquire_gpu(a.run_done + a.dep_list[i]) >= (unsigned int)kWarps);
-        }
-        return __all_sync(0xffffffffu, ok) != 0;
-    };
     auto issue = [&](const Cursor& c) {   // lane 0 only: every HBM stream of the slice -> one stage, one mbarrier
-        const StepIO& io = a.io[c.step];
         const int s = a.reverse ? n_slices - 1 - c.s : c.s;
         long long off;
         uint32_t bytes;
@@ -777,73 +738,34 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
         // constant-hopping padding entries point at it)
         const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-        const uint32_t total = bytes + vbytes_in * kPair + ((a.first || GPUQT_PREV_DIRECT) ? 0u : vbytes * kPair);
+        const uint32_t total = bytes + vbytes_in * kPair + (a.first ? 0u : vbytes * kPair);
         unsigned char* dst = wstage + c.st * stage_bytes;
         unsigned char* vdst = dst + a.rec_bytes;
         const size_t voff = (size_t)s * 32 * B;
         mbar_expect_tx(&bars[c.st], total);
-        // the first step of a fused pair leaves the record in L2 for the second one
-        if (fused && c.step == 0) bulk_g2s_nohint(dst, m.rec + off, bytes, &bars[c.st]);
-        else bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
+        bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
         bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[c.st]);
         if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &bars[c.st]);
-        if (!a.first && !GPUQT_PREV_DIRECT) {
+        if (!a.first) {
             bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &bars[c.st], policy);
             if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &bars[c.st], policy);
         }
     };
 
-    // Both cursors are advanced by all lanes (warp-uniform control flow); only the TMA issue itself
-    // is lane 0's.  Items in which this warp has no slice are skipped (first-step ones are signalled).
-    Cursor prod{}, cons{};
-    prod.t = blockIdx.x;
-    load_item(prod);
-    while (prod.cnt == 0 && prod.t < n_total) {
-        prod.t += G;
-        load_item(prod);
+    Cursor prod{(int)blockIdx.x * a.run + warp, 0, 0, 0u}, cons = prod;
+    int issued = 0;
+    if (lane == 0) {
+        for (; issued < stages - 1 && issued < n_my; ++issued) {
+            issue(prod);
+            advance(prod);
+        }
     }
-    cons.t = blockIdx.x;
-    load_item(cons);
-    while (cons.cnt == 0 && cons.t < n_total) {
-        if (fused && cons.step == 0 && cons.run != kNoRun && lane == 0) red_release_gpu_inc(a.run_done + cons.run);
-        cons.t += G;
-        load_item(cons);
-    }
-    int inflight = 0;          // slices issued and not yet consumed
-    bool dep_ok = false;       // the producer's item has passed its dependency check
-    int red_step = cons.step;  // step whose dots the register accumulators hold
-    // A finished first-step item is published (release on run_done) one slice later, from inside the
-    // next slice's walk right after its gathers have been issued: the fence then overlaps with the
-    // gather latency instead of stalling the warp on the write acknowledgements.
-    unsigned int* pending = nullptr;
-
-    while (cons.t < n_total) {
-        while (prod.t < n_total && inflight < stages) {
-            if (fused && prod.step == 1 && !dep_ok) {
-                if (!deps_done(prod.run)) {
-                    if (inflight > 0) break;                     // keep consuming; retry later
-                    if (pending && lane == 0) red_release_gpu_inc(pending);   // nothing of mine may stay unpublished
-                    pending = nullptr;
-                    do __nanosleep(200);
-                    while (!deps_done(prod.run));
-                }
-                // The rows were stored through the generic proxy by other SMs, fenced and released at
-                // gpu scope (they are in L2), and acquired above; the TMA reads that follow are issued
-                // behind that acquire by control dependency and go to L2.  (A reader-side
-                // fence.proxy.async compiles to a full MEMBAR.GPU per item and is not needed here.)
-                dep_ok = true;
-            }
-            if (lane == 0) issue(prod);
-            ++inflight;
-            next_stage(prod);
-            prod.s += kWarps;
-            if (++prod.k == prod.cnt) {
-                dep_ok = false;
-                do {
-                    prod.t += G;
-                    load_item(prod);
-                } while (prod.cnt == 0 && prod.t < n_total);
-            }
+    for (int i = 0; i < n_my; ++i) {
+        // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
+        if (lane == 0 && issued < n_my) {
+            issue(prod);
+            advance(prod);
+            ++issued;
         }
         mbar_wait(&bars[cons.st], cons.ph);
         const unsigned char* stage = wstage + cons.st * stage_bytes;
@@ -852,36 +774,219 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         if (KT == 0) w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
         const int row0 = slice * 32;
         const int rows_valid = N - row0;          // >= 32 except in the last slice
-        const StepIO& io = a.io[cons.step];
 #pragma unroll 1
-        for (int j = 0; j < ROUNDS; ++j) {
-            walk_round<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, scale, red, pending);
-            pending = nullptr;
-        }
+        for (int j = 0; j < ROUNDS; ++j) walk_round<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, scale, red, nullptr);
+        advance(cons);
         __syncwarp();
-        --inflight;
-        next_stage(cons);
-        cons.s += kWarps;
-        if (++cons.k == cons.cnt) {
-            // item finished: publish the T_m rows of a first-step item, move to my next item
-            if (fused && cons.step == 0) pending = a.run_done + cons.run;
-            do {
-                cons.t += G;
-                load_item(cons);
-                if (fused && cons.cnt == 0 && cons.step == 0 && cons.run != kNoRun && lane == 0)
-                    red_release_gpu_inc(a.run_done + cons.run);
-            } while (cons.cnt == 0 && cons.t < n_total);
-            if (DOTS && cons.t < n_total && cons.step != red_step) {
+    }
+    if (DOTS) {
+        warp_flush<B, Q, V>(red, s_part + warp * QB, lane);
+        block_finish(s_part, QB, QB, a.partials, a.ticket, io.result, io.result);
+    }
+}
+
+
+// TWO consecutive recurrence steps in one launch (a.n_steps == 2; opt-in, GPUQT_FUSE=1): the second
+// step trails the first by a fixed slack of the work list so that it finds T_m, T_{m-1} and the matrix records in L2: per pair of steps DRAM then sees T_{m-1},
+// T_{m-2} read and T_m, T_{m+1} written once each and the matrix once, instead of 6 vector passes
+// and 2 matrix passes.
+//
+// Persistent, warp-specialised CTAs of kWarps consumer warps + 1 producer warp.  The slices are cut
+// into runs of a.run consecutive slices; the work list is a sequence of items = (step, run); CTA c
+// takes items c, c + G, c + 2G, ...; inside a run consumer warp w takes slices w, w + kWarps, ...
+// Single-step launches use the arithmetic list item t = run t; fused launches read the list from
+// a.sched (built on the host from the table's sparsity, host_util.h).
+//   producer warp   walks the CTA's items; lane w < kWarps feeds consumer warp w: it waits for a
+//                   free stage of that warp (mbarrier empty[w][st]), writes a 16-byte header
+//                   {slice, step, flags, run} and issues the TMA bulk copies of the slice onto
+//                   full[w][st].  Before a second-step item it checks, all 32 lanes at once with
+//                   acquire loads, that the first-step runs the item gathers from are complete
+//                   (run_done[r] == kWarps) and sleeps otherwise.  The consumers never touch the
+//                   work list.
+//   consumer warp   waits full[w][st], walks the slice, arrives on empty[w][st].  After the last
+//                   slice of a first-step item it owes a release on run_done[run]; it pays one slice
+//                   later, right after that slice's gathers have been issued (the fence then overlaps
+//                   the gather latency), or at once when no slice is ready.
+// An item depends only on earlier items of the list and every warp publishes what it owes before
+// it blocks, so the scheme cannot deadlock as long as all CTAs are co-resident (the grid is sized
+// by occupancy).
+constexpr int kHdrBytes = 128;                    // per stage: the slice header
+constexpr int kFlagEnd = 1, kFlagOwesRelease = 2;
+
+template <int B, int KT, int HOP, int MODE>
+__global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) cheb_pair_kernel(const Mat m, const StepArgs a) {
+    constexpr int Q = ModeTraits<MODE>::Q;
+    constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
+    constexpr int RB = B * 16, QB = Q * B;
+    constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
+    constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ double s_part[DOTS ? kWarps * 2 * QB : 1];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
+    const int stages = a.stages;
+    const int stage_bytes = a.stage_bytes;                     // record | vector rows | header
+    const int hdr_off = stage_bytes - kHdrBytes;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [kWarps][kMaxStages]
+    uint64_t* empty = full + kWarps * kMaxStages;              // [kWarps][kMaxStages]
+    unsigned char* stage_base = smem + 128 * ((2 * kWarps * kMaxStages * 8 + 127) / 128);
+    const int P = a.n_steps * QB;                 // dot values per block
+
+    const int N = (int)m.N, n_slices = (int)m.n_slices;
+    const int n_runs = (n_slices + a.run - 1) / a.run;
+    const int G = gridDim.x;
+    const bool fused = a.sched != nullptr;
+    const int n_total = fused ? a.n_items : n_runs;
+
+    if (warp < kWarps && lane == 0) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(&full[warp * kMaxStages + s], 1);
+            mbar_init(&empty[warp * kMaxStages + s], 1);
+        }
+        fence_mbar_init();
+    }
+    if (DOTS && warp < kWarps) {
+        for (int i = lane; i < P; i += 32) s_part[warp * P + i] = 0.0;
+    }
+    __syncthreads();
+
+    if (warp == kWarps) {
+        // ------------------------------------------------------------------ producer warp
+        const int cw = lane < kWarps ? lane : kWarps - 1;       // consumer warp this lane feeds
+        const bool feeds = lane < kWarps;
+        unsigned char* my_stages = stage_base + (size_t)cw * stages * stage_bytes;
+        uint64_t* my_full = full + cw * kMaxStages;
+        uint64_t* my_empty = empty + cw * kMaxStages;
+        int st = 0;
+        uint32_t ph = 0;
+        const uint64_t policy = policy_evict_first();
+        auto deps_done = [&](int run) {   // whole warp: have all first-step runs this run gathers from finished?
+            const int b = a.dep_ptr[run], e = a.dep_ptr[run + 1];
+            bool ok = true;
+#pragma unroll 1
+            for (int i0 = b; i0 < e; i0 += 32) {      // every lane acquires (lanes past the end re-read the last entry)
+                const int i = i0 + lane < e ? i0 + lane : e - 1;
+                ok = ok && (ld_acquire_gpu(a.run_done + a.dep_list[i]) >= (unsigned int)kWarps);
+            }
+            return __all_sync(0xffffffffu, ok) != 0;
+        };
+        for (int t = blockIdx.x; t < n_total; t += G) {
+            int run = t, step = 0;
+            if (fused) {
+                const int2 e = a.sched[t];
+                run = e.x & kNoRun;
+                step = (e.x >> 30) & 1;
+            }
+            if (run == kNoRun) continue;
+            if (fused && step == 1) {
+                // rows stored through the generic proxy by other SMs, fenced and released at gpu scope
+                // (they are in L2) and acquired here; the TMA reads below are issued behind the acquire
+                // by control dependency and go to L2
+                while (!deps_done(run)) __nanosleep(200);
+            }
+            const StepIO& io = a.io[step];
+            int len = n_slices - run * a.run;
+            len = len < a.run ? len : a.run;
+            for (int k0 = 0; k0 < len; k0 += kWarps) {
+                if (feeds && k0 + lane < len) {
+                    const int vs = run * a.run + k0 + lane;                 // slice in sweep order
+                    const int s = a.reverse ? n_slices - 1 - vs : vs;
+                    mbar_wait(&my_empty[st], ph ^ 1u);                      // stage free (passes at once the first time round)
+                    unsigned char* dst = my_stages + st * stage_bytes;
+                    int flags = 0;
+                    if (fused && step == 0 && k0 + lane + kWarps >= len) flags |= kFlagOwesRelease;
+                    *reinterpret_cast<int4*>(dst + hdr_off) = make_int4(s, step, flags, run);
+                    long long off;
+                    uint32_t bytes;
+                    if (KT > 0) {
+                        bytes = (uint32_t)record_bytes(KT, hop_doubles(HOP));
+                        off = (long long)s * bytes;
+                    } else {
+                        off = m.slice_off[s];
+                        bytes = (uint32_t)(m.slice_off[s + 1] - off);
+                    }
+                    const int left = N - s * 32;
+                    const uint32_t vbytes = (uint32_t)((left < 32 ? left : 32) * RB);
+                    // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
+                    // constant-hopping padding entries point at it)
+                    const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
+                    const uint32_t total = bytes + vbytes_in * kPair + (a.first ? 0u : vbytes * kPair);
+                    unsigned char* vdst = dst + a.rec_bytes;
+                    const size_t voff = (size_t)s * 32 * B;
+                    mbar_expect_tx(&my_full[st], total);
+                    // the first step of a fused pair leaves the record in L2 for the second one
+                    if (fused && step == 0) bulk_g2s_nohint(dst, m.rec + off, bytes, &my_full[st]);
+                    else bulk_g2s(dst, m.rec + off, bytes, &my_full[st], policy);
+                    bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &my_full[st]);
+                    if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &my_full[st]);
+                    if (!a.first) {
+                        bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &my_full[st], policy);
+                        if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &my_full[st], policy);
+                    }
+                    if (++st == stages) {
+                        st = 0;
+                        ph ^= 1u;
+                    }
+                }
+            }
+            // consumer warps without a slice in this (short, last) run owe nothing: the producer counts for them
+            if (fused && step == 0 && feeds && lane >= len) red_release_gpu_inc(a.run_done + run);
+        }
+        if (feeds) {   // end marker
+            mbar_wait(&my_empty[st], ph ^ 1u);
+            *reinterpret_cast<int4*>(my_stages + st * stage_bytes + hdr_off) = make_int4(0, 0, kFlagEnd, 0);
+            mbar_arrive(&my_full[st]);
+        }
+    } else {
+        // ------------------------------------------------------------------ consumer warps
+        unsigned char* my_stages = stage_base + (size_t)warp * stages * stage_bytes;
+        uint64_t* my_full = full + warp * kMaxStages;
+        uint64_t* my_empty = empty + warp * kMaxStages;
+        double* my_part = s_part + warp * P;
+        double red[Q * V];
+#pragma unroll
+        for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
+        const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
+        int st = 0;
+        uint32_t ph = 0;
+        int red_step = 0;                   // step whose dots the register accumulators hold
+        unsigned int* pending = nullptr;    // release owed for a finished first-step item
+        while (true) {
+            if (pending && !mbar_test(&my_full[st], ph)) {     // nothing ready: pay now, then wait
+                if (lane == 0) red_release_gpu_inc(pending);
+                pending = nullptr;
+            }
+            mbar_wait(&my_full[st], ph);
+            const unsigned char* stage = my_stages + st * stage_bytes;
+            const int4 hdr = *reinterpret_cast<const int4*>(stage + hdr_off);
+            if (hdr.z & kFlagEnd) break;
+            const int slice = hdr.x, step = hdr.y;
+            if (DOTS && step != red_step) {
                 warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
-                red_step = cons.step;
+                red_step = step;
+            }
+            int w = KT;
+            if (KT == 0) w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
+            const int row0 = slice * 32;
+            const int rows_valid = N - row0;          // >= 32 except in the last slice
+            const StepIO& io = a.io[step];
+#pragma unroll 1
+            for (int j = 0; j < ROUNDS; ++j) {
+                walk_round<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, scale, red, pending);
+                pending = nullptr;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&my_empty[st]);
+            if (hdr.z & kFlagOwesRelease) pending = a.run_done + hdr.w;
+            if (++st == stages) {
+                st = 0;
+                ph ^= 1u;
             }
         }
+        if (pending && lane == 0) red_release_gpu_inc(pending);
+        if (DOTS) warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
     }
-    if (pending && lane == 0) red_release_gpu_inc(pending);
-    if (DOTS) {
-        warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
-        block_finish(s_part, P, QB, a.partials, a.ticket, a.io[0].result, a.io[1].result);
-    }
+    if (DOTS) block_finish(s_part, P, QB, a.partials, a.ticket, a.io[0].result, a.io[1].result);
 }
 
 // Address of entry (row, k) pieces inside the packed records (plain global reads; used by the
