@@ -283,9 +283,8 @@ def run_ours(args, w):
                              "stored_bytes_per_launch": stored_row_launch * model.N,
                              "stored_gbs": stored_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9,
                              "avg_launch_us": dom_ms * 1e3 / max(dom_n, 1), "launches": dom_n,
-                             "note": "per recurrence step: a launch of the step kernel performs two consecutive "
-                                     "steps (fused through L2) except the first / an odd last one; bytes and time "
-                                     "are both per step, so achieved = algorithmic bytes of a launch / its duration",
+                             "note": "launches = recurrence steps; one step per kernel launch by default, two per "
+                                     "launch with GPUQT_FUSE=1 (bytes and time are then both per step)",
                              "share_of_step": dom_ms / ms,
                              "per_class_ms": {names[c]: stats[c][0] for c in names}},
                 }
