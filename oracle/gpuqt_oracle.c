@@ -476,3 +476,39 @@ int oracle_kpm_transform(const oracle_model *m, const double *moments, int32_t n
     free(g);
     return ORACLE_OK;
 }
+
+/* Running conductivity from the transformed correlation functions (units e = 1), Eq. 2,
+ * :92 Eq. 5, :123 Eq. 11; discretisation readings [A25][A26] of DESIGN.md:
+ *   kind 0 (VAC)  in[k][j] = rho(E_j) C_vv(E_j, t_k), rows at t_k = sum_{i<k} dt_i  (measure, evolve [A4]);
+ *                 sigma[k][j] = int_0^{t_k} rho C_vv dt by the trapezoid rule, sigma[0][j] = 0.
+ *   kind 1 (MSD)  in[k][j] = rho(E_j) dX^2(E_j, t_{k+1}), rows at t_{k+1} = sum_{i<=k} dt_i (evolve, measure),
+ *                 dX^2(t = 0) = 0;  sigma[k][j] = (in[k][j] - in[k-1][j]) / (2 dt_k): the time derivative of
+ *                 Eq. 5 by the difference over step k, i.e. the running conductivity at the MIDDLE of step k;
+ *                 length[k][j] = 2 sqrt(in[k][j] / dos[j])  (Eq. 11; 0 where dos <= 0 or in < 0).
+ * dos[j] = rho(E_j) (Eq. 4) is used for the length only; length may be NULL.                      */
+int oracle_running_conductivity(int kind, const double *in, const double *dos, const double *dt,
+                                int32_t n_t, int32_t n_e, double *sigma, double *length)
+{
+    if (!in || !dt || !sigma || n_t < 1 || n_e < 1 || (kind != 0 && kind != 1)) return ORACLE_ERR_ARG;
+    for (int32_t j = 0; j < n_e; ++j) {
+        if (kind == 0) {
+            double acc = 0.0;
+            sigma[j] = 0.0;
+            for (int32_t k = 1; k < n_t; ++k) {
+                acc += 0.5 * (in[(size_t)(k - 1) * n_e + j] + in[(size_t)k * n_e + j]) * dt[k - 1];
+                sigma[(size_t)k * n_e + j] = acc;
+            }
+        } else {
+            for (int32_t k = 0; k < n_t; ++k) {
+                double now = in[(size_t)k * n_e + j];
+                double before = k > 0 ? in[(size_t)(k - 1) * n_e + j] : 0.0;
+                sigma[(size_t)k * n_e + j] = (now - before) / (2.0 * dt[k]);
+                if (length) {
+                    double r = (dos && dos[j] > 0.0 && now > 0.0) ? now / dos[j] : 0.0;
+                    length[(size_t)k * n_e + j] = 2.0 * sqrt(r);
+                }
+            }
+        }
+    }
+    return ORACLE_OK;
+}

@@ -165,3 +165,17 @@ def jackson(n):
     g = np.empty(n)
     _check(lib().oracle_jackson(C.c_int32(n), _d(g)), "jackson")
     return g
+
+
+def running_conductivity(kind, corr, dos, dt):
+    """oracle_running_conductivity: kind 'vac' or 'msd'; corr [n_t][n_E]; returns (sigma, length or None)."""
+    corr = np.ascontiguousarray(corr, np.float64)
+    dt = np.ascontiguousarray(dt, np.float64)
+    n_t, n_e = corr.shape
+    assert dt.size >= (n_t - 1 if kind == "vac" else n_t)
+    sigma = np.empty_like(corr)
+    length = np.empty_like(corr) if kind == "msd" else None
+    dos_a = None if dos is None else np.ascontiguousarray(dos, np.float64)
+    _check(lib().oracle_running_conductivity(C.c_int(0 if kind == "vac" else 1), _d(corr), _d(dos_a), _d(dt),
+                                             C.c_int32(n_t), C.c_int32(n_e), _d(sigma), _d(length)), "running_conductivity")
+    return sigma, length

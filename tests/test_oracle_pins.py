@@ -365,3 +365,67 @@ def test_transform_rejects_energy_outside_band(oracle_mod):
     o = oracle_mod.Oracle(model)
     with pytest.raises(RuntimeError):
         o.kpm_transform(np.ones((1, 4)), np.array([model.energy_scale * 1.01]))
+
+
+# ------------------------------------------------------------------ running conductivity (Eq. 2, 5, 7-11)
+def test_running_conductivity_closed_forms(oracle_mod):
+    """oracle_running_conductivity against closed forms: ballistic (plane wave: rho C_vv = c constant,
+    rho dX^2 = c t^2, PAPER.md 8(c) of SURVEY) and the diffusive regime of the paper's own Eq. 7-10
+    (C_vv = v^2 exp(-t/tau))."""
+    dt = np.array([0.1, 0.2, 0.3, 0.5, 1.0, 1.0, 2.0])                    # non-uniform steps [A18]
+    t = np.concatenate([[0.0], np.cumsum(dt)])
+    c = np.array([3.0, 0.25])
+    # ballistic VAC: the trapezoid rule is exact for a constant: sigma(t_k) = c t_k
+    sig, _ = oracle_mod.running_conductivity("vac", np.tile(c, (t.size, 1)), None, dt)
+    assert np.allclose(sig, np.outer(t, c), rtol=0, atol=1e-14)
+    # ballistic MSD: (c t_k^2 - c t_{k-1}^2) / (2 dt_k) = c (t_k + t_{k-1}) / 2: the value at mid-step
+    dos = np.array([0.5, 2.0])
+    msd = np.outer(t[1:] ** 2, c)
+    sig, length = oracle_mod.running_conductivity("msd", msd, dos, dt)
+    assert np.allclose(sig, np.outer(0.5 * (t[1:] + t[:-1]), c), rtol=1e-14, atol=0)
+    assert np.allclose(length, 2.0 * np.outer(t[1:], np.sqrt(c / dos)), rtol=1e-14)     # Eq. 11
+    # diffusive regime (Eq. 7): rho C_vv = rho v^2 exp(-t/tau)
+    rho, v2, tau = 0.7, 4.0, 1.5
+    dtf = np.full(600, 0.02)
+    tf = np.concatenate([[0.0], np.cumsum(dtf)])
+    sig, _ = oracle_mod.running_conductivity("vac", (rho * v2 * np.exp(-tf / tau))[:, None], None, dtf)
+    exact = rho * v2 * tau * (1.0 - np.exp(-tf / tau))
+    assert np.max(np.abs(sig[:, 0] - exact)) <= 2e-5 * exact[-1]         # trapezoid error ~ dt^2 / (12 tau^2)
+    assert abs(sig[-1, 0] / (rho * v2 * tau) - 1.0) < 1e-3               # -> sigma_sc = rho v^2 tau   (Eq. 8)
+    # the same physics through the MSD: rho dX^2 = 2 rho v^2 tau (t - tau (1 - exp(-t/tau)))  (d/2dt = sigma)
+    x2 = 2.0 * rho * v2 * tau * (tf[1:] - tau * (1.0 - np.exp(-tf[1:] / tau)))
+    sig_m, length = oracle_mod.running_conductivity("msd", x2[:, None], np.array([rho]), dtf)
+    mid = 0.5 * (tf[1:] + tf[:-1])
+    assert np.max(np.abs(sig_m[:, 0] - rho * v2 * tau * (1.0 - np.exp(-mid / tau)))) <= 2e-5 * exact[-1]
+    assert abs(x2[-1] / rho / (2.0 * tf[-1]) / (v2 * tau) - 1.0) < 0.15  # Einstein relation (Eq. 10), t = 8 tau
+    assert np.allclose(length[:, 0], 2.0 * np.sqrt(x2 / rho))
+    # sigma^VAC and sigma^MSD are the same function of time (PAPER.md:369): compare at the mid-steps
+    sig_v_mid = 0.5 * (sig[1:, 0] + sig[:-1, 0])
+    assert np.max(np.abs(sig_v_mid - sig_m[:, 0])) <= 1e-4 * exact[-1]
+
+
+def test_running_conductivity_on_a_lattice(oracle_mod):
+    """The two routes to sigma(E, t) agree on a clean periodic chain with a plane-wave state, where both
+    correlation functions are known exactly: rho C_vv = rho v_k^2, rho dX^2 = rho v_k^2 t^2."""
+    Lc, kq = 64, 5
+    model = L.chain(Lc, energy_scale=2.5)
+    k = 2 * np.pi * kq / Lc
+    phi = np.stack([np.cos(k * model.x), np.sin(k * model.x)], axis=1)[None]
+    o = oracle_mod.Oracle(model, batch=1, modes=oracle_mod.MODE_VAC | oracle_mod.MODE_MSD)
+    o.set_state(phi)
+    nm, dts = 64, [0.5, 0.5, 1.0]
+    E = np.array([-2.0 * np.cos(k)])                                      # eps_k for hopping -1
+    dos = o.kpm_transform(o.dos_moments(nm), E)[0]
+    vac_rows, msd_rows = [], []
+    for dt in dts:
+        vac_rows.append(o.kpm_transform(o.vac(nm), E)[0])
+        o.evolve(dt, 40)
+        msd_rows.append(o.kpm_transform(o.msd(nm), E)[0])
+    vac_rows.append(o.kpm_transform(o.vac(nm), E)[0])
+    sv, _ = oracle_mod.running_conductivity("vac", np.array(vac_rows), dos, np.array(dts))
+    sm, length = oracle_mod.running_conductivity("msd", np.array(msd_rows), dos, np.array(dts))
+    vk2 = (2.0 * np.sin(k)) ** 2
+    t = np.concatenate([[0.0], np.cumsum(dts)])
+    assert np.allclose(sv[:, 0], dos[0] * vk2 * t, rtol=1e-9)
+    assert np.allclose(sm[:, 0], dos[0] * vk2 * 0.5 * (t[1:] + t[:-1]), rtol=1e-9)
+    assert np.allclose(length[:, 0], 2.0 * np.sqrt(vk2) * t[1:], rtol=1e-9)
