@@ -137,6 +137,24 @@ int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_m
                         int32_t n_sets, const double* energies_host, int32_t n_energies,
                         double* out_host);
 
+/* Running conductivity sigma(E, t) in units e = 1 from the TRANSFORMED correlation functions
+ * (outputs of gpuqt_kpm_transform), one row per time (PAPER.md:81 Eq. 2, :92 Eq. 5, :123 Eq. 11;
+ * discretisation readings A25/A26 of DESIGN.md).  All arrays are host arrays.
+ *   kind = GPUQT_SIGMA_FROM_VAC: corr[k][j] = rho(E_j) C_vv(E_j, t_k) with t_k = sum_{i<k} dt_i
+ *          (measure, then evolve [A4]); dt has n_times - 1 entries;
+ *          sigma[k][j] = integral_0^{t_k} rho C_vv dt by the trapezoid rule (sigma[0] = 0).
+ *   kind = GPUQT_SIGMA_FROM_MSD: corr[k][j] = rho(E_j) dX^2(E_j, t_{k+1}) with t_{k+1} = sum_{i<=k} dt_i
+ *          (evolve, then measure), dX^2(0) = 0; dt has n_times entries;
+ *          sigma[k][j] = (corr[k][j] - corr[k-1][j]) / (2 dt_k), the running conductivity at the middle
+ *          of step k; length[k][j] = 2 sqrt(corr[k][j] / dos[j]) (Eq. 11; 0 where dos <= 0 or corr < 0).
+ * dos ([n_energies], Eq. 4) and length ([n_times][n_energies]) may be NULL.  Non-positive or
+ * non-finite time steps => GPUQT_ERR_ARG.                                                         */
+#define GPUQT_SIGMA_FROM_VAC 0
+#define GPUQT_SIGMA_FROM_MSD 1
+int gpuqt_running_conductivity(gpuqt_handle* h, int kind, const double* corr_host, const double* dos_host,
+                               const double* dt_host, int32_t n_times, int32_t n_energies, double* sigma_host,
+                               double* length_host);
+
 /* Copy a state back: host [batch][N][2].                                                          */
 int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host);
 

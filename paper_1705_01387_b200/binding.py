@@ -38,6 +38,7 @@ _SIGNATURES = {
     "gpuqt_vac": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_msd": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_kpm_transform": (C.c_int, [C.c_void_p, _dp, C.c_int32, C.c_int32, _dp, C.c_int32, _dp]),
+    "gpuqt_running_conductivity": (C.c_int, [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int32, C.c_int32, _dp, _dp]),
     "gpuqt_get_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "gpuqt_get_table": (C.c_int, [C.c_void_p, _ip, _dp, _dp, _dp]),
     "gpuqt_bessel_coeffs": (C.c_int, [C.c_double, C.c_double, C.c_int32, _dp, _dp]),
@@ -236,6 +237,19 @@ class GpuQT:
         self._ck(load().gpuqt_kpm_transform(self._h, _d(m2), C.c_int32(m2.shape[1]), C.c_int32(m2.shape[0]),
                                             _d(energies), C.c_int32(energies.size), _d(out)), "gpuqt_kpm_transform")
         return out
+
+    def running_conductivity(self, kind, corr, dos, dt):
+        """kind 'vac' or 'msd'; corr [n_t][n_E] from kpm_transform; returns (sigma, length or None)."""
+        corr = np.ascontiguousarray(corr, np.float64)
+        dt = np.ascontiguousarray(dt, np.float64)
+        dos = None if dos is None else np.ascontiguousarray(dos, np.float64)
+        n_t, n_e = corr.shape
+        sigma = np.empty_like(corr)
+        length = np.empty_like(corr) if (kind == "msd" and dos is not None) else None
+        self._ck(load().gpuqt_running_conductivity(self._h, 0 if kind == "vac" else 1, _d(corr), _d(dos), _d(dt),
+                                                   C.c_int32(n_t), C.c_int32(n_e), _d(sigma), _d(length)),
+                 "gpuqt_running_conductivity")
+        return sigma, length
 
     # ---- timing
     def kernel_stats(self, cls):

@@ -762,6 +762,38 @@ int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_m
     return GPUQT_OK;
 }
 
+int gpuqt_running_conductivity(gpuqt_handle* h, int kind, const double* corr_host, const double* dos_host,
+                               const double* dt_host, int32_t n_times, int32_t n_energies, double* sigma_host,
+                               double* length_host) {
+    if (!h || !corr_host || !dt_host || !sigma_host || n_times < 1 || n_energies < 1 ||
+        (kind != GPUQT_SIGMA_FROM_VAC && kind != GPUQT_SIGMA_FROM_MSD))
+        return fail(h, GPUQT_ERR_ARG, "null or non-positive argument");
+    const int n_dt = kind == GPUQT_SIGMA_FROM_VAC ? n_times - 1 : n_times;
+    for (int k = 0; k < n_dt; ++k)
+        if (!(dt_host[k] > 0.0) || !std::isfinite(dt_host[k])) return fail(h, GPUQT_ERR_ARG, "time steps must be positive");
+    const bool want_len = kind == GPUQT_SIGMA_FROM_MSD && length_host && dos_host;
+    const size_t bc = (size_t)n_times * n_energies * sizeof(double), be = (size_t)n_energies * sizeof(double),
+                 bt = (size_t)n_times * sizeof(double);
+    const size_t oc = 0, od = align_up(bc), ot = od + align_up(be), os = ot + align_up(bt), ol = os + align_up(bc),
+                 tot = ol + align_up(bc);
+    CU(ensure_scratch(h, tot));
+    char* s = h->scratch;
+    cudaError_t e = cudaMemcpyAsync(s + oc, corr_host, bc, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess && dos_host) e = cudaMemcpyAsync(s + od, dos_host, be, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess && n_dt > 0) e = cudaMemcpyAsync(s + ot, dt_host, (size_t)n_dt * sizeof(double), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+        conductivity_kernel<<<(n_energies + 127) / 128, 128, 0, h->stream>>>(
+            kind, n_times, n_energies, (const double*)(s + oc), dos_host ? (const double*)(s + od) : nullptr,
+            (const double*)(s + ot), (double*)(s + os), want_len ? (double*)(s + ol) : nullptr);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(sigma_host, s + os, bc, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && want_len) e = cudaMemcpyAsync(length_host, s + ol, bc, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "running_conductivity");
+    return GPUQT_OK;
+}
+
 int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host) {
     if (!h || !out_host) return fail(h, GPUQT_ERR_ARG, "null argument");
     const double2* src = which == GPUQT_STATE_PSI ? h->psi : which == GPUQT_STATE_CHI ? h->chi

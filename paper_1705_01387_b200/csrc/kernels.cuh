@@ -1145,6 +1145,37 @@ __global__ void transform_kernel(int n_moments, int n_sets, int n_energies, cons
     out[i] = pref * sum;
 }
 
+// Running conductivity (units e = 1) from the transformed correlation functions, one thread per
+// energy, a sequential walk over the time rows (PAPER.md:81 Eq. 2, :92 Eq. 5, :123 Eq. 11):
+//   kind 0  in[k][j] = rho C_vv(E_j, t_k), t_k = sum_{i<k} dt_i:  sigma[k][j] = trapezoid integral to t_k  [A25]
+//   kind 1  in[k][j] = rho dX^2(E_j, t_{k+1}), dX^2(0) = 0:        sigma[k][j] = (in[k] - in[k-1]) / (2 dt_k), the
+//           value at the middle of step k [A26];  length[k][j] = 2 sqrt(in[k][j] / dos[j])
+__global__ void conductivity_kernel(int kind, int n_t, int n_e, const double* __restrict__ in,
+                                    const double* __restrict__ dos, const double* __restrict__ dt,
+                                    double* __restrict__ sigma, double* __restrict__ length) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_e) return;
+    if (kind == 0) {
+        double acc = 0.0, before = in[j];
+        sigma[j] = 0.0;
+        for (int k = 1; k < n_t; ++k) {
+            const double now = in[(size_t)k * n_e + j];
+            acc += 0.5 * (before + now) * dt[k - 1];
+            sigma[(size_t)k * n_e + j] = acc;
+            before = now;
+        }
+    } else {
+        double before = 0.0;
+        const double rho = dos ? dos[j] : 0.0;
+        for (int k = 0; k < n_t; ++k) {
+            const double now = in[(size_t)k * n_e + j];
+            sigma[(size_t)k * n_e + j] = (now - before) / (2.0 * dt[k]);
+            if (length) length[(size_t)k * n_e + j] = 2.0 * sqrt((rho > 0.0 && now > 0.0) ? now / rho : 0.0);
+            before = now;
+        }
+    }
+}
+
 // Decode the packed records back to canonical padded row-major arrays (bit-exact check)
 __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __restrict__ re,
                              double* __restrict__ im, double* __restrict__ dx) {

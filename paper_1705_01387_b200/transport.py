@@ -1,0 +1,53 @@
+"""The paper's simulation loop on top of the C-ABI calls (PAPER.md:134-205 section 3, :343-347 the
+output rows, :359-409 the two examples): DOS, VAC and/or MSD at every time step on an energy grid,
+averaged over the B random vectors of the handle, and the running conductivities of Eq. 2 / Eq. 5.
+
+Call sequencing only -- every number is produced by libgpuqt.so's kernels (`engine` is a
+`binding.GpuQT`; anything with the same methods works, which is how the tests drive the oracle
+through the identical loop).
+"""
+import numpy as np
+
+
+def time_axis(dts):
+    """t_0 = 0, t_k = sum_{i<k} dt_i."""
+    return np.concatenate([[0.0], np.cumsum(np.asarray(dts, np.float64))])
+
+
+def run(engine, phi, dts, n_moments, energies, order_of, vac=True, msd=True):
+    """One pass of the method for the handle's B random vectors.
+
+    phi       host [B][N][2] random-phase vectors
+    dts       time steps (may be non-uniform)
+    order_of  callable dt -> N_p (number of Chebyshev terms of that step, [A5])
+    Row conventions [A4]: VAC row k is measured at t_k BEFORE step k (N_t rows, the last evolution of
+    the VAC branches is skipped only if MSD is off); MSD row k is measured at t_{k+1} AFTER step k.
+    Returns a dict of arrays averaged over the B vectors: dos [n_E], rho_vac / rho_msd [N_t][n_E]
+    (= rho C_vv, rho dX^2), sigma_vac (at t_k), sigma_msd (at the middle of step k), length (Eq. 11).
+    """
+    dts = np.asarray(dts, np.float64)
+    energies = np.ascontiguousarray(energies, np.float64)
+    engine.set_state(phi)
+    out = {"times": time_axis(dts), "energies": energies}
+    dos = engine.kpm_transform(engine.dos_moments(n_moments), energies).mean(axis=0)
+    out["dos"] = dos
+    vac_rows, msd_rows = [], []
+    for k, dt in enumerate(dts):
+        if vac:
+            vac_rows.append(engine.kpm_transform(engine.vac(n_moments), energies).mean(axis=0))
+        if msd or k + 1 < len(dts):
+            engine.evolve(float(dt), int(order_of(float(dt))))
+        if msd:
+            msd_rows.append(engine.kpm_transform(engine.msd(n_moments), energies).mean(axis=0))
+    if vac:
+        out["rho_vac"] = np.array(vac_rows)
+        out["sigma_vac"], _ = engine.running_conductivity("vac", out["rho_vac"], dos, dts[:len(dts) - 1])
+    if msd:
+        out["rho_msd"] = np.array(msd_rows)
+        out["sigma_msd"], out["length"] = engine.running_conductivity("msd", out["rho_msd"], dos, dts)
+    return out
+
+
+def semiclassical(sigma):
+    """sigma_sc(E) = max_t sigma(E, t)."""
+    return np.max(np.asarray(sigma), axis=0)

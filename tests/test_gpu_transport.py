@@ -1,0 +1,95 @@
+"""GPU parity of the post-processing step and of the paper's whole simulation loop:
+gpuqt_running_conductivity against the oracle, and transport.run on the CUDA library against the same
+loop driven through the oracle, on reduced-size versions of the paper's two examples
+(PAPER.md:359-409).  Tolerance: max |d| / max |ref| <= 1e-10 per output array (A22)."""
+import numpy as np
+import pytest
+
+from workloads import configs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gq():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1705_01387_b200 as g
+    return g
+
+
+class OracleEngine:
+    """The oracle behind the method names transport.run uses."""
+
+    def __init__(self, oracle_mod, model, batch, modes):
+        self.o = oracle_mod.Oracle(model, batch=batch, modes=modes)
+        self.mod = oracle_mod
+
+    def __getattr__(self, name):
+        return getattr(self.o, name)
+
+    def running_conductivity(self, kind, corr, dos, dt):
+        return self.mod.running_conductivity(kind, corr, dos, dt)
+
+
+def rel(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+def test_running_conductivity_parity(gq, oracle_mod):
+    from workloads import lattices as L
+    rng_ = np.random.default_rng(3)
+    g = gq.GpuQT(L.square(8, 8), batch=1, modes=0)
+    for n_t, n_e in ((1, 1), (7, 5), (30, 601), (20, 1000)):
+        corr = rng_.standard_normal((n_t, n_e)) ** 2
+        dos = rng_.random(n_e) + 0.1
+        dos[0] = 0.0                                                   # degenerate: no states at this energy
+        dt = rng_.random(n_t) + 0.05
+        for kind in ("vac", "msd"):
+            s_ref, l_ref = oracle_mod.running_conductivity(kind, corr, dos, dt)
+            s_got, l_got = g.running_conductivity(kind, corr, dos, dt)
+            assert rel(s_got, s_ref) <= 1e-14 or np.max(np.abs(s_ref)) == 0
+            if kind == "msd":
+                assert rel(l_got, l_ref) <= 1e-14
+                assert np.all(l_got[:, 0] == 0.0)
+    with pytest.raises(gq.GpuqtError):
+        g.running_conductivity("msd", np.ones((2, 2)), None, np.array([0.1, -0.1]))
+    g.close()
+
+
+@pytest.mark.parametrize("key,scale", [("e1", 0.04), ("e2", 0.0005)])
+def test_paper_examples_reduced(gq, oracle_mod, key, scale):
+    from paper_1705_01387_b200 import binding, transport
+    ex = configs.EXAMPLES[key]
+    model = ex.build(scale)                                             # e1: 80 x 80, e2: chain of 2000
+    dts = ex.dts[:8] if key == "e1" else ex.dts[:14]                   # oracle cost control
+    nm = 200
+    phi = ex.phases(model)
+    mg = (gq.MODE_VAC if ex.vac else 0) | (gq.MODE_MSD if ex.msd else 0)
+    mo = (oracle_mod.MODE_VAC if ex.vac else 0) | (oracle_mod.MODE_MSD if ex.msd else 0)
+    order_of = lambda dt: binding.choose_order(model.energy_scale, dt)
+    g = gq.GpuQT(model, batch=ex.batch, modes=mg)
+    got = transport.run(g, phi, dts, nm, ex.energies(), order_of, vac=ex.vac, msd=ex.msd)
+    ref = transport.run(OracleEngine(oracle_mod, model, ex.batch, mo), phi, dts, nm, ex.energies(), order_of,
+                        vac=ex.vac, msd=ex.msd)
+    for name in ("dos", "rho_vac", "sigma_vac", "rho_msd", "sigma_msd"):
+        if name in ref:
+            assert rel(got[name], ref[name]) <= TOL, name
+    if "length" in ref:
+        # L = 2 sqrt(rho dX^2 / rho) is a ratio: where the DOS vanishes (band tails, |E| -> dE) it divides two
+        # rounding-level numbers, so it is compared where it is conditioned, rho > 1e-3 max rho
+        ok = ref["dos"] > 1e-3 * np.max(ref["dos"])
+        assert rel(got["length"][:, ok], ref["length"][:, ok]) <= TOL
+    # what the paper says about its figures, on quantities that are exact for any size:
+    E = ex.energies()
+    assert abs(np.trapezoid(got["dos"], E) - 2.0) < 0.02                    # int rho dE = 2 per site (spin factor, Eq. 4)
+    if ex.msd:
+        j0 = int(np.argmin(np.abs(E)))
+        x2 = got["rho_msd"][:, j0] / got["dos"][j0]
+        t = transport.time_axis(dts)[1:]
+        assert np.all(np.diff(x2[:4]) > 0)                              # the MSD grows from zero ...
+        assert abs(x2[0] / t[0] ** 2 / (x2[1] / t[1] ** 2) - 1.0) < 0.2  # ... quadratically at short times (ballistic)
+    g.close()

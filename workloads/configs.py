@@ -71,3 +71,49 @@ def small_variant(key: str):
         "c4": lambda: L.cubic(20, W=16.5, seed=rng.stream_seed(4, 0), energy_scale=16.0),
         "c5": lambda: L.graphene_peierls_correlated(60, 32, config=5),
     }[key]()
+
+
+# ------------------------------------------------------------------ the paper's two examples (section 5)
+@dataclass
+class Example:
+    key: str
+    description: str
+    build: Callable[[float], "L.TBModel"]   # argument: linear scale factor (1.0 = the paper's size)
+    batch: int              # N_r
+    n_moments: int
+    dts: tuple              # time steps (hbar / gamma)
+    e_max: float            # energy grid -e_max .. e_max in steps of 0.02 gamma
+    vac: bool
+    msd: bool
+    config_id: int
+
+    def phases(self, model, first_vector=0):
+        return L.random_phase_vectors(model.N, self.batch, self.config_id, first_vector)
+
+    def energies(self):
+        import numpy as np
+        n = int(round(2 * self.e_max / 0.02)) + 1
+        return np.linspace(-self.e_max, self.e_max, n)
+
+
+def _e1(scale=1.0):
+    n = max(8, int(round(2000 * scale)))
+    return L.square(n, n, W=4.0, seed=rng.stream_seed(11, 0), energy_scale=6.1)
+
+
+def _e2(scale=1.0):
+    n = max(16, int(round(4000000 * scale)))
+    return L.chain(n, W=4.0, seed=rng.stream_seed(12, 0), energy_scale=4.1)
+
+
+EXAMPLES = {
+    # 2000 x 2000 square lattice, W = 4, periodic, dE = 6.1, N_m = 1000, N_r = 1,
+    # 20 steps of 0.2, energies -6 .. 6 step 0.02 (601 points), VAC and MSD
+    "e1": Example("e1", "paper example 5.1: 2D square lattice 2000^2, W=4, dE=6.1, N_m=1000, 20 x dt=0.2, VAC+MSD",
+                  _e1, 1, 1000, tuple([0.2] * 20), 6.0, True, True, 11),
+    # chain of 4e6 sites, W = 4, periodic, dE = 4.1, N_m = 500, N_r = 2, 30 growing steps
+    # 0.1 .. 1.0, 1 .. 10, 10 .. 100, energies -4 .. 4 step 0.02 (401 points), MSD only
+    "e2": Example("e2", "paper example 5.2: 1D chain 4e6, W=4, dE=4.1, N_m=500, N_r=2, 30 growing steps, MSD",
+                  _e2, 2, 500, tuple([0.1 * i for i in range(1, 11)] + [1.0 * i for i in range(1, 11)]
+                                     + [10.0 * i for i in range(1, 11)]), 4.0, False, True, 12),
+}
