@@ -68,7 +68,7 @@ typedef enum {
 /* kernel classes for gpuqt_kernel_stats */
 #define GPUQT_KERNEL_KPM_DOUBLING 0  /* fused SpMV + recurrence + 2 dots (DOS, MSD moments)       */
 #define GPUQT_KERNEL_KPM_LEFT 1      /* fused SpMV + recurrence + <phi_L|.> (VAC moments)         */
-#define GPUQT_KERNEL_EVOLVE 2        /* fused SpMV + recurrence + Bessel-weighted accumulate      */
+#define GPUQT_KERNEL_EVOLVE 2        /* fused SpMV + Clenshaw recurrence with the Bessel weights   */
 #define GPUQT_KERNEL_EVOLVE_MSD 3    /* the same for (psi, chi) with the [X,H~] walk fused in     */
 #define GPUQT_KERNEL_VELOCITY 4      /* V apply                                                   */
 #define GPUQT_KERNEL_CLASSES 5

@@ -361,33 +361,37 @@ void flush_stats(gpuqt_handle* h) {
 }
 
 // ---------------------------------------------------------------- building blocks
-// Driver of one three-term recurrence: terms m = 1 .. terms-1, T_m from T_{m-1}, T_{m-2} (and the
-// e-chain of the MSD pair).  Term 1 is a single-step launch (no T_{-1}, factor 1); after it two
-// consecutive terms share one launch when fusing is on (kernels.cuh, cheb_step_kernel).
-// fill(io, m) sets the per-term fields (coefficient, dot destination, store flag).
+// Driver of one three-term recurrence: launches m = 1 .. terms-1, each x_m = 2 H~ x_{m-1} - x_{m-2} (+ ...)
+// (and the e-chain of the MSD pair).  Launch 1 has no x_{-1}.  Forward recurrences (moments) apply
+// factor 1 in launch 1 (T_1 = H~ T_0); Clenshaw recurrences (evolution) apply factor 1 in the LAST
+// launch.  In between two consecutive terms share one launch when fusing is on (kernels.cuh,
+// cheb_pair_kernel).  fill(io, m) sets the per-term fields (coefficient, dot destination, store flag,
+// output override).
 template <class Fill>
 int run_recurrence(gpuqt_handle* h, int mode, int cls, int terms, const double2* t0, const double2* e0,
-                   const StepArgs& base, Fill fill) {
+                   const StepArgs& base, bool clenshaw, Fill fill) {
     StatScope s(h, cls);
     const double2 *tm1 = t0, *tm2 = nullptr, *em1 = e0, *em2 = nullptr;
     int slot = 0, m = 1;
     while (m < terms) {
         StepArgs a = base;
         a.first = (m == 1);
-        a.n_steps = (h->fuse && m >= 2 && m + 1 < terms) ? 2 : 1;
+        a.half = clenshaw ? (m == terms - 1) : (m == 1);
+        a.n_steps = (h->fuse && m >= 2 && m + 1 + (clenshaw ? 1 : 0) < terms) ? 2 : 1;
         for (int k = 0; k < a.n_steps; ++k) {
             StepIO& io = a.io[k];
             double2* tnew = h->ring[slot];
             io.in = tm1; io.prev = tm2; io.out = tnew;
-            tm2 = tm1; tm1 = tnew;
             if (e0) {
-                double2* enew = h->ringe[slot];
-                io.in_e = em1; io.prev_e = em2; io.out_e = enew;
-                em2 = em1; em1 = enew;
+                io.in_e = em1; io.prev_e = em2; io.out_e = h->ringe[slot];
             }
             slot = (slot + 1) % kRing;
             io.store = 1;
             fill(io, m + k);
+            tm2 = tm1; tm1 = io.out;
+            if (e0) {
+                em2 = em1; em1 = io.out_e;
+            }
         }
         CU(launch_step(h, mode, a));
         s.count(1, a.n_steps);
@@ -396,34 +400,53 @@ int run_recurrence(gpuqt_handle* h, int mode, int cls, int terms, const double2*
     return GPUQT_OK;
 }
 
-// out_vec <- sum_{m<order} c_m T_m(H~) in_vec   (Eq. 17, 21, 23), recurrence and accumulation in
-// one kernel.  `in` is left untouched; `out` must differ from in and from the ring buffers.
-int evolve_one(gpuqt_handle* h, const double2* in, double2* out, const std::vector<double>& cr,
-               const std::vector<double>& ci, int order) {
+cudaError_t launch_scale(gpuqt_handle* h, double cr, double ci, const double2* in, double2* out) {
+    const long long n = (long long)h->vec_elems;
+    scale_vec<<<(int)((n + 255) / 256), 256, 0, h->stream>>>(n, cr, ci, in, out);
+    return cudaGetLastError();
+}
+
+// out <- sum_{k<order} c_k T_k(H~) in  (Eq. 17, 21, 23) by Clenshaw's backward recurrence
+//   b_{order-1} = c_{order-1} in,  b_k = c_k in + 2 H~ b_{k+1} - b_{k+2},  out = c_0 in + H~ b_1 - b_2:
+// the same order - 1 SpMV launches as the forward form, but no accumulator is read-modified-written
+// (64 instead of 80 bytes per row and term).  The same for the (psi, chi) pair with the block operator
+// [[H~, 0], [[X,H~], H~]] (a_m = T_m psi, e_m = T_m chi + [X,T_m] psi, Eq. 18, 22, 24).
+// `in` is left untouched; `out` must differ from in and from the ring buffers.
+int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const double2* in_e, double2* out,
+                    double2* out_e, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
+    if (order == 1) {
+        CU(launch_scale(h, cr[0], ci[0], in, out));
+        if (in_e) CU(launch_scale(h, cr[0], ci[0], in_e, out_e));
+        return GPUQT_OK;
+    }
+    // b_{order-1} lives in the last ring slot: the recurrence writes slots 0, 1, 2, ... and needs it
+    // only in its first two launches
+    double2* b0 = h->ring[kRing - 1];
+    double2* b0_e = in_e ? h->ringe[kRing - 1] : nullptr;
+    CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in, b0));
+    if (in_e) CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in_e, b0_e));
     StepArgs base{};
-    base.acc = out;
-    base.c0r = cr[0]; base.c0i = ci[0];
-    const int terms = order < 2 ? 2 : order;   // order 1: U ~ c_0 -> the first-term kernel with c_1 = 0
-    return run_recurrence(h, kModeEvolve, GPUQT_KERNEL_EVOLVE, terms, in, nullptr, base, [&](StepIO& io, int m) {
-        io.cr = order < 2 ? 0.0 : cr[(size_t)m];
-        io.ci = order < 2 ? 0.0 : ci[(size_t)m];
-        io.store = (m + 1 < terms);
+    base.src = in;
+    base.src_e = in_e;
+    return run_recurrence(h, mode, cls, order, b0, b0_e, base, true, [&](StepIO& io, int m) {
+        const int k = order - 1 - m;            // this launch produces b_k
+        io.cr = cr[(size_t)k];
+        io.ci = ci[(size_t)k];
+        if (k == 0) {
+            io.out = out;
+            if (in_e) io.out_e = out_e;
+        }
     });
 }
 
-// (psi, chi) <- (U psi, U chi + [X,U] psi) with the fused e-recursion
-//   a_m = T_m psi, e_m = T_m chi + [X,T_m] psi:  e_m = 2 H~ e_{m-1} - e_{m-2} + 2 [X,H~] a_{m-1}
+int evolve_one(gpuqt_handle* h, const double2* in, double2* out, const std::vector<double>& cr,
+               const std::vector<double>& ci, int order) {
+    return evolve_clenshaw(h, kModeEvolve, GPUQT_KERNEL_EVOLVE, in, nullptr, out, nullptr, cr, ci, order);
+}
+
+// (psi, chi) <- (U psi, U chi + [X,U] psi)
 int evolve_msd_pair(gpuqt_handle* h, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
-    StepArgs base{};
-    base.acc = h->out0; base.acc_e = h->out1;
-    base.c0r = cr[0]; base.c0i = ci[0];
-    const int terms = order < 2 ? 2 : order;
-    int rc = run_recurrence(h, kModeEvolveMsd, GPUQT_KERNEL_EVOLVE_MSD, terms, h->psi, h->chi, base,
-                            [&](StepIO& io, int m) {
-                                io.cr = order < 2 ? 0.0 : cr[(size_t)m];
-                                io.ci = order < 2 ? 0.0 : ci[(size_t)m];
-                                io.store = (m + 1 < terms);
-                            });
+    int rc = evolve_clenshaw(h, kModeEvolveMsd, GPUQT_KERNEL_EVOLVE_MSD, h->psi, h->chi, h->out0, h->out1, cr, ci, order);
     if (rc) return rc;
     std::swap(h->psi, h->out0);
     std::swap(h->chi, h->out1);
@@ -434,7 +457,7 @@ int evolve_msd_pair(gpuqt_handle* h, const std::vector<double>& cr, const std::v
 int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
     const int n_steps = n_moments / 2;   // step j gives C_{2j+1}, C_{2j+2}
     StepArgs base{};
-    int rc = run_recurrence(h, kModeDoubling, GPUQT_KERNEL_KPM_DOUBLING, n_steps + 1, v, nullptr, base,
+    int rc = run_recurrence(h, kModeDoubling, GPUQT_KERNEL_KPM_DOUBLING, n_steps + 1, v, nullptr, base, false,
                             [&](StepIO& io, int m) {
                                 io.store = (m < n_steps);
                                 io.result = h->dots + (size_t)(m - 1) * 3 * h->B;
@@ -451,7 +474,7 @@ int moments_left(gpuqt_handle* h, const double2* l, const double2* r, int n_mome
     CU(launch_dot(h, l, r, h->dots));
     StepArgs base{};
     base.phiL = l;
-    int rc = run_recurrence(h, kModeLeft, GPUQT_KERNEL_KPM_LEFT, n_moments, r, nullptr, base, [&](StepIO& io, int n) {
+    int rc = run_recurrence(h, kModeLeft, GPUQT_KERNEL_KPM_LEFT, n_moments, r, nullptr, base, false, [&](StepIO& io, int n) {
         io.store = (n + 1 < n_moments);
         io.result = h->dots + (size_t)n * 2 * h->B;
     });

@@ -86,8 +86,8 @@ struct Mat {
 enum Mode : int {
     kModeDoubling = 0,   // T_new, dots |T_new|^2, Re<T_new|T_in>, |T_in|^2          (Eq. 28, 30)
     kModeLeft = 1,       // T_new, dot <phi_L|T_new>                                 (Eq. 29)
-    kModeEvolve = 2,     // T_new, acc += c T_new                                    (Eq. 17, 21)
-    kModeEvolveMsd = 3,  // (a, e) pair with the [X,H~] weights in the same walk     (Eq. 18, 22)
+    kModeEvolve = 2,     // Clenshaw term b_k = c_k src + 2 H~ b_{k+1} - b_{k+2}      (Eq. 17, 21)
+    kModeEvolveMsd = 3,  // the same for the (a, e) pair, [X,H~] weights in the walk (Eq. 18, 22)
 };
 
 // Operands of one recurrence step.  A launch performs one step, or two consecutive steps fused
@@ -107,11 +107,11 @@ struct StepIO {
 
 struct StepArgs {
     StepIO io[2];
-    double2* __restrict__ acc;           // evolve: sum_m c_m T_m
-    double2* __restrict__ acc_e;         // evolve MSD: sum_m c_m e_m
+    const double2* __restrict__ src;     // evolve: the vector being evolved (psi; a; b), read-only
+    const double2* __restrict__ src_e;   // evolve MSD: chi
     const double2* __restrict__ phiL;    // kModeLeft
-    double c0r, c0i;                     // c_0, used when first (acc = c_0 T_0 + c_1 T_1)
-    int first;                           // T_1 = H~ T_0 (no factor 2, no prev); single-step launches only
+    int first;                           // no T_{m-2} term (first launch of a recurrence); single-step launches only
+    int half;                            // factor 1 instead of 2 on H~ (T_1 = H~ T_0; last Clenshaw term); single-step only
     int n_steps;                         // 1, or 2 (fused pair, scheduled by `sched`)
     int reverse;                         // sweep the slices from the top (L2 reuse between launches)
     int run;                             // consecutive slices one CTA walks before jumping (multiple of kWarps)
@@ -469,10 +469,8 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
 
     // streamed read-modify-write operands: issued first, consumed last
     CV<V> other = cv_zero<V>(), other_e = cv_zero<V>();
-    if (!a.first) {
-        if (MODE == kModeEvolve || MSD) other = cv_ld_stream<V>(&a.acc[vi]);
-        if (MSD) other_e = cv_ld_stream<V>(&a.acc_e[vi]);
-    }
+    if (MODE == kModeEvolve || MSD) other = cv_ld_stream<V>(&a.src[vi]);
+    if (MSD) other_e = cv_ld_stream<V>(&a.src_e[vi]);
     if (MODE == kModeLeft) other = cv_ld_stream<V>(&a.phiL[vi]);
     double xm = 0.0;
     if (MSD) xm = m.x[row0 + (ok ? r : 0)];
@@ -537,7 +535,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     }
     const double hs = CONST ? scale * m.hop_const : scale;              // scale of the neighbour sums
     const double os = scale * on;                                       // scale of the on-site term
-    CV<V> t, te, acc, ae;   // T_m, e_m, and the accumulators
+    CV<V> t, te;   // T_m (b_k) and e_m
 #pragma unroll
     for (int q = 0; q < V; ++q) {
         t.re[q] = fma(hs, sum.re[q], fma(os, self.re[q], -prev.re[q]));
@@ -550,37 +548,20 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
             red[0 * V + q] += other.re[q] * t.re[q] + other.im[q] * t.im[q];
             red[1 * V + q] += other.re[q] * t.im[q] - other.im[q] * t.re[q];
         } else {
-            if (a.first) {
-                acc.re[q] = a.c0r * self.re[q] - a.c0i * self.im[q];
-                acc.im[q] = a.c0r * self.im[q] + a.c0i * self.re[q];
-            } else {
-                acc.re[q] = other.re[q];
-                acc.im[q] = other.im[q];
-            }
-            acc.re[q] += io.cr * t.re[q] - io.ci * t.im[q];
-            acc.im[q] += io.cr * t.im[q] + io.ci * t.re[q];
+            // Clenshaw: b_k = c_k src + 2 H~ b_{k+1} - b_{k+2}; no accumulator is read or written
+            t.re[q] += io.cr * other.re[q] - io.ci * other.im[q];
+            t.im[q] += io.cr * other.im[q] + io.ci * other.re[q];
             if (MSD) {
                 te.re[q] = fma(hs, sum_e.re[q] + sum_x.re[q], fma(os, self_e.re[q], -prev_e.re[q]));
                 te.im[q] = fma(hs, sum_e.im[q] + sum_x.im[q], fma(os, self_e.im[q], -prev_e.im[q]));
-                if (a.first) {
-                    ae.re[q] = a.c0r * self_e.re[q] - a.c0i * self_e.im[q];
-                    ae.im[q] = a.c0r * self_e.im[q] + a.c0i * self_e.re[q];
-                } else {
-                    ae.re[q] = other_e.re[q];
-                    ae.im[q] = other_e.im[q];
-                }
-                ae.re[q] += io.cr * te.re[q] - io.ci * te.im[q];
-                ae.im[q] += io.cr * te.im[q] + io.ci * te.re[q];
+                te.re[q] += io.cr * other_e.re[q] - io.ci * other_e.im[q];
+                te.im[q] += io.cr * other_e.im[q] + io.ci * other_e.re[q];
             }
         }
     }
-    if (ok) {
-        if (io.store) cv_st<V>(&io.out[vi], t);
-        if (MODE == kModeEvolve || MSD) cv_st<V>(&a.acc[vi], acc);
-        if (MSD) {
-            if (io.store) cv_st<V>(&io.out_e[vi], te);
-            cv_st<V>(&a.acc_e[vi], ae);
-        }
+    if (ok && io.store) {
+        cv_st<V>(&io.out[vi], t);
+        if (MSD) cv_st<V>(&io.out_e[vi], te);
     }
 }
 
@@ -682,7 +663,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     if (DOTS) {
         for (int i = lane; i < QB; i += 32) s_part[warp * QB + i] = 0.0;
     }
-    const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
+    const double scale = a.half ? m.inv_dE : 2.0 * m.inv_dE;
 
     const int N = (int)m.N, n_slices = (int)m.n_slices;
     const int per = a.run / kWarps;
@@ -946,7 +927,7 @@ __global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) c
         double red[Q * V];
 #pragma unroll
         for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
-        const double scale = a.first ? m.inv_dE : 2.0 * m.inv_dE;
+        const double scale = a.half ? m.inv_dE : 2.0 * m.inv_dE;
         int st = 0;
         uint32_t ph = 0;
         int red_step = 0;                   // step whose dots the register accumulators hold
@@ -1083,6 +1064,13 @@ __global__ void from_device_layout(long long N, int B, const double2* __restrict
     const long long row = i / B;
     const int b = (int)(i % B);
     dst[(size_t)b * N + row] = src[i];
+}
+// out = c * in (complex): the start b_{N_p-1} = c_{N_p-1} psi of the Clenshaw recurrence
+__global__ void scale_vec(long long n, double cr, double ci, const double2* __restrict__ in, double2* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double2 v = in[i];
+    out[i] = make_double2(cr * v.x - ci * v.y, cr * v.y + ci * v.x);
 }
 __global__ void zero_vec(long long n, double2* __restrict__ v) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
