@@ -211,7 +211,8 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items, int t
 // bytes of one stage of a step kernel: the record plus the staged own rows of T_{m-1}, T_{m-2}
 // (and e_{m-1}, e_{m-2} for the (a, e) pair)
 int mode_stage_bytes_for(const gpuqt_handle* h, int mode, bool pair = false) {
-    const int streams = (mode == kModeEvolveMsd) ? 4 : 2;
+    int streams = (mode == kModeEvolveMsd) ? 4 : 2;
+    if (h->B >= 8) streams /= 2;   // PrevDirect<8>: T_{m-2} rows are not staged
     return h->rec_bytes + streams * 32 * h->B * (int)sizeof(double2) + (pair ? kHdrBytes : 0);
 }
 

@@ -288,6 +288,14 @@ struct ModeTraits {
     static constexpr int kMinBlocks = (MODE == kModeEvolveMsd) ? GPUQT_MINB_MSD : GPUQT_MINB;   // register cap
 };
 
+// B = 8: a slice's rows are 4 KB per stream; staging T_{m-2} as well would leave room for one CTA per
+// SM only, so T_{m-2} own rows are read by a streaming 256-bit load at the top of the round instead
+// (the occupancy is worth more than the TMA staging there; at B <= 4 it is the other way round).
+template <int B>
+struct PrevDirect {
+    static constexpr bool value = (B >= 8);
+};
+
 // Number of vector streams staged per slice: own rows of T_{m-1}, T_{m-2} (x2 for the (a, e) pair).
 template <int MODE>
 struct StagedStreams {
@@ -474,6 +482,12 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     if (MODE == kModeLeft) other = cv_ld_stream<V>(&a.phiL[vi]);
     double xm = 0.0;
     if (MSD) xm = m.x[row0 + (ok ? r : 0)];
+    constexpr bool PD = PrevDirect<B>::value;
+    CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
+    if (PD && !a.first && ok) {         // rows past the end keep prev = 0 (their T_m must stay 0 for the dots)
+        prev = cv_ld_stream<V>(&io.prev[vi]);
+        if (MSD) prev_e = cv_ld_stream<V>(&io.prev_e[vi]);
+    }
 
     const CV<V> self = ok ? cv_lds<V>(s_in + si_) : cv_zero<V>();
     const CV<V> self_e = (MSD && ok) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
@@ -528,8 +542,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
             }
         }
     }
-    CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
-    if (!a.first && ok) {
+    if (!PD && !a.first && ok) {
         prev = cv_lds<V>(s_prev + si_);
         if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
     }
@@ -719,7 +732,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
         // constant-hopping padding entries point at it)
         const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-        const uint32_t total = bytes + vbytes_in * kPair + (a.first ? 0u : vbytes * kPair);
+        const uint32_t total = bytes + vbytes_in * kPair + ((a.first || PrevDirect<B>::value) ? 0u : vbytes * kPair);
         unsigned char* dst = wstage + c.st * stage_bytes;
         unsigned char* vdst = dst + a.rec_bytes;
         const size_t voff = (size_t)s * 32 * B;
@@ -727,7 +740,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
         bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[c.st]);
         if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &bars[c.st]);
-        if (!a.first) {
+        if (!a.first && !PrevDirect<B>::value) {
             bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &bars[c.st], policy);
             if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &bars[c.st], policy);
         }
@@ -891,7 +904,7 @@ __global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) c
                     // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
                     // constant-hopping padding entries point at it)
                     const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-                    const uint32_t total = bytes + vbytes_in * kPair + (a.first ? 0u : vbytes * kPair);
+                    const uint32_t total = bytes + vbytes_in * kPair + ((a.first || PrevDirect<B>::value) ? 0u : vbytes * kPair);
                     unsigned char* vdst = dst + a.rec_bytes;
                     const size_t voff = (size_t)s * 32 * B;
                     mbar_expect_tx(&my_full[st], total);
@@ -900,7 +913,7 @@ __global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) c
                     else bulk_g2s(dst, m.rec + off, bytes, &my_full[st], policy);
                     bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &my_full[st]);
                     if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &my_full[st]);
-                    if (!a.first) {
+                    if (!a.first && !PrevDirect<B>::value) {
                         bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &my_full[st], policy);
                         if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &my_full[st], policy);
                     }
