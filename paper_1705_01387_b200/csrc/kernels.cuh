@@ -475,7 +475,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     const int si_ = r * B + l * V;                                     // element inside the staged rows
     const size_t vi = (size_t)(row0 + (ok ? r : 0)) * B + l * V;       // element in global memory
 
-    // streamed read-modify-write operands: issued first, consumed last
+    // streamed own-row operands (evolved vector / phi_L): issued first, consumed last
     CV<V> other = cv_zero<V>(), other_e = cv_zero<V>();
     if (MODE == kModeEvolve || MSD) other = cv_ld_stream<V>(&a.src[vi]);
     if (MSD) other_e = cv_ld_stream<V>(&a.src_e[vi]);
