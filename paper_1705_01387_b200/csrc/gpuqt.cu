@@ -1,4 +1,5 @@
 // C-ABI of the B200-native GPUQT hot path (include/gpuqt.h): host logic + kernel launches.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -63,6 +64,9 @@ struct gpuqt_handle {
     // (stream-ordered pool allocations can trim at every synchronisation and stall the step)
     char* scratch = nullptr;
     size_t scratch_bytes = 0;
+    // B >= 2: one TMA tensor map (128-byte swizzle) per vector buffer, in device memory
+    std::vector<const double2*> map_bufs;
+    CUtensorMap* d_maps = nullptr;
     double *partials = nullptr, *dots = nullptr, *moments = nullptr;
     unsigned int* ticket = nullptr;
     int grid[8] = {0};                  // [mode + 4 * pair]
@@ -303,6 +307,43 @@ cudaError_t launch_dot(gpuqt_handle* h, const double2* l, const double2* r, doub
     return cudaLaunchKernel(fn, dim3(h->grid_aux), dim3(kThreads), args, 0, h->stream);
 }
 
+// device address of the tensor map of a vector buffer (nullptr at B = 1, where plain bulk copies are used)
+const void* tensor_map_of(const gpuqt_handle* h, const double2* buf) {
+    if (!h->d_maps || !buf) return nullptr;
+    for (size_t i = 0; i < h->map_bufs.size(); ++i)
+        if (h->map_bufs[i] == buf) return h->d_maps + i;
+    return nullptr;
+}
+
+// Tensor maps over the vector buffers: a buffer is seen as 128-byte lines (8 complex numbers; the last
+// line may reach into the buffer's zeroed alignment padding); one box = the 4 * B lines of one slice,
+// written to shared memory with the 128-byte swizzle; lines past the end are zero-filled.
+int build_tensor_maps(gpuqt_handle* h) {
+    if (h->B < 2) return GPUQT_OK;
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fp = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qres));
+    if (!fp || qres != cudaDriverEntryPointSuccess) return fail(h, GPUQT_ERR_CUDA, "cuTensorMapEncodeTiled is not available");
+    EncodeFn encode = (EncodeFn)fp;
+    std::vector<CUtensorMap> maps(h->map_bufs.size());
+    for (size_t i = 0; i < maps.size(); ++i) {
+        const cuuint64_t dims[2] = {16, ((cuuint64_t)(h->N + 1) * (cuuint64_t)h->B * 16 + 127) / 128};
+        const cuuint64_t strides[1] = {128};
+        const cuuint32_t box[2] = {16, (cuuint32_t)(4 * h->B)};
+        const cuuint32_t estr[2] = {1, 1};
+        CUresult r = encode(&maps[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)h->map_bufs[i], dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(h, GPUQT_ERR_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r));
+    }
+    CU(cudaMalloc((void**)&h->d_maps, maps.size() * sizeof(CUtensorMap)));
+    CU(cudaMemcpy(h->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+    return GPUQT_OK;
+}
+
 cudaError_t ensure_scratch(gpuqt_handle* h, size_t bytes) {
     if (bytes <= h->scratch_bytes) return cudaSuccess;
     cudaError_t e = cudaStreamSynchronize(h->stream);
@@ -388,6 +429,10 @@ int run_recurrence(gpuqt_handle* h, int mode, int cls, int terms, const double2*
             }
             slot = (slot + 1) % kRing;
             io.store = 1;
+            io.tm_in = tensor_map_of(h, io.in);
+            io.tm_prev = tensor_map_of(h, io.prev);
+            io.tm_in_e = tensor_map_of(h, io.in_e);
+            io.tm_prev_e = tensor_map_of(h, io.prev_e);
             fill(io, m + k);
             tm2 = tm1; tm1 = io.out;
             if (e0) {
@@ -590,7 +635,7 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     SellHost sell;
     build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, env_int("GPUQT_HOP_CONST", 1) != 0, sell);
     h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : kHopConst;
-    const int stage_bytes = (int)record_bytes(K_max, sell.nd);
+    const int stage_bytes = (int)align_up((size_t)record_bytes(K_max, sell.nd), 256);   // keeps the vector rows 256-byte aligned
     h->rec_bytes = stage_bytes;
     if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd, true), true) > kSmemBudget) {
         fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "
@@ -662,6 +707,7 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     auto nextv = [&]() {
         double2* p = (double2*)v;
         v += vstride;
+        h->map_bufs.push_back(p);
         return p;
     };
     h->psi = nextv(); h->out0 = nextv();
@@ -677,6 +723,12 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->dots = (double*)(base + L.dots);
     h->moments = (double*)(base + L.moments);
     h->ticket = (unsigned int*)(base + L.ticket);
+    rc = build_tensor_maps(h);
+    if (rc != GPUQT_OK) {
+        fprintf(stderr, "gpuqt_create: %s\n", h->err.c_str());
+        gpuqt_destroy(h);
+        return rc;
+    }
     *out = h;
     return GPUQT_OK;
 }
@@ -886,6 +938,7 @@ void gpuqt_destroy(gpuqt_handle* h) {
     flush_stats(h);
     for (auto e : h->free_events) cudaEventDestroy(e);
     if (h->scratch) cudaFree(h->scratch);
+    if (h->d_maps) cudaFree(h->d_maps);
     for (auto& d : h->schedules) {
         cudaFree(d.items);
         cudaFree(d.dep_ptr);

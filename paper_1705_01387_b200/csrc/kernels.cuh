@@ -99,6 +99,8 @@ struct StepIO {
     const double2* in_e;     // MSD pair: e_{m-1}
     const double2* prev_e;   //           e_{m-2}
     double2* out_e;          //           e_m
+    // B >= 2: device addresses of the TMA tensor maps (CUtensorMap, 128-byte swizzle) of in / prev / in_e / prev_e
+    const void *tm_in, *tm_prev, *tm_in_e, *tm_prev_e;
     double cr, ci;           // c_m
     double* result;          // [Q][B] reduced dots of this step
     int store;               // write T_m (0 on the last term of an evolve)
@@ -199,6 +201,28 @@ __device__ __forceinline__ void bulk_g2s_nohint(void* dst, const void* src, uint
         "l"(src), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
+
+// 2-D tiled TMA copy global -> shared through a tensor map (box = one slice's rows of one vector set as
+// 128-byte lines, 128-byte swizzle); completion is signalled on `bar`.  c1 = index of the first line.
+__device__ __forceinline__ void tensor_g2s(void* dst, const void* tmap, int c1, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::
+            "r"(smem_u32(dst)),
+        "l"(tmap), "r"(0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void tensor_g2s_hint(void* dst, const void* tmap, int c1, uint64_t* bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;" ::
+            "r"(smem_u32(dst)),
+        "l"(tmap), "r"(0), "r"(c1), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+// Staged vector rows are written by the TMA with the 128-byte swizzle (16-byte chunk index, address
+// bits 4-6, ^= address bits 7-9; box rows are whole 128-byte lines): a lane's two 16-byte reads at a
+// 32-byte lane stride then fall on distinct banks for every group of 8 lanes (without it: a 2-way
+// bank conflict on every 128-bit read).  Uses the absolute shared address, as the TMA does.
+__device__ __forceinline__ uint32_t swz32(uint32_t sa) { return sa ^ ((sa >> 3) & 0x70u); }
 
 __device__ __forceinline__ uint64_t policy_evict_last() {
     uint64_t p;
@@ -334,6 +358,21 @@ __device__ __forceinline__ CV<V> cv_lds(const double2* p) {
     }
     return v;
 }
+// shared memory written by a swizzled tensor copy: V consecutive double2 at shared address sa (V = 2)
+__device__ __forceinline__ CV<2> cv_lds_swz(uint32_t sa) {
+    const uint32_t p0 = swz32(sa);
+    CV<2> v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.re[0]), "=d"(v.im[0]) : "r"(p0));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.re[1]), "=d"(v.im[1]) : "r"(p0 ^ 16u));
+    return v;
+}
+template <int V>
+__device__ __forceinline__ CV<V> cv_lds_staged(const double2* p);
+template <>
+__device__ __forceinline__ CV<1> cv_lds_staged<1>(const double2* p) { return cv_lds<1>(p); }
+template <>
+__device__ __forceinline__ CV<2> cv_lds_staged<2>(const double2* p) { return cv_lds_swz(smem_u32(p)); }
+
 // global memory, read once (evict-first)
 template <int V>
 __device__ __forceinline__ CV<V> cv_ld_stream(const double2* p);
@@ -397,7 +436,8 @@ __device__ __forceinline__ CV<1> cv_gather<1>(const char* g_l, uint32_t s_l, int
 template <>
 __device__ __forceinline__ CV<2> cv_gather<2>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
-    const uint32_t sa = s_l + (uint32_t)(c * RB);
+    const uint32_t sa = swz32(s_l + (uint32_t)(c * RB));
+    const uint32_t sb = sa ^ 16u;
     const char* ga = g_l + (long long)c * RB;
     CV<2> v;
     asm volatile(
@@ -405,7 +445,7 @@ __device__ __forceinline__ CV<2> cv_gather<2>(const char* g_l, uint32_t s_l, int
         ".reg .pred p;\n"
         "setp.lt.u32 p, %6, 32;\n"
         "@p ld.shared.v2.f64 {%0, %1}, [%4];\n"
-        "@p ld.shared.v2.f64 {%2, %3}, [%4+16];\n"
+        "@p ld.shared.v2.f64 {%2, %3}, [%7];\n"
 #if GPUQT_GATHER_POLICY == 1
         "@!p ld.global.L2::evict_last.v4.f64 {%0, %1, %2, %3}, [%5];\n"
 #else
@@ -413,7 +453,7 @@ __device__ __forceinline__ CV<2> cv_gather<2>(const char* g_l, uint32_t s_l, int
 #endif
         "}"
         : "=d"(v.re[0]), "=d"(v.im[0]), "=d"(v.re[1]), "=d"(v.im[1])
-        : "r"(sa), "l"(ga), "r"(d));
+        : "r"(sa), "l"(ga), "r"(d), "r"(sb));
     return v;
 }
 
@@ -489,8 +529,8 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
         if (MSD) prev_e = cv_ld_stream<V>(&io.prev_e[vi]);
     }
 
-    const CV<V> self = ok ? cv_lds<V>(s_in + si_) : cv_zero<V>();
-    const CV<V> self_e = (MSD && ok) ? cv_lds<V>(s_in_e + si_) : cv_zero<V>();
+    const CV<V> self = ok ? cv_lds_staged<V>(s_in + si_) : cv_zero<V>();
+    const CV<V> self_e = (MSD && ok) ? cv_lds_staged<V>(s_in_e + si_) : cv_zero<V>();
     const double on = s_on[r];
 
     CV<V> sum = cv_zero<V>(), sum_e = cv_zero<V>(), sum_x = cv_zero<V>();   // H T, H e, [X,H] T (unscaled)
@@ -543,8 +583,8 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
         }
     }
     if (!PD && !a.first && ok) {
-        prev = cv_lds<V>(s_prev + si_);
-        if (MSD) prev_e = cv_lds<V>(s_prev_e + si_);
+        prev = cv_lds_staged<V>(s_prev + si_);
+        if (MSD) prev_e = cv_lds_staged<V>(s_prev_e + si_);
     }
     const double hs = CONST ? scale * m.hop_const : scale;              // scale of the neighbour sums
     const double os = scale * on;                                       // scale of the on-site term
@@ -662,7 +702,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     __shared__ double s_part[DOTS ? kWarps * QB : 1];
     const StepIO& io = a.io[0];
     constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
     const int stages = a.stages;
@@ -732,17 +772,32 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
         // constant-hopping padding entries point at it)
         const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-        const uint32_t total = bytes + vbytes_in * kPair + ((a.first || PrevDirect<B>::value) ? 0u : vbytes * kPair);
+        const bool with_prev = !a.first && !PrevDirect<B>::value;
         unsigned char* dst = wstage + c.st * stage_bytes;
         unsigned char* vdst = dst + a.rec_bytes;
-        const size_t voff = (size_t)s * 32 * B;
-        mbar_expect_tx(&bars[c.st], total);
-        bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
-        bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[c.st]);
-        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &bars[c.st]);
-        if (!a.first && !PrevDirect<B>::value) {
-            bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &bars[c.st], policy);
-            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &bars[c.st], policy);
+        if (B >= 2) {
+            // tensor copies: always the full 32-row box (rows past the end of the buffer are zero-filled)
+            const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
+            const int unit = s * 4 * B;           // first 128-byte line of the slice
+            mbar_expect_tx(&bars[c.st], total);
+            bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
+            tensor_g2s(vdst, io.tm_in, unit, &bars[c.st]);
+            if (MODE == kModeEvolveMsd) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &bars[c.st]);
+            if (with_prev) {
+                tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &bars[c.st], policy);
+                if (MODE == kModeEvolveMsd) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &bars[c.st], policy);
+            }
+        } else {
+            const uint32_t total = bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
+            const size_t voff = (size_t)s * 32 * B;
+            mbar_expect_tx(&bars[c.st], total);
+            bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
+            bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[c.st]);
+            if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &bars[c.st]);
+            if (with_prev) {
+                bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &bars[c.st], policy);
+                if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &bars[c.st], policy);
+            }
         }
     };
 
@@ -804,7 +859,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
 // An item depends only on earlier items of the list and every warp publishes what it owes before
 // it blocks, so the scheme cannot deadlock as long as all CTAs are co-resident (the grid is sized
 // by occupancy).
-constexpr int kHdrBytes = 128;                    // per stage: the slice header
+constexpr int kHdrBytes = 256;                    // per stage: the slice header (keeps the stages 256-byte aligned)
 constexpr int kFlagEnd = 1, kFlagOwesRelease = 2;
 
 template <int B, int KT, int HOP, int MODE>
@@ -814,7 +869,7 @@ __global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) c
     constexpr int RB = B * 16, QB = Q * B;
     constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
     constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ double s_part[DOTS ? kWarps * 2 * QB : 1];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
@@ -904,18 +959,30 @@ __global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) c
                     // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
                     // constant-hopping padding entries point at it)
                     const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-                    const uint32_t total = bytes + vbytes_in * kPair + ((a.first || PrevDirect<B>::value) ? 0u : vbytes * kPair);
+                    const bool with_prev = !a.first && !PrevDirect<B>::value;
+                    const uint32_t total = B >= 2 ? bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u)
+                                                  : bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
                     unsigned char* vdst = dst + a.rec_bytes;
                     const size_t voff = (size_t)s * 32 * B;
+                    const int unit = s * 4 * B;           // first 128-byte line of the slice (tensor copies, B >= 2)
                     mbar_expect_tx(&my_full[st], total);
                     // the first step of a fused pair leaves the record in L2 for the second one
                     if (fused && step == 0) bulk_g2s_nohint(dst, m.rec + off, bytes, &my_full[st]);
                     else bulk_g2s(dst, m.rec + off, bytes, &my_full[st], policy);
-                    bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &my_full[st]);
-                    if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &my_full[st]);
-                    if (!a.first && !PrevDirect<B>::value) {
-                        bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &my_full[st], policy);
-                        if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &my_full[st], policy);
+                    if (B >= 2) {
+                        tensor_g2s(vdst, io.tm_in, unit, &my_full[st]);
+                        if (MODE == kModeEvolveMsd) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &my_full[st]);
+                        if (with_prev) {
+                            tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &my_full[st], policy);
+                            if (MODE == kModeEvolveMsd) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &my_full[st], policy);
+                        }
+                    } else {
+                        bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &my_full[st]);
+                        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &my_full[st]);
+                        if (with_prev) {
+                            bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &my_full[st], policy);
+                            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &my_full[st], policy);
+                        }
                     }
                     if (++st == stages) {
                         st = 0;
