@@ -248,6 +248,10 @@ def run_ours(args, w):
             model.hop_re.reshape(model.N, model.K)[np.arange(model.K)[None, :] < model.nbr_count[:, None]]).size <= 1)
         hop_const = hop_const and os.environ.get("GPUQT_HOP_CONST", "1") != "0"
         stored_row_launch = per_row_launch - (8 * model.K if hop_const else 0)
+        # ... and 16-bit columns (base + delta) when the table is uniform, unpadded and N % 32 == 0
+        if (hop_const and model.K in (3, 4, 6) and model.N % 32 == 0 and int(model.nbr_count.min()) == model.K
+                and os.environ.get("GPUQT_IDX16", "1") != "0"):
+            stored_row_launch -= 2 * model.K - 1
         dom_ms, dom_n = stats[dom]
         achieved = per_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9
         peak, peak_src = load_peak()

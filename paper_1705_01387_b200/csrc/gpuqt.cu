@@ -148,6 +148,9 @@ bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
 // ---------------------------------------------------------------- kernel dispatch
 template <int MODE, int BB, int KK>
 void* step_fn(int hop, bool pair) {
+    if (KK > 0 && hop == kHopConst16)      // 16-bit columns exist for the unrolled uniform tables only
+        return pair ? (void*)cheb_pair_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>
+                    : (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>;
     if (pair)
         return hop == kHopComplex ? (void*)cheb_pair_kernel<BB, KK, kHopComplex, MODE>
                : hop == kHopConst ? (void*)cheb_pair_kernel<BB, KK, kHopConst, MODE>
@@ -634,8 +637,10 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
 
     SellHost sell;
     build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, env_int("GPUQT_HOP_CONST", 1) != 0, sell);
-    h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : kHopConst;
-    const int stage_bytes = (int)align_up((size_t)record_bytes(K_max, sell.nd), 256);   // keeps the vector rows 256-byte aligned
+    // 16-bit columns: only where the unrolled uniform kernels exist (K_max 3, 4, 6)
+    if (env_int("GPUQT_IDX16", 1) != 0 && (K_max == 3 || K_max == 4 || K_max == 6)) try_idx16(sell, K_max);
+    h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : sell.idx16 ? kHopConst16 : kHopConst;
+    const int stage_bytes = (int)align_up((size_t)hop_record_bytes(K_max, h->hop), 256);   // keeps the vector rows 256-byte aligned
     h->rec_bytes = stage_bytes;
     if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd, true), true) > kSmemBudget) {
         fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "

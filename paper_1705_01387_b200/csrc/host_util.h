@@ -103,12 +103,20 @@ struct SellHost {
     int uniform = 1;                    // every record has width K_max
     int nd = 1;                         // doubles per entry: 0 constant hopping, 1 real, 2 complex
     double hop_const = 0.0;
+    int idx16 = 0;                      // constant hopping with 16-bit columns (see try_idx16)
     std::vector<int> nbr_ptr, nbr_slices;   // CSR over slices: the slices a slice gathers from (sorted, itself included)
     std::vector<long long> slice_off;   // [n_slices + 1] byte offsets of the records
     std::vector<unsigned char> rec;
 };
 
 inline long long host_record_bytes(int w, int nd) { return 32LL * (8LL * w * nd + 8 + 4LL * w); }
+
+// Re-encode a uniform constant-hopping table (records: onsite[32] | int32 col[K][32]) with 16-bit
+// columns: record = double onsite[32] | int32 base[8] | uint16 delta[K][32], col = base[k] + delta.
+// Possible when K <= 8 and, inside every (slice, k), the columns spread less than 65536 (padding
+// entries, col = N, included).  Returns false and leaves the table untouched otherwise.
+struct SellHost;
+inline bool try_idx16(SellHost& s, int K);
 
 // true (and the value) if hop_im is absent and all listed hoppings carry the same bit pattern
 inline bool constant_hopping(int64_t N, int32_t K, const int32_t* cnt, const double* hre, const double* him,
@@ -311,4 +319,34 @@ inline void bessel_coeffs(double dE, double dt, int order, std::vector<double>& 
     }
 }
 
+}  // namespace gpuqt
+
+namespace gpuqt {
+inline bool try_idx16(SellHost& s, int K) {
+    if (s.nd != 0 || !s.uniform || K > 8) return false;
+    const size_t old_bytes = 256 + 128 * (size_t)K, new_bytes = 288 + 64 * (size_t)K;
+    std::vector<unsigned char> out((size_t)s.n_slices * new_bytes, 0);
+    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+        const unsigned char* src = s.rec.data() + (size_t)sl * old_bytes;
+        unsigned char* dst = out.data() + (size_t)sl * new_bytes;
+        std::memcpy(dst, src, 256);                                            // onsite
+        const int32_t* col = reinterpret_cast<const int32_t*>(src + 256);
+        int32_t* base = reinterpret_cast<int32_t*>(dst + 256);
+        uint16_t* delta = reinterpret_cast<uint16_t*>(dst + 288);
+        for (int k = 0; k < K; ++k) {
+            int32_t lo = col[k * 32], hi = col[k * 32];
+            for (int lane = 1; lane < 32; ++lane) {
+                lo = std::min(lo, col[k * 32 + lane]);
+                hi = std::max(hi, col[k * 32 + lane]);
+            }
+            if ((int64_t)hi - lo > 65535) return false;
+            base[k] = lo;
+            for (int lane = 0; lane < 32; ++lane) delta[k * 32 + lane] = (uint16_t)(col[k * 32 + lane] - lo);
+        }
+    }
+    s.rec.swap(out);
+    for (int64_t sl = 0; sl <= s.n_slices; ++sl) s.slice_off[(size_t)sl] = (long long)((size_t)sl * new_bytes);
+    s.idx16 = 1;
+    return true;
+}
 }  // namespace gpuqt

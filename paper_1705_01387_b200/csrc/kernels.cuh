@@ -65,8 +65,16 @@ __host__ __device__ __forceinline__ long long record_bytes(int w, int nd) {
 __host__ __device__ __forceinline__ int record_width(long long bytes, int nd) {
     return (int)((bytes / 32 - 8) / (4 + 8 * nd));
 }
-enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2 };
-__host__ __device__ constexpr int hop_doubles(int hop) { return hop == kHopConst ? 0 : hop == kHopComplex ? 2 : 1; }
+// kHopConst16: constant hopping AND 16-bit columns -- the record is
+//     double onsite[32] | int32 base[8] (first w used) | uint16 delta[w][32],   col = base[k] + delta[k][lane]
+// (uniform tables without padding whose columns spread less than 65536 inside every (slice, k); lattices
+// in natural order do).  288 + 64 w bytes instead of 256 + 128 w.
+enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2, kHopConst16 = 3 };
+__host__ __device__ constexpr bool hop_is_const(int hop) { return hop == kHopConst || hop == kHopConst16; }
+__host__ __device__ constexpr int hop_doubles(int hop) { return hop_is_const(hop) ? 0 : hop == kHopComplex ? 2 : 1; }
+__host__ __device__ __forceinline__ long long hop_record_bytes(int w, int hop) {
+    return hop == kHopConst16 ? 288LL + 64LL * w : record_bytes(w, hop_doubles(hop));
+}
 
 struct Mat {
     const unsigned char* __restrict__ rec;      // packed slice records
@@ -493,12 +501,13 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     constexpr int KU = KT > 0 ? KT : 1;
     constexpr int RB = B * 16;   // bytes of one row of a vector set
     constexpr bool MSD = (MODE == kModeEvolveMsd);
-    constexpr bool CPLX = (HOP == kHopComplex), CONST = (HOP == kHopConst);
+    constexpr bool CPLX = (HOP == kHopComplex), CONST = hop_is_const(HOP), IDX16 = (HOP == kHopConst16);
     const int rl = lane / LPR, l = lane % LPR;
     const double* s_hre = reinterpret_cast<const double*>(stage);
     const double* s_him = s_hre + w * 32;
     const double* s_on = s_hre + w * 32 * hop_doubles(HOP);
-    const int* s_col = reinterpret_cast<const int*>(s_on + 32);
+    const int* s_col = reinterpret_cast<const int*>(s_on + 32);                        // int32 columns, or base[8]
+    const unsigned short* s_d16 = reinterpret_cast<const unsigned short*>(s_col + 8);   // kHopConst16: deltas
     // staged vector rows: [in | (in_e) | prev | (prev_e)], each 32 * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
     const double2* s_in_e = s_in + 32 * B;
@@ -540,7 +549,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
         double xn[MSD ? KU : 1];
 #pragma unroll
         for (int k = 0; k < KU; ++k) {
-            const int c = s_col[k * 32 + r];
+            const int c = IDX16 ? s_col[k] + (int)s_d16[k * 32 + r] : s_col[k * 32 + r];
             v[k] = cv_gather<V>(gl_in, sl_in, c, row0, RB);
             if (MSD) {
                 ve[k] = cv_gather<V>(gl_in_e, sl_in_e, c, row0, RB);
@@ -566,7 +575,7 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
     } else {
         if (signal && lane == 0) red_release_gpu_inc(signal);
         for (int k = 0; k < w; ++k) {
-            const int c = s_col[k * 32 + r];
+            const int c = IDX16 ? s_col[k] + (int)s_d16[k * 32 + r] : s_col[k * 32 + r];
             double hr = 1.0, hi = 0.0;
             if (!CONST) hr = s_hre[k * 32 + r];
             if (CPLX) hi = s_him[k * 32 + r];
@@ -761,7 +770,7 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
         long long off;
         uint32_t bytes;
         if (KT > 0) {
-            bytes = (uint32_t)record_bytes(KT, hop_doubles(HOP));
+            bytes = (uint32_t)hop_record_bytes(KT, HOP);
             off = (long long)s * bytes;
         } else {
             off = m.slice_off[s];
@@ -948,7 +957,7 @@ __global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) c
                     long long off;
                     uint32_t bytes;
                     if (KT > 0) {
-                        bytes = (uint32_t)record_bytes(KT, hop_doubles(HOP));
+                        bytes = (uint32_t)hop_record_bytes(KT, HOP);
                         off = (long long)s * bytes;
                     } else {
                         off = m.slice_off[s];
@@ -1056,25 +1065,30 @@ struct RecView {
     const double* hre;
     const double* him;
     const double* on;
-    const int* col;
+    const int* col;                  // int32 columns, or base[8] of the 16-bit variant
+    const unsigned short* d16;       // 16-bit variant: deltas, else nullptr
     int w;
+    __device__ __forceinline__ int col_at(int k, int r) const {
+        return d16 ? col[k] + (int)d16[k * 32 + r] : col[k * 32 + r];
+    }
 };
 __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
     long long off, bytes;
     const int nd = hop_doubles(m.hop);
     if (m.uniform) {
-        bytes = record_bytes(m.K, nd);
+        bytes = hop_record_bytes(m.K, m.hop);
         off = slice * bytes;
     } else {
         off = m.slice_off[slice];
         bytes = m.slice_off[slice + 1] - off;
     }
     RecView v;
-    v.w = record_width(bytes, nd);
+    v.w = m.hop == kHopConst16 ? m.K : record_width(bytes, nd);     // the 16-bit variant is always uniform
     v.hre = reinterpret_cast<const double*>(m.rec + off);
     v.him = v.hre + (size_t)v.w * 32;
     v.on = v.hre + (size_t)v.w * 32 * nd;
     v.col = reinterpret_cast<const int*>(v.on + 32);
+    v.d16 = m.hop == kHopConst16 ? reinterpret_cast<const unsigned short*>(v.col + 8) : nullptr;
     return v;
 }
 
@@ -1094,8 +1108,8 @@ __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const d
         const double xm = m.x[row];
         double sr = 0.0, si = 0.0;
         for (int k = 0; k < rv.w; ++k) {
-            const int c = rv.col[k * 32 + r];               // constant-hopping padding: the zero row N
-            const double hr = (m.hop == kHopConst) ? m.hop_const : rv.hre[k * 32 + r];
+            const int c = rv.col_at(k, r);                  // constant-hopping padding: the zero row N
+            const double hr = hop_is_const(m.hop) ? m.hop_const : rv.hre[k * 32 + r];
             const double dx = min_image(m.x[c] - xm, m.box);
             const double wr = dx * hr;
             const double2 v = in[(size_t)c * B + b];
@@ -1256,8 +1270,8 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
     int c = (int)row;
     double hr = 0.0, hi = 0.0, d = 0.0;
     if (k < rv.w) {
-        c = rv.col[k * 32 + r];
-        if (m.hop == kHopConst) {
+        c = rv.col_at(k, r);
+        if (hop_is_const(m.hop)) {
             hr = c < m.N ? m.hop_const : 0.0;
             c = c < m.N ? c : (int)row;
         } else {

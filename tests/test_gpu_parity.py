@@ -49,6 +49,10 @@ def small_models():
         ("square_bonddis", L.with_bond_disorder(L.square(52, 33, W=1.0, seed=13), 0.5, 21)),
         ("graphene_vac_bonddis", L.with_bond_disorder(L.graphene(23, 17, vacancy_fraction=0.05, vacancy_seed=4), 0.3, 22)),
         ("cubic_bonddis", L.with_bond_disorder(L.cubic(11, W=8.0, seed=14, energy_scale=11.0), 0.2, 23)),
+        # N a multiple of 32, no padding, constant hopping: stored with 16-bit columns (kHopConst16)
+        ("square_idx16", L.square(64, 32, W=2.0, seed=15)),
+        ("cubic_idx16", L.cubic(16, W=16.5, seed=16, energy_scale=16.0)),
+        ("graphene_idx16", L.graphene(16, 8, W=1.0, seed=17)),
     ]
 
 
@@ -309,3 +313,30 @@ def test_two_steps_per_launch(gq, oracle_mod, monkeypatch, env):
             assert np.max(np.abs(g.msd(30) - o.msd(30)) / (norms(chi) ** 2)[:, None]) <= TOL
         g.close()
         o.close()
+
+
+def test_16bit_columns_match_32bit(gq, oracle_mod, monkeypatch):
+    """The same table stored with 16-bit (base + delta) and with 32-bit columns decodes to the same
+    canonical table and gives the same moments / vectors."""
+    model = L.cubic(16, W=16.5, seed=16, energy_scale=16.0)
+    phi = L.random_phase_vectors(model.N, 4, config=60)
+    o = oracle_mod.Oracle(model, batch=4, modes=oracle_mod.MODE_MSD | oracle_mod.MODE_VAC)
+    o.set_state(phi)
+    ref_tab, ref_dos, ref_vac = o.get_table(), o.dos_moments(48), o.vac(48)
+    o.evolve(1.0, 44)
+    ref_chi = o.get_state(oracle_mod.CHI)
+    outs = []
+    for flag in ("1", "0"):
+        monkeypatch.setenv("GPUQT_IDX16", flag)
+        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC)
+        for a, b in zip(g.get_table(), ref_tab):
+            assert a.tobytes() == b.tobytes()
+        g.set_state(phi)
+        dos = g.dos_moments(48)
+        assert np.max(np.abs(dos - ref_dos)) / model.N <= TOL
+        assert np.max(np.abs(g.vac(48) - ref_vac)) / np.max(np.abs(ref_vac[:, 0])) <= TOL
+        g.evolve(1.0, 44)
+        assert vec_err(g.get_state(gq.STATE_CHI), ref_chi) <= TOL
+        outs.append(dos.copy())
+        g.close()
+    assert outs[0].tobytes() == outs[1].tobytes()        # same arithmetic, only the column encoding differs
