@@ -605,7 +605,8 @@ __device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, cons
         if (MODE == kModeDoubling) {
             red[0 * V + q] += t.re[q] * t.re[q] + t.im[q] * t.im[q];
             red[1 * V + q] += t.re[q] * self.re[q] + t.im[q] * self.im[q];
-            red[2 * V + q] += self.re[q] * self.re[q] + self.im[q] * self.im[q];
+            // <T_{m-1}|T_{m-1}> is only used from the first launch (C_0); later ones had it as <T_m|T_m>
+            if (a.first) red[2 * V + q] += self.re[q] * self.re[q] + self.im[q] * self.im[q];
         } else if (MODE == kModeLeft) {   // conj(l) * t
             red[0 * V + q] += other.re[q] * t.re[q] + other.im[q] * t.im[q];
             red[1 * V + q] += other.re[q] * t.im[q] - other.im[q] * t.re[q];
@@ -1172,7 +1173,7 @@ __global__ void zero_vec(long long n, double2* __restrict__ v) {
 }
 
 // Doubling identity (T_2m = 2 T_m^2 - 1, T_2m+1 = 2 T_m+1 T_m - T_1):
-// dots[j] = {<a_{j+1}|a_{j+1}>, Re<a_{j+1}|a_j>, <a_j|a_j>}[B]  ->  C[b][n]
+// dots[j] = {<a_{j+1}|a_{j+1}>, Re<a_{j+1}|a_j>, <a_j|a_j> (j = 0 only)}[B]  ->  C[b][n]
 //   C_0 = <a_0|a_0>, C_1 = <a_1|a_0>, C_{2j+2} = 2<a_{j+1}|a_{j+1}> - C_0, C_{2j+1} = 2<a_{j+1}|a_j> - C_1
 __global__ void finalize_doubling(int B, int n_moments, int n_steps, const double* __restrict__ dots,
                                   double* __restrict__ C) {
