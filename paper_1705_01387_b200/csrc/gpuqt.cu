@@ -464,16 +464,22 @@ cudaError_t launch_scale(gpuqt_handle* h, double cr, double ci, const double2* i
 int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const double2* in_e, double2* out,
                     double2* out_e, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
     if (order == 1) {
+        StatScope s(h, cls);
         CU(launch_scale(h, cr[0], ci[0], in, out));
         if (in_e) CU(launch_scale(h, cr[0], ci[0], in_e, out_e));
+        s.count(in_e ? 2 : 1, 0);
         return GPUQT_OK;
     }
     // b_{order-1} lives in the last ring slot: the recurrence writes slots 0, 1, 2, ... and needs it
     // only in its first two launches
     double2* b0 = h->ring[kRing - 1];
     double2* b0_e = in_e ? h->ringe[kRing - 1] : nullptr;
-    CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in, b0));
-    if (in_e) CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in_e, b0_e));
+    {
+        StatScope s(h, cls);       // counted as launches of the class, not as recurrence steps
+        CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in, b0));
+        if (in_e) CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in_e, b0_e));
+        s.count(in_e ? 2 : 1, 0);
+    }
     StepArgs base{};
     base.src = in;
     base.src_e = in_e;
