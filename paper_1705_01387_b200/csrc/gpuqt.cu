@@ -51,6 +51,7 @@ struct gpuqt_handle {
     double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr, nullptr},
             *ringe[kRing] = {nullptr, nullptr, nullptr, nullptr};
     // fused pairs of steps: dependency structure of the table and the cached work lists
+    int small = 1;                      // GPUQT_SMALL: one-CTA whole-recurrence kernel when everything fits one SM
     int fuse = 1, lag = 2;              // GPUQT_FUSE, GPUQT_LAG (slack of the second step in half rounds)
     std::vector<int> nbr_ptr, nbr_slices;
     struct DevSchedule {
@@ -406,6 +407,36 @@ void flush_stats(gpuqt_handle* h) {
 }
 
 // ---------------------------------------------------------------- building blocks
+// ---- small lattices: the whole recurrence in one launch of one CTA (kernels.cuh, cheb_small_kernel)
+size_t small_smem_bytes(const gpuqt_handle* h) {
+    const size_t NB = (size_t)h->N * h->B, KN = (size_t)h->K * h->N;
+    return 4 * NB * sizeof(double2) + (size_t)h->N * 8 + KN * 8 * (size_t)hop_doubles(h->hop) + KN * 4 + 16;
+}
+bool small_ok(const gpuqt_handle* h) { return h->small && small_smem_bytes(h) <= 210 * 1024; }
+
+template <int MODE>
+void* small_fn(int B) {
+    switch (B) {
+    case 1: return (void*)cheb_small_kernel<1, MODE>;
+    case 2: return (void*)cheb_small_kernel<2, MODE>;
+    case 4: return (void*)cheb_small_kernel<4, MODE>;
+    default: return (void*)cheb_small_kernel<8, MODE>;
+    }
+}
+cudaError_t launch_small(gpuqt_handle* h, int mode, SmallArgs& a) {
+    void* fn = mode == kModeDoubling ? small_fn<kModeDoubling>(h->B)
+               : mode == kModeLeft   ? small_fn<kModeLeft>(h->B)
+                                     : small_fn<kModeEvolve>(h->B);
+    const size_t smem = small_smem_bytes(h);
+    if (std::find(h->smem_set.begin(), h->smem_set.end(), fn) == h->smem_set.end()) {
+        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        h->smem_set.push_back(fn);
+    }
+    void* args[] = {(void*)&h->mat, (void*)&a};
+    return cudaLaunchKernel(fn, dim3(1), dim3(kSmallThreads), args, smem, h->stream);
+}
+
 // Driver of one three-term recurrence: launches m = 1 .. terms-1, each x_m = 2 H~ x_{m-1} - x_{m-2} (+ ...)
 // (and the e-chain of the MSD pair).  Launch 1 has no x_{-1}.  Forward recurrences (moments) apply
 // factor 1 in launch 1 (T_1 = H~ T_0); Clenshaw recurrences (evolution) apply factor 1 in the LAST
@@ -463,6 +494,20 @@ cudaError_t launch_scale(gpuqt_handle* h, double cr, double ci, const double2* i
 // `in` is left untouched; `out` must differ from in and from the ring buffers.
 int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const double2* in_e, double2* out,
                     double2* out_e, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
+    if (!in_e && small_ok(h) && (size_t)order * 2 <= (size_t)GPUQT_MAX_MOMENTS * 8) {
+        std::vector<double> c((size_t)order * 2);
+        for (int k = 0; k < order; ++k) {
+            c[(size_t)2 * k] = cr[(size_t)k];
+            c[(size_t)2 * k + 1] = ci[(size_t)k];
+        }
+        CU(cudaMemcpyAsync(h->moments, c.data(), c.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        SmallArgs a{};
+        a.aux = in; a.out = out; a.coef = (const double2*)h->moments; a.n_terms = order;
+        StatScope s(h, cls);
+        CU(launch_small(h, kModeEvolve, a));
+        s.count(1, order > 1 ? order - 1 : 0);
+        return GPUQT_OK;
+    }
     if (order == 1) {
         StatScope s(h, cls);
         CU(launch_scale(h, cr[0], ci[0], in, out));
@@ -511,6 +556,19 @@ int evolve_msd_pair(gpuqt_handle* h, const std::vector<double>& cr, const std::v
 // moments with the doubling identity: C_n = <v|T_n|v>, n < n_moments  -> h->moments [B][n]
 int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
     const int n_steps = n_moments / 2;   // step j gives C_{2j+1}, C_{2j+2}
+    if (small_ok(h)) {
+        SmallArgs a{};
+        a.v0 = v; a.dots = h->dots; a.n_terms = n_steps + 1;
+        {
+            StatScope s(h, GPUQT_KERNEL_KPM_DOUBLING);
+            CU(launch_small(h, kModeDoubling, a));
+            s.count(1, n_steps);
+        }
+        const int total = h->B * n_moments;
+        finalize_doubling<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, n_steps, h->dots, h->moments);
+        CU(cudaGetLastError());
+        return GPUQT_OK;
+    }
     StepArgs base{};
     int rc = run_recurrence(h, kModeDoubling, GPUQT_KERNEL_KPM_DOUBLING, n_steps + 1, v, nullptr, base, false,
                             [&](StepIO& io, int m) {
@@ -527,6 +585,19 @@ int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
 // C_n = <l|T_n|r>  -> h->moments [B][n] (real part)
 int moments_left(gpuqt_handle* h, const double2* l, const double2* r, int n_moments) {
     CU(launch_dot(h, l, r, h->dots));
+    if (small_ok(h)) {
+        SmallArgs a{};
+        a.v0 = r; a.aux = l; a.dots = h->dots; a.n_terms = n_moments;
+        {
+            StatScope s(h, GPUQT_KERNEL_KPM_LEFT);
+            CU(launch_small(h, kModeLeft, a));
+            s.count(1, n_moments - 1);
+        }
+        const int total = h->B * n_moments;
+        finalize_left<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, h->dots, h->moments);
+        CU(cudaGetLastError());
+        return GPUQT_OK;
+    }
     StepArgs base{};
     base.phiL = l;
     int rc = run_recurrence(h, kModeLeft, GPUQT_KERNEL_KPM_LEFT, n_moments, r, nullptr, base, false, [&](StepIO& io, int n) {
@@ -706,6 +777,7 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     // two steps per launch (cheb_pair_kernel) are opt-in: they cut the DRAM bytes of a step pair by a
     // third but are time-neutral at best on B200 so far
     h->fuse = env_int("GPUQT_FUSE", 0);
+    h->small = env_int("GPUQT_SMALL", 1);
     h->lag = std::max(1, env_int("GPUQT_LAG", 2));
     h->nbr_ptr.swap(sell.nbr_ptr);
     h->nbr_slices.swap(sell.nbr_slices);

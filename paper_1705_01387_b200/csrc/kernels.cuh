@@ -1288,3 +1288,166 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
 }
 
 }  // namespace gpuqt
+
+namespace gpuqt {
+
+// ---------------------------------------------------------------------------------- small lattices
+// Lattices whose matrix and four vector sets fit one SM's shared memory (config c1: 2304 orbitals) are
+// launch-latency bound on the streaming kernels (one launch per recurrence term).  cheb_small_kernel
+// runs a WHOLE recurrence in one launch of one CTA: matrix (decoded to plain arrays) and vectors live in
+// shared memory, the terms are separated by __syncthreads(), the per-term dots are reduced in a fixed
+// order (warp shuffle -> shared memory over warps) and written straight to dots[term].
+//   MODE doubling : T_m from v0; dots {<T_m|T_m>, Re<T_m|T_{m-1}>, <T_{m-1}|T_{m-1}>} per term   (Eq. 28, 30)
+//   MODE left     : T_n from v0; dots <aux|T_n> (Re, Im) per term                                  (Eq. 29)
+//   MODE evolve   : out = sum_k c_k T_k(H~) aux by Clenshaw (v0 unused; coef[k] = c_k)             (Eq. 17)
+constexpr int kSmallThreads = 1024;
+
+struct SmallArgs {
+    const double2* v0;      // doubling / left: T_0
+    const double2* aux;     // left: phi_L; evolve: the vector being evolved
+    double2* out;           // evolve: result
+    const double2* coef;    // evolve: c_k, k < n_terms
+    double* dots;           // doubling: [term-1][3][B]; left: [term][2][B]
+    int n_terms;            // doubling / left: terms m = 1 .. n_terms-1; evolve: order
+};
+
+template <int B, int MODE>
+__global__ void __launch_bounds__(kSmallThreads, 1) cheb_small_kernel(const Mat m, const SmallArgs a) {
+    constexpr int Q = (MODE == kModeDoubling) ? 3 : 2;
+    constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    __shared__ double s_red[kSmallThreads / 32][Q * B];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int N = (int)m.N, K = m.K, NB = N * B;
+    const int nd = hop_doubles(m.hop);
+    double2* vec = reinterpret_cast<double2*>(sm_raw);                  // 3 ring slots
+    double2* aux = vec + 3 * (size_t)NB;
+    double* on = reinterpret_cast<double*>(aux + NB);
+    double* hre = on + N;                                               // [K][N] if nd >= 1
+    double* him = hre + (nd >= 1 ? (size_t)K * N : 0);                  // [K][N] if nd == 2
+    int* col = reinterpret_cast<int*>(him + (nd == 2 ? (size_t)K * N : 0));   // [K][N]; padding -> row itself, weight 0
+    double* wpad = nullptr;
+    (void)wpad;
+    // decode the records into plain arrays
+    for (int row = tid; row < N; row += kSmallThreads) {
+        const RecView rv = record_view(m, row >> 5);
+        const int r = row & 31;
+        on[row] = rv.on[r];
+        for (int k = 0; k < K; ++k) {
+            int c = row;
+            double hr = 0.0, hi = 0.0;
+            if (k < rv.w) {
+                c = rv.col_at(k, r);
+                if (hop_is_const(m.hop)) {
+                    hr = c < N ? m.hop_const : 0.0;
+                    c = c < N ? c : row;
+                } else {
+                    hr = rv.hre[k * 32 + r];
+                    if (nd == 2) hi = rv.him[k * 32 + r];
+                }
+            }
+            col[k * N + row] = hop_is_const(m.hop) && hr == 0.0 ? -1 : c;   // const variant: -1 marks "no entry"
+            if (nd >= 1) hre[k * N + row] = hr;
+            if (nd == 2) him[k * N + row] = hi;
+        }
+    }
+    const double2* src0 = (MODE == kModeEvolve) ? a.aux : a.v0;
+    for (int i = tid; i < NB; i += kSmallThreads) {
+        if (MODE == kModeEvolve) {
+            const double2 s = a.aux[i], c = a.coef[a.n_terms - 1];
+            aux[i] = s;
+            vec[i] = make_double2(c.x * s.x - c.y * s.y, c.x * s.y + c.y * s.x);   // b_{order-1} = c_{order-1} src
+        } else {
+            vec[i] = src0[i];
+            if (MODE == kModeLeft) aux[i] = a.aux[i];
+        }
+    }
+    __syncthreads();
+    if (MODE == kModeEvolve && a.n_terms == 1) {
+        for (int i = tid; i < NB; i += kSmallThreads) a.out[i] = vec[i];
+        return;
+    }
+    int cur = 0;                     // slot of x_{m-1}; x_{m-2} in (cur + 2) % 3; x_m goes to (cur + 1) % 3
+    for (int t = 1; t < a.n_terms; ++t) {
+        const double2* in = vec + (size_t)cur * NB;
+        const double2* prev = vec + (size_t)((cur + 2) % 3) * NB;
+        double2* out = vec + (size_t)((cur + 1) % 3) * NB;
+        const bool first = (t == 1);
+        const bool half = (MODE == kModeEvolve) ? (t == a.n_terms - 1) : first;
+        const double scale = half ? m.inv_dE : 2.0 * m.inv_dE;
+        double2 ck = make_double2(0.0, 0.0);
+        if (MODE == kModeEvolve) ck = a.coef[a.n_terms - 1 - t];
+        double red[Q];
+#pragma unroll
+        for (int q = 0; q < Q; ++q) red[q] = 0.0;
+        for (int i = tid; i < NB; i += kSmallThreads) {
+            const int row = i / B, b = i % B;
+            const double2 self = in[i];
+            double sr = on[row] * self.x, si = on[row] * self.y;
+            for (int k = 0; k < K; ++k) {
+                const int c = col[k * N + row];
+                if (hop_is_const(m.hop)) {
+                    if (c >= 0) {
+                        const double2 v = in[c * B + b];
+                        sr = fma(m.hop_const, v.x, sr);
+                        si = fma(m.hop_const, v.y, si);
+                    }
+                } else {
+                    const double2 v = in[c * B + b];
+                    const double hr = hre[k * N + row];
+                    sr = fma(hr, v.x, sr);
+                    si = fma(hr, v.y, si);
+                    if (nd == 2) {
+                        const double hi = him[k * N + row];
+                        sr = fma(-hi, v.y, sr);
+                        si = fma(hi, v.x, si);
+                    }
+                }
+            }
+            double2 tt = make_double2(scale * sr, scale * si);
+            if (!first) {
+                const double2 p = prev[i];
+                tt.x -= p.x;
+                tt.y -= p.y;
+            }
+            if (MODE == kModeEvolve) {
+                const double2 s = aux[i];
+                tt.x += ck.x * s.x - ck.y * s.y;
+                tt.y += ck.x * s.y + ck.y * s.x;
+                if (half) a.out[i] = tt;
+            } else if (MODE == kModeDoubling) {
+                red[0] += tt.x * tt.x + tt.y * tt.y;
+                red[1] += tt.x * self.x + tt.y * self.y;
+                if (first) red[2] += self.x * self.x + self.y * self.y;
+            } else {
+                const double2 l = aux[i];
+                red[0] += l.x * tt.x + l.y * tt.y;
+                red[1] += l.x * tt.y - l.y * tt.x;
+            }
+            out[i] = tt;
+        }
+        if (DOTS) {
+            // fixed-order reduction over the threads that hold vector b = tid % B
+#pragma unroll
+            for (int q = 0; q < Q; ++q) {
+#pragma unroll
+                for (int off = 16; off >= B; off >>= 1) red[q] += __shfl_xor_sync(0xffffffffu, red[q], off);
+            }
+            if (lane < B) {
+#pragma unroll
+                for (int q = 0; q < Q; ++q) s_red[wid][q * B + lane] = red[q];
+            }
+            __syncthreads();
+            if (tid < Q * B) {
+                double s = 0.0;
+                for (int w = 0; w < kSmallThreads / 32; ++w) s += s_red[w][tid];
+                const size_t base = (MODE == kModeDoubling) ? (size_t)(t - 1) * 3 * B : (size_t)t * 2 * B;
+                a.dots[base + tid] = s;
+            }
+        }
+        __syncthreads();
+        cur = (cur + 1) % 3;
+    }
+}
+
+}  // namespace gpuqt

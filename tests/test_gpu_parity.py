@@ -17,6 +17,13 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-10
 
 
+@pytest.fixture(autouse=True, params=["streaming", "small_path"])
+def small_lattice_path(request, monkeypatch):
+    """Every case runs twice: on the streaming kernels only (GPUQT_SMALL=0) and with the one-CTA
+    whole-recurrence kernel enabled, which takes over wherever matrix + vectors fit one SM's shared memory."""
+    monkeypatch.setenv("GPUQT_SMALL", "0" if request.param == "streaming" else "1")
+
+
 @pytest.fixture(scope="module")
 def gq():
     import torch
