@@ -21,8 +21,11 @@
  *
  * Ownership: the caller owns every array it passes and the device workspace; gpuqt_create copies
  * the host inputs and keeps no host pointer.  Results are written to caller-allocated buffers and
- * are complete when the call returns (the call synchronises the stream).  gpuqt_destroy frees only
- * the handle.
+ * are complete when the call returns (the call synchronises the stream).  All vectors and the
+ * matrix live in the caller's workspace; the handle itself owns only small device objects (the TMA
+ * tensor maps of the vector buffers, a grow-on-demand scratch buffer for gpuqt_kpm_transform /
+ * gpuqt_running_conductivity / gpuqt_get_table, the work lists of the opt-in two-step kernel), which
+ * gpuqt_destroy frees together with the handle; the workspace stays the caller's.
  *
  * Errors: every call returns a gpuqt_status (0 = ok, < 0 = error); nothing throws or aborts across
  * the ABI; the handle stays valid after an error; gpuqt_last_error gives text.
