@@ -1,4 +1,7 @@
-"""Build libgpuqt.so (sm_100a only) in-tree with nvcc.  `python -m paper_1705_01387_b200.build`."""
+"""Build libgpuqt.so (sm_100a only) in-tree with nvcc.  `python -m paper_1705_01387_b200.build`.
+
+Two translation units (gpuqt.cu: the C-ABI and the single-step kernels; pair_kernels.cu: the opt-in
+two-step kernel) are compiled in parallel and linked into one shared library."""
 import os
 import subprocess
 import sys
@@ -6,11 +9,11 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("GPUQT_LIB") or os.path.join(HERE, "libgpuqt.so")
-SOURCES = [os.path.join(CSRC, "gpuqt.cu")]
+SOURCES = [os.path.join(CSRC, "gpuqt.cu"), os.path.join(CSRC, "pair_kernels.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "host_util.h")] + [
     os.path.join(os.path.dirname(HERE), "include", "gpuqt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC"]
 
 
 def needs_build() -> bool:
@@ -23,9 +26,16 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        extra = os.environ.get("GPUQT_NVCC_EXTRA", "").split()      # e.g. -DGPUQT_U_KPM=4 (kernel tuning macros)
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
-        subprocess.check_call(cmd)
+        extra = os.environ.get("GPUQT_NVCC_EXTRA", "").split()      # e.g. -DGPUQT_MINB=1 (kernel tuning macros)
+        flags = NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else [])
+        objs = [LIB + "." + os.path.basename(s) + ".o" for s in SOURCES]
+        procs = [subprocess.Popen([nvcc] + flags + ["-c", "-o", o, s]) for s, o in zip(SOURCES, objs)]
+        codes = [p.wait() for p in procs]
+        if any(codes):
+            raise subprocess.CalledProcessError(max(codes), "nvcc -c")
+        subprocess.check_call([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
+        for o in objs:
+            os.remove(o)
     return LIB
 
 

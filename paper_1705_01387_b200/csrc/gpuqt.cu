@@ -13,6 +13,10 @@
 
 using namespace gpuqt;
 
+namespace gpuqt {
+void* pair_kernel_fn(int mode, int B, int kt, int hop);   // pair_kernels.cu
+}
+
 namespace {
 
 constexpr int kMaxGrid = 4096;
@@ -148,42 +152,38 @@ bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
 
 // ---------------------------------------------------------------- kernel dispatch
 template <int MODE, int BB, int KK>
-void* step_fn(int hop, bool pair) {
+void* step_fn(int hop) {
     if (KK > 0 && hop == kHopConst16)      // 16-bit columns exist for the unrolled uniform tables only
-        return pair ? (void*)cheb_pair_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>
-                    : (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>;
-    if (pair)
-        return hop == kHopComplex ? (void*)cheb_pair_kernel<BB, KK, kHopComplex, MODE>
-               : hop == kHopConst ? (void*)cheb_pair_kernel<BB, KK, kHopConst, MODE>
-                                  : (void*)cheb_pair_kernel<BB, KK, kHopReal, MODE>;
+        return (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>;
     return hop == kHopComplex ? (void*)cheb_step_kernel<BB, KK, kHopComplex, MODE>
            : hop == kHopConst ? (void*)cheb_step_kernel<BB, KK, kHopConst, MODE>
                               : (void*)cheb_step_kernel<BB, KK, kHopReal, MODE>;
 }
 template <int MODE, int BB>
-void* step_fn_k(int kt, int hop, bool pair) {
+void* step_fn_k(int kt, int hop) {
     switch (kt) {
-    case 3: return step_fn<MODE, BB, 3>(hop, pair);
-    case 4: return step_fn<MODE, BB, 4>(hop, pair);
-    case 6: return step_fn<MODE, BB, 6>(hop, pair);
-    default: return step_fn<MODE, BB, 0>(hop, pair);
+    case 3: return step_fn<MODE, BB, 3>(hop);
+    case 4: return step_fn<MODE, BB, 4>(hop);
+    case 6: return step_fn<MODE, BB, 6>(hop);
+    default: return step_fn<MODE, BB, 0>(hop);
     }
 }
 template <int MODE>
-void* step_fn_b(int B, int kt, int hop, bool pair) {
+void* step_fn_b(int B, int kt, int hop) {
     switch (B) {
-    case 1: return step_fn_k<MODE, 1>(kt, hop, pair);
-    case 2: return step_fn_k<MODE, 2>(kt, hop, pair);
-    case 4: return step_fn_k<MODE, 4>(kt, hop, pair);
-    default: return step_fn_k<MODE, 8>(kt, hop, pair);
+    case 1: return step_fn_k<MODE, 1>(kt, hop);
+    case 2: return step_fn_k<MODE, 2>(kt, hop);
+    case 4: return step_fn_k<MODE, 4>(kt, hop);
+    default: return step_fn_k<MODE, 8>(kt, hop);
     }
 }
 void* step_kernel(const gpuqt_handle* h, int mode, bool pair) {
+    if (pair) return pair_kernel_fn(mode, h->B, h->kt, h->hop);     // pair_kernels.cu
     switch (mode) {
-    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->hop, pair);
-    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->hop, pair);
-    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->hop, pair);
-    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->hop, pair);
+    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->hop);
+    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->hop);
+    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->hop);
+    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->hop);
     }
 }
 

@@ -1145,6 +1145,7 @@ __global__ void __launch_bounds__(kThreads) dot_kernel(long long N, const double
     block_reduce_and_finish<B, 2>(red, partials, ticket, result);
 }
 
+#ifndef GPUQT_PAIR_TU   // the non-template kernels below belong to gpuqt.cu's translation unit only
 // [batch][N] (host order) <-> [N][B] (device order)
 __global__ void to_device_layout(long long N, int B, const double2* __restrict__ src, double2* __restrict__ dst) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1286,6 +1287,8 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
     if (im) im[i] = hi;
     if (dx) dx[i] = d;
 }
+
+#endif  // GPUQT_PAIR_TU
 
 }  // namespace gpuqt
 
