@@ -14,7 +14,7 @@ def time_axis(dts):
     return np.concatenate([[0.0], np.cumsum(np.asarray(dts, np.float64))])
 
 
-def run(engine, phi, dts, n_moments, energies, order_of, vac=True, msd=True):
+def run(engine, phi, dts, n_moments, energies, order_of, vac=True, msd=True, per_vector=False):
     """One pass of the method for the handle's B random vectors.
 
     phi       host [B][N][2] random-phase vectors
@@ -24,26 +24,33 @@ def run(engine, phi, dts, n_moments, energies, order_of, vac=True, msd=True):
     the VAC branches is skipped only if MSD is off); MSD row k is measured at t_{k+1} AFTER step k.
     Returns a dict of arrays averaged over the B vectors: dos [n_E], rho_vac / rho_msd [N_t][n_E]
     (= rho C_vv, rho dX^2), sigma_vac (at t_k), sigma_msd (at the middle of step k), length (Eq. 11).
+    With per_vector=True nothing is averaged and no conductivity is formed: dos [B][n_E], rho_vac /
+    rho_msd [N_t][B][n_E] -- the rows of the paper's dos.out / vac.out / msd.out.
     """
     dts = np.asarray(dts, np.float64)
     energies = np.ascontiguousarray(energies, np.float64)
     engine.set_state(phi)
     out = {"times": time_axis(dts), "energies": energies}
-    dos = engine.kpm_transform(engine.dos_moments(n_moments), energies).mean(axis=0)
+    avg = (lambda a: a) if per_vector else (lambda a: a.mean(axis=0))
+    dos = avg(engine.kpm_transform(engine.dos_moments(n_moments), energies))
     out["dos"] = dos
     vac_rows, msd_rows = [], []
     for k, dt in enumerate(dts):
         if vac:
-            vac_rows.append(engine.kpm_transform(engine.vac(n_moments), energies).mean(axis=0))
+            vac_rows.append(avg(engine.kpm_transform(engine.vac(n_moments), energies)))
         if msd or k + 1 < len(dts):
             engine.evolve(float(dt), int(order_of(float(dt))))
         if msd:
-            msd_rows.append(engine.kpm_transform(engine.msd(n_moments), energies).mean(axis=0))
+            msd_rows.append(avg(engine.kpm_transform(engine.msd(n_moments), energies)))
     if vac:
-        out["rho_vac"] = np.array(vac_rows)
+        out["rho_vac"] = np.array(vac_rows).reshape((len(vac_rows),) + np.shape(dos))
+    if msd:
+        out["rho_msd"] = np.array(msd_rows).reshape((len(msd_rows),) + np.shape(dos))
+    if per_vector:
+        return out
+    if vac:
         out["sigma_vac"], _ = engine.running_conductivity("vac", out["rho_vac"], dos, dts[:len(dts) - 1])
     if msd:
-        out["rho_msd"] = np.array(msd_rows)
         out["sigma_msd"], out["length"] = engine.running_conductivity("msd", out["rho_msd"], dos, dts)
     return out
 

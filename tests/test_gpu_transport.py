@@ -93,3 +93,25 @@ def test_paper_examples_reduced(gq, oracle_mod, key, scale):
         assert np.all(np.diff(x2[:4]) > 0)                              # the MSD grows from zero ...
         assert abs(x2[0] / t[0] ** 2 / (x2[1] / t[1] ** 2) - 1.0) < 0.2  # ... quadratically at short times (ballistic)
     g.close()
+
+
+def test_file_front_end_matches_oracle(gq, oracle_mod, tmp_path):
+    """The paper's workflow: a simulation folder run through the CUDA library writes
+    the same dos.out / vac.out / msd.out as the oracle driven through the identical front-end."""
+    from paper_1705_01387_b200 import frontend as F
+    from workloads import lattices as L
+    model = L.square(40, 32, W=4.0, seed=3, energy_scale=6.1)
+    E = np.linspace(-6.0, 6.0, 121)
+    para = {"calculate_vac": True, "calculate_msd": True, "number_of_random_vectors": 3, "number_of_moments": 128}
+    for name in ("gpu", "cpu"):
+        F.write_folder(str(tmp_path / name), model, E, [0.2, 0.2, 0.5, 1.0], para)
+
+    def make(mdl, b, vac, msd):
+        modes = (oracle_mod.MODE_VAC if vac else 0) | (oracle_mod.MODE_MSD if msd else 0)
+        return OracleEngine(oracle_mod, mdl, b, modes)
+    F.run_folder(str(tmp_path / "gpu"), seed=11)
+    F.run_folder(str(tmp_path / "cpu"), seed=11, make_engine=make)
+    for out, rows in (("dos.out", 3), ("vac.out", 12), ("msd.out", 12)):
+        a, b = np.loadtxt(tmp_path / "gpu" / out), np.loadtxt(tmp_path / "cpu" / out)
+        assert a.shape == b.shape == (rows, 121)
+        assert rel(a, b) <= TOL, out
