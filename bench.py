@@ -39,12 +39,35 @@ def walks_per_step(w, order):
     return 2 * (order - 1), 1 + (w.n_moments - 1)       # a and b branches; V a + N_m - 1 steps
 
 
-def bytes_per_orbital_spmv(model, batch, kind):
-    """Algorithmic bytes of one orbital-SpMV from the sliced-ELL layout."""
+L2_BYTES = 126e6      # B200 L2 (B200_PROFILING.md)
+
+
+def contract_bytes_per_row(model, batch, kernel):
+    """SURVEY 8(d)'s ELL-contract bytes one launch (= one recurrence step) moves per row: int32 index +
+    fp64 (re, im) hopping per entry + on-site, and each vector element once per pass (evolve: with the
+    read-modify-write of an accumulator the Clenshaw form does not have)."""
     cplx = model.hop_im is not None
     mat = model.K * (4 + (16 if cplx else 8)) + 8
-    vec = {"kpm_doubling": 48, "kpm_left": 64, "evolve": 80}[kind]
-    return mat / batch + vec
+    if kernel == "evolve_msd":                  # (psi, chi) pair: matrix once + x, two vector streams
+        return mat + 8 + batch * 2 * 80
+    return mat + batch * {"kpm_doubling": 48, "kpm_left": 64, "evolve": 80}[kernel]
+
+
+def stored_bytes_per_row(model, batch, kernel, stored_matrix_bytes):
+    """Bytes the stored layout must move per row and step: the packed records as gpuqt_create built
+    them (no hopping array when the hopping is one constant, 16-bit columns where possible; from
+    gpuqt_get_info), x for the commutator walk, and the vector streams the kernel really has
+    (Clenshaw evolution: x_{m-1}, x_{m-2}, src read, x_m written = 64 B per vector)."""
+    rec = (stored_matrix_bytes - 8 * (model.N + 1)) / model.N
+    vec = {"kpm_doubling": 48, "kpm_left": 64, "evolve": 64, "evolve_msd": 128}[kernel] * batch
+    return rec + vec + (8 if kernel == "evolve_msd" else 0)
+
+
+def working_set_bytes(model, batch, kernel, stored_matrix_bytes):
+    """Distinct bytes one step of the dominant kernel touches (what has to stay in L2 for the next step
+    to find it there)."""
+    streams = {"kpm_doubling": 3, "kpm_left": 4, "evolve": 4, "evolve_msd": 8}[kernel]
+    return stored_matrix_bytes + streams * 16 * batch * model.N
 
 
 def energies_for(model):
@@ -133,13 +156,34 @@ def oracle_sample(w, model, order, seconds_hint=15.0):
     return task, executed, dt, cores, desc
 
 
+def oracle_one_thread(w, model, seconds_hint=8.0):
+    """The oracle on ONE host thread ("once with 1 thread and once with all cores"): a short
+    moment set of the workload's kind on 1 vector at full N, sized for about 10 s; executed row-walks / s."""
+    import ctypes
+    from oracle import oracle
+    oracle.lib()
+    gomp = ctypes.CDLL("libgomp.so.1")
+    before = gomp.omp_get_max_threads()
+    nm = int(max(4, min(w.n_moments, (seconds_hint * 3.5e7 / model.N) // 2 * 2)))
+    o = oracle.Oracle(model, batch=1, modes=oracle.MODE_MSD if w.path == "msd" else oracle.MODE_VAC)
+    o.set_state(w.phases(model)[:1])
+    gomp.omp_set_num_threads(1)
+    try:
+        t0 = time.perf_counter()
+        o.dos_moments(nm)                      # nm - 1 walks, no doubling
+        dt = time.perf_counter() - t0
+    finally:
+        gomp.omp_set_num_threads(before)
+    o.close()
+    return model.N * (nm - 1) / dt, f"{nm}-moment DOS set on 1 vector at full N, {dt:.1f} s"
+
+
 def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from paper_1705_01387_b200 import binding
     model = w.build()
-    order = w.order or binding.choose_order(model.energy_scale, w.dt)
+    order = w.order
     times, task = [], 0
     for i in range(args.warmup + args.steps):
         task, executed, dt, cores, desc = oracle_sample(w, model, order)
@@ -160,6 +204,7 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+
 # ------------------------------------------------------------------------------------ CUDA leg
 def run_ours(args, w):
     import torch
@@ -174,11 +219,11 @@ def run_ours(args, w):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     model = w.build()
-    order = w.order or binding.choose_order(model.energy_scale, w.dt)
+    order = w.order
     modes = gq.MODE_MSD if w.path == "msd" else gq.MODE_VAC
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
-        g = gq.GpuQT(model, batch=w.batch, modes=modes, stream=stream)
+        g = gq.GpuQT(model, batch=w.batch, modes=modes, stream=stream, options=args.options)
         # replicas over random vectors: rank r owns vectors [r*B, (r+1)*B)
         phi_host = torch.from_numpy(w.phases(model, first_vector=replicas.first_vector(rank, w.batch))).pin_memory()
         phi_dev = phi_host.to("cuda", non_blocking=True)
@@ -186,16 +231,25 @@ def run_ours(args, w):
         energies = energies_for(model)
         stream.synchronize()
 
+        copy_ev = []                                # (start, stop) pairs around the e2e host->device load
+
         def step(e2e):
             if e2e:
-                g.set_state(phi_host)              # H2D of this step's input from pinned memory
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                g.set_state(phi_host)              # H2D of this step's input from pinned memory (+ layout change, V phi)
+                e1.record(stream)
+                copy_ev.append((e0, e1))
             if w.path == "msd":
                 g.evolve(w.dt, order)
                 g.msd(w.n_moments, out=mom_host)   # D2H of the step's result
             else:
                 g.vac(w.n_moments, out=mom_host)
                 g.evolve(w.dt, order)
-            return g.kpm_transform(mom_host.numpy(), energies)
+            out = g.kpm_transform(mom_host.numpy(), energies)
+            if e2e and world > 1:                  # the one exchange of the replicas scheme: all ranks' moment blocks
+                replicas.gather_moments(mom_host.to("cuda", non_blocking=True))
+            return out
 
         def barrier():
             if world > 1:
@@ -207,6 +261,7 @@ def run_ours(args, w):
             for _ in range(args.warmup):
                 step(e2e)
             g.reset_stats()
+            copy_ev.clear()
             barrier()
             ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ev0.record(stream)
@@ -222,9 +277,18 @@ def run_ours(args, w):
             sampler.start()
         ms, out = timed(False)
         clocks = sampler.stop()
-        stats = {c: (g.kernel_stats(c)[0], g.kernel_steps(c)) for c in range(5)}       # (ms, recurrence steps)
-        n_launches = sum(g.kernel_stats(c)[1] for c in range(5))
+        stats = {c: (g.kernel_stats(c)[0], g.kernel_steps(c), g.kernel_stats(c)[1]) for c in range(5)}   # (ms, steps, launches)
+        n_launches = sum(stats[c][2] for c in range(5))
         ms_e2e, _ = timed(True)
+        set_state_ms = sum(a.elapsed_time(b) for a, b in copy_ev) / max(len(copy_ev), 1)
+        # the bare pinned H2D copy of the same bytes, alone on the stream (for the PCIe rate)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        phi_dev.copy_(phi_host, non_blocking=True)
+        e1.record(stream)
+        stream.synchronize()
+        h2d_ms = e0.elapsed_time(e1)
+        info = {k: g.info(getattr(binding, "INFO_" + k)) for k in ("STORED_MATRIX_BYTES", "HOP_VARIANT", "SMALL_PATH", "PERSISTENT")}
 
     ev_w, mom_w = walks_per_step(w, order)
     units_step = model.N * w.batch * (ev_w + mom_w) * world
@@ -236,66 +300,73 @@ def run_ours(args, w):
         # roofline of the dominant kernel class (most device time in the timed region)
         names = {0: "kpm_doubling", 1: "kpm_left", 2: "evolve", 3: "evolve_msd"}
         dom = max(names, key=lambda c: stats[c][0])
-        kind = {0: "kpm_doubling", 1: "kpm_left", 2: "evolve", 3: "evolve"}[dom]
-        bpo = bytes_per_orbital_spmv(model, w.batch, kind)
-        if dom == 3:   # (psi, chi) pair: matrix read once + x, two vector streams
-            cplx = model.hop_im is not None
-            per_row_launch = (model.K * (4 + (16 if cplx else 8)) + 8 + 8) + w.batch * 2 * 80
-        else:
-            per_row_launch = bpo * w.batch
-        # bytes the stored layout really holds per row (constant-hopping records carry no hop array)
-        hop_const = model.hop_im is None and (model.hop_re is None or np.unique(
-            model.hop_re.reshape(model.N, model.K)[np.arange(model.K)[None, :] < model.nbr_count[:, None]]).size <= 1)
-        hop_const = hop_const and os.environ.get("GPUQT_HOP_CONST", "1") != "0"
-        stored_row_launch = per_row_launch - (8 * model.K if hop_const else 0)
-        # ... and 16-bit columns (base + delta) when the table is uniform, unpadded and N % 32 == 0
-        if (hop_const and model.K in (3, 4, 6) and model.N % 32 == 0 and int(model.nbr_count.min()) == model.K
-                and os.environ.get("GPUQT_IDX16", "1") != "0"):
-            stored_row_launch -= 2 * model.K - 1
-        dom_ms, dom_n = stats[dom]
-        achieved = per_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9
+        kernel = names[dom]
+        dom_ms, dom_steps, dom_launches = stats[dom]
+        step_s = dom_ms * 1e-3 / max(dom_steps, 1)                 # one recurrence step of that kernel
+        stored = stored_bytes_per_row(model, w.batch, kernel, info["STORED_MATRIX_BYTES"]) * model.N
+        contract = contract_bytes_per_row(model, w.batch, kernel) * model.N
+        wset = working_set_bytes(model, w.batch, kernel, info["STORED_MATRIX_BYTES"])
+        achieved = stored / step_s / 1e9
         peak, peak_src = load_peak()
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):
             try:
-                traffic = json.load(open(tp)).get(f"{w.key}:{names[dom]}")
+                traffic = json.load(open(tp)).get(f"{w.key}:{kernel}")
             except Exception:
                 traffic = None
-        launches = n_launches + args.steps * 3      # + finalize, jackson, transform
+        in_l2 = wset < L2_BYTES
+        l2_note = ("working set of a recurrence step %.0f MB < 126 MB L2: the %d dependent steps of a moment set re-read it "
+                   "by construction (no flush is possible inside a step), so the HBM roofline does not bound this config"
+                   % (wset / 1e6, w.n_moments)) if in_l2 else (
+                   "inputs larger than L2: a recurrence step touches %.0f MB (vector set %.0f MB, stored matrix %.0f MB) "
+                   "vs 126 MB L2; no flush" % (wset / 1e6, model.N * w.batch * 16 / 1e6, info["STORED_MATRIX_BYTES"] / 1e6))
+        launches = n_launches + args.steps * 3      # + finalize, damping, transform
         line = {"metric": "orbital-SpMV/s in Chebyshev evolution + KPM moments", "value": value,
                 "unit": "orbital-SpMV/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": w.key, "description": w.description, "N": model.N, "K": model.K,
                            "batch_per_gpu": w.batch, "n_moments": w.n_moments, "order": order, "dt": w.dt,
-                           "n_energies": N_ENERGIES, "path": w.path,
-                           "l2": "inputs larger than L2 (each vector set %.0f MB, matrix %.0f MB vs 126 MB L2); no flush"
-                                 % (model.N * w.batch * 16 / 1e6,
-                                    model.N * (model.K * (20 if model.hop_im is not None else 12) + 8) / 1e6),
+                           "n_energies": N_ENERGIES, "path": w.path, "l2": l2_note,
+                           "storage": {"hop_variant": ["real", "complex", "constant, int32 columns", "constant, 16-bit columns"][info["HOP_VARIANT"]],
+                                       "stored_matrix_bytes": info["STORED_MATRIX_BYTES"],
+                                       "launch_form": "one-CTA whole-recurrence kernel" if info["SMALL_PATH"] else
+                                                      "one cooperative launch per recurrence" if info["PERSISTENT"] else
+                                                      "one launch per recurrence step"},
                            "parallelism": f"replicas-over-vectors x{world}",
-                           "seconds_per_time_step": ms / args.steps * 1e-3},
+                           "seconds_per_time_step": ms / args.steps * 1e-3,
+                           **({"options": args.options} if args.options else {})},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": "orbital-SpMV/s", "ms_per_step": ms_e2e / args.steps,
                         "h2d_bytes_per_step": int(phi_host.numel() * 8 + (w.n_moments * w.batch + N_ENERGIES) * 8),
-                        "d2h_bytes_per_step": int(mom_host.numel() * 8 + w.batch * N_ENERGIES * 8)},
+                        "d2h_bytes_per_step": int(mom_host.numel() * 8 + w.batch * N_ENERGIES * 8),
+                        "set_state_ms_per_step": set_state_ms,
+                        "h2d_copy_alone_ms": h2d_ms, "h2d_copy_alone_gbs": phi_host.numel() * 8 / (h2d_ms * 1e-3) / 1e9,
+                        "note": "set_state = pinned H2D copy of the B random vectors + layout change (+ V phi in VAC mode), "
+                                "timed with its own CUDA events inside the e2e loop; the bare copy is timed alone afterwards"},
                 "gpu_launches": int(launches),
-                "roofline": {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak,
+                "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
                              "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                             "bytes_per_launch": stored,
+                             "bytes_note": "achieved = bytes the STORED layout moves per recurrence step (records as built + "
+                                           "vector streams) / average step time; the ELL contract of SURVEY 8(d) (int32 + fp64 "
+                                           "per entry) is kept beside it as contract_*",
+                             "contract_bytes_per_launch": contract, "contract_gbs": contract / step_s / 1e9,
+                             "contract_frac": contract / step_s / 1e9 / peak,
+                             "dram_gbs_from_ncu_traffic": (traffic / step_s / 1e9) if traffic else None,
                              "frac_of_nominal_8000": achieved / 8000.0,
-                             "bytes_per_launch": per_row_launch * model.N,
-                             "stored_bytes_per_launch": stored_row_launch * model.N,
-                             "stored_gbs": stored_row_launch * model.N / (dom_ms * 1e-3 / max(dom_n, 1)) / 1e9,
-                             "avg_launch_us": dom_ms * 1e3 / max(dom_n, 1), "launches": dom_n,
-                             "note": "launches = recurrence steps; one step per kernel launch by default, two per "
-                                     "launch with GPUQT_FUSE=1 (bytes and time are then both per step)",
+                             "working_set_bytes": wset, "l2_resident": bool(in_l2),
+                             "avg_step_us": step_s * 1e6, "steps": dom_steps, "launches": dom_launches,
                              "share_of_step": dom_ms / ms,
                              "per_class_ms": {names[c]: stats[c][0] for c in names}},
                 }
         if world == 1 and not args.no_cpu_baseline:
             task, executed, dt, cores, desc = oracle_sample(w, model, order)
+            one, one_desc = oracle_one_thread(w, model)
             line["cpu_baseline"] = {"value": task / dt, "unit": "orbital-SpMV/s", "cores": cores, "kind": "oracle",
-                                    "sample": desc, "seconds": dt, "executed_value": executed / dt}
+                                    "sample": desc, "seconds": dt, "executed_value": executed / dt,
+                                    "executed_value_1_thread": one, "sample_1_thread": one_desc}
         print(json.dumps(line), flush=True)
     g.close()
     if world > 1:
@@ -311,7 +382,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-clock-sampler", action="store_true", help="diagnostic: do not poll nvidia-smi during the timed region")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="gpuqt_options override for tuning runs, e.g. --opt persistent=0 (default: the library defaults)")
     args = ap.parse_args()
+    args.options = {k: int(v) for k, v in (kv.split("=", 1) for kv in args.opt)}
     w = configs.WORKLOADS[args.config]
     if args.impl == "reference":
         run_reference(args, w)

@@ -22,13 +22,15 @@
  * Ownership: the caller owns every array it passes and the device workspace; gpuqt_create copies
  * the host inputs and keeps no host pointer.  Results are written to caller-allocated buffers and
  * are complete when the call returns (the call synchronises the stream).  All vectors and the
- * matrix live in the caller's workspace; the handle itself owns only small device objects (the TMA
- * tensor maps of the vector buffers, a grow-on-demand scratch buffer for gpuqt_kpm_transform /
- * gpuqt_running_conductivity / gpuqt_get_table, the work lists of the opt-in two-step kernel), which
- * gpuqt_destroy frees together with the handle; the workspace stays the caller's.
+ * matrix live in the caller's workspace; the handle itself owns only small objects (the TMA tensor
+ * maps of the vector buffers, a grow-on-demand device scratch buffer for gpuqt_kpm_transform /
+ * gpuqt_running_conductivity / gpuqt_get_table, a few KB of pinned host memory and its device mirror
+ * for the Bessel coefficients of a time step), which gpuqt_destroy frees together with the handle;
+ * the workspace stays the caller's.
  *
- * Errors: every call returns a gpuqt_status (0 = ok, < 0 = error); nothing throws or aborts across
- * the ABI; the handle stays valid after an error; gpuqt_last_error gives text.
+ * Errors: every call returns a gpuqt_status (0 = ok, < 0 = error); nothing throws, aborts or prints
+ * across the ABI; the handle stays valid after an error; gpuqt_last_error(handle) gives text, and
+ * gpuqt_last_error(NULL) the text of the last failed gpuqt_create on the calling thread.
  *
  * Threading: a handle is not thread-safe; all work is issued on the stream given at create.
  */
@@ -77,9 +79,39 @@ typedef enum {
 #define GPUQT_KERNEL_CLASSES 5
 
 #define GPUQT_MAX_MOMENTS 16384
+#define GPUQT_MAX_ORDER 4096         /* largest N_p of one gpuqt_evolve call                          */
 
-/* Bytes of device workspace gpuqt_create needs for this problem (0 on invalid arguments).
- * nnz_slots = number of sliced-ELL entries; pass 0 to use the upper bound ceil32(N) * K_max.    */
+/* Tuning options of gpuqt_create_with_options.  gpuqt_default_options fills in the defaults, which are
+ * what gpuqt_create uses and what bench.py times; nothing is read from the environment.
+ *   struct_bytes   sizeof(gpuqt_options) as the caller compiled it (set by gpuqt_default_options)
+ *   stages         shared-memory pipeline stages per warp, 1..4;            0 = by batch (4, 3, 2, 2)
+ *   blocks_per_sm  cap on resident CTAs per SM;                             0 = what fits
+ *   run            consecutive tiles a CTA walks before it jumps (rounded to a multiple of 8);
+ *                                                                           0 = 16, or 8 for short sweeps
+ *   alternate      1: the sweep direction alternates between recurrence steps (L2 reuse across the
+ *                  step boundary)
+ *   hop_const      1: store no hopping array when every listed hopping is the same real number
+ *   idx16          1: 16-bit (base + delta) columns where the table allows it
+ *   small          1: one-CTA whole-recurrence kernel when matrix and vectors fit one SM's shared memory
+ *   persistent     whole recurrences in ONE cooperative launch with grid-wide barriers between the
+ *                  steps: 1 always, 0 never, -1 when a step is short enough for launch gaps to matter
+ *                  (N * batch <= 32768 rows per SM)                                                   */
+typedef struct gpuqt_options {
+    int32_t struct_bytes;
+    int32_t stages;
+    int32_t blocks_per_sm;
+    int32_t run;
+    int32_t alternate;
+    int32_t hop_const;
+    int32_t idx16;
+    int32_t small;
+    int32_t persistent;
+} gpuqt_options;
+void gpuqt_default_options(gpuqt_options* opt);
+
+/* Bytes of device workspace gpuqt_create needs for this problem (0 on invalid arguments): an upper
+ * bound that holds for every storage variant (every slice record padded to K_max, per-entry fp64
+ * hoppings, int32 columns).                                                                       */
 size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes);
 
 /* Host-only validation of the four input data sets: argument sanity, index range
@@ -103,13 +135,27 @@ int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int
  *   workspace  device memory of at least gpuqt_workspace_bytes(...) bytes, 256-byte aligned,
  *              owned by the caller and alive until gpuqt_destroy
  *   cuda_stream a cudaStream_t (NULL = default stream)
- * Storage: slices of 32 rows, column-major inside a slice, int32 columns, SoA fp64 hoppings
- * (imaginary plane absent in the real variant); padding entries are (own row, 0.0).             */
+ * Storage: slices of 32 rows, one packed record per slice, column-major inside it.
+ * Per-entry variants: SoA fp64 hoppings (imaginary plane absent when hop_im == NULL) + int32 columns,
+ * padding entries = (own row, 0.0).  When hop_im == NULL and every listed hopping has the same bit
+ * pattern (the paper's default "all hoppings -1") no hopping array is stored and
+ * padding entries point at an all-zero row N that every vector buffer carries; such a table keeps
+ * its columns as int32 base + uint16 delta per (slice, k) when they spread less than 65535 there.
+ * gpuqt_get_table decodes every variant back to the canonical padded table.
+ * Errors: the gpuqt_validate codes; GPUQT_ERR_ARG (batch, volume, modes, alignment, K_max too large
+ * for one record per warp in shared memory), GPUQT_ERR_NOMEM (workspace too small), GPUQT_ERR_CUDA.
+ * On failure *out = NULL and gpuqt_last_error(NULL) describes it.                                */
 int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nbr_count,
                  const int32_t* nbr_index, const double* hop_re, const double* hop_im,
                  const double* onsite, const double* x, double box_length, double volume,
                  double energy_scale, int32_t batch, int modes, void* workspace,
                  size_t workspace_bytes, void* cuda_stream);
+/* The same with explicit tuning options (NULL = defaults).                                        */
+int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nbr_count,
+                 const int32_t* nbr_index, const double* hop_re, const double* hop_im,
+                 const double* onsite, const double* x, double box_length, double volume,
+                 double energy_scale, int32_t batch, int modes, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream, const gpuqt_options* options);
 
 /* Load B random vectors (Eq. 13; generated by the caller [A7]) and reset time to 0:
  * psi = phi, chi = 0, a = phi, b = V phi (Eq. 34).  phi: [batch][N][2].                          */
@@ -123,7 +169,7 @@ int gpuqt_dos_moments(gpuqt_handle* h, int32_t n_moments, double* out_host);
 /* One Chebyshev time step of N_p = order terms (Eq. 17-24) for every enabled
  * branch:  psi <- U(dt) psi;  chi <- U(dt) chi + [X,U(dt)] psi  [A3];  a <- U(-dt) a,
  * b <- U(-dt) b  [A1].  dt may differ from call to call and may be negative.
- * order >= 1.                                                                                     */
+ * 1 <= order <= GPUQT_MAX_ORDER.                                                                  */
 int gpuqt_evolve(gpuqt_handle* h, double dt, int32_t order);
 
 /* C_n^VAC(t) = Re <V a|T_n(H~)|b> (Eq. 29) at the current time; does not advance it.
@@ -139,6 +185,20 @@ int gpuqt_msd(gpuqt_handle* h, int32_t n_moments, double* out_host);
 int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_moments,
                         int32_t n_sets, const double* energies_host, int32_t n_energies,
                         double* out_host);
+
+/* The same resummation with another damping kernel g_n of the kernel polynomial method (the paper's
+ * ref. [33]; SURVEY 8(f) 5 -- the paper itself uses Jackson only):
+ *   GPUQT_DAMPING_JACKSON    Eq. 31 (identical to gpuqt_kpm_transform; lambda ignored)
+ *   GPUQT_DAMPING_LORENTZ    g_n = sinh(lambda (1 - n / N_m)) / sinh(lambda), lambda > 0 (typically 3..5):
+ *                            Lorentzian broadening of half width ~ lambda dE / N_m (Green functions)
+ *   GPUQT_DAMPING_NONE       g_n = 1 (plain truncated series, Gibbs oscillations)
+ * Unknown kernel or lambda <= 0 for Lorentz => GPUQT_ERR_ARG.                                      */
+#define GPUQT_DAMPING_JACKSON 0
+#define GPUQT_DAMPING_LORENTZ 1
+#define GPUQT_DAMPING_NONE 2
+int gpuqt_kpm_transform_damped(gpuqt_handle* h, int damping, double lambda, const double* moments_host,
+                               int32_t n_moments, int32_t n_sets, const double* energies_host,
+                               int32_t n_energies, double* out_host);
 
 /* Running conductivity sigma(E, t) in units e = 1 from the TRANSFORMED correlation functions
  * (outputs of gpuqt_kpm_transform), one row per time (PAPER.md:81 Eq. 2, :92 Eq. 5, :123 Eq. 11;
@@ -170,26 +230,27 @@ int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, doubl
  * c_m = (2 - delta_0m) (-i sgn dt)^m J_m(dE |dt|), m < order   (Eq. 17).            */
 int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im);
 
-/* Host only: the work list of a launch that performs two consecutive recurrence steps (DESIGN.md 6,
- * "two steps per launch").  nbr_ptr/nbr_slices: CSR over the 32-row slices of the slices each one
- * gathers from (itself included); the table is cut into runs of `run` slices, CTA c of `grid` takes
- * items c, c + grid, ...  items[2t] = run | step << 30 (run = 2^30 - 1: no-op), items[2t+1] = -1;
- * a second-step item of run R may start when the first step of the runs
- * dep_list[dep_ptr[R] .. dep_ptr[R+1]) is complete; `slack` = items by which it trails them in the
- * list.  items / dep_ptr+dep_list may be NULL to query the sizes.  Exposed so that the schedule's
- * invariants can be tested without a GPU.                                                         */
-int gpuqt_fused_schedule(int32_t n_slices, int32_t run, int32_t grid, int reverse, int32_t slack,
-                         const int32_t* nbr_ptr, const int32_t* nbr_slices, int32_t* items, int32_t capacity,
-                         int32_t* n_items, int32_t* dep_ptr, int32_t* dep_list, int32_t dep_capacity, int32_t* n_dep);
+/* Facts about the handle (what the builder chose), for reports and tests.                          */
+#define GPUQT_INFO_STORED_MATRIX_BYTES 0   /* bytes of the packed records + the x array               */
+#define GPUQT_INFO_HOP_VARIANT 1           /* 0 real per entry, 1 complex per entry, 2 constant hopping
+                                              with int32 columns, 3 constant hopping with 16-bit columns */
+#define GPUQT_INFO_UNIFORM 2               /* 1: every record has width K_max                          */
+#define GPUQT_INFO_UNROLLED_WIDTH 3        /* K_max when the unrolled walk is used (2, 3, 4, 6), else 0 */
+#define GPUQT_INFO_SMALL_PATH 4            /* 1: the one-CTA whole-recurrence kernel is in use         */
+#define GPUQT_INFO_PERSISTENT 5            /* 1: recurrences run as one cooperative multi-step launch  */
+#define GPUQT_INFO_WORKSPACE_USED 6        /* bytes of the workspace actually carved up                */
+int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value);
 
 /* Accumulated device time (CUDA events on the handle's stream around each run of launches) and
  * number of launches of one kernel class since the last reset.                                    */
 int gpuqt_kernel_stats(gpuqt_handle* h, int kernel_class, double* ms, int64_t* launches);
-/* Number of recurrence steps (Eq. 21/23 applications) those launches performed: a launch of the
- * step kernels performs one step, or two consecutive steps fused through L2.        */
+/* Number of recurrence steps (Eq. 21/23 applications) those launches performed: a launch performs
+ * one step, or a whole recurrence in the multi-step forms (persistent / one-CTA kernels).         */
 int gpuqt_kernel_steps(gpuqt_handle* h, int kernel_class, int64_t* steps);
 int gpuqt_reset_stats(gpuqt_handle* h);
 
+/* Text of the last error on this handle; with h == NULL, of the last failed gpuqt_create on the
+ * calling thread.  The pointer stays valid until the next failing call on the same handle / thread. */
 const char* gpuqt_last_error(const gpuqt_handle* h);
 void gpuqt_destroy(gpuqt_handle* h);
 

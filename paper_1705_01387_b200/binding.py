@@ -17,6 +17,21 @@ MODE_VAC, MODE_MSD, MODE_PSI = 1, 2, 4
 STATE_PSI, STATE_CHI, STATE_VAC_A, STATE_VAC_B = 0, 1, 2, 3
 KERNEL_KPM_DOUBLING, KERNEL_KPM_LEFT, KERNEL_EVOLVE, KERNEL_EVOLVE_MSD, KERNEL_VELOCITY = range(5)
 MAX_MOMENTS = 16384
+MAX_ORDER = 4096
+DAMPING_JACKSON, DAMPING_LORENTZ, DAMPING_NONE = 0, 1, 2
+(INFO_STORED_MATRIX_BYTES, INFO_HOP_VARIANT, INFO_UNIFORM, INFO_UNROLLED_WIDTH, INFO_SMALL_PATH, INFO_PERSISTENT,
+ INFO_WORKSPACE_USED) = range(7)
+
+
+class Options(C.Structure):
+    """gpuqt_options (include/gpuqt.h)."""
+    _fields_ = [(n, C.c_int32) for n in ("struct_bytes", "stages", "blocks_per_sm", "run", "alternate", "hop_const",
+                                          "idx16", "small", "persistent")]
+
+
+# overrides applied to every GpuQT() that does not pass its own `options` (the GPU tests run every
+# small case on both the streaming and the one-CTA kernels this way); empty = the library defaults
+DEFAULT_OPTIONS = {}
 
 STATUS = {0: "GPUQT_OK", -1: "GPUQT_ERR_ARG", -2: "GPUQT_ERR_INDEX", -3: "GPUQT_ERR_NOT_HERMITIAN",
           -4: "GPUQT_ERR_SCALE", -5: "GPUQT_ERR_ENERGY", -6: "GPUQT_ERR_STATE", -7: "GPUQT_ERR_CUDA",
@@ -29,8 +44,11 @@ _model_args = [C.c_int64, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp, C.c_double]
 _SIGNATURES = {
     "gpuqt_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int32, C.c_int, C.c_int32, C.c_int]),
     "gpuqt_validate": (C.c_int, _model_args + [C.c_double]),
+    "gpuqt_default_options": (None, [C.POINTER(Options)]),
     "gpuqt_create": (C.c_int, [C.POINTER(C.c_void_p)] + _model_args + [C.c_double, C.c_double, C.c_int32, C.c_int,
                                                                        C.c_void_p, C.c_size_t, C.c_void_p]),
+    "gpuqt_create_with_options": (C.c_int, [C.POINTER(C.c_void_p)] + _model_args + [
+        C.c_double, C.c_double, C.c_int32, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(Options)]),
     "gpuqt_set_state": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gpuqt_set_state_device": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gpuqt_dos_moments": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
@@ -38,13 +56,13 @@ _SIGNATURES = {
     "gpuqt_vac": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_msd": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_kpm_transform": (C.c_int, [C.c_void_p, _dp, C.c_int32, C.c_int32, _dp, C.c_int32, _dp]),
+    "gpuqt_kpm_transform_damped": (C.c_int, [C.c_void_p, C.c_int, C.c_double, _dp, C.c_int32, C.c_int32, _dp, C.c_int32, _dp]),
+    "gpuqt_get_info": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "gpuqt_running_conductivity": (C.c_int, [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int32, C.c_int32, _dp, _dp]),
     "gpuqt_get_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "gpuqt_get_table": (C.c_int, [C.c_void_p, _ip, _dp, _dp, _dp]),
     "gpuqt_bessel_coeffs": (C.c_int, [C.c_double, C.c_double, C.c_int32, _dp, _dp]),
     "gpuqt_kernel_stats": (C.c_int, [C.c_void_p, C.c_int, _dp, C.POINTER(C.c_int64)]),
-    "gpuqt_fused_schedule": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.c_int, C.c_int32, _ip, _ip, _ip, C.c_int32, _ip,
-                                       _ip, _ip, C.c_int32, _ip]),
     "gpuqt_kernel_steps": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "gpuqt_reset_stats": (C.c_int, [C.c_void_p]),
     "gpuqt_last_error": (C.c_char_p, [C.c_void_p]),
@@ -118,31 +136,21 @@ def choose_order(dE, dt, tol=1e-15):
     return int(big[-1]) + 1 if big.size else 1
 
 
-def fused_schedule(nbr_ptr, nbr_slices, run, grid, reverse=0, slack=None):
-    """gpuqt_fused_schedule (host only) -> (items int32 [n_items][2], dep_ptr, dep_list)."""
-    nbr_ptr = np.ascontiguousarray(nbr_ptr, np.int32)
-    nbr_slices = np.ascontiguousarray(nbr_slices, np.int32)
-    n_slices = nbr_ptr.size - 1
-    slack = grid if slack is None else slack
-    n, nd = C.c_int32(), C.c_int32()
-    fn = load().gpuqt_fused_schedule
-    rc = fn(n_slices, run, grid, reverse, slack, _i(nbr_ptr), _i(nbr_slices), None, 0, C.byref(n), None, None, 0, C.byref(nd))
-    if rc:
-        raise GpuqtError(rc, "gpuqt_fused_schedule")
-    items = np.empty((n.value, 2), np.int32)
-    dep_ptr = np.empty((n_slices + run - 1) // run + 1, np.int32)
-    dep_list = np.empty(max(nd.value, 1), np.int32)
-    rc = fn(n_slices, run, grid, reverse, slack, _i(nbr_ptr), _i(nbr_slices), _i(items), n.value, C.byref(n),
-            _i(dep_ptr), _i(dep_list), nd.value, C.byref(nd))
-    if rc:
-        raise GpuqtError(rc, "gpuqt_fused_schedule")
-    return items, dep_ptr, dep_list[:nd.value]
+def default_options(**overrides) -> Options:
+    """gpuqt_default_options, then the given fields overridden."""
+    o = Options()
+    load().gpuqt_default_options(C.byref(o))
+    for k, v in overrides.items():
+        if not hasattr(o, k):
+            raise KeyError(f"unknown gpuqt option {k!r}")
+        setattr(o, k, int(v))
+    return o
 
 
 class GpuQT:
     """One gpuqt_handle on the current CUDA device; workspace and stream come from torch."""
 
-    def __init__(self, model, batch=1, modes=MODE_VAC | MODE_MSD, stream=None):
+    def __init__(self, model, batch=1, modes=MODE_VAC | MODE_MSD, stream=None, options=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("gpuqt needs a CUDA device (no CPU fallback)")
@@ -155,13 +163,14 @@ class GpuQT:
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         self._h = C.c_void_p()
-        rc = lib.gpuqt_create(C.byref(self._h), *_model_tuple(model), C.c_double(model.volume),
-                              C.c_double(model.energy_scale), C.c_int32(batch), C.c_int(modes),
-                              C.c_void_p(self.workspace.data_ptr()), C.c_size_t(nbytes),
-                              C.c_void_p(self.stream.cuda_stream))
+        self.options = default_options(**(DEFAULT_OPTIONS if options is None else options))
+        rc = lib.gpuqt_create_with_options(C.byref(self._h), *_model_tuple(model), C.c_double(model.volume),
+                                           C.c_double(model.energy_scale), C.c_int32(batch), C.c_int(modes),
+                                           C.c_void_p(self.workspace.data_ptr()), C.c_size_t(nbytes),
+                                           C.c_void_p(self.stream.cuda_stream), C.byref(self.options))
         if rc:
             self._h = C.c_void_p()
-            raise GpuqtError(rc, "gpuqt_create")
+            raise GpuqtError(rc, "gpuqt_create", (lib.gpuqt_last_error(None) or b"").decode())
 
     def _ck(self, rc, what):
         if rc:
@@ -229,14 +238,25 @@ class GpuQT:
     def evolve(self, dt, order):
         self._ck(load().gpuqt_evolve(self._h, C.c_double(dt), C.c_int32(order)), "gpuqt_evolve")
 
-    def kpm_transform(self, moments, energies):
+    def kpm_transform(self, moments, energies, damping=None, lam=0.0):
+        """gpuqt_kpm_transform (Jackson, Eq. 31), or gpuqt_kpm_transform_damped with damping = DAMPING_*."""
         moments = np.ascontiguousarray(moments, np.float64)
         energies = np.ascontiguousarray(energies, np.float64)
         m2 = moments.reshape(-1, moments.shape[-1])
         out = np.empty((m2.shape[0], energies.size), np.float64)
-        self._ck(load().gpuqt_kpm_transform(self._h, _d(m2), C.c_int32(m2.shape[1]), C.c_int32(m2.shape[0]),
-                                            _d(energies), C.c_int32(energies.size), _d(out)), "gpuqt_kpm_transform")
+        if damping is None:
+            self._ck(load().gpuqt_kpm_transform(self._h, _d(m2), C.c_int32(m2.shape[1]), C.c_int32(m2.shape[0]),
+                                                _d(energies), C.c_int32(energies.size), _d(out)), "gpuqt_kpm_transform")
+        else:
+            self._ck(load().gpuqt_kpm_transform_damped(self._h, C.c_int(damping), C.c_double(lam), _d(m2),
+                                                       C.c_int32(m2.shape[1]), C.c_int32(m2.shape[0]), _d(energies),
+                                                       C.c_int32(energies.size), _d(out)), "gpuqt_kpm_transform_damped")
         return out
+
+    def info(self, what):
+        v = C.c_int64()
+        self._ck(load().gpuqt_get_info(self._h, what, C.byref(v)), "gpuqt_get_info")
+        return v.value
 
     def running_conductivity(self, kind, corr, dos, dt):
         """kind 'vac' or 'msd'; corr [n_t][n_E] from kpm_transform; returns (sigma, length or None)."""

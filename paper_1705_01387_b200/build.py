@@ -1,7 +1,7 @@
 """Build libgpuqt.so (sm_100a only) in-tree with nvcc.  `python -m paper_1705_01387_b200.build`.
 
-Two translation units (gpuqt.cu: the C-ABI and the single-step kernels; pair_kernels.cu: the opt-in
-two-step kernel) are compiled in parallel and linked into one shared library."""
+Five translation units compiled in parallel and linked into one shared library: gpuqt.cu (the C-ABI,
+host logic and the small kernels) and step_kernels.cu once per Mode of the step kernel."""
 import os
 import subprocess
 import sys
@@ -9,8 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("GPUQT_LIB") or os.path.join(HERE, "libgpuqt.so")
-SOURCES = [os.path.join(CSRC, "gpuqt.cu"), os.path.join(CSRC, "pair_kernels.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "host_util.h")] + [
+UNITS = [("gpuqt.cu", [])] + [("step_kernels.cu", [f"-DGPUQT_TU_MODE={m}"]) for m in range(4)]
+DEPS = [os.path.join(CSRC, f) for f in ("gpuqt.cu", "step_kernels.cu", "kernels.cuh", "host_util.h")] + [
     os.path.join(os.path.dirname(HERE), "include", "gpuqt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
@@ -28,8 +28,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         extra = os.environ.get("GPUQT_NVCC_EXTRA", "").split()      # e.g. -DGPUQT_MINB=1 (kernel tuning macros)
         flags = NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else [])
-        objs = [LIB + "." + os.path.basename(s) + ".o" for s in SOURCES]
-        procs = [subprocess.Popen([nvcc] + flags + ["-c", "-o", o, s]) for s, o in zip(SOURCES, objs)]
+        objs, procs = [], []
+        for i, (src, defs) in enumerate(UNITS):
+            obj = f"{LIB}.{i}.o"
+            objs.append(obj)
+            procs.append(subprocess.Popen([nvcc] + flags + defs + ["-c", "-o", obj, os.path.join(CSRC, src)]))
         codes = [p.wait() for p in procs]
         if any(codes):
             raise subprocess.CalledProcessError(max(codes), "nvcc -c")

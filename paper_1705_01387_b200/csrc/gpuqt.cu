@@ -4,6 +4,8 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <map>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -14,14 +16,15 @@
 using namespace gpuqt;
 
 namespace gpuqt {
-void* pair_kernel_fn(int mode, int B, int kt, int hop);   // pair_kernels.cu
+void* step_kernel_fn(int mode, int B, int kt, int hop);     // step_kernels.cu
 }
 
 namespace {
 
 constexpr int kMaxGrid = 4096;
-constexpr int kPartialDoubles = 64;   // n_steps*Q*B <= 48
-constexpr int kRing = 4;              // recurrence ring: a fused pair reads two slots and writes two
+constexpr int kPartialDoubles = 64;   // 2 * Q*B <= 48 per block
+constexpr int kRing = 3;              // recurrence ring x_m -> ring[(m - 1) % 3]
+constexpr int kCoefSlots = 8;         // Bessel-coefficient uploads in flight (pinned host ring + device mirror)
 
 struct PendingStat {
     int cls;
@@ -29,59 +32,57 @@ struct PendingStat {
     int64_t launches, steps;
 };
 
+thread_local std::string g_create_error;   // gpuqt_last_error(NULL)
+
 }  // namespace
 
 struct gpuqt_handle {
     int64_t N = 0;
     int32_t K = 0, B = 0;
     int modes = 0, cplx = 0, kt = 0, hop = 0;
-    int max_blocks_per_sm = 0;          // GPUQT_BLOCKS_PER_SM (tuning override), 0 = occupancy limit
-    int run = kWarps;                   // GPUQT_RUN: consecutive slices per CTA run (multiple of kWarps)
-    int alternate = 1;                  // GPUQT_ALTERNATE: sweep direction alternates between launches
-    int rec_bytes = 0;                  // bytes of one (widest) slice record
+    gpuqt_options opt{};
+    int run = 16;                       // consecutive tiles per CTA run (multiple of kWarps)
+    int rec_bytes = 0;                  // bytes reserved for the records of one tile inside a stage
     int want_stages = 2;                // requested pipeline depth per warp
-    // per launch configuration [mode + 4 * pair]: stages, bytes per stage, dynamic smem
-    int mode_stages[8] = {0};
-    int mode_stage_bytes[8] = {0};
-    size_t mode_smem[8] = {0};
-    std::vector<void*> smem_set;        // kernels whose dynamic-smem attribute has been raised
+    int persistent = 0;                 // whole recurrences as one cooperative launch
+    int coop_ok = 0;                    // the device supports cooperative launches
+    // per launch configuration [mode]: stages, bytes per stage, dynamic smem
+    int mode_stages[4] = {0};
+    int mode_stage_bytes[4] = {0};
+    size_t mode_smem[4] = {0};
     double dE = 0, box = 0, volume = 0;
     cudaStream_t stream = nullptr;
     int n_sm = 0;
     Mat mat{};
     size_t vec_elems = 0;   // N * B double2
+    size_t stored_matrix_bytes = 0, workspace_used = 0;
     // vectors (device, inside the caller's workspace)
     double2 *psi = nullptr, *chi = nullptr, *va = nullptr, *vb = nullptr, *phiL = nullptr;
-    double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr, nullptr},
-            *ringe[kRing] = {nullptr, nullptr, nullptr, nullptr};
-    // fused pairs of steps: dependency structure of the table and the cached work lists
-    int small = 1;                      // GPUQT_SMALL: one-CTA whole-recurrence kernel when everything fits one SM
-    int fuse = 1, lag = 2;              // GPUQT_FUSE, GPUQT_LAG (slack of the second step in half rounds)
-    std::vector<int> nbr_ptr, nbr_slices;
-    struct DevSchedule {
-        int G, reverse, n_items, n_runs;
-        int2* items;
-        int *dep_ptr, *dep_list;
-        unsigned int* run_done;
-    };
-    std::vector<DevSchedule> schedules;
+    double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr},
+            *ringe[kRing] = {nullptr, nullptr, nullptr};
     // library-owned scratch for the small transform / table-decode calls: grown on demand, kept
     // (stream-ordered pool allocations can trim at every synchronisation and stall the step)
     char* scratch = nullptr;
     size_t scratch_bytes = 0;
+    // Bessel coefficients of the running time steps: pinned host ring -> device mirror
+    double* coef_host = nullptr;
+    double* coef_dev = nullptr;
+    cudaEvent_t coef_event[kCoefSlots] = {nullptr};
+    bool coef_used[kCoefSlots] = {false};
+    int coef_next = 0;
     // B >= 2: one TMA tensor map (128-byte swizzle) per vector buffer, in device memory
     std::vector<const double2*> map_bufs;
     CUtensorMap* d_maps = nullptr;
     double *partials = nullptr, *dots = nullptr, *moments = nullptr;
-    unsigned int* ticket = nullptr;
-    int grid[8] = {0};                  // [mode + 4 * pair]
+    unsigned int *ticket = nullptr, *barrier = nullptr;
+    int grid[4] = {0};                  // [mode]
     int grid_aux = 0;
-    int sweep = 0;                      // direction of the next step launch (reset per building block)
+    int sweep = 0;                      // direction of the next step (reset per building block)
     bool state_set = false;
     std::string err;
     double stat_ms[GPUQT_KERNEL_CLASSES] = {0};
     int64_t stat_launches[GPUQT_KERNEL_CLASSES] = {0};
-    int64_t stat_steps[GPUQT_KERNEL_CLASSES] = {0};     // recurrence steps (a fused launch does two)
+    int64_t stat_steps[GPUQT_KERNEL_CLASSES] = {0};     // recurrence steps (a multi-step launch does many)
     std::vector<PendingStat> pending;
     std::vector<cudaEvent_t> free_events;
 };
@@ -122,7 +123,7 @@ Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
         off = align_up(off + bytes);
         return o;
     };
-    const size_t n_slices = (size_t)((N + 31) / 32);
+    const size_t n_slices = (size_t)((N + 31) / 32) + kTilePad;
     L.rec = take(rec_bytes);
     L.slice_off = take((n_slices + 1) * sizeof(long long));
     L.x = take((size_t)(N + 1) * sizeof(double));
@@ -131,61 +132,38 @@ Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
     L.partials = take((size_t)kMaxGrid * kPartialDoubles * sizeof(double));
     L.dots = take((size_t)GPUQT_MAX_MOMENTS * 3 * 8 * sizeof(double));
     L.moments = take((size_t)GPUQT_MAX_MOMENTS * 8 * sizeof(double));
-    L.ticket = take(256);
+    L.ticket = take(256);                           // [0] last-block ticket, [32] grid-barrier counter
     L.total = off;
     return L;
 }
 
-// shared memory of one step-kernel CTA: mbarriers, then kWarps * stages record buffers
-size_t step_smem_bytes(int stages, int stage_bytes, bool pair = false) {
-    return 128 * (((pair ? 2 : 1) * (size_t)kWarps * kMaxStages * 8 + 127) / 128) + (size_t)kWarps * stages * stage_bytes;
+// shared memory of one step-kernel CTA: mbarriers, then kWarps * stages tile buffers
+size_t step_smem_bytes(int stages, int stage_bytes) {
+    return 128 * (((size_t)kWarps * kMaxStages * 8 + 127) / 128) + (size_t)kWarps * stages * stage_bytes;
 }
 constexpr size_t kSmemBudget = 200 * 1024;   // per CTA; leaves room for the static reduction buffers
 constexpr size_t kSmemPerSm = 227 * 1024;
 
-int env_int(const char* name, int dflt) {
-    const char* v = getenv(name);
-    return (v && *v) ? atoi(v) : dflt;
-}
-
 bool batch_ok(int B) { return B == 1 || B == 2 || B == 4 || B == 8; }
+bool unrolled_width(int K) { return K == 2 || K == 3 || K == 4 || K == 6; }
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of the kernel in this process, not of a
+// handle: raise it (never lower it) under a lock, whichever handle asks
+cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
+    static std::mutex mu;
+    static std::map<void*, size_t> granted;
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t& g = granted[fn];
+    if (bytes <= g) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) g = bytes;
+    return e;
+}
 
 // ---------------------------------------------------------------- kernel dispatch
-template <int MODE, int BB, int KK>
-void* step_fn(int hop) {
-    if (KK > 0 && hop == kHopConst16)      // 16-bit columns exist for the unrolled uniform tables only
-        return (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>;
-    return hop == kHopComplex ? (void*)cheb_step_kernel<BB, KK, kHopComplex, MODE>
-           : hop == kHopConst ? (void*)cheb_step_kernel<BB, KK, kHopConst, MODE>
-                              : (void*)cheb_step_kernel<BB, KK, kHopReal, MODE>;
-}
-template <int MODE, int BB>
-void* step_fn_k(int kt, int hop) {
-    switch (kt) {
-    case 3: return step_fn<MODE, BB, 3>(hop);
-    case 4: return step_fn<MODE, BB, 4>(hop);
-    case 6: return step_fn<MODE, BB, 6>(hop);
-    default: return step_fn<MODE, BB, 0>(hop);
-    }
-}
-template <int MODE>
-void* step_fn_b(int B, int kt, int hop) {
-    switch (B) {
-    case 1: return step_fn_k<MODE, 1>(kt, hop);
-    case 2: return step_fn_k<MODE, 2>(kt, hop);
-    case 4: return step_fn_k<MODE, 4>(kt, hop);
-    default: return step_fn_k<MODE, 8>(kt, hop);
-    }
-}
-void* step_kernel(const gpuqt_handle* h, int mode, bool pair) {
-    if (pair) return pair_kernel_fn(mode, h->B, h->kt, h->hop);     // pair_kernels.cu
-    switch (mode) {
-    case kModeDoubling: return step_fn_b<kModeDoubling>(h->B, h->kt, h->hop);
-    case kModeLeft: return step_fn_b<kModeLeft>(h->B, h->kt, h->hop);
-    case kModeEvolve: return step_fn_b<kModeEvolve>(h->B, h->kt, h->hop);
-    default: return step_fn_b<kModeEvolveMsd>(h->B, h->kt, h->hop);
-    }
-}
+// the cheb_step_kernel instantiations live in step_kernels.cu, one translation unit per Mode
+void* step_kernel(const gpuqt_handle* h, int mode) { return gpuqt::step_kernel_fn(mode, h->B, h->kt, h->hop); }
 
 void* velocity_fn(const gpuqt_handle* h) {
     switch (h->B) {
@@ -208,7 +186,7 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items, int t
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem) != cudaSuccess || per_sm < 1)
         per_sm = 1;
-    if (h->max_blocks_per_sm > 0 && per_sm > h->max_blocks_per_sm) per_sm = h->max_blocks_per_sm;
+    if (h->opt.blocks_per_sm > 0 && per_sm > h->opt.blocks_per_sm) per_sm = h->opt.blocks_per_sm;
     long long g = (long long)per_sm * h->n_sm;
     if (g > work_items) g = work_items;
     if (g > kMaxGrid) g = kMaxGrid;
@@ -216,84 +194,57 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items, int t
     return (int)g;
 }
 
-// bytes of one stage of a step kernel: the record plus the staged own rows of T_{m-1}, T_{m-2}
-// (and e_{m-1}, e_{m-2} for the (a, e) pair)
-int mode_stage_bytes_for(const gpuqt_handle* h, int mode, bool pair = false) {
+// bytes of one stage of a step kernel: the records of a tile plus the staged own rows of x_{m-1},
+// x_{m-2} (and e_{m-1}, e_{m-2} for the (a, e) pair)
+int mode_stage_bytes_for(const gpuqt_handle* h, int mode) {
     int streams = (mode == kModeEvolveMsd) ? 4 : 2;
-    if (h->B >= 8) streams /= 2;   // PrevDirect<8>: T_{m-2} rows are not staged
-    return h->rec_bytes + streams * 32 * h->B * (int)sizeof(double2) + (pair ? kHdrBytes : 0);
+    if (h->B >= 8) streams /= 2;   // PrevDirect<8>: x_{m-2} rows are not staged
+    return h->rec_bytes + streams * tile_slices(h->B, h->kt) * 32 * h->B * (int)sizeof(double2);
 }
 
-cudaError_t launch_step(gpuqt_handle* h, int mode, StepArgs& a) {
-    const bool pair = a.n_steps == 2;
-    const int cfg = mode + (pair ? 4 : 0);
-    const int threads = pair ? kThreads + 32 : kThreads;     // the pair kernel has a producer warp
-    void* fn = step_kernel(h, mode, pair);
-    if (!h->grid[cfg]) {
-        const int sb = mode_stage_bytes_for(h, mode, pair);
-        int stages = h->want_stages;
-        while (stages > 1 && step_smem_bytes(stages, sb, pair) > kSmemBudget) --stages;
-        // prefer two resident CTAs per SM over a deeper pipeline
-        while (stages > 2 && 2 * (step_smem_bytes(stages, sb, pair) + 4096) > kSmemPerSm) --stages;
-        h->mode_stages[cfg] = stages;
-        h->mode_stage_bytes[cfg] = sb;
-        h->mode_smem[cfg] = step_smem_bytes(stages, sb, pair);
-        if (h->mode_smem[cfg] > 48 * 1024) {
-            cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->mode_smem[cfg]);
-            if (e != cudaSuccess) return e;
-        }
-        h->grid[cfg] = grid_for(h, fn, h->mode_smem[cfg], (h->mat.n_slices + h->run - 1) / h->run, threads);
-    }
-    a.sched = nullptr;
-    a.n_items = 0;
-    a.run_done = nullptr;
-    a.dep_ptr = nullptr;
-    a.dep_list = nullptr;
-    if (a.n_steps == 2) {
-        const int reverse = h->alternate ? (h->sweep & 1) : 0;
-        const gpuqt_handle::DevSchedule* ds = nullptr;
-        for (const auto& d : h->schedules)
-            if (d.G == h->grid[cfg] && d.reverse == reverse) ds = &d;
-        if (!ds) {
-            FusedSchedule fs;
-            build_fused_schedule((int)h->mat.n_slices, h->run, h->grid[cfg], reverse, std::max(1, h->lag * h->grid[cfg] / 2),
-                                 kNoRun, h->nbr_ptr, h->nbr_slices, fs);
-            gpuqt_handle::DevSchedule d{};
-            d.G = h->grid[cfg];
-            d.reverse = reverse;
-            d.n_items = (int)(fs.items.size() / 2);
-            d.n_runs = (int)fs.dep_ptr.size() - 1;
-            auto up = [&](void** dst, const std::vector<int>& v) {
-                cudaError_t e = cudaMalloc(dst, std::max<size_t>(v.size(), 1) * sizeof(int));
-                if (e == cudaSuccess && !v.empty()) e = cudaMemcpy(*dst, v.data(), v.size() * sizeof(int), cudaMemcpyHostToDevice);
-                return e;
-            };
-            cudaError_t e = up((void**)&d.items, fs.items);
-            if (e == cudaSuccess) e = up((void**)&d.dep_ptr, fs.dep_ptr);
-            if (e == cudaSuccess) e = up((void**)&d.dep_list, fs.dep_list);
-            if (e == cudaSuccess) e = cudaMalloc((void**)&d.run_done, (size_t)d.n_runs * sizeof(unsigned int));
-            if (e != cudaSuccess) return e;
-            h->schedules.push_back(d);
-            ds = &h->schedules.back();
-        }
-        cudaError_t e = cudaMemsetAsync(ds->run_done, 0, (size_t)ds->n_runs * sizeof(unsigned int), h->stream);
-        if (e != cudaSuccess) return e;
-        a.sched = ds->items;
-        a.n_items = ds->n_items;
-        a.run_done = ds->run_done;
-        a.dep_ptr = ds->dep_ptr;
-        a.dep_list = ds->dep_list;
-    }
-    a.stages = h->mode_stages[cfg];
-    a.stage_bytes = h->mode_stage_bytes[cfg];
+long long n_tiles_of(const gpuqt_handle* h) {
+    const int S = tile_slices(h->B, h->kt);
+    return (h->mat.n_slices + S - 1) / S;
+}
+
+cudaError_t configure_mode(gpuqt_handle* h, int mode) {
+    if (h->grid[mode]) return cudaSuccess;
+    void* fn = step_kernel(h, mode);
+    const int sb = mode_stage_bytes_for(h, mode);
+    int stages = h->want_stages;
+    while (stages > 1 && step_smem_bytes(stages, sb) > kSmemBudget) --stages;
+    // prefer two resident CTAs per SM over a deeper pipeline
+    while (stages > 2 && 2 * (step_smem_bytes(stages, sb) + 4096) > kSmemPerSm) --stages;
+    h->mode_stages[mode] = stages;
+    h->mode_stage_bytes[mode] = sb;
+    h->mode_smem[mode] = step_smem_bytes(stages, sb);
+    cudaError_t e = ensure_dynamic_smem(fn, h->mode_smem[mode]);
+    if (e != cudaSuccess) return e;
+    h->grid[mode] = grid_for(h, fn, h->mode_smem[mode], (n_tiles_of(h) + h->run - 1) / h->run);
+    return cudaSuccess;
+}
+
+// steps [a.m_begin, a.m_end) of a recurrence: a plain launch for one step, a cooperative launch for several
+cudaError_t launch_steps(gpuqt_handle* h, int mode, RecArgs& a) {
+    cudaError_t e = configure_mode(h, mode);
+    if (e != cudaSuccess) return e;
+    void* fn = step_kernel(h, mode);
+    a.stages = h->mode_stages[mode];
+    a.stage_bytes = h->mode_stage_bytes[mode];
     a.rec_bytes = h->rec_bytes;
     a.partials = h->partials;
     a.ticket = h->ticket;
-    a.reverse = h->alternate ? (h->sweep & 1) : 0;
+    a.barrier = h->barrier;
+    a.alternate = h->opt.alternate;
+    a.sweep0 = h->opt.alternate ? (h->sweep & 1) : 0;
     a.run = h->run;
-    h->sweep ^= 1;
+    const int n = a.m_end - a.m_begin;
+    h->sweep += n;
     void* args[] = {(void*)&h->mat, (void*)&a};
-    return cudaLaunchKernel(fn, dim3(h->grid[cfg]), dim3(threads), args, h->mode_smem[cfg], h->stream);
+    if (!a.multi) return cudaLaunchKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, h->mode_smem[mode], h->stream);
+    e = cudaMemsetAsync(h->barrier, 0, sizeof(unsigned int), h->stream);
+    if (e != cudaSuccess) return e;
+    return cudaLaunchCooperativeKernel(fn, dim3(h->grid[mode]), dim3(kThreads), args, h->mode_smem[mode], h->stream);
 }
 
 cudaError_t launch_velocity(gpuqt_handle* h, const double2* in, double2* out) {
@@ -361,6 +312,32 @@ cudaError_t ensure_scratch(gpuqt_handle* h, size_t bytes) {
     return e;
 }
 
+// The c_k of one time step -> device, through a ring of pinned host slots (no pageable copy, so the
+// host never waits for the stream).  Returns the device address of (re, im) pairs, k < order.
+cudaError_t upload_coefs(gpuqt_handle* h, const std::vector<double>& cr, const std::vector<double>& ci, int order,
+                         const double** dev) {
+    const int slot = h->coef_next;
+    h->coef_next = (slot + 1) % kCoefSlots;
+    cudaError_t e;
+    if (h->coef_used[slot]) {
+        e = cudaEventSynchronize(h->coef_event[slot]);      // the copy out of this pinned slot has run
+        if (e != cudaSuccess) return e;
+    }
+    double* hs = h->coef_host + (size_t)slot * 2 * GPUQT_MAX_ORDER;
+    double* ds = h->coef_dev + (size_t)slot * 2 * GPUQT_MAX_ORDER;
+    for (int k = 0; k < order; ++k) {
+        hs[2 * k] = cr[(size_t)k];
+        hs[2 * k + 1] = ci[(size_t)k];
+    }
+    e = cudaMemcpyAsync(ds, hs, (size_t)order * 2 * sizeof(double), cudaMemcpyHostToDevice, h->stream);
+    if (e != cudaSuccess) return e;
+    e = cudaEventRecord(h->coef_event[slot], h->stream);
+    if (e != cudaSuccess) return e;
+    h->coef_used[slot] = true;
+    *dev = ds;
+    return cudaSuccess;
+}
+
 // ---------------------------------------------------------------- timing statistics
 cudaEvent_t get_event(gpuqt_handle* h) {
     if (!h->free_events.empty()) {
@@ -412,7 +389,7 @@ size_t small_smem_bytes(const gpuqt_handle* h) {
     const size_t NB = (size_t)h->N * h->B, KN = (size_t)h->K * h->N;
     return 4 * NB * sizeof(double2) + (size_t)h->N * 8 + KN * 8 * (size_t)hop_doubles(h->hop) + KN * 4 + 16;
 }
-bool small_ok(const gpuqt_handle* h) { return h->small && small_smem_bytes(h) <= 210 * 1024; }
+bool small_ok(const gpuqt_handle* h) { return h->opt.small && small_smem_bytes(h) <= 210 * 1024; }
 
 template <int MODE>
 void* small_fn(int B) {
@@ -428,54 +405,47 @@ cudaError_t launch_small(gpuqt_handle* h, int mode, SmallArgs& a) {
                : mode == kModeLeft   ? small_fn<kModeLeft>(h->B)
                                      : small_fn<kModeEvolve>(h->B);
     const size_t smem = small_smem_bytes(h);
-    if (std::find(h->smem_set.begin(), h->smem_set.end(), fn) == h->smem_set.end()) {
-        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        h->smem_set.push_back(fn);
-    }
+    cudaError_t e = ensure_dynamic_smem(fn, smem);
+    if (e != cudaSuccess) return e;
     void* args[] = {(void*)&h->mat, (void*)&a};
     return cudaLaunchKernel(fn, dim3(1), dim3(kSmallThreads), args, smem, h->stream);
 }
 
-// Driver of one three-term recurrence: launches m = 1 .. terms-1, each x_m = 2 H~ x_{m-1} - x_{m-2} (+ ...)
-// (and the e-chain of the MSD pair).  Launch 1 has no x_{-1}.  Forward recurrences (moments) apply
-// factor 1 in launch 1 (T_1 = H~ T_0); Clenshaw recurrences (evolution) apply factor 1 in the LAST
-// launch.  In between two consecutive terms share one launch when fusing is on (kernels.cuh,
-// cheb_pair_kernel).  fill(io, m) sets the per-term fields (coefficient, dot destination, store flag,
-// output override).
-template <class Fill>
-int run_recurrence(gpuqt_handle* h, int mode, int cls, int terms, const double2* t0, const double2* e0,
-                   const StepArgs& base, bool clenshaw, Fill fill) {
+// Driver of one three-term recurrence x_m = 2 H~ x_{m-1} - x_{m-2} (+ ...), m = 1 .. terms-1 (and the
+// e-chain of the MSD pair).  Forward recurrences (moments) apply factor 1 in step 1 (T_1 = H~ T_0);
+// Clenshaw recurrences (evolution) in the LAST step.  One plain launch per step, or -- persistent
+// mode -- the whole recurrence in one cooperative launch with grid barriers between the steps.
+int run_recurrence(gpuqt_handle* h, int mode, int cls, RecArgs a) {
     StatScope s(h, cls);
-    const double2 *tm1 = t0, *tm2 = nullptr, *em1 = e0, *em2 = nullptr;
-    int slot = 0, m = 1;
-    while (m < terms) {
-        StepArgs a = base;
-        a.first = (m == 1);
-        a.half = clenshaw ? (m == terms - 1) : (m == 1);
-        a.n_steps = (h->fuse && m >= 2 && m + 1 + (clenshaw ? 1 : 0) < terms) ? 2 : 1;
-        for (int k = 0; k < a.n_steps; ++k) {
-            StepIO& io = a.io[k];
-            double2* tnew = h->ring[slot];
-            io.in = tm1; io.prev = tm2; io.out = tnew;
-            if (e0) {
-                io.in_e = em1; io.prev_e = em2; io.out_e = h->ringe[slot];
-            }
-            slot = (slot + 1) % kRing;
-            io.store = 1;
-            io.tm_in = tensor_map_of(h, io.in);
-            io.tm_prev = tensor_map_of(h, io.prev);
-            io.tm_in_e = tensor_map_of(h, io.in_e);
-            io.tm_prev_e = tensor_map_of(h, io.prev_e);
-            fill(io, m + k);
-            tm2 = tm1; tm1 = io.out;
-            if (e0) {
-                em2 = em1; em1 = io.out_e;
-            }
+    for (int i = 0; i < kRing; ++i) {
+        a.ring[i] = h->ring[i];
+        a.tm_ring[i] = tensor_map_of(h, h->ring[i]);
+        a.ring_e[i] = a.e0 ? h->ringe[i] : nullptr;
+        a.tm_ring_e[i] = a.e0 ? tensor_map_of(h, h->ringe[i]) : nullptr;
+    }
+    a.tm_x0 = tensor_map_of(h, a.x0);
+    a.tm_e0 = tensor_map_of(h, a.e0);
+    if (a.terms < 2) return GPUQT_OK;
+    if (h->persistent) {
+        a.multi = 1;
+        a.m_begin = 1;
+        a.m_end = a.terms;
+        cudaError_t e = launch_steps(h, mode, a);
+        if (e == cudaSuccess) {
+            s.count(1, a.terms - 1);
+            return GPUQT_OK;
         }
-        CU(launch_step(h, mode, a));
-        s.count(1, a.n_steps);
-        m += a.n_steps;
+        if (e != cudaErrorCooperativeLaunchTooLarge && e != cudaErrorNotSupported) return cuda_fail(h, e, "cooperative launch");
+        (void)cudaGetLastError();       // the device is shared (MPS, another context): fall back to one launch per step
+        h->persistent = 0;
+        h->sweep -= a.terms - 1;
+    }
+    a.multi = 0;
+    for (int m = 1; m < a.terms; ++m) {
+        a.m_begin = m;
+        a.m_end = m + 1;
+        CU(launch_steps(h, mode, a));
+        s.count(1, 1);
     }
     return GPUQT_OK;
 }
@@ -488,26 +458,12 @@ cudaError_t launch_scale(gpuqt_handle* h, double cr, double ci, const double2* i
 
 // out <- sum_{k<order} c_k T_k(H~) in  (Eq. 17, 21, 23) by Clenshaw's backward recurrence
 //   b_{order-1} = c_{order-1} in,  b_k = c_k in + 2 H~ b_{k+1} - b_{k+2},  out = c_0 in + H~ b_1 - b_2:
-// the same order - 1 SpMV launches as the forward form, but no accumulator is read-modified-written
+// the same order - 1 SpMV steps as the forward form, but no accumulator is read-modified-written
 // (64 instead of 80 bytes per row and term).  The same for the (psi, chi) pair with the block operator
 // [[H~, 0], [[X,H~], H~]] (a_m = T_m psi, e_m = T_m chi + [X,T_m] psi, Eq. 18, 22, 24).
 // `in` is left untouched; `out` must differ from in and from the ring buffers.
 int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const double2* in_e, double2* out,
                     double2* out_e, const std::vector<double>& cr, const std::vector<double>& ci, int order) {
-    if (!in_e && small_ok(h) && (size_t)order * 2 <= (size_t)GPUQT_MAX_MOMENTS * 8) {
-        std::vector<double> c((size_t)order * 2);
-        for (int k = 0; k < order; ++k) {
-            c[(size_t)2 * k] = cr[(size_t)k];
-            c[(size_t)2 * k + 1] = ci[(size_t)k];
-        }
-        CU(cudaMemcpyAsync(h->moments, c.data(), c.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-        SmallArgs a{};
-        a.aux = in; a.out = out; a.coef = (const double2*)h->moments; a.n_terms = order;
-        StatScope s(h, cls);
-        CU(launch_small(h, kModeEvolve, a));
-        s.count(1, order > 1 ? order - 1 : 0);
-        return GPUQT_OK;
-    }
     if (order == 1) {
         StatScope s(h, cls);
         CU(launch_scale(h, cr[0], ci[0], in, out));
@@ -515,8 +471,18 @@ int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const
         s.count(in_e ? 2 : 1, 0);
         return GPUQT_OK;
     }
-    // b_{order-1} lives in the last ring slot: the recurrence writes slots 0, 1, 2, ... and needs it
-    // only in its first two launches
+    const double* coef = nullptr;
+    CU(upload_coefs(h, cr, ci, order, &coef));
+    if (!in_e && small_ok(h)) {
+        SmallArgs a{};
+        a.aux = in; a.out = out; a.coef = (const double2*)coef; a.n_terms = order;
+        StatScope s(h, cls);
+        CU(launch_small(h, kModeEvolve, a));
+        s.count(1, order - 1);
+        return GPUQT_OK;
+    }
+    // x_0 = b_{order-1} lives in the last ring slot: the recurrence writes slots 0, 1, 2, 0, ... and
+    // needs x_0 only in its first two steps
     double2* b0 = h->ring[kRing - 1];
     double2* b0_e = in_e ? h->ringe[kRing - 1] : nullptr;
     {
@@ -525,18 +491,15 @@ int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const
         if (in_e) CU(launch_scale(h, cr[(size_t)order - 1], ci[(size_t)order - 1], in_e, b0_e));
         s.count(in_e ? 2 : 1, 0);
     }
-    StepArgs base{};
-    base.src = in;
-    base.src_e = in_e;
-    return run_recurrence(h, mode, cls, order, b0, b0_e, base, true, [&](StepIO& io, int m) {
-        const int k = order - 1 - m;            // this launch produces b_k
-        io.cr = cr[(size_t)k];
-        io.ci = ci[(size_t)k];
-        if (k == 0) {
-            io.out = out;
-            if (in_e) io.out_e = out_e;
-        }
-    });
+    RecArgs a{};
+    a.x0 = b0; a.e0 = b0_e;
+    a.src = in; a.src_e = in_e;
+    a.coef = coef;
+    a.terms = order;
+    a.clenshaw = 1;
+    a.store_last = 1;
+    a.last_out = out; a.last_out_e = out_e;
+    return run_recurrence(h, mode, cls, a);
 }
 
 int evolve_one(gpuqt_handle* h, const double2* in, double2* out, const std::vector<double>& cr,
@@ -559,23 +522,18 @@ int moments_doubling(gpuqt_handle* h, const double2* v, int n_moments) {
     if (small_ok(h)) {
         SmallArgs a{};
         a.v0 = v; a.dots = h->dots; a.n_terms = n_steps + 1;
-        {
-            StatScope s(h, GPUQT_KERNEL_KPM_DOUBLING);
-            CU(launch_small(h, kModeDoubling, a));
-            s.count(1, n_steps);
-        }
-        const int total = h->B * n_moments;
-        finalize_doubling<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, n_steps, h->dots, h->moments);
-        CU(cudaGetLastError());
-        return GPUQT_OK;
+        StatScope s(h, GPUQT_KERNEL_KPM_DOUBLING);
+        CU(launch_small(h, kModeDoubling, a));
+        s.count(1, n_steps);
+    } else {
+        RecArgs a{};
+        a.x0 = v;
+        a.terms = n_steps + 1;
+        a.dots = h->dots;        // step m -> dots[(m - 1) * 3 B]
+        a.dot_m0 = 1;
+        int rc = run_recurrence(h, kModeDoubling, GPUQT_KERNEL_KPM_DOUBLING, a);
+        if (rc) return rc;
     }
-    StepArgs base{};
-    int rc = run_recurrence(h, kModeDoubling, GPUQT_KERNEL_KPM_DOUBLING, n_steps + 1, v, nullptr, base, false,
-                            [&](StepIO& io, int m) {
-                                io.store = (m < n_steps);
-                                io.result = h->dots + (size_t)(m - 1) * 3 * h->B;
-                            });
-    if (rc) return rc;
     const int total = h->B * n_moments;
     finalize_doubling<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, n_steps, h->dots, h->moments);
     CU(cudaGetLastError());
@@ -588,23 +546,19 @@ int moments_left(gpuqt_handle* h, const double2* l, const double2* r, int n_mome
     if (small_ok(h)) {
         SmallArgs a{};
         a.v0 = r; a.aux = l; a.dots = h->dots; a.n_terms = n_moments;
-        {
-            StatScope s(h, GPUQT_KERNEL_KPM_LEFT);
-            CU(launch_small(h, kModeLeft, a));
-            s.count(1, n_moments - 1);
-        }
-        const int total = h->B * n_moments;
-        finalize_left<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, h->dots, h->moments);
-        CU(cudaGetLastError());
-        return GPUQT_OK;
+        StatScope s(h, GPUQT_KERNEL_KPM_LEFT);
+        CU(launch_small(h, kModeLeft, a));
+        s.count(1, n_moments - 1);
+    } else {
+        RecArgs a{};
+        a.x0 = r;
+        a.phiL = l;
+        a.terms = n_moments;
+        a.dots = h->dots;        // step n -> dots[n * 2 B]
+        a.dot_m0 = 0;
+        int rc = run_recurrence(h, kModeLeft, GPUQT_KERNEL_KPM_LEFT, a);
+        if (rc) return rc;
     }
-    StepArgs base{};
-    base.phiL = l;
-    int rc = run_recurrence(h, kModeLeft, GPUQT_KERNEL_KPM_LEFT, n_moments, r, nullptr, base, false, [&](StepIO& io, int n) {
-        io.store = (n + 1 < n_moments);
-        io.result = h->dots + (size_t)n * 2 * h->B;
-    });
-    if (rc) return rc;
     const int total = h->B * n_moments;
     finalize_left<<<(total + 255) / 256, 256, 0, h->stream>>>(h->B, n_moments, h->dots, h->moments);
     CU(cudaGetLastError());
@@ -643,10 +597,23 @@ int finish_set_state(gpuqt_handle* h) {
 // =================================================================== C ABI
 extern "C" {
 
+void gpuqt_default_options(gpuqt_options* o) {
+    if (!o) return;
+    o->struct_bytes = (int32_t)sizeof(gpuqt_options);
+    o->stages = 0;
+    o->blocks_per_sm = 0;
+    o->run = 0;
+    o->alternate = 1;
+    o->hop_const = 1;
+    o->idx16 = 1;
+    o->small = 1;
+    o->persistent = -1;
+}
+
 size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes) {
     if (N <= 0 || K_max <= 0 || !batch_ok(batch)) return 0;
-    // upper bound: every slice record padded to K_max
-    const size_t rec = (size_t)((N + 31) / 32) * (size_t)record_bytes(K_max, is_complex ? 2 : 1);
+    // upper bound: every slice record padded to K_max, per-entry hoppings, int32 columns
+    const size_t rec = (size_t)((N + 31) / 32 + kTilePad) * (size_t)record_bytes(K_max, is_complex ? 2 : 1);
     return make_layout(N, batch, modes, rec).total;
 }
 
@@ -655,27 +622,6 @@ int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int
                    const double* x, double box_length, double energy_scale) {
     std::string msg;
     return validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
-}
-
-int gpuqt_fused_schedule(int32_t n_slices, int32_t run, int32_t grid, int reverse, int32_t slack,
-                         const int32_t* nbr_ptr, const int32_t* nbr_slices, int32_t* items, int32_t capacity,
-                         int32_t* n_items, int32_t* dep_ptr, int32_t* dep_list, int32_t dep_capacity, int32_t* n_dep) {
-    if (n_slices < 1 || run < 1 || grid < 1 || slack < 1 || !nbr_ptr || !nbr_slices || !n_items || !n_dep) return GPUQT_ERR_ARG;
-    std::vector<int> np(nbr_ptr, nbr_ptr + n_slices + 1), ns(nbr_slices, nbr_slices + nbr_ptr[n_slices]);
-    FusedSchedule fs;
-    build_fused_schedule(n_slices, run, grid, reverse, slack, kNoRun, np, ns, fs);
-    *n_items = (int32_t)(fs.items.size() / 2);
-    *n_dep = (int32_t)fs.dep_list.size();
-    if (items) {
-        if (*n_items > capacity) return GPUQT_ERR_NOMEM;
-        for (size_t i = 0; i < fs.items.size(); ++i) items[i] = fs.items[i];
-    }
-    if (dep_ptr && dep_list) {
-        if (*n_dep > dep_capacity) return GPUQT_ERR_NOMEM;
-        for (size_t i = 0; i < fs.dep_ptr.size(); ++i) dep_ptr[i] = fs.dep_ptr[i];
-        for (size_t i = 0; i < fs.dep_list.size(); ++i) dep_list[i] = fs.dep_list[i];
-    }
-    return GPUQT_OK;
 }
 
 int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im) {
@@ -694,50 +640,73 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
                  const double* onsite, const double* x, double box_length, double volume,
                  double energy_scale, int32_t batch, int modes, void* workspace,
                  size_t workspace_bytes, void* cuda_stream) {
-    if (!out) return GPUQT_ERR_ARG;
+    return gpuqt_create_with_options(out, N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, volume,
+                                     energy_scale, batch, modes, workspace, workspace_bytes, cuda_stream, nullptr);
+}
+
+int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nbr_count,
+                 const int32_t* nbr_index, const double* hop_re, const double* hop_im,
+                 const double* onsite, const double* x, double box_length, double volume,
+                 double energy_scale, int32_t batch, int modes, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream, const gpuqt_options* options) {
+    auto bad = [&](int code, const std::string& msg) {
+        g_create_error = "gpuqt_create: " + msg;
+        return code;
+    };
+    if (!out) return bad(GPUQT_ERR_ARG, "null output pointer");
     *out = nullptr;
-    if (!batch_ok(batch) || !workspace || !(volume > 0.0) || (modes & ~7)) return GPUQT_ERR_ARG;
+    if (!batch_ok(batch)) return bad(GPUQT_ERR_ARG, "batch must be 1, 2, 4 or 8");
+    if (!workspace || !(volume > 0.0) || (modes & ~7)) return bad(GPUQT_ERR_ARG, "null workspace, non-positive volume or unknown mode bits");
+    gpuqt_options opt;
+    gpuqt_default_options(&opt);
+    if (options) {
+        if (options->struct_bytes < (int32_t)sizeof(int32_t) || options->struct_bytes > (int32_t)sizeof(gpuqt_options))
+            return bad(GPUQT_ERR_ARG, "gpuqt_options.struct_bytes does not match this library (use gpuqt_default_options)");
+        std::memcpy(&opt, options, (size_t)options->struct_bytes);     // an older, shorter struct keeps the newer defaults
+        opt.struct_bytes = (int32_t)sizeof(gpuqt_options);
+    }
+    if (opt.stages < 0 || opt.stages > kMaxStages || opt.blocks_per_sm < 0 || opt.run < 0 || opt.persistent < -1 || opt.persistent > 1)
+        return bad(GPUQT_ERR_ARG, "option out of range");
     std::string msg;
     int rc = validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
-    if (rc != GPUQT_OK) {
-        fprintf(stderr, "gpuqt_create: %s\n", msg.c_str());
-        return rc;
-    }
-    if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return GPUQT_ERR_ARG;
+    if (rc != GPUQT_OK) return bad(rc, msg);
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return bad(GPUQT_ERR_ARG, "workspace must be 256-byte aligned");
     if (modes & GPUQT_MODE_MSD) modes |= GPUQT_MODE_PSI;
     gpuqt_handle* h = new (std::nothrow) gpuqt_handle();
-    if (!h) return GPUQT_ERR_NOMEM;
+    if (!h) return bad(GPUQT_ERR_NOMEM, "out of host memory");
     h->N = N; h->K = K_max; h->B = batch; h->modes = modes; h->cplx = hop_im ? 1 : 0;
+    h->opt = opt;
     h->dE = energy_scale; h->box = box_length; h->volume = volume;
     h->stream = (cudaStream_t)cuda_stream;
     h->vec_elems = (size_t)N * batch;
 
     SellHost sell;
-    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, env_int("GPUQT_HOP_CONST", 1) != 0, sell);
-    // 16-bit columns: only where the unrolled uniform kernels exist (K_max 3, 4, 6)
-    if (env_int("GPUQT_IDX16", 1) != 0 && (K_max == 3 || K_max == 4 || K_max == 6)) try_idx16(sell, K_max);
+    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell);
+    // 16-bit columns: only where the unrolled uniform kernels exist
+    if (opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, N);
     h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : sell.idx16 ? kHopConst16 : kHopConst;
-    const int stage_bytes = (int)align_up((size_t)hop_record_bytes(K_max, h->hop), 256);   // keeps the vector rows 256-byte aligned
-    h->rec_bytes = stage_bytes;
-    if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd, true), true) > kSmemBudget) {
-        fprintf(stderr, "gpuqt_create: K_max = %d is too large: one slice record (%d bytes) per warp must fit in "
-                        "shared memory\n", K_max, stage_bytes);
+    h->kt = (sell.uniform && unrolled_width(K_max)) ? K_max : 0;
+    // bytes reserved for the records of one tile inside a stage (keeps the vector rows 256-byte aligned)
+    h->rec_bytes = (int)align_up((size_t)hop_record_bytes(K_max, h->hop) * tile_slices(batch, h->kt), 256);
+    if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd)) > kSmemBudget) {
         delete h;
-        return GPUQT_ERR_ARG;
+        return bad(GPUQT_ERR_ARG, "K_max = " + std::to_string(K_max) + " is too large: one slice record per warp must fit in shared memory");
     }
     const size_t rec_bytes = sell.rec.size();
     const Layout L = make_layout(N, batch, modes, rec_bytes);
     if (L.total > workspace_bytes) {
         delete h;
-        return GPUQT_ERR_NOMEM;
+        return bad(GPUQT_ERR_NOMEM, "workspace too small: " + std::to_string(L.total) + " bytes needed");
     }
+    h->workspace_used = L.total;
+    h->stored_matrix_bytes = rec_bytes + (size_t)(N + 1) * sizeof(double);
     int dev = 0;
     cudaError_t ce = cudaGetDevice(&dev);
     if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&h->coop_ok, cudaDevAttrCooperativeLaunch, dev);
     if (ce != cudaSuccess) {
-        fprintf(stderr, "gpuqt_create: no usable CUDA device: %s\n", cudaGetErrorString(ce));
         delete h;
-        return GPUQT_ERR_CUDA;
+        return bad(GPUQT_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(ce));
     }
     char* base = (char*)workspace;
     unsigned char* d_rec = (unsigned char*)(base + L.rec);
@@ -755,35 +724,29 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     if (ce == cudaSuccess) ce = up(d_sp, sell.slice_off.data(), sell.slice_off.size() * sizeof(long long));
     if (ce == cudaSuccess) ce = cudaMemsetAsync(base + L.ticket, 0, 256, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+    if (ce == cudaSuccess) ce = cudaMallocHost((void**)&h->coef_host, (size_t)kCoefSlots * 2 * GPUQT_MAX_ORDER * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&h->coef_dev, (size_t)kCoefSlots * 2 * GPUQT_MAX_ORDER * sizeof(double));
+    for (int i = 0; i < kCoefSlots && ce == cudaSuccess; ++i) ce = cudaEventCreateWithFlags(&h->coef_event[i], cudaEventDisableTiming);
     if (ce != cudaSuccess) {
-        fprintf(stderr, "gpuqt_create: upload failed: %s\n", cudaGetErrorString(ce));
-        delete h;
-        return GPUQT_ERR_CUDA;
+        const std::string why = cudaGetErrorString(ce);
+        gpuqt_destroy(h);
+        return bad(GPUQT_ERR_CUDA, "upload failed: " + why);
     }
     h->mat.rec = d_rec; h->mat.slice_off = d_sp; h->mat.x = d_x;
     h->mat.N = N; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
     h->mat.cplx = h->cplx; h->mat.hop = h->hop; h->mat.hop_const = sell.hop_const;
     h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
-    h->kt = (sell.uniform && (K_max == 3 || K_max == 4 || K_max == 6)) ? K_max : 0;
-    // Shared-memory stages per warp: one sub-step of a slice takes about one memory latency and a
-    // slice has `batch` sub-steps, so small batches need a deeper prefetch.  Tuning overrides:
-    // GPUQT_STAGES, GPUQT_BLOCKS_PER_SM, GPUQT_ALTERNATE.
-    int stages = env_int("GPUQT_STAGES", batch == 1 ? 4 : batch == 2 ? 3 : 2);
-    stages = std::max(1, std::min(stages, kMaxStages));
-    h->want_stages = stages;
-    h->max_blocks_per_sm = env_int("GPUQT_BLOCKS_PER_SM", 0);
-    h->alternate = env_int("GPUQT_ALTERNATE", 1);
-    h->run = std::max(1, env_int("GPUQT_RUN", 16) / kWarps) * kWarps;
-    // two steps per launch (cheb_pair_kernel) are opt-in: they cut the DRAM bytes of a step pair by a
-    // third but are time-neutral at best on B200 so far
-    h->fuse = env_int("GPUQT_FUSE", 0);
-    h->small = env_int("GPUQT_SMALL", 1);
-    h->lag = std::max(1, env_int("GPUQT_LAG", 2));
-    h->nbr_ptr.swap(sell.nbr_ptr);
-    h->nbr_slices.swap(sell.nbr_slices);
-    // without locality in the table (a slice gathering from very many others) a second step cannot
-    // trail the first through L2: single-step launches only
-    if (h->nbr_slices.size() > (size_t)24 * (size_t)sell.n_slices) h->fuse = 0;
+    // Shared-memory stages per warp: one round of a tile takes about one memory latency and a slice has
+    // `batch / 2` rounds, so small batches need a deeper prefetch.
+    int stages = opt.stages ? opt.stages : (batch == 1 ? 4 : batch == 2 ? 3 : 2);
+    h->want_stages = std::max(1, std::min(stages, kMaxStages));
+    // whole recurrences in one cooperative launch when a step is so short that launch gaps matter
+    h->persistent = h->coop_ok && (opt.persistent == 1 || (opt.persistent == -1 && N * batch <= (int64_t)32768 * h->n_sm));
+    // tiles per CTA run: 16 keeps a CTA on a contiguous band (the sweep front stays tight in L2); short sweeps
+    // take the finest granularity for load balance
+    const long long tiles = n_tiles_of(h);
+    int run = opt.run ? opt.run : (tiles < (long long)64 * kWarps * h->n_sm ? kWarps : 2 * kWarps);
+    h->run = std::max(1, run / kWarps) * kWarps;
 
     const size_t vstride = align_up((size_t)(N + 1) * batch * sizeof(double2));
     char* v = base + L.vectors;
@@ -806,11 +769,12 @@ int gpuqt_create(gpuqt_handle** out, int64_t N, int32_t K_max, const int32_t* nb
     h->dots = (double*)(base + L.dots);
     h->moments = (double*)(base + L.moments);
     h->ticket = (unsigned int*)(base + L.ticket);
+    h->barrier = h->ticket + 32;
     rc = build_tensor_maps(h);
     if (rc != GPUQT_OK) {
-        fprintf(stderr, "gpuqt_create: %s\n", h->err.c_str());
+        const std::string why = h->err;
         gpuqt_destroy(h);
-        return rc;
+        return bad(rc, why);
     }
     *out = h;
     return GPUQT_OK;
@@ -864,7 +828,7 @@ int gpuqt_vac(gpuqt_handle* h, int32_t n_moments, double* out_host) {
 
 int gpuqt_evolve(gpuqt_handle* h, double dt, int32_t order) {
     if (h) h->sweep = 0;
-    if (!h || order < 1 || !std::isfinite(dt)) return fail(h, GPUQT_ERR_ARG, "bad dt or order");
+    if (!h || order < 1 || order > GPUQT_MAX_ORDER || !std::isfinite(dt)) return fail(h, GPUQT_ERR_ARG, "bad dt or order");
     if (!h->state_set) return fail(h, GPUQT_ERR_STATE, "gpuqt_set_state has not been called");
     std::vector<double> cr, ci;
     int rc;
@@ -891,11 +855,14 @@ int gpuqt_evolve(gpuqt_handle* h, double dt, int32_t order) {
     return GPUQT_OK;
 }
 
-int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_moments,
-                        int32_t n_sets, const double* energies_host, int32_t n_energies,
-                        double* out_host) {
+int gpuqt_kpm_transform_damped(gpuqt_handle* h, int damping, double lambda, const double* moments_host,
+                               int32_t n_moments, int32_t n_sets, const double* energies_host,
+                               int32_t n_energies, double* out_host) {
     if (!h || !moments_host || !energies_host || !out_host || n_moments < 1 || n_sets < 1 || n_energies < 1)
         return fail(h, GPUQT_ERR_ARG, "null or non-positive argument");
+    if (damping < GPUQT_DAMPING_JACKSON || damping > GPUQT_DAMPING_NONE ||
+        (damping == GPUQT_DAMPING_LORENTZ && !(lambda > 0.0 && std::isfinite(lambda))))
+        return fail(h, GPUQT_ERR_ARG, "unknown damping kernel or non-positive lambda");
     for (int j = 0; j < n_energies; ++j)
         if (!(std::fabs(energies_host[j] / h->dE) < 1.0))
             return fail(h, GPUQT_ERR_ENERGY, "energy point outside (-energy_scale, energy_scale)");
@@ -907,7 +874,7 @@ int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_m
     cudaError_t e = cudaMemcpyAsync(s + om, moments_host, bm, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(s + oe, energies_host, be, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) {
-        jackson_kernel<<<(n_moments + 255) / 256, 256, 0, h->stream>>>(n_moments, (double*)(s + og));
+        damping_kernel<<<(n_moments + 255) / 256, 256, 0, h->stream>>>(damping, lambda, n_moments, (double*)(s + og));
         const int total = n_sets * n_energies;
         transform_kernel<<<(total + 127) / 128, 128, 0, h->stream>>>(n_moments, n_sets, n_energies, (double*)(s + og),
                                                                      (double*)(s + om), (double*)(s + oe), 1.0 / h->dE,
@@ -919,6 +886,13 @@ int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_m
     if (e != cudaSuccess) return cuda_fail(h, e, "kpm_transform");
     flush_stats(h);
     return GPUQT_OK;
+}
+
+int gpuqt_kpm_transform(gpuqt_handle* h, const double* moments_host, int32_t n_moments,
+                        int32_t n_sets, const double* energies_host, int32_t n_energies,
+                        double* out_host) {
+    return gpuqt_kpm_transform_damped(h, GPUQT_DAMPING_JACKSON, 0.0, moments_host, n_moments, n_sets, energies_host,
+                                      n_energies, out_host);
 }
 
 int gpuqt_running_conductivity(gpuqt_handle* h, int kind, const double* corr_host, const double* dos_host,
@@ -987,6 +961,21 @@ int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, doubl
     return GPUQT_OK;
 }
 
+int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value) {
+    if (!h || !value) return GPUQT_ERR_ARG;
+    switch (what) {
+    case GPUQT_INFO_STORED_MATRIX_BYTES: *value = (int64_t)h->stored_matrix_bytes; break;
+    case GPUQT_INFO_HOP_VARIANT: *value = h->hop; break;
+    case GPUQT_INFO_UNIFORM: *value = h->mat.uniform; break;
+    case GPUQT_INFO_UNROLLED_WIDTH: *value = h->kt; break;
+    case GPUQT_INFO_SMALL_PATH: *value = small_ok(h) ? 1 : 0; break;
+    case GPUQT_INFO_PERSISTENT: *value = h->persistent; break;
+    case GPUQT_INFO_WORKSPACE_USED: *value = (int64_t)h->workspace_used; break;
+    default: return fail(h, GPUQT_ERR_ARG, "unknown info key");
+    }
+    return GPUQT_OK;
+}
+
 int gpuqt_kernel_stats(gpuqt_handle* h, int kernel_class, double* ms, int64_t* launches) {
     if (!h || kernel_class < 0 || kernel_class >= GPUQT_KERNEL_CLASSES) return GPUQT_ERR_ARG;
     flush_stats(h);
@@ -1013,21 +1002,19 @@ int gpuqt_reset_stats(gpuqt_handle* h) {
     return GPUQT_OK;
 }
 
-const char* gpuqt_last_error(const gpuqt_handle* h) { return h ? h->err.c_str() : "null handle"; }
+const char* gpuqt_last_error(const gpuqt_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
 void gpuqt_destroy(gpuqt_handle* h) {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
     flush_stats(h);
     for (auto e : h->free_events) cudaEventDestroy(e);
+    for (auto e : h->coef_event)
+        if (e) cudaEventDestroy(e);
+    if (h->coef_host) cudaFreeHost(h->coef_host);
+    if (h->coef_dev) cudaFree(h->coef_dev);
     if (h->scratch) cudaFree(h->scratch);
     if (h->d_maps) cudaFree(h->d_maps);
-    for (auto& d : h->schedules) {
-        cudaFree(d.items);
-        cudaFree(d.dep_ptr);
-        cudaFree(d.dep_list);
-        cudaFree(d.run_done);
-    }
     delete h;
 }
 

@@ -97,26 +97,29 @@ inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32
 // "all hoppings -1", and every clean-lattice model) -- then padding is col = N, the
 // all-zero row every device vector carries.  If padding every record to K_max costs less
 // than 1/16 extra bytes the table is stored uniform (w = K_max everywhere), which lets the
-// kernels compute record offsets arithmetically and unroll the neighbour walk.
+// kernels compute record offsets arithmetically and unroll the neighbour walk.  The record array is
+// padded with all-padding records to a multiple of `pad_to` slices, so that a tile of several
+// consecutive slices is always one contiguous copy.
 struct SellHost {
-    int64_t n_slices = 0;
+    int64_t n_slices = 0;               // real slices, ceil(N / 32)
     int uniform = 1;                    // every record has width K_max
     int nd = 1;                         // doubles per entry: 0 constant hopping, 1 real, 2 complex
     double hop_const = 0.0;
     int idx16 = 0;                      // constant hopping with 16-bit columns (see try_idx16)
-    std::vector<int> nbr_ptr, nbr_slices;   // CSR over slices: the slices a slice gathers from (sorted, itself included)
-    std::vector<long long> slice_off;   // [n_slices + 1] byte offsets of the records
+    int64_t n_slices_padded = 0;        // records stored: n_slices rounded up to a multiple of pad_to (all-padding records behind)
+    std::vector<long long> slice_off;   // [n_slices_padded + 1] byte offsets of the records
     std::vector<unsigned char> rec;
 };
 
 inline long long host_record_bytes(int w, int nd) { return 32LL * (8LL * w * nd + 8 + 4LL * w); }
 
 // Re-encode a uniform constant-hopping table (records: onsite[32] | int32 col[K][32]) with 16-bit
-// columns: record = double onsite[32] | int32 base[8] | uint16 delta[K][32], col = base[k] + delta.
-// Possible when K <= 8 and, inside every (slice, k), the columns spread less than 65536 (padding
-// entries, col = N, included).  Returns false and leaves the table untouched otherwise.
+// columns: record = double onsite[32] | int32 base[8] | uint16 delta[K][32], col = base[k] + delta, and
+// delta = 0xffff stands for a padding entry (col = N, the zero row).  Possible when K <= 8 and, inside
+// every (slice, k), the real columns spread less than 65535.  Returns false and leaves the table
+// untouched otherwise.
 struct SellHost;
-inline bool try_idx16(SellHost& s, int K);
+inline bool try_idx16(SellHost& s, int K, int64_t N);
 
 // true (and the value) if hop_im is absent and all listed hoppings carry the same bit pattern
 inline bool constant_hopping(int64_t N, int32_t K, const int32_t* cnt, const double* hre, const double* him,
@@ -143,12 +146,13 @@ inline bool constant_hopping(int64_t N, int32_t K, const int32_t* cnt, const dou
 
 inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
                        const double* hre, const double* him, const double* onsite, bool allow_const,
-                       SellHost& s) {
+                       int pad_to, SellHost& s) {
     s.nd = him ? 2 : 1;
     if (allow_const && constant_hopping(N, K, cnt, hre, him, s.hop_const)) s.nd = 0;
     const int cplx = s.nd;   // doubles per entry
     s.n_slices = (N + 31) / 32;
-    std::vector<int> width((size_t)s.n_slices, 0);
+    s.n_slices_padded = (s.n_slices + pad_to - 1) / pad_to * pad_to;
+    std::vector<int> width((size_t)s.n_slices_padded, 0);
     long long ragged = 0;
     for (int64_t sl = 0; sl < s.n_slices; ++sl) {
         int w = 0;
@@ -158,26 +162,13 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
     }
     const long long padded = (long long)s.n_slices * host_record_bytes(K, cplx);
     s.uniform = (padded <= ragged + ragged / 16) ? 1 : 0;
-    s.slice_off.assign((size_t)s.n_slices + 1, 0);
-    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+    s.slice_off.assign((size_t)s.n_slices_padded + 1, 0);
+    for (int64_t sl = 0; sl < s.n_slices_padded; ++sl) {
         if (s.uniform) width[(size_t)sl] = K;
         s.slice_off[(size_t)sl + 1] = s.slice_off[(size_t)sl] + host_record_bytes(width[(size_t)sl], cplx);
     }
-    s.rec.assign((size_t)s.slice_off[(size_t)s.n_slices], 0);
-    s.nbr_ptr.assign((size_t)s.n_slices + 1, 0);
-    s.nbr_slices.clear();
-    std::vector<int> tmp;
-    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
-        tmp.clear();
-        tmp.push_back((int)sl);
-        for (int64_t m = sl * 32; m < std::min<int64_t>(N, sl * 32 + 32); ++m)
-            for (int32_t k = 0; k < cnt[m]; ++k) tmp.push_back(idx[(size_t)m * K + k] >> 5);
-        std::sort(tmp.begin(), tmp.end());
-        tmp.erase(std::unique(tmp.begin(), tmp.end()), tmp.end());
-        s.nbr_slices.insert(s.nbr_slices.end(), tmp.begin(), tmp.end());
-        s.nbr_ptr[(size_t)sl + 1] = (int)s.nbr_slices.size();
-    }
-    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+    s.rec.assign((size_t)s.slice_off[(size_t)s.n_slices_padded], 0);
+    for (int64_t sl = 0; sl < s.n_slices_padded; ++sl) {
         const int w = width[(size_t)sl];
         unsigned char* base = s.rec.data() + s.slice_off[(size_t)sl];
         double* r_hre = reinterpret_cast<double*>(base);
@@ -200,77 +191,6 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
                 }
             }
         }
-    }
-}
-
-// Work list of a launch that performs two consecutive recurrence steps (kernels.cuh,
-// cheb_step_kernel).  Items are (step, run); CTA c of G takes items c, c + G, ...  First-step items
-// come in sweep order.  The second step of run R gathers T_m from a few runs dep(R) (from the
-// table's sparsity); it is emitted once the first-step item of the farthest of them lies at least
-// `slack` items back, so that when a CTA reaches it those runs are normally finished and their
-// T_m, T_{m-1} and matrix records are still in L2.  Steps alternate along the list with the
-// parity flipped every 4 G items, so every CTA (and SM) gets both kinds of work, four items of a
-// kind in a row.  Runs whose
-// dependency wraps around the end of the table (periodic boundaries) follow after the first
-// sweep; no-op items pad while nothing is eligible.
-//   items[2t] = run | step << 30 (run = no_run: no-op), items[2t+1] = -1 (reserved)
-//   dep_ptr / dep_list: CSR over runs of the first-step runs a second-step item waits for
-struct FusedSchedule {
-    std::vector<int> items;
-    std::vector<int> dep_ptr, dep_list;
-};
-inline void build_fused_schedule(int n_slices, int run, int G, int reverse, int slack, int no_run,
-                                 const std::vector<int>& nbr_ptr, const std::vector<int>& nbr_slices,
-                                 FusedSchedule& out) {
-    const int n_runs = (n_slices + run - 1) / run;
-    std::vector<int> far((size_t)n_runs, 0), tmp;
-    out.dep_ptr.assign((size_t)n_runs + 1, 0);
-    out.dep_list.clear();
-    for (int R = 0; R < n_runs; ++R) {
-        tmp.clear();
-        for (int vs = R * run; vs < std::min(n_slices, (R + 1) * run); ++vs) {
-            const int s = reverse ? n_slices - 1 - vs : vs;
-            for (int i = nbr_ptr[(size_t)s]; i < nbr_ptr[(size_t)s + 1]; ++i) {
-                const int ns = nbr_slices[(size_t)i];
-                tmp.push_back((reverse ? n_slices - 1 - ns : ns) / run);
-            }
-        }
-        std::sort(tmp.begin(), tmp.end());
-        tmp.erase(std::unique(tmp.begin(), tmp.end()), tmp.end());
-        far[(size_t)R] = tmp.back();
-        out.dep_list.insert(out.dep_list.end(), tmp.begin(), tmp.end());
-        out.dep_ptr[(size_t)R + 1] = (int)out.dep_list.size();
-    }
-    std::vector<int> order((size_t)n_runs);
-    for (int R = 0; R < n_runs; ++R) order[(size_t)R] = R;
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return far[(size_t)a] < far[(size_t)b]; });
-    std::vector<int> pos1((size_t)n_runs, -1);
-    out.items.clear();
-    auto n_items = [&]() { return (int)(out.items.size() / 2); };
-    auto emit = [&](int x) {
-        out.items.push_back(x);
-        out.items.push_back(-1);
-    };
-    int i2 = 0, R1 = 0;
-    auto try_second = [&]() {
-        if (i2 >= n_runs) return false;
-        const int R2 = order[(size_t)i2];
-        const int d = pos1[(size_t)far[(size_t)R2]];
-        if (d < 0 || d + slack > n_items()) return false;
-        emit(R2 | (1 << 30));
-        ++i2;
-        return true;
-    };
-    while (R1 < n_runs || i2 < n_runs) {
-        const int t = n_items();
-        const bool want_second = (((t % G) + (t / (4 * G))) & 1) != 0;   // a CTA switches step every 4 items
-        if (want_second && try_second()) continue;
-        if (R1 < n_runs) {
-            pos1[(size_t)R1] = t;
-            emit(R1++);
-            continue;
-        }
-        if (!try_second()) emit(no_run);
     }
 }
 
@@ -322,11 +242,11 @@ inline void bessel_coeffs(double dE, double dt, int order, std::vector<double>& 
 }  // namespace gpuqt
 
 namespace gpuqt {
-inline bool try_idx16(SellHost& s, int K) {
+inline bool try_idx16(SellHost& s, int K, int64_t N) {
     if (s.nd != 0 || !s.uniform || K > 8) return false;
     const size_t old_bytes = 256 + 128 * (size_t)K, new_bytes = 288 + 64 * (size_t)K;
-    std::vector<unsigned char> out((size_t)s.n_slices * new_bytes, 0);
-    for (int64_t sl = 0; sl < s.n_slices; ++sl) {
+    std::vector<unsigned char> out((size_t)s.n_slices_padded * new_bytes, 0);
+    for (int64_t sl = 0; sl < s.n_slices_padded; ++sl) {
         const unsigned char* src = s.rec.data() + (size_t)sl * old_bytes;
         unsigned char* dst = out.data() + (size_t)sl * new_bytes;
         std::memcpy(dst, src, 256);                                            // onsite
@@ -334,18 +254,24 @@ inline bool try_idx16(SellHost& s, int K) {
         int32_t* base = reinterpret_cast<int32_t*>(dst + 256);
         uint16_t* delta = reinterpret_cast<uint16_t*>(dst + 288);
         for (int k = 0; k < K; ++k) {
-            int32_t lo = col[k * 32], hi = col[k * 32];
-            for (int lane = 1; lane < 32; ++lane) {
-                lo = std::min(lo, col[k * 32 + lane]);
-                hi = std::max(hi, col[k * 32 + lane]);
+            int64_t lo = N, hi = -1;                                           // over the real columns (padding is col = N)
+            for (int lane = 0; lane < 32; ++lane) {
+                const int32_t c = col[k * 32 + lane];
+                if (c >= N) continue;
+                lo = std::min<int64_t>(lo, c);
+                hi = std::max<int64_t>(hi, c);
             }
-            if ((int64_t)hi - lo > 65535) return false;
-            base[k] = lo;
-            for (int lane = 0; lane < 32; ++lane) delta[k * 32 + lane] = (uint16_t)(col[k * 32 + lane] - lo);
+            if (hi < 0) lo = 0;                                                // nothing but padding
+            if (hi - lo > 65534) return false;                                 // 0xffff is reserved for the zero row
+            base[k] = (int32_t)lo;
+            for (int lane = 0; lane < 32; ++lane) {
+                const int32_t c = col[k * 32 + lane];
+                delta[k * 32 + lane] = c >= N ? (uint16_t)0xffffu : (uint16_t)(c - lo);
+            }
         }
     }
     s.rec.swap(out);
-    for (int64_t sl = 0; sl <= s.n_slices; ++sl) s.slice_off[(size_t)sl] = (long long)((size_t)sl * new_bytes);
+    for (int64_t sl = 0; sl <= s.n_slices_padded; ++sl) s.slice_off[(size_t)sl] = (long long)((size_t)sl * new_bytes);
     s.idx16 = 1;
     return true;
 }

@@ -2,29 +2,35 @@
 // the layout, the byte model and the roofline of each kernel.
 //
 // Layout
-//   vectors   complex fp64 [N][B] as double2: the B vectors of a row are contiguous (16*B bytes),
-//             so one neighbour index serves one 16*B-byte gather (B = 8: one 128-byte line).
+//   vectors   complex fp64 [N + 1][B] as double2: the B vectors of a row are contiguous (16*B bytes),
+//             so one neighbour index serves one 16*B-byte gather (B = 8: one 128-byte line).  Row N
+//             of every buffer is all zero and never written.
 //   matrix    packed sliced ELL.  A slice is 32 consecutive rows; slice s of width w is ONE
 //             contiguous record, column-major inside the record:
 //                 double hre[w][32] (per-entry variants) | double him[w][32] (complex variant) |
 //                 double onsite[32] | int32 col[w][32]
 //             record bytes = 32 * (8 w nd + 8 + 4 w), nd = doubles per entry (0, 1, 2), a multiple
 //             of 128.  Records are stored back to back; slice_off[s] is the byte offset of record
-//             s.  Padding entries are (own row, hop 0.0); in the constant-hopping variant (nd = 0:
+//             s.  Padding entries are (own row, hop 0.0); in the constant-hopping variants (nd = 0:
 //             every stored hopping is the same real number, kept in Mat::hop_const) padding is
-//             col = N: every vector buffer carries an all-zero row N (and x[N] = 0), so the walk
-//             needs no guard.  One record = one 1-D TMA bulk copy.
-//   warp      the unit of work is (consumer warp, slice).  A stage of a warp's shared-memory pipeline
-//             holds everything the slice streams from HBM exactly once: the packed record, the
-//             slice's own rows of T_{m-1} (and e_{m-1}) and of T_{m-2} (and e_{m-2}) -- each one
-//             1-D TMA bulk copy (cp.async.bulk + mbarrier) issued by the CTA's producer warp one or
-//             more slices ahead, so the DRAM streams never sit on a consumer's scoreboard and there
-//             is no CTA-wide barrier in the loop.  A consumer walks the slice in rounds of 32/LPR
-//             rows; a lane owns V = 2 consecutive vectors of a row (256-bit accesses) and LPR = B/V
-//             lanes share a row.  Neighbours inside the slice are read from the staged rows in
-//             shared memory; the others are gathered from global memory (L2 hits along the sweep
-//             front), all gathers of a round issued back to back.  Stores of a warp are one
-//             contiguous segment.
+//             col = N, the zero row (and x[N] = 0), so the walk needs no guard.  The table is padded
+//             with all-padding records up to a multiple of kTilePad slices, so a tile of several
+//             slices is always one contiguous copy.
+//   warp      the unit of work is (warp, tile); a tile is S consecutive slices (S = 2 at B = 1 on
+//             the unrolled uniform tables, else 1).  A stage of a warp's shared-memory pipeline holds
+//             everything the tile streams exactly once: the packed records and the tile's own rows
+//             of x_{m-1} (and e_{m-1}) and of x_{m-2} (and e_{m-2}) -- TMA copies (cp.async.bulk +
+//             mbarrier) issued by the warp's lane 0 one or more tiles ahead, so the streams never sit
+//             on the warp's scoreboard and there is no CTA-wide barrier in the loop.  A warp walks the
+//             tile in rounds of 32/LPR rows; a lane owns V = 2 consecutive vectors of a row (256-bit
+//             accesses) and LPR = B/V lanes share a row; at B = 1 the two rounds of a tile are walked
+//             together (all gathers of both first, then the arithmetic) for memory-level parallelism.
+//             Neighbours inside the tile are read from the staged rows in shared memory; the others
+//             are gathered from global memory (L2 hits along the sweep front).
+//   launch    a launch performs the recurrence steps m_begin .. m_end-1.  Single-step launches are
+//             plain launches; multi-step launches are cooperative (all CTAs co-resident) and separate
+//             the steps by a grid-wide barrier, so a whole moment set or a whole time step is ONE
+//             launch when the working set lives in L2 and the launch gaps would dominate.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -44,10 +50,7 @@
 #ifndef GPUQT_GATHER_POLICY   // 0: plain ld.global, 1: L2::evict_last
 #define GPUQT_GATHER_POLICY 1
 #endif
-#ifndef GPUQT_IN_POLICY       // own rows of T_{m-1} by TMA: 0 no hint, 1 evict_last
-#define GPUQT_IN_POLICY 0
-#endif
-#ifndef GPUQT_ST_POLICY       // stores of T_m / acc: 0 plain, 1 st.global.cs (evict-first)
+#ifndef GPUQT_ST_POLICY       // stores of x_m: 0 plain, 1 st.global.cs (evict-first)
 #define GPUQT_ST_POLICY 0
 #endif
 
@@ -57,6 +60,7 @@ constexpr int kThreads = GPUQT_THREADS;
 constexpr int kWarps = kThreads / 32;
 constexpr int kSlice = 32;
 constexpr int kMaxStages = 4;
+constexpr int kTilePad = 4;          // the record array is padded to a multiple of this many slices
 
 // nd = doubles stored per entry: 0 constant real hopping, 1 real, 2 complex
 __host__ __device__ __forceinline__ long long record_bytes(int w, int nd) {
@@ -66,80 +70,77 @@ __host__ __device__ __forceinline__ int record_width(long long bytes, int nd) {
     return (int)((bytes / 32 - 8) / (4 + 8 * nd));
 }
 // kHopConst16: constant hopping AND 16-bit columns -- the record is
-//     double onsite[32] | int32 base[8] (first w used) | uint16 delta[w][32],   col = base[k] + delta[k][lane]
-// (uniform tables without padding whose columns spread less than 65536 inside every (slice, k); lattices
-// in natural order do).  288 + 64 w bytes instead of 256 + 128 w.
+//     double onsite[32] | int32 base[8] (first w used) | uint16 delta[w][32]
+//     col = base[k] + delta[k][lane], or the zero row N when delta == 0xffff (padding entries)
+// (uniform tables whose real columns spread less than 65535 inside every (slice, k); lattices in
+// natural order do).  288 + 64 w bytes instead of 256 + 128 w.
 enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2, kHopConst16 = 3 };
 __host__ __device__ constexpr bool hop_is_const(int hop) { return hop == kHopConst || hop == kHopConst16; }
 __host__ __device__ constexpr int hop_doubles(int hop) { return hop_is_const(hop) ? 0 : hop == kHopComplex ? 2 : 1; }
 __host__ __device__ __forceinline__ long long hop_record_bytes(int w, int hop) {
     return hop == kHopConst16 ? 288LL + 64LL * w : record_bytes(w, hop_doubles(hop));
 }
+constexpr unsigned kPad16 = 0xffffu;     // 16-bit delta that stands for the zero row N
 
 struct Mat {
     const unsigned char* __restrict__ rec;      // packed slice records
-    const long long* __restrict__ slice_off;    // [n_slices + 1] byte offsets (ragged variant)
+    const long long* __restrict__ slice_off;    // [n_slices_padded + 1] byte offsets (ragged variant)
     const double* __restrict__ x;               // [N + 1], x[N] = 0
     long long N;
-    long long n_slices;
+    long long n_slices;                         // real slices, ceil(N / 32)
     int K;                                      // K_max
     int uniform;                                // every record has width K
     int cplx;
     int hop;                                    // Hop variant of the records
-    double hop_const;                           // kHopConst: the one hopping value
+    double hop_const;                           // constant-hopping variants: the one hopping value
     double inv_dE;
     double box;                                 // <= 0: open boundary
 };
 
 enum Mode : int {
-    kModeDoubling = 0,   // T_new, dots |T_new|^2, Re<T_new|T_in>, |T_in|^2          (Eq. 28, 30)
-    kModeLeft = 1,       // T_new, dot <phi_L|T_new>                                 (Eq. 29)
+    kModeDoubling = 0,   // x_m, dots |x_m|^2, Re<x_m|x_{m-1}>, |x_{m-1}|^2            (Eq. 28, 30)
+    kModeLeft = 1,       // x_m, dot <phi_L|x_m>                                      (Eq. 29)
     kModeEvolve = 2,     // Clenshaw term b_k = c_k src + 2 H~ b_{k+1} - b_{k+2}      (Eq. 17, 21)
     kModeEvolveMsd = 3,  // the same for the (a, e) pair, [X,H~] weights in the walk (Eq. 18, 22)
 };
 
-// Operands of one recurrence step.  A launch performs one step, or two consecutive steps fused
-// through L2 (see cheb_step_kernel): io[0] is T_m = 2 H~ T_{m-1} - T_{m-2}, io[1] is T_{m+1}.
-struct StepIO {
-    const double2* in;       // T_{m-1}: gathered and own row
-    const double2* prev;     // T_{m-2}: own row (unused when first)
-    double2* out;            // T_m (unused when !store)
-    const double2* in_e;     // MSD pair: e_{m-1}
-    const double2* prev_e;   //           e_{m-2}
-    double2* out_e;          //           e_m
-    // B >= 2: device addresses of the TMA tensor maps (CUtensorMap, 128-byte swizzle) of in / prev / in_e / prev_e
-    const void *tm_in, *tm_prev, *tm_in_e, *tm_prev_e;
-    double cr, ci;           // c_m
-    double* result;          // [Q][B] reduced dots of this step
-    int store;               // write T_m (0 on the last term of an evolve)
-    int pad_;
+// One three-term recurrence x_m = 2 H~ x_{m-1} - x_{m-2} (+ c_k src), m = 1 .. terms-1, and the steps
+// [m_begin, m_end) of it that this launch performs.  x_0 is given; x_m (m >= 1) lives in
+// ring[(m - 1) % 3] (the last term optionally somewhere else).  Forward recurrences (moments) apply
+// factor 1 instead of 2 in step 1 (T_1 = H~ T_0); Clenshaw recurrences (evolution) in the last step.
+struct RecArgs {
+    const double2* x0;           // x_0
+    double2* ring[3];
+    const double2* e0;           // MSD pair: e_0 and its ring
+    double2* ring_e[3];
+    // B >= 2: device addresses of the TMA tensor maps (CUtensorMap, 128-byte swizzle) of the buffers above
+    const void* tm_x0;
+    const void* tm_ring[3];
+    const void* tm_e0;
+    const void* tm_ring_e[3];
+    double2* last_out;           // evolve: destination of x_{terms-1} (instead of its ring slot)
+    double2* last_out_e;
+    const double2* src;          // evolve: the vector being evolved (psi; a; b), read-only
+    const double2* src_e;        // evolve MSD: chi
+    const double2* phiL;         // kModeLeft
+    const double* coef;          // evolve: c_k as (re, im) pairs, k < terms; step m adds c_{terms-1-m} src
+    double* dots;                // step m writes its Q*B reduced dots at dots[(m - dot_m0) * Q*B ...]
+    int terms;
+    int m_begin, m_end;
+    int clenshaw;
+    int store_last;              // is x_{terms-1} written at all (moments: no)
+    int dot_m0;
+    int sweep0;                  // direction of step m_begin: 1 = from the top
+    int alternate;               // the direction alternates from step to step (L2 reuse across the boundary)
+    int run;                     // consecutive tiles one CTA walks before jumping (multiple of kWarps)
+    int stages;                  // shared-memory stages per warp (<= kMaxStages)
+    int stage_bytes;             // bytes of one stage: records + staged vector rows
+    int rec_bytes;               // bytes reserved for the records inside a stage
+    int multi;                   // cooperative multi-step launch: grid barrier between steps
+    double* partials;            // [2][grid][Q*B]
+    unsigned int* ticket;        // single-step launches: last-block detection
+    unsigned int* barrier;       // multi-step launches: monotonically increasing arrival counter (zeroed by the host)
 };
-
-struct StepArgs {
-    StepIO io[2];
-    const double2* __restrict__ src;     // evolve: the vector being evolved (psi; a; b), read-only
-    const double2* __restrict__ src_e;   // evolve MSD: chi
-    const double2* __restrict__ phiL;    // kModeLeft
-    int first;                           // no T_{m-2} term (first launch of a recurrence); single-step launches only
-    int half;                            // factor 1 instead of 2 on H~ (T_1 = H~ T_0; last Clenshaw term); single-step only
-    int n_steps;                         // 1, or 2 (fused pair, scheduled by `sched`)
-    int reverse;                         // sweep the slices from the top (L2 reuse between launches)
-    int run;                             // consecutive slices one CTA walks before jumping (multiple of kWarps)
-    int stages;                          // shared-memory stages per warp (<= kMaxStages)
-    int stage_bytes;                     // bytes of one stage: record + staged vector rows
-    int rec_bytes;                       // bytes reserved for the record inside a stage
-    double* partials;                    // [grid][n_steps*Q*B]
-    unsigned int* ticket;
-    // fused pair: item t (taken by CTA t % G) = {run | step << 30 (run = kNoRun: nothing to do), -1};
-    // a second-step item of run R waits until run_done[r] == kWarps for r in dep_list[dep_ptr[R] ..
-    // dep_ptr[R+1]) (the first-step runs it gathers T_m from)
-    const int2* sched;
-    int n_items;
-    unsigned int* run_done;              // [runs] warps that have finished the first step of the run
-    const int* dep_ptr;
-    const int* dep_list;
-};
-constexpr int kNoRun = (1 << 30) - 1;
 
 // ------------------------------------------------------------------ PTX helpers (TMA / mbarrier)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -168,25 +169,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "r"(parity)
         : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, P1;\n"
-        "}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
@@ -201,7 +183,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
         "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
         : "memory");
 }
-
 __device__ __forceinline__ void bulk_g2s_nohint(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile(
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
@@ -209,7 +190,6 @@ __device__ __forceinline__ void bulk_g2s_nohint(void* dst, const void* src, uint
         "l"(src), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
-
 // 2-D tiled TMA copy global -> shared through a tensor map (box = one slice's rows of one vector set as
 // 128-byte lines, 128-byte swizzle); completion is signalled on `bar`.  c1 = index of the first line.
 __device__ __forceinline__ void tensor_g2s(void* dst, const void* tmap, int c1, uint64_t* bar) {
@@ -226,17 +206,17 @@ __device__ __forceinline__ void tensor_g2s_hint(void* dst, const void* tmap, int
         "l"(tmap), "r"(0), "r"(c1), "r"(smem_u32(bar)), "l"(policy)
         : "memory");
 }
+// Orders generic-proxy accesses (ordinary stores / loads) against async-proxy accesses (TMA) of the
+// executing thread.  Used on both sides of the grid barrier of a multi-step launch: x_m is written by
+// ordinary stores of one SM and read by TMA copies of another in the next step.
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
 // Staged vector rows are written by the TMA with the 128-byte swizzle (16-byte chunk index, address
 // bits 4-6, ^= address bits 7-9; box rows are whole 128-byte lines): a lane's two 16-byte reads at a
 // 32-byte lane stride then fall on distinct banks for every group of 8 lanes (without it: a 2-way
 // bank conflict on every 128-bit read).  Uses the absolute shared address, as the TMA does.
 __device__ __forceinline__ uint32_t swz32(uint32_t sa) { return sa ^ ((sa >> 3) & 0x70u); }
 
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
 __device__ __forceinline__ void st_vec(double2* p, double2 v) {
 #if GPUQT_ST_POLICY == 1
     __stcs(p, v);
@@ -244,10 +224,32 @@ __device__ __forceinline__ void st_vec(double2* p, double2 v) {
     *p = v;
 #endif
 }
+__device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void red_release_gpu_inc(unsigned int* p) {
     asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
 }
-__device__ __forceinline__ double2 ldcs2(const double2* p) { return __ldcs(p); }
+
+// Grid-wide barrier of a cooperative launch (all CTAs co-resident).  `counter` only ever grows; the
+// e-th barrier of the launch completes when it reaches e * gridDim.x.  Release/acquire at gpu scope:
+// everything the CTA wrote before the barrier is visible to every CTA after it; the proxy fences
+// extend that to the TMA (async proxy) reads that follow.
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int target) {
+    fence_proxy_async();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        red_release_gpu_inc(counter);
+        while (ld_acquire_gpu(counter) < target) {
+        }
+        __threadfence();
+    }
+    __syncthreads();
+    fence_proxy_async();
+}
 
 // minimum-image X_n - X_m  [A6]; pure add/sub so it is bit-identical to the oracle's
 __device__ __forceinline__ double min_image(double d, double box) {
@@ -320,28 +322,26 @@ struct ModeTraits {
     static constexpr int kMinBlocks = (MODE == kModeEvolveMsd) ? GPUQT_MINB_MSD : GPUQT_MINB;   // register cap
 };
 
-// B = 8: a slice's rows are 4 KB per stream; staging T_{m-2} as well would leave room for one CTA per
-// SM only, so T_{m-2} own rows are read by a streaming 256-bit load at the top of the round instead
+// B = 8: a slice's rows are 4 KB per stream; staging x_{m-2} as well would leave room for one CTA per
+// SM only, so x_{m-2} own rows are read by a streaming 256-bit load at the top of the round instead
 // (the occupancy is worth more than the TMA staging there; at B <= 4 it is the other way round).
 template <int B>
 struct PrevDirect {
     static constexpr bool value = (B >= 8);
 };
 
-// Number of vector streams staged per slice: own rows of T_{m-1}, T_{m-2} (x2 for the (a, e) pair).
-template <int MODE>
-struct StagedStreams {
-    static constexpr int value = (MODE == kModeEvolveMsd) ? 4 : 2;
-};
-
 // A lane owns V consecutive vectors of a row (V = 2 when B >= 2: one 256-bit access per operand).
-template <int B>
+// A tile is S consecutive slices and is walked in ROUNDS rounds of RS rows, U rounds at a time.
+template <int B, int KT>
 struct LaneShape {
     static constexpr int V = B >= 2 ? 2 : 1;
-    static constexpr int LPR = B / V;        // lanes per row
-    static constexpr int RS = 32 / LPR;      // rows per round
-    static constexpr int ROUNDS = LPR;       // rounds per slice
+    static constexpr int LPR = B / V;                      // lanes per row
+    static constexpr int RS = 32 / LPR;                    // rows per round
+    static constexpr int S = (B == 1 && KT > 0) ? 2 : 1;   // slices per tile
+    static constexpr int ROUNDS = S * LPR;                 // rounds per tile
+    static constexpr int U = (B == 1 && KT > 0) ? 2 : 1;   // rounds walked together
 };
+__host__ __device__ constexpr int tile_slices(int B, int kt) { return (B == 1 && kt > 0) ? 2 : 1; }
 
 template <int V>
 struct CV {   // V complex numbers
@@ -416,18 +416,19 @@ __device__ __forceinline__ void cv_st<2>(double2* p, const CV<2>& v) {
                  : "memory");
 #endif
 }
-// Gather of V consecutive vectors of row c of T_{m-1}: rows of the current slice come from the
-// staged copy in shared memory, the others from global memory with an L2 evict_last hint (they are
-// re-read by the neighbouring slices).  Both loads are predicated, so there is no branch.
+// Gather of V consecutive vectors of row c of x_{m-1}: rows of the current tile come from the staged
+// copy in shared memory, the others from global memory with an L2 evict_last hint (they are re-read
+// by the neighbouring tiles).  Both loads are predicated, so there is no branch.
 //   g_l  = byte address of (row 0, the lane's first vector) in global memory
-//   s_l  = shared-window address of the same element of the slice's staged rows, minus row0 * RB
-//   RB   = bytes of one row (16 B)
-template <int V>
+//   s_l  = shared-window address of the same element of the tile's staged rows, minus row0 * RB
+//          (mod 2^32: only rows of the tile are ever addressed through it)
+//   RB   = bytes of one row (16 B);  TR = rows of a tile
+template <int V, int TR>
 __device__ __forceinline__ CV<V> cv_gather(const char* g_l, uint32_t s_l, int c, int row0, int RB);
 template <>
-__device__ __forceinline__ CV<1> cv_gather<1>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+__device__ __forceinline__ CV<1> cv_gather<1, 32>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
-    const uint32_t sa = s_l + (uint32_t)(c * RB);
+    const uint32_t sa = s_l + (uint32_t)c * (uint32_t)RB;
     const char* ga = g_l + (long long)c * RB;
     CV<1> v;
     asm volatile(
@@ -442,9 +443,26 @@ __device__ __forceinline__ CV<1> cv_gather<1>(const char* g_l, uint32_t s_l, int
     return v;
 }
 template <>
-__device__ __forceinline__ CV<2> cv_gather<2>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+__device__ __forceinline__ CV<1> cv_gather<1, 64>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
-    const uint32_t sa = swz32(s_l + (uint32_t)(c * RB));
+    const uint32_t sa = s_l + (uint32_t)c * (uint32_t)RB;
+    const char* ga = g_l + (long long)c * RB;
+    CV<1> v;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.lt.u32 p, %4, 64;\n"
+        "@p ld.shared.v2.f64 {%0, %1}, [%2];\n"
+        "@!p ld.global.v2.f64 {%0, %1}, [%3];\n"
+        "}"
+        : "=d"(v.re[0]), "=d"(v.im[0])
+        : "r"(sa), "l"(ga), "r"(d));
+    return v;
+}
+template <>
+__device__ __forceinline__ CV<2> cv_gather<2, 32>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+    const unsigned d = (unsigned)(c - row0);
+    const uint32_t sa = swz32(s_l + (uint32_t)c * (uint32_t)RB);
     const uint32_t sb = sa ^ 16u;
     const char* ga = g_l + (long long)c * RB;
     CV<2> v;
@@ -488,143 +506,198 @@ __device__ __forceinline__ void cv_add(CV<V>& acc, const CV<V>& v) {
     }
 }
 
-// One round (RS rows) of one slice whose record and own rows sit in shared memory at `stage`.
-// Rows past the end of the table (last slice only) are computed like the others on zero inputs
-// (their staged self / prev are replaced by 0 and their entries are padding), so the dot products
-// need no guard; only their stores are predicated off.
+// Operands of one recurrence step (derived from RecArgs at the top of the step, CTA-uniform)
+struct StepCtx {
+    const double2* in;       // x_{m-1}: gathered and own row
+    const double2* prev;     // x_{m-2}: own row (unused when first)
+    double2* out;            // x_m (unused when !store)
+    const double2* in_e;     // MSD pair: e_{m-1}
+    const double2* prev_e;   //           e_{m-2}
+    double2* out_e;          //           e_m
+    const void *tm_in, *tm_prev, *tm_in_e, *tm_prev_e;
+    double cr, ci;           // c_k of this term (evolve)
+    double scale;            // 2 / dE, or 1 / dE in the half step
+    int first;               // no x_{m-2} term
+    int store;               // write x_m
+};
+
+// Column of entry k of row rr of the slice whose record starts at s_col (int32 columns, or the base[8]
+// table of the 16-bit variant with the deltas behind it)
+template <bool IDX16>
+__device__ __forceinline__ int col_of(const int* s_col, const unsigned short* s_d16, int k, int rr, int N) {
+    if (IDX16) {
+        const unsigned d = s_d16[k * 32 + rr];
+        return d == kPad16 ? N : s_col[k] + (int)d;
+    }
+    return s_col[k * 32 + rr];
+}
+
+// U consecutive rounds (RS rows each) of one tile whose records and own rows sit in shared memory at
+// `stage`.  Rows past the end of the table (last tile only) are computed like the others on zero
+// inputs (their staged self / prev are replaced by 0 and their entries are padding), so the dot
+// products need no guard; only their stores are predicated off.
 template <int B, int KT, int HOP, int MODE>
-__device__ __forceinline__ void walk_round(const Mat& m, const StepArgs& a, const StepIO& io, const unsigned char* stage, int w,
-                                           int row0, int rows_valid, int j, int lane, double scale,
-                                           double (&red)[ModeTraits<MODE>::Q * LaneShape<B>::V],
-                                           unsigned int* signal) {
-    constexpr int V = LaneShape<B>::V, LPR = LaneShape<B>::LPR, RS = LaneShape<B>::RS;
+__device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, const StepCtx& io, const unsigned char* stage, int w,
+                                            int row0, int rows_valid, int j0, int lane,
+                                            double (&red)[ModeTraits<MODE>::Q * LaneShape<B, KT>::V]) {
+    using LS = LaneShape<B, KT>;
+    constexpr int V = LS::V, LPR = LS::LPR, RS = LS::RS, U = LS::U, TR = 32 * LS::S;
     constexpr int KU = KT > 0 ? KT : 1;
     constexpr int RB = B * 16;   // bytes of one row of a vector set
     constexpr bool MSD = (MODE == kModeEvolveMsd);
     constexpr bool CPLX = (HOP == kHopComplex), CONST = hop_is_const(HOP), IDX16 = (HOP == kHopConst16);
+    constexpr int REC = KT > 0 ? (int)(HOP == kHopConst16 ? 288 + 64 * KT : 32 * (8 * KT * (CONST ? 0 : CPLX ? 2 : 1) + 8 + 4 * KT)) : 0;
     const int rl = lane / LPR, l = lane % LPR;
-    const double* s_hre = reinterpret_cast<const double*>(stage);
-    const double* s_him = s_hre + w * 32;
-    const double* s_on = s_hre + w * 32 * hop_doubles(HOP);
-    const int* s_col = reinterpret_cast<const int*>(s_on + 32);                        // int32 columns, or base[8]
-    const unsigned short* s_d16 = reinterpret_cast<const unsigned short*>(s_col + 8);   // kHopConst16: deltas
-    // staged vector rows: [in | (in_e) | prev | (prev_e)], each 32 * B double2
+    // staged vector rows: [in | (in_e) | prev | (prev_e)], each TR * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
-    const double2* s_in_e = s_in + 32 * B;
-    const double2* s_prev = s_in + (MSD ? 2 : 1) * 32 * B;
-    const double2* s_prev_e = s_prev + 32 * B;
+    const double2* s_in_e = s_in + TR * B;
+    const double2* s_prev = s_in + (MSD ? 2 : 1) * TR * B;
+    const double2* s_prev_e = s_prev + TR * B;
     // lane-relative bases of the gathers (see cv_gather)
-    const uint32_t sl_in = smem_u32(s_in + l * V) - (uint32_t)(row0 * RB);
-    const uint32_t sl_in_e = smem_u32(s_in_e + l * V) - (uint32_t)(row0 * RB);
+    const uint32_t sl_in = smem_u32(s_in + l * V) - (uint32_t)row0 * (uint32_t)RB;
+    const uint32_t sl_in_e = smem_u32(s_in_e + l * V) - (uint32_t)row0 * (uint32_t)RB;
     const char* gl_in = reinterpret_cast<const char*>(io.in + l * V);
     const char* gl_in_e = reinterpret_cast<const char*>(io.in_e + l * V);
-
-    const int r = j * RS + rl;
-    const bool ok = r < rows_valid;
-    const int si_ = r * B + l * V;                                     // element inside the staged rows
-    const size_t vi = (size_t)(row0 + (ok ? r : 0)) * B + l * V;       // element in global memory
-
-    // streamed own-row operands (evolved vector / phi_L): issued first, consumed last
-    CV<V> other = cv_zero<V>(), other_e = cv_zero<V>();
-    if (MODE == kModeEvolve || MSD) other = cv_ld_stream<V>(&a.src[vi]);
-    if (MSD) other_e = cv_ld_stream<V>(&a.src_e[vi]);
-    if (MODE == kModeLeft) other = cv_ld_stream<V>(&a.phiL[vi]);
-    double xm = 0.0;
-    if (MSD) xm = m.x[row0 + (ok ? r : 0)];
     constexpr bool PD = PrevDirect<B>::value;
-    CV<V> prev = cv_zero<V>(), prev_e = cv_zero<V>();
-    if (PD && !a.first && ok) {         // rows past the end keep prev = 0 (their T_m must stay 0 for the dots)
-        prev = cv_ld_stream<V>(&io.prev[vi]);
-        if (MSD) prev_e = cv_ld_stream<V>(&io.prev_e[vi]);
+    const int N = (int)m.N;
+
+    int r[U];                 // row inside the tile
+    bool ok[U];
+    size_t vi[U];             // element in global memory
+    const double* s_hre[U];
+    const double* s_on[U];
+    const int* s_col[U];
+    const unsigned short* s_d16[U];
+    CV<V> other[U], other_e[U], prev[U], prev_e[U], self[U], self_e[U];
+    double xm[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        r[u] = (j0 + u) * RS + rl;
+        ok[u] = r[u] < rows_valid;
+        vi[u] = (size_t)(row0 + (ok[u] ? r[u] : 0)) * B + l * V;
+        const unsigned char* rec = stage + (KT > 0 ? (r[u] >> 5) * REC : 0);
+        s_hre[u] = reinterpret_cast<const double*>(rec);
+        s_on[u] = s_hre[u] + w * 32 * hop_doubles(HOP);
+        s_col[u] = reinterpret_cast<const int*>(s_on[u] + 32);                          // int32 columns, or base[8]
+        s_d16[u] = reinterpret_cast<const unsigned short*>(s_col[u] + 8);                // kHopConst16: deltas
+        // streamed own-row operands (evolved vector / phi_L): issued first, consumed last
+        other[u] = cv_zero<V>();
+        other_e[u] = cv_zero<V>();
+        if (MODE == kModeEvolve || MSD) other[u] = cv_ld_stream<V>(&a.src[vi[u]]);
+        if (MSD) other_e[u] = cv_ld_stream<V>(&a.src_e[vi[u]]);
+        if (MODE == kModeLeft) other[u] = cv_ld_stream<V>(&a.phiL[vi[u]]);
+        xm[u] = 0.0;
+        if (MSD) xm[u] = m.x[row0 + (ok[u] ? r[u] : 0)];
+        prev[u] = cv_zero<V>();
+        prev_e[u] = cv_zero<V>();
+        if (PD && !io.first && ok[u]) {         // rows past the end keep prev = 0 (their x_m must stay 0 for the dots)
+            prev[u] = cv_ld_stream<V>(&io.prev[vi[u]]);
+            if (MSD) prev_e[u] = cv_ld_stream<V>(&io.prev_e[vi[u]]);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const int si_ = r[u] * B + l * V;                                 // element inside the staged rows
+        self[u] = ok[u] ? cv_lds_staged<V>(s_in + si_) : cv_zero<V>();
+        self_e[u] = (MSD && ok[u]) ? cv_lds_staged<V>(s_in_e + si_) : cv_zero<V>();
     }
 
-    const CV<V> self = ok ? cv_lds_staged<V>(s_in + si_) : cv_zero<V>();
-    const CV<V> self_e = (MSD && ok) ? cv_lds_staged<V>(s_in_e + si_) : cv_zero<V>();
-    const double on = s_on[r];
-
-    CV<V> sum = cv_zero<V>(), sum_e = cv_zero<V>(), sum_x = cv_zero<V>();   // H T, H e, [X,H] T (unscaled)
-    if (KT > 0) {
-        // all gathers of the row first (independent loads in flight), then the arithmetic
-        CV<V> v[KU], ve[MSD ? KU : 1];
-        double xn[MSD ? KU : 1];
+    CV<V> sum[U], sum_e[U], sum_x[U];   // H x, H e, [X,H] x (unscaled)
 #pragma unroll
-        for (int k = 0; k < KU; ++k) {
-            const int c = IDX16 ? s_col[k] + (int)s_d16[k * 32 + r] : s_col[k * 32 + r];
-            v[k] = cv_gather<V>(gl_in, sl_in, c, row0, RB);
-            if (MSD) {
-                ve[k] = cv_gather<V>(gl_in_e, sl_in_e, c, row0, RB);
-                xn[k] = m.x[c];
+    for (int u = 0; u < U; ++u) sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
+    if (KT > 0) {
+        // all gathers of the rows first (independent loads in flight), then the arithmetic
+        CV<V> v[U][KU], ve[U][MSD ? KU : 1];
+        double xn[U][MSD ? KU : 1];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int rr = r[u] & 31;
+#pragma unroll
+            for (int k = 0; k < KU; ++k) {
+                const int c = col_of<IDX16>(s_col[u], s_d16[u], k, rr, N);
+                v[u][k] = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
+                if (MSD) {
+                    ve[u][k] = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
+                    xn[u][k] = m.x[c];
+                }
             }
         }
-        if (signal && lane == 0) red_release_gpu_inc(signal);           // see cheb_step_kernel, `pending`
 #pragma unroll
-        for (int k = 0; k < KU; ++k) {
-            double hr = 1.0, hi = 0.0;                                  // CONST: the factor is applied once below
-            if (!CONST) hr = s_hre[k * 32 + r];
-            if (CPLX) hi = s_him[k * 32 + r];
-            if (CONST) cv_add<V>(sum, v[k]);
-            else cv_fma<V, CPLX>(sum, hr, hi, v[k]);
-            if (MSD) {
-                if (CONST) cv_add<V>(sum_e, ve[k]);
-                else cv_fma<V, CPLX>(sum_e, hr, hi, ve[k]);
-                // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
-                const double ndx = -min_image(xn[k] - xm, m.box);
-                cv_fma<V, CPLX>(sum_x, ndx * hr, ndx * hi, v[k]);
+        for (int u = 0; u < U; ++u) {
+            const int rr = r[u] & 31;
+#pragma unroll
+            for (int k = 0; k < KU; ++k) {
+                double hr = 1.0, hi = 0.0;                                  // CONST: the factor is applied once below
+                if (!CONST) hr = s_hre[u][k * 32 + rr];
+                if (CPLX) hi = (s_hre[u] + w * 32)[k * 32 + rr];
+                if (CONST) cv_add<V>(sum[u], v[u][k]);
+                else cv_fma<V, CPLX>(sum[u], hr, hi, v[u][k]);
+                if (MSD) {
+                    if (CONST) cv_add<V>(sum_e[u], ve[u][k]);
+                    else cv_fma<V, CPLX>(sum_e[u], hr, hi, ve[u][k]);
+                    // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
+                    const double ndx = -min_image(xn[u][k] - xm[u], m.box);
+                    cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, v[u][k]);
+                }
             }
         }
     } else {
-        if (signal && lane == 0) red_release_gpu_inc(signal);
+        const int rr = r[0] & 31;
         for (int k = 0; k < w; ++k) {
-            const int c = IDX16 ? s_col[k] + (int)s_d16[k * 32 + r] : s_col[k * 32 + r];
+            const int c = col_of<IDX16>(s_col[0], s_d16[0], k, rr, N);
             double hr = 1.0, hi = 0.0;
-            if (!CONST) hr = s_hre[k * 32 + r];
-            if (CPLX) hi = s_him[k * 32 + r];
-            const CV<V> vv = cv_gather<V>(gl_in, sl_in, c, row0, RB);
-            if (CONST) cv_add<V>(sum, vv);
-            else cv_fma<V, CPLX>(sum, hr, hi, vv);
+            if (!CONST) hr = s_hre[0][k * 32 + rr];
+            if (CPLX) hi = (s_hre[0] + w * 32)[k * 32 + rr];
+            const CV<V> vv = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
+            if (CONST) cv_add<V>(sum[0], vv);
+            else cv_fma<V, CPLX>(sum[0], hr, hi, vv);
             if (MSD) {
-                const CV<V> vve = cv_gather<V>(gl_in_e, sl_in_e, c, row0, RB);
-                if (CONST) cv_add<V>(sum_e, vve);
-                else cv_fma<V, CPLX>(sum_e, hr, hi, vve);
-                const double ndx = -min_image(m.x[c] - xm, m.box);
-                cv_fma<V, CPLX>(sum_x, ndx * hr, ndx * hi, vv);
+                const CV<V> vve = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
+                if (CONST) cv_add<V>(sum_e[0], vve);
+                else cv_fma<V, CPLX>(sum_e[0], hr, hi, vve);
+                const double ndx = -min_image(m.x[c] - xm[0], m.box);
+                cv_fma<V, CPLX>(sum_x[0], ndx * hr, ndx * hi, vv);
             }
         }
     }
-    if (!PD && !a.first && ok) {
-        prev = cv_lds_staged<V>(s_prev + si_);
-        if (MSD) prev_e = cv_lds_staged<V>(s_prev_e + si_);
-    }
-    const double hs = CONST ? scale * m.hop_const : scale;              // scale of the neighbour sums
-    const double os = scale * on;                                       // scale of the on-site term
-    CV<V> t, te;   // T_m (b_k) and e_m
+    const double hs = CONST ? io.scale * m.hop_const : io.scale;          // scale of the neighbour sums
 #pragma unroll
-    for (int q = 0; q < V; ++q) {
-        t.re[q] = fma(hs, sum.re[q], fma(os, self.re[q], -prev.re[q]));
-        t.im[q] = fma(hs, sum.im[q], fma(os, self.im[q], -prev.im[q]));
-        if (MODE == kModeDoubling) {
-            red[0 * V + q] += t.re[q] * t.re[q] + t.im[q] * t.im[q];
-            red[1 * V + q] += t.re[q] * self.re[q] + t.im[q] * self.im[q];
-            // <T_{m-1}|T_{m-1}> is only used from the first launch (C_0); later ones had it as <T_m|T_m>
-            if (a.first) red[2 * V + q] += self.re[q] * self.re[q] + self.im[q] * self.im[q];
-        } else if (MODE == kModeLeft) {   // conj(l) * t
-            red[0 * V + q] += other.re[q] * t.re[q] + other.im[q] * t.im[q];
-            red[1 * V + q] += other.re[q] * t.im[q] - other.im[q] * t.re[q];
-        } else {
-            // Clenshaw: b_k = c_k src + 2 H~ b_{k+1} - b_{k+2}; no accumulator is read or written
-            t.re[q] += io.cr * other.re[q] - io.ci * other.im[q];
-            t.im[q] += io.cr * other.im[q] + io.ci * other.re[q];
-            if (MSD) {
-                te.re[q] = fma(hs, sum_e.re[q] + sum_x.re[q], fma(os, self_e.re[q], -prev_e.re[q]));
-                te.im[q] = fma(hs, sum_e.im[q] + sum_x.im[q], fma(os, self_e.im[q], -prev_e.im[q]));
-                te.re[q] += io.cr * other_e.re[q] - io.ci * other_e.im[q];
-                te.im[q] += io.cr * other_e.im[q] + io.ci * other_e.re[q];
+    for (int u = 0; u < U; ++u) {
+        const int si_ = r[u] * B + l * V;
+        if (!PD && !io.first && ok[u]) {
+            prev[u] = cv_lds_staged<V>(s_prev + si_);
+            if (MSD) prev_e[u] = cv_lds_staged<V>(s_prev_e + si_);
+        }
+        const double os = io.scale * s_on[u][r[u] & 31];                  // scale of the on-site term
+        CV<V> t, te;   // x_m (b_k) and e_m
+#pragma unroll
+        for (int q = 0; q < V; ++q) {
+            t.re[q] = fma(hs, sum[u].re[q], fma(os, self[u].re[q], -prev[u].re[q]));
+            t.im[q] = fma(hs, sum[u].im[q], fma(os, self[u].im[q], -prev[u].im[q]));
+            if (MODE == kModeDoubling) {
+                red[0 * V + q] += t.re[q] * t.re[q] + t.im[q] * t.im[q];
+                red[1 * V + q] += t.re[q] * self[u].re[q] + t.im[q] * self[u].im[q];
+                // <x_{m-1}|x_{m-1}> is only used from the first step (C_0); later ones had it as <x_m|x_m>
+                if (io.first) red[2 * V + q] += self[u].re[q] * self[u].re[q] + self[u].im[q] * self[u].im[q];
+            } else if (MODE == kModeLeft) {   // conj(l) * t
+                red[0 * V + q] += other[u].re[q] * t.re[q] + other[u].im[q] * t.im[q];
+                red[1 * V + q] += other[u].re[q] * t.im[q] - other[u].im[q] * t.re[q];
+            } else {
+                // Clenshaw: b_k = c_k src + 2 H~ b_{k+1} - b_{k+2}; no accumulator is read or written
+                t.re[q] += io.cr * other[u].re[q] - io.ci * other[u].im[q];
+                t.im[q] += io.cr * other[u].im[q] + io.ci * other[u].re[q];
+                if (MSD) {
+                    te.re[q] = fma(hs, sum_e[u].re[q] + sum_x[u].re[q], fma(os, self_e[u].re[q], -prev_e[u].re[q]));
+                    te.im[q] = fma(hs, sum_e[u].im[q] + sum_x[u].im[q], fma(os, self_e[u].im[q], -prev_e[u].im[q]));
+                    te.re[q] += io.cr * other_e[u].re[q] - io.ci * other_e[u].im[q];
+                    te.im[q] += io.cr * other_e[u].im[q] + io.ci * other_e[u].re[q];
+                }
             }
         }
-    }
-    if (ok && io.store) {
-        cv_st<V>(&io.out[vi], t);
-        if (MSD) cv_st<V>(&io.out_e[vi], te);
+        if (ok[u] && io.store) {
+            cv_st<V>(&io.out[vi[u]], t);
+            if (MSD) cv_st<V>(&io.out_e[vi[u]], te);
+        }
     }
 }
 
@@ -642,38 +715,19 @@ __device__ __forceinline__ void warp_flush(double (&v)[Q * V], double* dst, int 
 #pragma unroll
         for (int q = 0; q < Q; ++q)
 #pragma unroll
-            for (int j = 0; j < V; ++j) dst[q * B + lane * V + j] += v[q * V + j];
+            for (int j = 0; j < V; ++j) dst[q * B + lane * V + j] = v[q * V + j];
     }
 #pragma unroll
     for (int q = 0; q < Q * V; ++q) v[q] = 0.0;
     __syncwarp();
 }
 
-// Deterministic CTA / grid stage of the reduction: s_part[warp][P] -> per-block partial -> the last
-// block to finish sums the per-block partials in a fixed order (no floating-point atomics).
-// Value p < P0 goes to r0[p], the others to r1[p - P0] (second step of a fused pair).
-__device__ __forceinline__ void block_finish(const double* s_part, int P, int P0, double* partials,
-                                             unsigned int* ticket, double* r0, double* r1) {
-    __shared__ double s_tree[kThreads + 32];   // the step kernel calls this with its producer warp as well
-    __shared__ int s_last;
+// Fixed-shape sum of the per-block partials [gridDim.x][P] (thread t handles value t % P, blocks
+// strand, strand + S, ...; then the strands in order): every block computes the same bits for the
+// same partials.  All kThreads threads of the CTA must call it.
+__device__ __forceinline__ void sum_partials(const double* partials, int P, double* result) {
+    __shared__ double s_tree[kThreads];
     const int tid = threadIdx.x;
-    __syncthreads();
-    if (tid < P) {
-        double s = 0.0;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) s += s_part[w * P + tid];
-        partials[(size_t)blockIdx.x * P + tid] = s;
-    }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-        unsigned int t = atomicAdd(ticket, 1u);
-        s_last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    // fixed-shape sum over blocks: thread t handles value (t % P), blocks strand, strand + S, ...
     const int S = kThreads / P;              // strands per value
     const int pv = tid % P, strand = tid / P;
     double s = 0.0;
@@ -684,34 +738,42 @@ __device__ __forceinline__ void block_finish(const double* s_part, int P, int P0
     if (tid < P) {
         double tot = 0.0;
         for (int j = 0; j < S; ++j) tot += s_tree[j * P + tid];
-        if (tid < P0) r0[tid] = tot;
-        else r1[tid - P0] = tot;
+        result[tid] = tot;
     }
-    if (tid == 0) *ticket = 0u;
+    __syncthreads();
 }
 
-__device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
-    unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
+// CTA stage of the deterministic reduction: s_part[warp][P] -> partials[block][P]
+__device__ __forceinline__ void block_partial(const double* s_part, int P, double* partials) {
+    const int tid = threadIdx.x;
+    __syncthreads();
+    if (tid < P) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) s += s_part[w * P + tid];
+        partials[(size_t)blockIdx.x * P + tid] = s;
+    }
 }
 
-
-// One Chebyshev recurrence step fused with what consumes it (single-step launches; the default).
-// Every warp issues its own TMA copies (lane 0) one or more slices ahead.  Persistent CTAs: the slices are cut
-// into runs of a.run consecutive slices; CTA c walks runs c, c + G, c + 2G, ...; inside a run warp w
-// takes slices w, w + kWarps, ...  A CTA therefore streams a contiguous band of rows and the grid
+// Recurrence steps [a.m_begin, a.m_end), each x_m = 2 H~ x_{m-1} - x_{m-2} fused with what consumes it.
+// Every warp issues its own TMA copies (lane 0) one or more tiles ahead.  Persistent CTAs: the tiles are
+// cut into runs of a.run consecutive tiles; CTA c walks runs c, c + G, c + 2G, ...; inside a run warp w
+// takes tiles w, w + kWarps, ...  A CTA therefore streams a contiguous band of rows and the grid
 // sweeps the vector as a tight front, so gathers to nearby rows (the +-x, +-y, +-z neighbours of a
 // lattice) are served by L1/L2.  All loop indices are kept incrementally (no divisions in the loop).
+// Between the steps of a multi-step (cooperative) launch: per-block dot partials, a grid barrier, and
+// block m % G sums the partials of step m in a fixed order while the others go on.
 template <int B, int KT, int HOP, int MODE>
-__global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const StepArgs a) {
+__global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const RecArgs a) {
+    using LS = LaneShape<B, KT>;
     constexpr int Q = ModeTraits<MODE>::Q;
-    constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
+    constexpr int V = LS::V, ROUNDS = LS::ROUNDS, U = LS::U, S = LS::S, TR = 32 * S;
     constexpr int RB = B * 16, QB = Q * B;
     constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
+    constexpr bool MSD = (MODE == kModeEvolveMsd);
+    constexpr int kPair = MSD ? 2 : 1;
     __shared__ double s_part[DOTS ? kWarps * QB : 1];
-    const StepIO& io = a.io[0];
-    constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
+    __shared__ int s_last;
     extern __shared__ __align__(1024) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
@@ -723,20 +785,17 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     double red[Q * V];
 #pragma unroll
     for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
-    if (DOTS) {
-        for (int i = lane; i < QB; i += 32) s_part[warp * QB + i] = 0.0;
-    }
-    const double scale = a.half ? m.inv_dE : 2.0 * m.inv_dE;
 
-    const int N = (int)m.N, n_slices = (int)m.n_slices;
+    const int N = (int)m.N;
+    const int n_tiles = ((int)m.n_slices + S - 1) / S;
     const int per = a.run / kWarps;
-    const int n_runs = (n_slices + a.run - 1) / a.run;
+    const int n_runs = (n_tiles + a.run - 1) / a.run;
     const int G = gridDim.x;
     const int my_runs = (int)blockIdx.x < n_runs ? (n_runs - (int)blockIdx.x + G - 1) / G : 0;
     int n_my = 0;
     if (my_runs > 0) {
         const int last = blockIdx.x + (my_runs - 1) * G;
-        const int rem = n_slices - last * a.run;          // slices in my last run (may be partial)
+        const int rem = n_tiles - last * a.run;          // tiles in my last run (may be partial)
         const int in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
         n_my = (my_runs - 1) * per + in_last;
     }
@@ -748,316 +807,159 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     }
     __syncwarp();
 
-    // position of a pipeline cursor: slice (forward order), index inside the run, stage, phase
-    struct Cursor {
-        int s, k, st;
-        uint32_t ph;
-    };
-    const int jump = G * a.run - (per - 1) * kWarps;     // last slice of a run -> first slice of my next run
-    auto advance = [&](Cursor& c) {
-        if (++c.k == per) {
-            c.k = 0;
-            c.s += jump;
-        } else {
-            c.s += kWarps;
+    const int jump = G * a.run - (per - 1) * kWarps;     // last tile of a run -> first tile of my next run
+    // the stage ring and its mbarrier phases run on across the steps of the launch
+    int p_st = 0, c_st = 0;
+    uint32_t c_ph = 0;
+    unsigned int epoch = 0;                               // grid barriers passed
+
+    for (int mm = a.m_begin; mm < a.m_end; ++mm) {
+        // ---- operands of step mm (CTA-uniform)
+        StepCtx io;
+        const int last_term = a.terms - 1;
+        io.first = (mm == 1);
+        const bool half = a.clenshaw ? (mm == last_term) : (mm == 1);
+        io.scale = half ? m.inv_dE : 2.0 * m.inv_dE;
+        const int s_in = (mm + 1) % 3, s_prev = mm % 3, s_out = (mm + 2) % 3;      // (m-2)%3, (m-3)%3, (m-1)%3
+        io.in = (mm == 1) ? a.x0 : a.ring[s_in];
+        io.tm_in = (mm == 1) ? a.tm_x0 : a.tm_ring[s_in];
+        io.prev = (mm == 2) ? a.x0 : a.ring[s_prev];
+        io.tm_prev = (mm == 2) ? a.tm_x0 : a.tm_ring[s_prev];
+        io.out = a.ring[s_out];
+        io.in_e = io.prev_e = nullptr;
+        io.out_e = nullptr;
+        io.tm_in_e = io.tm_prev_e = nullptr;
+        if (MSD) {
+            io.in_e = (mm == 1) ? a.e0 : a.ring_e[s_in];
+            io.tm_in_e = (mm == 1) ? a.tm_e0 : a.tm_ring_e[s_in];
+            io.prev_e = (mm == 2) ? a.e0 : a.ring_e[s_prev];
+            io.tm_prev_e = (mm == 2) ? a.tm_e0 : a.tm_ring_e[s_prev];
+            io.out_e = a.ring_e[s_out];
         }
-        if (++c.st == stages) {
-            c.st = 0;
-            c.ph ^= 1u;
-        }
-    };
-    auto issue = [&](const Cursor& c) {   // lane 0 only: every HBM stream of the slice -> one stage, one mbarrier
-        const int s = a.reverse ? n_slices - 1 - c.s : c.s;
-        long long off;
-        uint32_t bytes;
-        if (KT > 0) {
-            bytes = (uint32_t)hop_record_bytes(KT, HOP);
-            off = (long long)s * bytes;
-        } else {
-            off = m.slice_off[s];
-            bytes = (uint32_t)(m.slice_off[s + 1] - off);
-        }
-        const int left = N - s * 32;
-        const uint32_t vbytes = (uint32_t)((left < 32 ? left : 32) * RB);
-        // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
-        // constant-hopping padding entries point at it)
-        const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-        const bool with_prev = !a.first && !PrevDirect<B>::value;
-        unsigned char* dst = wstage + c.st * stage_bytes;
-        unsigned char* vdst = dst + a.rec_bytes;
-        if (B >= 2) {
-            // tensor copies: always the full 32-row box (rows past the end of the buffer are zero-filled)
-            const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
-            const int unit = s * 4 * B;           // first 128-byte line of the slice
-            mbar_expect_tx(&bars[c.st], total);
-            bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
-            tensor_g2s(vdst, io.tm_in, unit, &bars[c.st]);
-            if (MODE == kModeEvolveMsd) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &bars[c.st]);
-            if (with_prev) {
-                tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &bars[c.st], policy);
-                if (MODE == kModeEvolveMsd) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &bars[c.st], policy);
-            }
-        } else {
-            const uint32_t total = bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
-            const size_t voff = (size_t)s * 32 * B;
-            mbar_expect_tx(&bars[c.st], total);
-            bulk_g2s(dst, m.rec + off, bytes, &bars[c.st], policy);
-            bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[c.st]);
-            if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &bars[c.st]);
-            if (with_prev) {
-                bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &bars[c.st], policy);
-                if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &bars[c.st], policy);
+        io.store = 1;
+        if (mm == last_term) {
+            io.store = a.store_last;
+            if (a.last_out) {
+                io.out = a.last_out;
+                io.out_e = a.last_out_e;
             }
         }
-    };
-
-    Cursor prod{(int)blockIdx.x * a.run + warp, 0, 0, 0u}, cons = prod;
-    int issued = 0;
-    if (lane == 0) {
-        for (; issued < stages - 1 && issued < n_my; ++issued) {
-            issue(prod);
-            advance(prod);
+        io.cr = io.ci = 0.0;
+        if (MODE == kModeEvolve || MSD) {
+            io.cr = a.coef[2 * (last_term - mm)];
+            io.ci = a.coef[2 * (last_term - mm) + 1];
         }
-    }
-    for (int i = 0; i < n_my; ++i) {
-        // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
-        if (lane == 0 && issued < n_my) {
-            issue(prod);
-            advance(prod);
-            ++issued;
-        }
-        mbar_wait(&bars[cons.st], cons.ph);
-        const unsigned char* stage = wstage + cons.st * stage_bytes;
-        const int slice = a.reverse ? n_slices - 1 - cons.s : cons.s;
-        int w = KT;
-        if (KT == 0) w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
-        const int row0 = slice * 32;
-        const int rows_valid = N - row0;          // >= 32 except in the last slice
-#pragma unroll 1
-        for (int j = 0; j < ROUNDS; ++j) walk_round<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, scale, red, nullptr);
-        advance(cons);
-        __syncwarp();
-    }
-    if (DOTS) {
-        warp_flush<B, Q, V>(red, s_part + warp * QB, lane);
-        block_finish(s_part, QB, QB, a.partials, a.ticket, io.result, io.result);
-    }
-}
+        const int reverse = a.alternate ? ((a.sweep0 + (mm - a.m_begin)) & 1) : a.sweep0;
 
-
-// TWO consecutive recurrence steps in one launch (a.n_steps == 2; opt-in, GPUQT_FUSE=1): the second
-// step trails the first by a fixed slack of the work list so that it finds T_m, T_{m-1} and the matrix records in L2: per pair of steps DRAM then sees T_{m-1},
-// T_{m-2} read and T_m, T_{m+1} written once each and the matrix once, instead of 6 vector passes
-// and 2 matrix passes.
-//
-// Persistent, warp-specialised CTAs of kWarps consumer warps + 1 producer warp.  The slices are cut
-// into runs of a.run consecutive slices; the work list is a sequence of items = (step, run); CTA c
-// takes items c, c + G, c + 2G, ...; inside a run consumer warp w takes slices w, w + kWarps, ...
-// Single-step launches use the arithmetic list item t = run t; fused launches read the list from
-// a.sched (built on the host from the table's sparsity, host_util.h).
-//   producer warp   walks the CTA's items; lane w < kWarps feeds consumer warp w: it waits for a
-//                   free stage of that warp (mbarrier empty[w][st]), writes a 16-byte header
-//                   {slice, step, flags, run} and issues the TMA bulk copies of the slice onto
-//                   full[w][st].  Before a second-step item it checks, all 32 lanes at once with
-//                   acquire loads, that the first-step runs the item gathers from are complete
-//                   (run_done[r] == kWarps) and sleeps otherwise.  The consumers never touch the
-//                   work list.
-//   consumer warp   waits full[w][st], walks the slice, arrives on empty[w][st].  After the last
-//                   slice of a first-step item it owes a release on run_done[run]; it pays one slice
-//                   later, right after that slice's gathers have been issued (the fence then overlaps
-//                   the gather latency), or at once when no slice is ready.
-// An item depends only on earlier items of the list and every warp publishes what it owes before
-// it blocks, so the scheme cannot deadlock as long as all CTAs are co-resident (the grid is sized
-// by occupancy).
-constexpr int kHdrBytes = 256;                    // per stage: the slice header (keeps the stages 256-byte aligned)
-constexpr int kFlagEnd = 1, kFlagOwesRelease = 2;
-
-template <int B, int KT, int HOP, int MODE>
-__global__ void __launch_bounds__(kThreads + 32, ModeTraits<MODE>::kMinBlocks) cheb_pair_kernel(const Mat m, const StepArgs a) {
-    constexpr int Q = ModeTraits<MODE>::Q;
-    constexpr int V = LaneShape<B>::V, ROUNDS = LaneShape<B>::ROUNDS;
-    constexpr int RB = B * 16, QB = Q * B;
-    constexpr int kPair = (MODE == kModeEvolveMsd) ? 2 : 1;
-    constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
-    extern __shared__ __align__(1024) unsigned char smem[];
-    __shared__ double s_part[DOTS ? kWarps * 2 * QB : 1];
-    const int tid = threadIdx.x, lane = tid & 31;
-    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler
-    const int stages = a.stages;
-    const int stage_bytes = a.stage_bytes;                     // record | vector rows | header
-    const int hdr_off = stage_bytes - kHdrBytes;
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [kWarps][kMaxStages]
-    uint64_t* empty = full + kWarps * kMaxStages;              // [kWarps][kMaxStages]
-    unsigned char* stage_base = smem + 128 * ((2 * kWarps * kMaxStages * 8 + 127) / 128);
-    const int P = a.n_steps * QB;                 // dot values per block
-
-    const int N = (int)m.N, n_slices = (int)m.n_slices;
-    const int n_runs = (n_slices + a.run - 1) / a.run;
-    const int G = gridDim.x;
-    const bool fused = a.sched != nullptr;
-    const int n_total = fused ? a.n_items : n_runs;
-
-    if (warp < kWarps && lane == 0) {
-        for (int s = 0; s < stages; ++s) {
-            mbar_init(&full[warp * kMaxStages + s], 1);
-            mbar_init(&empty[warp * kMaxStages + s], 1);
-        }
-        fence_mbar_init();
-    }
-    if (DOTS && warp < kWarps) {
-        for (int i = lane; i < P; i += 32) s_part[warp * P + i] = 0.0;
-    }
-    __syncthreads();
-
-    if (warp == kWarps) {
-        // ------------------------------------------------------------------ producer warp
-        const int cw = lane < kWarps ? lane : kWarps - 1;       // consumer warp this lane feeds
-        const bool feeds = lane < kWarps;
-        unsigned char* my_stages = stage_base + (size_t)cw * stages * stage_bytes;
-        uint64_t* my_full = full + cw * kMaxStages;
-        uint64_t* my_empty = empty + cw * kMaxStages;
-        int st = 0;
-        uint32_t ph = 0;
-        const uint64_t policy = policy_evict_first();
-        auto deps_done = [&](int run) {   // whole warp: have all first-step runs this run gathers from finished?
-            const int b = a.dep_ptr[run], e = a.dep_ptr[run + 1];
-            bool ok = true;
-#pragma unroll 1
-            for (int i0 = b; i0 < e; i0 += 32) {      // every lane acquires (lanes past the end re-read the last entry)
-                const int i = i0 + lane < e ? i0 + lane : e - 1;
-                ok = ok && (ld_acquire_gpu(a.run_done + a.dep_list[i]) >= (unsigned int)kWarps);
+        auto issue = [&](int t_virtual, int st) {   // lane 0 only: every stream of the tile -> one stage, one mbarrier
+            const int t = reverse ? n_tiles - 1 - t_virtual : t_virtual;
+            const int s = t * S;                   // first slice of the tile
+            long long off;
+            uint32_t bytes;
+            if (KT > 0) {
+                bytes = (uint32_t)hop_record_bytes(KT, HOP) * S;        // the record array is padded to whole tiles
+                off = (long long)s * (long long)hop_record_bytes(KT, HOP);
+            } else {
+                off = m.slice_off[s];
+                bytes = (uint32_t)(m.slice_off[s + 1] - off);
             }
-            return __all_sync(0xffffffffu, ok) != 0;
-        };
-        for (int t = blockIdx.x; t < n_total; t += G) {
-            int run = t, step = 0;
-            if (fused) {
-                const int2 e = a.sched[t];
-                run = e.x & kNoRun;
-                step = (e.x >> 30) & 1;
-            }
-            if (run == kNoRun) continue;
-            if (fused && step == 1) {
-                // rows stored through the generic proxy by other SMs, fenced and released at gpu scope
-                // (they are in L2) and acquired here; the TMA reads below are issued behind the acquire
-                // by control dependency and go to L2
-                while (!deps_done(run)) __nanosleep(200);
-            }
-            const StepIO& io = a.io[step];
-            int len = n_slices - run * a.run;
-            len = len < a.run ? len : a.run;
-            for (int k0 = 0; k0 < len; k0 += kWarps) {
-                if (feeds && k0 + lane < len) {
-                    const int vs = run * a.run + k0 + lane;                 // slice in sweep order
-                    const int s = a.reverse ? n_slices - 1 - vs : vs;
-                    mbar_wait(&my_empty[st], ph ^ 1u);                      // stage free (passes at once the first time round)
-                    unsigned char* dst = my_stages + st * stage_bytes;
-                    int flags = 0;
-                    if (fused && step == 0 && k0 + lane + kWarps >= len) flags |= kFlagOwesRelease;
-                    *reinterpret_cast<int4*>(dst + hdr_off) = make_int4(s, step, flags, run);
-                    long long off;
-                    uint32_t bytes;
-                    if (KT > 0) {
-                        bytes = (uint32_t)hop_record_bytes(KT, HOP);
-                        off = (long long)s * bytes;
-                    } else {
-                        off = m.slice_off[s];
-                        bytes = (uint32_t)(m.slice_off[s + 1] - off);
-                    }
-                    const int left = N - s * 32;
-                    const uint32_t vbytes = (uint32_t)((left < 32 ? left : 32) * RB);
-                    // T_{m-1} rows include the all-zero row N when it falls into this slice's window (the
-                    // constant-hopping padding entries point at it)
-                    const uint32_t vbytes_in = (uint32_t)((left + 1 < 32 ? left + 1 : 32) * RB);
-                    const bool with_prev = !a.first && !PrevDirect<B>::value;
-                    const uint32_t total = B >= 2 ? bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u)
-                                                  : bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
-                    unsigned char* vdst = dst + a.rec_bytes;
-                    const size_t voff = (size_t)s * 32 * B;
-                    const int unit = s * 4 * B;           // first 128-byte line of the slice (tensor copies, B >= 2)
-                    mbar_expect_tx(&my_full[st], total);
-                    // the first step of a fused pair leaves the record in L2 for the second one
-                    if (fused && step == 0) bulk_g2s_nohint(dst, m.rec + off, bytes, &my_full[st]);
-                    else bulk_g2s(dst, m.rec + off, bytes, &my_full[st], policy);
-                    if (B >= 2) {
-                        tensor_g2s(vdst, io.tm_in, unit, &my_full[st]);
-                        if (MODE == kModeEvolveMsd) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &my_full[st]);
-                        if (with_prev) {
-                            tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &my_full[st], policy);
-                            if (MODE == kModeEvolveMsd) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &my_full[st], policy);
-                        }
-                    } else {
-                        bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &my_full[st]);
-                        if (MODE == kModeEvolveMsd) bulk_g2s_nohint(vdst + 512 * B, io.in_e + voff, vbytes_in, &my_full[st]);
-                        if (with_prev) {
-                            bulk_g2s(vdst + kPair * 512 * B, io.prev + voff, vbytes, &my_full[st], policy);
-                            if (MODE == kModeEvolveMsd) bulk_g2s(vdst + 3 * 512 * B, io.prev_e + voff, vbytes, &my_full[st], policy);
-                        }
-                    }
-                    if (++st == stages) {
-                        st = 0;
-                        ph ^= 1u;
-                    }
+            const int left = N - s * 32;
+            const uint32_t vbytes = (uint32_t)((left < TR ? left : TR) * RB);
+            // x_{m-1} rows include the all-zero row N when it falls into this tile's window (the
+            // constant-hopping padding entries point at it)
+            const uint32_t vbytes_in = (uint32_t)((left + 1 < TR ? left + 1 : TR) * RB);
+            const bool with_prev = !io.first && !PrevDirect<B>::value;
+            unsigned char* dst = wstage + st * stage_bytes;
+            unsigned char* vdst = dst + a.rec_bytes;
+            if (B >= 2) {
+                // tensor copies: always the full 32-row box (rows past the end of the buffer are zero-filled)
+                const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
+                const int unit = s * 4 * B;           // first 128-byte line of the slice
+                mbar_expect_tx(&bars[st], total);
+                bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
+                tensor_g2s(vdst, io.tm_in, unit, &bars[st]);
+                if (MSD) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &bars[st]);
+                if (with_prev) {
+                    tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &bars[st], policy);
+                    if (MSD) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &bars[st], policy);
+                }
+            } else {
+                const uint32_t total = bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
+                const size_t voff = (size_t)s * 32 * B;
+                mbar_expect_tx(&bars[st], total);
+                bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
+                bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[st]);
+                if (MSD) bulk_g2s_nohint(vdst + TR * RB, io.in_e + voff, vbytes_in, &bars[st]);
+                if (with_prev) {
+                    bulk_g2s(vdst + kPair * TR * RB, io.prev + voff, vbytes, &bars[st], policy);
+                    if (MSD) bulk_g2s(vdst + 3 * TR * RB, io.prev_e + voff, vbytes, &bars[st], policy);
                 }
             }
-            // consumer warps without a slice in this (short, last) run owe nothing: the producer counts for them
-            if (fused && step == 0 && feeds && lane >= len) red_release_gpu_inc(a.run_done + run);
-        }
-        if (feeds) {   // end marker
-            mbar_wait(&my_empty[st], ph ^ 1u);
-            *reinterpret_cast<int4*>(my_stages + st * stage_bytes + hdr_off) = make_int4(0, 0, kFlagEnd, 0);
-            mbar_arrive(&my_full[st]);
-        }
-    } else {
-        // ------------------------------------------------------------------ consumer warps
-        unsigned char* my_stages = stage_base + (size_t)warp * stages * stage_bytes;
-        uint64_t* my_full = full + warp * kMaxStages;
-        uint64_t* my_empty = empty + warp * kMaxStages;
-        double* my_part = s_part + warp * P;
-        double red[Q * V];
-#pragma unroll
-        for (int q = 0; q < Q * V; ++q) red[q] = 0.0;
-        const double scale = a.half ? m.inv_dE : 2.0 * m.inv_dE;
-        int st = 0;
-        uint32_t ph = 0;
-        int red_step = 0;                   // step whose dots the register accumulators hold
-        unsigned int* pending = nullptr;    // release owed for a finished first-step item
-        while (true) {
-            if (pending && !mbar_test(&my_full[st], ph)) {     // nothing ready: pay now, then wait
-                if (lane == 0) red_release_gpu_inc(pending);
-                pending = nullptr;
+        };
+        // position of a pipeline cursor inside the step: tile (sweep order), index inside the run
+        int p_t = (int)blockIdx.x * a.run + warp, p_k = 0;
+        int c_t = p_t, c_k = 0;
+        int issued = 0;
+        if (lane == 0) {
+            for (; issued < stages - 1 && issued < n_my; ++issued) {
+                issue(p_t, p_st);
+                if (++p_k == per) { p_k = 0; p_t += jump; } else p_t += kWarps;
+                if (++p_st == stages) p_st = 0;
             }
-            mbar_wait(&my_full[st], ph);
-            const unsigned char* stage = my_stages + st * stage_bytes;
-            const int4 hdr = *reinterpret_cast<const int4*>(stage + hdr_off);
-            if (hdr.z & kFlagEnd) break;
-            const int slice = hdr.x, step = hdr.y;
-            if (DOTS && step != red_step) {
-                warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
-                red_step = step;
+        }
+        for (int i = 0; i < n_my; ++i) {
+            // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
+            if (lane == 0 && issued < n_my) {
+                issue(p_t, p_st);
+                if (++p_k == per) { p_k = 0; p_t += jump; } else p_t += kWarps;
+                if (++p_st == stages) p_st = 0;
+                ++issued;
             }
+            mbar_wait(&bars[c_st], c_ph);
+            const unsigned char* stage = wstage + c_st * stage_bytes;
+            const int tile = reverse ? n_tiles - 1 - c_t : c_t;
             int w = KT;
-            if (KT == 0) w = record_width(m.slice_off[slice + 1] - m.slice_off[slice], hop_doubles(HOP));
-            const int row0 = slice * 32;
-            const int rows_valid = N - row0;          // >= 32 except in the last slice
-            const StepIO& io = a.io[step];
+            if (KT == 0) w = record_width(m.slice_off[tile + 1] - m.slice_off[tile], hop_doubles(HOP));
+            const int row0 = tile * TR;
+            const int rows_valid = N - row0;          // >= TR except in the last tile
 #pragma unroll 1
-            for (int j = 0; j < ROUNDS; ++j) {
-                walk_round<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, scale, red, pending);
-                pending = nullptr;
-            }
+            for (int j = 0; j < ROUNDS; j += U) walk_rounds<B, KT, HOP, MODE>(m, a, io, stage, w, row0, rows_valid, j, lane, red);
+            if (++c_k == per) { c_k = 0; c_t += jump; } else c_t += kWarps;
+            if (++c_st == stages) { c_st = 0; c_ph ^= 1u; }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&my_empty[st]);
-            if (hdr.z & kFlagOwesRelease) pending = a.run_done + hdr.w;
-            if (++st == stages) {
-                st = 0;
-                ph ^= 1u;
-            }
         }
-        if (pending && lane == 0) red_release_gpu_inc(pending);
-        if (DOTS) warp_flush<B, Q, V>(red, my_part + red_step * QB, lane);
+        // lane 0's producer stage index may run ahead of the other lanes' view: only lane 0 uses p_st
+
+        // ---- end of the step: dots, and the barrier before the next one
+        double* result = DOTS ? a.dots + (size_t)(mm - a.dot_m0) * QB : nullptr;
+        if (!a.multi) {
+            if (DOTS) {
+                warp_flush<B, Q, V>(red, s_part + warp * QB, lane);
+                block_partial(s_part, QB, a.partials);
+                __threadfence();
+                __syncthreads();
+                if (tid == 0) {
+                    const unsigned int t = atomicAdd(a.ticket, 1u);
+                    s_last = (t == gridDim.x - 1);
+                }
+                __syncthreads();
+                if (s_last) {                       // CTA-uniform
+                    __threadfence();
+                    sum_partials(a.partials, QB, result);
+                    if (tid == 0) *a.ticket = 0u;
+                }
+            }
+        } else {
+            double* part = a.partials + (size_t)(mm & 1) * G * QB;
+            if (DOTS) {
+                warp_flush<B, Q, V>(red, s_part + warp * QB, lane);
+                block_partial(s_part, QB, part);
+            }
+            ++epoch;
+            grid_barrier(a.barrier, epoch * (unsigned int)G);
+            if (DOTS && (int)blockIdx.x == mm % G) sum_partials(part, QB, result);
+        }
     }
-    if (DOTS) block_finish(s_part, P, QB, a.partials, a.ticket, a.io[0].result, a.io[1].result);
 }
 
 // Address of entry (row, k) pieces inside the packed records (plain global reads; used by the
@@ -1069,8 +971,13 @@ struct RecView {
     const int* col;                  // int32 columns, or base[8] of the 16-bit variant
     const unsigned short* d16;       // 16-bit variant: deltas, else nullptr
     int w;
+    int N;
     __device__ __forceinline__ int col_at(int k, int r) const {
-        return d16 ? col[k] + (int)d16[k * 32 + r] : col[k * 32 + r];
+        if (d16) {
+            const unsigned d = d16[k * 32 + r];
+            return d == kPad16 ? N : col[k] + (int)d;
+        }
+        return col[k * 32 + r];
     }
 };
 __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
@@ -1084,6 +991,7 @@ __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
         bytes = m.slice_off[slice + 1] - off;
     }
     RecView v;
+    v.N = (int)m.N;
     v.w = m.hop == kHopConst16 ? m.K : record_width(bytes, nd);     // the 16-bit variant is always uniform
     v.hre = reinterpret_cast<const double*>(m.rec + off);
     v.him = v.hre + (size_t)v.w * 32;
@@ -1145,7 +1053,7 @@ __global__ void __launch_bounds__(kThreads) dot_kernel(long long N, const double
     block_reduce_and_finish<B, 2>(red, partials, ticket, result);
 }
 
-#ifndef GPUQT_PAIR_TU   // the non-template kernels below belong to gpuqt.cu's translation unit only
+#ifndef GPUQT_STEP_TU   // the non-template kernels below belong to gpuqt.cu's translation unit only
 // [batch][N] (host order) <-> [N][B] (device order)
 __global__ void to_device_layout(long long N, int B, const double2* __restrict__ src, double2* __restrict__ dst) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1197,15 +1105,23 @@ __global__ void finalize_left(int B, int n_moments, const double* __restrict__ d
     C[(size_t)b * n_moments + n] = dots[((size_t)n * 2 + 0) * B + b];
 }
 
-// Jackson damping folded with the (2 - delta_n0) factor: mu_scale[n] = g_n (2 - delta_n0)  (Eq. 31)
-__global__ void jackson_kernel(int n_moments, double* __restrict__ gs) {
+// Damping factors folded with the (2 - delta_n0) factor: gs[n] = g_n (2 - delta_n0).
+//   kind 0  Jackson, Eq. 31:  g_n = (1 - n a) cos(pi n a) + a sin(pi n a) cot(pi a), a = 1 / (N_m + 1)
+//   kind 1  Lorentz (Weisse et al., the paper's ref. [33]):  g_n = sinh(lambda (1 - n / N_m)) / sinh(lambda)
+//   kind 2  none (Dirichlet):  g_n = 1
+__global__ void damping_kernel(int kind, double lambda, int n_moments, double* __restrict__ gs) {
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= n_moments) return;
-    const double alpha = 1.0 / (n_moments + 1.0);
-    double s, c, s1, c1;
-    sincospi(n * alpha, &s, &c);
-    sincospi(alpha, &s1, &c1);
-    const double g = (1.0 - n * alpha) * c + alpha * s * (c1 / s1);
+    double g = 1.0;
+    if (kind == 0) {
+        const double alpha = 1.0 / (n_moments + 1.0);
+        double s, c, s1, c1;
+        sincospi(n * alpha, &s, &c);
+        sincospi(alpha, &s1, &c1);
+        g = (1.0 - n * alpha) * c + alpha * s * (c1 / s1);
+    } else if (kind == 1) {
+        g = sinh(lambda * (1.0 - (double)n / (double)n_moments)) / sinh(lambda);
+    }
     gs[n] = (n == 0) ? g : 2.0 * g;
 }
 
@@ -1288,18 +1204,14 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
     if (dx) dx[i] = d;
 }
 
-#endif  // GPUQT_PAIR_TU
-
-}  // namespace gpuqt
-
-namespace gpuqt {
+#endif  // GPUQT_STEP_TU
 
 // ---------------------------------------------------------------------------------- small lattices
 // Lattices whose matrix and four vector sets fit one SM's shared memory (config c1: 2304 orbitals) are
-// launch-latency bound on the streaming kernels (one launch per recurrence term).  cheb_small_kernel
-// runs a WHOLE recurrence in one launch of one CTA: matrix (decoded to plain arrays) and vectors live in
-// shared memory, the terms are separated by __syncthreads(), the per-term dots are reduced in a fixed
-// order (warp shuffle -> shared memory over warps) and written straight to dots[term].
+// launch-latency bound on the streaming kernels.  cheb_small_kernel runs a WHOLE recurrence in one
+// launch of one CTA: matrix (decoded to plain arrays) and vectors live in shared memory, the terms are
+// separated by __syncthreads(), the per-term dots are reduced in a fixed order (warp shuffle -> shared
+// memory over warps) and written straight to dots[term].
 //   MODE doubling : T_m from v0; dots {<T_m|T_m>, Re<T_m|T_{m-1}>, <T_{m-1}|T_{m-1}>} per term   (Eq. 28, 30)
 //   MODE left     : T_n from v0; dots <aux|T_n> (Re, Im) per term                                  (Eq. 29)
 //   MODE evolve   : out = sum_k c_k T_k(H~) aux by Clenshaw (v0 unused; coef[k] = c_k)             (Eq. 17)
@@ -1329,8 +1241,6 @@ __global__ void __launch_bounds__(kSmallThreads, 1) cheb_small_kernel(const Mat 
     double* hre = on + N;                                               // [K][N] if nd >= 1
     double* him = hre + (nd >= 1 ? (size_t)K * N : 0);                  // [K][N] if nd == 2
     int* col = reinterpret_cast<int*>(him + (nd == 2 ? (size_t)K * N : 0));   // [K][N]; padding -> row itself, weight 0
-    double* wpad = nullptr;
-    (void)wpad;
     // decode the records into plain arrays
     for (int row = tid; row < N; row += kSmallThreads) {
         const RecView rv = record_view(m, row >> 5);

@@ -1,6 +1,8 @@
 """Host-side logic of the C-ABI library, no GPU: the library loads, exports every symbol that
 include/gpuqt.h declares, validates inputs with the documented status codes, and its Bessel table
-(Miller recurrence) agrees with identities, textbook values and the oracle's libm-based table."""
+(Miller recurrence) agrees with identities, textbook values and the oracle's libm-based table, the
+tuning options have the documented defaults and create-time failures report through
+gpuqt_last_error(NULL)."""
 import ctypes
 import os
 import re
@@ -104,68 +106,35 @@ def test_no_gpu_fails_loudly(gq):
         gq.GpuQT(L.chain(8), batch=1)
 
 
-def _csr(sets):
-    ptr = np.zeros(len(sets) + 1, np.int32)
-    ptr[1:] = np.cumsum([len(x) for x in sets])
-    return ptr, np.array([v for x in sets for v in sorted(x)], np.int32)
-
-
-def _check_schedule(sets, run, grid, reverse, slack):
-    """Invariants the fused kernel relies on (kernels.cuh, cheb_step_kernel): `sets[s]` = slices that
-    slice s gathers from."""
+def test_options_and_create_errors(gq):
+    """gpuqt_default_options documents the defaults; a failing gpuqt_create leaves its reason in
+    gpuqt_last_error(NULL) instead of printing (checks that need no GPU run before any CUDA call)."""
     from paper_1705_01387_b200 import binding
-    n = len(sets)
-    ptr, lst = _csr(sets)
-    items, dep_ptr, dep_list = binding.fused_schedule(ptr, lst, run, grid, reverse, slack)
-    NO = (1 << 30) - 1
-    n_runs = (n + run - 1) // run
-    runs, steps = items[:, 0] & NO, (items[:, 0] >> 30) & 1
-    real = runs != NO
-    # every run exactly once per step; first-step items in sweep order
-    assert list(runs[real & (steps == 0)]) == list(range(n_runs))
-    assert sorted(runs[real & (steps == 1)]) == list(range(n_runs))
-    assert np.all(steps[~real] == 0)
-    pos1 = {int(r): t for t, r in enumerate(runs) if r != NO and steps[t] == 0}
-    virt = (lambda s_: n - 1 - s_) if reverse else (lambda s_: s_)
-    for R in range(n_runs):
-        need = set()
-        for vs in range(R * run, min(n, (R + 1) * run)):
-            need |= {virt(d) // run for d in sets[virt(vs)]}
-        assert R in need
-        assert sorted(need) == list(dep_list[dep_ptr[R]:dep_ptr[R + 1]])     # exactly the runs gathered from
-    for t in np.nonzero(real & (steps == 1))[0]:
-        deps = dep_list[dep_ptr[runs[t]]:dep_ptr[runs[t] + 1]]
-        # a second-step item depends only on EARLIER items (no deadlock), at least `slack` back
-        assert max(pos1[int(r)] for r in deps) + slack <= t
-    return items
+    o = binding.default_options()
+    assert o.struct_bytes == ctypes.sizeof(binding.Options)
+    assert (o.stages, o.blocks_per_sm, o.run, o.alternate, o.hop_const, o.idx16, o.small, o.persistent) == \
+        (0, 0, 0, 1, 1, 1, 1, -1)
+    with pytest.raises(KeyError):
+        binding.default_options(no_such_option=1)
+    lib = gq.load()
+    m = L.square(6, 5, W=2.0, seed=1)
+    h = ctypes.c_void_p()
+    dummy = ctypes.c_void_p(256)                      # never dereferenced: the calls below fail before any CUDA work
 
-
-def test_fused_schedule_invariants():
-    rng_ = np.random.default_rng(5)
-    # periodic cubic 12^3 in slices of 32 rows: neighbours +-1, +-12, +-144 rows with wrap-around
-    L3 = 12
-    N = L3 ** 3
-    n = (N + 31) // 32
-    sets = [{s_} for s_ in range(n)]
-    for m in range(N):
-        x, y, z = m % L3, (m // L3) % L3, m // (L3 * L3)
-        for c in (((x - 1) % L3, y, z), ((x + 1) % L3, y, z), (x, (y - 1) % L3, z), (x, (y + 1) % L3, z),
-                  (x, y, (z - 1) % L3), (x, y, (z + 1) % L3)):
-            sets[m >> 5].add((c[0] + L3 * (c[1] + L3 * c[2])) >> 5)
-    for run, grid, reverse, slack in ((8, 3, 0, 3), (8, 3, 1, 1), (16, 2, 0, 2), (8, 7, 1, 10), (8, 100, 0, 100)):
-        _check_schedule(sets, run, grid, reverse, slack)
-    # banded open chain: the second sweep follows the first at a constant distance, few no-ops
-    n = 4000
-    sets = [{max(s_ - 1, 0), s_, min(s_ + 1, n - 1)} for s_ in range(n)]
-    items = _check_schedule(sets, 8, 16, 0, 16)
-    assert len(items) <= 2 * 500 + 3 * 16
-    # both kinds of work reach every CTA: within any two consecutive rounds a CTA sees both steps
-    steps = (items[:, 0] >> 30) & 1
-    for c in range(16):
-        mine = steps[c::16][2:-3]
-        assert 0 < mine.mean() < 1
-    # arbitrary sparsity: still valid (the second step simply follows the whole first sweep)
-    n = 300
-    sets = [{s_, int(rng_.integers(0, n)), int(rng_.integers(0, n))} for s_ in range(n)]
-    _check_schedule(sets, 8, 5, 0, 5)
-    _check_schedule(sets, 8, 5, 1, 5)
+    def create(model, batch=1, options=None, volume=None):
+        return lib.gpuqt_create_with_options(ctypes.byref(h), *binding._model_tuple(model),
+                                             ctypes.c_double(model.volume if volume is None else volume),
+                                             ctypes.c_double(model.energy_scale), ctypes.c_int32(batch), ctypes.c_int(0),
+                                             dummy, ctypes.c_size_t(1 << 30), None,
+                                             None if options is None else ctypes.byref(options))
+    assert create(m, batch=3) == -1 and b"batch" in lib.gpuqt_last_error(None)
+    assert create(m, volume=0.0) == -1
+    bad = binding.default_options()
+    bad.struct_bytes = 4096
+    assert create(m, options=bad) == -1 and b"struct_bytes" in lib.gpuqt_last_error(None)
+    assert create(m, options=binding.default_options(stages=9)) == -1
+    broken = L.square(6, 5, W=2.0, seed=1)
+    broken.nbr_index = broken.nbr_index.copy()
+    broken.nbr_index[7] = broken.N
+    assert create(broken) == -2 and b"out of range" in lib.gpuqt_last_error(None)
+    assert h.value is None

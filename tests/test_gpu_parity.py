@@ -17,11 +17,28 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-10
 
 
-@pytest.fixture(autouse=True, params=["streaming", "small_path"])
-def small_lattice_path(request, monkeypatch):
-    """Every case runs twice: on the streaming kernels only (GPUQT_SMALL=0) and with the one-CTA
-    whole-recurrence kernel enabled, which takes over wherever matrix + vectors fit one SM's shared memory."""
-    monkeypatch.setenv("GPUQT_SMALL", "0" if request.param == "streaming" else "1")
+PATHS = {
+    # one plain launch per recurrence step
+    "streaming": {"small": 0, "persistent": 0},
+    # the one-CTA whole-recurrence kernel wherever matrix + vectors fit one SM's shared memory
+    "small_path": {"small": 1, "persistent": 0},
+    # whole recurrences as ONE cooperative launch of the streaming kernel, grid barriers between the steps
+    "persistent": {"small": 0, "persistent": 1},
+}
+
+
+@pytest.fixture(autouse=True, params=list(PATHS))
+def launch_path(request, monkeypatch):
+    """Every case runs on each of the three launch forms of the recurrences (gpuqt_options)."""
+    from paper_1705_01387_b200 import binding
+    monkeypatch.setattr(binding, "DEFAULT_OPTIONS", dict(PATHS[request.param]))
+    return request.param
+
+
+def opts(**kw):
+    """The launch path of this test run plus explicit option overrides."""
+    from paper_1705_01387_b200 import binding
+    return {**binding.DEFAULT_OPTIONS, **kw}
 
 
 @pytest.fixture(scope="module")
@@ -261,10 +278,40 @@ def test_config_families_small(gq, oracle_mod, key):
     g.close()
 
 
-def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod, monkeypatch):
-    """The constant-hopping record variant (no hop array, padding col = -1) and the per-entry
-    variant (GPUQT_HOP_CONST=0) of the same model decode to the same table and give moments and
-    vectors within rounding of the oracle."""
+def test_deep_recurrences(gq, oracle_mod):
+    """Moment sets as deep as the benchmarked configs run them (N_m = 3000 / 2000 / 1000; dots[] indexed
+    deep into its buffer, late-moment drift) on the streaming kernels, all moments against the oracle:
+    c2's family (VAC, B = 1), c3's (MSD, B = 1, ragged rows), c4's (MSD, B = 4)."""
+    from workloads import configs
+    for key, nm in (("c2", 3000), ("c3", 2000), ("c4", 1000)):
+        w = configs.WORKLOADS[key]
+        model = configs.small_variant(key)
+        B = w.batch
+        phi = w.phases(model)
+        mg = gq.MODE_MSD if w.path == "msd" else gq.MODE_VAC
+        mo = oracle_mod.MODE_MSD if w.path == "msd" else oracle_mod.MODE_VAC
+        g, o = gq.GpuQT(model, batch=B, modes=mg, options=opts(small=0)), oracle_mod.Oracle(model, batch=B, modes=mo)
+        g.set_state(phi)
+        o.set_state(phi)
+        assert np.max(np.abs(g.dos_moments(nm) - o.dos_moments(nm))) / model.N <= TOL
+        g.evolve(w.dt, w.order)
+        o.evolve(w.dt, w.order)
+        if w.path == "vac":
+            va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+            scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(B)])
+            assert np.max(np.abs(g.vac(nm) - o.vac(nm)) / scale[:, None]) <= TOL
+        else:
+            chi = o.get_state(oracle_mod.CHI)
+            assert np.max(np.abs(g.msd(nm) - o.msd(nm)) / (norms(chi) ** 2)[:, None]) <= TOL
+        g.close()
+        o.close()
+
+
+def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod):
+    """The constant-hopping record variant (no hop array, padding col = N, the zero row) and the
+    per-entry variant (option hop_const = 0) of the same model decode to the same table and give
+    moments and vectors within rounding of the oracle."""
+    from paper_1705_01387_b200 import binding
     model = L.graphene(31, 19, W=0.5, seed=3, vacancy_fraction=0.2, vacancy_seed=9)   # many padded rows
     phi = L.random_phase_vectors(model.N, 4, config=58)
     o = oracle_mod.Oracle(model, batch=4, modes=oracle_mod.MODE_MSD | oracle_mod.MODE_VAC)
@@ -273,9 +320,9 @@ def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod, monkeypatch)
     ref_dos, ref_vac = o.dos_moments(40), o.vac(40)
     o.evolve(0.8, 45)
     ref_chi = o.get_state(oracle_mod.CHI)
-    for flag in ("1", "0"):
-        monkeypatch.setenv("GPUQT_HOP_CONST", flag)
-        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC)
+    for flag in (1, 0):
+        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC, options=opts(hop_const=flag))
+        assert g.info(binding.INFO_HOP_VARIANT) == (2 if flag else 0)
         for a, b in zip(g.get_table(), ref_tab):
             assert a.tobytes() == b.tobytes()
         g.set_state(phi)
@@ -286,46 +333,71 @@ def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod, monkeypatch)
         g.close()
 
 
-@pytest.mark.parametrize("env", [{"GPUQT_FUSE": "0"}, {"GPUQT_FUSE": "1", "GPUQT_RUN": "8", "GPUQT_LAG": "1"},
-                                 {"GPUQT_FUSE": "1", "GPUQT_BLOCKS_PER_SM": "1", "GPUQT_STAGES": "4"},
-                                 {"GPUQT_FUSE": "1", "GPUQT_ALTERNATE": "0", "GPUQT_RUN": "32", "GPUQT_LAG": "3"}],
-                         ids=["unfused", "fused_run8_lag1", "fused_1cta_4stages", "fused_noalt_run32"])
-def test_two_steps_per_launch(gq, oracle_mod, monkeypatch, env):
-    """Launches that perform two recurrence steps (second step trailing the first through L2, ordered
-    by the round counters) against single-step launches and the oracle, on lattices large enough
-    for many runs per CTA, every mode, odd and even term counts, periodic wrap-around dependencies."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+@pytest.mark.parametrize("o", [{"persistent": 0}, {"persistent": 1, "run": 8}, {"persistent": 1, "blocks_per_sm": 1, "stages": 4},
+                               {"persistent": 1, "alternate": 0, "run": 32, "stages": 1}],
+                         ids=["single_step", "multi_run8", "multi_1cta_4stages", "multi_noalt_run32_1stage"])
+def test_multi_step_launches(gq, oracle_mod, o):
+    """Whole recurrences in one cooperative launch (grid barrier between the steps, the stage ring and
+    the dot partials running on across them) against one launch per step and the oracle, on lattices
+    large enough for many runs per CTA: every mode, odd and even term counts, periodic wrap-around."""
+    from paper_1705_01387_b200 import binding
     for model, B in ((L.cubic(40, W=16.5, seed=4, energy_scale=16.0), 4),                    # 64000 rows, K = 6
                      (L.graphene(150, 101, vacancy_fraction=0.02, vacancy_seed=9), 1),       # ragged, B = 1
+                     (L.square(300, 211, W=2.0, seed=3), 1),                                 # two-slice tiles, odd tail
+                     (L.chain(50001, W=1.0, seed=8), 2),                                     # K = 2, B = 2
                      (L.square_peierls(240, 130, flux_quanta=5, W=1.5, seed=7), 8)):         # complex, B = 8
         phi = L.random_phase_vectors(model.N, B, config=59)
         modes = gq.MODE_VAC | gq.MODE_MSD
-        o = oracle_mod.Oracle(model, batch=B, modes=modes)
-        g = gq.GpuQT(model, batch=B, modes=modes)
-        o.set_state(phi)
+        o_ = oracle_mod.Oracle(model, batch=B, modes=modes)
+        g = gq.GpuQT(model, batch=B, modes=modes, options={"small": 0, **o})
+        assert g.info(binding.INFO_PERSISTENT) == o["persistent"]
+        o_.set_state(phi)
         g.set_state(phi)
         for nm in (37, 64):
-            assert np.max(np.abs(g.dos_moments(nm) - o.dos_moments(nm))) / model.N <= TOL
+            assert np.max(np.abs(g.dos_moments(nm) - o_.dos_moments(nm))) / model.N <= TOL
         for dt, order in ((0.7, 24), (0.35, 17)):
-            va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
-            scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(B)])
-            assert np.max(np.abs(g.vac(33) - o.vac(33)) / scale[:, None]) <= TOL
-            o.evolve(dt, order)
+            va, vb = o_.get_state(oracle_mod.VAC_A), o_.get_state(oracle_mod.VAC_B)
+            scale = np.array([np.linalg.norm(o_.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(B)])
+            assert np.max(np.abs(g.vac(33) - o_.vac(33)) / scale[:, None]) <= TOL
+            o_.evolve(dt, order)
             g.evolve(dt, order)
             for sg, so in ((gq.STATE_PSI, oracle_mod.PSI), (gq.STATE_CHI, oracle_mod.CHI),
                            (gq.STATE_VAC_A, oracle_mod.VAC_A), (gq.STATE_VAC_B, oracle_mod.VAC_B)):
-                assert vec_err(g.get_state(sg), o.get_state(so)) <= TOL
-            chi = o.get_state(oracle_mod.CHI)
-            assert np.max(np.abs(g.msd(30) - o.msd(30)) / (norms(chi) ** 2)[:, None]) <= TOL
+                assert vec_err(g.get_state(sg), o_.get_state(so)) <= TOL
+            chi = o_.get_state(oracle_mod.CHI)
+            assert np.max(np.abs(g.msd(30) - o_.msd(30)) / (norms(chi) ** 2)[:, None]) <= TOL
         g.close()
-        o.close()
+        o_.close()
 
 
-def test_16bit_columns_match_32bit(gq, oracle_mod, monkeypatch):
+def test_launch_counts(gq):
+    """The multi-step forms really are one launch per recurrence (gpuqt_kernel_stats)."""
+    from paper_1705_01387_b200 import binding
+    model = L.square(48, 40, W=2.0, seed=2)                  # 1920 orbitals: fits one SM's shared memory
+    phi = L.random_phase_vectors(model.N, 1, config=61)
+    for o, per_rec in (({"small": 0, "persistent": 1}, 1), ({"small": 1, "persistent": 0}, 1), ({"small": 0, "persistent": 0}, None)):
+        g = gq.GpuQT(model, batch=1, modes=gq.MODE_VAC, options=o)
+        g.set_state(phi)
+        g.reset_stats()
+        g.dos_moments(100)
+        g.vac(64)
+        g.evolve(0.5, 20)
+        ms, n = g.kernel_stats(binding.KERNEL_KPM_DOUBLING)
+        assert n == (per_rec or 50) and g.kernel_steps(binding.KERNEL_KPM_DOUBLING) == 50
+        ms, n = g.kernel_stats(binding.KERNEL_KPM_LEFT)
+        assert n == (per_rec or 63) and g.kernel_steps(binding.KERNEL_KPM_LEFT) == 63
+        ms, n = g.kernel_stats(binding.KERNEL_EVOLVE)          # two branches; + the scale launch each on the streaming forms
+        assert n == (2 if o["small"] else 4 if per_rec else 2 * 20) and g.kernel_steps(binding.KERNEL_EVOLVE) == 2 * 19
+        g.close()
+
+
+@pytest.mark.parametrize("model", [L.cubic(16, W=16.5, seed=16, energy_scale=16.0),
+                                   L.graphene(40, 24, vacancy_fraction=0.04, vacancy_seed=5)],     # padding entries: delta 0xffff
+                         ids=["cubic", "graphene_vacancies"])
+def test_16bit_columns_match_32bit(gq, oracle_mod, model):
     """The same table stored with 16-bit (base + delta) and with 32-bit columns decodes to the same
     canonical table and gives the same moments / vectors."""
-    model = L.cubic(16, W=16.5, seed=16, energy_scale=16.0)
+    from paper_1705_01387_b200 import binding
     phi = L.random_phase_vectors(model.N, 4, config=60)
     o = oracle_mod.Oracle(model, batch=4, modes=oracle_mod.MODE_MSD | oracle_mod.MODE_VAC)
     o.set_state(phi)
@@ -333,9 +405,9 @@ def test_16bit_columns_match_32bit(gq, oracle_mod, monkeypatch):
     o.evolve(1.0, 44)
     ref_chi = o.get_state(oracle_mod.CHI)
     outs = []
-    for flag in ("1", "0"):
-        monkeypatch.setenv("GPUQT_IDX16", flag)
-        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC)
+    for flag in (1, 0):
+        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC, options=opts(idx16=flag))
+        assert g.info(binding.INFO_HOP_VARIANT) == (3 if flag else 2)
         for a, b in zip(g.get_table(), ref_tab):
             assert a.tobytes() == b.tobytes()
         g.set_state(phi)

@@ -1,10 +1,13 @@
 """GPU parity of the post-processing step and of the paper's whole simulation loop:
-gpuqt_running_conductivity against the oracle, and transport.run on the CUDA library against the same
-loop driven through the oracle, on reduced-size versions of the paper's two examples
-(PAPER.md:359-409).  Tolerance: max |d| / max |ref| <= 1e-10 per output array (A22)."""
+gpuqt_running_conductivity against the oracle, and transport.run on the CUDA library against the
+test-side loop of tests/ref_loop.py driven through the oracle (no shared code: the row convention
+[A4], the averaging and the N_p rule [A5] are restated there), on reduced-size versions of the
+paper's two examples.  Tolerance: max |d| / max |ref| <= 1e-10 per output array
+(A22)."""
 import numpy as np
 import pytest
 
+from tests import ref_loop
 from workloads import configs
 
 pytestmark = pytest.mark.gpu
@@ -19,20 +22,6 @@ def gq():
         pytest.skip("no CUDA device")
     import paper_1705_01387_b200 as g
     return g
-
-
-class OracleEngine:
-    """The oracle behind the method names transport.run uses."""
-
-    def __init__(self, oracle_mod, model, batch, modes):
-        self.o = oracle_mod.Oracle(model, batch=batch, modes=modes)
-        self.mod = oracle_mod
-
-    def __getattr__(self, name):
-        return getattr(self.o, name)
-
-    def running_conductivity(self, kind, corr, dos, dt):
-        return self.mod.running_conductivity(kind, corr, dos, dt)
 
 
 def rel(a, b):
@@ -69,12 +58,12 @@ def test_paper_examples_reduced(gq, oracle_mod, key, scale):
     nm = 200
     phi = ex.phases(model)
     mg = (gq.MODE_VAC if ex.vac else 0) | (gq.MODE_MSD if ex.msd else 0)
-    mo = (oracle_mod.MODE_VAC if ex.vac else 0) | (oracle_mod.MODE_MSD if ex.msd else 0)
     order_of = lambda dt: binding.choose_order(model.energy_scale, dt)
+    for dt in set(dts):                                                 # the product's N_p rule against the oracle-side one
+        assert order_of(dt) == ref_loop.order_rule(oracle_mod, model.energy_scale, dt)
     g = gq.GpuQT(model, batch=ex.batch, modes=mg)
     got = transport.run(g, phi, dts, nm, ex.energies(), order_of, vac=ex.vac, msd=ex.msd)
-    ref = transport.run(OracleEngine(oracle_mod, model, ex.batch, mo), phi, dts, nm, ex.energies(), order_of,
-                        vac=ex.vac, msd=ex.msd)
+    ref = ref_loop.simulation_loop(oracle_mod, model, phi, dts, nm, ex.energies(), ex.vac, ex.msd)
     for name in ("dos", "rho_vac", "sigma_vac", "rho_msd", "sigma_msd"):
         if name in ref:
             assert rel(got[name], ref[name]) <= TOL, name
@@ -97,21 +86,19 @@ def test_paper_examples_reduced(gq, oracle_mod, key, scale):
 
 def test_file_front_end_matches_oracle(gq, oracle_mod, tmp_path):
     """The paper's workflow: a simulation folder run through the CUDA library writes
-    the same dos.out / vac.out / msd.out as the oracle driven through the identical front-end."""
+    the dos.out / vac.out / msd.out rows the oracle gives for the same model and vectors, each vector
+    run alone through tests/ref_loop.py (no product code on the expected side)."""
     from paper_1705_01387_b200 import frontend as F
     from workloads import lattices as L
     model = L.square(40, 32, W=4.0, seed=3, energy_scale=6.1)
     E = np.linspace(-6.0, 6.0, 121)
+    dts = [0.2, 0.2, 0.5, 1.0]
     para = {"calculate_vac": True, "calculate_msd": True, "number_of_random_vectors": 3, "number_of_moments": 128}
-    for name in ("gpu", "cpu"):
-        F.write_folder(str(tmp_path / name), model, E, [0.2, 0.2, 0.5, 1.0], para)
-
-    def make(mdl, b, vac, msd):
-        modes = (oracle_mod.MODE_VAC if vac else 0) | (oracle_mod.MODE_MSD if msd else 0)
-        return OracleEngine(oracle_mod, mdl, b, modes)
+    F.write_folder(str(tmp_path / "gpu"), model, E, dts, para)
     F.run_folder(str(tmp_path / "gpu"), seed=11)
-    F.run_folder(str(tmp_path / "cpu"), seed=11, make_engine=make)
-    for out, rows in (("dos.out", 3), ("vac.out", 12), ("msd.out", 12)):
-        a, b = np.loadtxt(tmp_path / "gpu" / out), np.loadtxt(tmp_path / "cpu" / out)
-        assert a.shape == b.shape == (rows, 121)
-        assert rel(a, b) <= TOL, out
+    phi = F.random_phase_vectors(model.N, 3, 11)                      # the front-end's input generator (no method arithmetic)
+    dos, vac, msd = ref_loop.per_vector_rows(oracle_mod, model, phi, dts, 128, E, True, True)
+    for out, ref in (("dos.out", dos), ("vac.out", vac.reshape(12, 121)), ("msd.out", msd.reshape(12, 121))):
+        a = np.loadtxt(tmp_path / "gpu" / out)
+        assert a.shape == ref.shape
+        assert rel(a, ref) <= TOL, out

@@ -17,7 +17,9 @@ class Workload:
     n_moments: int          # N_m ("KPM order")
     dt: float
     n_steps: int
-    order: int              # N_p Chebyshev terms per step
+    order: int              # N_p Chebyshev terms per step: given by BASELINE.json (c1, c2), else the smallest N_p with
+                            # |J_m(dE dt)| < 1e-15 for all m >= N_p [A5], evaluated once with scipy.special.jv at the
+                            # generated model's dE (c3: x = 20 -> 50, c4: x = 16 -> 44, c5: dE = 10.7, x = 10.7 -> 36)
     path: str               # "vac" or "msd"
     config_id: int
 
@@ -56,8 +58,8 @@ WORKLOADS = {
     "c4": Workload("c4", "simple-cubic Anderson 160^3 (4.096e6 orbitals), W=16.5, dE=16, N_m=1000, "
                    "MSD 40 steps dt=1, N_p=44, B=4", _c4, 4, 1000, 1.0, 40, 44, "msd", 4),
     "c5": Workload("c5", "graphene 2828x1414 four-atom cells (15995168 orbitals), Peierls flux 1e-4/hexagon, "
-                   "Gaussian-correlated potential, N_m=3000, VAC 30 steps dt=1, N_p=34..38 (tail rule), B=8",
-                   _c5, 8, 3000, 1.0, 30, 0, "vac", 5),
+                   "Gaussian-correlated potential, dE=10.7 eV, N_m=3000, VAC 30 steps dt=1, N_p=36 (tail rule), B=8",
+                   _c5, 8, 3000, 1.0, 30, 36, "vac", 5),
 }
 
 
