@@ -78,7 +78,7 @@ def energies_for(model):
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw")
 
     def __init__(self, index):
         self.index, self.rows, self.proc = index, [], None
@@ -106,8 +106,14 @@ class ClockSampler:
         mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i].startswith("Active") for r in self.rows)]
+        pw = []
+        for r in self.rows:
+            try:
+                pw.append(float(r[6]))
+            except (IndexError, ValueError):
+                pass
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+                "reasons": reasons, "samples": len(sm), "power_w": float(np.median(pw)) if pw else None}
 
 
 def load_peak():
@@ -329,7 +335,8 @@ def run_ours(args, w):
                 "config": {"workload": w.key, "description": w.description, "N": model.N, "K": model.K,
                            "batch_per_gpu": w.batch, "n_moments": w.n_moments, "order": order, "dt": w.dt,
                            "n_energies": N_ENERGIES, "path": w.path, "l2": l2_note,
-                           "storage": {"hop_variant": ["real", "complex", "constant, int32 columns", "constant, 16-bit columns"][info["HOP_VARIANT"]],
+                           "storage": {"hop_variant": ["real", "complex", "constant, int32 columns", "constant, 16-bit columns",
+                                                       "constant, 16-bit columns with padding"][info["HOP_VARIANT"]],
                                        "stored_matrix_bytes": info["STORED_MATRIX_BYTES"],
                                        "launch_form": "one-CTA whole-recurrence kernel" if info["SMALL_PATH"] else
                                                       "one cooperative launch per recurrence" if info["PERSISTENT"] else

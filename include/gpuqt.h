@@ -94,8 +94,8 @@ typedef enum {
  *   idx16          1: 16-bit (base + delta) columns where the table allows it
  *   small          1: one-CTA whole-recurrence kernel when matrix and vectors fit one SM's shared memory
  *   persistent     whole recurrences in ONE cooperative launch with grid-wide barriers between the
- *                  steps: 1 always, 0 never, -1 when a step is short enough for launch gaps to matter
- *                  (N * batch <= 32768 rows per SM)                                                   */
+ *                  steps: 1 always, 0 never, -1 when a whole recurrence is short enough to be one kernel
+ *                  (N * batch <= 131072 rows per SM: a step of at most a few hundred microseconds)    */
 typedef struct gpuqt_options {
     int32_t struct_bytes;
     int32_t stages;
@@ -233,12 +233,14 @@ int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c
 /* Facts about the handle (what the builder chose), for reports and tests.                          */
 #define GPUQT_INFO_STORED_MATRIX_BYTES 0   /* bytes of the packed records + the x array               */
 #define GPUQT_INFO_HOP_VARIANT 1           /* 0 real per entry, 1 complex per entry, 2 constant hopping
-                                              with int32 columns, 3 constant hopping with 16-bit columns */
+                                              with int32 columns, 3 constant hopping with 16-bit columns,
+                                              4 the same with padding entries (delta 0xffff = zero row) */
 #define GPUQT_INFO_UNIFORM 2               /* 1: every record has width K_max                          */
 #define GPUQT_INFO_UNROLLED_WIDTH 3        /* K_max when the unrolled walk is used (2, 3, 4, 6), else 0 */
 #define GPUQT_INFO_SMALL_PATH 4            /* 1: the one-CTA whole-recurrence kernel is in use         */
 #define GPUQT_INFO_PERSISTENT 5            /* 1: recurrences run as one cooperative multi-step launch  */
 #define GPUQT_INFO_WORKSPACE_USED 6        /* bytes of the workspace actually carved up                */
+#define GPUQT_INFO_SMALL_PATH_MSD 7        /* 1: the (psi, chi) time step is one launch of one CTA too    */
 int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value);
 
 /* Accumulated device time (CUDA events on the handle's stream around each run of launches) and

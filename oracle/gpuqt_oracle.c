@@ -451,14 +451,38 @@ int oracle_jackson(int32_t n_moments, double *g)
     return ORACLE_OK;
 }
 
+/* Other damping kernels of the kernel polynomial method (the paper's ref. [33]; the paper
+ * itself uses Jackson only -- SURVEY.md 8(f) 5):
+ *   kind 0  Jackson, Eq. 31
+ *   kind 1  Lorentz:  g_n = sinh(lambda (1 - n / N_m)) / sinh(lambda), lambda > 0
+ *           (turns delta(x - a) into a Lorentzian of half width lambda / N_m in the rescaled variable)
+ *   kind 2  none (Dirichlet):  g_n = 1, the plain truncated Chebyshev series                        */
+int oracle_damping(int kind, double lambda, int32_t n_moments, double *g)
+{
+    if (kind == 0) return oracle_jackson(n_moments, g);
+    if (kind == 1) {
+        if (!(lambda > 0.0)) return ORACLE_ERR_ARG;
+        for (int32_t n = 0; n < n_moments; ++n)
+            g[n] = sinh(lambda * (1.0 - (double)n / (double)n_moments)) / sinh(lambda);
+        return ORACLE_OK;
+    }
+    if (kind == 2) {
+        for (int32_t n = 0; n < n_moments; ++n) g[n] = 1.0;
+        return ORACLE_OK;
+    }
+    return ORACLE_ERR_ARG;
+}
+
 /* out[s][j] = 2 / (pi Omega dE sqrt(1 - E~^2)) sum_n g_n (2 - delta_n0) T_n(E~) C_n[s]
  * with E~ = E_j / dE and T_n(E~) = cos(n arccos E~).     PAPER.md:184-188 Eq. 25-27 [A15][A21] */
-int oracle_kpm_transform(const oracle_model *m, const double *moments, int32_t n_moments,
-                         int32_t n_sets, const double *energies, int32_t n_energies, double *out)
+int oracle_kpm_transform_damped(const oracle_model *m, int kind, double lambda, const double *moments,
+                                int32_t n_moments, int32_t n_sets, const double *energies,
+                                int32_t n_energies, double *out)
 {
     double *g = (double *)malloc((size_t)n_moments * sizeof(double));
     if (!g) return ORACLE_ERR_NOMEM;
-    oracle_jackson(n_moments, g);
+    int rc = oracle_damping(kind, lambda, n_moments, g);
+    if (rc != ORACLE_OK) { free(g); return rc; }
     for (int32_t j = 0; j < n_energies; ++j)
         if (!(fabs(energies[j] / m->dE) < 1.0)) { free(g); return ORACLE_ERR_ENERGY; }
 #pragma omp parallel for schedule(static)
@@ -475,6 +499,12 @@ int oracle_kpm_transform(const oracle_model *m, const double *moments, int32_t n
     }
     free(g);
     return ORACLE_OK;
+}
+
+int oracle_kpm_transform(const oracle_model *m, const double *moments, int32_t n_moments,
+                         int32_t n_sets, const double *energies, int32_t n_energies, double *out)
+{
+    return oracle_kpm_transform_damped(m, 0, 0.0, moments, n_moments, n_sets, energies, n_energies, out);
 }
 
 /* Running conductivity from the transformed correlation functions (units e = 1), Eq. 2,

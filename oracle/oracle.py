@@ -145,13 +145,15 @@ class Oracle:
     def vac(self, n):
         return self._moments(lib().oracle_vac, n)
 
-    def kpm_transform(self, moments, energies):
+    def kpm_transform(self, moments, energies, damping=0, lam=0.0):
+        """damping: 0 Jackson (Eq. 31), 1 Lorentz(lam), 2 none."""
         moments = np.ascontiguousarray(moments, np.float64)
         energies = np.ascontiguousarray(energies, np.float64)
         n_sets, n_m = moments.reshape(-1, moments.shape[-1]).shape
         out = np.empty((n_sets, energies.size), np.float64)
-        _check(lib().oracle_kpm_transform(self._h, _d(moments), C.c_int32(n_m), C.c_int32(n_sets),
-                                          _d(energies), C.c_int32(energies.size), _d(out)), "kpm_transform")
+        _check(lib().oracle_kpm_transform_damped(self._h, C.c_int(damping), C.c_double(lam), _d(moments), C.c_int32(n_m),
+                                                 C.c_int32(n_sets), _d(energies), C.c_int32(energies.size), _d(out)),
+               "kpm_transform")
         return out
 
 
@@ -164,6 +166,12 @@ def bessel_coeffs(dE, dt, order):
 def jackson(n):
     g = np.empty(n)
     _check(lib().oracle_jackson(C.c_int32(n), _d(g)), "jackson")
+    return g
+
+
+def damping(kind, lam, n):
+    g = np.empty(n)
+    _check(lib().oracle_damping(C.c_int(kind), C.c_double(lam), C.c_int32(n), _d(g)), "damping")
     return g
 
 

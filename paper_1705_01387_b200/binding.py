@@ -20,7 +20,7 @@ MAX_MOMENTS = 16384
 MAX_ORDER = 4096
 DAMPING_JACKSON, DAMPING_LORENTZ, DAMPING_NONE = 0, 1, 2
 (INFO_STORED_MATRIX_BYTES, INFO_HOP_VARIANT, INFO_UNIFORM, INFO_UNROLLED_WIDTH, INFO_SMALL_PATH, INFO_PERSISTENT,
- INFO_WORKSPACE_USED) = range(7)
+ INFO_WORKSPACE_USED, INFO_SMALL_PATH_MSD) = range(8)
 
 
 class Options(C.Structure):

@@ -45,6 +45,7 @@ struct gpuqt_handle {
     int rec_bytes = 0;                  // bytes reserved for the records of one tile inside a stage
     int want_stages = 2;                // requested pipeline depth per warp
     int persistent = 0;                 // whole recurrences as one cooperative launch
+    int alternate = 1;                  // the sweep direction alternates from step to step
     int coop_ok = 0;                    // the device supports cooperative launches
     // per launch configuration [mode]: stages, bytes per stage, dynamic smem
     int mode_stages[4] = {0};
@@ -198,7 +199,7 @@ int grid_for(gpuqt_handle* h, void* fn, size_t smem, long long work_items, int t
 // x_{m-2} (and e_{m-1}, e_{m-2} for the (a, e) pair)
 int mode_stage_bytes_for(const gpuqt_handle* h, int mode) {
     int streams = (mode == kModeEvolveMsd) ? 4 : 2;
-    if (h->B >= 8) streams /= 2;   // PrevDirect<8>: x_{m-2} rows are not staged
+    if (prev_direct(h->B, mode)) streams /= 2;   // x_{m-2} rows are not staged
     return h->rec_bytes + streams * tile_slices(h->B, h->kt) * 32 * h->B * (int)sizeof(double2);
 }
 
@@ -235,8 +236,8 @@ cudaError_t launch_steps(gpuqt_handle* h, int mode, RecArgs& a) {
     a.partials = h->partials;
     a.ticket = h->ticket;
     a.barrier = h->barrier;
-    a.alternate = h->opt.alternate;
-    a.sweep0 = h->opt.alternate ? (h->sweep & 1) : 0;
+    a.alternate = h->alternate;
+    a.sweep0 = h->alternate ? (h->sweep & 1) : 0;
     a.run = h->run;
     const int n = a.m_end - a.m_begin;
     h->sweep += n;
@@ -390,6 +391,9 @@ size_t small_smem_bytes(const gpuqt_handle* h) {
     return 4 * NB * sizeof(double2) + (size_t)h->N * 8 + KN * 8 * (size_t)hop_doubles(h->hop) + KN * 4 + 16;
 }
 bool small_ok(const gpuqt_handle* h) { return h->opt.small && small_smem_bytes(h) <= 210 * 1024; }
+// the (psi, chi) kernel keeps the x array in shared memory as well
+size_t small_msd_smem_bytes(const gpuqt_handle* h) { return small_smem_bytes(h) + (size_t)h->N * 8; }
+bool small_msd_ok(const gpuqt_handle* h) { return h->opt.small && small_msd_smem_bytes(h) <= 210 * 1024; }
 
 template <int MODE>
 void* small_fn(int B) {
@@ -400,11 +404,20 @@ void* small_fn(int B) {
     default: return (void*)cheb_small_kernel<8, MODE>;
     }
 }
+void* small_msd_fn(int B) {
+    switch (B) {
+    case 1: return (void*)cheb_small_msd_kernel<1>;
+    case 2: return (void*)cheb_small_msd_kernel<2>;
+    case 4: return (void*)cheb_small_msd_kernel<4>;
+    default: return (void*)cheb_small_msd_kernel<8>;
+    }
+}
 cudaError_t launch_small(gpuqt_handle* h, int mode, SmallArgs& a) {
     void* fn = mode == kModeDoubling ? small_fn<kModeDoubling>(h->B)
                : mode == kModeLeft   ? small_fn<kModeLeft>(h->B)
-                                     : small_fn<kModeEvolve>(h->B);
-    const size_t smem = small_smem_bytes(h);
+               : mode == kModeEvolve ? small_fn<kModeEvolve>(h->B)
+                                     : small_msd_fn(h->B);
+    const size_t smem = mode == kModeEvolveMsd ? small_msd_smem_bytes(h) : small_smem_bytes(h);
     cudaError_t e = ensure_dynamic_smem(fn, smem);
     if (e != cudaSuccess) return e;
     void* args[] = {(void*)&h->mat, (void*)&a};
@@ -473,11 +486,11 @@ int evolve_clenshaw(gpuqt_handle* h, int mode, int cls, const double2* in, const
     }
     const double* coef = nullptr;
     CU(upload_coefs(h, cr, ci, order, &coef));
-    if (!in_e && small_ok(h)) {
+    if (in_e ? small_msd_ok(h) : small_ok(h)) {
         SmallArgs a{};
-        a.aux = in; a.out = out; a.coef = (const double2*)coef; a.n_terms = order;
+        a.aux = in; a.aux_e = in_e; a.out = out; a.out_e = out_e; a.coef = (const double2*)coef; a.n_terms = order;
         StatScope s(h, cls);
-        CU(launch_small(h, kModeEvolve, a));
+        CU(launch_small(h, in_e ? kModeEvolveMsd : kModeEvolve, a));
         s.count(1, order - 1);
         return GPUQT_OK;
     }
@@ -684,7 +697,7 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell);
     // 16-bit columns: only where the unrolled uniform kernels exist
     if (opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, N);
-    h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : sell.idx16 ? kHopConst16 : kHopConst;
+    h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : sell.idx16 == 2 ? kHopConst16P : sell.idx16 ? kHopConst16 : kHopConst;
     h->kt = (sell.uniform && unrolled_width(K_max)) ? K_max : 0;
     // bytes reserved for the records of one tile inside a stage (keeps the vector rows 256-byte aligned)
     h->rec_bytes = (int)align_up((size_t)hop_record_bytes(K_max, h->hop) * tile_slices(batch, h->kt), 256);
@@ -741,7 +754,8 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     int stages = opt.stages ? opt.stages : (batch == 1 ? 4 : batch == 2 ? 3 : 2);
     h->want_stages = std::max(1, std::min(stages, kMaxStages));
     // whole recurrences in one cooperative launch when a step is so short that launch gaps matter
-    h->persistent = h->coop_ok && (opt.persistent == 1 || (opt.persistent == -1 && N * batch <= (int64_t)32768 * h->n_sm));
+    h->persistent = h->coop_ok && (opt.persistent == 1 || (opt.persistent == -1 && N * batch <= (int64_t)131072 * h->n_sm));
+    h->alternate = opt.alternate;
     // tiles per CTA run: 16 keeps a CTA on a contiguous band (the sweep front stays tight in L2); short sweeps
     // take the finest granularity for load balance
     const long long tiles = n_tiles_of(h);
@@ -971,6 +985,7 @@ int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value) {
     case GPUQT_INFO_SMALL_PATH: *value = small_ok(h) ? 1 : 0; break;
     case GPUQT_INFO_PERSISTENT: *value = h->persistent; break;
     case GPUQT_INFO_WORKSPACE_USED: *value = (int64_t)h->workspace_used; break;
+    case GPUQT_INFO_SMALL_PATH_MSD: *value = small_msd_ok(h) ? 1 : 0; break;
     default: return fail(h, GPUQT_ERR_ARG, "unknown info key");
     }
     return GPUQT_OK;

@@ -105,7 +105,7 @@ struct SellHost {
     int uniform = 1;                    // every record has width K_max
     int nd = 1;                         // doubles per entry: 0 constant hopping, 1 real, 2 complex
     double hop_const = 0.0;
-    int idx16 = 0;                      // constant hopping with 16-bit columns (see try_idx16)
+    int idx16 = 0;                      // constant hopping with 16-bit columns (see try_idx16): 1 plain, 2 with 0xffff padding entries
     int64_t n_slices_padded = 0;        // records stored: n_slices rounded up to a multiple of pad_to (all-padding records behind)
     std::vector<long long> slice_off;   // [n_slices_padded + 1] byte offsets of the records
     std::vector<unsigned char> rec;
@@ -246,6 +246,7 @@ inline bool try_idx16(SellHost& s, int K, int64_t N) {
     if (s.nd != 0 || !s.uniform || K > 8) return false;
     const size_t old_bytes = 256 + 128 * (size_t)K, new_bytes = 288 + 64 * (size_t)K;
     std::vector<unsigned char> out((size_t)s.n_slices_padded * new_bytes, 0);
+    bool any_pad = false;
     for (int64_t sl = 0; sl < s.n_slices_padded; ++sl) {
         const unsigned char* src = s.rec.data() + (size_t)sl * old_bytes;
         unsigned char* dst = out.data() + (size_t)sl * new_bytes;
@@ -261,18 +262,21 @@ inline bool try_idx16(SellHost& s, int K, int64_t N) {
                 lo = std::min<int64_t>(lo, c);
                 hi = std::max<int64_t>(hi, c);
             }
-            if (hi < 0) lo = 0;                                                // nothing but padding
+            if (hi < 0) lo = N;                                                // nothing but padding: base = N, delta = 0
             if (hi - lo > 65534) return false;                                 // 0xffff is reserved for the zero row
             base[k] = (int32_t)lo;
             for (int lane = 0; lane < 32; ++lane) {
                 const int32_t c = col[k * 32 + lane];
-                delta[k * 32 + lane] = c >= N ? (uint16_t)0xffffu : (uint16_t)(c - lo);
+                // a padding entry is an ordinary delta when the zero row is in reach, else the sentinel
+                const bool sentinel = c >= N && (int64_t)N - lo > 65534;
+                delta[k * 32 + lane] = sentinel ? (uint16_t)0xffffu : (uint16_t)(c - lo);
+                any_pad = any_pad || sentinel;
             }
         }
     }
     s.rec.swap(out);
     for (int64_t sl = 0; sl <= s.n_slices_padded; ++sl) s.slice_off[(size_t)sl] = (long long)((size_t)sl * new_bytes);
-    s.idx16 = 1;
+    s.idx16 = any_pad ? 2 : 1;
     return true;
 }
 }  // namespace gpuqt

@@ -42,8 +42,16 @@
 #ifndef GPUQT_MINB
 #define GPUQT_MINB 2
 #endif
+#ifndef GPUQT_MINB_B1
+#define GPUQT_MINB_B1 2
+#endif
+// (psi, chi) evolve kernel: 1 = two CTAs per SM (x_{m-2}, e_{m-2} rows by streaming loads instead of
+// staging, the neighbour gathers in two halves so that the walk fits 128 registers); 0 = one CTA per SM
+#ifndef GPUQT_MSD_OCC
+#define GPUQT_MSD_OCC 0
+#endif
 #ifndef GPUQT_MINB_MSD
-#define GPUQT_MINB_MSD 1
+#define GPUQT_MINB_MSD (GPUQT_MSD_OCC ? 2 : 1)
 #endif
 
 // L2 policy experiments
@@ -69,16 +77,18 @@ __host__ __device__ __forceinline__ long long record_bytes(int w, int nd) {
 __host__ __device__ __forceinline__ int record_width(long long bytes, int nd) {
     return (int)((bytes / 32 - 8) / (4 + 8 * nd));
 }
-// kHopConst16: constant hopping AND 16-bit columns -- the record is
+// kHopConst16 / kHopConst16P: constant hopping AND 16-bit columns -- the record is
 //     double onsite[32] | int32 base[8] (first w used) | uint16 delta[w][32]
-//     col = base[k] + delta[k][lane], or the zero row N when delta == 0xffff (padding entries)
+//     col = base[k] + delta[k][lane];  in the P variant delta == 0xffff stands for the zero row N
+//     (tables with padding entries: vacancies, open boundaries)
 // (uniform tables whose real columns spread less than 65535 inside every (slice, k); lattices in
 // natural order do).  288 + 64 w bytes instead of 256 + 128 w.
-enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2, kHopConst16 = 3 };
-__host__ __device__ constexpr bool hop_is_const(int hop) { return hop == kHopConst || hop == kHopConst16; }
+enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2, kHopConst16 = 3, kHopConst16P = 4 };
+__host__ __device__ constexpr bool hop_is_16(int hop) { return hop == kHopConst16 || hop == kHopConst16P; }
+__host__ __device__ constexpr bool hop_is_const(int hop) { return hop == kHopConst || hop_is_16(hop); }
 __host__ __device__ constexpr int hop_doubles(int hop) { return hop_is_const(hop) ? 0 : hop == kHopComplex ? 2 : 1; }
 __host__ __device__ __forceinline__ long long hop_record_bytes(int w, int hop) {
-    return hop == kHopConst16 ? 288LL + 64LL * w : record_bytes(w, hop_doubles(hop));
+    return hop_is_16(hop) ? 288LL + 64LL * w : record_bytes(w, hop_doubles(hop));
 }
 constexpr unsigned kPad16 = 0xffffu;     // 16-bit delta that stands for the zero row N
 
@@ -319,16 +329,23 @@ __device__ __forceinline__ void block_reduce_and_finish(double (&v)[Q * V], doub
 template <int MODE>
 struct ModeTraits {
     static constexpr int Q = (MODE == kModeDoubling) ? 3 : 2;
-    static constexpr int kMinBlocks = (MODE == kModeEvolveMsd) ? GPUQT_MINB_MSD : GPUQT_MINB;   // register cap
 };
+// resident CTAs per SM the register allocation aims at
+__host__ __device__ constexpr int min_blocks(int B, int mode) {
+    return mode == kModeEvolveMsd ? GPUQT_MINB_MSD : B == 1 ? GPUQT_MINB_B1 : GPUQT_MINB;
+}
 
 // B = 8: a slice's rows are 4 KB per stream; staging x_{m-2} as well would leave room for one CTA per
 // SM only, so x_{m-2} own rows are read by a streaming 256-bit load at the top of the round instead
 // (the occupancy is worth more than the TMA staging there; at B <= 4 it is the other way round).
-template <int B>
-struct PrevDirect {
-    static constexpr bool value = (B >= 8);
-};
+// The (psi, chi) evolve kernel does the same at every B when GPUQT_MSD_OCC is on (four staged streams
+// would leave room for one CTA per SM).
+#ifndef GPUQT_PREV_DIRECT     // experiment: x_{m-2} by streaming loads at every B
+#define GPUQT_PREV_DIRECT 0
+#endif
+__host__ __device__ constexpr bool prev_direct(int B, int mode) {
+    return B >= 8 || GPUQT_PREV_DIRECT || (GPUQT_MSD_OCC && mode == kModeEvolveMsd);
+}
 
 // A lane owns V consecutive vectors of a row (V = 2 when B >= 2: one 256-bit access per operand).
 // A tile is S consecutive slices and is walked in ROUNDS rounds of RS rows, U rounds at a time.
@@ -523,11 +540,12 @@ struct StepCtx {
 
 // Column of entry k of row rr of the slice whose record starts at s_col (int32 columns, or the base[8]
 // table of the 16-bit variant with the deltas behind it)
-template <bool IDX16>
+template <int HOP>
 __device__ __forceinline__ int col_of(const int* s_col, const unsigned short* s_d16, int k, int rr, int N) {
-    if (IDX16) {
+    if (hop_is_16(HOP)) {
         const unsigned d = s_d16[k * 32 + rr];
-        return d == kPad16 ? N : s_col[k] + (int)d;
+        if (HOP == kHopConst16P) return d == kPad16 ? N : s_col[k] + (int)d;
+        return s_col[k] + (int)d;
     }
     return s_col[k * 32 + rr];
 }
@@ -545,8 +563,8 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     constexpr int KU = KT > 0 ? KT : 1;
     constexpr int RB = B * 16;   // bytes of one row of a vector set
     constexpr bool MSD = (MODE == kModeEvolveMsd);
-    constexpr bool CPLX = (HOP == kHopComplex), CONST = hop_is_const(HOP), IDX16 = (HOP == kHopConst16);
-    constexpr int REC = KT > 0 ? (int)(HOP == kHopConst16 ? 288 + 64 * KT : 32 * (8 * KT * (CONST ? 0 : CPLX ? 2 : 1) + 8 + 4 * KT)) : 0;
+    constexpr bool CPLX = (HOP == kHopComplex), CONST = hop_is_const(HOP);
+    constexpr int REC = KT > 0 ? (int)(hop_is_16(HOP) ? 288 + 64 * KT : 32 * (8 * KT * (CONST ? 0 : CPLX ? 2 : 1) + 8 + 4 * KT)) : 0;
     const int rl = lane / LPR, l = lane % LPR;
     // staged vector rows: [in | (in_e) | prev | (prev_e)], each TR * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
@@ -558,7 +576,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     const uint32_t sl_in_e = smem_u32(s_in_e + l * V) - (uint32_t)row0 * (uint32_t)RB;
     const char* gl_in = reinterpret_cast<const char*>(io.in + l * V);
     const char* gl_in_e = reinterpret_cast<const char*>(io.in_e + l * V);
-    constexpr bool PD = PrevDirect<B>::value;
+    constexpr bool PD = prev_direct(B, MODE);
     const int N = (int)m.N;
 
     int r[U];                 // row inside the tile
@@ -575,7 +593,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
         r[u] = (j0 + u) * RS + rl;
         ok[u] = r[u] < rows_valid;
         vi[u] = (size_t)(row0 + (ok[u] ? r[u] : 0)) * B + l * V;
-        const unsigned char* rec = stage + (KT > 0 ? (r[u] >> 5) * REC : 0);
+        const unsigned char* rec = stage + (LS::S > 1 ? (r[u] >> 5) * REC : 0);
         s_hre[u] = reinterpret_cast<const double*>(rec);
         s_on[u] = s_hre[u] + w * 32 * hop_doubles(HOP);
         s_col[u] = reinterpret_cast<const int*>(s_on[u] + 32);                          // int32 columns, or base[8]
@@ -606,45 +624,56 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
 #pragma unroll
     for (int u = 0; u < U; ++u) sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
     if (KT > 0) {
-        // all gathers of the rows first (independent loads in flight), then the arithmetic
-        CV<V> v[U][KU], ve[U][MSD ? KU : 1];
-        double xn[U][MSD ? KU : 1];
+        // all gathers of the rows first (independent loads in flight), then the arithmetic; the (psi, chi)
+        // walk does it in two halves of the neighbour list when it has to fit 128 registers
+        constexpr int CH = (MSD && GPUQT_MSD_OCC) ? (KU + 1) / 2 : KU;
 #pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int rr = r[u] & 31;
+        for (int k0 = 0; k0 < KU; k0 += CH) {
+            CV<V> v[U][CH], ve[U][MSD ? CH : 1];
+            double xn[U][MSD ? CH : 1];
 #pragma unroll
-            for (int k = 0; k < KU; ++k) {
-                const int c = col_of<IDX16>(s_col[u], s_d16[u], k, rr, N);
-                v[u][k] = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
-                if (MSD) {
-                    ve[u][k] = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
-                    xn[u][k] = m.x[c];
+            for (int u = 0; u < U; ++u) {
+                const int rr = LS::S > 1 ? (r[u] & 31) : r[u];
+#pragma unroll
+                for (int kk = 0; kk < CH; ++kk) {
+                    const int k = k0 + kk;
+                    if (k < KU) {
+                        const int c = col_of<HOP>(s_col[u], s_d16[u], k, rr, N);
+                        v[u][kk] = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
+                        if (MSD) {
+                            ve[u][kk] = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
+                            xn[u][kk] = m.x[c];
+                        }
+                    }
                 }
             }
-        }
 #pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int rr = r[u] & 31;
+            for (int u = 0; u < U; ++u) {
+                const int rr = LS::S > 1 ? (r[u] & 31) : r[u];
 #pragma unroll
-            for (int k = 0; k < KU; ++k) {
-                double hr = 1.0, hi = 0.0;                                  // CONST: the factor is applied once below
-                if (!CONST) hr = s_hre[u][k * 32 + rr];
-                if (CPLX) hi = (s_hre[u] + w * 32)[k * 32 + rr];
-                if (CONST) cv_add<V>(sum[u], v[u][k]);
-                else cv_fma<V, CPLX>(sum[u], hr, hi, v[u][k]);
-                if (MSD) {
-                    if (CONST) cv_add<V>(sum_e[u], ve[u][k]);
-                    else cv_fma<V, CPLX>(sum_e[u], hr, hi, ve[u][k]);
-                    // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
-                    const double ndx = -min_image(xn[u][k] - xm[u], m.box);
-                    cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, v[u][k]);
+                for (int kk = 0; kk < CH; ++kk) {
+                    const int k = k0 + kk;
+                    if (k < KU) {
+                        double hr = 1.0, hi = 0.0;                              // CONST: the factor is applied once below
+                        if (!CONST) hr = s_hre[u][k * 32 + rr];
+                        if (CPLX) hi = (s_hre[u] + w * 32)[k * 32 + rr];
+                        if (CONST) cv_add<V>(sum[u], v[u][kk]);
+                        else cv_fma<V, CPLX>(sum[u], hr, hi, v[u][kk]);
+                        if (MSD) {
+                            if (CONST) cv_add<V>(sum_e[u], ve[u][kk]);
+                            else cv_fma<V, CPLX>(sum_e[u], hr, hi, ve[u][kk]);
+                            // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
+                            const double ndx = -min_image(xn[u][kk] - xm[u], m.box);
+                            cv_fma<V, CPLX>(sum_x[u], ndx * hr, ndx * hi, v[u][kk]);
+                        }
+                    }
                 }
             }
         }
     } else {
         const int rr = r[0] & 31;
         for (int k = 0; k < w; ++k) {
-            const int c = col_of<IDX16>(s_col[0], s_d16[0], k, rr, N);
+            const int c = col_of<HOP>(s_col[0], s_d16[0], k, rr, N);
             double hr = 1.0, hi = 0.0;
             if (!CONST) hr = s_hre[0][k * 32 + rr];
             if (CPLX) hi = (s_hre[0] + w * 32)[k * 32 + rr];
@@ -668,7 +697,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
             prev[u] = cv_lds_staged<V>(s_prev + si_);
             if (MSD) prev_e[u] = cv_lds_staged<V>(s_prev_e + si_);
         }
-        const double os = io.scale * s_on[u][r[u] & 31];                  // scale of the on-site term
+        const double os = io.scale * s_on[u][LS::S > 1 ? (r[u] & 31) : r[u]];   // scale of the on-site term
         CV<V> t, te;   // x_m (b_k) and e_m
 #pragma unroll
         for (int q = 0; q < V; ++q) {
@@ -764,7 +793,7 @@ __device__ __forceinline__ void block_partial(const double* s_part, int P, doubl
 // Between the steps of a multi-step (cooperative) launch: per-block dot partials, a grid barrier, and
 // block m % G sums the partials of step m in a fixed order while the others go on.
 template <int B, int KT, int HOP, int MODE>
-__global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_step_kernel(const Mat m, const RecArgs a) {
+__global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kernel(const Mat m, const RecArgs a) {
     using LS = LaneShape<B, KT>;
     constexpr int Q = ModeTraits<MODE>::Q;
     constexpr int V = LS::V, ROUNDS = LS::ROUNDS, U = LS::U, S = LS::S, TR = 32 * S;
@@ -813,8 +842,8 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
     uint32_t c_ph = 0;
     unsigned int epoch = 0;                               // grid barriers passed
 
-    for (int mm = a.m_begin; mm < a.m_end; ++mm) {
-        // ---- operands of step mm (CTA-uniform)
+    // operands of step mm (CTA-uniform)
+    auto make_ctx = [&](int mm) {
         StepCtx io;
         const int last_term = a.terms - 1;
         io.first = (mm == 1);
@@ -849,70 +878,87 @@ __global__ void __launch_bounds__(kThreads, ModeTraits<MODE>::kMinBlocks) cheb_s
             io.cr = a.coef[2 * (last_term - mm)];
             io.ci = a.coef[2 * (last_term - mm) + 1];
         }
-        const int reverse = a.alternate ? ((a.sweep0 + (mm - a.m_begin)) & 1) : a.sweep0;
+        return io;
+    };
+    // lane 0 only: every stream of tile t_virtual (sweep order) of the step `io` -> one stage, one mbarrier
+    auto issue = [&](const StepCtx& io, int reverse, int t_virtual, int st) {
+        const int t = reverse ? n_tiles - 1 - t_virtual : t_virtual;
+        const int s = t * S;                   // first slice of the tile
+        long long off;
+        uint32_t bytes;
+        if (KT > 0) {
+            bytes = (uint32_t)hop_record_bytes(KT, HOP) * S;        // the record array is padded to whole tiles
+            off = (long long)s * (long long)hop_record_bytes(KT, HOP);
+        } else {
+            off = m.slice_off[s];
+            bytes = (uint32_t)(m.slice_off[s + 1] - off);
+        }
+        const int left = N - s * 32;
+        const uint32_t vbytes = (uint32_t)((left < TR ? left : TR) * RB);
+        // x_{m-1} rows include the all-zero row N when it falls into this tile's window (the
+        // constant-hopping padding entries point at it)
+        const uint32_t vbytes_in = (uint32_t)((left + 1 < TR ? left + 1 : TR) * RB);
+        const bool with_prev = !io.first && !prev_direct(B, MODE);
+        unsigned char* dst = wstage + st * stage_bytes;
+        unsigned char* vdst = dst + a.rec_bytes;
+        if (B >= 2) {
+            // tensor copies: always the full 32-row box (rows past the end of the buffer are zero-filled)
+            const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
+            const int unit = s * 4 * B;           // first 128-byte line of the slice
+            mbar_expect_tx(&bars[st], total);
+            bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
+            tensor_g2s(vdst, io.tm_in, unit, &bars[st]);
+            if (MSD) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &bars[st]);
+            if (with_prev) {
+                tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &bars[st], policy);
+                if (MSD) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &bars[st], policy);
+            }
+        } else {
+            const uint32_t total = bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
+            const size_t voff = (size_t)s * 32 * B;
+            mbar_expect_tx(&bars[st], total);
+            bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
+            bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[st]);
+            if (MSD) bulk_g2s_nohint(vdst + TR * RB, io.in_e + voff, vbytes_in, &bars[st]);
+            if (with_prev) {
+                bulk_g2s(vdst + kPair * TR * RB, io.prev + voff, vbytes, &bars[st], policy);
+                if (MSD) bulk_g2s(vdst + 3 * TR * RB, io.prev_e + voff, vbytes, &bars[st], policy);
+            }
+        }
+    };
+    // producer cursor (lane 0): tile in sweep order, index inside the run
+    int p_t = 0, p_k = 0;
+    auto p_reset = [&]() {
+        p_t = (int)blockIdx.x * a.run + warp;
+        p_k = 0;
+    };
+    auto p_advance = [&]() {
+        if (++p_k == per) {
+            p_k = 0;
+            p_t += jump;
+        } else {
+            p_t += kWarps;
+        }
+        if (++p_st == stages) p_st = 0;
+    };
 
-        auto issue = [&](int t_virtual, int st) {   // lane 0 only: every stream of the tile -> one stage, one mbarrier
-            const int t = reverse ? n_tiles - 1 - t_virtual : t_virtual;
-            const int s = t * S;                   // first slice of the tile
-            long long off;
-            uint32_t bytes;
-            if (KT > 0) {
-                bytes = (uint32_t)hop_record_bytes(KT, HOP) * S;        // the record array is padded to whole tiles
-                off = (long long)s * (long long)hop_record_bytes(KT, HOP);
-            } else {
-                off = m.slice_off[s];
-                bytes = (uint32_t)(m.slice_off[s + 1] - off);
-            }
-            const int left = N - s * 32;
-            const uint32_t vbytes = (uint32_t)((left < TR ? left : TR) * RB);
-            // x_{m-1} rows include the all-zero row N when it falls into this tile's window (the
-            // constant-hopping padding entries point at it)
-            const uint32_t vbytes_in = (uint32_t)((left + 1 < TR ? left + 1 : TR) * RB);
-            const bool with_prev = !io.first && !PrevDirect<B>::value;
-            unsigned char* dst = wstage + st * stage_bytes;
-            unsigned char* vdst = dst + a.rec_bytes;
-            if (B >= 2) {
-                // tensor copies: always the full 32-row box (rows past the end of the buffer are zero-filled)
-                const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
-                const int unit = s * 4 * B;           // first 128-byte line of the slice
-                mbar_expect_tx(&bars[st], total);
-                bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
-                tensor_g2s(vdst, io.tm_in, unit, &bars[st]);
-                if (MSD) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &bars[st]);
-                if (with_prev) {
-                    tensor_g2s_hint(vdst + kPair * 512 * B, io.tm_prev, unit, &bars[st], policy);
-                    if (MSD) tensor_g2s_hint(vdst + 3 * 512 * B, io.tm_prev_e, unit, &bars[st], policy);
-                }
-            } else {
-                const uint32_t total = bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
-                const size_t voff = (size_t)s * 32 * B;
-                mbar_expect_tx(&bars[st], total);
-                bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
-                bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[st]);
-                if (MSD) bulk_g2s_nohint(vdst + TR * RB, io.in_e + voff, vbytes_in, &bars[st]);
-                if (with_prev) {
-                    bulk_g2s(vdst + kPair * TR * RB, io.prev + voff, vbytes, &bars[st], policy);
-                    if (MSD) bulk_g2s(vdst + 3 * TR * RB, io.prev_e + voff, vbytes, &bars[st], policy);
-                }
-            }
-        };
-        // position of a pipeline cursor inside the step: tile (sweep order), index inside the run
-        int p_t = (int)blockIdx.x * a.run + warp, p_k = 0;
-        int c_t = p_t, c_k = 0;
+    for (int mm = a.m_begin; mm < a.m_end; ++mm) {
+        const StepCtx io = make_ctx(mm);
+        const int reverse = a.alternate ? ((a.sweep0 + (mm - a.m_begin)) & 1) : a.sweep0;
+        int c_t = (int)blockIdx.x * a.run + warp, c_k = 0;      // consumer cursor
         int issued = 0;
         if (lane == 0) {
+            p_reset();
             for (; issued < stages - 1 && issued < n_my; ++issued) {
-                issue(p_t, p_st);
-                if (++p_k == per) { p_k = 0; p_t += jump; } else p_t += kWarps;
-                if (++p_st == stages) p_st = 0;
+                issue(io, reverse, p_t, p_st);
+                p_advance();
             }
         }
         for (int i = 0; i < n_my; ++i) {
             // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
             if (lane == 0 && issued < n_my) {
-                issue(p_t, p_st);
-                if (++p_k == per) { p_k = 0; p_t += jump; } else p_t += kWarps;
-                if (++p_st == stages) p_st = 0;
+                issue(io, reverse, p_t, p_st);
+                p_advance();
                 ++issued;
             }
             mbar_wait(&bars[c_st], c_ph);
@@ -972,10 +1018,11 @@ struct RecView {
     const unsigned short* d16;       // 16-bit variant: deltas, else nullptr
     int w;
     int N;
+    bool pad16;                      // 0xffff deltas stand for the zero row
     __device__ __forceinline__ int col_at(int k, int r) const {
         if (d16) {
             const unsigned d = d16[k * 32 + r];
-            return d == kPad16 ? N : col[k] + (int)d;
+            return (pad16 && d == kPad16) ? N : col[k] + (int)d;
         }
         return col[k * 32 + r];
     }
@@ -992,12 +1039,13 @@ __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
     }
     RecView v;
     v.N = (int)m.N;
-    v.w = m.hop == kHopConst16 ? m.K : record_width(bytes, nd);     // the 16-bit variant is always uniform
+    v.w = hop_is_16(m.hop) ? m.K : record_width(bytes, nd);         // the 16-bit variants are always uniform
+    v.pad16 = m.hop == kHopConst16P;
     v.hre = reinterpret_cast<const double*>(m.rec + off);
     v.him = v.hre + (size_t)v.w * 32;
     v.on = v.hre + (size_t)v.w * 32 * nd;
     v.col = reinterpret_cast<const int*>(v.on + 32);
-    v.d16 = m.hop == kHopConst16 ? reinterpret_cast<const unsigned short*>(v.col + 8) : nullptr;
+    v.d16 = hop_is_16(m.hop) ? reinterpret_cast<const unsigned short*>(v.col + 8) : nullptr;
     return v;
 }
 
@@ -1215,12 +1263,16 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
 //   MODE doubling : T_m from v0; dots {<T_m|T_m>, Re<T_m|T_{m-1}>, <T_{m-1}|T_{m-1}>} per term   (Eq. 28, 30)
 //   MODE left     : T_n from v0; dots <aux|T_n> (Re, Im) per term                                  (Eq. 29)
 //   MODE evolve   : out = sum_k c_k T_k(H~) aux by Clenshaw (v0 unused; coef[k] = c_k)             (Eq. 17)
+//   MODE evolve_msd: (out, out_e) = the same for the (psi, chi) pair with the block operator
+//                   [[H~, 0], [[X,H~], H~]] (Eq. 18, 22, 24), see cheb_small_msd_kernel below
 constexpr int kSmallThreads = 1024;
 
 struct SmallArgs {
     const double2* v0;      // doubling / left: T_0
-    const double2* aux;     // left: phi_L; evolve: the vector being evolved
+    const double2* aux;     // left: phi_L; evolve: the vector being evolved (psi)
+    const double2* aux_e;   // evolve_msd: chi
     double2* out;           // evolve: result
+    double2* out_e;         // evolve_msd: the new chi
     const double2* coef;    // evolve: c_k, k < n_terms
     double* dots;           // doubling: [term-1][3][B]; left: [term][2][B]
     int n_terms;            // doubling / left: terms m = 1 .. n_terms-1; evolve: order
@@ -1360,6 +1412,125 @@ __global__ void __launch_bounds__(kSmallThreads, 1) cheb_small_kernel(const Mat 
         }
         __syncthreads();
         cur = (cur + 1) % 3;
+    }
+}
+
+// The (psi, chi) time step of a small lattice in one launch of one CTA (PAPER.md:156 Eq. 18, :170 Eq. 22,
+// :176 Eq. 24; composition [A3]): Clenshaw recurrence of the pair
+//     b_k = c_k psi + 2 H~ b_{k+1} - b_{k+2}
+//     f_k = c_k chi + 2 H~ f_{k+1} - f_{k+2} + 2 [X,H~] b_{k+1},     [X,H~]_mn = (X_m - X_n) H_mn / dE
+// with b, f in shared memory.  x_m only needs x_{m-2} at its OWN element, so it overwrites it: two ring
+// slots per chain (4 N B double2 in all, as in cheb_small_kernel) and one __syncthreads() per term.  psi and
+// chi are read from global memory each term (L1/L2 hits).
+template <int B>
+__global__ void __launch_bounds__(kSmallThreads, 1) cheb_small_msd_kernel(const Mat m, const SmallArgs a) {
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    const int tid = threadIdx.x;
+    const int N = (int)m.N, K = m.K, NB = N * B;
+    const int nd = hop_doubles(m.hop);
+    double2* va = reinterpret_cast<double2*>(sm_raw);                   // b chain: 2 slots
+    double2* ve = va + 2 * (size_t)NB;                                  // f chain: 2 slots
+    double* on = reinterpret_cast<double*>(ve + 2 * (size_t)NB);
+    double* xs = on + N;
+    double* hre = xs + N;                                               // [K][N] if nd >= 1
+    double* him = hre + (nd >= 1 ? (size_t)K * N : 0);                  // [K][N] if nd == 2
+    int* col = reinterpret_cast<int*>(him + (nd == 2 ? (size_t)K * N : 0));   // [K][N]; -1 = no entry
+    for (int row = tid; row < N; row += kSmallThreads) {
+        const RecView rv = record_view(m, row >> 5);
+        const int r = row & 31;
+        on[row] = rv.on[r];
+        xs[row] = m.x[row];
+        for (int k = 0; k < K; ++k) {
+            int c = -1;
+            double hr = 0.0, hi = 0.0;
+            if (k < rv.w) {
+                c = rv.col_at(k, r);
+                if (hop_is_const(m.hop)) {
+                    hr = m.hop_const;
+                    if (c >= N) c = -1;                                 // padding entry (the zero row)
+                } else {
+                    hr = rv.hre[k * 32 + r];
+                    if (nd == 2) hi = rv.him[k * 32 + r];
+                    if (hr == 0.0 && hi == 0.0) c = -1;                 // padding entry (own row, weight 0)
+                }
+            }
+            col[k * N + row] = c;
+            if (nd >= 1) hre[k * N + row] = hr;
+            if (nd == 2) him[k * N + row] = hi;
+        }
+    }
+    const double2 c_last = a.coef[a.n_terms - 1];
+    for (int i = tid; i < NB; i += kSmallThreads) {
+        const double2 p = a.aux[i], q = a.aux_e[i];
+        va[i] = make_double2(c_last.x * p.x - c_last.y * p.y, c_last.x * p.y + c_last.y * p.x);
+        ve[i] = make_double2(c_last.x * q.x - c_last.y * q.y, c_last.x * q.y + c_last.y * q.x);
+    }
+    __syncthreads();
+    if (a.n_terms == 1) {
+        for (int i = tid; i < NB; i += kSmallThreads) {
+            a.out[i] = va[i];
+            a.out_e[i] = ve[i];
+        }
+        return;
+    }
+    int cur = 0;                     // slot of x_{m-1}; x_{m-2} sits in the other slot and is overwritten by x_m
+    for (int t = 1; t < a.n_terms; ++t) {
+        const double2* in = va + (size_t)cur * NB;
+        const double2* in_e = ve + (size_t)cur * NB;
+        double2* out = va + (size_t)(cur ^ 1) * NB;
+        double2* out_e = ve + (size_t)(cur ^ 1) * NB;
+        const bool first = (t == 1), half = (t == a.n_terms - 1);
+        const double scale = half ? m.inv_dE : 2.0 * m.inv_dE;
+        const double2 ck = a.coef[a.n_terms - 1 - t];
+        for (int i = tid; i < NB; i += kSmallThreads) {
+            const int row = i / B, b = i % B;
+            const double2 self = in[i], self_e = in_e[i];
+            const double xm = xs[row];
+            double sr = on[row] * self.x, si = on[row] * self.y;
+            double er = on[row] * self_e.x, ei = on[row] * self_e.y;
+            for (int k = 0; k < K; ++k) {
+                const int c = col[k * N + row];
+                if (c < 0) continue;
+                const double2 v = in[c * B + b], w = in_e[c * B + b];
+                const double hr = hop_is_const(m.hop) ? m.hop_const : hre[k * N + row];
+                const double ndx = -min_image(xs[c] - xm, m.box);       // [X,H]_mn = (X_m - X_n) H_mn
+                sr = fma(hr, v.x, sr);
+                si = fma(hr, v.y, si);
+                er = fma(hr, w.x, er);
+                ei = fma(hr, w.y, ei);
+                er = fma(ndx * hr, v.x, er);
+                ei = fma(ndx * hr, v.y, ei);
+                if (nd == 2) {
+                    const double hi = him[k * N + row];
+                    sr = fma(-hi, v.y, sr);
+                    si = fma(hi, v.x, si);
+                    er = fma(-hi, w.y, er);
+                    ei = fma(hi, w.x, ei);
+                    er = fma(-ndx * hi, v.y, er);
+                    ei = fma(ndx * hi, v.x, ei);
+                }
+            }
+            double2 ta = make_double2(scale * sr, scale * si), te = make_double2(scale * er, scale * ei);
+            if (!first) {
+                const double2 p = out[i], q = out_e[i];                 // x_{m-2}, own element only
+                ta.x -= p.x; ta.y -= p.y;
+                te.x -= q.x; te.y -= q.y;
+            }
+            const double2 s = a.aux[i], se = a.aux_e[i];
+            ta.x += ck.x * s.x - ck.y * s.y;
+            ta.y += ck.x * s.y + ck.y * s.x;
+            te.x += ck.x * se.x - ck.y * se.y;
+            te.y += ck.x * se.y + ck.y * se.x;
+            if (half) {
+                a.out[i] = ta;
+                a.out_e[i] = te;
+            } else {
+                out[i] = ta;
+                out_e[i] = te;
+            }
+        }
+        __syncthreads();
+        cur ^= 1;
     }
 }
 

@@ -183,6 +183,16 @@ def test_transform(gq, oracle_mod):
     with pytest.raises(gq.GpuqtError) as ei:
         g.kpm_transform(C, np.array([model.energy_scale]))
     assert ei.value.status == -5
+    # the other damping kernels: Lorentz(lambda), none; Jackson through the same entry point
+    for kind, lam in ((gq.DAMPING_JACKSON, 0.0), (gq.DAMPING_LORENTZ, 4.0), (gq.DAMPING_LORENTZ, 0.7), (gq.DAMPING_NONE, 0.0)):
+        ref = o.kpm_transform(C, E, damping=kind, lam=lam)
+        got = g.kpm_transform(C, E, damping=kind, lam=lam)
+        assert np.max(np.abs(got - ref)) / np.max(np.abs(ref)) <= TOL
+    assert np.array_equal(g.kpm_transform(C, E, damping=gq.DAMPING_JACKSON), g.kpm_transform(C, E))
+    for kind, lam in ((gq.DAMPING_LORENTZ, 0.0), (gq.DAMPING_LORENTZ, -1.0), (7, 1.0)):
+        with pytest.raises(gq.GpuqtError) as ei:
+            g.kpm_transform(C, E, damping=kind, lam=lam)
+        assert ei.value.status == -1
     g.close()
 
 
@@ -322,7 +332,7 @@ def test_constant_hopping_variant_matches_per_entry(gq, oracle_mod):
     ref_chi = o.get_state(oracle_mod.CHI)
     for flag in (1, 0):
         g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC, options=opts(hop_const=flag))
-        assert g.info(binding.INFO_HOP_VARIANT) == (2 if flag else 0)
+        assert g.info(binding.INFO_HOP_VARIANT) == (3 if flag else 0)      # constant hopping, 16-bit columns (zero row in reach) / per entry
         for a, b in zip(g.get_table(), ref_tab):
             assert a.tobytes() == b.tobytes()
         g.set_state(phi)
@@ -343,6 +353,7 @@ def test_multi_step_launches(gq, oracle_mod, o):
     from paper_1705_01387_b200 import binding
     for model, B in ((L.cubic(40, W=16.5, seed=4, energy_scale=16.0), 4),                    # 64000 rows, K = 6
                      (L.graphene(150, 101, vacancy_fraction=0.02, vacancy_seed=9), 1),       # ragged, B = 1
+                     (L.square(300, 230, W=1.0, seed=6, periodic=False), 1),                 # open edges: padding entries out of 16-bit reach
                      (L.square(300, 211, W=2.0, seed=3), 1),                                 # two-slice tiles, odd tail
                      (L.chain(50001, W=1.0, seed=8), 2),                                     # K = 2, B = 2
                      (L.square_peierls(240, 130, flux_quanta=5, W=1.5, seed=7), 8)):         # complex, B = 8
@@ -351,6 +362,8 @@ def test_multi_step_launches(gq, oracle_mod, o):
         o_ = oracle_mod.Oracle(model, batch=B, modes=modes)
         g = gq.GpuQT(model, batch=B, modes=modes, options={"small": 0, **o})
         assert g.info(binding.INFO_PERSISTENT) == o["persistent"]
+        if model.name.startswith("square") and model.box_length <= 0:
+            assert g.info(binding.INFO_HOP_VARIANT) == 4      # 16-bit columns with the 0xffff sentinel for the zero row
         o_.set_state(phi)
         g.set_state(phi)
         for nm in (37, 64):
@@ -388,6 +401,16 @@ def test_launch_counts(gq):
         assert n == (per_rec or 63) and g.kernel_steps(binding.KERNEL_KPM_LEFT) == 63
         ms, n = g.kernel_stats(binding.KERNEL_EVOLVE)          # two branches; + the scale launch each on the streaming forms
         assert n == (2 if o["small"] else 4 if per_rec else 2 * 20) and g.kernel_steps(binding.KERNEL_EVOLVE) == 2 * 19
+        g.close()
+        # the (psi, chi) time step (SURVEY 7 hard part 5): one launch on the one-CTA path too
+        g = gq.GpuQT(model, batch=1, modes=gq.MODE_MSD, options=o)
+        assert g.info(binding.INFO_SMALL_PATH_MSD) == o["small"]
+        g.set_state(phi)
+        g.reset_stats()
+        for _ in range(3):
+            g.evolve(0.5, 20)
+        ms, n = g.kernel_stats(binding.KERNEL_EVOLVE_MSD)      # + two scale launches per step on the streaming forms
+        assert n == 3 * (1 if o["small"] else 3 if per_rec else 2 + 19) and g.kernel_steps(binding.KERNEL_EVOLVE_MSD) == 3 * 19
         g.close()
 
 

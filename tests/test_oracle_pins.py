@@ -360,6 +360,54 @@ def test_transform_integral_and_chain_dos(oracle_mod):
     assert abs(out - 2 / (np.pi * model.volume * dE * np.sqrt(1 - e * e)) * g[2] * 2 * (2 * e * e - 1)) < 1e-15
 
 
+def test_other_damping_kernels(oracle_mod):
+    """Lorentz and undamped kernels (the paper's ref. [33]) pinned by what they DO, not by
+    their formula: (i) any kernel's damped moment g_k C_k is recovered exactly by the Chebyshev-Gauss
+    projection of the transformed density, which ties the transform to oracle_damping term by term and
+    fixes g_0 = 1 (norm conservation); (ii) the undamped series reproduces a polynomial density exactly;
+    (iii) the Lorentz kernel turns a single level delta(x - a) into the Lorentzian
+    (1/pi) eps / ((x - a)^2 + eps^2) with eps = lambda / N_m -- its defining property."""
+    model = L.chain(16, energy_scale=1.0)             # dE = 1 and Omega = 16: out = 2 / (16 pi sqrt(1 - x^2)) sum ...
+    o = oracle_mod.Oracle(model)
+    rng_ = np.random.default_rng(11)
+    nm, Kq = 40, 128
+    nodes = np.cos(np.pi * (np.arange(Kq) + 0.5) / Kq)
+    C = rng_.standard_normal((1, nm))
+    for kind, lam in ((0, 0.0), (1, 3.5), (2, 0.0)):
+        g = oracle_mod.damping(kind, lam, nm)
+        rho = o.kpm_transform(C, nodes, damping=kind, lam=lam)[0]
+        for k in (0, 1, 7, nm - 1):
+            proj = np.sum(rho * np.cos(k * np.arccos(nodes)) * np.sqrt(1 - nodes ** 2)) * np.pi / Kq
+            assert abs(proj - 2.0 / model.volume * g[k] * C[0, k]) < 1e-13        # int rho T_k dE = (2 / Omega) g_k C_k
+        assert g[0] == 1.0 and np.all(g <= 1.0) and np.all(g >= 0.0)
+    assert np.all(oracle_mod.damping(2, 0.0, nm) == 1.0)
+    assert np.array_equal(oracle_mod.damping(0, 0.0, nm), oracle_mod.jackson(nm))
+    gl = oracle_mod.damping(1, 4.0, 1000)
+    assert np.all(np.diff(gl) < 0) and abs(gl[500] - np.sinh(2.0) / np.sinh(4.0)) < 1e-15
+    with pytest.raises(RuntimeError):
+        oracle_mod.damping(1, 0.0, 8)
+    # (ii) density (1 + x) / (pi sqrt(1 - x^2)): moments mu_0 = 1, mu_1 = 1/2, the rest 0
+    mu = np.zeros((1, 12))
+    mu[0, 0], mu[0, 1] = 1.0, 0.5
+    x = np.linspace(-0.9, 0.9, 7)
+    rho = o.kpm_transform(mu, x, damping=2)[0] * model.volume / 2.0
+    assert np.allclose(rho, (1 + x) / (np.pi * np.sqrt(1 - x ** 2)), rtol=1e-14)
+    # (iii) one level at a: mu_n = T_n(a); Lorentz kernel -> half width eps = lambda / N_m in arccos x, i.e.
+    # eps sqrt(1 - a^2) in x; the kernel is exp(-lambda n / N_m) up to O(exp(-lambda)) corrections
+    a_, nm = 0.3, 4000
+    mu = np.cos(np.arange(nm) * np.arccos(a_))[None]
+    for lam, tol in ((4.0, 0.05), (6.0, 0.01)):
+        eps = lam / nm
+        w = eps * np.sqrt(1 - a_ ** 2)
+        x = a_ + w * np.array([-3.0, -1.0, -0.3, 0.0, 0.5, 2.0])
+        rho = o.kpm_transform(mu, x, damping=1, lam=lam)[0] * model.volume / 2.0
+        lorentz = w / (np.pi * ((x - a_) ** 2 + w ** 2))
+        assert np.max(np.abs(rho - lorentz) / lorentz) < tol
+    # while Jackson gives a Gaussian-like peak of width pi / N_m: much lower tails at 3 eps
+    jack = o.kpm_transform(mu, x, damping=0)[0] * model.volume / 2.0
+    assert jack[0] < 0.2 * rho[0]
+
+
 def test_transform_rejects_energy_outside_band(oracle_mod):
     model = L.chain(8)
     o = oracle_mod.Oracle(model)
