@@ -336,7 +336,8 @@ def run_ours(args, w):
                            "batch_per_gpu": w.batch, "n_moments": w.n_moments, "order": order, "dt": w.dt,
                            "n_energies": N_ENERGIES, "path": w.path, "l2": l2_note,
                            "storage": {"hop_variant": ["real", "complex", "constant, int32 columns", "constant, 16-bit columns",
-                                                       "constant, 16-bit columns with padding"][info["HOP_VARIANT"]],
+                                                       "constant, 16-bit columns with padding",
+                                                       "constant, implicit stencil (pattern dictionary, no index array)"][info["HOP_VARIANT"]],
                                        "stored_matrix_bytes": info["STORED_MATRIX_BYTES"],
                                        "launch_form": "one-CTA whole-recurrence kernel" if info["SMALL_PATH"] else
                                                       "one cooperative launch per recurrence" if info["PERSISTENT"] else

@@ -95,7 +95,14 @@ typedef enum {
  *   small          1: one-CTA whole-recurrence kernel when matrix and vectors fit one SM's shared memory
  *   persistent     whole recurrences in ONE cooperative launch with grid-wide barriers between the
  *                  steps: 1 always, 0 never, -1 when a whole recurrence is short enough to be one kernel
- *                  (N * batch <= 131072 rows per SM: a step of at most a few hundred microseconds)    */
+ *                  (N * batch <= 131072 rows per SM: a step of at most a few hundred microseconds)
+ *   stencil        implicit stencil for constant-hopping tables of regular lattices ("all
+ *                  hopping integrals ... are -1", the lattices of PAPER.md:359, :381): no index array is
+ *                  streamed; the distinct per-slice patterns of relative columns are kept in a small
+ *                  dictionary and a slice names its pattern.  1: when the dictionary is at most 1/16 of
+ *                  the index array (and <= 8 MB) AND a recurrence step's working set (three vector sets +
+ *                  the table) exceeds the L2 cache, i.e. when the index array would come from HBM in
+ *                  every step; 0: never; 2: whenever the table is uniform (tests)                      */
 typedef struct gpuqt_options {
     int32_t struct_bytes;
     int32_t stages;
@@ -106,6 +113,7 @@ typedef struct gpuqt_options {
     int32_t idx16;
     int32_t small;
     int32_t persistent;
+    int32_t stencil;
 } gpuqt_options;
 void gpuqt_default_options(gpuqt_options* opt);
 
@@ -120,6 +128,17 @@ size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t b
 int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index,
                    const double* hop_re, const double* hop_im, const double* onsite,
                    const double* x, double box_length, double energy_scale);
+
+/* Host only, no GPU: the storage variant gpuqt_create would choose for this table and batch under `options`
+ * (NULL = defaults) on a device with l2_bytes of L2 cache (0 = B200's 126 MB), and the bytes it takes on the
+ * device ("waste memory" is about exactly this).
+ * hop_variant as GPUQT_INFO_HOP_VARIANT, stored_matrix_bytes as
+ * GPUQT_INFO_STORED_MATRIX_BYTES, stencil_patterns as GPUQT_INFO_STENCIL_PATTERNS; any output may be NULL.
+ * Checks counts and index range only (GPUQT_ERR_INDEX); run gpuqt_validate for the full checks.     */
+int gpuqt_plan_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index,
+                       const double* hop_re, const double* hop_im, int32_t batch, int64_t l2_bytes,
+                       const gpuqt_options* options, int32_t* hop_variant, int64_t* stored_matrix_bytes,
+                       int64_t* stencil_patterns);
 
 /* Build the model on the GPU.
  *   nbr_count  host [N]          number of neighbours of site m
@@ -234,13 +253,15 @@ int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c
 #define GPUQT_INFO_STORED_MATRIX_BYTES 0   /* bytes of the packed records + the x array               */
 #define GPUQT_INFO_HOP_VARIANT 1           /* 0 real per entry, 1 complex per entry, 2 constant hopping
                                               with int32 columns, 3 constant hopping with 16-bit columns,
-                                              4 the same with padding entries (delta 0xffff = zero row) */
+                                              4 the same with padding entries (delta 0xffff = zero row),
+                                              5 constant hopping, implicit stencil (pattern dictionary)  */
 #define GPUQT_INFO_UNIFORM 2               /* 1: every record has width K_max                          */
 #define GPUQT_INFO_UNROLLED_WIDTH 3        /* K_max when the unrolled walk is used (2, 3, 4, 6), else 0 */
 #define GPUQT_INFO_SMALL_PATH 4            /* 1: the one-CTA whole-recurrence kernel is in use         */
 #define GPUQT_INFO_PERSISTENT 5            /* 1: recurrences run as one cooperative multi-step launch  */
 #define GPUQT_INFO_WORKSPACE_USED 6        /* bytes of the workspace actually carved up                */
 #define GPUQT_INFO_SMALL_PATH_MSD 7        /* 1: the (psi, chi) time step is one launch of one CTA too    */
+#define GPUQT_INFO_STENCIL_PATTERNS 8      /* patterns in the implicit-stencil dictionary (0: not in use)  */
 int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value);
 
 /* Accumulated device time (CUDA events on the handle's stream around each run of launches) and

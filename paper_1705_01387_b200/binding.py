@@ -20,13 +20,13 @@ MAX_MOMENTS = 16384
 MAX_ORDER = 4096
 DAMPING_JACKSON, DAMPING_LORENTZ, DAMPING_NONE = 0, 1, 2
 (INFO_STORED_MATRIX_BYTES, INFO_HOP_VARIANT, INFO_UNIFORM, INFO_UNROLLED_WIDTH, INFO_SMALL_PATH, INFO_PERSISTENT,
- INFO_WORKSPACE_USED, INFO_SMALL_PATH_MSD) = range(8)
+ INFO_WORKSPACE_USED, INFO_SMALL_PATH_MSD, INFO_STENCIL_PATTERNS) = range(9)
 
 
 class Options(C.Structure):
     """gpuqt_options (include/gpuqt.h)."""
     _fields_ = [(n, C.c_int32) for n in ("struct_bytes", "stages", "blocks_per_sm", "run", "alternate", "hop_const",
-                                          "idx16", "small", "persistent")]
+                                          "idx16", "small", "persistent", "stencil")]
 
 
 # overrides applied to every GpuQT() that does not pass its own `options` (the GPU tests run every
@@ -45,6 +45,8 @@ _SIGNATURES = {
     "gpuqt_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int32, C.c_int, C.c_int32, C.c_int]),
     "gpuqt_validate": (C.c_int, _model_args + [C.c_double]),
     "gpuqt_default_options": (None, [C.POINTER(Options)]),
+    "gpuqt_plan_storage": (C.c_int, [C.c_int64, C.c_int32, _ip, _ip, _dp, _dp, C.c_int32, C.c_int64, C.POINTER(Options),
+                                     C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
     "gpuqt_create": (C.c_int, [C.POINTER(C.c_void_p)] + _model_args + [C.c_double, C.c_double, C.c_int32, C.c_int,
                                                                        C.c_void_p, C.c_size_t, C.c_void_p]),
     "gpuqt_create_with_options": (C.c_int, [C.POINTER(C.c_void_p)] + _model_args + [
@@ -145,6 +147,17 @@ def default_options(**overrides) -> Options:
             raise KeyError(f"unknown gpuqt option {k!r}")
         setattr(o, k, int(v))
     return o
+
+
+def plan_storage(model, batch=1, options=None, l2_bytes=0):
+    """gpuqt_plan_storage (host only): (hop_variant, stored_matrix_bytes, stencil_patterns) gpuqt_create would choose."""
+    o = default_options(**(DEFAULT_OPTIONS if options is None else options))
+    hop, nbytes, pats = C.c_int32(), C.c_int64(), C.c_int64()
+    rc = load().gpuqt_plan_storage(model.N, model.K, _i(model.nbr_count), _i(model.nbr_index), _d(model.hop_re),
+                                   _d(model.hop_im), batch, l2_bytes, C.byref(o), C.byref(hop), C.byref(nbytes), C.byref(pats))
+    if rc != 0:
+        raise GpuqtError(rc, "gpuqt_plan_storage")
+    return hop.value, nbytes.value, pats.value
 
 
 class GpuQT:

@@ -57,6 +57,7 @@ struct gpuqt_handle {
     Mat mat{};
     size_t vec_elems = 0;   // N * B double2
     size_t stored_matrix_bytes = 0, workspace_used = 0;
+    int64_t stencil_patterns = 0;
     // vectors (device, inside the caller's workspace)
     double2 *psi = nullptr, *chi = nullptr, *va = nullptr, *vb = nullptr, *phiL = nullptr;
     double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr},
@@ -160,6 +161,32 @@ cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     if (e == cudaSuccess) g = bytes;
     return e;
+}
+
+// The storage variant of a table: packed sliced ELL; no hopping array when every
+// hopping is the same number; then the implicit stencil, else 16-bit columns, where the unrolled uniform
+// kernels exist.  Returns the Hop variant; `sell` (and `sten`) hold the records to upload.
+// The stencil saves HBM bytes and costs two more (small) TMA copies per slice: it is taken (option 1) only when
+// a recurrence step's working set -- three vector sets and the table -- does not fit the L2, i.e. when the
+// index array would really come from HBM every step (c2, 72 MB, is faster with the explicit array: 12.3 vs
+// 20.0 us per step; c4, 786 MB, is faster with the stencil: 156 vs 162 us).
+constexpr int64_t kB200L2Bytes = 126LL << 20;
+int choose_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index, const double* hop_re,
+                   const double* hop_im, const double* onsite, const gpuqt_options& opt, int batch, int64_t l2_bytes,
+                   SellHost& sell, StencilHost& sten) {
+    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell);
+    const int64_t working_set = 3 * (N + 1) * (int64_t)batch * 16 + (int64_t)sell.rec.size();
+    const bool want_stencil = opt.stencil == 2 || (opt.stencil == 1 && working_set > (l2_bytes > 0 ? l2_bytes : kB200L2Bytes));
+    const bool use_stencil = want_stencil && unrolled_width(K_max) && try_stencil(sell, K_max, N, opt.stencil == 2, sten);
+    if (!use_stencil && opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, N);
+    return sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : use_stencil ? kHopStencil
+           : sell.idx16 == 2 ? kHopConst16P : sell.idx16 ? kHopConst16 : kHopConst;
+}
+// bytes the table takes on the device: records (+ dictionary and pattern ids) + the x array
+size_t stored_bytes_of(int64_t N, int hop, const SellHost& sell, const StencilHost& sten) {
+    size_t rec = sell.rec.size();
+    if (hop == kHopStencil) rec = align_up(rec) + sten.dict.size() * sizeof(int32_t) + sten.pid.size() * sizeof(int32_t);
+    return rec + (size_t)(N + 1) * sizeof(double);
 }
 
 // ---------------------------------------------------------------- kernel dispatch
@@ -621,6 +648,7 @@ void gpuqt_default_options(gpuqt_options* o) {
     o->idx16 = 1;
     o->small = 1;
     o->persistent = -1;
+    o->stencil = 1;
 }
 
 size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes) {
@@ -635,6 +663,30 @@ int gpuqt_validate(int64_t N, int32_t K_max, const int32_t* nbr_count, const int
                    const double* x, double box_length, double energy_scale) {
     std::string msg;
     return validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
+}
+
+int gpuqt_plan_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index, const double* hop_re,
+                       const double* hop_im, int32_t batch, int64_t l2_bytes, const gpuqt_options* options,
+                       int32_t* hop_variant, int64_t* stored_matrix_bytes, int64_t* stencil_patterns) {
+    if (N <= 0 || K_max <= 0 || N > 0x7fffffffLL || !nbr_count || !nbr_index || !batch_ok(batch) || l2_bytes < 0) return GPUQT_ERR_ARG;
+    gpuqt_options opt;
+    gpuqt_default_options(&opt);
+    if (options) {
+        if (options->struct_bytes < (int32_t)sizeof(int32_t) || options->struct_bytes > (int32_t)sizeof(gpuqt_options)) return GPUQT_ERR_ARG;
+        std::memcpy(&opt, options, (size_t)options->struct_bytes);
+    }
+    for (int64_t m = 0; m < N; ++m) {
+        if (nbr_count[m] < 0 || nbr_count[m] > K_max) return GPUQT_ERR_INDEX;
+        for (int32_t k = 0; k < nbr_count[m]; ++k)
+            if (nbr_index[(size_t)m * K_max + k] < 0 || nbr_index[(size_t)m * K_max + k] >= N) return GPUQT_ERR_INDEX;
+    }
+    SellHost sell;
+    StencilHost sten;
+    const int hop = choose_storage(N, K_max, nbr_count, nbr_index, hop_re, hop_im, nullptr, opt, batch, l2_bytes, sell, sten);
+    if (hop_variant) *hop_variant = hop;
+    if (stored_matrix_bytes) *stored_matrix_bytes = (int64_t)stored_bytes_of(N, hop, sell, sten);
+    if (stencil_patterns) *stencil_patterns = hop == kHopStencil ? sten.n_patterns : 0;
+    return GPUQT_OK;
 }
 
 int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c_re, double* c_im) {
@@ -678,7 +730,8 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
         std::memcpy(&opt, options, (size_t)options->struct_bytes);     // an older, shorter struct keeps the newer defaults
         opt.struct_bytes = (int32_t)sizeof(gpuqt_options);
     }
-    if (opt.stages < 0 || opt.stages > kMaxStages || opt.blocks_per_sm < 0 || opt.run < 0 || opt.persistent < -1 || opt.persistent > 1)
+    if (opt.stages < 0 || opt.stages > kMaxStages || opt.blocks_per_sm < 0 || opt.run < 0 || opt.persistent < -1 || opt.persistent > 1 ||
+        opt.stencil < 0 || opt.stencil > 2)
         return bad(GPUQT_ERR_ARG, "option out of range");
     std::string msg;
     int rc = validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
@@ -694,25 +747,35 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     h->vec_elems = (size_t)N * batch;
 
     SellHost sell;
-    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell);
-    // 16-bit columns: only where the unrolled uniform kernels exist
-    if (opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, N);
-    h->hop = sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : sell.idx16 == 2 ? kHopConst16P : sell.idx16 ? kHopConst16 : kHopConst;
+    StencilHost sten;
+    int l2_bytes = 0;
+    {
+        int dev0 = 0;
+        if (cudaGetDevice(&dev0) != cudaSuccess || cudaDeviceGetAttribute(&l2_bytes, cudaDevAttrL2CacheSize, dev0) != cudaSuccess) {
+            (void)cudaGetLastError();
+            l2_bytes = 0;                   // no device: gpuqt_create fails below with GPUQT_ERR_CUDA
+        }
+    }
+    h->hop = choose_storage(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt, batch, l2_bytes, sell, sten);
+    const bool use_stencil = h->hop == kHopStencil;
+    h->stencil_patterns = use_stencil ? sten.n_patterns : 0;
     h->kt = (sell.uniform && unrolled_width(K_max)) ? K_max : 0;
-    // bytes reserved for the records of one tile inside a stage (keeps the vector rows 256-byte aligned)
-    h->rec_bytes = (int)align_up((size_t)hop_record_bytes(K_max, h->hop) * tile_slices(batch, h->kt), 256);
+    // bytes reserved for the record images of one tile inside a stage (keeps the vector rows 256-byte aligned)
+    h->rec_bytes = (int)align_up((size_t)hop_stage_bytes(K_max, h->hop) * tile_slices(batch, h->kt), 256);
     if (step_smem_bytes(1, mode_stage_bytes_for(h, kModeEvolveMsd)) > kSmemBudget) {
         delete h;
         return bad(GPUQT_ERR_ARG, "K_max = " + std::to_string(K_max) + " is too large: one slice record per warp must fit in shared memory");
     }
-    const size_t rec_bytes = sell.rec.size();
+    // the stencil dictionary lives behind the records
+    const size_t dict_off = align_up(sell.rec.size()), dict_bytes = sten.dict.size() * sizeof(int32_t);
+    const size_t rec_bytes = use_stencil ? dict_off + dict_bytes : sell.rec.size();
     const Layout L = make_layout(N, batch, modes, rec_bytes);
     if (L.total > workspace_bytes) {
         delete h;
         return bad(GPUQT_ERR_NOMEM, "workspace too small: " + std::to_string(L.total) + " bytes needed");
     }
     h->workspace_used = L.total;
-    h->stored_matrix_bytes = rec_bytes + (size_t)(N + 1) * sizeof(double);
+    h->stored_matrix_bytes = stored_bytes_of(N, h->hop, sell, sten);
     int dev = 0;
     cudaError_t ce = cudaGetDevice(&dev);
     if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -728,13 +791,17 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     auto up = [&](void* d, const void* s, size_t bytes) {
         return bytes ? cudaMemcpyAsync(d, s, bytes, cudaMemcpyHostToDevice, h->stream) : cudaSuccess;
     };
-    ce = up(d_rec, sell.rec.data(), rec_bytes);
+    ce = up(d_rec, sell.rec.data(), sell.rec.size());
+    if (ce == cudaSuccess && use_stencil) ce = up(d_rec + dict_off, sten.dict.data(), dict_bytes);
     if (ce == cudaSuccess) ce = up(d_x, x, (size_t)N * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMemsetAsync(d_x + N, 0, sizeof(double), h->stream);
     if (ce == cudaSuccess)
         ce = cudaMemsetAsync(base + L.vectors, 0, (size_t)n_vectors(modes) * align_up((size_t)(N + 1) * batch * sizeof(double2)),
                              h->stream);
-    if (ce == cudaSuccess) ce = up(d_sp, sell.slice_off.data(), sell.slice_off.size() * sizeof(long long));
+    // the slice_off slot holds the byte offsets of ragged tables, or the pattern ids of the stencil variant
+    if (ce == cudaSuccess)
+        ce = use_stencil ? up(d_sp, sten.pid.data(), sten.pid.size() * sizeof(int32_t))
+                         : up(d_sp, sell.slice_off.data(), sell.slice_off.size() * sizeof(long long));
     if (ce == cudaSuccess) ce = cudaMemsetAsync(base + L.ticket, 0, 256, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
     if (ce == cudaSuccess) ce = cudaMallocHost((void**)&h->coef_host, (size_t)kCoefSlots * 2 * GPUQT_MAX_ORDER * sizeof(double));
@@ -749,6 +816,8 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     h->mat.N = N; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
     h->mat.cplx = h->cplx; h->mat.hop = h->hop; h->mat.hop_const = sell.hop_const;
     h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
+    h->mat.pid = use_stencil ? (const int*)d_sp : nullptr;
+    h->mat.dict = use_stencil ? (const int*)(d_rec + dict_off) : nullptr;
     // Shared-memory stages per warp: one round of a tile takes about one memory latency and a slice has
     // `batch / 2` rounds, so small batches need a deeper prefetch.
     int stages = opt.stages ? opt.stages : (batch == 1 ? 4 : batch == 2 ? 3 : 2);
@@ -986,6 +1055,7 @@ int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value) {
     case GPUQT_INFO_PERSISTENT: *value = h->persistent; break;
     case GPUQT_INFO_WORKSPACE_USED: *value = (int64_t)h->workspace_used; break;
     case GPUQT_INFO_SMALL_PATH_MSD: *value = small_msd_ok(h) ? 1 : 0; break;
+    case GPUQT_INFO_STENCIL_PATTERNS: *value = h->stencil_patterns; break;
     default: return fail(h, GPUQT_ERR_ARG, "unknown info key");
     }
     return GPUQT_OK;

@@ -7,6 +7,7 @@
 #include <cstdint>
 #include <cstring>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/gpuqt.h"
@@ -277,6 +278,53 @@ inline bool try_idx16(SellHost& s, int K, int64_t N) {
     s.rec.swap(out);
     for (int64_t sl = 0; sl <= s.n_slices_padded; ++sl) s.slice_off[(size_t)sl] = (long long)((size_t)sl * new_bytes);
     s.idx16 = any_pad ? 2 : 1;
+    return true;
+}
+}  // namespace gpuqt
+
+namespace gpuqt {
+// Implicit stencil (kHopStencil in kernels.cuh): re-encode a uniform constant-hopping table
+// (records: onsite[32] | int32 col[K][32]) as  record = onsite[32],  pid[slice],  dict[pattern][K][32]  with
+// dict = the distinct arrays  rel[k][lane] = col - 32 slice  of the table.  On a regular lattice in natural
+// order the relative columns repeat from slice to slice and differ only where a periodic wrap falls into
+// the slice, so a few hundred patterns describe millions of rows; vacancies, open edges in the bulk or a
+// shuffled numbering make every slice its own pattern and the table is left as it is (returns false).
+//   force = false: only when the dictionary is at most 1/16 of the index array it replaces (and <= 8 MB,
+//                  so that it stays L2 resident);  force = true: whenever the table is uniform (tests).
+struct StencilHost {
+    std::vector<int32_t> pid;           // [n_slices_padded]
+    std::vector<int32_t> dict;          // [n_patterns][K][32]
+    int64_t n_patterns = 0;
+};
+inline bool try_stencil(SellHost& s, int K, int64_t N, bool force, StencilHost& st) {
+    (void)N;
+    if (s.nd != 0 || !s.uniform || s.idx16) return false;
+    const size_t old_bytes = 256 + 128 * (size_t)K, pat = (size_t)K * 32;
+    const size_t index_bytes = (size_t)s.n_slices_padded * pat * 4;
+    size_t max_patterns = (size_t)s.n_slices_padded;
+    if (!force) max_patterns = std::min<size_t>(index_bytes / 16, (size_t)8 << 20) / (pat * 4);
+    std::unordered_map<std::string, int32_t> seen;
+    std::vector<int32_t> rel(pat);
+    st.pid.assign((size_t)s.n_slices_padded, 0);
+    st.dict.clear();
+    for (int64_t sl = 0; sl < s.n_slices_padded; ++sl) {
+        const int32_t* col = reinterpret_cast<const int32_t*>(s.rec.data() + (size_t)sl * old_bytes + 256);
+        for (size_t e = 0; e < pat; ++e) rel[e] = (int32_t)((int64_t)col[e] - sl * 32);
+        std::string key(reinterpret_cast<const char*>(rel.data()), pat * 4);
+        auto it = seen.find(key);
+        if (it == seen.end()) {
+            if (seen.size() >= max_patterns) return false;
+            it = seen.emplace(std::move(key), (int32_t)seen.size()).first;
+            st.dict.insert(st.dict.end(), rel.begin(), rel.end());
+        }
+        st.pid[(size_t)sl] = it->second;
+    }
+    st.n_patterns = (int64_t)seen.size();
+    std::vector<unsigned char> out((size_t)s.n_slices_padded * 256);
+    for (int64_t sl = 0; sl < s.n_slices_padded; ++sl)
+        std::memcpy(out.data() + (size_t)sl * 256, s.rec.data() + (size_t)sl * old_bytes, 256);      // onsite
+    s.rec.swap(out);
+    for (int64_t sl = 0; sl <= s.n_slices_padded; ++sl) s.slice_off[(size_t)sl] = (long long)sl * 256;
     return true;
 }
 }  // namespace gpuqt

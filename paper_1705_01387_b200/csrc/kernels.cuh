@@ -83,12 +83,26 @@ __host__ __device__ __forceinline__ int record_width(long long bytes, int nd) {
 //     (tables with padding entries: vacancies, open boundaries)
 // (uniform tables whose real columns spread less than 65535 inside every (slice, k); lattices in
 // natural order do).  288 + 64 w bytes instead of 256 + 128 w.
-enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2, kHopConst16 = 3, kHopConst16P = 4 };
+// kHopStencil: constant hopping on a REGULAR lattice -- no index array is streamed at all (SURVEY 8(f) 3,
+// "implicit stencil"; the paper's own examples are such lattices).  The columns of a
+// slice RELATIVE to its first row, rel[k][lane] = col - 32 s, repeat from slice to slice on a regular lattice
+// (they differ only where a periodic wrap falls inside the slice), so the table is stored as
+//     record  s : double onsite[32]                         (256 bytes, streamed from HBM)
+//     pid[s]    : int32 index of the slice's pattern        (4 bytes per slice)
+//     dict[p]   : int32 rel[K][32]                          (a few hundred distinct patterns at most: L2 resident)
+// and a stage of the pipeline is filled by two bulk copies per slice (record from HBM, pattern from L2) to the
+// same image the kHopConst walk reads: onsite[32] | int32 rel[K][32];  col = 32 s + rel.
+enum Hop : int { kHopReal = 0, kHopComplex = 1, kHopConst = 2, kHopConst16 = 3, kHopConst16P = 4, kHopStencil = 5 };
 __host__ __device__ constexpr bool hop_is_16(int hop) { return hop == kHopConst16 || hop == kHopConst16P; }
-__host__ __device__ constexpr bool hop_is_const(int hop) { return hop == kHopConst || hop_is_16(hop); }
+__host__ __device__ constexpr bool hop_is_const(int hop) { return hop == kHopConst || hop_is_16(hop) || hop == kHopStencil; }
 __host__ __device__ constexpr int hop_doubles(int hop) { return hop_is_const(hop) ? 0 : hop == kHopComplex ? 2 : 1; }
+// bytes of one slice record as stored (and streamed from HBM)
 __host__ __device__ __forceinline__ long long hop_record_bytes(int w, int hop) {
-    return hop_is_16(hop) ? 288LL + 64LL * w : record_bytes(w, hop_doubles(hop));
+    return hop == kHopStencil ? 256LL : hop_is_16(hop) ? 288LL + 64LL * w : record_bytes(w, hop_doubles(hop));
+}
+// bytes one slice's record image takes inside a pipeline stage (kHopStencil: record + pattern)
+__host__ __device__ __forceinline__ long long hop_stage_bytes(int w, int hop) {
+    return hop == kHopStencil ? 256LL + 128LL * w : hop_record_bytes(w, hop);
 }
 constexpr unsigned kPad16 = 0xffffu;     // 16-bit delta that stands for the zero row N
 
@@ -96,6 +110,8 @@ struct Mat {
     const unsigned char* __restrict__ rec;      // packed slice records
     const long long* __restrict__ slice_off;    // [n_slices_padded + 1] byte offsets (ragged variant)
     const double* __restrict__ x;               // [N + 1], x[N] = 0
+    const int* __restrict__ pid;                // kHopStencil: [n_slices_padded] pattern of each slice
+    const int* __restrict__ dict;               // kHopStencil: [n_patterns][K][32] columns relative to the slice's first row
     long long N;
     long long n_slices;                         // real slices, ceil(N / 32)
     int K;                                      // K_max
@@ -564,7 +580,9 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     constexpr int RB = B * 16;   // bytes of one row of a vector set
     constexpr bool MSD = (MODE == kModeEvolveMsd);
     constexpr bool CPLX = (HOP == kHopComplex), CONST = hop_is_const(HOP);
-    constexpr int REC = KT > 0 ? (int)(hop_is_16(HOP) ? 288 + 64 * KT : 32 * (8 * KT * (CONST ? 0 : CPLX ? 2 : 1) + 8 + 4 * KT)) : 0;
+    constexpr bool STENCIL = (HOP == kHopStencil);
+    constexpr int REC = KT > 0 ? (int)(STENCIL ? 256 + 128 * KT : hop_is_16(HOP) ? 288 + 64 * KT
+                                                : 32 * (8 * KT * (CONST ? 0 : CPLX ? 2 : 1) + 8 + 4 * KT)) : 0;
     const int rl = lane / LPR, l = lane % LPR;
     // staged vector rows: [in | (in_e) | prev | (prev_e)], each TR * B double2
     const double2* s_in = reinterpret_cast<const double2*>(stage + a.rec_bytes);
@@ -584,6 +602,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     size_t vi[U];             // element in global memory
     const double* s_hre[U];
     const double* s_on[U];
+    int srow0[U];             // kHopStencil: first row of the row's slice (the columns are relative to it)
     const int* s_col[U];
     const unsigned short* s_d16[U];
     CV<V> other[U], other_e[U], prev[U], prev_e[U], self[U], self_e[U];
@@ -594,6 +613,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
         ok[u] = r[u] < rows_valid;
         vi[u] = (size_t)(row0 + (ok[u] ? r[u] : 0)) * B + l * V;
         const unsigned char* rec = stage + (LS::S > 1 ? (r[u] >> 5) * REC : 0);
+        srow0[u] = STENCIL ? row0 + (LS::S > 1 ? (r[u] & ~31) : 0) : 0;
         s_hre[u] = reinterpret_cast<const double*>(rec);
         s_on[u] = s_hre[u] + w * 32 * hop_doubles(HOP);
         s_col[u] = reinterpret_cast<const int*>(s_on[u] + 32);                          // int32 columns, or base[8]
@@ -638,7 +658,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
                 for (int kk = 0; kk < CH; ++kk) {
                     const int k = k0 + kk;
                     if (k < KU) {
-                        const int c = col_of<HOP>(s_col[u], s_d16[u], k, rr, N);
+                        const int c = col_of<HOP>(s_col[u], s_d16[u], k, rr, N) + srow0[u];
                         v[u][kk] = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
                         if (MSD) {
                             ve[u][kk] = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
@@ -673,7 +693,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     } else {
         const int rr = r[0] & 31;
         for (int k = 0; k < w; ++k) {
-            const int c = col_of<HOP>(s_col[0], s_d16[0], k, rr, N);
+            const int c = col_of<HOP>(s_col[0], s_d16[0], k, rr, N) + srow0[0];
             double hr = 1.0, hi = 0.0;
             if (!CONST) hr = s_hre[0][k * 32 + rr];
             if (CPLX) hi = (s_hre[0] + w * 32)[k * 32 + rr];
@@ -800,6 +820,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
     constexpr int RB = B * 16, QB = Q * B;
     constexpr bool DOTS = (MODE == kModeDoubling || MODE == kModeLeft);
     constexpr bool MSD = (MODE == kModeEvolveMsd);
+    constexpr bool STENCIL = (HOP == kHopStencil);
     constexpr int kPair = MSD ? 2 : 1;
     __shared__ double s_part[DOTS ? kWarps * QB : 1];
     __shared__ int s_last;
@@ -880,6 +901,23 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         }
         return io;
     };
+    int pp[S];                                 // kHopStencil, lane 0: patterns of the tile the producer cursor points at
+#pragma unroll
+    for (int j = 0; j < S; ++j) pp[j] = 0;
+    // the record image of a tile -> dst: one bulk copy, or (kHopStencil) per slice the on-site record from HBM
+    // and the slice's pattern from the dictionary
+    auto copy_records = [&](unsigned char* dst, long long off, uint32_t bytes, uint64_t* bar) {
+        if (STENCIL) {
+#pragma unroll
+            for (int j = 0; j < S; ++j) {
+                unsigned char* d = dst + j * (256 + 128 * KT);
+                bulk_g2s(d, m.rec + off + 256 * j, 256u, bar, policy);
+                bulk_g2s_nohint(d + 256, m.dict + (size_t)pp[j] * (KT * 32), (uint32_t)(128 * KT), bar);
+            }
+        } else {
+            bulk_g2s(dst, m.rec + off, bytes, bar, policy);
+        }
+    };
     // lane 0 only: every stream of tile t_virtual (sweep order) of the step `io` -> one stage, one mbarrier
     auto issue = [&](const StepCtx& io, int reverse, int t_virtual, int st) {
         const int t = reverse ? n_tiles - 1 - t_virtual : t_virtual;
@@ -887,7 +925,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         long long off;
         uint32_t bytes;
         if (KT > 0) {
-            bytes = (uint32_t)hop_record_bytes(KT, HOP) * S;        // the record array is padded to whole tiles
+            bytes = (uint32_t)hop_stage_bytes(KT, HOP) * S;         // the record array is padded to whole tiles
             off = (long long)s * (long long)hop_record_bytes(KT, HOP);
         } else {
             off = m.slice_off[s];
@@ -906,7 +944,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
             const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
             const int unit = s * 4 * B;           // first 128-byte line of the slice
             mbar_expect_tx(&bars[st], total);
-            bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
+            copy_records(dst, off, bytes, &bars[st]);
             tensor_g2s(vdst, io.tm_in, unit, &bars[st]);
             if (MSD) tensor_g2s(vdst + 512 * B, io.tm_in_e, unit, &bars[st]);
             if (with_prev) {
@@ -917,7 +955,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
             const uint32_t total = bytes + vbytes_in * kPair + (with_prev ? vbytes * kPair : 0u);
             const size_t voff = (size_t)s * 32 * B;
             mbar_expect_tx(&bars[st], total);
-            bulk_g2s(dst, m.rec + off, bytes, &bars[st], policy);
+            copy_records(dst, off, bytes, &bars[st]);
             bulk_g2s_nohint(vdst, io.in + voff, vbytes_in, &bars[st]);
             if (MSD) bulk_g2s_nohint(vdst + TR * RB, io.in_e + voff, vbytes_in, &bars[st]);
             if (with_prev) {
@@ -928,9 +966,21 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
     };
     // producer cursor (lane 0): tile in sweep order, index inside the run
     int p_t = 0, p_k = 0;
-    auto p_reset = [&]() {
+    int p_reverse = 0;                         // sweep direction of the step being issued
+    auto p_patterns = [&]() {                  // kHopStencil: pattern ids of the tile at the cursor, one tile ahead of their use
+        if (STENCIL) {
+            const int t = p_reverse ? n_tiles - 1 - p_t : p_t;
+            if (t >= 0 && t < n_tiles) {
+#pragma unroll
+                for (int j = 0; j < S; ++j) pp[j] = __ldg(&m.pid[t * S + j]);
+            }
+        }
+    };
+    auto p_reset = [&](int reverse) {
         p_t = (int)blockIdx.x * a.run + warp;
         p_k = 0;
+        p_reverse = reverse;
+        p_patterns();
     };
     auto p_advance = [&]() {
         if (++p_k == per) {
@@ -940,6 +990,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
             p_t += kWarps;
         }
         if (++p_st == stages) p_st = 0;
+        p_patterns();
     };
 
     for (int mm = a.m_begin; mm < a.m_end; ++mm) {
@@ -948,7 +999,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         int c_t = (int)blockIdx.x * a.run + warp, c_k = 0;      // consumer cursor
         int issued = 0;
         if (lane == 0) {
-            p_reset();
+            p_reset(reverse);
             for (; issued < stages - 1 && issued < n_my; ++issued) {
                 issue(io, reverse, p_t, p_st);
                 p_advance();
@@ -1019,12 +1070,13 @@ struct RecView {
     int w;
     int N;
     bool pad16;                      // 0xffff deltas stand for the zero row
+    int add;                         // kHopStencil: first row of the slice (col[] is relative to it), else 0
     __device__ __forceinline__ int col_at(int k, int r) const {
         if (d16) {
             const unsigned d = d16[k * 32 + r];
             return (pad16 && d == kPad16) ? N : col[k] + (int)d;
         }
-        return col[k * 32 + r];
+        return col[k * 32 + r] + add;
     }
 };
 __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
@@ -1039,12 +1091,17 @@ __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
     }
     RecView v;
     v.N = (int)m.N;
-    v.w = hop_is_16(m.hop) ? m.K : record_width(bytes, nd);         // the 16-bit variants are always uniform
+    v.w = (hop_is_16(m.hop) || m.hop == kHopStencil) ? m.K : record_width(bytes, nd);   // these variants are always uniform
     v.pad16 = m.hop == kHopConst16P;
+    v.add = 0;
     v.hre = reinterpret_cast<const double*>(m.rec + off);
     v.him = v.hre + (size_t)v.w * 32;
     v.on = v.hre + (size_t)v.w * 32 * nd;
     v.col = reinterpret_cast<const int*>(v.on + 32);
+    if (m.hop == kHopStencil) {
+        v.col = m.dict + (size_t)m.pid[slice] * (m.K * 32);
+        v.add = (int)(slice * 32);
+    }
     v.d16 = hop_is_16(m.hop) ? reinterpret_cast<const unsigned short*>(v.col + 8) : nullptr;
     return v;
 }

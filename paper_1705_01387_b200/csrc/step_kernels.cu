@@ -16,6 +16,8 @@ void* step_fn(int hop) {
     if (KK > 0 && hop == kHopConst16)      // 16-bit columns exist for the unrolled uniform tables only
         return (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopConst16, MODE>;
     if (KK > 0 && hop == kHopConst16P) return (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopConst16P, MODE>;
+    if (KK > 0 && hop == kHopStencil)      // pattern-dictionary columns: unrolled uniform tables only
+        return (void*)cheb_step_kernel<BB, (KK > 0 ? KK : 3), kHopStencil, MODE>;
     return hop == kHopComplex ? (void*)cheb_step_kernel<BB, KK, kHopComplex, MODE>
            : hop == kHopConst ? (void*)cheb_step_kernel<BB, KK, kHopConst, MODE>
                               : (void*)cheb_step_kernel<BB, KK, kHopReal, MODE>;

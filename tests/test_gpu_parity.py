@@ -360,10 +360,13 @@ def test_multi_step_launches(gq, oracle_mod, o):
         phi = L.random_phase_vectors(model.N, B, config=59)
         modes = gq.MODE_VAC | gq.MODE_MSD
         o_ = oracle_mod.Oracle(model, batch=B, modes=modes)
-        g = gq.GpuQT(model, batch=B, modes=modes, options={"small": 0, **o})
+        stencil = 2 if model.name.startswith("cubic") else 1     # the implicit stencil on multi-step launches too
+        g = gq.GpuQT(model, batch=B, modes=modes, options={"small": 0, "stencil": stencil, **o})
         assert g.info(binding.INFO_PERSISTENT) == o["persistent"]
         if model.name.startswith("square") and model.box_length <= 0:
             assert g.info(binding.INFO_HOP_VARIANT) == 4      # 16-bit columns with the 0xffff sentinel for the zero row
+        if model.name.startswith("cubic"):
+            assert g.info(binding.INFO_HOP_VARIANT) == 5 and g.info(binding.INFO_STENCIL_PATTERNS) == 27
         o_.set_state(phi)
         g.set_state(phi)
         for nm in (37, 64):
@@ -429,7 +432,7 @@ def test_16bit_columns_match_32bit(gq, oracle_mod, model):
     ref_chi = o.get_state(oracle_mod.CHI)
     outs = []
     for flag in (1, 0):
-        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC, options=opts(idx16=flag))
+        g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD | gq.MODE_VAC, options=opts(idx16=flag, stencil=0))
         assert g.info(binding.INFO_HOP_VARIANT) == (3 if flag else 2)
         for a, b in zip(g.get_table(), ref_tab):
             assert a.tobytes() == b.tobytes()
@@ -442,3 +445,48 @@ def test_16bit_columns_match_32bit(gq, oracle_mod, model):
         outs.append(dos.copy())
         g.close()
     assert outs[0].tobytes() == outs[1].tobytes()        # same arithmetic, only the column encoding differs
+
+
+@pytest.mark.parametrize("batch", [1, 2, 4, 8])
+@pytest.mark.parametrize("model", [L.cubic(16, W=16.5, seed=16, energy_scale=16.0),      # lines aligned with the slices
+                                   L.cubic(13, W=8.0, seed=4, energy_scale=11.0),        # nothing aligned, ragged tail
+                                   L.square(70, 37, W=2.0, seed=3),
+                                   L.graphene(29, 17, W=1.0, seed=5),                    # 4-atom cell: period 4 in the row index
+                                   L.chain(3001, W=1.0, seed=8)],
+                         ids=["cubic16", "cubic13", "square70x37", "graphene29x17", "chain3001"])
+def test_implicit_stencil_matches_explicit_columns(gq, oracle_mod, model, batch):
+    """the same regular lattice stored as an implicit stencil (on-site
+    records + pattern dictionary, option stencil = 2: forced) and with an explicit column array decodes to
+    the same canonical table, bit for bit the oracle's, and gives the same moments / vectors -- identical
+    bits, since only the column encoding differs."""
+    from paper_1705_01387_b200 import binding
+    phi = L.random_phase_vectors(model.N, batch, config=62)
+    modes = gq.MODE_MSD | gq.MODE_VAC
+    o = oracle_mod.Oracle(model, batch=batch, modes=modes)
+    o.set_state(phi)
+    ref_tab, ref_dos, ref_vac = o.get_table(), o.dos_moments(48), o.vac(31)
+    va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+    scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(batch)])
+    o.evolve(1.0, 44)
+    ref_chi, ref_a = o.get_state(oracle_mod.CHI), o.get_state(oracle_mod.VAC_A)
+    ref_msd = o.msd(20)
+    outs = []
+    for flag in (2, 0):
+        g = gq.GpuQT(model, batch=batch, modes=modes, options=opts(stencil=flag, idx16=0))
+        assert g.info(binding.INFO_HOP_VARIANT) == (5 if flag else 2)
+        assert (g.info(binding.INFO_STENCIL_PATTERNS) > 0) == bool(flag)
+        for a, b in zip(g.get_table(), ref_tab):
+            assert a.tobytes() == b.tobytes()
+        g.set_state(phi)
+        dos, vac = g.dos_moments(48), g.vac(31)
+        assert np.max(np.abs(dos - ref_dos)) / model.N <= TOL
+        assert np.max(np.abs(vac - ref_vac) / scale[:, None]) <= TOL
+        g.evolve(1.0, 44)
+        chi = g.get_state(gq.STATE_CHI)
+        assert vec_err(chi, ref_chi) <= TOL and vec_err(g.get_state(gq.STATE_VAC_A), ref_a) <= TOL
+        msd = g.msd(20)
+        assert np.max(np.abs(msd - ref_msd) / (norms(ref_chi) ** 2)[:, None]) <= TOL
+        outs.append((dos.copy(), vac.copy(), chi.copy(), msd.copy()))
+        g.close()
+    for a, b in zip(*outs):
+        assert a.tobytes() == b.tobytes()
