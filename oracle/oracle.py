@@ -11,7 +11,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gpuqt_oracle.c")
-_LIB = os.path.join(_HERE, "libgpuqt_oracle.so")
+# GPUQT_ORACLE_SANITIZE=1: a second build with -fsanitize=address,undefined (run the pins under it with
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so); summary in profiles/)
+_SAN = os.environ.get("GPUQT_ORACLE_SANITIZE", "0") == "1"
+_LIB = os.path.join(_HERE, "libgpuqt_oracle_san.so" if _SAN else "libgpuqt_oracle.so")
 
 MODE_VAC, MODE_MSD = 1, 2
 PSI, CHI, VAC_A, VAC_B = 0, 1, 2, 3
@@ -20,8 +23,9 @@ PSI, CHI, VAC_A, VAC_B = 0, 1, 2, 3
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain C99 + OpenMP over rows)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-std=c99", "-D_DEFAULT_SOURCE", "-fPIC", "-shared",
-                               "-fopenmp", "-o", _LIB, _SRC, "-lm"])
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if _SAN else ["-O2"]
+        subprocess.check_call(["gcc"] + opt + ["-std=c99", "-D_DEFAULT_SOURCE", "-fPIC", "-shared",
+                                               "-fopenmp", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 
