@@ -300,7 +300,8 @@ const void* tensor_map_of(const gpuqt_handle* h, const double2* buf) {
 
 // Tensor maps over the vector buffers: a buffer is seen as 128-byte lines (8 complex numbers; the last
 // line may reach into the buffer's zeroed alignment padding); one box = the 4 * B lines of one slice,
-// written to shared memory with the 128-byte swizzle; lines past the end are zero-filled.
+// written to shared memory with the 128-byte swizzle; lines past the end are zero-filled.  (kSwizzleLineBytes = 64:
+// the GPUQT_SWZ64 experiment of kernels.cuh.)
 int build_tensor_maps(gpuqt_handle* h) {
     if (h->B < 2) return GPUQT_OK;
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -313,13 +314,14 @@ int build_tensor_maps(gpuqt_handle* h) {
     EncodeFn encode = (EncodeFn)fp;
     std::vector<CUtensorMap> maps(h->map_bufs.size());
     for (size_t i = 0; i < maps.size(); ++i) {
-        const cuuint64_t dims[2] = {16, ((cuuint64_t)(h->N + 1) * (cuuint64_t)h->B * 16 + 127) / 128};
-        const cuuint64_t strides[1] = {128};
-        const cuuint32_t box[2] = {16, (cuuint32_t)(4 * h->B)};
+        constexpr cuuint64_t LB = kSwizzleLineBytes;
+        const cuuint64_t dims[2] = {LB / 8, ((cuuint64_t)(h->N + 1) * (cuuint64_t)h->B * 16 + LB - 1) / LB};
+        const cuuint64_t strides[1] = {LB};
+        const cuuint32_t box[2] = {(cuuint32_t)(LB / 8), (cuuint32_t)(512 / LB * h->B)};
         const cuuint32_t estr[2] = {1, 1};
         CUresult r = encode(&maps[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)h->map_bufs[i], dims, strides, box, estr,
-                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, LB == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(h, GPUQT_ERR_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r));
     }
     CU(cudaMalloc((void**)&h->d_maps, maps.size() * sizeof(CUtensorMap)));

@@ -50,8 +50,13 @@
 #ifndef GPUQT_MSD_OCC
 #define GPUQT_MSD_OCC 0
 #endif
+// (psi, chi) evolve kernel, second route to two CTAs per SM: a lane owns ONE vector of a row (128-bit accesses,
+// half the registers of the 256-bit ownership) and x_{m-2}, e_{m-2} rows are read by streaming loads
+#ifndef GPUQT_MSD_V1
+#define GPUQT_MSD_V1 0
+#endif
 #ifndef GPUQT_MINB_MSD
-#define GPUQT_MINB_MSD (GPUQT_MSD_OCC ? 2 : 1)
+#define GPUQT_MINB_MSD ((GPUQT_MSD_OCC || GPUQT_MSD_V1) ? 2 : 1)
 #endif
 
 // L2 policy experiments
@@ -60,6 +65,18 @@
 #endif
 #ifndef GPUQT_ST_POLICY       // stores of x_m: 0 plain, 1 st.global.cs (evict-first)
 #define GPUQT_ST_POLICY 0
+#endif
+
+// -DGPUQT_CHECKED=1: range checks of every gathered column, staged-row offset and pipeline index inside the
+// kernels (__trap() on violation -> the next CUDA call fails).  A test build: compute-sanitizer is not
+// available on the GPU pool this was developed on (profiles/r2_sanitizers.md).
+#ifndef GPUQT_CHECKED
+#define GPUQT_CHECKED 0
+#endif
+#if GPUQT_CHECKED
+#define GPUQT_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define GPUQT_CHECK(cond) do { } while (0)
 #endif
 
 namespace gpuqt {
@@ -237,11 +254,27 @@ __device__ __forceinline__ void tensor_g2s_hint(void* dst, const void* tmap, int
 // ordinary stores of one SM and read by TMA copies of another in the next step.
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-// Staged vector rows are written by the TMA with the 128-byte swizzle (16-byte chunk index, address
-// bits 4-6, ^= address bits 7-9; box rows are whole 128-byte lines): a lane's two 16-byte reads at a
-// 32-byte lane stride then fall on distinct banks for every group of 8 lanes (without it: a 2-way
-// bank conflict on every 128-bit read).  Uses the absolute shared address, as the TMA does.
-__device__ __forceinline__ uint32_t swz32(uint32_t sa) { return sa ^ ((sa >> 3) & 0x70u); }
+// Staged vector rows are written by the TMA with the 128-byte swizzle (16-byte chunk index, address bits 4-6,
+// ^= address bits 7-9; box rows are whole 128-byte lines): a lane's two 16-byte reads at a 32-byte lane stride then
+// fall on distinct banks for every group of 8 lanes when it reads its OWN row (without it: a 2-way bank conflict on
+// every 128-bit read).  Uses the absolute shared address, as the TMA does.  An in-slice gather of the row one
+// further on (the +-x neighbours of a lattice in natural order; 64 bytes at B = 4) still takes 6 instead of 4
+// wavefronts: the 256 bytes a group reads then span half of line L, line L + 1 and half of line L + 2, and for
+// lines L = 2, 6 (mod 8) the two halves collide under this swizzle (ncu, round 2: 20 % of the shared-memory
+// wavefronts of the c4 step).  GPUQT_SWZ64 = 1 is the experiment that removes it -- 64-byte lines with the
+// 64-byte swizzle, where address bit 6 keeps the halves apart: conflict-free and parity-green, but the TMA then
+// moves 64-byte lines and the c4 step went from 156 to 164 us, so it is off.
+#ifndef GPUQT_SWZ64
+#define GPUQT_SWZ64 0
+#endif
+constexpr int kSwizzleLineBytes = GPUQT_SWZ64 ? 64 : 128;     // bytes of one line of the tensor maps
+__device__ __forceinline__ uint32_t swz32(uint32_t sa) {
+#if GPUQT_SWZ64
+    return sa ^ ((sa >> 3) & 0x30u);
+#else
+    return sa ^ ((sa >> 3) & 0x70u);
+#endif
+}
 
 __device__ __forceinline__ void st_vec(double2* p, double2 v) {
 #if GPUQT_ST_POLICY == 1
@@ -360,14 +393,15 @@ __host__ __device__ constexpr int min_blocks(int B, int mode) {
 #define GPUQT_PREV_DIRECT 0
 #endif
 __host__ __device__ constexpr bool prev_direct(int B, int mode) {
-    return B >= 8 || GPUQT_PREV_DIRECT || (GPUQT_MSD_OCC && mode == kModeEvolveMsd);
+    return B >= 8 || GPUQT_PREV_DIRECT || ((GPUQT_MSD_OCC || GPUQT_MSD_V1) && mode == kModeEvolveMsd);
 }
 
 // A lane owns V consecutive vectors of a row (V = 2 when B >= 2: one 256-bit access per operand).
 // A tile is S consecutive slices and is walked in ROUNDS rounds of RS rows, U rounds at a time.
-template <int B, int KT>
+template <int B, int KT, int MODE = kModeDoubling>
 struct LaneShape {
-    static constexpr int V = B >= 2 ? 2 : 1;
+    static constexpr int V = (B >= 2 && !(GPUQT_MSD_V1 && MODE == kModeEvolveMsd)) ? 2 : 1;
+    static constexpr bool SWZ = B >= 2;                    // staged rows are written by swizzled tensor copies
     static constexpr int LPR = B / V;                      // lanes per row
     static constexpr int RS = 32 / LPR;                    // rows per round
     static constexpr int S = (B == 1 && KT > 0) ? 2 : 1;   // slices per tile
@@ -407,12 +441,18 @@ __device__ __forceinline__ CV<2> cv_lds_swz(uint32_t sa) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.re[1]), "=d"(v.im[1]) : "r"(p0 ^ 16u));
     return v;
 }
-template <int V>
-__device__ __forceinline__ CV<V> cv_lds_staged(const double2* p);
-template <>
-__device__ __forceinline__ CV<1> cv_lds_staged<1>(const double2* p) { return cv_lds<1>(p); }
-template <>
-__device__ __forceinline__ CV<2> cv_lds_staged<2>(const double2* p) { return cv_lds_swz(smem_u32(p)); }
+template <int V, bool SWZ>
+__device__ __forceinline__ CV<V> cv_lds_staged(const double2* p) {
+    if constexpr (V == 2) {
+        return cv_lds_swz(smem_u32(p));
+    } else if constexpr (SWZ) {
+        CV<1> v;
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.re[0]), "=d"(v.im[0]) : "r"(swz32(smem_u32(p))));
+        return v;
+    } else {
+        return cv_lds<1>(p);
+    }
+}
 
 // global memory, read once (evict-first)
 template <int V>
@@ -456,10 +496,27 @@ __device__ __forceinline__ void cv_st<2>(double2* p, const CV<2>& v) {
 //   s_l  = shared-window address of the same element of the tile's staged rows, minus row0 * RB
 //          (mod 2^32: only rows of the tile are ever addressed through it)
 //   RB   = bytes of one row (16 B);  TR = rows of a tile
-template <int V, int TR>
+template <int V, int TR, bool SWZ = false>
 __device__ __forceinline__ CV<V> cv_gather(const char* g_l, uint32_t s_l, int c, int row0, int RB);
 template <>
-__device__ __forceinline__ CV<1> cv_gather<1, 32>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+__device__ __forceinline__ CV<1> cv_gather<1, 32, true>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+    const unsigned d = (unsigned)(c - row0);
+    const uint32_t sa = swz32(s_l + (uint32_t)c * (uint32_t)RB);
+    const char* ga = g_l + (long long)c * RB;
+    CV<1> v;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.lt.u32 p, %4, 32;\n"
+        "@p ld.shared.v2.f64 {%0, %1}, [%2];\n"
+        "@!p ld.global.v2.f64 {%0, %1}, [%3];\n"          // (the L2::evict_last qualifier exists for 256-bit loads only)
+        "}"
+        : "=d"(v.re[0]), "=d"(v.im[0])
+        : "r"(sa), "l"(ga), "r"(d));
+    return v;
+}
+template <>
+__device__ __forceinline__ CV<1> cv_gather<1, 32, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
     const uint32_t sa = s_l + (uint32_t)c * (uint32_t)RB;
     const char* ga = g_l + (long long)c * RB;
@@ -476,7 +533,7 @@ __device__ __forceinline__ CV<1> cv_gather<1, 32>(const char* g_l, uint32_t s_l,
     return v;
 }
 template <>
-__device__ __forceinline__ CV<1> cv_gather<1, 64>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+__device__ __forceinline__ CV<1> cv_gather<1, 64, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
     const uint32_t sa = s_l + (uint32_t)c * (uint32_t)RB;
     const char* ga = g_l + (long long)c * RB;
@@ -493,7 +550,7 @@ __device__ __forceinline__ CV<1> cv_gather<1, 64>(const char* g_l, uint32_t s_l,
     return v;
 }
 template <>
-__device__ __forceinline__ CV<2> cv_gather<2, 32>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+__device__ __forceinline__ CV<2> cv_gather<2, 32, true>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
     const uint32_t sa = swz32(s_l + (uint32_t)c * (uint32_t)RB);
     const uint32_t sb = sa ^ 16u;
@@ -573,8 +630,8 @@ __device__ __forceinline__ int col_of(const int* s_col, const unsigned short* s_
 template <int B, int KT, int HOP, int MODE>
 __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, const StepCtx& io, const unsigned char* stage, int w,
                                             int row0, int rows_valid, int j0, int lane,
-                                            double (&red)[ModeTraits<MODE>::Q * LaneShape<B, KT>::V]) {
-    using LS = LaneShape<B, KT>;
+                                            double (&red)[ModeTraits<MODE>::Q * LaneShape<B, KT, MODE>::V]) {
+    using LS = LaneShape<B, KT, MODE>;
     constexpr int V = LS::V, LPR = LS::LPR, RS = LS::RS, U = LS::U, TR = 32 * LS::S;
     constexpr int KU = KT > 0 ? KT : 1;
     constexpr int RB = B * 16;   // bytes of one row of a vector set
@@ -636,8 +693,9 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         const int si_ = r[u] * B + l * V;                                 // element inside the staged rows
-        self[u] = ok[u] ? cv_lds_staged<V>(s_in + si_) : cv_zero<V>();
-        self_e[u] = (MSD && ok[u]) ? cv_lds_staged<V>(s_in_e + si_) : cv_zero<V>();
+        GPUQT_CHECK(si_ >= 0 && si_ + V <= TR * B && r[u] < TR);
+        self[u] = ok[u] ? cv_lds_staged<V, LS::SWZ>(s_in + si_) : cv_zero<V>();
+        self_e[u] = (MSD && ok[u]) ? cv_lds_staged<V, LS::SWZ>(s_in_e + si_) : cv_zero<V>();
     }
 
     CV<V> sum[U], sum_e[U], sum_x[U];   // H x, H e, [X,H] x (unscaled)
@@ -659,9 +717,10 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
                     const int k = k0 + kk;
                     if (k < KU) {
                         const int c = col_of<HOP>(s_col[u], s_d16[u], k, rr, N) + srow0[u];
-                        v[u][kk] = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
+                        GPUQT_CHECK((unsigned)c <= (unsigned)N);
+                        v[u][kk] = cv_gather<V, TR, LS::SWZ>(gl_in, sl_in, c, row0, RB);
                         if (MSD) {
-                            ve[u][kk] = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
+                            ve[u][kk] = cv_gather<V, TR, LS::SWZ>(gl_in_e, sl_in_e, c, row0, RB);
                             xn[u][kk] = m.x[c];
                         }
                     }
@@ -694,14 +753,15 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
         const int rr = r[0] & 31;
         for (int k = 0; k < w; ++k) {
             const int c = col_of<HOP>(s_col[0], s_d16[0], k, rr, N) + srow0[0];
+            GPUQT_CHECK((unsigned)c <= (unsigned)N);
             double hr = 1.0, hi = 0.0;
             if (!CONST) hr = s_hre[0][k * 32 + rr];
             if (CPLX) hi = (s_hre[0] + w * 32)[k * 32 + rr];
-            const CV<V> vv = cv_gather<V, TR>(gl_in, sl_in, c, row0, RB);
+            const CV<V> vv = cv_gather<V, TR, LS::SWZ>(gl_in, sl_in, c, row0, RB);
             if (CONST) cv_add<V>(sum[0], vv);
             else cv_fma<V, CPLX>(sum[0], hr, hi, vv);
             if (MSD) {
-                const CV<V> vve = cv_gather<V, TR>(gl_in_e, sl_in_e, c, row0, RB);
+                const CV<V> vve = cv_gather<V, TR, LS::SWZ>(gl_in_e, sl_in_e, c, row0, RB);
                 if (CONST) cv_add<V>(sum_e[0], vve);
                 else cv_fma<V, CPLX>(sum_e[0], hr, hi, vve);
                 const double ndx = -min_image(m.x[c] - xm[0], m.box);
@@ -714,8 +774,8 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     for (int u = 0; u < U; ++u) {
         const int si_ = r[u] * B + l * V;
         if (!PD && !io.first && ok[u]) {
-            prev[u] = cv_lds_staged<V>(s_prev + si_);
-            if (MSD) prev_e[u] = cv_lds_staged<V>(s_prev_e + si_);
+            prev[u] = cv_lds_staged<V, LS::SWZ>(s_prev + si_);
+            if (MSD) prev_e[u] = cv_lds_staged<V, LS::SWZ>(s_prev_e + si_);
         }
         const double os = io.scale * s_on[u][LS::S > 1 ? (r[u] & 31) : r[u]];   // scale of the on-site term
         CV<V> t, te;   // x_m (b_k) and e_m
@@ -814,7 +874,7 @@ __device__ __forceinline__ void block_partial(const double* s_part, int P, doubl
 // block m % G sums the partials of step m in a fixed order while the others go on.
 template <int B, int KT, int HOP, int MODE>
 __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kernel(const Mat m, const RecArgs a) {
-    using LS = LaneShape<B, KT>;
+    using LS = LaneShape<B, KT, MODE>;
     constexpr int Q = ModeTraits<MODE>::Q;
     constexpr int V = LS::V, ROUNDS = LS::ROUNDS, U = LS::U, S = LS::S, TR = 32 * S;
     constexpr int RB = B * 16, QB = Q * B;
@@ -921,6 +981,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
     // lane 0 only: every stream of tile t_virtual (sweep order) of the step `io` -> one stage, one mbarrier
     auto issue = [&](const StepCtx& io, int reverse, int t_virtual, int st) {
         const int t = reverse ? n_tiles - 1 - t_virtual : t_virtual;
+        GPUQT_CHECK(t >= 0 && t < n_tiles && st >= 0 && st < stages);
         const int s = t * S;                   // first slice of the tile
         long long off;
         uint32_t bytes;
@@ -942,7 +1003,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         if (B >= 2) {
             // tensor copies: always the full 32-row box (rows past the end of the buffer are zero-filled)
             const uint32_t total = bytes + (uint32_t)(32 * RB) * kPair * (with_prev ? 2u : 1u);
-            const int unit = s * 4 * B;           // first 128-byte line of the slice
+            const int unit = s * (512 / kSwizzleLineBytes) * B;    // first line of the slice
             mbar_expect_tx(&bars[st], total);
             copy_records(dst, off, bytes, &bars[st]);
             tensor_g2s(vdst, io.tm_in, unit, &bars[st]);
@@ -1015,6 +1076,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
             mbar_wait(&bars[c_st], c_ph);
             const unsigned char* stage = wstage + c_st * stage_bytes;
             const int tile = reverse ? n_tiles - 1 - c_t : c_t;
+            GPUQT_CHECK(c_st >= 0 && c_st < stages && tile >= 0 && tile < n_tiles);
             int w = KT;
             if (KT == 0) w = record_width(m.slice_off[tile + 1] - m.slice_off[tile], hop_doubles(HOP));
             const int row0 = tile * TR;
@@ -1123,6 +1185,7 @@ __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const d
         double sr = 0.0, si = 0.0;
         for (int k = 0; k < rv.w; ++k) {
             const int c = rv.col_at(k, r);                  // constant-hopping padding: the zero row N
+            GPUQT_CHECK((unsigned)c <= (unsigned)m.N);
             const double hr = hop_is_const(m.hop) ? m.hop_const : rv.hre[k * 32 + r];
             const double dx = min_image(m.x[c] - xm, m.box);
             const double wr = dx * hr;
