@@ -277,6 +277,68 @@ int gpuqt_reset_stats(gpuqt_handle* h);
 const char* gpuqt_last_error(const gpuqt_handle* h);
 void gpuqt_destroy(gpuqt_handle* h);
 
+/* ------------------------------------------------------------------ row-slab decomposition
+ * One lattice too large (or too slow) for one GPU is cut into SLABS of consecutive rows.  A slab owns n_own rows
+ * of H and of every state vector; the columns of its rows that belong to other slabs are its n_halo HALO rows,
+ * stored behind the owned rows (local index n_own + j), so a slab is an ordinary (rectangular) table for the
+ * kernels above.  Every recurrence step x_m = 2 H~ x_{m-1} - x_{m-2} (Eq. 21) needs the halo rows of
+ * x_{m-1}: after each step a slab PUSHES the owned rows its neighbours need straight into their halo rows (stores
+ * to the peer's vector buffer: a local buffer, or a peer-mapped one over NVLink), and the next step starts when
+ * every neighbour has pushed (same stream for slabs of one group; a release/acquire flag per sender at system
+ * scope for slabs on other GPUs).  The paper is single-GPU and limited by one card's memory
+ * (PAPER.md:51); this is the scale-out past that limit.  Inner products are partial sums over the owned rows:
+ * every moment call returns the sum over the slabs of THIS group, and the caller adds the groups' results
+ * (moments are linear in the partial sums).
+ *
+ * A gpuqt_slab_group is the set of slabs resident on one GPU (normally one; several emulate a multi-GPU
+ * decomposition on one device, which is how the tests run).  All slabs of all groups must make the same
+ * sequence of calls.  Slabs always run one launch per recurrence step (no cooperative / one-CTA forms).       */
+typedef struct gpuqt_slab_group gpuqt_slab_group;
+#define GPUQT_MAX_SLABS 64
+typedef struct gpuqt_slab_desc {
+    int32_t global_id;            /* id of this slab among all slabs of the decomposition, < GPUQT_MAX_SLABS   */
+    int64_t n_own;                /* rows this slab owns (computes)                                            */
+    int64_t n_halo;               /* halo rows, local indices n_own .. n_own + n_halo - 1                      */
+    const int32_t* nbr_count;     /* host [n_own]                                                              */
+    const int32_t* nbr_index;     /* host [n_own][K_max], LOCAL indices in [0, n_own + n_halo)                 */
+    const double* hop_re;         /* host [n_own][K_max] or NULL (-1)                                          */
+    const double* hop_im;         /* host [n_own][K_max] or NULL (real H)                                      */
+    const double* onsite;         /* host [n_own] or NULL (0)                                                  */
+    const double* x;              /* host [n_own + n_halo] positions (owned rows, then halo rows)              */
+    int32_t n_sends;              /* segments of owned rows other slabs need                                   */
+    const int32_t* send_peer;     /* host [n_sends] global id of the receiving slab                            */
+    const int64_t* send_count;    /* host [n_sends] rows in the segment                                        */
+    const int64_t* send_dst_row;  /* host [n_sends] first local row (>= the peer's n_own) it fills in the peer */
+    const int32_t* send_rows;     /* host, the segments' local owned-row indices, concatenated                 */
+    void* workspace;              /* device, 256-byte aligned, >= gpuqt_slab_workspace_bytes(...)              */
+    size_t workspace_bytes;
+} gpuqt_slab_desc;
+size_t gpuqt_slab_workspace_bytes(int64_t n_own, int64_t n_halo, int32_t K_max, int is_complex, int32_t batch, int modes);
+/* Builds the slabs (each validated like gpuqt_create; Hermiticity is checked for the owned-owned block only).
+ * Sends to slabs of this group are connected here; sends to other groups need gpuqt_slab_connect.  Errors of
+ * this call: gpuqt_last_error(NULL).                                                                         */
+int gpuqt_slab_create(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_desc* slabs, int32_t K_max,
+                      double box_length, double volume, double energy_scale, int32_t batch, int modes,
+                      void* cuda_stream);
+/* Device addresses another group needs to push into local slab `local_slab`: its vector buffers (in the fixed
+ * order every slab uses; gpuqt_slab_buffer_count of them) and its flag array (uint32[GPUQT_MAX_SLABS]).  The
+ * caller maps them into the peer process (CUDA IPC) and hands the mapped addresses to gpuqt_slab_connect there. */
+int32_t gpuqt_slab_buffer_count(const gpuqt_slab_group* g);
+int gpuqt_slab_export(gpuqt_slab_group* g, int32_t local_slab, void** buffers, void** flags);
+int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const* peer_buffers, void* peer_flags);
+/* phi_host[i]: host [batch][n_own of local slab i][2].  chi = 0; VAC mode: a = phi, b = V phi.                 */
+int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host);
+/* As gpuqt_dos_moments / gpuqt_evolve / gpuqt_vac / gpuqt_msd; moments: host [batch][n_moments], the partial
+ * sums over this group's slabs.                                                                              */
+int gpuqt_slab_dos_moments(gpuqt_slab_group* g, int32_t n_moments, double* out_host);
+int gpuqt_slab_evolve(gpuqt_slab_group* g, double dt, int32_t order);
+int gpuqt_slab_vac(gpuqt_slab_group* g, int32_t n_moments, double* out_host);
+int gpuqt_slab_msd(gpuqt_slab_group* g, int32_t n_moments, double* out_host);
+/* State of one local slab's owned rows: host [batch][n_own][2].                                               */
+int gpuqt_slab_get_state(gpuqt_slab_group* g, int32_t local_slab, int which, double* out_host);
+const char* gpuqt_slab_last_error(const gpuqt_slab_group* g);
+void gpuqt_slab_destroy(gpuqt_slab_group* g);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,6 +23,16 @@ DAMPING_JACKSON, DAMPING_LORENTZ, DAMPING_NONE = 0, 1, 2
  INFO_WORKSPACE_USED, INFO_SMALL_PATH_MSD, INFO_STENCIL_PATTERNS) = range(9)
 
 
+class SlabDesc(C.Structure):
+    """gpuqt_slab_desc (include/gpuqt.h)."""
+    _fields_ = [("global_id", C.c_int32), ("n_own", C.c_int64), ("n_halo", C.c_int64),
+                ("nbr_count", C.POINTER(C.c_int32)), ("nbr_index", C.POINTER(C.c_int32)),
+                ("hop_re", C.POINTER(C.c_double)), ("hop_im", C.POINTER(C.c_double)), ("onsite", C.POINTER(C.c_double)),
+                ("x", C.POINTER(C.c_double)), ("n_sends", C.c_int32), ("send_peer", C.POINTER(C.c_int32)),
+                ("send_count", C.POINTER(C.c_int64)), ("send_dst_row", C.POINTER(C.c_int64)),
+                ("send_rows", C.POINTER(C.c_int32)), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
 class Options(C.Structure):
     """gpuqt_options (include/gpuqt.h)."""
     _fields_ = [(n, C.c_int32) for n in ("struct_bytes", "stages", "blocks_per_sm", "run", "alternate", "hop_const",
@@ -69,6 +79,21 @@ _SIGNATURES = {
     "gpuqt_reset_stats": (C.c_int, [C.c_void_p]),
     "gpuqt_last_error": (C.c_char_p, [C.c_void_p]),
     "gpuqt_destroy": (None, [C.c_void_p]),
+    # row-slab decomposition
+    "gpuqt_slab_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int64, C.c_int32, C.c_int, C.c_int32, C.c_int]),
+    "gpuqt_slab_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int32, C.POINTER(SlabDesc), C.c_int32, C.c_double, C.c_double,
+                                    C.c_double, C.c_int32, C.c_int, C.c_void_p]),
+    "gpuqt_slab_buffer_count": (C.c_int32, [C.c_void_p]),
+    "gpuqt_slab_export": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "gpuqt_slab_connect": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.c_void_p]),
+    "gpuqt_slab_set_state": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
+    "gpuqt_slab_dos_moments": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
+    "gpuqt_slab_evolve": (C.c_int, [C.c_void_p, C.c_double, C.c_int32]),
+    "gpuqt_slab_vac": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
+    "gpuqt_slab_msd": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
+    "gpuqt_slab_get_state": (C.c_int, [C.c_void_p, C.c_int32, C.c_int, C.c_void_p]),
+    "gpuqt_slab_last_error": (C.c_char_p, [C.c_void_p]),
+    "gpuqt_slab_destroy": (None, [C.c_void_p]),
 }
 
 _lib = None

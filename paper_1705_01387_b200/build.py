@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("GPUQT_LIB") or os.path.join(HERE, "libgpuqt.so")
 UNITS = [("gpuqt.cu", [])] + [("step_kernels.cu", [f"-DGPUQT_TU_MODE={m}"]) for m in range(4)]
-DEPS = [os.path.join(CSRC, f) for f in ("gpuqt.cu", "step_kernels.cu", "kernels.cuh", "host_util.h")] + [
+DEPS = [os.path.join(CSRC, f) for f in ("gpuqt.cu", "step_kernels.cu", "kernels.cuh", "host_util.h", "slab_group.inl")] + [
     os.path.join(os.path.dirname(HERE), "include", "gpuqt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

@@ -4,6 +4,7 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <functional>
 #include <map>
 #include <mutex>
 #include <string>
@@ -37,7 +38,9 @@ thread_local std::string g_create_error;   // gpuqt_last_error(NULL)
 }  // namespace
 
 struct gpuqt_handle {
-    int64_t N = 0;
+    int64_t N = 0;                      // rows of the table (owned rows)
+    int64_t NV = 0;                     // zero row of the vector buffers: N, or N + n_halo for a row slab
+    int slab = 0;                       // member of a gpuqt_slab_group: one launch per step, no one-CTA kernels
     int32_t K = 0, B = 0;
     int modes = 0, cplx = 0, kt = 0, hop = 0;
     gpuqt_options opt{};
@@ -117,6 +120,7 @@ struct Layout {
     size_t rec, slice_off, x, vectors, partials, dots, moments, ticket, total;
 };
 
+// N = rows of the vector buffers below the zero row (owned rows + halo rows of a slab)
 Layout make_layout(int64_t N, int32_t B, int modes, size_t rec_bytes) {
     Layout L{};
     size_t off = 0;
@@ -173,12 +177,13 @@ cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
 constexpr int64_t kB200L2Bytes = 126LL << 20;
 int choose_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index, const double* hop_re,
                    const double* hop_im, const double* onsite, const gpuqt_options& opt, int batch, int64_t l2_bytes,
-                   SellHost& sell, StencilHost& sten) {
-    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell);
+                   SellHost& sell, StencilHost& sten, int64_t NV = -1) {
+    if (NV < 0) NV = N;
+    build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell, NV);
     const int64_t working_set = 3 * (N + 1) * (int64_t)batch * 16 + (int64_t)sell.rec.size();
     const bool want_stencil = opt.stencil == 2 || (opt.stencil == 1 && working_set > (l2_bytes > 0 ? l2_bytes : kB200L2Bytes));
     const bool use_stencil = want_stencil && unrolled_width(K_max) && try_stencil(sell, K_max, N, opt.stencil == 2, sten);
-    if (!use_stencil && opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, N);
+    if (!use_stencil && opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, NV);
     return sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : use_stencil ? kHopStencil
            : sell.idx16 == 2 ? kHopConst16P : sell.idx16 ? kHopConst16 : kHopConst;
 }
@@ -188,6 +193,10 @@ size_t stored_bytes_of(int64_t N, int hop, const SellHost& sell, const StencilHo
     if (hop == kHopStencil) rec = align_up(rec) + sten.dict.size() * sizeof(int32_t) + sten.pid.size() * sizeof(int32_t);
     return rec + (size_t)(N + 1) * sizeof(double);
 }
+int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, const int32_t* nbr_count,
+                  const int32_t* nbr_index, const double* hop_re, const double* hop_im, const double* onsite,
+                  const double* x, double box_length, double volume, double energy_scale, int32_t batch, int modes,
+                  void* workspace, size_t workspace_bytes, void* cuda_stream, const gpuqt_options* options, bool is_slab);
 
 // ---------------------------------------------------------------- kernel dispatch
 // the cheb_step_kernel instantiations live in step_kernels.cu, one translation unit per Mode
@@ -315,7 +324,7 @@ int build_tensor_maps(gpuqt_handle* h) {
     std::vector<CUtensorMap> maps(h->map_bufs.size());
     for (size_t i = 0; i < maps.size(); ++i) {
         constexpr cuuint64_t LB = kSwizzleLineBytes;
-        const cuuint64_t dims[2] = {LB / 8, ((cuuint64_t)(h->N + 1) * (cuuint64_t)h->B * 16 + LB - 1) / LB};
+        const cuuint64_t dims[2] = {LB / 8, ((cuuint64_t)(h->NV + 1) * (cuuint64_t)h->B * 16 + LB - 1) / LB};
         const cuuint64_t strides[1] = {LB};
         const cuuint32_t box[2] = {(cuuint32_t)(LB / 8), (cuuint32_t)(512 / LB * h->B)};
         const cuuint32_t estr[2] = {1, 1};
@@ -419,10 +428,10 @@ size_t small_smem_bytes(const gpuqt_handle* h) {
     const size_t NB = (size_t)h->N * h->B, KN = (size_t)h->K * h->N;
     return 4 * NB * sizeof(double2) + (size_t)h->N * 8 + KN * 8 * (size_t)hop_doubles(h->hop) + KN * 4 + 16;
 }
-bool small_ok(const gpuqt_handle* h) { return h->opt.small && small_smem_bytes(h) <= 210 * 1024; }
+bool small_ok(const gpuqt_handle* h) { return h->opt.small && !h->slab && small_smem_bytes(h) <= 210 * 1024; }
 // the (psi, chi) kernel keeps the x array in shared memory as well
 size_t small_msd_smem_bytes(const gpuqt_handle* h) { return small_smem_bytes(h) + (size_t)h->N * 8; }
-bool small_msd_ok(const gpuqt_handle* h) { return h->opt.small && small_msd_smem_bytes(h) <= 210 * 1024; }
+bool small_msd_ok(const gpuqt_handle* h) { return h->opt.small && !h->slab && small_msd_smem_bytes(h) <= 210 * 1024; }
 
 template <int MODE>
 void* small_fn(int B) {
@@ -457,8 +466,8 @@ cudaError_t launch_small(gpuqt_handle* h, int mode, SmallArgs& a) {
 // e-chain of the MSD pair).  Forward recurrences (moments) apply factor 1 in step 1 (T_1 = H~ T_0);
 // Clenshaw recurrences (evolution) in the LAST step.  One plain launch per step, or -- persistent
 // mode -- the whole recurrence in one cooperative launch with grid barriers between the steps.
-int run_recurrence(gpuqt_handle* h, int mode, int cls, RecArgs a) {
-    StatScope s(h, cls);
+// ring buffers and tensor maps of a recurrence whose x_0 (e_0) the caller has set
+void fill_rec_args(const gpuqt_handle* h, RecArgs& a) {
     for (int i = 0; i < kRing; ++i) {
         a.ring[i] = h->ring[i];
         a.tm_ring[i] = tensor_map_of(h, h->ring[i]);
@@ -467,6 +476,11 @@ int run_recurrence(gpuqt_handle* h, int mode, int cls, RecArgs a) {
     }
     a.tm_x0 = tensor_map_of(h, a.x0);
     a.tm_e0 = tensor_map_of(h, a.e0);
+}
+
+int run_recurrence(gpuqt_handle* h, int mode, int cls, RecArgs a) {
+    StatScope s(h, cls);
+    fill_rec_args(h, a);
     if (a.terms < 2) return GPUQT_OK;
     if (h->persistent) {
         a.multi = 1;
@@ -716,6 +730,18 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
                  const double* onsite, const double* x, double box_length, double volume,
                  double energy_scale, int32_t batch, int modes, void* workspace,
                  size_t workspace_bytes, void* cuda_stream, const gpuqt_options* options) {
+    return create_handle(out, N, 0, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, volume, energy_scale,
+                         batch, modes, workspace, workspace_bytes, cuda_stream, options, false);
+}
+}  // extern "C"
+
+namespace {
+// gpuqt_create_with_options (n_halo = 0), or one row slab of a gpuqt_slab_group (n_halo >= 0 halo rows behind the
+// N owned rows; x has N + n_halo entries)
+int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, const int32_t* nbr_count,
+                  const int32_t* nbr_index, const double* hop_re, const double* hop_im, const double* onsite,
+                  const double* x, double box_length, double volume, double energy_scale, int32_t batch, int modes,
+                  void* workspace, size_t workspace_bytes, void* cuda_stream, const gpuqt_options* options, bool is_slab) {
     auto bad = [&](int code, const std::string& msg) {
         g_create_error = "gpuqt_create: " + msg;
         return code;
@@ -736,13 +762,18 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
         opt.stencil < 0 || opt.stencil > 2)
         return bad(GPUQT_ERR_ARG, "option out of range");
     std::string msg;
-    int rc = validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg);
+    int rc = validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg, n_halo);
     if (rc != GPUQT_OK) return bad(rc, msg);
     if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return bad(GPUQT_ERR_ARG, "workspace must be 256-byte aligned");
+    const int64_t NV = N + n_halo;
+    if (is_slab) {              // the steps of a slab are separated by halo exchanges: one launch per step, streaming kernels
+        opt.small = 0;
+        opt.persistent = 0;
+    }
     if (modes & GPUQT_MODE_MSD) modes |= GPUQT_MODE_PSI;
     gpuqt_handle* h = new (std::nothrow) gpuqt_handle();
     if (!h) return bad(GPUQT_ERR_NOMEM, "out of host memory");
-    h->N = N; h->K = K_max; h->B = batch; h->modes = modes; h->cplx = hop_im ? 1 : 0;
+    h->N = N; h->NV = NV; h->slab = is_slab ? 1 : 0; h->K = K_max; h->B = batch; h->modes = modes; h->cplx = hop_im ? 1 : 0;
     h->opt = opt;
     h->dE = energy_scale; h->box = box_length; h->volume = volume;
     h->stream = (cudaStream_t)cuda_stream;
@@ -758,7 +789,7 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
             l2_bytes = 0;                   // no device: gpuqt_create fails below with GPUQT_ERR_CUDA
         }
     }
-    h->hop = choose_storage(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt, batch, l2_bytes, sell, sten);
+    h->hop = choose_storage(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt, batch, l2_bytes, sell, sten, NV);
     const bool use_stencil = h->hop == kHopStencil;
     h->stencil_patterns = use_stencil ? sten.n_patterns : 0;
     h->kt = (sell.uniform && unrolled_width(K_max)) ? K_max : 0;
@@ -771,13 +802,13 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     // the stencil dictionary lives behind the records
     const size_t dict_off = align_up(sell.rec.size()), dict_bytes = sten.dict.size() * sizeof(int32_t);
     const size_t rec_bytes = use_stencil ? dict_off + dict_bytes : sell.rec.size();
-    const Layout L = make_layout(N, batch, modes, rec_bytes);
+    const Layout L = make_layout(NV, batch, modes, rec_bytes);
     if (L.total > workspace_bytes) {
         delete h;
         return bad(GPUQT_ERR_NOMEM, "workspace too small: " + std::to_string(L.total) + " bytes needed");
     }
     h->workspace_used = L.total;
-    h->stored_matrix_bytes = stored_bytes_of(N, h->hop, sell, sten);
+    h->stored_matrix_bytes = stored_bytes_of(NV, h->hop, sell, sten);
     int dev = 0;
     cudaError_t ce = cudaGetDevice(&dev);
     if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -795,10 +826,10 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     };
     ce = up(d_rec, sell.rec.data(), sell.rec.size());
     if (ce == cudaSuccess && use_stencil) ce = up(d_rec + dict_off, sten.dict.data(), dict_bytes);
-    if (ce == cudaSuccess) ce = up(d_x, x, (size_t)N * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMemsetAsync(d_x + N, 0, sizeof(double), h->stream);
+    if (ce == cudaSuccess) ce = up(d_x, x, (size_t)NV * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(d_x + NV, 0, sizeof(double), h->stream);
     if (ce == cudaSuccess)
-        ce = cudaMemsetAsync(base + L.vectors, 0, (size_t)n_vectors(modes) * align_up((size_t)(N + 1) * batch * sizeof(double2)),
+        ce = cudaMemsetAsync(base + L.vectors, 0, (size_t)n_vectors(modes) * align_up((size_t)(NV + 1) * batch * sizeof(double2)),
                              h->stream);
     // the slice_off slot holds the byte offsets of ragged tables, or the pattern ids of the stencil variant
     if (ce == cudaSuccess)
@@ -815,7 +846,7 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
         return bad(GPUQT_ERR_CUDA, "upload failed: " + why);
     }
     h->mat.rec = d_rec; h->mat.slice_off = d_sp; h->mat.x = d_x;
-    h->mat.N = N; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
+    h->mat.N = N; h->mat.NV = NV; h->mat.n_slices = sell.n_slices; h->mat.K = K_max; h->mat.uniform = sell.uniform;
     h->mat.cplx = h->cplx; h->mat.hop = h->hop; h->mat.hop_const = sell.hop_const;
     h->mat.inv_dE = 1.0 / energy_scale; h->mat.box = box_length;
     h->mat.pid = use_stencil ? (const int*)d_sp : nullptr;
@@ -833,7 +864,7 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     int run = opt.run ? opt.run : (tiles < (long long)64 * kWarps * h->n_sm ? kWarps : 2 * kWarps);
     h->run = std::max(1, run / kWarps) * kWarps;
 
-    const size_t vstride = align_up((size_t)(N + 1) * batch * sizeof(double2));
+    const size_t vstride = align_up((size_t)(NV + 1) * batch * sizeof(double2));
     char* v = base + L.vectors;
     auto nextv = [&]() {
         double2* p = (double2*)v;
@@ -864,6 +895,9 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
     *out = h;
     return GPUQT_OK;
 }
+}  // namespace
+
+extern "C" {
 
 int gpuqt_set_state(gpuqt_handle* h, const double* phi_host) {
     if (!h || !phi_host) return fail(h, GPUQT_ERR_ARG, "null argument");
@@ -1106,3 +1140,5 @@ void gpuqt_destroy(gpuqt_handle* h) {
 }
 
 }  // extern "C"
+
+#include "slab_group.inl"

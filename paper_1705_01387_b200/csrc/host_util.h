@@ -23,10 +23,13 @@ inline double host_min_image(double d, double box) {
 }
 
 // Validation of the paper's four data sets.  Returns a gpuqt_status and a message.
+// n_halo > 0: the table is a row slab of a decomposed lattice -- columns may point at the halo rows
+// N .. N + n_halo - 1 (values owned by another slab; x has N + n_halo entries), and Hermiticity can only be
+// checked for the entries whose column is an owned row.
 inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
                            const double* hre, const double* him, const double* onsite,
-                           const double* x, double box, double dE, std::string& msg) {
-    if (N <= 0 || K <= 0 || !cnt || !idx || !x || !(dE > 0.0) || N > 0x7fffffffLL) {
+                           const double* x, double box, double dE, std::string& msg, int64_t n_halo = 0) {
+    if (N <= 0 || K <= 0 || !cnt || !idx || !x || !(dE > 0.0) || n_halo < 0 || N + n_halo > 0x7fffffffLL) {
         msg = "invalid argument (N, K_max, energy_scale must be positive; nbr_count, nbr_index, x required; N < 2^31)";
         return GPUQT_ERR_ARG;
     }
@@ -43,7 +46,7 @@ inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32
         }
         for (int32_t k = 0; k < c; ++k) {
             const int32_t n = idx[(size_t)m * K + k];
-            if (n < 0 || n >= N) {
+            if (n < 0 || n >= N + n_halo) {
                 msg = "neighbour index out of range at site " + std::to_string(m);
                 return GPUQT_ERR_INDEX;
             }
@@ -69,12 +72,12 @@ inline int validate_inputs(int64_t N, int32_t K, const int32_t* cnt, const int32
                 H(m, j, r2, i2);
                 if (idx[(size_t)m * K + j] == n && r2 == re && i2 == im) ++here;
             }
-            for (int32_t j = 0; j < cnt[n]; ++j) {
+            for (int32_t j = 0; n < N && j < cnt[n]; ++j) {
                 double r2, i2;
                 H(n, j, r2, i2);
                 if (idx[(size_t)n * K + j] == (int32_t)m && r2 == re && i2 == -im) ++there;
             }
-            if (here != there) {
+            if (n < N && here != there) {
                 msg = "H is not Hermitian: entry (" + std::to_string(m) + "," + std::to_string(n) + ") has no conjugate partner";
                 return GPUQT_ERR_NOT_HERMITIAN;
             }
@@ -145,9 +148,11 @@ inline bool constant_hopping(int64_t N, int32_t K, const int32_t* cnt, const dou
     return true;
 }
 
+// pad_col = index of the all-zero vector row (N; N + n_halo for a row slab)
 inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
                        const double* hre, const double* him, const double* onsite, bool allow_const,
-                       int pad_to, SellHost& s) {
+                       int pad_to, SellHost& s, int64_t pad_col = -1) {
+    if (pad_col < 0) pad_col = N;
     s.nd = him ? 2 : 1;
     if (allow_const && constant_hopping(N, K, cnt, hre, him, s.hop_const)) s.nd = 0;
     const int cplx = s.nd;   // doubles per entry
@@ -186,7 +191,7 @@ inline void build_sell(int64_t N, int32_t K, const int32_t* cnt, const int32_t* 
                     if (s.nd >= 1) r_hre[e] = hre ? hre[(size_t)m * K + k] : -1.0;
                     if (s.nd == 2) r_him[e] = him[(size_t)m * K + k];
                 } else if (s.nd == 0) {
-                    r_col[e] = (int32_t)N;                                     // padding: the zero row
+                    r_col[e] = (int32_t)pad_col;                               // padding: the zero row
                 } else {
                     r_col[e] = (int32_t)(m < N ? m : N - 1);                   // padding: own row, hop 0
                 }

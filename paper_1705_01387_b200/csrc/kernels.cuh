@@ -126,10 +126,13 @@ constexpr unsigned kPad16 = 0xffffu;     // 16-bit delta that stands for the zer
 struct Mat {
     const unsigned char* __restrict__ rec;      // packed slice records
     const long long* __restrict__ slice_off;    // [n_slices_padded + 1] byte offsets (ragged variant)
-    const double* __restrict__ x;               // [N + 1], x[N] = 0
+    const double* __restrict__ x;               // [NV + 1], x[NV] = 0
     const int* __restrict__ pid;                // kHopStencil: [n_slices_padded] pattern of each slice
     const int* __restrict__ dict;               // kHopStencil: [n_patterns][K][32] columns relative to the slice's first row
-    long long N;
+    long long N;                                // rows of the table = rows this device computes
+    long long NV;                               // index of the all-zero row of every vector buffer (vector rows: NV + 1).
+                                                // NV = N, except for a row slab of a decomposed lattice, whose vectors
+                                                // carry the halo rows N .. NV-1 behind the owned rows (columns may point there)
     long long n_slices;                         // real slices, ceil(N / 32)
     int K;                                      // K_max
     int uniform;                                // every record has width K
@@ -652,7 +655,7 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
     const char* gl_in = reinterpret_cast<const char*>(io.in + l * V);
     const char* gl_in_e = reinterpret_cast<const char*>(io.in_e + l * V);
     constexpr bool PD = prev_direct(B, MODE);
-    const int N = (int)m.N;
+    const int N = (int)m.NV;  // columns run over [0, NV]: owned rows, halo rows, the zero row
 
     int r[U];                 // row inside the tile
     bool ok[U];
@@ -994,9 +997,10 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         }
         const int left = N - s * 32;
         const uint32_t vbytes = (uint32_t)((left < TR ? left : TR) * RB);
-        // x_{m-1} rows include the all-zero row N when it falls into this tile's window (the
-        // constant-hopping padding entries point at it)
-        const uint32_t vbytes_in = (uint32_t)((left + 1 < TR ? left + 1 : TR) * RB);
+        // x_{m-1} rows include the halo rows and the all-zero row NV when they fall into this tile's window
+        // (columns of the last owned rows / the constant-hopping padding entries point at them)
+        const int left_in = (int)m.NV + 1 - s * 32;
+        const uint32_t vbytes_in = (uint32_t)((left_in < TR ? left_in : TR) * RB);
         const bool with_prev = !io.first && !prev_direct(B, MODE);
         unsigned char* dst = wstage + st * stage_bytes;
         unsigned char* vdst = dst + a.rec_bytes;
@@ -1152,7 +1156,7 @@ __device__ __forceinline__ RecView record_view(const Mat& m, long long slice) {
         bytes = m.slice_off[slice + 1] - off;
     }
     RecView v;
-    v.N = (int)m.N;
+    v.N = (int)m.NV;
     v.w = (hop_is_16(m.hop) || m.hop == kHopStencil) ? m.K : record_width(bytes, nd);   // these variants are always uniform
     v.pad16 = m.hop == kHopConst16P;
     v.add = 0;
@@ -1185,7 +1189,7 @@ __global__ void __launch_bounds__(kThreads) velocity_kernel(const Mat m, const d
         double sr = 0.0, si = 0.0;
         for (int k = 0; k < rv.w; ++k) {
             const int c = rv.col_at(k, r);                  // constant-hopping padding: the zero row N
-            GPUQT_CHECK((unsigned)c <= (unsigned)m.N);
+            GPUQT_CHECK((unsigned)c <= (unsigned)m.NV);
             const double hr = hop_is_const(m.hop) ? m.hop_const : rv.hre[k * 32 + r];
             const double dx = min_image(m.x[c] - xm, m.box);
             const double wr = dx * hr;
@@ -1358,8 +1362,8 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
     if (k < rv.w) {
         c = rv.col_at(k, r);
         if (hop_is_const(m.hop)) {
-            hr = c < m.N ? m.hop_const : 0.0;
-            c = c < m.N ? c : (int)row;
+            hr = c < m.NV ? m.hop_const : 0.0;
+            c = c < m.NV ? c : (int)row;
         } else {
             hr = rv.hre[k * 32 + r];
         }
