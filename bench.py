@@ -381,6 +381,55 @@ def run_ours(args, w):
         dist.destroy_process_group()
 
 
+def run_slabs(args, w):
+    """Secondary measurement (not the bench contract's line): the workload cut into --slabs row slabs, all resident
+    on this one GPU (the multi-GPU decomposition emulated on one device: same launches and halo
+    pushes, no cross-GPU flags).  Shows what the decomposition costs against the single-handle path."""
+    import torch
+    import paper_1705_01387_b200 as gq
+    from paper_1705_01387_b200 import slab
+    torch.cuda.set_device(0)
+    model = w.build()
+    order = w.order
+    modes = gq.MODE_MSD if w.path == "msd" else gq.MODE_VAC
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        slabs = slab.partition(model, args.slabs)
+        g = slab.SlabGroup(model, slabs, batch=w.batch, modes=modes, stream=stream)
+        g.set_state(w.phases(model))
+
+        def step():
+            if w.path == "msd":
+                g.evolve(w.dt, order)
+                return g.msd(w.n_moments, reduce=False)
+            out = g.vac(w.n_moments, reduce=False)
+            g.evolve(w.dt, order)
+            return out
+
+        for _ in range(args.warmup):
+            step()
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(args.steps):
+            out = step()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1)
+    ev_w, mom_w = walks_per_step(w, order)
+    value = model.N * w.batch * (ev_w + mom_w) * args.steps / (ms * 1e-3)
+    assert np.all(np.isfinite(out))
+    print(json.dumps({"metric": "orbital-SpMV/s in Chebyshev evolution + KPM moments", "value": value, "unit": "orbital-SpMV/s",
+                      "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                      "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": w.key, "N": model.N, "batch_per_gpu": w.batch, "n_moments": w.n_moments,
+                                 "order": order, "slabs": args.slabs, "slabs_resident_on_one_gpu": True,
+                                 "rows_per_slab": [s.n_own for s in slabs], "halo_rows_per_slab": [s.n_halo for s in slabs],
+                                 "note": "row-slab decomposition emulated on one device; no kpm_transform in this line"}}),
+          flush=True)
+    g.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -392,11 +441,15 @@ def main():
     ap.add_argument("--no-clock-sampler", action="store_true", help="diagnostic: do not poll nvidia-smi during the timed region")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="gpuqt_options override for tuning runs, e.g. --opt persistent=0 (default: the library defaults)")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="secondary measurement: cut the workload into this many row slabs resident on ONE GPU (SURVEY 8(f) 4)")
     args = ap.parse_args()
     args.options = {k: int(v) for k, v in (kv.split("=", 1) for kv in args.opt)}
     w = configs.WORKLOADS[args.config]
     if args.impl == "reference":
         run_reference(args, w)
+    elif args.slabs > 0:
+        run_slabs(args, w)
     else:
         run_ours(args, w)
 

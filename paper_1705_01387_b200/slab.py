@@ -205,3 +205,71 @@ def slabs_of_rank(n_slabs, rank, world):
     """Global slab ids rank `rank` holds when `n_slabs` slabs are dealt to `world` ranks in consecutive blocks."""
     per = (n_slabs + world - 1) // world
     return list(range(rank * per, min(n_slabs, (rank + 1) * per)))
+
+
+# ------------------------------------------------------------------ slabs on other ranks: CUDA IPC
+class _IpcHandle(C.Structure):
+    _fields_ = [("reserved", C.c_char * 64)]
+
+
+def _cuda_libs():
+    rt = None
+    for name in ("libcudart.so.12", "libcudart.so", "/usr/local/cuda/lib64/libcudart.so"):
+        try:
+            rt = C.CDLL(name)
+            break
+        except OSError:
+            continue
+    if rt is None:
+        raise RuntimeError("libcudart not found (CUDA IPC needs it)")
+    return rt, C.CDLL("libcuda.so.1")
+
+
+def _export_pointer(rt, drv, ptr):
+    """(ipc handle bytes, offset of ptr inside its allocation)."""
+    base, size = C.c_uint64(), C.c_size_t()
+    if drv.cuMemGetAddressRange_v2(C.byref(base), C.byref(size), C.c_uint64(ptr)) != 0:
+        raise RuntimeError("cuMemGetAddressRange failed")
+    h = _IpcHandle()
+    if rt.cudaIpcGetMemHandle(C.byref(h), C.c_void_p(base.value)) != 0:
+        raise RuntimeError("cudaIpcGetMemHandle failed")
+    return bytes(h.reserved), ptr - base.value
+
+
+def connect_ranks(group, dist=None):
+    """One slab group per rank, one rank per GPU: every rank publishes CUDA IPC handles of its slabs' vector buffers
+    and flag arrays (all_gather_object), opens those of the slabs its own slabs send to, and hands the mapped
+    addresses to gpuqt_slab_connect.  The pushes then go straight into the peer GPU's memory over NVLink.
+    Host plumbing only.  (Not exercised in this repository's tests: they run on one GPU, where all slabs live in
+    one group and need no connection.)"""
+    if dist is None:
+        import torch.distributed as dist
+    lib = binding.load()
+    rt, drv = _cuda_libs()
+    n_buf = lib.gpuqt_slab_buffer_count(group._g)
+    mine = {}
+    for i, s in enumerate(group.slabs):
+        bufs, flags = (C.c_void_p * n_buf)(), C.c_void_p()
+        group._ck(lib.gpuqt_slab_export(group._g, i, bufs, C.byref(flags)), "gpuqt_slab_export")
+        mine[s.global_id] = ([_export_pointer(rt, drv, int(b)) for b in bufs], _export_pointer(rt, drv, flags.value))
+    everyone = [None] * dist.get_world_size()
+    dist.all_gather_object(everyone, mine)
+    wanted = {peer for s in group.slabs for peer, _, _ in s.sends} - {s.global_id for s in group.slabs}
+    opened = {}
+
+    def open_(handle, offset):
+        if handle not in opened:
+            h, p = _IpcHandle(), C.c_void_p()
+            C.memmove(h.reserved, handle, 64)
+            if rt.cudaIpcOpenMemHandle(C.byref(p), h, C.c_uint(1)) != 0:       # cudaIpcMemLazyEnablePeerAccess
+                raise RuntimeError("cudaIpcOpenMemHandle failed (peer access between the two GPUs is required)")
+            opened[handle] = p.value
+        return opened[handle] + offset
+
+    for published in everyone:
+        for gid, (bufs, flags) in published.items():
+            if gid in wanted:
+                ptrs = (C.c_void_p * n_buf)(*[open_(h, off) for h, off in bufs])
+                group._ck(lib.gpuqt_slab_connect(group._g, gid, ptrs, C.c_void_p(open_(*flags))), "gpuqt_slab_connect")
+    group._ipc = opened
+    dist.barrier()
