@@ -100,9 +100,10 @@ typedef enum {
  *                  hopping integrals ... are -1", the lattices of PAPER.md:359, :381): no index array is
  *                  streamed; the distinct per-slice patterns of relative columns are kept in a small
  *                  dictionary and a slice names its pattern.  1: when the dictionary is at most 1/16 of
- *                  the index array (and <= 8 MB) AND a recurrence step's working set (three vector sets +
- *                  the table) exceeds the L2 cache, i.e. when the index array would come from HBM in
- *                  every step; 0: never; 2: whenever the table is uniform (tests)                      */
+ *                  the index array (and <= 8 MB) AND batch >= 4 AND a recurrence step's working set (three
+ *                  vector sets + the table) exceeds the L2 cache, i.e. when the index array would come from
+ *                  HBM in every step and a tile streams enough bytes to pay for the extra copies;
+ *                  0: never; 2: whenever the table is uniform (tests)                                  */
 typedef struct gpuqt_options {
     int32_t struct_bytes;
     int32_t stages;

@@ -173,7 +173,10 @@ cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
 // The stencil saves HBM bytes and costs two more (small) TMA copies per slice: it is taken (option 1) only when
 // a recurrence step's working set -- three vector sets and the table -- does not fit the L2, i.e. when the
 // index array would really come from HBM every step (c2, 72 MB, is faster with the explicit array: 12.3 vs
-// 20.0 us per step; c4, 786 MB, is faster with the stencil: 156 vs 162 us).
+// 20.0 us per step; c4, 786 MB, is faster with the stencil: 156 vs 162 us), and only at batch >= 4: at B = 1 a
+// tile streams so few bytes that the two extra copies per slice cost more than the index bytes they save (the
+// paper's example 5.1, a 2000 x 2000 square lattice with one vector: 1.57 s with explicit columns, 2.07 s with the
+// stencil).
 constexpr int64_t kB200L2Bytes = 126LL << 20;
 int choose_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index, const double* hop_re,
                    const double* hop_im, const double* onsite, const gpuqt_options& opt, int batch, int64_t l2_bytes,
@@ -181,7 +184,7 @@ int choose_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int
     if (NV < 0) NV = N;
     build_sell(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt.hop_const != 0, kTilePad, sell, NV);
     const int64_t working_set = 3 * (N + 1) * (int64_t)batch * 16 + (int64_t)sell.rec.size();
-    const bool want_stencil = opt.stencil == 2 || (opt.stencil == 1 && working_set > (l2_bytes > 0 ? l2_bytes : kB200L2Bytes));
+    const bool want_stencil = opt.stencil == 2 || (opt.stencil == 1 && batch >= 4 && working_set > (l2_bytes > 0 ? l2_bytes : kB200L2Bytes));
     const bool use_stencil = want_stencil && unrolled_width(K_max) && try_stencil(sell, K_max, N, opt.stencil == 2, sten);
     if (!use_stencil && opt.idx16 && unrolled_width(K_max)) try_idx16(sell, K_max, NV);
     return sell.nd == 2 ? kHopComplex : sell.nd == 1 ? kHopReal : use_stencil ? kHopStencil

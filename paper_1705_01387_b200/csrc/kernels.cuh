@@ -399,6 +399,11 @@ __host__ __device__ constexpr bool prev_direct(int B, int mode) {
     return B >= 8 || GPUQT_PREV_DIRECT || ((GPUQT_MSD_OCC || GPUQT_MSD_V1) && mode == kModeEvolveMsd);
 }
 
+// slices per tile at B = 1 on the unrolled uniform tables (2 or 4; kTilePad is a multiple): a tile's bookkeeping
+// (pipeline cursors, TMA issues, mbarrier wait: ~150 warp instructions) is paid once per tile
+#ifndef GPUQT_B1_SLICES
+#define GPUQT_B1_SLICES 2
+#endif
 // A lane owns V consecutive vectors of a row (V = 2 when B >= 2: one 256-bit access per operand).
 // A tile is S consecutive slices and is walked in ROUNDS rounds of RS rows, U rounds at a time.
 template <int B, int KT, int MODE = kModeDoubling>
@@ -407,11 +412,11 @@ struct LaneShape {
     static constexpr bool SWZ = B >= 2;                    // staged rows are written by swizzled tensor copies
     static constexpr int LPR = B / V;                      // lanes per row
     static constexpr int RS = 32 / LPR;                    // rows per round
-    static constexpr int S = (B == 1 && KT > 0) ? 2 : 1;   // slices per tile
+    static constexpr int S = (B == 1 && KT > 0) ? GPUQT_B1_SLICES : 1;   // slices per tile
     static constexpr int ROUNDS = S * LPR;                 // rounds per tile
     static constexpr int U = (B == 1 && KT > 0) ? 2 : 1;   // rounds walked together
 };
-__host__ __device__ constexpr int tile_slices(int B, int kt) { return (B == 1 && kt > 0) ? 2 : 1; }
+__host__ __device__ constexpr int tile_slices(int B, int kt) { return (B == 1 && kt > 0) ? GPUQT_B1_SLICES : 1; }
 
 template <int V>
 struct CV {   // V complex numbers
@@ -518,8 +523,9 @@ __device__ __forceinline__ CV<1> cv_gather<1, 32, true>(const char* g_l, uint32_
         : "r"(sa), "l"(ga), "r"(d));
     return v;
 }
-template <>
-__device__ __forceinline__ CV<1> cv_gather<1, 32, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+// V = 1, plain (unswizzled) staged rows, any tile height
+template <int TR>
+__device__ __forceinline__ CV<1> cv_gather_plain(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     const unsigned d = (unsigned)(c - row0);
     const uint32_t sa = s_l + (uint32_t)c * (uint32_t)RB;
     const char* ga = g_l + (long long)c * RB;
@@ -527,30 +533,25 @@ __device__ __forceinline__ CV<1> cv_gather<1, 32, false>(const char* g_l, uint32
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "setp.lt.u32 p, %4, 32;\n"
+        "setp.lt.u32 p, %4, %5;\n"
         "@p ld.shared.v2.f64 {%0, %1}, [%2];\n"
         "@!p ld.global.v2.f64 {%0, %1}, [%3];\n"
         "}"
         : "=d"(v.re[0]), "=d"(v.im[0])
-        : "r"(sa), "l"(ga), "r"(d));
+        : "r"(sa), "l"(ga), "r"(d), "n"(TR));
     return v;
 }
 template <>
+__device__ __forceinline__ CV<1> cv_gather<1, 32, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+    return cv_gather_plain<32>(g_l, s_l, c, row0, RB);
+}
+template <>
 __device__ __forceinline__ CV<1> cv_gather<1, 64, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
-    const unsigned d = (unsigned)(c - row0);
-    const uint32_t sa = s_l + (uint32_t)c * (uint32_t)RB;
-    const char* ga = g_l + (long long)c * RB;
-    CV<1> v;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "setp.lt.u32 p, %4, 64;\n"
-        "@p ld.shared.v2.f64 {%0, %1}, [%2];\n"
-        "@!p ld.global.v2.f64 {%0, %1}, [%3];\n"
-        "}"
-        : "=d"(v.re[0]), "=d"(v.im[0])
-        : "r"(sa), "l"(ga), "r"(d));
-    return v;
+    return cv_gather_plain<64>(g_l, s_l, c, row0, RB);
+}
+template <>
+__device__ __forceinline__ CV<1> cv_gather<1, 128, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+    return cv_gather_plain<128>(g_l, s_l, c, row0, RB);
 }
 template <>
 __device__ __forceinline__ CV<2> cv_gather<2, 32, true>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
@@ -912,11 +913,10 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         const int in_last = rem >= a.run ? per : (warp < rem ? (rem - warp + kWarps - 1) / kWarps : 0);
         n_my = (my_runs - 1) * per + in_last;
     }
-    uint64_t policy = 0;
+    const uint64_t policy = policy_evict_first();        // in every lane: the operands of the TMA issues stay warp-uniform
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(&bars[s], 1);
         fence_mbar_init();
-        policy = policy_evict_first();
     }
     __syncwarp();
 
@@ -964,7 +964,7 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         }
         return io;
     };
-    int pp[S];                                 // kHopStencil, lane 0: patterns of the tile the producer cursor points at
+    int pp[S];                                 // kHopStencil: patterns of the tile the producer cursor points at (lane 0, or all lanes: UP)
 #pragma unroll
     for (int j = 0; j < S; ++j) pp[j] = 0;
     // the record image of a tile -> dst: one bulk copy, or (kHopStencil) per slice the on-site record from HBM
@@ -1029,7 +1029,13 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
             }
         }
     };
-    // producer cursor (lane 0): tile in sweep order, index inside the run
+    // Producer cursor: tile in sweep order, index inside the run.  UP (uniform producer): every lane keeps the cursor
+    // and only the issue itself is lane 0's, so the operands of the TMA instructions are warp-uniform and the
+    // compiler issues them from uniform registers (no per-lane loop with R2UR broadcasts around each; 2008 -> 1624
+    // SASS instructions).  Measured on c4, same box: evolve_msd 199.6 -> 192.2 ms per 10 steps, but kpm_doubling
+    // 158.5 -> 164.0 us per step (c2, c3, c5 unchanged) -- so it is taken for the (psi, chi) kernel only; elsewhere
+    // lane 0 alone keeps the cursor.
+    constexpr bool UP = MSD;
     int p_t = 0, p_k = 0;
     int p_reverse = 0;                         // sweep direction of the step being issued
     auto p_patterns = [&]() {                  // kHopStencil: pattern ids of the tile at the cursor, one tile ahead of their use
@@ -1063,17 +1069,17 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
         const int reverse = a.alternate ? ((a.sweep0 + (mm - a.m_begin)) & 1) : a.sweep0;
         int c_t = (int)blockIdx.x * a.run + warp, c_k = 0;      // consumer cursor
         int issued = 0;
-        if (lane == 0) {
+        if (UP || lane == 0) {
             p_reset(reverse);
             for (; issued < stages - 1 && issued < n_my; ++issued) {
-                issue(io, reverse, p_t, p_st);
+                if (!UP || lane == 0) issue(io, reverse, p_t, p_st);
                 p_advance();
             }
         }
         for (int i = 0; i < n_my; ++i) {
             // the stage the producer cursor points at was consumed by the whole warp in the previous iteration
-            if (lane == 0 && issued < n_my) {
-                issue(io, reverse, p_t, p_st);
+            if ((UP || lane == 0) && issued < n_my) {
+                if (!UP || lane == 0) issue(io, reverse, p_t, p_st);
                 p_advance();
                 ++issued;
             }
@@ -1091,7 +1097,6 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
             if (++c_st == stages) { c_st = 0; c_ph ^= 1u; }
             __syncwarp();
         }
-        // lane 0's producer stage index may run ahead of the other lanes' view: only lane 0 uses p_st
 
         // ---- end of the step: dots, and the barrier before the next one
         double* result = DOTS ? a.dots + (size_t)(mm - a.dot_m0) * QB : nullptr;

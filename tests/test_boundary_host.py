@@ -149,21 +149,26 @@ def test_storage_plan_regular_lattices_need_no_index_array(gq):
     MB = 1 << 20              # pretend L2 size: the stencil is only taken when a step's working set exceeds the L2
     # cubic 64^3: x-lines are two slices long -> patterns = {first, second half of a line} x {y = 0, mid, 63} x {z = 0, mid, 63}
     m = L.cubic(64, W=16.5, seed=1, energy_scale=16.0)
-    hop, nbytes, pats = gq.plan_storage(m, l2_bytes=MB)
+    hop, nbytes, pats = gq.plan_storage(m, batch=4, l2_bytes=MB)
     assert hop == STENCIL and pats == 2 * 3 * 3               # N is a multiple of 128 rows: no all-padding tail records
     assert nbytes < 8.2 * m.N + 8 * (m.N + 1)                  # 8 B on-site + 0.125 B pattern id per row (+ x)
-    hop16, nbytes16, _ = gq.plan_storage(m, l2_bytes=MB, options={"stencil": 0})
+    hop16, nbytes16, _ = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"stencil": 0})
     assert hop16 == CONST16 and nbytes16 > nbytes + 12 * m.N   # 16-bit columns: 21 B per row at K = 6
-    hop32, nbytes32, _ = gq.plan_storage(m, l2_bytes=MB, options={"stencil": 0, "idx16": 0})
+    hop32, nbytes32, _ = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"stencil": 0, "idx16": 0})
     assert hop32 == CONST32 and nbytes32 == (m.N // 32) * (256 + 128 * 6) + 8 * (m.N + 1)
     # square 1000 x 96 (lines not aligned with slices): a dozen patterns
     m = L.square(1000, 96, W=2.0, seed=2)
-    hop, nbytes, pats = gq.plan_storage(m, l2_bytes=MB)
+    hop, nbytes, pats = gq.plan_storage(m, batch=4, l2_bytes=MB)
     assert hop == STENCIL and 5 <= pats <= 40                   # where the line end falls in the slice x (first, middle, last line)
     # chain: K = 2
-    assert gq.plan_storage(L.chain(100000, W=1.0, seed=3), l2_bytes=MB)[0] == STENCIL
+    assert gq.plan_storage(L.chain(100000, W=1.0, seed=3), batch=8, l2_bytes=MB)[0] == STENCIL
     # graphene (4-atom cell, period 4 in the row index)
-    assert gq.plan_storage(L.graphene(256, 64, W=1.0, seed=4), l2_bytes=MB)[0] == STENCIL
+    assert gq.plan_storage(L.graphene(256, 64, W=1.0, seed=4), batch=4, l2_bytes=MB)[0] == STENCIL
+    # one or two vectors: a tile streams too few bytes to pay for the stencil's extra copies (the paper's example 5.1: 1.57 s
+    # with explicit columns, 2.07 s with the stencil) -- explicit columns unless forced
+    m1 = L.square(1000, 96, W=2.0, seed=2)
+    assert gq.plan_storage(m1, batch=1, l2_bytes=MB)[0] != STENCIL and gq.plan_storage(m1, batch=2, l2_bytes=MB)[0] != STENCIL
+    assert gq.plan_storage(m1, batch=1, l2_bytes=MB, options={"stencil": 2})[0] == STENCIL
     # fall-backs: vacancies (every slice its own pattern), bond disorder (per-entry hoppings), Peierls phases
     assert gq.plan_storage(L.graphene(256, 64, vacancy_fraction=0.01, vacancy_seed=5), l2_bytes=MB)[0] in (CONST32, CONST16, CONST16P)
     assert gq.plan_storage(L.with_bond_disorder(L.square(256, 64, W=1.0, seed=6), 0.3, 7), l2_bytes=MB)[0] == REAL
