@@ -390,8 +390,10 @@ __host__ __device__ constexpr int min_blocks(int B, int mode) {
 // B = 8: a slice's rows are 4 KB per stream; staging x_{m-2} as well would leave room for one CTA per
 // SM only, so x_{m-2} own rows are read by a streaming 256-bit load at the top of the round instead
 // (the occupancy is worth more than the TMA staging there; at B <= 4 it is the other way round).
-// The (psi, chi) evolve kernel does the same at every B when GPUQT_MSD_OCC is on (four staged streams
-// would leave room for one CTA per SM).
+// The (psi, chi) evolve kernel does the same at every B when GPUQT_MSD_OCC / GPUQT_MSD_V1 is on (four staged
+// streams would leave room for one CTA per SM).  Direct reads for it alone, at one CTA per SM, change nothing
+// (c4: evolve_msd 195.3 vs 197.2 ms per 10 steps); GPUQT_PREV_DIRECT = 1 for every kernel costs the KPM kernels
+// 7 % at B = 4 (158 -> 170 us per step).
 #ifndef GPUQT_PREV_DIRECT     // experiment: x_{m-2} by streaming loads at every B
 #define GPUQT_PREV_DIRECT 0
 #endif
