@@ -253,8 +253,8 @@ cudaError_t configure_mode(gpuqt_handle* h, int mode) {
     const int sb = mode_stage_bytes_for(h, mode);
     int stages = h->want_stages;
     while (stages > 1 && step_smem_bytes(stages, sb) > kSmemBudget) --stages;
-    // prefer two resident CTAs per SM over a deeper pipeline
-    while (stages > 2 && 2 * (step_smem_bytes(stages, sb) + 4096) > kSmemPerSm) --stages;
+    // prefer two resident CTAs per SM over a deeper pipeline (where the registers allow two at all)
+    while (min_blocks(h->B, mode) >= 2 && stages > 2 && 2 * (step_smem_bytes(stages, sb) + 4096) > kSmemPerSm) --stages;
     h->mode_stages[mode] = stages;
     h->mode_stage_bytes[mode] = sb;
     h->mode_smem[mode] = step_smem_bytes(stages, sb);

@@ -55,6 +55,24 @@
 #ifndef GPUQT_MSD_V1
 #define GPUQT_MSD_V1 0
 #endif
+// KPM / evolve kernels: a lane owns FOUR vectors of a row (two 256-bit accesses per operand) at B = 8 -- two lanes
+// per row instead of four halve the per-row address / predicate / column / hopping reads; 180 registers, one CTA
+// per SM (c5: kpm_left 1710 -> 1532 us per step).  GPUQT_V4 = 1 does the same at B = 4 (one lane per row, 224
+// registers): the c4 KPM step goes from 157.5 to 190.8 us (8 warps per SM hide too little latency), so it is off.
+#ifndef GPUQT_V4
+#define GPUQT_V4 0
+#endif
+#ifndef GPUQT_V4_B8
+#define GPUQT_V4_B8 1
+#endif
+// B = 8, KPM / evolve kernels: x_{m-2} rows by streaming loads (1) or staged by TMA (0).  With one CTA per SM the
+// staged form fits (10.5 KB per stage) and wins: c5 kpm_left 1530.7 (direct) -> 1505.4 us (staged), 0.94 of the copy peak
+#ifndef GPUQT_PD8
+#define GPUQT_PD8 0
+#endif
+__host__ __device__ constexpr bool lane_owns_four(int B, int mode) {
+    return mode != 3 /* kModeEvolveMsd */ && ((GPUQT_V4_B8 && B >= 8) || (GPUQT_V4 && B >= 4));
+}
 #ifndef GPUQT_MINB_MSD
 #define GPUQT_MINB_MSD ((GPUQT_MSD_OCC || GPUQT_MSD_V1) ? 2 : 1)
 #endif
@@ -384,12 +402,13 @@ struct ModeTraits {
 };
 // resident CTAs per SM the register allocation aims at
 __host__ __device__ constexpr int min_blocks(int B, int mode) {
-    return mode == kModeEvolveMsd ? GPUQT_MINB_MSD : B == 1 ? GPUQT_MINB_B1 : GPUQT_MINB;
+    return mode == kModeEvolveMsd ? GPUQT_MINB_MSD : B == 1 ? GPUQT_MINB_B1 : lane_owns_four(B, mode) ? 1 : GPUQT_MINB;
 }
 
-// B = 8: a slice's rows are 4 KB per stream; staging x_{m-2} as well would leave room for one CTA per
-// SM only, so x_{m-2} own rows are read by a streaming 256-bit load at the top of the round instead
-// (the occupancy is worth more than the TMA staging there; at B <= 4 it is the other way round).
+// B = 8, (psi, chi) kernel: a slice's rows are 4 KB per stream and four staged streams do not fit two stages, so
+// x_{m-2}, e_{m-2} own rows are read by streaming 256-bit loads at the top of the round instead.  (Round 1 did the
+// same in the KPM kernels at B = 8 to keep two CTAs per SM; with four vectors per lane there is one CTA per SM and
+// the staged form is back, see GPUQT_PD8.)
 // The (psi, chi) evolve kernel does the same at every B when GPUQT_MSD_OCC / GPUQT_MSD_V1 is on (four staged
 // streams would leave room for one CTA per SM).  Direct reads for it alone, at one CTA per SM, change nothing
 // (c4: evolve_msd 195.3 vs 197.2 ms per 10 steps); GPUQT_PREV_DIRECT = 1 for every kernel costs the KPM kernels
@@ -398,7 +417,8 @@ __host__ __device__ constexpr int min_blocks(int B, int mode) {
 #define GPUQT_PREV_DIRECT 0
 #endif
 __host__ __device__ constexpr bool prev_direct(int B, int mode) {
-    return B >= 8 || GPUQT_PREV_DIRECT || ((GPUQT_MSD_OCC || GPUQT_MSD_V1) && mode == kModeEvolveMsd);
+    return (B >= 8 && (GPUQT_PD8 || mode == kModeEvolveMsd)) || GPUQT_PREV_DIRECT ||
+           ((GPUQT_MSD_OCC || GPUQT_MSD_V1) && mode == kModeEvolveMsd);
 }
 
 // slices per tile at B = 1 on the unrolled uniform tables (2 or 4; kTilePad is a multiple): a tile's bookkeeping
@@ -410,7 +430,8 @@ __host__ __device__ constexpr bool prev_direct(int B, int mode) {
 // A tile is S consecutive slices and is walked in ROUNDS rounds of RS rows, U rounds at a time.
 template <int B, int KT, int MODE = kModeDoubling>
 struct LaneShape {
-    static constexpr int V = (B >= 2 && !(GPUQT_MSD_V1 && MODE == kModeEvolveMsd)) ? 2 : 1;
+    static constexpr int V = lane_owns_four(B, MODE) ? 4
+                             : (B >= 2 && !(GPUQT_MSD_V1 && MODE == kModeEvolveMsd)) ? 2 : 1;
     static constexpr bool SWZ = B >= 2;                    // staged rows are written by swizzled tensor copies
     static constexpr int LPR = B / V;                      // lanes per row
     static constexpr int RS = 32 / LPR;                    // rows per round
@@ -453,7 +474,14 @@ __device__ __forceinline__ CV<2> cv_lds_swz(uint32_t sa) {
 }
 template <int V, bool SWZ>
 __device__ __forceinline__ CV<V> cv_lds_staged(const double2* p) {
-    if constexpr (V == 2) {
+    if constexpr (V == 4) {                 // 64 bytes, 64-byte aligned: the four chunks stay inside one half line
+        const uint32_t p0 = swz32(smem_u32(p));
+        CV<4> v;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.re[j]), "=d"(v.im[j]) : "r"(p0 ^ (16u * j)));
+        return v;
+    } else if constexpr (V == 2) {
         return cv_lds_swz(smem_u32(p));
     } else if constexpr (SWZ) {
         CV<1> v;
@@ -483,8 +511,22 @@ __device__ __forceinline__ CV<2> cv_ld_stream<2>(const double2* p) {
                  : "l"(p));
     return v;
 }
+template <>
+__device__ __forceinline__ CV<4> cv_ld_stream<4>(const double2* p) {
+    CV<4> v;
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];"
+                 : "=d"(v.re[0]), "=d"(v.im[0]), "=d"(v.re[1]), "=d"(v.im[1]) : "l"(p));
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];"
+                 : "=d"(v.re[2]), "=d"(v.im[2]), "=d"(v.re[3]), "=d"(v.im[3]) : "l"(p + 2));
+    return v;
+}
 template <int V>
 __device__ __forceinline__ void cv_st(double2* p, const CV<V>& v);
+template <>
+__device__ __forceinline__ void cv_st<4>(double2* p, const CV<4>& v) {
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v.re[0]), "d"(v.im[0]), "d"(v.re[1]), "d"(v.im[1]) : "memory");
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p + 2), "d"(v.re[2]), "d"(v.im[2]), "d"(v.re[3]), "d"(v.im[3]) : "memory");
+}
 template <>
 __device__ __forceinline__ void cv_st<1>(double2* p, const CV<1>& v) {
     st_vec(p, make_double2(v.re[0], v.im[0]));
@@ -554,6 +596,27 @@ __device__ __forceinline__ CV<1> cv_gather<1, 64, false>(const char* g_l, uint32
 template <>
 __device__ __forceinline__ CV<1> cv_gather<1, 128, false>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
     return cv_gather_plain<128>(g_l, s_l, c, row0, RB);
+}
+template <>
+__device__ __forceinline__ CV<4> cv_gather<4, 32, true>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
+    const unsigned d = (unsigned)(c - row0);
+    const uint32_t s0 = swz32(s_l + (uint32_t)c * (uint32_t)RB);
+    const char* ga = g_l + (long long)c * RB;
+    CV<4> v;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.lt.u32 p, %10, 32;\n"
+        "@p ld.shared.v2.f64 {%0, %1}, [%8];\n"
+        "@p ld.shared.v2.f64 {%2, %3}, [%11];\n"
+        "@p ld.shared.v2.f64 {%4, %5}, [%12];\n"
+        "@p ld.shared.v2.f64 {%6, %7}, [%13];\n"
+        "@!p ld.global.L2::evict_last.v4.f64 {%0, %1, %2, %3}, [%9];\n"
+        "@!p ld.global.L2::evict_last.v4.f64 {%4, %5, %6, %7}, [%9+32];\n"
+        "}"
+        : "=d"(v.re[0]), "=d"(v.im[0]), "=d"(v.re[1]), "=d"(v.im[1]), "=d"(v.re[2]), "=d"(v.im[2]), "=d"(v.re[3]), "=d"(v.im[3])
+        : "r"(s0), "l"(ga), "r"(d), "r"(s0 ^ 16u), "r"(s0 ^ 32u), "r"(s0 ^ 48u));
+    return v;
 }
 template <>
 __device__ __forceinline__ CV<2> cv_gather<2, 32, true>(const char* g_l, uint32_t s_l, int c, int row0, int RB) {
