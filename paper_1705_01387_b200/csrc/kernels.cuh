@@ -805,10 +805,13 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
                         double hr = 1.0, hi = 0.0;                              // CONST: the factor is applied once below
                         if (!CONST) hr = s_hre[u][k * 32 + rr];
                         if (CPLX) hi = (s_hre[u] + w * 32)[k * 32 + rr];
-                        if (CONST) cv_add<V>(sum[u], v[u][kk]);
+                        // constant hopping: the first neighbour starts the sum (no 0 + x additions)
+                        if (CONST && k == 0) sum[u] = v[u][kk];
+                        else if (CONST) cv_add<V>(sum[u], v[u][kk]);
                         else cv_fma<V, CPLX>(sum[u], hr, hi, v[u][kk]);
                         if (MSD) {
-                            if (CONST) cv_add<V>(sum_e[u], ve[u][kk]);
+                            if (CONST && k == 0) sum_e[u] = ve[u][kk];
+                            else if (CONST) cv_add<V>(sum_e[u], ve[u][kk]);
                             else cv_fma<V, CPLX>(sum_e[u], hr, hi, ve[u][kk]);
                             // [X,H]_mn = (X_m - X_n) H_mn = -dx H_mn
                             const double ndx = -min_image(xn[u][kk] - xm[u], m.box);
