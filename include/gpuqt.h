@@ -160,7 +160,10 @@ int gpuqt_plan_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const
  * padding entries = (own row, 0.0).  When hop_im == NULL and every listed hopping has the same bit
  * pattern (the paper's default "all hoppings -1") no hopping array is stored and
  * padding entries point at an all-zero row N that every vector buffer carries; such a table keeps
- * its columns as int32 base + uint16 delta per (slice, k) when they spread less than 65535 there.
+ * its columns as int32 base + uint16 delta per (slice, k) when they spread less than 65535 there
+ * (0xffff = the zero row, for tables with padding entries), or -- regular lattice, batch >= 4, working
+ * set beyond the L2: gpuqt_options.stencil -- as no index array at all (per-slice pattern id + a small
+ * dictionary of relative-column patterns).  gpuqt_plan_storage reports the choice without a GPU;
  * gpuqt_get_table decodes every variant back to the canonical padded table.
  * Errors: the gpuqt_validate codes; GPUQT_ERR_ARG (batch, volume, modes, alignment, K_max too large
  * for one record per warp in shared memory), GPUQT_ERR_NOMEM (workspace too small), GPUQT_ERR_CUDA.
