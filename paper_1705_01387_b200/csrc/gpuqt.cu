@@ -23,7 +23,7 @@ void* step_kernel_fn(int mode, int B, int kt, int hop);     // step_kernels.cu
 namespace {
 
 constexpr int kMaxGrid = 4096;
-constexpr int kPartialDoubles = 64;   // 2 * Q*B <= 48 per block
+constexpr int kPartialDoubles = 96;   // 3 * Q*B <= 72 per block (three step buffers of a multi-step launch)
 constexpr int kRing = 3;              // recurrence ring x_m -> ring[(m - 1) % 3]
 constexpr int kCoefSlots = 8;         // Bessel-coefficient uploads in flight (pinned host ring + device mirror)
 

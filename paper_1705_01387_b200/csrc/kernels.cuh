@@ -201,7 +201,7 @@ struct RecArgs {
     int stage_bytes;             // bytes of one stage: records + staged vector rows
     int rec_bytes;               // bytes reserved for the records inside a stage
     int multi;                   // cooperative multi-step launch: grid barrier between steps
-    double* partials;            // [2][grid][Q*B]
+    double* partials;            // [3][grid][Q*B] (multi-step launches: by step % 3)
     unsigned int* ticket;        // single-step launches: last-block detection
     unsigned int* barrier;       // multi-step launches: monotonically increasing arrival counter (zeroed by the host)
 };
@@ -313,19 +313,22 @@ __device__ __forceinline__ void red_release_gpu_inc(unsigned int* p) {
     asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
 }
 
-// Grid-wide barrier of a cooperative launch (all CTAs co-resident).  `counter` only ever grows; the
-// e-th barrier of the launch completes when it reaches e * gridDim.x.  Release/acquire at gpu scope:
-// everything the CTA wrote before the barrier is visible to every CTA after it; the proxy fences
-// extend that to the TMA (async proxy) reads that follow.
-__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int target) {
+// Grid-wide barrier of a cooperative launch (all CTAs co-resident), in two halves so that a CTA can do work that
+// nobody waits for between its arrival and the completion (the deferred reduction of the previous step's dots).
+// `counter` only ever grows; the e-th barrier of the launch completes when it reaches e * gridDim.x.
+// Ordering: every thread's stores -> bar.sync -> thread 0's red.release.gpu (cumulative) ... thread 0's
+// ld.acquire.gpu -> bar.sync -> every thread's loads: everything the CTA wrote before the barrier is visible to every
+// CTA after it, without separate membar.gl fences; the proxy fences extend that to the TMA (async proxy) reads that
+// follow x_m's ordinary stores.
+__device__ __forceinline__ void grid_arrive(unsigned int* counter) {
     fence_proxy_async();
     __syncthreads();
+    if (threadIdx.x == 0) red_release_gpu_inc(counter);
+}
+__device__ __forceinline__ void grid_wait(unsigned int* counter, unsigned int target) {
     if (threadIdx.x == 0) {
-        __threadfence();
-        red_release_gpu_inc(counter);
         while (ld_acquire_gpu(counter) < target) {
         }
-        __threadfence();
     }
     __syncthreads();
     fence_proxy_async();
@@ -912,8 +915,19 @@ __device__ __forceinline__ void sum_partials(const double* partials, int P, doub
     const int S = kThreads / P;              // strands per value
     const int pv = tid % P, strand = tid / P;
     double s = 0.0;
-    if (strand < S)
-        for (unsigned int g = strand; g < gridDim.x; g += S) s += __ldcg(&partials[(size_t)g * P + pv]);
+    if (strand < S) {
+        // four independent loads in flight, added in the order of g (a missing block adds +0.0)
+        for (unsigned int g = strand; g < gridDim.x; g += 4 * S) {
+            double v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const unsigned int gg = g + j * S;
+                v[j] = gg < gridDim.x ? __ldcg(&partials[(size_t)gg * P + pv]) : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) s += v[j];
+        }
+    }
     s_tree[tid] = (strand < S) ? s : 0.0;
     __syncthreads();
     if (tid < P) {
@@ -1186,14 +1200,22 @@ __global__ void __launch_bounds__(kThreads, min_blocks(B, MODE)) cheb_step_kerne
                 }
             }
         } else {
-            double* part = a.partials + (size_t)(mm & 1) * G * QB;
+            // per-block partials of step mm -> buffer mm % 3; block (mm - 1) % G sums the partials of step mm - 1
+            // (complete since the previous barrier) between its arrival at this barrier and the barrier's completion,
+            // where nobody waits for it; the last step's partials are summed after the last barrier.  Three buffers:
+            // buffer (mm - 1) % 3 is written again at the end of step mm + 2, after a barrier the summing block has
+            // arrived at only after its sum.
+            double* part = a.partials + (size_t)(mm % 3) * G * QB;
             if (DOTS) {
                 warp_flush<B, Q, V>(red, s_part + warp * QB, lane);
                 block_partial(s_part, QB, part);
             }
             ++epoch;
-            grid_barrier(a.barrier, epoch * (unsigned int)G);
-            if (DOTS && (int)blockIdx.x == mm % G) sum_partials(part, QB, result);
+            grid_arrive(a.barrier);
+            if (DOTS && mm > a.m_begin && (int)blockIdx.x == (mm - 1) % G)
+                sum_partials(a.partials + (size_t)((mm - 1) % 3) * G * QB, QB, result - QB);
+            grid_wait(a.barrier, epoch * (unsigned int)G);
+            if (DOTS && mm + 1 == a.m_end && (int)blockIdx.x == mm % G) sum_partials(part, QB, result);
         }
     }
 }
