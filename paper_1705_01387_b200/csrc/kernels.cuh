@@ -2,9 +2,10 @@
 // the layout, the byte model and the roofline of each kernel.
 //
 // Layout
-//   vectors   complex fp64 [N + 1][B] as double2: the B vectors of a row are contiguous (16*B bytes),
-//             so one neighbour index serves one 16*B-byte gather (B = 8: one 128-byte line).  Row N
-//             of every buffer is all zero and never written.
+//   vectors   complex fp64 [NV + 1][B] as double2: the B vectors of a row are contiguous (16*B bytes),
+//             so one neighbour index serves one 16*B-byte gather (B = 8: one 128-byte line).  Row NV
+//             of every buffer is all zero and never written (NV = N; a row slab of a decomposed lattice
+//             keeps its halo rows N .. NV-1 in between, see Mat).
 //   matrix    packed sliced ELL.  A slice is 32 consecutive rows; slice s of width w is ONE
 //             contiguous record, column-major inside the record:
 //                 double hre[w][32] (per-entry variants) | double him[w][32] (complex variant) |
@@ -13,7 +14,7 @@
 //             of 128.  Records are stored back to back; slice_off[s] is the byte offset of record
 //             s.  Padding entries are (own row, hop 0.0); in the constant-hopping variants (nd = 0:
 //             every stored hopping is the same real number, kept in Mat::hop_const) padding is
-//             col = N, the zero row (and x[N] = 0), so the walk needs no guard.  The table is padded
+//             col = NV, the zero row (and x[NV] = 0), so the walk needs no guard.  The table is padded
 //             with all-padding records up to a multiple of kTilePad slices, so a tile of several
 //             slices is always one contiguous copy.
 //   warp      the unit of work is (warp, tile); a tile is S consecutive slices (S = 2 at B = 1 on
@@ -22,8 +23,9 @@
 //             of x_{m-1} (and e_{m-1}) and of x_{m-2} (and e_{m-2}) -- TMA copies (cp.async.bulk +
 //             mbarrier) issued by the warp's lane 0 one or more tiles ahead, so the streams never sit
 //             on the warp's scoreboard and there is no CTA-wide barrier in the loop.  A warp walks the
-//             tile in rounds of 32/LPR rows; a lane owns V = 2 consecutive vectors of a row (256-bit
-//             accesses) and LPR = B/V lanes share a row; at B = 1 the two rounds of a tile are walked
+//             tile in rounds of 32/LPR rows; a lane owns V consecutive vectors of a row (V = 1 at B = 1;
+//             2 at B = 2, 4: one 256-bit access per operand; 4 at B = 8 in the KPM / evolve kernels: two)
+//             and LPR = B/V lanes share a row; at B = 1 the two rounds of a tile are walked
 //             together (all gathers of both first, then the arithmetic) for memory-level parallelism.
 //             Neighbours inside the tile are read from the staged rows in shared memory; the others
 //             are gathered from global memory (L2 hits along the sweep front).
