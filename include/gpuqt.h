@@ -184,6 +184,14 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
  * psi = phi, chi = 0, a = phi, b = V phi (Eq. 34).  phi: [batch][N][2].                          */
 int gpuqt_set_state(gpuqt_handle* h, const double* phi_host);
 int gpuqt_set_state_device(gpuqt_handle* h, const double* phi_device);
+/* The same in two halves, for the loop over the N_r random vector sets of a run: the upload of
+ * the NEXT batch overlaps the computation on the current one.  gpuqt_prefetch_state starts an asynchronous copy of
+ * phi_host (pinned host memory, [batch][N][2]; must stay valid and unchanged until the matching
+ * gpuqt_set_state_prefetched) into a staging buffer of the workspace on a stream the handle owns, and returns at
+ * once; gpuqt_set_state_prefetched makes the handle's stream wait for that copy and then does what gpuqt_set_state
+ * does after its copy.  GPUQT_ERR_STATE without a pending prefetch.                                           */
+int gpuqt_prefetch_state(gpuqt_handle* h, const double* phi_host);
+int gpuqt_set_state_prefetched(gpuqt_handle* h);
 
 /* C_n^DOS = <psi|T_n(H~)|psi>, n < n_moments (Eq. 28) at the current psi (= phi when
  * called before any gpuqt_evolve).  out: host [batch][n_moments].  2 <= n_moments <= MAX.        */

@@ -63,6 +63,8 @@ _SIGNATURES = {
         C.c_double, C.c_double, C.c_int32, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(Options)]),
     "gpuqt_set_state": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gpuqt_set_state_device": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "gpuqt_prefetch_state": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "gpuqt_set_state_prefetched": (C.c_int, [C.c_void_p]),
     "gpuqt_dos_moments": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_evolve": (C.c_int, [C.c_void_p, C.c_double, C.c_int32]),
     "gpuqt_vac": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
@@ -236,6 +238,16 @@ class GpuQT:
             assert phi.device.type == "cpu" and phi.is_contiguous() and phi.dtype == self._torch.float64
             assert tuple(phi.shape) == (self.batch, self.N, 2)
             self._ck(load().gpuqt_set_state(self._h, C.c_void_p(phi.data_ptr())), "gpuqt_set_state")
+
+    def prefetch_state(self, phi):
+        """Start the asynchronous upload of the next batch (pinned CPU torch tensor [batch][N][2]); keep it alive."""
+        assert phi.device.type == "cpu" and phi.is_pinned() and phi.is_contiguous() and phi.dtype == self._torch.float64
+        assert tuple(phi.shape) == (self.batch, self.N, 2)
+        self._prefetch_keep = phi
+        self._ck(load().gpuqt_prefetch_state(self._h, C.c_void_p(phi.data_ptr())), "gpuqt_prefetch_state")
+
+    def set_state_prefetched(self):
+        self._ck(load().gpuqt_set_state_prefetched(self._h), "gpuqt_set_state_prefetched")
 
     def set_state_device(self, phi):
         assert phi.is_cuda and phi.is_contiguous() and phi.dtype == self._torch.float64

@@ -65,6 +65,12 @@ struct gpuqt_handle {
     double2 *psi = nullptr, *chi = nullptr, *va = nullptr, *vb = nullptr, *phiL = nullptr;
     double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr},
             *ringe[kRing] = {nullptr, nullptr, nullptr};
+    // gpuqt_prefetch_state: the next batch of random vectors, copied on the library's own stream while the
+    // caller's stream computes
+    double2* stage_in = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_copy_done = nullptr, ev_stage_free = nullptr;
+    bool prefetched = false, stage_read = false;
     // library-owned scratch for the small transform / table-decode calls: grown on demand, kept
     // (stream-ordered pool allocations can trim at every synchronisation and stall the step)
     char* scratch = nullptr;
@@ -110,7 +116,7 @@ int cuda_fail(gpuqt_handle* h, cudaError_t e, const char* what) {
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 int n_vectors(int modes) {
-    int n = 2 + kRing;                              // psi, out0, ring
+    int n = 3 + kRing;                              // psi, out0, ring, the staging buffer of gpuqt_prefetch_state
     if (modes & GPUQT_MODE_MSD) n += 2 + kRing;     // chi, out1, ringe
     if (modes & GPUQT_MODE_VAC) n += 3;             // a, b, phi_L
     return n;
@@ -631,11 +637,11 @@ int copy_moments_out(gpuqt_handle* h, int n_moments, double* out_host) {
     return GPUQT_OK;
 }
 
-int finish_set_state(gpuqt_handle* h) {
-    // ring[0] holds phi in [batch][N] order
+int finish_set_state(gpuqt_handle* h, const double2* src) {
+    // src holds phi in [batch][N] order
     const long long total = (long long)h->vec_elems;
     const int blocks = (int)((total + 255) / 256);
-    to_device_layout<<<blocks, 256, 0, h->stream>>>(h->N, h->B, h->ring[0], h->psi);
+    to_device_layout<<<blocks, 256, 0, h->stream>>>(h->N, h->B, src, h->psi);
     CU(cudaGetLastError());
     if (h->modes & GPUQT_MODE_MSD) {
         zero_vec<<<blocks, 256, 0, h->stream>>>(total, h->chi);
@@ -884,6 +890,7 @@ int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, 
     if (modes & GPUQT_MODE_VAC) {
         h->va = nextv(); h->vb = nextv(); h->phiL = nextv();
     }
+    h->stage_in = nextv();
     h->partials = (double*)(base + L.partials);
     h->dots = (double*)(base + L.dots);
     h->moments = (double*)(base + L.moments);
@@ -905,13 +912,40 @@ extern "C" {
 int gpuqt_set_state(gpuqt_handle* h, const double* phi_host) {
     if (!h || !phi_host) return fail(h, GPUQT_ERR_ARG, "null argument");
     CU(cudaMemcpyAsync(h->ring[0], phi_host, h->vec_elems * sizeof(double2), cudaMemcpyHostToDevice, h->stream));
-    return finish_set_state(h);
+    return finish_set_state(h, h->ring[0]);
+}
+
+int gpuqt_prefetch_state(gpuqt_handle* h, const double* phi_host) {
+    if (!h || !phi_host) return fail(h, GPUQT_ERR_ARG, "null argument");
+    if (!h->copy_stream) {
+        CU(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&h->ev_copy_done, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&h->ev_stage_free, cudaEventDisableTiming));
+    }
+    // the staging buffer may still be read by the layout kernel of the previous gpuqt_set_state_prefetched
+    if (h->stage_read) CU(cudaStreamWaitEvent(h->copy_stream, h->ev_stage_free, 0));
+    CU(cudaMemcpyAsync(h->stage_in, phi_host, h->vec_elems * sizeof(double2), cudaMemcpyHostToDevice, h->copy_stream));
+    CU(cudaEventRecord(h->ev_copy_done, h->copy_stream));
+    h->prefetched = true;
+    return GPUQT_OK;
+}
+
+int gpuqt_set_state_prefetched(gpuqt_handle* h) {
+    if (!h) return GPUQT_ERR_ARG;
+    if (!h->prefetched) return fail(h, GPUQT_ERR_STATE, "gpuqt_prefetch_state has not been called since the last gpuqt_set_state_prefetched");
+    CU(cudaStreamWaitEvent(h->stream, h->ev_copy_done, 0));
+    int rc = finish_set_state(h, h->stage_in);
+    if (rc) return rc;
+    CU(cudaEventRecord(h->ev_stage_free, h->stream));     // psi = layout(stage_in) has been launched: the buffer is free after it
+    h->stage_read = true;
+    h->prefetched = false;
+    return GPUQT_OK;
 }
 
 int gpuqt_set_state_device(gpuqt_handle* h, const double* phi_device) {
     if (!h || !phi_device) return fail(h, GPUQT_ERR_ARG, "null argument");
     CU(cudaMemcpyAsync(h->ring[0], phi_device, h->vec_elems * sizeof(double2), cudaMemcpyDeviceToDevice, h->stream));
-    return finish_set_state(h);
+    return finish_set_state(h, h->ring[0]);
 }
 
 int gpuqt_dos_moments(gpuqt_handle* h, int32_t n_moments, double* out_host) {
@@ -1139,6 +1173,12 @@ void gpuqt_destroy(gpuqt_handle* h) {
     if (h->coef_dev) cudaFree(h->coef_dev);
     if (h->scratch) cudaFree(h->scratch);
     if (h->d_maps) cudaFree(h->d_maps);
+    if (h->copy_stream) {
+        cudaStreamSynchronize(h->copy_stream);
+        cudaStreamDestroy(h->copy_stream);
+    }
+    if (h->ev_copy_done) cudaEventDestroy(h->ev_copy_done);
+    if (h->ev_stage_free) cudaEventDestroy(h->ev_stage_free);
     delete h;
 }
 

@@ -196,6 +196,34 @@ def test_transform(gq, oracle_mod):
     g.close()
 
 
+def test_prefetched_state_equals_set_state(gq):
+    """gpuqt_prefetch_state + gpuqt_set_state_prefetched (upload on the library's copy stream, overlapping compute)
+    leave exactly the state gpuqt_set_state does -- also when a prefetch is issued while the previous batch computes."""
+    import torch
+    model = L.cubic(13, W=16.5, seed=4, energy_scale=16.0)
+    a = gq.GpuQT(model, batch=4, modes=gq.MODE_VAC | gq.MODE_MSD, options=opts())
+    b = gq.GpuQT(model, batch=4, modes=gq.MODE_VAC | gq.MODE_MSD, options=opts())
+    with pytest.raises(gq.GpuqtError):
+        b.set_state_prefetched()                         # nothing pending
+    batches = [torch.from_numpy(L.random_phase_vectors(model.N, 4, 91, 4 * i)).pin_memory() for i in range(3)]
+    b.prefetch_state(batches[0])
+    for i, phi in enumerate(batches):
+        a.set_state(phi)
+        b.set_state_prefetched()
+        if i + 1 < len(batches):
+            b.prefetch_state(batches[i + 1])             # overlaps the work below
+        for g in (a, b):
+            g.evolve(0.7, 20)
+        assert a.msd(32).tobytes() == b.msd(32).tobytes()
+        assert a.vac(32).tobytes() == b.vac(32).tobytes()
+        for which in (gq.STATE_PSI, gq.STATE_CHI, gq.STATE_VAC_A, gq.STATE_VAC_B):
+            assert a.get_state(which).tobytes() == b.get_state(which).tobytes()
+    with pytest.raises(gq.GpuqtError):
+        b.set_state_prefetched()                         # consumed
+    a.close()
+    b.close()
+
+
 def test_errors_and_call_order(gq):
     model = L.square(10, 10, W=1.0, seed=1)
     g = gq.GpuQT(model, batch=1, modes=gq.MODE_MSD)
