@@ -9,9 +9,12 @@
 //      (st.release.sys after a system fence; the pushes before it in the stream are complete), and one halo_wait_kernel
 //      per slab spins (ld.acquire.sys) until every remote sender has published it.
 // Slabs of one group share a stream, so their pushes are ordered before the next step without flags.  Write-after-read
-// on a halo: push number e into ring slot s overwrites what push e-3 put there; the sender runs step e only after the
-// receiver published push e-1, which the receiver issues after its step e-1 -- the last reader of slot s's old contents
-// (step e-2) has completed by then.
+// on a halo, remote case: a push of exchange e is issued after the sender's wait of exchange e-1, i.e. after the receiver
+// published e-1, i.e. after everything the receiver ran BEFORE its exchange e-1.  Inside a recurrence push e goes to ring
+// slot (e-1) % 3, whose previous contents (exchange e-3) were last read by the receiver's step e-2, before its exchange
+// e-1: safe.  Across calls the same buffer could be exchanged twice with only one exchange in between and a reader after
+// it (the last step of one recurrence, the first exchange of the next), so every top-level phase starts with
+// slab_fence(): an exchange without pushes, after which every peer has finished all it ran before.
 
 namespace {
 
@@ -135,6 +138,25 @@ int slab_exchange(gpuqt_slab_group* g, const std::vector<const double2*>& bufs) 
     return GPUQT_OK;
 }
 
+// all remote peers have completed everything they issued before their matching slab_fence (no-op without remote peers)
+int slab_fence(gpuqt_slab_group* g) {
+    bool any = false;
+    for (int r : g->n_remote) any = any || r > 0;
+    if (!any) return GPUQT_OK;
+    ++g->epoch;
+    for (size_t i = 0; i < g->h.size(); ++i)
+        if (g->n_remote[i] > 0) {
+            halo_signal_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[i], g->d_signal[i], g->epoch);
+            GCU(cudaGetLastError());
+        }
+    for (size_t i = 0; i < g->h.size(); ++i)
+        if (g->n_remote[i] > 0) {
+            halo_wait_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[i], g->d_flags[i], g->d_senders[i], g->epoch);
+            GCU(cudaGetLastError());
+        }
+    return GPUQT_OK;
+}
+
 template <class F>
 std::vector<const double2*> each_buffer(gpuqt_slab_group* g, F sel) {      // sel(i) = the buffer of local slab i
     std::vector<const double2*> v;
@@ -153,7 +175,8 @@ int slab_recurrence(gpuqt_slab_group* g, int mode, std::vector<RecArgs>& args) {
         fill_rec_args(g->h[i], args[i]);
         args[i].multi = 0;
     }
-    int rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return args[i].x0; }));
+    int rc = slab_fence(g);
+    if (rc == GPUQT_OK) rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return args[i].x0; }));
     if (rc == GPUQT_OK && pair) rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return args[i].e0; }));
     if (rc) return rc;
     for (int m = 1; m < terms; ++m) {
@@ -407,7 +430,8 @@ int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host) {
         h->state_set = true;
     }
     if (g->modes & GPUQT_MODE_VAC) {          // b = V phi needs the halo rows of phi
-        int rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return (const double2*)g->h[i]->psi; }));
+        int rc = slab_fence(g);
+        if (rc == GPUQT_OK) rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return (const double2*)g->h[i]->psi; }));
         if (rc) return rc;
         for (size_t i = 0; i < n; ++i) GCU(launch_velocity(g->h[i], g->h[i]->psi, g->h[i]->vb));
     }
@@ -440,7 +464,8 @@ int gpuqt_slab_vac(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
     if (rc) return rc;
     const size_t n = g->h.size();
     // phi_L = V a (needs the halo rows of a); C_0 = <phi_L|b>
-    rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return (const double2*)g->h[i]->va; }));
+    rc = slab_fence(g);
+    if (rc == GPUQT_OK) rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return (const double2*)g->h[i]->va; }));
     if (rc) return rc;
     std::vector<RecArgs> args(n);
     for (size_t i = 0; i < n; ++i) {
