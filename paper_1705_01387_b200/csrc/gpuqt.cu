@@ -164,7 +164,8 @@ bool unrolled_width(int K) { return K == 2 || K == 3 || K == 4 || K == 6; }
 cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
     static std::mutex mu;
     static std::map<void*, size_t> granted;
-    if (bytes <= 48 * 1024) return cudaSuccess;
+    // below 32 KB the default 48 KB limit holds even with the kernels' static shared memory (<= 9 KB) on top
+    if (bytes <= 32 * 1024) return cudaSuccess;
     std::lock_guard<std::mutex> lock(mu);
     size_t& g = granted[fn];
     if (bytes <= g) return cudaSuccess;

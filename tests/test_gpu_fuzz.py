@@ -1,0 +1,97 @@
+"""GPU parity on random sparse Hermitian graphs (workloads/lattices.py::random_graph): rows of 0 .. K neighbours in
+random order, random real or complex hoppings, random on-site energies and positions, sizes from 1 row to a few
+thousand with ragged tails, every batch size, all three launch forms -- the storage variants and the generic-width walk
+get inputs no lattice produces.  Same norms and tolerance as tests/test_gpu_parity.py (1e-10, A22); the table decode
+is bit-exact.
+"""
+import numpy as np
+import pytest
+
+from workloads import lattices as L
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+PATHS = {"streaming": {"small": 0, "persistent": 0}, "small_path": {"small": 1, "persistent": 0},
+         "persistent": {"small": 0, "persistent": 1}}
+
+#        N     K  seed complex fill  locality batch
+CASES = [(1,    2, 11, False, 0.7, 0,  1),
+         (31,   3, 12, True,  0.9, 0,  2),
+         (33,   1, 13, False, 1.0, 0,  4),
+         (64,   8, 14, True,  0.6, 9,  8),
+         (257,  5, 15, False, 0.8, 0,  1),
+         (700,  7, 16, True,  0.9, 50, 4),
+         (1500, 6, 17, False, 0.7, 33, 8),
+         (2049, 4, 18, True,  0.5, 0,  2),
+         (3000, 3, 19, False, 0.9, 64, 1),
+         (4100, 2, 20, True,  1.0, 5,  8)]
+
+
+@pytest.fixture(scope="module")
+def gq():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1705_01387_b200 as g
+    return g
+
+
+def vec_err(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("N,K,seed,cplx,fill,loc,batch", CASES, ids=[f"N{c[0]}-K{c[1]}-B{c[6]}{'-c' if c[3] else ''}" for c in CASES])
+def test_random_graph_matches_the_oracle(gq, oracle_mod, N, K, seed, cplx, fill, loc, batch, path):
+    model = L.random_graph(N, K, seed, complex_hops=cplx, degree_fill=fill, locality=loc, open_x=(seed % 2 == 1))
+    phi = L.random_phase_vectors(model.N, batch, 90 + seed, 0)
+    g = gq.GpuQT(model, batch=batch, modes=gq.MODE_VAC | gq.MODE_MSD, options=PATHS[path])
+    o = oracle_mod.Oracle(model, batch=batch, modes=oracle_mod.MODE_VAC | oracle_mod.MODE_MSD)
+    # table: bit-exact decode of whatever storage variant was chosen
+    col, re, im, dx = g.get_table()
+    oc, ore, oim, odx = o.get_table()
+    assert np.array_equal(col, oc) and re.tobytes() == ore.tobytes() and im.tobytes() == oim.tobytes() and dx.tobytes() == odx.tobytes()
+    g.set_state(phi)
+    o.set_state(phi)
+    nm, order, dt = 40, 18, 0.6
+    assert np.max(np.abs(g.dos_moments(nm) - o.dos_moments(nm))) / model.N <= TOL
+    for step in range(2):
+        va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+        scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(batch)])
+        scale = np.where(scale > 0, scale, 1.0)                       # a site without bonds has V phi = 0
+        assert np.max(np.abs(g.vac(nm) - o.vac(nm)) / scale[:, None]) <= TOL
+        g.evolve(dt if step == 0 else -0.3, order)
+        o.evolve(dt if step == 0 else -0.3, order)
+        chi = o.get_state(oracle_mod.CHI)
+        cs = np.sum(chi * chi, axis=(1, 2))
+        cs = np.where(cs > 0, cs, 1.0)
+        assert np.max(np.abs(g.msd(nm) - o.msd(nm)) / cs[:, None]) <= TOL
+    for which, ow in ((gq.STATE_PSI, oracle_mod.PSI), (gq.STATE_CHI, oracle_mod.CHI), (gq.STATE_VAC_A, oracle_mod.VAC_A),
+                      (gq.STATE_VAC_B, oracle_mod.VAC_B)):
+        ref = o.get_state(ow)
+        if np.max(np.abs(ref)) > 0:
+            assert vec_err(g.get_state(which), ref) <= TOL
+        else:
+            assert np.max(np.abs(g.get_state(which))) == 0.0
+    g.close()
+    o.close()
+
+
+@pytest.mark.parametrize("n_slabs", [2, 3])
+def test_random_graph_in_slabs(gq, oracle_mod, n_slabs):
+    """Non-local random bonds: every slab has halo rows from every other slab, in no particular order."""
+    from paper_1705_01387_b200 import slab
+    model = L.random_graph(1500, 5, 31, complex_hops=True, degree_fill=0.9, locality=0, open_x=True)
+    phi = L.random_phase_vectors(model.N, 2, 95, 0)
+    g = slab.SlabGroup(model, slab.partition(model, n_slabs), batch=2, modes=gq.MODE_MSD)
+    o = oracle_mod.Oracle(model, batch=2, modes=oracle_mod.MODE_MSD)
+    g.set_state(phi)
+    o.set_state(phi)
+    g.evolve(0.5, 16)
+    o.evolve(0.5, 16)
+    chi = o.get_state(oracle_mod.CHI)
+    assert np.max(np.abs(g.msd(32) - o.msd(32)) / np.sum(chi * chi, axis=(1, 2))[:, None]) <= TOL
+    assert vec_err(g.get_state(gq.STATE_CHI, model.N), chi) <= TOL
+    g.close()
+    o.close()

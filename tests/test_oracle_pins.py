@@ -28,6 +28,8 @@ def models():
         L.graphene(3, 3, W=1.0, seed=14),                     # explicit real hoppings -2.7
         L.graphene(4, 3, vacancy_fraction=0.1, vacancy_seed=5),  # rows with 0-3 neighbours
         L.chain(9, W=0.5, seed=15),
+        L.random_graph(40, 5, 16, complex_hops=True, degree_fill=0.8),    # random bonds, rows of 0..5 neighbours in random order
+        L.random_graph(37, 3, 17, complex_hops=False, degree_fill=0.9, locality=6, open_x=False),
     ]
 
 

@@ -131,3 +131,26 @@ def test_bond_disorder_is_hermitian_and_not_constant():
     assert np.unique(h[valid]).size > 10
     assert np.all(np.abs(h[valid] / -2.7 - 1.0) <= 0.2 + 1e-12)
     assert np.all(h[~valid] == 0.0)
+
+
+def test_random_graph_generator_is_hermitian_and_reproducible():
+    """workloads.random_graph (fuzz input of tests/test_gpu_fuzz.py): degrees within K, no self or double bonds,
+    H_nm = conj(H_mn) bit for bit, the stated Gershgorin margin, same seed -> same arrays."""
+    for cplx in (False, True):
+        m = L.random_graph(300, 6, 41, complex_hops=cplx, degree_fill=0.8, locality=20)
+        again = L.random_graph(300, 6, 41, complex_hops=cplx, degree_fill=0.8, locality=20)
+        assert m.nbr_index.tobytes() == again.nbr_index.tobytes() and m.hop_re.tobytes() == again.hop_re.tobytes()
+        idx = m.nbr_index.reshape(m.N, m.K)
+        assert m.nbr_count.max() <= m.K and m.nbr_count.min() >= 0
+        g = np.zeros(m.N)
+        for i in range(m.N):
+            row = idx[i, :m.nbr_count[i]]
+            assert len(set(row)) == len(row) and i not in row and np.all(idx[i, m.nbr_count[i]:] == -1)
+            for k, j in enumerate(row):
+                back = list(idx[j, :m.nbr_count[j]]).index(i)
+                assert m.hop_re[i * m.K + k] == m.hop_re[j * m.K + back]
+                if cplx:
+                    assert m.hop_im[i * m.K + k] == -m.hop_im[j * m.K + back]
+                g[i] += np.hypot(m.hop_re[i * m.K + k], m.hop_im[i * m.K + k] if cplx else 0.0)
+        assert np.max(g + np.abs(m.onsite)) < m.energy_scale
+        assert (m.hop_im is not None) == cplx

@@ -347,3 +347,48 @@ def _gaussian_potential(xy, Lx, Ly, centres, eps, xi):
             ok = valid & (r2 <= rc * rc)
             np.add.at(U, site[ok], eps[ok] * np.exp(-r2[ok] / (2.0 * xi * xi)))
     return U
+
+
+# --------------------------------------------------------------------------- random sparse Hermitian graphs
+def random_graph(N: int, K: int, seed: int, complex_hops: bool = False, degree_fill: float = 0.7,
+                 locality: int = 0, open_x: bool = True) -> TBModel:
+    """A random sparse Hermitian tight-binding model for fuzzing the storage paths: every site proposes bonds to
+    random partners (anywhere, or within `locality` rows), a bond is kept while both ends have fewer than K
+    neighbours, hoppings are random (real, or complex with conj symmetry bit for bit), on-site energies random,
+    positions random in a box (open boundary by default, so every X_n - X_m is unambiguous).  Rows with 0 .. K
+    neighbours in random order; not a lattice the paper discusses, only an input the library must handle
+    (PAPER.md:256 'the inputs are made as general as possible')."""
+    u = rng.uniform01(seed, 4 * N * K + 4 * N + 8)
+    nbrs = [[] for _ in range(N)]
+    hops = {}
+    pos = 0
+    for m in range(N):
+        for _ in range(K):
+            r0, r1, r2, r3 = u[pos:pos + 4]
+            pos += 4
+            if r0 > degree_fill:
+                continue
+            n = int(r1 * N) if locality <= 0 else (m + 1 + int(r1 * locality)) % N
+            if n == m or n in nbrs[m] or len(nbrs[m]) >= K or len(nbrs[n]) >= K:
+                continue
+            h = complex(-0.5 - r2, (r3 - 0.5) if complex_hops else 0.0)
+            nbrs[m].append(n)
+            nbrs[n].append(m)
+            hops[(m, n)] = h
+            hops[(n, m)] = h.conjugate()
+    count = np.array([len(v) for v in nbrs], dtype=np.int32)
+    index = np.full((N, K), -1, dtype=np.int32)
+    hre = np.zeros((N, K))
+    him = np.zeros((N, K))
+    for m in range(N):
+        for k, n in enumerate(nbrs[m]):
+            index[m, k] = n
+            hre[m, k] = hops[(m, n)].real
+            him[m, k] = hops[(m, n)].imag
+    tail = u[4 * N * K:]
+    onsite = tail[:N] - 0.5
+    x = np.cumsum(0.25 + tail[N:2 * N]) if locality > 0 else 100.0 * tail[N:2 * N]
+    dE = 1.05 * float(np.max(np.abs(onsite) + np.sum(np.hypot(hre, him), axis=1))) + 0.1
+    box = 0.0 if open_x else 4.0 * float(np.max(x) - np.min(x)) + 4.0     # a box so wide that no image is closer
+    return _pack(f"random_N{N}_K{K}_s{seed}{'_c' if complex_hops else ''}", count, index, hre,
+                 him if complex_hops else None, onsite, x, box, float(N), dE)
