@@ -95,3 +95,44 @@ def test_random_graph_in_slabs(gq, oracle_mod, n_slabs):
     assert vec_err(g.get_state(gq.STATE_CHI, model.N), chi) <= TOL
     g.close()
     o.close()
+
+
+#           N     K  seed fill loc  batch hop   options
+OPT_CASES = [(2048, 6, 51, 1.0, 40,  4, -1.0, {"stencil": 2}),                       # forced pattern dictionary on an irregular table
+             (1024, 4, 52, 0.6, 0,   1, -1.0, {"stencil": 2, "persistent": 1, "small": 0}),
+             (4096, 3, 53, 0.9, 900, 2, -2.7, {"idx16": 1, "small": 0}),              # 16-bit columns with padding sentinels
+             (4096, 3, 53, 0.9, 900, 2, -2.7, {"idx16": 0, "small": 0}),
+             (70001, 6, 54, 0.8, 0, 8, -1.0, {"small": 0, "stages": 1}),               # column spread beyond 16 bits -> int32
+             (1999, 2, 55, 0.7, 3,   4, 0.5,  {"small": 0, "stages": 4, "run": 32}),
+             (2500, 4, 56, 0.9, 100, 1, -1.0, {"small": 0, "persistent": 1, "run": 8, "blocks_per_sm": 1, "alternate": 0}),
+             (900,  12, 57, 0.9, 0,  8, None, {"small": 0}),                           # wide rows, complex: generic-width walk
+             (300,  16, 58, 1.0, 0,  2, None, {"small": 0, "persistent": 1}),
+             (128,  10, 59, 0.8, 0,  4, -1.0, {"hop_const": 0}),                       # constant hopping stored per entry
+             ]
+
+
+@pytest.mark.parametrize("N,K,seed,fill,loc,batch,hop,options", OPT_CASES,
+                         ids=[f"N{c[0]}-K{c[1]}-B{c[5]}-" + "_".join(f"{k}{v}" for k, v in c[7].items()) for c in OPT_CASES])
+def test_random_graph_storage_variants_and_options(gq, oracle_mod, N, K, seed, fill, loc, batch, hop, options):
+    model = L.random_graph(N, K, seed, complex_hops=(hop is None), degree_fill=fill, locality=loc, hop_value=hop)
+    phi = L.random_phase_vectors(model.N, batch, 190 + seed, 0)
+    g = gq.GpuQT(model, batch=batch, modes=gq.MODE_VAC | gq.MODE_MSD, options=options)
+    o = oracle_mod.Oracle(model, batch=batch, modes=oracle_mod.MODE_VAC | oracle_mod.MODE_MSD)
+    col, re, im, dx = g.get_table()
+    oc, ore, oim, odx = o.get_table()
+    assert np.array_equal(col, oc) and re.tobytes() == ore.tobytes() and im.tobytes() == oim.tobytes() and dx.tobytes() == odx.tobytes()
+    g.set_state(phi)
+    o.set_state(phi)
+    nm = 64
+    assert np.max(np.abs(g.dos_moments(nm) - o.dos_moments(nm))) / model.N <= TOL
+    g.evolve(0.8, 22)
+    o.evolve(0.8, 22)
+    va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+    scale = np.array([np.linalg.norm(o.apply_v(va[b])) * np.linalg.norm(vb[b]) for b in range(batch)])
+    assert np.max(np.abs(g.vac(nm) - o.vac(nm)) / scale[:, None]) <= TOL
+    chi = o.get_state(oracle_mod.CHI)
+    assert np.max(np.abs(g.msd(nm) - o.msd(nm)) / np.sum(chi * chi, axis=(1, 2))[:, None]) <= TOL
+    assert vec_err(g.get_state(gq.STATE_CHI), chi) <= TOL
+    assert vec_err(g.get_state(gq.STATE_VAC_B), vb) <= TOL
+    g.close()
+    o.close()

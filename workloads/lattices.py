@@ -351,7 +351,7 @@ def _gaussian_potential(xy, Lx, Ly, centres, eps, xi):
 
 # --------------------------------------------------------------------------- random sparse Hermitian graphs
 def random_graph(N: int, K: int, seed: int, complex_hops: bool = False, degree_fill: float = 0.7,
-                 locality: int = 0, open_x: bool = True) -> TBModel:
+                 locality: int = 0, open_x: bool = True, hop_value: Optional[float] = None) -> TBModel:
     """A random sparse Hermitian tight-binding model for fuzzing the storage paths: every site proposes bonds to
     random partners (anywhere, or within `locality` rows), a bond is kept while both ends have fewer than K
     neighbours, hoppings are random (real, or complex with conj symmetry bit for bit), on-site energies random,
@@ -372,6 +372,8 @@ def random_graph(N: int, K: int, seed: int, complex_hops: bool = False, degree_f
             if n == m or n in nbrs[m] or len(nbrs[m]) >= K or len(nbrs[n]) >= K:
                 continue
             h = complex(-0.5 - r2, (r3 - 0.5) if complex_hops else 0.0)
+            if hop_value is not None:              # one hopping value everywhere: the constant-hopping record variants
+                h = complex(hop_value, 0.0)
             nbrs[m].append(n)
             nbrs[n].append(m)
             hops[(m, n)] = h
@@ -390,5 +392,6 @@ def random_graph(N: int, K: int, seed: int, complex_hops: bool = False, degree_f
     x = np.cumsum(0.25 + tail[N:2 * N]) if locality > 0 else 100.0 * tail[N:2 * N]
     dE = 1.05 * float(np.max(np.abs(onsite) + np.sum(np.hypot(hre, him), axis=1))) + 0.1
     box = 0.0 if open_x else 4.0 * float(np.max(x) - np.min(x)) + 4.0     # a box so wide that no image is closer
-    return _pack(f"random_N{N}_K{K}_s{seed}{'_c' if complex_hops else ''}", count, index, hre,
-                 him if complex_hops else None, onsite, x, box, float(N), dE)
+    return _pack(f"random_N{N}_K{K}_s{seed}{'_c' if complex_hops else ''}", count, index,
+                 None if hop_value == -1.0 else hre,                       # None = the paper's default, every hopping -1
+                 him if (complex_hops and hop_value is None) else None, onsite, x, box, float(N), dE)
