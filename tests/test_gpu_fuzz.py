@@ -136,3 +136,26 @@ def test_random_graph_storage_variants_and_options(gq, oracle_mod, N, K, seed, f
     assert vec_err(g.get_state(gq.STATE_VAC_B), vb) <= TOL
     g.close()
     o.close()
+
+
+def test_live_handles_sharing_a_kernel_with_different_shared_memory_needs(gq, oracle_mod):
+    """Two handles alive at once whose tables run the SAME kernel instantiation (generic-width walk, B = 2) with different
+    shared-memory sizes (K = 5 and K = 16), used alternately: the dynamic shared-memory limit is a property of the kernel
+    in the process, not of a handle (it must only ever be raised)."""
+    ma = L.random_graph(800, 16, 61, complex_hops=True, degree_fill=1.0)
+    mb = L.random_graph(900, 5, 62, complex_hops=True, degree_fill=0.9)
+    ha = gq.GpuQT(ma, batch=2, modes=gq.MODE_PSI, options={"small": 0})
+    hb = gq.GpuQT(mb, batch=2, modes=gq.MODE_PSI, options={"small": 0})
+    oa, ob = oracle_mod.Oracle(ma, batch=2, modes=0), oracle_mod.Oracle(mb, batch=2, modes=0)
+    pa, pb = L.random_phase_vectors(ma.N, 2, 161, 0), L.random_phase_vectors(mb.N, 2, 162, 0)
+    for h, o, p in ((ha, oa, pa), (hb, ob, pb)):
+        h.set_state(p)
+        o.set_state(p)
+    for _ in range(2):
+        for h, o, m in ((hb, ob, mb), (ha, oa, ma), (hb, ob, mb)):
+            assert np.max(np.abs(h.dos_moments(24) - o.dos_moments(24))) / m.N <= TOL
+            h.evolve(0.4, 12)
+            o.evolve(0.4, 12)
+            assert vec_err(h.get_state(gq.STATE_PSI), o.get_state(oracle_mod.PSI)) <= TOL
+    for x in (ha, hb, oa, ob):
+        x.close()
