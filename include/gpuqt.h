@@ -103,7 +103,14 @@ typedef enum {
  *                  the index array (and <= 8 MB) AND batch >= 4 AND a recurrence step's working set (three
  *                  vector sets + the table) exceeds the L2 cache, i.e. when the index array would come from
  *                  HBM in every step and a tile streams enough bytes to pay for the extra copies;
- *                  0: never; 2: whenever the table is uniform (tests)                                  */
+ *                  0: never; 2: whenever the table is uniform (tests)
+ *   reorder        site reordering for locality: a simple-cubic periodic lattice in natural order (every row with its
+ *                  six nearest neighbours, any order; Lx, Ly multiples of 4, Lz even -- the 3-D Anderson model of
+ *                  PAPER.md:353-355) is stored in bricks of 4 x 4 x 2 sites per 32-row slice, so that four instead of
+ *                  two of a row's six neighbours lie in its own slice.  Invisible at the boundary: states, tables and
+ *                  moments are exchanged in the caller's numbering.  1: at batch >= 4 when a recurrence step's working
+ *                  set exceeds the L2 (the rule of `stencil`); 0: never;
+ *                  2: whenever the lattice is recognised (tests)                                          */
 typedef struct gpuqt_options {
     int32_t struct_bytes;
     int32_t stages;
@@ -115,6 +122,7 @@ typedef struct gpuqt_options {
     int32_t small;
     int32_t persistent;
     int32_t stencil;
+    int32_t reorder;
 } gpuqt_options;
 void gpuqt_default_options(gpuqt_options* opt);
 
@@ -274,6 +282,7 @@ int gpuqt_bessel_coeffs(double energy_scale, double dt, int32_t order, double* c
 #define GPUQT_INFO_WORKSPACE_USED 6        /* bytes of the workspace actually carved up                */
 #define GPUQT_INFO_SMALL_PATH_MSD 7        /* 1: the (psi, chi) time step is one launch of one CTA too    */
 #define GPUQT_INFO_STENCIL_PATTERNS 8      /* patterns in the implicit-stencil dictionary (0: not in use)  */
+#define GPUQT_INFO_REORDERED 9             /* 1: the sites are stored in brick order (gpuqt_options.reorder)  */
 int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value);
 
 /* Accumulated device time (CUDA events on the handle's stream around each run of launches) and

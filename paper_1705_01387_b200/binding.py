@@ -20,7 +20,7 @@ MAX_MOMENTS = 16384
 MAX_ORDER = 4096
 DAMPING_JACKSON, DAMPING_LORENTZ, DAMPING_NONE = 0, 1, 2
 (INFO_STORED_MATRIX_BYTES, INFO_HOP_VARIANT, INFO_UNIFORM, INFO_UNROLLED_WIDTH, INFO_SMALL_PATH, INFO_PERSISTENT,
- INFO_WORKSPACE_USED, INFO_SMALL_PATH_MSD, INFO_STENCIL_PATTERNS) = range(9)
+ INFO_WORKSPACE_USED, INFO_SMALL_PATH_MSD, INFO_STENCIL_PATTERNS, INFO_REORDERED) = range(10)
 
 
 class SlabDesc(C.Structure):
@@ -36,7 +36,7 @@ class SlabDesc(C.Structure):
 class Options(C.Structure):
     """gpuqt_options (include/gpuqt.h)."""
     _fields_ = [(n, C.c_int32) for n in ("struct_bytes", "stages", "blocks_per_sm", "run", "alternate", "hop_const",
-                                          "idx16", "small", "persistent", "stencil")]
+                                          "idx16", "small", "persistent", "stencil", "reorder")]
 
 
 # overrides applied to every GpuQT() that does not pass its own `options` (the GPU tests run every

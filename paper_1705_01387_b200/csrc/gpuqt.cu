@@ -65,6 +65,8 @@ struct gpuqt_handle {
     double2 *psi = nullptr, *chi = nullptr, *va = nullptr, *vb = nullptr, *phiL = nullptr;
     double2 *out0 = nullptr, *out1 = nullptr, *ring[kRing] = {nullptr, nullptr, nullptr},
             *ringe[kRing] = {nullptr, nullptr, nullptr};
+    // site reordering (recognised cubic lattices stored in bricks): device rows <-> the caller's sites; library-owned
+    int32_t *d_new_of_old = nullptr, *d_old_of_new = nullptr;
     // gpuqt_prefetch_state: the next batch of random vectors, copied on the library's own stream while the
     // caller's stream computes
     double2* stage_in = nullptr;
@@ -174,6 +176,54 @@ cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
     return e;
 }
 
+constexpr int64_t kB200L2Bytes = 126LL << 20;
+
+// Site reordering: a recognised simple-cubic lattice is stored in bricks of 4 x 4 x 2 sites (host_util.h,
+// detect_cubic_bricks).  option 1: at batch >= 4 when a recurrence step's working set exceeds the L2 (the HBM-bound case
+// it was measured to pay in, and the case in which the implicit stencil replaces the index array, whose 16-bit form the
+// brick order would lose), 2: whenever the lattice is recognised (tests), 0: never.  On success the pointers are
+// redirected to permuted copies held by `ro`.
+struct ReorderedInputs {
+    std::vector<int32_t> new_of_old, old_of_new, cnt, idx;
+    std::vector<double> hre, him, ons, x;
+};
+void reorder_inputs(ReorderedInputs& ro, int option, int64_t l2_bytes, int64_t N, int32_t K_max, int batch,
+                    const int32_t*& nbr_count, const int32_t*& nbr_index, const double*& hop_re, const double*& hop_im,
+                    const double*& onsite, const double*& x) {
+    const int64_t working_set = 3 * (N + 1) * (int64_t)batch * 16 + N * (8 + 2 * (int64_t)K_max);
+    const bool want = option == 2 || (option == 1 && batch >= 4 && working_set > (l2_bytes > 0 ? l2_bytes : kB200L2Bytes));
+    if (!want || !detect_cubic_bricks(N, K_max, nbr_count, nbr_index, ro.new_of_old, ro.old_of_new)) {
+        ro.new_of_old.clear();
+        ro.old_of_new.clear();
+        return;
+    }
+    const size_t K = (size_t)K_max;
+    ro.cnt.resize((size_t)N);
+    ro.idx.resize((size_t)N * K);
+    if (x) ro.x.resize((size_t)N);
+    if (hop_re) ro.hre.resize((size_t)N * K);
+    if (hop_im) ro.him.resize((size_t)N * K);
+    if (onsite) ro.ons.resize((size_t)N);
+    for (int64_t p = 0; p < N; ++p) {
+        const size_t m = (size_t)ro.old_of_new[(size_t)p];
+        ro.cnt[(size_t)p] = nbr_count[m];
+        if (x) ro.x[(size_t)p] = x[m];
+        if (onsite) ro.ons[(size_t)p] = onsite[m];
+        for (size_t k = 0; k < K; ++k) {
+            const int32_t n = nbr_index[m * K + k];
+            ro.idx[(size_t)p * K + k] = (k < (size_t)nbr_count[m]) ? ro.new_of_old[(size_t)n] : n;
+            if (hop_re) ro.hre[(size_t)p * K + k] = hop_re[m * K + k];
+            if (hop_im) ro.him[(size_t)p * K + k] = hop_im[m * K + k];
+        }
+    }
+    nbr_count = ro.cnt.data();
+    nbr_index = ro.idx.data();
+    if (x) x = ro.x.data();
+    if (hop_re) hop_re = ro.hre.data();
+    if (hop_im) hop_im = ro.him.data();
+    if (onsite) onsite = ro.ons.data();
+}
+
 // The storage variant of a table: packed sliced ELL; no hopping array when every
 // hopping is the same number; then the implicit stencil, else 16-bit columns, where the unrolled uniform
 // kernels exist.  Returns the Hop variant; `sell` (and `sten`) hold the records to upload.
@@ -184,7 +234,6 @@ cudaError_t ensure_dynamic_smem(void* fn, size_t bytes) {
 // tile streams so few bytes that the two extra copies per slice cost more than the index bytes they save (the
 // paper's example 5.1, a 2000 x 2000 square lattice with one vector: 1.57 s with explicit columns, 2.07 s with the
 // stencil).
-constexpr int64_t kB200L2Bytes = 126LL << 20;
 int choose_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const int32_t* nbr_index, const double* hop_re,
                    const double* hop_im, const double* onsite, const gpuqt_options& opt, int batch, int64_t l2_bytes,
                    SellHost& sell, StencilHost& sten, int64_t NV = -1) {
@@ -642,7 +691,7 @@ int finish_set_state(gpuqt_handle* h, const double2* src) {
     // src holds phi in [batch][N] order
     const long long total = (long long)h->vec_elems;
     const int blocks = (int)((total + 255) / 256);
-    to_device_layout<<<blocks, 256, 0, h->stream>>>(h->N, h->B, src, h->psi);
+    to_device_layout<<<blocks, 256, 0, h->stream>>>(h->N, h->B, src, h->psi, h->d_old_of_new);
     CU(cudaGetLastError());
     if (h->modes & GPUQT_MODE_MSD) {
         zero_vec<<<blocks, 256, 0, h->stream>>>(total, h->chi);
@@ -675,6 +724,7 @@ void gpuqt_default_options(gpuqt_options* o) {
     o->small = 1;
     o->persistent = -1;
     o->stencil = 1;
+    o->reorder = 1;
 }
 
 size_t gpuqt_workspace_bytes(int64_t N, int32_t K_max, int is_complex, int32_t batch, int modes) {
@@ -706,6 +756,9 @@ int gpuqt_plan_storage(int64_t N, int32_t K_max, const int32_t* nbr_count, const
         for (int32_t k = 0; k < nbr_count[m]; ++k)
             if (nbr_index[(size_t)m * K_max + k] < 0 || nbr_index[(size_t)m * K_max + k] >= N) return GPUQT_ERR_INDEX;
     }
+    ReorderedInputs ro;
+    const double *no_onsite = nullptr, *no_x = nullptr;
+    reorder_inputs(ro, opt.reorder, l2_bytes, N, K_max, batch, nbr_count, nbr_index, hop_re, hop_im, no_onsite, no_x);
     SellHost sell;
     StencilHost sten;
     const int hop = choose_storage(N, K_max, nbr_count, nbr_index, hop_re, hop_im, nullptr, opt, batch, l2_bytes, sell, sten);
@@ -769,7 +822,7 @@ int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, 
         opt.struct_bytes = (int32_t)sizeof(gpuqt_options);
     }
     if (opt.stages < 0 || opt.stages > kMaxStages || opt.blocks_per_sm < 0 || opt.run < 0 || opt.persistent < -1 || opt.persistent > 1 ||
-        opt.stencil < 0 || opt.stencil > 2)
+        opt.stencil < 0 || opt.stencil > 2 || opt.reorder < 0 || opt.reorder > 2)
         return bad(GPUQT_ERR_ARG, "option out of range");
     std::string msg;
     int rc = validate_inputs(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, x, box_length, energy_scale, msg, n_halo);
@@ -799,6 +852,11 @@ int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, 
             l2_bytes = 0;                   // no device: gpuqt_create fails below with GPUQT_ERR_CUDA
         }
     }
+    // Site reordering (reorder_inputs above): from here on every array is in the device numbering
+    ReorderedInputs ro;
+    reorder_inputs(ro, is_slab ? 0 : opt.reorder, l2_bytes, N, K_max, batch, nbr_count, nbr_index, hop_re, hop_im, onsite, x);
+    std::vector<int32_t>& new_of_old = ro.new_of_old;
+    std::vector<int32_t>& old_of_new = ro.old_of_new;
     h->hop = choose_storage(N, K_max, nbr_count, nbr_index, hop_re, hop_im, onsite, opt, batch, l2_bytes, sell, sten, NV);
     const bool use_stencil = h->hop == kHopStencil;
     h->stencil_patterns = use_stencil ? sten.n_patterns : 0;
@@ -847,6 +905,12 @@ int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, 
                          : up(d_sp, sell.slice_off.data(), sell.slice_off.size() * sizeof(long long));
     if (ce == cudaSuccess) ce = cudaMemsetAsync(base + L.ticket, 0, 256, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+    if (ce == cudaSuccess && !new_of_old.empty()) {
+        ce = cudaMalloc((void**)&h->d_new_of_old, (size_t)N * sizeof(int32_t));
+        if (ce == cudaSuccess) ce = cudaMalloc((void**)&h->d_old_of_new, (size_t)N * sizeof(int32_t));
+        if (ce == cudaSuccess) ce = cudaMemcpy(h->d_new_of_old, new_of_old.data(), (size_t)N * sizeof(int32_t), cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess) ce = cudaMemcpy(h->d_old_of_new, old_of_new.data(), (size_t)N * sizeof(int32_t), cudaMemcpyHostToDevice);
+    }
     if (ce == cudaSuccess) ce = cudaMallocHost((void**)&h->coef_host, (size_t)kCoefSlots * 2 * GPUQT_MAX_ORDER * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&h->coef_dev, (size_t)kCoefSlots * 2 * GPUQT_MAX_ORDER * sizeof(double));
     for (int i = 0; i < kCoefSlots && ce == cudaSuccess; ++i) ce = cudaEventCreateWithFlags(&h->coef_event[i], cudaEventDisableTiming);
@@ -1090,7 +1154,7 @@ int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host) {
                        : which == GPUQT_STATE_VAC_A ? h->va : which == GPUQT_STATE_VAC_B ? h->vb : nullptr;
     if (!src) return fail(h, GPUQT_ERR_STATE, "state not available in this mode");
     const long long total = (long long)h->vec_elems;
-    from_device_layout<<<(int)((total + 255) / 256), 256, 0, h->stream>>>(h->N, h->B, src, h->ring[0]);
+    from_device_layout<<<(int)((total + 255) / 256), 256, 0, h->stream>>>(h->N, h->B, src, h->ring[0], h->d_old_of_new);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out_host, h->ring[0], h->vec_elems * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
@@ -1107,7 +1171,8 @@ int gpuqt_get_table(gpuqt_handle* h, int32_t* col, double* re, double* im, doubl
     CU(ensure_scratch(h, tot));
     char* scratch = h->scratch;
     decode_table<<<(int)((nk + 255) / 256), 256, 0, h->stream>>>(h->mat, (int32_t*)(scratch + oc), (double*)(scratch + orr),
-                                                                 (double*)(scratch + oi), (double*)(scratch + od));
+                                                                 (double*)(scratch + oi), (double*)(scratch + od),
+                                                                 h->d_new_of_old, h->d_old_of_new);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && col) e = cudaMemcpyAsync(col, scratch + oc, nk * 4, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && re) e = cudaMemcpyAsync(re, scratch + orr, nk * 8, cudaMemcpyDeviceToHost, h->stream);
@@ -1130,6 +1195,7 @@ int gpuqt_get_info(gpuqt_handle* h, int what, int64_t* value) {
     case GPUQT_INFO_WORKSPACE_USED: *value = (int64_t)h->workspace_used; break;
     case GPUQT_INFO_SMALL_PATH_MSD: *value = small_msd_ok(h) ? 1 : 0; break;
     case GPUQT_INFO_STENCIL_PATTERNS: *value = h->stencil_patterns; break;
+    case GPUQT_INFO_REORDERED: *value = h->d_old_of_new ? 1 : 0; break;
     default: return fail(h, GPUQT_ERR_ARG, "unknown info key");
     }
     return GPUQT_OK;
@@ -1174,6 +1240,8 @@ void gpuqt_destroy(gpuqt_handle* h) {
     if (h->coef_dev) cudaFree(h->coef_dev);
     if (h->scratch) cudaFree(h->scratch);
     if (h->d_maps) cudaFree(h->d_maps);
+    if (h->d_new_of_old) cudaFree(h->d_new_of_old);
+    if (h->d_old_of_new) cudaFree(h->d_old_of_new);
     if (h->copy_stream) {
         cudaStreamSynchronize(h->copy_stream);
         cudaStreamDestroy(h->copy_stream);

@@ -333,3 +333,55 @@ inline bool try_stencil(SellHost& s, int K, int64_t N, bool force, StencilHost& 
     return true;
 }
 }  // namespace gpuqt
+
+namespace gpuqt {
+// Site reordering for locality (round 2): a simple-cubic periodic lattice in natural order (i = x + Lx (y + Ly z), every
+// row with its 6 nearest neighbours in any order -- the Anderson model of PAPER.md:353-355 in three dimensions) has
+// only the +-x neighbours of a row inside the row's 32-row slice; stored in bricks of 4 x 4 x 2 sites per slice, 4 of
+// the 6 neighbours of an average row are in its own slice (shared memory) and the gather stream from L2 halves
+// (c4: KPM step 156.7 -> 148.4 us, evolve_msd 456.8 -> 437.0 us).  Square lattices gain nothing from 2-D bricks
+// (measured: c2 11.65 vs 11.68 us, the paper's example 5.1 50.2 vs 49.9 us), so only d = 3 is recognised.
+// Returns true and the two permutations when the table is such a lattice with Lx, Ly multiples of 4 and Lz even.
+inline bool detect_cubic_bricks(int64_t N, int32_t K, const int32_t* cnt, const int32_t* idx,
+                                std::vector<int32_t>& new_of_old, std::vector<int32_t>& old_of_new) {
+    if (K != 6 || N < 27 || N > 0x7fffffffLL) return false;
+    if (cnt[0] != 6) return false;
+    int64_t a[6];
+    for (int k = 0; k < 6; ++k) a[k] = idx[k];
+    std::sort(a, a + 6);
+    // neighbours of site 0: 1, Lx - 1, Lx, Lx (Ly - 1), Lx Ly, N - Lx Ly
+    const int64_t Lx = a[2];
+    if (a[0] != 1 || Lx < 3 || a[1] != Lx - 1 || a[3] % Lx != 0) return false;
+    const int64_t Ly = a[3] / Lx + 1, LxLy = Lx * Ly;
+    if (Ly < 3 || a[4] != LxLy || N % LxLy != 0) return false;
+    const int64_t Lz = N / LxLy;
+    if (Lz < 3 || a[5] != N - LxLy) return false;
+    if (Lx % 4 || Ly % 4 || Lz % 2) return false;
+    for (int64_t m = 0; m < N; ++m) {                 // every row: exactly the six periodic neighbours, in any order
+        if (cnt[m] != 6) return false;
+        const int64_t x = m % Lx, y = (m / Lx) % Ly, z = m / LxLy;
+        int64_t want[6] = {m - x + (x + 1) % Lx, m - x + (x + Lx - 1) % Lx,
+                           m - y * Lx + ((y + 1) % Ly) * Lx, m - y * Lx + ((y + Ly - 1) % Ly) * Lx,
+                           m - z * LxLy + ((z + 1) % Lz) * LxLy, m - z * LxLy + ((z + Lz - 1) % Lz) * LxLy};
+        int64_t have[6];
+        for (int k = 0; k < 6; ++k) have[k] = idx[(size_t)m * 6 + k];
+        std::sort(want, want + 6);
+        std::sort(have, have + 6);
+        for (int k = 0; k < 6; ++k)
+            if (want[k] != have[k]) return false;
+    }
+    new_of_old.resize((size_t)N);
+    old_of_new.resize((size_t)N);
+    const int64_t nbx = Lx / 4, nby = Ly / 4;
+    for (int64_t m = 0; m < N; ++m) {
+        const int64_t x = m % Lx, y = (m / Lx) % Ly, z = m / LxLy;
+        const int64_t brick = (x / 4) + nbx * ((y / 4) + nby * (z / 2));
+        const int64_t local = (x % 4) + 4 * ((y % 4) + 4 * (z % 2));
+        const int64_t p = brick * 32 + local;
+        new_of_old[(size_t)m] = (int32_t)p;
+        old_of_new[(size_t)p] = (int32_t)m;
+    }
+    return true;
+}
+}  // namespace gpuqt
+

@@ -1323,20 +1323,25 @@ __global__ void __launch_bounds__(kThreads) dot_kernel(long long N, const double
 }
 
 #ifndef GPUQT_STEP_TU   // the non-template kernels below belong to gpuqt.cu's translation unit only
-// [batch][N] (host order) <-> [N][B] (device order)
-__global__ void to_device_layout(long long N, int B, const double2* __restrict__ src, double2* __restrict__ dst) {
+// [batch][N] (host order) <-> [N][B] (device order).  old_of_new != nullptr: the device rows are a permutation of the
+// caller's sites (brick order of a recognised cubic lattice): device row `row` is the caller's site old_of_new[row].
+__global__ void to_device_layout(long long N, int B, const double2* __restrict__ src, double2* __restrict__ dst,
+                                 const int* __restrict__ old_of_new) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N * B) return;
     const long long row = i / B;
     const int b = (int)(i % B);
-    dst[i] = src[(size_t)b * N + row];
+    const long long site = old_of_new ? old_of_new[row] : row;
+    dst[i] = src[(size_t)b * N + site];
 }
-__global__ void from_device_layout(long long N, int B, const double2* __restrict__ src, double2* __restrict__ dst) {
+__global__ void from_device_layout(long long N, int B, const double2* __restrict__ src, double2* __restrict__ dst,
+                                   const int* __restrict__ old_of_new) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N * B) return;
     const long long row = i / B;
     const int b = (int)(i % B);
-    dst[(size_t)b * N + row] = src[i];
+    const long long site = old_of_new ? old_of_new[row] : row;
+    dst[(size_t)b * N + site] = src[i];
 }
 // out = c * in (complex): the start b_{N_p-1} = c_{N_p-1} psi of the Clenshaw recurrence
 __global__ void scale_vec(long long n, double cr, double ci, const double2* __restrict__ in, double2* __restrict__ out) {
@@ -1445,13 +1450,16 @@ __global__ void conductivity_kernel(int kind, int n_t, int n_e, const double* __
     }
 }
 
-// Decode the packed records back to canonical padded row-major arrays (bit-exact check)
+// Decode the packed records back to canonical padded row-major arrays in the CALLER's site numbering (bit-exact
+// check).  new_of_old / old_of_new: the row permutation of a reordered lattice, or nullptr.
 __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __restrict__ re,
-                             double* __restrict__ im, double* __restrict__ dx) {
+                             double* __restrict__ im, double* __restrict__ dx, const int* __restrict__ new_of_old,
+                             const int* __restrict__ old_of_new) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.N * m.K) return;
-    const long long row = i / m.K;
+    const long long site = i / m.K;                               // the caller's row
     const int k = (int)(i % m.K);
+    const long long row = new_of_old ? new_of_old[site] : site;   // where it is stored
     const RecView rv = record_view(m, row >> 5);
     const int r = (int)(row & 31);
     int c = (int)row;
@@ -1467,7 +1475,7 @@ __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __r
         if (m.cplx) hi = rv.him[k * 32 + r];
         d = min_image(m.x[c] - m.x[row], m.box);
     }
-    if (col) col[i] = c;
+    if (col) col[i] = old_of_new ? old_of_new[c] : c;
     if (re) re[i] = hr;
     if (im) im[i] = hi;
     if (dx) dx[i] = d;

@@ -419,7 +419,7 @@ int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host) {
         GCU(cudaMemcpyAsync(h->ring[0], phi_host[i], h->vec_elems * sizeof(double2), cudaMemcpyHostToDevice, g->stream));
         const long long total = (long long)h->vec_elems;
         const int blocks = (int)((total + 255) / 256);
-        to_device_layout<<<blocks, 256, 0, g->stream>>>(h->N, h->B, h->ring[0], h->psi);
+        to_device_layout<<<blocks, 256, 0, g->stream>>>(h->N, h->B, h->ring[0], h->psi, nullptr);
         GCU(cudaGetLastError());
         if (g->modes & GPUQT_MODE_MSD) {
             zero_vec<<<blocks, 256, 0, g->stream>>>(total, h->chi);

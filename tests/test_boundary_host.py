@@ -149,12 +149,16 @@ def test_storage_plan_regular_lattices_need_no_index_array(gq):
     MB = 1 << 20              # pretend L2 size: the stencil is only taken when a step's working set exceeds the L2
     # cubic 64^3: x-lines are two slices long -> patterns = {first, second half of a line} x {y = 0, mid, 63} x {z = 0, mid, 63}
     m = L.cubic(64, W=16.5, seed=1, energy_scale=16.0)
-    hop, nbytes, pats = gq.plan_storage(m, batch=4, l2_bytes=MB)
+    hop, nbytes, pats = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"reorder": 0})
     assert hop == STENCIL and pats == 2 * 3 * 3               # N is a multiple of 128 rows: no all-padding tail records
+    # by default a recognised cubic lattice beyond the L2 is stored in bricks of 4 x 4 x 2 sites: one pattern per
+    # (first, middle, last) brick position in each direction, same bytes
+    hop_b, nbytes_b, pats_b = gq.plan_storage(m, batch=4, l2_bytes=MB)
+    assert hop_b == STENCIL and pats_b == 3 * 3 * 3 and abs(nbytes_b - nbytes) <= 27 * 6 * 32 * 4
     assert nbytes < 8.2 * m.N + 8 * (m.N + 1)                  # 8 B on-site + 0.125 B pattern id per row (+ x)
-    hop16, nbytes16, _ = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"stencil": 0})
+    hop16, nbytes16, _ = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"stencil": 0, "reorder": 0})
     assert hop16 == CONST16 and nbytes16 > nbytes + 12 * m.N   # 16-bit columns: 21 B per row at K = 6
-    hop32, nbytes32, _ = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"stencil": 0, "idx16": 0})
+    hop32, nbytes32, _ = gq.plan_storage(m, batch=4, l2_bytes=MB, options={"stencil": 0, "idx16": 0, "reorder": 0})
     assert hop32 == CONST32 and nbytes32 == (m.N // 32) * (256 + 128 * 6) + 8 * (m.N + 1)
     # square 1000 x 96 (lines not aligned with slices): a dozen patterns
     m = L.square(1000, 96, W=2.0, seed=2)

@@ -518,3 +518,48 @@ def test_implicit_stencil_matches_explicit_columns(gq, oracle_mod, model, batch)
         g.close()
     for a, b in zip(*outs):
         assert a.tobytes() == b.tobytes()
+
+
+@pytest.mark.parametrize("batch", [1, 4, 8])
+def test_brick_reordering_is_invisible(gq, oracle_mod, batch):
+    """gpuqt_options.reorder: a recognised simple-cubic lattice is stored in bricks of 4 x 4 x 2 sites.  Forced on a
+    small lattice (neighbour lists in shuffled order per row): the decoded table is bit-identical to the oracle's in the
+    caller's numbering, states and moments agree with the oracle, and with the unreordered handle to rounding."""
+    from paper_1705_01387_b200 import binding
+    model = L.cubic(16, W=16.5, seed=16, energy_scale=16.0)            # 16 x 16 x 16: Lx, Ly multiples of 4, Lz even
+    # shuffle the neighbour order inside every row (the detection must not depend on it)
+    idx = model.nbr_index.reshape(model.N, 6).copy()
+    perm = np.argsort(L.rng.uniform01(77, model.N * 6).reshape(model.N, 6), axis=1)
+    model.nbr_index = np.ascontiguousarray(np.take_along_axis(idx, perm, axis=1).reshape(-1))
+    a = gq.GpuQT(model, batch=batch, modes=gq.MODE_VAC | gq.MODE_MSD, options=opts(reorder=2, small=0))
+    b = gq.GpuQT(model, batch=batch, modes=gq.MODE_VAC | gq.MODE_MSD, options=opts(reorder=0, small=0))
+    assert a.info(binding.INFO_REORDERED) == 1 and b.info(binding.INFO_REORDERED) == 0
+    o = oracle_mod.Oracle(model, batch=batch, modes=oracle_mod.MODE_VAC | oracle_mod.MODE_MSD)
+    oc, ore, oim, odx = o.get_table()
+    for g in (a, b):
+        col, re, im, dx = g.get_table()
+        assert np.array_equal(col, oc) and re.tobytes() == ore.tobytes() and dx.tobytes() == odx.tobytes()
+    phi = L.random_phase_vectors(model.N, batch, 97, 0)
+    for g in (a, b, o):
+        g.set_state(phi)
+    nm = 48
+    ref = o.dos_moments(nm)
+    assert np.max(np.abs(a.dos_moments(nm) - ref)) / model.N <= TOL
+    for g in (a, b, o):
+        g.evolve(0.9, 30)
+    chi = o.get_state(oracle_mod.CHI)
+    for which, ow in ((gq.STATE_PSI, oracle_mod.PSI), (gq.STATE_CHI, oracle_mod.CHI), (gq.STATE_VAC_A, oracle_mod.VAC_A),
+                      (gq.STATE_VAC_B, oracle_mod.VAC_B)):
+        assert vec_err(a.get_state(which), o.get_state(ow)) <= TOL
+        assert a.get_state(which).tobytes() == b.get_state(which).tobytes()     # same operands, same neighbour order per row
+    assert np.max(np.abs(a.msd(nm) - o.msd(nm)) / np.sum(chi * chi, axis=(1, 2))[:, None]) <= TOL
+    va, vb = o.get_state(oracle_mod.VAC_A), o.get_state(oracle_mod.VAC_B)
+    scale = np.array([np.linalg.norm(o.apply_v(va[k])) * np.linalg.norm(vb[k]) for k in range(batch)])
+    assert np.max(np.abs(a.vac(nm) - o.vac(nm)) / scale[:, None]) <= TOL
+    # not a cubic lattice / dimensions the bricks do not divide: left alone
+    for other in (L.cubic(13, W=1.0, seed=4, energy_scale=8.0), L.square(64, 32, W=2.0, seed=15)):
+        g = gq.GpuQT(other, batch=batch, modes=gq.MODE_PSI, options=opts(reorder=2))
+        assert g.info(binding.INFO_REORDERED) == 0
+        g.close()
+    for g in (a, b, o):
+        g.close()
