@@ -563,3 +563,27 @@ def test_brick_reordering_is_invisible(gq, oracle_mod, batch):
         g.close()
     for g in (a, b, o):
         g.close()
+
+
+@pytest.mark.parametrize("size", [4, 8, 12, 20])
+def test_brick_reordering_small_and_odd_brick_counts(gq, oracle_mod, size):
+    """Cubes whose brick grid is 1 x 1 x 2 (4^3), 2 x 2 x 4, 3 x 3 x 6 and 5 x 5 x 10: every wrap falls on a brick boundary,
+    one brick can be its own neighbour in x and y."""
+    from paper_1705_01387_b200 import binding
+    model = L.cubic(size, W=16.5, seed=size, energy_scale=16.0)
+    g = gq.GpuQT(model, batch=4, modes=gq.MODE_MSD, options=opts(reorder=2, small=0))
+    assert g.info(binding.INFO_REORDERED) == 1
+    o = oracle_mod.Oracle(model, batch=4, modes=oracle_mod.MODE_MSD)
+    col, re, im, dx = g.get_table()
+    oc, ore, oim, odx = o.get_table()
+    assert np.array_equal(col, oc) and re.tobytes() == ore.tobytes() and dx.tobytes() == odx.tobytes()
+    phi = L.random_phase_vectors(model.N, 4, 98, 0)
+    g.set_state(phi)
+    o.set_state(phi)
+    g.evolve(1.0, 44)
+    o.evolve(1.0, 44)
+    chi = o.get_state(oracle_mod.CHI)
+    assert vec_err(g.get_state(gq.STATE_CHI), chi) <= TOL
+    assert np.max(np.abs(g.msd(64) - o.msd(64)) / np.sum(chi * chi, axis=(1, 2))[:, None]) <= TOL
+    g.close()
+    o.close()
