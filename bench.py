@@ -303,7 +303,7 @@ def run_ours(args, w):
         e1.record(stream)
         stream.synchronize()
         h2d_ms = e0.elapsed_time(e1)
-        info = {k: g.info(getattr(binding, "INFO_" + k)) for k in ("STORED_MATRIX_BYTES", "HOP_VARIANT", "SMALL_PATH", "PERSISTENT")}
+        info = {k: g.info(getattr(binding, "INFO_" + k)) for k in ("STORED_MATRIX_BYTES", "HOP_VARIANT", "SMALL_PATH", "PERSISTENT", "REORDERED")}
 
     ev_w, mom_w = walks_per_step(w, order)
     units_step = model.N * w.batch * (ev_w + mom_w) * world
@@ -348,6 +348,8 @@ def run_ours(args, w):
                                                        "constant, 16-bit columns with padding",
                                                        "constant, implicit stencil (pattern dictionary, no index array)"][info["HOP_VARIANT"]],
                                        "stored_matrix_bytes": info["STORED_MATRIX_BYTES"],
+                                       "site_order": "bricks of 4 x 4 x 2 sites per slice (recognised cubic lattice)" if info["REORDERED"]
+                                                     else "the caller's",
                                        "launch_form": "one-CTA whole-recurrence kernel" if info["SMALL_PATH"] else
                                                       "one cooperative launch per recurrence" if info["PERSISTENT"] else
                                                       "one launch per recurrence step"},
