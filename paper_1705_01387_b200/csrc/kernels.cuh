@@ -47,13 +47,9 @@
 #ifndef GPUQT_MINB_B1
 #define GPUQT_MINB_B1 2
 #endif
-// (psi, chi) evolve kernel: 1 = two CTAs per SM (x_{m-2}, e_{m-2} rows by streaming loads instead of
-// staging, the neighbour gathers in two halves so that the walk fits 128 registers); 0 = one CTA per SM
-#ifndef GPUQT_MSD_OCC
-#define GPUQT_MSD_OCC 0
-#endif
-// (psi, chi) evolve kernel, second route to two CTAs per SM: a lane owns ONE vector of a row (128-bit accesses,
-// half the registers of the 256-bit ownership) and x_{m-2}, e_{m-2} rows are read by streaming loads
+// (psi, chi) evolve kernel, experiment: two CTAs per SM -- a lane owns ONE vector of a row (128-bit accesses, half the
+// registers of the 256-bit ownership) and x_{m-2}, e_{m-2} rows are read by streaming loads.  Measured: no gain
+// (profiles/r2_ncu_summary.md), so it is off.
 #ifndef GPUQT_MSD_V1
 #define GPUQT_MSD_V1 0
 #endif
@@ -76,15 +72,7 @@ __host__ __device__ constexpr bool lane_owns_four(int B, int mode) {
     return mode != 3 /* kModeEvolveMsd */ && ((GPUQT_V4_B8 && B >= 8) || (GPUQT_V4 && B >= 4));
 }
 #ifndef GPUQT_MINB_MSD
-#define GPUQT_MINB_MSD ((GPUQT_MSD_OCC || GPUQT_MSD_V1) ? 2 : 1)
-#endif
-
-// L2 policy experiments
-#ifndef GPUQT_GATHER_POLICY   // 0: plain ld.global, 1: L2::evict_last
-#define GPUQT_GATHER_POLICY 1
-#endif
-#ifndef GPUQT_ST_POLICY       // stores of x_m: 0 plain, 1 st.global.cs (evict-first)
-#define GPUQT_ST_POLICY 0
+#define GPUQT_MINB_MSD (GPUQT_MSD_V1 ? 2 : 1)
 #endif
 
 // -DGPUQT_CHECKED=1: range checks of every gathered column, staged-row offset and pipeline index inside the
@@ -299,13 +287,7 @@ __device__ __forceinline__ uint32_t swz32(uint32_t sa) {
 #endif
 }
 
-__device__ __forceinline__ void st_vec(double2* p, double2 v) {
-#if GPUQT_ST_POLICY == 1
-    __stcs(p, v);
-#else
-    *p = v;
-#endif
-}
+__device__ __forceinline__ void st_vec(double2* p, double2 v) { *p = v; }
 __device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
     unsigned int v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -414,7 +396,7 @@ __host__ __device__ constexpr int min_blocks(int B, int mode) {
 // x_{m-2}, e_{m-2} own rows are read by streaming 256-bit loads at the top of the round instead.  (Round 1 did the
 // same in the KPM kernels at B = 8 to keep two CTAs per SM; with four vectors per lane there is one CTA per SM and
 // the staged form is back, see GPUQT_PD8.)
-// The (psi, chi) evolve kernel does the same at every B when GPUQT_MSD_OCC / GPUQT_MSD_V1 is on (four staged
+// The (psi, chi) evolve kernel does the same at every B when GPUQT_MSD_V1 is on (four staged
 // streams would leave room for one CTA per SM).  Direct reads for it alone, at one CTA per SM, change nothing
 // (c4: evolve_msd 195.3 vs 197.2 ms per 10 steps); GPUQT_PREV_DIRECT = 1 for every kernel costs the KPM kernels
 // 7 % at B = 4 (158 -> 170 us per step).
@@ -423,7 +405,7 @@ __host__ __device__ constexpr int min_blocks(int B, int mode) {
 #endif
 __host__ __device__ constexpr bool prev_direct(int B, int mode) {
     return (B >= 8 && (GPUQT_PD8 || mode == kModeEvolveMsd)) || GPUQT_PREV_DIRECT ||
-           ((GPUQT_MSD_OCC || GPUQT_MSD_V1) && mode == kModeEvolveMsd);
+           (GPUQT_MSD_V1 && mode == kModeEvolveMsd);
 }
 
 // slices per tile at B = 1 on the unrolled uniform tables (2 or 4; kTilePad is a multiple): a tile's bookkeeping
@@ -538,13 +520,8 @@ __device__ __forceinline__ void cv_st<1>(double2* p, const CV<1>& v) {
 }
 template <>
 __device__ __forceinline__ void cv_st<2>(double2* p, const CV<2>& v) {
-#if GPUQT_ST_POLICY == 1
-    asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v.re[0]), "d"(v.im[0]), "d"(v.re[1]), "d"(v.im[1])
-                 : "memory");
-#else
     asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v.re[0]), "d"(v.im[0]), "d"(v.re[1]), "d"(v.im[1])
                  : "memory");
-#endif
 }
 // Gather of V consecutive vectors of row c of x_{m-1}: rows of the current tile come from the staged
 // copy in shared memory, the others from global memory with an L2 evict_last hint (they are re-read
@@ -636,11 +613,7 @@ __device__ __forceinline__ CV<2> cv_gather<2, 32, true>(const char* g_l, uint32_
         "setp.lt.u32 p, %6, 32;\n"
         "@p ld.shared.v2.f64 {%0, %1}, [%4];\n"
         "@p ld.shared.v2.f64 {%2, %3}, [%7];\n"
-#if GPUQT_GATHER_POLICY == 1
         "@!p ld.global.L2::evict_last.v4.f64 {%0, %1, %2, %3}, [%5];\n"
-#else
-        "@!p ld.global.v4.f64 {%0, %1, %2, %3}, [%5];\n"
-#endif
         "}"
         : "=d"(v.re[0]), "=d"(v.im[0]), "=d"(v.re[1]), "=d"(v.im[1])
         : "r"(sa), "l"(ga), "r"(d), "r"(sb));
@@ -776,9 +749,8 @@ __device__ __forceinline__ void walk_rounds(const Mat& m, const RecArgs& a, cons
 #pragma unroll
     for (int u = 0; u < U; ++u) sum[u] = sum_e[u] = sum_x[u] = cv_zero<V>();
     if (KT > 0) {
-        // all gathers of the rows first (independent loads in flight), then the arithmetic; the (psi, chi)
-        // walk does it in two halves of the neighbour list when it has to fit 128 registers
-        constexpr int CH = (MSD && GPUQT_MSD_OCC) ? (KU + 1) / 2 : KU;
+        // all gathers of the rows first (independent loads in flight), then the arithmetic
+        constexpr int CH = KU;
 #pragma unroll
         for (int k0 = 0; k0 < KU; k0 += CH) {
             CV<V> v[U][CH], ve[U][MSD ? CH : 1];
