@@ -25,8 +25,10 @@
  * matrix live in the caller's workspace; the handle itself owns only small objects (the TMA tensor
  * maps of the vector buffers, a grow-on-demand device scratch buffer for gpuqt_kpm_transform /
  * gpuqt_running_conductivity / gpuqt_get_table, a few KB of pinned host memory and its device mirror
- * for the Bessel coefficients of a time step), which gpuqt_destroy frees together with the handle;
- * the workspace stays the caller's.
+ * for the Bessel coefficients of a time step, the copy stream and two events of gpuqt_prefetch_state,
+ * and -- for a lattice stored in brick order, gpuqt_options.reorder -- two int32[N] device arrays with
+ * the site permutation), which gpuqt_destroy frees together with the handle; the workspace stays the
+ * caller's.
  *
  * Errors: every call returns a gpuqt_status (0 = ok, < 0 = error); nothing throws, aborts or prints
  * across the ABI; the handle stays valid after an error; gpuqt_last_error(handle) gives text, and
