@@ -88,8 +88,7 @@ typedef enum {
  *   struct_bytes   sizeof(gpuqt_options) as the caller compiled it (set by gpuqt_default_options)
  *   stages         shared-memory pipeline stages per warp, 1..4;            0 = by batch (4, 3, 2, 2)
  *   blocks_per_sm  cap on resident CTAs per SM;                             0 = what fits
- *   run            consecutive tiles a CTA walks before it jumps (rounded to a multiple of 8);
- *                                                                           0 = 16, or 8 for short sweeps
+ *   run            consecutive tiles a CTA walks before it jumps (rounded to a multiple of 8);   0 = 8
  *   alternate      1: the sweep direction alternates between recurrence steps (L2 reuse across the
  *                  step boundary)
  *   hop_const      1: store no hopping array when every listed hopping is the same real number

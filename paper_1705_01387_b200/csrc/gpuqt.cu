@@ -932,10 +932,9 @@ int create_handle(gpuqt_handle** out, int64_t N, int64_t n_halo, int32_t K_max, 
     // whole recurrences in one cooperative launch when a step is so short that launch gaps matter
     h->persistent = h->coop_ok && (opt.persistent == 1 || (opt.persistent == -1 && N * batch <= (int64_t)131072 * h->n_sm));
     h->alternate = opt.alternate;
-    // tiles per CTA run: 16 keeps a CTA on a contiguous band (the sweep front stays tight in L2); short sweeps
-    // take the finest granularity for load balance
-    const long long tiles = n_tiles_of(h);
-    int run = opt.run ? opt.run : (tiles < (long long)64 * kWarps * h->n_sm ? kWarps : 2 * kWarps);
+    // tiles per CTA run: one tile per warp -- the finest granularity (load balance of short sweeps) and, measured,
+    // never slower than longer runs (c4: 147.8 us per KPM step at 8, 149.2 at 16, 152.3 at 32; c5 indifferent)
+    int run = opt.run ? opt.run : kWarps;
     h->run = std::max(1, run / kWarps) * kWarps;
 
     const size_t vstride = align_up((size_t)(NV + 1) * batch * sizeof(double2));
