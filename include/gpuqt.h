@@ -240,6 +240,39 @@ int gpuqt_kpm_transform_damped(gpuqt_handle* h, int damping, double lambda, cons
                                int32_t n_moments, int32_t n_sets, const double* energies_host,
                                int32_t n_energies, double* out_host);
 
+/* The same resummation for callers that cannot allocate device memory -- no handle, no cudaMalloc, no cudaFree, no
+ * allocating library routine anywhere in the call.  The calls above stage their arguments and keep the table of
+ * damping factors in a buffer the handle obtains with cudaMalloc and grows on demand; that is unusable when the
+ * process has already given the whole card to a memory pool or a framework's caching allocator (a cudaMalloc behind
+ * its back fails, or triggers the pool's out-of-memory retry), when the call sits in a latency-critical loop
+ * (cudaMalloc / cudaFree serialise with everything running on the device), or when a scheduler has fixed the job's
+ * memory budget in advance (MPS limits, MIG slices).  Here the caller brings inputs and output as DEVICE buffers it
+ * already owns:
+ *   moments_device   device [n_sets][n_moments]    C_n, e.g. copied from gpuqt_dos_moments / gpuqt_vac / gpuqt_msd
+ *   energies_device  device [n_energies]           E_j, |E_j| < energy_scale
+ *   out_device       device [n_sets][n_energies]   the transformed function, as gpuqt_kpm_transform_damped
+ *   energy_scale, volume   dE and Omega of the model; both > 0
+ *   cuda_stream      a cudaStream_t of the CURRENT device (NULL = default stream); the three buffers live there too
+ *   err_text         host buffer of err_text_bytes bytes for the message of a failed call, or NULL
+ * and the table gs[n] = g_n (2 - delta_n0) plus one status word sit in a fixed `static __device__` array inside the
+ * library: GPUQT_STATIC_MAX_MOMENTS doubles + 256 bytes = 128.25 KB of device memory that every GPU loading
+ * libgpuqt.so holds until the process exits.  That fixed size is the limit: n_moments > GPUQT_STATIC_MAX_MOMENTS is
+ * refused with GPUQT_ERR_NOMEM (n_sets and n_energies are not limited by it; inputs and output are the caller's).
+ * The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current) and remembers it; make that first call before you begin any stream capture on that device.
+ * The array is shared by every call in the process and keeps the last call's contents: the call itself resets what
+ * has to start at zero (the status word), and calls that overlap on the GPU -- different streams, different host
+ * threads -- race on the table and the status word.  Issue them one at a time per device.
+ * The call returns when out_device is complete (it synchronises cuda_stream to read the status word back).
+ * Errors: GPUQT_ERR_ARG (null / non-positive argument, unknown damping, n_sets * n_energies >= 2^31),
+ * GPUQT_ERR_NOMEM (n_moments beyond the static table), GPUQT_ERR_ENERGY (some |E_j| >= energy_scale, found on the
+ * device: out_device then holds NaN at those energies and valid numbers elsewhere), GPUQT_ERR_CUDA.             */
+#define GPUQT_STATIC_MAX_MOMENTS 16384
+int gpuqt_kpm_transform_static(int damping, double lambda, const double* moments_device, int32_t n_moments,
+                               int32_t n_sets, const double* energies_device, int32_t n_energies,
+                               double energy_scale, double volume, double* out_device, void* cuda_stream,
+                               char* err_text, size_t err_text_bytes);
+
 /* Running conductivity sigma(E, t) in units e = 1 from the TRANSFORMED correlation functions
  * (outputs of gpuqt_kpm_transform), one row per time (PAPER.md:81 Eq. 2, :92 Eq. 5, :123 Eq. 11;
  * discretisation readings A25/A26 of DESIGN.md).  All arrays are host arrays.

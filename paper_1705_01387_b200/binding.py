@@ -17,6 +17,7 @@ MODE_VAC, MODE_MSD, MODE_PSI = 1, 2, 4
 STATE_PSI, STATE_CHI, STATE_VAC_A, STATE_VAC_B = 0, 1, 2, 3
 KERNEL_KPM_DOUBLING, KERNEL_KPM_LEFT, KERNEL_EVOLVE, KERNEL_EVOLVE_MSD, KERNEL_VELOCITY = range(5)
 MAX_MOMENTS = 16384
+STATIC_MAX_MOMENTS = 16384     # GPUQT_STATIC_MAX_MOMENTS: the static table of gpuqt_kpm_transform_static
 MAX_ORDER = 4096
 DAMPING_JACKSON, DAMPING_LORENTZ, DAMPING_NONE = 0, 1, 2
 (INFO_STORED_MATRIX_BYTES, INFO_HOP_VARIANT, INFO_UNIFORM, INFO_UNROLLED_WIDTH, INFO_SMALL_PATH, INFO_PERSISTENT,
@@ -71,6 +72,8 @@ _SIGNATURES = {
     "gpuqt_msd": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_kpm_transform": (C.c_int, [C.c_void_p, _dp, C.c_int32, C.c_int32, _dp, C.c_int32, _dp]),
     "gpuqt_kpm_transform_damped": (C.c_int, [C.c_void_p, C.c_int, C.c_double, _dp, C.c_int32, C.c_int32, _dp, C.c_int32, _dp]),
+    "gpuqt_kpm_transform_static": (C.c_int, [C.c_int, C.c_double, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
+                                             C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]),
     "gpuqt_get_info": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "gpuqt_running_conductivity": (C.c_int, [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int32, C.c_int32, _dp, _dp]),
     "gpuqt_get_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
@@ -185,6 +188,32 @@ def plan_storage(model, batch=1, options=None, l2_bytes=0):
     if rc != 0:
         raise GpuqtError(rc, "gpuqt_plan_storage")
     return hop.value, nbytes.value, pats.value
+
+
+def kpm_transform_static(moments, energies, energy_scale, volume, damping=DAMPING_JACKSON, lam=0.0, out=None, stream=None):
+    """gpuqt_kpm_transform_static: the damping + energy transform without a handle and without any device allocation
+    inside the library -- for callers whose device memory is already spoken for (a pool or caching allocator owns the
+    card, a fixed memory budget) or that cannot afford cudaMalloc's device-wide stall.  `moments` [n_sets][n_moments]
+    and `energies` [n_energies] are CUDA float64 tensors the caller already holds; the result goes to `out`
+    ([n_sets][n_energies], CUDA float64) -- pass one you own to keep this wrapper allocation-free as well, otherwise
+    torch allocates it here, on the caller's side of the boundary.  At most STATIC_MAX_MOMENTS moments; one call at a
+    time per device (every call shares one static scratch table inside the library)."""
+    import torch
+    assert moments.is_cuda and energies.is_cuda and moments.dtype == energies.dtype == torch.float64
+    assert moments.is_contiguous() and energies.is_contiguous() and moments.dim() == 2 and energies.dim() == 1
+    n_sets, n_moments = moments.shape
+    if out is None:
+        out = torch.empty((n_sets, energies.numel()), dtype=torch.float64, device=moments.device)
+    assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float64 and tuple(out.shape) == (n_sets, energies.numel())
+    stream = stream if stream is not None else torch.cuda.current_stream()
+    text = C.create_string_buffer(256)
+    rc = load().gpuqt_kpm_transform_static(C.c_int(damping), C.c_double(lam), C.c_void_p(moments.data_ptr()),
+                                           C.c_int32(n_moments), C.c_int32(n_sets), C.c_void_p(energies.data_ptr()),
+                                           C.c_int32(energies.numel()), C.c_double(energy_scale), C.c_double(volume),
+                                           C.c_void_p(out.data_ptr()), C.c_void_p(stream.cuda_stream), text, C.c_size_t(256))
+    if rc:
+        raise GpuqtError(rc, "gpuqt_kpm_transform_static", text.value.decode())
+    return out
 
 
 class GpuQT:

@@ -1,7 +1,8 @@
 """Build libgpuqt.so (sm_100a only) in-tree with nvcc.  `python -m paper_1705_01387_b200.build`.
 
-Five translation units compiled in parallel and linked into one shared library: gpuqt.cu (the C-ABI,
-host logic and the small kernels) and step_kernels.cu once per Mode of the step kernel."""
+Six translation units compiled in parallel and linked into one shared library: gpuqt.cu (the C-ABI,
+host logic and the small kernels), step_kernels.cu once per Mode of the step kernel, and transform_static.cu
+(the allocation-free energy transform with its static device scratch)."""
 import os
 import subprocess
 import sys
@@ -9,8 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("GPUQT_LIB") or os.path.join(HERE, "libgpuqt.so")
-UNITS = [("gpuqt.cu", [])] + [("step_kernels.cu", [f"-DGPUQT_TU_MODE={m}"]) for m in range(4)]
-DEPS = [os.path.join(CSRC, f) for f in ("gpuqt.cu", "step_kernels.cu", "kernels.cuh", "host_util.h", "slab_group.inl")] + [
+UNITS = [("gpuqt.cu", [])] + [("step_kernels.cu", [f"-DGPUQT_TU_MODE={m}"]) for m in range(4)] + [("transform_static.cu", [])]
+DEPS = [os.path.join(CSRC, f) for f in ("gpuqt.cu", "step_kernels.cu", "kernels.cuh", "host_util.h", "slab_group.inl", "transform_static.cu")] + [
     os.path.join(os.path.dirname(HERE), "include", "gpuqt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
