@@ -209,7 +209,23 @@ def slabs_of_rank(n_slabs, rank, world):
 
 # ------------------------------------------------------------------ slabs on other ranks: CUDA IPC
 class _IpcHandle(C.Structure):
-    _fields_ = [("reserved", C.c_char * 64)]
+    """cudaIpcMemHandle_t: 64 opaque bytes.  Declared as unsigned bytes, not c_char: ctypes hands a c_char array back
+    as a Python bytes object cut at the first NUL, and a handle is binary data full of NULs."""
+    _fields_ = [("reserved", C.c_ubyte * 64)]
+
+
+def _handle_to_bytes(h):
+    """All 64 bytes of the handle, NULs included."""
+    return C.string_at(C.addressof(h), 64)
+
+
+def _handle_from_bytes(raw):
+    """A handle structure holding exactly the 64 bytes `raw`."""
+    if len(raw) != 64:
+        raise ValueError(f"a CUDA IPC handle has 64 bytes, got {len(raw)}")
+    h = _IpcHandle()
+    C.memmove(C.addressof(h), raw, 64)
+    return h
 
 
 def _cuda_libs():
@@ -222,7 +238,14 @@ def _cuda_libs():
             continue
     if rt is None:
         raise RuntimeError("libcudart not found (CUDA IPC needs it)")
-    return rt, C.CDLL("libcuda.so.1")
+    drv = C.CDLL("libcuda.so.1")
+    rt.cudaIpcGetMemHandle.restype = C.c_int
+    rt.cudaIpcGetMemHandle.argtypes = [C.POINTER(_IpcHandle), C.c_void_p]
+    rt.cudaIpcOpenMemHandle.restype = C.c_int
+    rt.cudaIpcOpenMemHandle.argtypes = [C.POINTER(C.c_void_p), _IpcHandle, C.c_uint]      # the handle goes by value
+    drv.cuMemGetAddressRange_v2.restype = C.c_int
+    drv.cuMemGetAddressRange_v2.argtypes = [C.POINTER(C.c_uint64), C.POINTER(C.c_size_t), C.c_uint64]
+    return rt, drv
 
 
 def _export_pointer(rt, drv, ptr):
@@ -233,7 +256,7 @@ def _export_pointer(rt, drv, ptr):
     h = _IpcHandle()
     if rt.cudaIpcGetMemHandle(C.byref(h), C.c_void_p(base.value)) != 0:
         raise RuntimeError("cudaIpcGetMemHandle failed")
-    return bytes(h.reserved), ptr - base.value
+    return _handle_to_bytes(h), ptr - base.value
 
 
 def connect_ranks(group, dist=None):
@@ -259,8 +282,7 @@ def connect_ranks(group, dist=None):
 
     def open_(handle, offset):
         if handle not in opened:
-            h, p = _IpcHandle(), C.c_void_p()
-            C.memmove(h.reserved, handle, 64)
+            h, p = _handle_from_bytes(handle), C.c_void_p()
             if rt.cudaIpcOpenMemHandle(C.byref(p), h, C.c_uint(1)) != 0:       # cudaIpcMemLazyEnablePeerAccess
                 raise RuntimeError("cudaIpcOpenMemHandle failed (peer access between the two GPUs is required)")
             opened[handle] = p.value

@@ -9,6 +9,7 @@
   arithmetic here is a stand-in written for the test; what is under test is the decomposition bookkeeping
   that the CUDA slabs use unchanged (tests/test_gpu_slab.py covers those against the oracle on the GPU).
 """
+import ctypes as C
 import os
 import socket
 
@@ -91,6 +92,21 @@ def test_partition_rejects_too_many_slabs():
     with pytest.raises(ValueError):
         slab.partition(L.chain(40, W=0.0, seed=1), 3)
     assert slab.slabs_of_rank(5, 1, 2) == [3, 4] and slab.slabs_of_rank(4, 0, 4) == [0]
+
+
+def test_ipc_handle_survives_nul_bytes():
+    """A cudaIpcMemHandle is 64 bytes of binary data; the marshalling in slab.connect_ranks must carry every byte,
+    NULs included (a c_char array would cut it at the first NUL), and refuse a handle of another length."""
+    from paper_1705_01387_b200 import slab
+    raw = bytes([7, 0, 0, 9] + [0] * 28 + list(range(32)))
+    assert len(raw) == 64 and raw[1] == 0
+    h = slab._handle_from_bytes(raw)
+    assert C.sizeof(h) == 64
+    assert slab._handle_to_bytes(h) == raw
+    assert bytes(h.reserved) == raw
+    assert slab._handle_to_bytes(slab._IpcHandle()) == bytes(64)
+    with pytest.raises(ValueError):
+        slab._handle_from_bytes(raw[:2])
 
 
 # ------------------------------------------------------------------------------- world_size 2 over gloo
