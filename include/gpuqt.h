@@ -190,7 +190,13 @@ int gpuqt_create_with_options(gpuqt_handle** out, int64_t N, int32_t K_max, cons
                  size_t workspace_bytes, void* cuda_stream, const gpuqt_options* options);
 
 /* Load B random vectors (Eq. 13; generated by the caller [A7]) and reset time to 0:
- * psi = phi, chi = 0, a = phi, b = V phi (Eq. 34).  phi: [batch][N][2].                          */
+ * psi = phi, chi = 0, a = phi, b = V phi (Eq. 34).  phi: [batch][N][2].
+ * gpuqt_set_state ENQUEUES the upload and the set-up kernels on the handle's stream and returns without
+ * synchronising (the exception to "complete when the call returns"; the next call on the handle is ordered
+ * behind it).  With pageable phi_host the runtime has staged the data by then; with PINNED phi_host the copy
+ * reads the buffer when the stream gets there, so keep it valid and unchanged until the stream has passed the
+ * copy (a synchronising call on the handle -- any moment call, gpuqt_get_state -- or a stream synchronise).
+ * gpuqt_slab_set_state behaves the same way.                                                      */
 int gpuqt_set_state(gpuqt_handle* h, const double* phi_host);
 int gpuqt_set_state_device(gpuqt_handle* h, const double* phi_device);
 /* The same in two halves, for the loop over the N_r random vector sets of a run: the upload of
@@ -370,27 +376,47 @@ typedef struct gpuqt_slab_desc {
 } gpuqt_slab_desc;
 size_t gpuqt_slab_workspace_bytes(int64_t n_own, int64_t n_halo, int32_t K_max, int is_complex, int32_t batch, int modes);
 /* Builds the slabs (each validated like gpuqt_create; Hermiticity is checked for the owned-owned block only).
- * Sends to slabs of this group are connected here; sends to other groups need gpuqt_slab_connect.  Errors of
- * this call: gpuqt_last_error(NULL).                                                                         */
+ * Sends to slabs of this group are connected here; sends to other groups need gpuqt_slab_connect.  Two local slabs
+ * with the same global_id are refused (GPUQT_ERR_ARG).  Errors of this call: gpuqt_last_error(NULL).           */
 int gpuqt_slab_create(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_desc* slabs, int32_t K_max,
                       double box_length, double volume, double energy_scale, int32_t batch, int modes,
                       void* cuda_stream);
-/* Device addresses another group needs to push into local slab `local_slab`: its vector buffers (in the fixed
- * order every slab uses; gpuqt_slab_buffer_count of them) and its flag array (uint32[GPUQT_MAX_SLABS]).  The
- * caller maps them into the peer process (CUDA IPC) and hands the mapped addresses to gpuqt_slab_connect there. */
+/* The same with explicit tuning options for every slab (NULL = defaults); small, persistent and reorder are
+ * ignored for slabs (one launch per recurrence step, the caller's row order).                                  */
+int gpuqt_slab_create_with_options(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_desc* slabs, int32_t K_max,
+                                   double box_length, double volume, double energy_scale, int32_t batch, int modes,
+                                   void* cuda_stream, const gpuqt_options* options);
+/* What another group needs to push into local slab `local_slab`: the device addresses of its vector buffers (in the
+ * fixed order every slab uses; gpuqt_slab_buffer_count of them) and of its flag array, and its row counts n_own /
+ * n_halo (either may be NULL).  The caller maps the addresses into the peer process (CUDA IPC) and hands the mapped
+ * addresses and the two counts to gpuqt_slab_connect there, which refuses (GPUQT_ERR_INDEX) a send segment that does
+ * not lie inside the peer's halo rows [peer_n_own, peer_n_own + peer_n_halo), and (GPUQT_ERR_ARG) a peer id that
+ * belongs to the connecting group itself.  Every slab of another group that a local slab sends to must be connected
+ * before the first compute call (GPUQT_ERR_STATE otherwise).                                                   */
 int32_t gpuqt_slab_buffer_count(const gpuqt_slab_group* g);
-int gpuqt_slab_export(gpuqt_slab_group* g, int32_t local_slab, void** buffers, void** flags);
-int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const* peer_buffers, void* peer_flags);
-/* phi_host[i]: host [batch][n_own of local slab i][2].  chi = 0; VAC mode: a = phi, b = V phi.                 */
+int gpuqt_slab_export(gpuqt_slab_group* g, int32_t local_slab, void** buffers, void** flags, int64_t* n_own,
+                      int64_t* n_halo);
+int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const* peer_buffers, void* peer_flags,
+                       int64_t peer_n_own, int64_t peer_n_halo);
+/* How long a halo exchange waits on the GPU for a slab of another group before it gives up (default 60 s; 0 <
+ * seconds <= 3600).  A wait that gave up surfaces as GPUQT_ERR_STATE from the call's next synchronisation
+ * (the moment calls, gpuqt_slab_get_state).  After that error, as after any error that strikes once a compute call
+ * has started issuing work, the group's buffers and exchange counter no longer match its peers': every further call
+ * returns GPUQT_ERR_STATE until the group is destroyed and rebuilt (on all ranks).                               */
+int gpuqt_slab_set_wait_budget(gpuqt_slab_group* g, double seconds);
+/* phi_host[i]: host [batch][n_own of local slab i][2].  chi = 0; VAC mode: a = phi, b = V phi.  Enqueued, not
+ * synchronised: pinned phi_host buffers must stay valid and unchanged as for gpuqt_set_state.                  */
 int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host);
-/* As gpuqt_dos_moments / gpuqt_evolve / gpuqt_vac / gpuqt_msd; moments: host [batch][n_moments], the partial
- * sums over this group's slabs.                                                                              */
+/* As gpuqt_dos_moments / gpuqt_evolve / gpuqt_vac / gpuqt_msd (gpuqt_slab_dos_moments answers in every mode, psi
+ * being set in every mode); moments: host [batch][n_moments], the partial sums over this group's slabs.        */
 int gpuqt_slab_dos_moments(gpuqt_slab_group* g, int32_t n_moments, double* out_host);
 int gpuqt_slab_evolve(gpuqt_slab_group* g, double dt, int32_t order);
 int gpuqt_slab_vac(gpuqt_slab_group* g, int32_t n_moments, double* out_host);
 int gpuqt_slab_msd(gpuqt_slab_group* g, int32_t n_moments, double* out_host);
 /* State of one local slab's owned rows: host [batch][n_own][2].                                               */
 int gpuqt_slab_get_state(gpuqt_slab_group* g, int32_t local_slab, int which, double* out_host);
+/* gpuqt_get_info (GPUQT_INFO_*) of one local slab: what the builder chose for its table.                      */
+int gpuqt_slab_get_info(gpuqt_slab_group* g, int32_t local_slab, int what, int64_t* value);
 const char* gpuqt_slab_last_error(const gpuqt_slab_group* g);
 void gpuqt_slab_destroy(gpuqt_slab_group* g);
 

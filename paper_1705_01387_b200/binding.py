@@ -89,14 +89,19 @@ _SIGNATURES = {
     "gpuqt_slab_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int32, C.POINTER(SlabDesc), C.c_int32, C.c_double, C.c_double,
                                     C.c_double, C.c_int32, C.c_int, C.c_void_p]),
     "gpuqt_slab_buffer_count": (C.c_int32, [C.c_void_p]),
-    "gpuqt_slab_export": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
-    "gpuqt_slab_connect": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.c_void_p]),
+    "gpuqt_slab_create_with_options": (C.c_int, [C.POINTER(C.c_void_p), C.c_int32, C.POINTER(SlabDesc), C.c_int32, C.c_double,
+                                                 C.c_double, C.c_double, C.c_int32, C.c_int, C.c_void_p, C.POINTER(Options)]),
+    "gpuqt_slab_export": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_int64),
+                                    C.POINTER(C.c_int64)]),
+    "gpuqt_slab_connect": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.c_void_p, C.c_int64, C.c_int64]),
+    "gpuqt_slab_set_wait_budget": (C.c_int, [C.c_void_p, C.c_double]),
     "gpuqt_slab_set_state": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
     "gpuqt_slab_dos_moments": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_slab_evolve": (C.c_int, [C.c_void_p, C.c_double, C.c_int32]),
     "gpuqt_slab_vac": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_slab_msd": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p]),
     "gpuqt_slab_get_state": (C.c_int, [C.c_void_p, C.c_int32, C.c_int, C.c_void_p]),
+    "gpuqt_slab_get_info": (C.c_int, [C.c_void_p, C.c_int32, C.c_int, C.POINTER(C.c_int64)]),
     "gpuqt_slab_last_error": (C.c_char_p, [C.c_void_p]),
     "gpuqt_slab_destroy": (None, [C.c_void_p]),
 }

@@ -33,14 +33,26 @@ __global__ void halo_signal_kernel(int n, unsigned int* const* __restrict__ flag
     __threadfence_system();
     asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(flags[k]), "r"(epoch) : "memory");
 }
-// my_flags[sender[k]] >= epoch for every remote sender k
-__global__ void halo_wait_kernel(int n, const unsigned int* __restrict__ my_flags, const int* __restrict__ sender, unsigned int epoch) {
+// my_flags[sender[k]] >= epoch for every remote sender k.  The spin is bounded: a sender that has not published
+// `epoch` within budget_ns (a peer that died, took an error path, or was never given the same sequence of calls)
+// makes the thread give up and raise *timed_out, which the host turns into GPUQT_ERR_STATE at its next
+// synchronisation instead of hanging the stream for ever.
+__global__ void halo_wait_kernel(int n, const unsigned int* __restrict__ my_flags, const int* __restrict__ sender, unsigned int epoch,
+                                 unsigned long long budget_ns, unsigned int* __restrict__ timed_out) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
+    unsigned long long t0, t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
     unsigned int v;
-    do {
+    for (;;) {
         asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(my_flags + sender[k]) : "memory");
-    } while ((int)(v - epoch) < 0);
+        if ((int)(v - epoch) >= 0) break;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        if (t - t0 > budget_ns) {
+            atomicExch(timed_out, 1u);
+            break;
+        }
+    }
     __threadfence_system();
 }
 // dst[i] += src[i]: the partial dots of the slabs of a group
@@ -68,15 +80,19 @@ struct gpuqt_slab_group {
     std::vector<std::vector<SlabSend>> sends;       // [local slab]
     std::map<int, SlabRemote> remote;               // by global id
     std::vector<int32_t*> d_rows;                   // per local slab: all send rows (device)
-    std::vector<unsigned int*> d_flags;             // per local slab: uint32[GPUQT_MAX_SLABS], written by remote senders
+    std::vector<unsigned int*> d_flags;             // per local slab: uint32[GPUQT_MAX_SLABS], written by remote senders,
+                                                    // + one word [GPUQT_MAX_SLABS] a timed-out wait of this slab raises
     // per local slab, rebuilt by gpuqt_slab_connect: where to signal, whom to wait for
     std::vector<unsigned int**> d_signal;
     std::vector<int*> d_senders;
     std::vector<int> n_remote;
     unsigned int epoch = 0;
+    unsigned long long wait_budget_ns = 60ull * 1000000000ull;     // gpuqt_slab_set_wait_budget
     cudaStream_t stream = nullptr;
     int B = 0, modes = 0;
     bool state_set = false;
+    bool poisoned = false;                          // an error struck in the middle of a sequence: see slab_done
+    std::string poison_reason;
     std::string err;
 };
 
@@ -131,19 +147,22 @@ int slab_exchange(gpuqt_slab_group* g, const std::vector<const double2*>& bufs) 
             }
         for (int i = 0; i < n; ++i)
             if (g->n_remote[(size_t)i] > 0) {
-                halo_wait_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[(size_t)i], g->d_flags[(size_t)i], g->d_senders[(size_t)i], g->epoch);
+                halo_wait_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[(size_t)i], g->d_flags[(size_t)i], g->d_senders[(size_t)i], g->epoch,
+                                                          g->wait_budget_ns, g->d_flags[(size_t)i] + GPUQT_MAX_SLABS);
                 GCU(cudaGetLastError());
             }
     }
     return GPUQT_OK;
 }
 
-// all remote peers have completed everything they issued before their matching slab_fence (no-op without remote peers)
+// all remote peers have completed everything they issued before their matching slab_fence (no launches without remote
+// peers).  The exchange number advances in every case, so that groups whose calls match keep matching numbers whatever
+// the order of their gpuqt_slab_connect calls was.
 int slab_fence(gpuqt_slab_group* g) {
+    ++g->epoch;
     bool any = false;
     for (int r : g->n_remote) any = any || r > 0;
     if (!any) return GPUQT_OK;
-    ++g->epoch;
     for (size_t i = 0; i < g->h.size(); ++i)
         if (g->n_remote[i] > 0) {
             halo_signal_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[i], g->d_signal[i], g->epoch);
@@ -151,9 +170,47 @@ int slab_fence(gpuqt_slab_group* g) {
         }
     for (size_t i = 0; i < g->h.size(); ++i)
         if (g->n_remote[i] > 0) {
-            halo_wait_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[i], g->d_flags[i], g->d_senders[i], g->epoch);
+            halo_wait_kernel<<<1, 64, 0, g->stream>>>(g->n_remote[i], g->d_flags[i], g->d_senders[i], g->epoch, g->wait_budget_ns,
+                                                      g->d_flags[i] + GPUQT_MAX_SLABS);
             GCU(cudaGetLastError());
         }
+    return GPUQT_OK;
+}
+
+// Before any work is issued: the group is usable and every slab of another group that a local slab sends to has been
+// connected (an exchange that found a peer missing half way would leave the groups' exchange numbers apart).
+int slab_ready(gpuqt_slab_group* g) {
+    if (g->poisoned)
+        return gfail(g, GPUQT_ERR_STATE, "the group is unusable after an earlier error in the middle of a sequence (" + g->poison_reason +
+                                             "); destroy it and build a new one");
+    for (size_t i = 0; i < g->h.size(); ++i)
+        for (const SlabSend& s : g->sends[i])
+            if (s.peer_local < 0 && g->remote.find(s.peer_global) == g->remote.end())
+                return gfail(g, GPUQT_ERR_STATE, "slab " + std::to_string(s.peer_global) + " is not connected (gpuqt_slab_connect)");
+    return GPUQT_OK;
+}
+
+// The end of a compute call that had started issuing work: after an error the states, the ring buffers and the
+// exchange number no longer mean on this side what they mean on the peers' side, so the group refuses further work.
+int slab_done(gpuqt_slab_group* g, int rc) {
+    if (rc != GPUQT_OK && !g->poisoned) {
+        g->poisoned = true;
+        g->poison_reason = g->err;
+    }
+    return rc;
+}
+
+// Wait for the stream, then ask whether a wait for a remote sender gave up.
+int slab_sync(gpuqt_slab_group* g) {
+    GCU(cudaStreamSynchronize(g->stream));
+    for (size_t i = 0; i < g->h.size(); ++i) {
+        if (g->n_remote[i] == 0) continue;
+        unsigned int gave_up = 0;
+        GCU(cudaMemcpy(&gave_up, g->d_flags[i] + GPUQT_MAX_SLABS, sizeof(gave_up), cudaMemcpyDeviceToHost));
+        if (gave_up)
+            return gfail(g, GPUQT_ERR_STATE, "a slab of another group did not arrive at a halo exchange within " +
+                                                 std::to_string((double)g->wait_budget_ns * 1e-9) + " s (gpuqt_slab_set_wait_budget)");
+    }
     return GPUQT_OK;
 }
 
@@ -207,9 +264,9 @@ int slab_sum_dots(gpuqt_slab_group* g, long long n_values) {
 
 int slab_copy_moments(gpuqt_slab_group* g, int n_moments, double* out_host) {
     GCU(cudaMemcpyAsync(out_host, g->h[0]->moments, (size_t)g->B * n_moments * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
-    GCU(cudaStreamSynchronize(g->stream));
+    const int rc = slab_sync(g);
     for (gpuqt_handle* h : g->h) flush_stats(h);
-    return GPUQT_OK;
+    return rc;
 }
 
 // C_n = <v|T_n|v> with the doubling identity, v = psi or chi of every slab
@@ -289,6 +346,13 @@ size_t gpuqt_slab_workspace_bytes(int64_t n_own, int64_t n_halo, int32_t K_max, 
 int gpuqt_slab_create(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_desc* slabs, int32_t K_max,
                       double box_length, double volume, double energy_scale, int32_t batch, int modes,
                       void* cuda_stream) {
+    return gpuqt_slab_create_with_options(out, n_local, slabs, K_max, box_length, volume, energy_scale, batch, modes,
+                                          cuda_stream, nullptr);
+}
+
+int gpuqt_slab_create_with_options(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_desc* slabs, int32_t K_max,
+                                   double box_length, double volume, double energy_scale, int32_t batch, int modes,
+                                   void* cuda_stream, const gpuqt_options* options) {
     auto bad = [&](int code, const std::string& msg) {
         g_create_error = "gpuqt_slab_create: " + msg;
         return code;
@@ -310,10 +374,13 @@ int gpuqt_slab_create(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_
         if (d.global_id < 0 || d.global_id >= GPUQT_MAX_SLABS || d.n_sends < 0 || d.n_halo < 0 ||
             (d.n_sends > 0 && (!d.send_peer || !d.send_count || !d.send_dst_row || !d.send_rows)))
             return fail_create(GPUQT_ERR_ARG, "bad descriptor of local slab " + std::to_string(i));
+        for (int j = 0; j < i; ++j)
+            if (slabs[j].global_id == d.global_id)
+                return fail_create(GPUQT_ERR_ARG, "global id " + std::to_string(d.global_id) + " is given to two local slabs");
         gpuqt_handle* h = nullptr;
         int rc = create_handle(&h, d.n_own, d.n_halo, K_max, d.nbr_count, d.nbr_index, d.hop_re, d.hop_im, d.onsite, d.x,
                                box_length, volume, energy_scale, batch, modes, d.workspace, d.workspace_bytes, cuda_stream,
-                               nullptr, true);
+                               options, true);
         if (rc != GPUQT_OK) {
             const std::string why = g_create_error;
             gpuqt_slab_destroy(g);
@@ -344,8 +411,8 @@ int gpuqt_slab_create(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_
             e = cudaMalloc((void**)&g->d_rows[(size_t)i], (size_t)total * sizeof(int32_t));
             if (e == cudaSuccess) e = cudaMemcpy(g->d_rows[(size_t)i], d.send_rows, (size_t)total * sizeof(int32_t), cudaMemcpyHostToDevice);
         }
-        if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_flags[(size_t)i], GPUQT_MAX_SLABS * sizeof(unsigned int));
-        if (e == cudaSuccess) e = cudaMemset(g->d_flags[(size_t)i], 0, GPUQT_MAX_SLABS * sizeof(unsigned int));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_flags[(size_t)i], (GPUQT_MAX_SLABS + 1) * sizeof(unsigned int));
+        if (e == cudaSuccess) e = cudaMemset(g->d_flags[(size_t)i], 0, (GPUQT_MAX_SLABS + 1) * sizeof(unsigned int));
         if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_signal[(size_t)i], GPUQT_MAX_SLABS * sizeof(unsigned int*));
         if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_senders[(size_t)i], GPUQT_MAX_SLABS * sizeof(int));
         if (e != cudaSuccess) return fail_create(GPUQT_ERR_CUDA, std::string("send lists: ") + cudaGetErrorString(e));
@@ -375,22 +442,35 @@ int gpuqt_slab_create(gpuqt_slab_group** out, int32_t n_local, const gpuqt_slab_
 
 int32_t gpuqt_slab_buffer_count(const gpuqt_slab_group* g) { return g && !g->h.empty() ? (int32_t)g->h[0]->map_bufs.size() : 0; }
 
-int gpuqt_slab_export(gpuqt_slab_group* g, int32_t local_slab, void** buffers, void** flags) {
+int gpuqt_slab_export(gpuqt_slab_group* g, int32_t local_slab, void** buffers, void** flags, int64_t* n_own, int64_t* n_halo) {
     if (!g || local_slab < 0 || local_slab >= (int32_t)g->h.size() || !buffers || !flags) return gfail(g, GPUQT_ERR_ARG, "bad argument");
     const gpuqt_handle* h = g->h[(size_t)local_slab];
     for (size_t i = 0; i < h->map_bufs.size(); ++i) buffers[i] = (void*)h->map_bufs[i];
     *flags = g->d_flags[(size_t)local_slab];
+    if (n_own) *n_own = h->N;
+    if (n_halo) *n_halo = h->NV - h->N;
     return GPUQT_OK;
 }
 
-int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const* peer_buffers, void* peer_flags) {
-    if (!g || !peer_buffers || !peer_flags || peer_global_id < 0 || peer_global_id >= GPUQT_MAX_SLABS)
+int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const* peer_buffers, void* peer_flags,
+                       int64_t peer_n_own, int64_t peer_n_halo) {
+    if (!g || !peer_buffers || !peer_flags || peer_global_id < 0 || peer_global_id >= GPUQT_MAX_SLABS || peer_n_own < 1 ||
+        peer_n_halo < 0)
         return gfail(g, GPUQT_ERR_ARG, "bad argument");
+    for (int id : g->global_id)
+        if (id == peer_global_id) return gfail(g, GPUQT_ERR_ARG, "slab " + std::to_string(peer_global_id) + " belongs to this group");
+    // every segment sent to this peer must land inside its halo rows (the pushes are plain stores into its memory)
+    for (size_t i = 0; i < g->h.size(); ++i)
+        for (const SlabSend& s : g->sends[i])
+            if (s.peer_global == peer_global_id && (s.dst_row0 < peer_n_own || s.dst_row0 + s.n_rows > peer_n_own + peer_n_halo))
+                return gfail(g, GPUQT_ERR_INDEX, "a send segment of local slab " + std::to_string(i) + " lies outside the halo rows of slab " +
+                                                     std::to_string(peer_global_id));
     SlabRemote r;
     for (int32_t i = 0; i < gpuqt_slab_buffer_count(g); ++i) r.bufs.push_back((double2*)peer_buffers[i]);
     r.flags = (unsigned int*)peer_flags;
     g->remote[peer_global_id] = r;
-    // per local slab: the remote slabs it sends to (= the remote slabs that send to it: H is Hermitian [A10])
+    // per local slab: the remote slabs it sends to (= the remote slabs that send to it: H is Hermitian [A10]), each ONCE
+    // however many segments go there -- at most GPUQT_MAX_SLABS - 1 entries, the size of d_signal / d_senders
     for (size_t i = 0; i < g->h.size(); ++i) {
         std::vector<unsigned int*> sig;
         std::vector<int> snd;
@@ -398,6 +478,9 @@ int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const*
             if (s.peer_local >= 0) continue;
             auto it = g->remote.find(s.peer_global);
             if (it == g->remote.end()) continue;
+            bool listed = false;
+            for (int p : snd) listed = listed || p == s.peer_global;
+            if (listed) continue;
             sig.push_back(it->second.flags + g->global_id[i]);
             snd.push_back(s.peer_global);
         }
@@ -410,12 +493,16 @@ int gpuqt_slab_connect(gpuqt_slab_group* g, int32_t peer_global_id, void* const*
     return GPUQT_OK;
 }
 
-int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host) {
-    if (!g || !phi_host) return gfail(g, GPUQT_ERR_ARG, "null argument");
+int gpuqt_slab_set_wait_budget(gpuqt_slab_group* g, double seconds) {
+    if (!g || !(seconds > 0.0) || !(seconds <= 3600.0)) return gfail(g, GPUQT_ERR_ARG, "the wait budget must lie in (0, 3600] seconds");
+    g->wait_budget_ns = (unsigned long long)(seconds * 1e9);
+    return GPUQT_OK;
+}
+
+static int slab_set_state_body(gpuqt_slab_group* g, const double* const* phi_host) {
     const size_t n = g->h.size();
     for (size_t i = 0; i < n; ++i) {
         gpuqt_handle* h = g->h[i];
-        if (!phi_host[i]) return gfail(g, GPUQT_ERR_ARG, "null state of a slab");
         GCU(cudaMemcpyAsync(h->ring[0], phi_host[i], h->vec_elems * sizeof(double2), cudaMemcpyHostToDevice, g->stream));
         const long long total = (long long)h->vec_elems;
         const int blocks = (int)((total + 255) / 256);
@@ -439,30 +526,40 @@ int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host) {
     return GPUQT_OK;
 }
 
+int gpuqt_slab_set_state(gpuqt_slab_group* g, const double* const* phi_host) {
+    if (!g || !phi_host) return gfail(g, GPUQT_ERR_ARG, "null argument");
+    for (size_t i = 0; i < g->h.size(); ++i)
+        if (!phi_host[i]) return gfail(g, GPUQT_ERR_ARG, "null state of a slab");
+    if (g->poisoned || (g->modes & GPUQT_MODE_VAC)) {          // b = V phi exchanges halos: every send peer must be there
+        const int ready = slab_ready(g);
+        if (ready) return ready;
+    }
+    return slab_done(g, slab_set_state_body(g, phi_host));
+}
+
 static int slab_check_moments(gpuqt_slab_group* g, int32_t n_moments, const double* out_host, int need_mode) {
     if (!g || !out_host || n_moments < 2 || n_moments > GPUQT_MAX_MOMENTS) return gfail(g, GPUQT_ERR_ARG, "bad n_moments or null output");
     if (need_mode && !(g->modes & need_mode)) return gfail(g, GPUQT_ERR_STATE, "group was created without the mode this call needs");
     if (!g->state_set) return gfail(g, GPUQT_ERR_STATE, "gpuqt_slab_set_state has not been called");
-    return GPUQT_OK;
+    return slab_ready(g);
 }
 
+// As gpuqt_dos_moments: psi is allocated and set in every mode, so a VAC-only group answers too.
 int gpuqt_slab_dos_moments(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
     int rc = slab_check_moments(g, n_moments, out_host, 0);
     if (rc) return rc;
-    if (!(g->modes & (GPUQT_MODE_PSI | GPUQT_MODE_MSD))) return gfail(g, GPUQT_ERR_STATE, "DOS moments need GPUQT_MODE_PSI or _MSD");
-    return slab_moments_doubling(g, false, n_moments, out_host);
+    return slab_done(g, slab_moments_doubling(g, false, n_moments, out_host));
 }
 
 int gpuqt_slab_msd(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
     int rc = slab_check_moments(g, n_moments, out_host, GPUQT_MODE_MSD);
     if (rc) return rc;
-    return slab_moments_doubling(g, true, n_moments, out_host);
+    return slab_done(g, slab_moments_doubling(g, true, n_moments, out_host));
 }
 
-int gpuqt_slab_vac(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
-    int rc = slab_check_moments(g, n_moments, out_host, GPUQT_MODE_VAC);
-    if (rc) return rc;
+static int slab_vac_body(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
     const size_t n = g->h.size();
+    int rc;
     // phi_L = V a (needs the halo rows of a); C_0 = <phi_L|b>
     rc = slab_fence(g);
     if (rc == GPUQT_OK) rc = slab_exchange(g, each_buffer(g, [&](size_t i) { return (const double2*)g->h[i]->va; }));
@@ -491,9 +588,13 @@ int gpuqt_slab_vac(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
     return slab_copy_moments(g, n_moments, out_host);
 }
 
-int gpuqt_slab_evolve(gpuqt_slab_group* g, double dt, int32_t order) {
-    if (!g || order < 1 || order > GPUQT_MAX_ORDER || !std::isfinite(dt)) return gfail(g, GPUQT_ERR_ARG, "bad dt or order");
-    if (!g->state_set) return gfail(g, GPUQT_ERR_STATE, "gpuqt_slab_set_state has not been called");
+int gpuqt_slab_vac(gpuqt_slab_group* g, int32_t n_moments, double* out_host) {
+    int rc = slab_check_moments(g, n_moments, out_host, GPUQT_MODE_VAC);
+    if (rc) return rc;
+    return slab_done(g, slab_vac_body(g, n_moments, out_host));
+}
+
+static int slab_evolve_body(gpuqt_slab_group* g, double dt, int32_t order) {
     int rc;
     auto swap_all = [&](double2* gpuqt_handle::*a, double2* gpuqt_handle::*b) {
         for (gpuqt_handle* h : g->h) std::swap(h->*a, h->*b);
@@ -527,10 +628,30 @@ int gpuqt_slab_evolve(gpuqt_slab_group* g, double dt, int32_t order) {
     return GPUQT_OK;
 }
 
+int gpuqt_slab_evolve(gpuqt_slab_group* g, double dt, int32_t order) {
+    if (!g || order < 1 || order > GPUQT_MAX_ORDER || !std::isfinite(dt)) return gfail(g, GPUQT_ERR_ARG, "bad dt or order");
+    if (!g->state_set) return gfail(g, GPUQT_ERR_STATE, "gpuqt_slab_set_state has not been called");
+    int rc = slab_ready(g);
+    if (rc) return rc;
+    return slab_done(g, slab_evolve_body(g, dt, order));
+}
+
 int gpuqt_slab_get_state(gpuqt_slab_group* g, int32_t local_slab, int which, double* out_host) {
     if (!g || local_slab < 0 || local_slab >= (int32_t)g->h.size() || !out_host) return gfail(g, GPUQT_ERR_ARG, "bad argument");
+    if (g->poisoned) return slab_ready(g);
     gpuqt_handle* h = g->h[(size_t)local_slab];
-    int rc = gpuqt_get_state(h, which, out_host);
+    int rc = gpuqt_get_state(h, which, out_host);           // synchronises the stream
+    if (rc) {
+        g->err = h->err;
+        return rc;
+    }
+    return slab_done(g, slab_sync(g));                      // a wait that gave up leaves halo rows, hence states, undefined
+}
+
+int gpuqt_slab_get_info(gpuqt_slab_group* g, int32_t local_slab, int what, int64_t* value) {
+    if (!g || local_slab < 0 || local_slab >= (int32_t)g->h.size() || !value) return gfail(g, GPUQT_ERR_ARG, "bad argument");
+    gpuqt_handle* h = g->h[(size_t)local_slab];
+    const int rc = gpuqt_get_info(h, what, value);
     if (rc) g->err = h->err;
     return rc;
 }

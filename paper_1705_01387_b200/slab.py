@@ -97,7 +97,7 @@ def partition(model, n_slabs):
 class SlabGroup:
     """The slabs `mine` (global ids; default all) of a decomposition on the current CUDA device."""
 
-    def __init__(self, model, slabs, mine=None, batch=1, modes=binding.MODE_VAC | binding.MODE_MSD, stream=None):
+    def __init__(self, model, slabs, mine=None, batch=1, modes=binding.MODE_VAC | binding.MODE_MSD, stream=None, options=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("gpuqt needs a CUDA device (no CPU fallback)")
@@ -131,9 +131,10 @@ class SlabGroup:
             d.send_rows = rows.ctypes.data_as(C.POINTER(C.c_int32))
             d.workspace, d.workspace_bytes = ws.data_ptr(), nbytes
         self._g = C.c_void_p()
-        rc = lib.gpuqt_slab_create(C.byref(self._g), len(self.slabs), descs, model.K, C.c_double(model.box_length),
-                                   C.c_double(model.volume), C.c_double(model.energy_scale), batch, modes,
-                                   C.c_void_p(self.stream.cuda_stream))
+        self.options = binding.default_options(**(options or {}))
+        rc = lib.gpuqt_slab_create_with_options(C.byref(self._g), len(self.slabs), descs, model.K, C.c_double(model.box_length),
+                                                C.c_double(model.volume), C.c_double(model.energy_scale), batch, modes,
+                                                C.c_void_p(self.stream.cuda_stream), C.byref(self.options))
         if rc:
             self._g = C.c_void_p()
             raise binding.GpuqtError(rc, "gpuqt_slab_create", (lib.gpuqt_last_error(None) or b"").decode())
@@ -152,6 +153,34 @@ class SlabGroup:
             self.close()
         except Exception:
             pass
+
+    def info(self, i, what):
+        """gpuqt_slab_get_info of local slab i (binding.INFO_*)."""
+        v = C.c_int64()
+        self._ck(binding.load().gpuqt_slab_get_info(self._g, i, what, C.byref(v)), "gpuqt_slab_get_info")
+        return v.value
+
+    def hop_variants(self):
+        """The record variant (GPUQT_INFO_HOP_VARIANT) of every local slab."""
+        return [self.info(i, binding.INFO_HOP_VARIANT) for i in range(len(self.slabs))]
+
+    def set_wait_budget(self, seconds):
+        """How long a halo exchange waits for a slab of another group before the call fails (gpuqt_slab_set_wait_budget)."""
+        self._ck(binding.load().gpuqt_slab_set_wait_budget(self._g, C.c_double(seconds)), "gpuqt_slab_set_wait_budget")
+
+    def export(self, i):
+        """gpuqt_slab_export of local slab i: (buffer addresses, flag array address, n_own, n_halo)."""
+        lib = binding.load()
+        bufs, flags = (C.c_void_p * lib.gpuqt_slab_buffer_count(self._g))(), C.c_void_p()
+        n_own, n_halo = C.c_int64(), C.c_int64()
+        self._ck(lib.gpuqt_slab_export(self._g, i, bufs, C.byref(flags), C.byref(n_own), C.byref(n_halo)), "gpuqt_slab_export")
+        return [int(b) for b in bufs], flags.value, n_own.value, n_halo.value
+
+    def connect(self, peer_global_id, buffers, flags, n_own, n_halo):
+        """gpuqt_slab_connect: addresses (valid in THIS process) and row counts of a slab held by another group."""
+        ptrs = (C.c_void_p * len(buffers))(*buffers)
+        self._ck(binding.load().gpuqt_slab_connect(self._g, peer_global_id, ptrs, C.c_void_p(flags), C.c_int64(n_own),
+                                                   C.c_int64(n_halo)), "gpuqt_slab_connect")
 
     def set_state(self, phi):
         """phi: host [batch][N][2] of the GLOBAL lattice; every local slab takes its rows."""
@@ -267,14 +296,11 @@ def connect_ranks(group, dist=None):
     one group and need no connection.)"""
     if dist is None:
         import torch.distributed as dist
-    lib = binding.load()
     rt, drv = _cuda_libs()
-    n_buf = lib.gpuqt_slab_buffer_count(group._g)
     mine = {}
     for i, s in enumerate(group.slabs):
-        bufs, flags = (C.c_void_p * n_buf)(), C.c_void_p()
-        group._ck(lib.gpuqt_slab_export(group._g, i, bufs, C.byref(flags)), "gpuqt_slab_export")
-        mine[s.global_id] = ([_export_pointer(rt, drv, int(b)) for b in bufs], _export_pointer(rt, drv, flags.value))
+        bufs, flags, n_own, n_halo = group.export(i)
+        mine[s.global_id] = ([_export_pointer(rt, drv, b) for b in bufs], _export_pointer(rt, drv, flags), n_own, n_halo)
     everyone = [None] * dist.get_world_size()
     dist.all_gather_object(everyone, mine)
     wanted = {peer for s in group.slabs for peer, _, _ in s.sends} - {s.global_id for s in group.slabs}
@@ -289,9 +315,8 @@ def connect_ranks(group, dist=None):
         return opened[handle] + offset
 
     for published in everyone:
-        for gid, (bufs, flags) in published.items():
+        for gid, (bufs, flags, n_own, n_halo) in published.items():
             if gid in wanted:
-                ptrs = (C.c_void_p * n_buf)(*[open_(h, off) for h, off in bufs])
-                group._ck(lib.gpuqt_slab_connect(group._g, gid, ptrs, C.c_void_p(open_(*flags))), "gpuqt_slab_connect")
+                group.connect(gid, [open_(h, off) for h, off in bufs], open_(*flags), n_own, n_halo)
     group._ipc = opened
     dist.barrier()
