@@ -2,16 +2,20 @@
 options, the config's own batch B, N_m and N_p).
 
 The oracle cannot run a whole config in seconds, so it follows the parity schedule of SURVEY.md
-8(d): ONE sampled random vector (the last slot of the batch, so the [N][B] interleave is exercised)
-at full N; the oracle runs the evolutions of the schedule and the evolved state vectors of the sample
-are compared element by element; the sample's moments are compared over the WHOLE N_m at the first
-and at the last measured time step and on the prefix n < 64 at every step in between (C_n does not
-depend on N_m [A19]).  c1 and c2 run all their time steps; c3 and c4 run the first STEPS[key] of
-them (all of them with GPUQT_PARITY_ALL_STEPS=1); c5's oracle cost (1.6e7 orbitals, complex
-hoppings, N_m = 3000) allows the prefix only, and its full depth is covered on a reduced lattice of
-the same family (test_c5_family_full_depth).  Properties that hold at any size cover the other B - 1
-vectors: C_0 = <phi|phi> = N, norm conservation of U, |C_n| <= ||phi_L|| ||phi_R||, run-to-run bit
-identity.
+8(d): ONE sampled random vector (slot SLOT[key] of the batch, an inner slot, so the [N][B] interleave
+is exercised) at full N through the config's OWN number of time steps; the oracle runs the evolutions
+of the schedule and the evolved state vectors of the sample are compared element by element; the
+sample's moments are compared over the WHOLE N_m at the first and at the last measured time step and
+on the prefix n < 64 at every step in between (C_n does not depend on N_m [A19]).  Before that, EVERY
+slot of the batch goes through one time step against the oracle (states element by element, prefix
+moments), so no slot is left to properties alone.  c1-c4 run all their time steps (10, 20, 50, 40).
+c5 (1.6e7 orbitals, complex hoppings, N_m = 3000, 30 steps) runs its first 2 steps with prefix moments
+by default; GPUQT_PARITY_ALL_STEPS=1 runs all 30, GPUQT_PARITY_C5_FULL=1 adds the full N_m = 3000 VAC
+comparison at full N at the first measured step (minutes of host time each: run once per round under
+gpurun, log in profiles/r3_parity_full_schedule.txt); its full depth is also covered on a reduced
+lattice of the same family in every run (test_c5_family_full_depth).  Properties that hold at any
+size cover the other B - 1 vectors beyond the first step: C_0 = <phi|phi> = N, norm conservation of U,
+|C_n| <= ||phi_L|| ||phi_R||, run-to-run bit identity.
 
 Tolerances as in test_gpu_parity.py (north_star: 1e-10 in the norms of A22; tables bit-exact).
 """
@@ -28,7 +32,9 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-10
 PREFIX = 64
 ALL_STEPS = os.environ.get("GPUQT_PARITY_ALL_STEPS", "0") == "1"
-STEPS = {"c1": 10, "c2": 20, "c3": 8, "c4": 8, "c5": 2}        # time steps run here (c1, c2: all of them)
+C5_FULL = os.environ.get("GPUQT_PARITY_C5_FULL", "0") == "1"
+STEPS = {"c1": 10, "c2": 20, "c3": 50, "c4": 40, "c5": 2}      # time steps run here (c1-c4: all of them)
+SLOT = {"c4": 2, "c5": 5}                                      # the vector of the batch the oracle follows (default 0)
 
 
 @pytest.fixture(scope="module")
@@ -48,13 +54,46 @@ def norm(v):
     return float(np.sqrt(np.sum(v * v)))
 
 
-def run_schedule(gq, oracle_mod, w, model, n_steps, full_depth, vector_checks):
-    """The schedule of the module docstring for one workload; `full_depth`: compare all N_m moments at
-    the first and last measured step (else the prefix there as well); `vector_checks`: the steps (0-based)
-    after whose evolution the state vectors are compared."""
+def every_slot_one_step(gq, oracle_mod, w, model, g, o, phi):
+    """One time step of EVERY vector of the batch against the oracle (one vector at a time on the host): evolved
+    states element by element, the first PREFIX moments in the A22 norms."""
+    B, P = w.batch, min(PREFIX, w.n_moments)
+    g.set_state(phi)
+    g.evolve(w.dt, w.order)
+    if w.path == "vac":
+        got = {gq.STATE_VAC_A: g.get_state(gq.STATE_VAC_A), gq.STATE_VAC_B: g.get_state(gq.STATE_VAC_B)}
+        names = {gq.STATE_VAC_A: oracle_mod.VAC_A, gq.STATE_VAC_B: oracle_mod.VAC_B}
+        mom = g.vac(P)
+    else:
+        got = {gq.STATE_PSI: g.get_state(gq.STATE_PSI), gq.STATE_CHI: g.get_state(gq.STATE_CHI)}
+        names = {gq.STATE_PSI: oracle_mod.PSI, gq.STATE_CHI: oracle_mod.CHI}
+        mom = g.msd(P)
+    worst = 0.0
+    for b in range(B):
+        o.set_state(phi[b:b + 1])
+        o.evolve(w.dt, w.order)
+        for which, ow in names.items():
+            err = vec_err(got[which][b], o.get_state(ow)[0])
+            assert err <= TOL, (b, which, err)
+        if w.path == "vac":
+            scale = norm(o.apply_v(o.get_state(oracle_mod.VAC_A)[0])) * norm(o.get_state(oracle_mod.VAC_B)[0])
+            err = np.max(np.abs(mom[b] - o.vac(P)[0])) / scale
+        else:
+            err = np.max(np.abs(mom[b] - o.msd(P)[0])) / norm(o.get_state(oracle_mod.CHI)[0]) ** 2
+        worst = max(worst, err)
+        assert err <= TOL, (b, err)
+    print(f"{w.key}: every slot of B={B} through one step: worst moment error {worst:.2e}")
+
+
+def run_schedule(gq, oracle_mod, w, model, n_steps, full_depth, vector_checks, full_at=None, dos_full=None, sb=0):
+    """The schedule of the module docstring for one workload; `full_depth`: compare all N_m moments at the measured
+    steps `full_at` (default: the first and the last; else the prefix there as well) and, with `dos_full` (default:
+    full_depth), of the DOS; `vector_checks`: the steps (0-based) after whose evolution the state vectors are compared;
+    `sb`: the slot of the batch the oracle follows."""
     order = w.order
     B, nm = w.batch, w.n_moments
-    sb = B - 1                                        # sampled vector
+    full_at = {0, n_steps - 1} if full_at is None else full_at
+    dos_full = full_depth if dos_full is None else dos_full
     phi = w.phases(model)
     modes_g = gq.MODE_MSD if w.path == "msd" else gq.MODE_VAC
     modes_o = oracle_mod.MODE_MSD if w.path == "msd" else oracle_mod.MODE_VAC
@@ -65,18 +104,21 @@ def run_schedule(gq, oracle_mod, w, model, n_steps, full_depth, vector_checks):
     for a, b in zip(g.get_table(), o.get_table()):
         assert a.tobytes() == b.tobytes()
 
+    if B > 1:
+        every_slot_one_step(gq, oracle_mod, w, model, g, o, phi)
+
     g.set_state(phi)
     o.set_state(phi[sb:sb + 1])
 
     def depth(k):                                     # moments the oracle computes at measured step k
-        return nm if (full_depth and k in (0, n_steps - 1)) else min(PREFIX, nm)
+        return nm if (full_depth and k in full_at) else min(PREFIX, nm)
 
     # a6 (DOS): full N_m on the GPU
     dos = g.dos_moments(nm)
     assert dos.shape == (B, nm)
     assert np.max(np.abs(dos[:, 0] - model.N)) <= TOL * model.N            # C_0 = <phi|phi> = N  [A7]
     assert np.max(np.abs(dos)) <= model.N * (1 + 1e-9)                     # |T_n| <= 1 on the spectrum
-    P = nm if full_depth else min(PREFIX, nm)
+    P = nm if dos_full else min(PREFIX, nm)
     assert np.max(np.abs(dos[sb, :P] - o.dos_moments(P)[0])) / model.N <= TOL
 
     worst = 0.0
@@ -125,7 +167,9 @@ def run_schedule(gq, oracle_mod, w, model, n_steps, full_depth, vector_checks):
             assert err <= TOL, (k, P, err)
         again = g.msd(nm)                                                 # fixed-order reductions
         assert again.tobytes() == msd.tobytes()
-    print(f"{w.key}: N={model.N} B={B} N_m={nm} steps={n_steps}: worst moment error {worst:.2e} (A22 norm)")
+    deep = sorted(k for k in full_at if 0 <= k < n_steps) if full_depth else []
+    print(f"{w.key}: N={model.N} B={B} slot={sb} N_m={nm} steps={n_steps} (all N_m at steps {deep}, n < {PREFIX} elsewhere): "
+          f"worst moment error {worst:.2e} (A22 norm), states at steps {sorted(k for k in vector_checks if 0 <= k < n_steps)} <= {TOL:g}")
     g.close()
     o.close()
 
@@ -135,8 +179,12 @@ def test_full_size_config(gq, oracle_mod, key):
     w = configs.WORKLOADS[key]
     model = w.build()
     n_steps = w.n_steps if ALL_STEPS else min(STEPS[key], w.n_steps)
-    checks = {0, 1, n_steps - 2, n_steps - 1}
-    run_schedule(gq, oracle_mod, w, model, n_steps, full_depth=(key != "c5"), vector_checks=checks)
+    checks = {0, 1, n_steps // 2, n_steps - 2, n_steps - 1}
+    if key == "c5":           # full N_m = 3000 of the VAC at the first measured step only, and only on request
+        run_schedule(gq, oracle_mod, w, model, n_steps, full_depth=C5_FULL, vector_checks=checks, full_at={0}, dos_full=False,
+                     sb=SLOT[key])
+    else:
+        run_schedule(gq, oracle_mod, w, model, n_steps, full_depth=True, vector_checks=checks, sb=SLOT.get(key, 0))
 
 
 def test_c5_family_full_depth(gq, oracle_mod):
