@@ -544,6 +544,19 @@ def main():
     args = ap.parse_args()
     args.options = {k: int(v) for k, v in (kv.split("=", 1) for kv in args.opt)}
     w = configs.WORKLOADS[args.config]
+    from paper_1705_01387_b200 import replicas
+    if args.impl == "ours" and args.slabs == 0 and replicas.needs_launch(args.gpus):
+        # --gpus N without torchrun around it: start the N ranks ourselves (one process per GPU, NCCL), rank 0 prints
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            sys.exit(f"bench.py: --gpus {args.gpus} but {have} CUDA device(s) are visible")
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")          # the communicator lines (transport, NVLS) go to stderr
+        cmd = replicas.launch_command(os.path.abspath(__file__), sys.argv[1:], args.gpus, replicas.free_port())
+        sys.exit(subprocess.call(cmd, env=env))
+    if args.impl == "ours" and args.slabs == 0 and args.gpus != replicas.world()[2]:
+        sys.exit(f"bench.py: --gpus {args.gpus} does not match WORLD_SIZE={replicas.world()[2]}")
     if args.impl == "reference":
         run_reference(args, w)
     elif args.slabs > 0:

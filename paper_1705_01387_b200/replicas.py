@@ -12,6 +12,29 @@ def world():
             int(os.environ.get("WORLD_SIZE", "1")))
 
 
+def launch_command(script, argv, n_ranks, port, python=None):
+    """The command that starts `script argv...` as `n_ranks` ranks of one node, one process per GPU -- the same
+    launch the bench contract uses (`python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr
+    127.0.0.1 --master-port P script ...`).  bench.py re-executes itself with it when it is asked for --gpus N > 1
+    outside a torchrun environment."""
+    import sys
+    return [python or sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={int(n_ranks)}",
+            "--master-addr", "127.0.0.1", "--master-port", str(int(port)), script, *argv]
+
+
+def needs_launch(n_gpus: int, env=None) -> bool:
+    """True when more than one rank is wanted and this process was not started by torchrun (no WORLD_SIZE)."""
+    env = os.environ if env is None else env
+    return n_gpus > 1 and "WORLD_SIZE" not in env
+
+
+def free_port() -> int:
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
 def first_vector(rank: int, batch: int) -> int:
     """Rank r owns the global random vectors [r*B, (r+1)*B)."""
     return rank * batch

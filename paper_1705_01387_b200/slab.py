@@ -292,8 +292,9 @@ def connect_ranks(group, dist=None):
     """One slab group per rank, one rank per GPU: every rank publishes CUDA IPC handles of its slabs' vector buffers
     and flag arrays (all_gather_object), opens those of the slabs its own slabs send to, and hands the mapped
     addresses to gpuqt_slab_connect.  The pushes then go straight into the peer GPU's memory over NVLink.
-    Host plumbing only.  (Not exercised in this repository's tests: they run on one GPU, where all slabs live in
-    one group and need no connection.)"""
+    Host plumbing only.  Exercised by tests/test_gpu_slab_ipc.py, which needs two GPUs with peer access and is skipped
+    on a one-GPU box (every box this repository has run on so far: the path below has not executed on hardware yet; the
+    one-GPU tests keep all slabs in one group, which needs no connection -- see DESIGN.md "Multi-GPU")."""
     if dist is None:
         import torch.distributed as dist
     rt, drv = _cuda_libs()

@@ -89,3 +89,15 @@ def test_vector_streams_are_disjoint():
     r1 = L.random_phase_vectors(N, 2, CONFIG, 2)
     assert r1.tobytes() == allv[2:4].tobytes()
     assert not np.array_equal(allv[0], allv[2])
+
+
+def test_bench_starts_its_own_ranks():
+    """bench.py --gpus N outside torchrun re-executes itself as N ranks with the contract's launch line."""
+    from paper_1705_01387_b200 import replicas
+    assert not replicas.needs_launch(1, env={})
+    assert replicas.needs_launch(8, env={})
+    assert not replicas.needs_launch(8, env={"WORLD_SIZE": "8"})
+    cmd = replicas.launch_command("/x/bench.py", ["--gpus", "4", "--steps", "2"], 4, 29512, python="python")
+    assert cmd == ["python", "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=4", "--master-addr", "127.0.0.1",
+                   "--master-port", "29512", "/x/bench.py", "--gpus", "4", "--steps", "2"]
+    assert 1024 < replicas.free_port() < 65536
