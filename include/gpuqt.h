@@ -297,6 +297,16 @@ int gpuqt_running_conductivity(gpuqt_handle* h, int kind, const double* corr_hos
                                const double* dt_host, int32_t n_times, int32_t n_energies, double* sigma_host,
                                double* length_host);
 
+/* Localization length xi(E) = lim_{t -> inf} L(E, t) / (2 pi)  (Eq. 12) from the propagating length
+ * L(E, t) of Eq. 11 (the `length` output of gpuqt_running_conductivity, kind GPUQT_SIGMA_FROM_MSD).  The limit is read as
+ * the last measured time [A27]:  xi[j] = length[n_times - 1][j] / (2 pi).  Eq. 12 holds once L has saturated
+ * (PAPER.md:125); whether it has is reported as growth[j] = (L[n_times-1][j] - L[n_times-2][j]) / L[n_times-1][j], the
+ * relative change over the last step (0 where L[n_times-1][j] == 0; 1 with a single row) -- the caller decides how small
+ * is small enough.  length_host: host [n_times][n_energies]; xi_host, growth_host: host [n_energies]; growth_host may
+ * be NULL.                                                                                                       */
+int gpuqt_localization_length(gpuqt_handle* h, const double* length_host, int32_t n_times, int32_t n_energies,
+                              double* xi_host, double* growth_host);
+
 /* Copy a state back: host [batch][N][2].                                                          */
 int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host);
 

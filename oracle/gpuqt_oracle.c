@@ -542,3 +542,24 @@ int oracle_running_conductivity(int kind, const double *in, const double *dos, c
     }
     return ORACLE_OK;
 }
+
+/* Localization length from the propagating length (Eq. 12):  xi(E_j) = lim_t L(E_j, t) / (2 pi).
+ * The limit is read as the LAST measured time [A27]:  xi[j] = length[n_t - 1][j] / (2 pi), and the saturation that
+ * Eq. 12 presupposes ("the propagating length will finally saturate") is reported beside it as the
+ * relative change of L over the last step,  growth[j] = (L[n_t-1][j] - L[n_t-2][j]) / L[n_t-1][j]
+ * (0 where L[n_t-1][j] == 0; 1 when there is only one row: nothing is known about saturation).  growth may be NULL. */
+int oracle_localization_length(const double *length, int32_t n_t, int32_t n_e, double *xi, double *growth)
+{
+    if (!length || !xi || n_t < 1 || n_e < 1) return ORACLE_ERR_ARG;
+    const double two_pi = 2.0 * 3.14159265358979323846;
+    for (int32_t j = 0; j < n_e; ++j) {
+        double last = length[(size_t)(n_t - 1) * n_e + j];
+        xi[j] = last / two_pi;
+        if (growth) {
+            if (last == 0.0) growth[j] = 0.0;
+            else if (n_t == 1) growth[j] = 1.0;
+            else growth[j] = (last - length[(size_t)(n_t - 2) * n_e + j]) / last;
+        }
+    }
+    return ORACLE_OK;
+}

@@ -191,3 +191,13 @@ def running_conductivity(kind, corr, dos, dt):
     _check(lib().oracle_running_conductivity(C.c_int(0 if kind == "vac" else 1), _d(corr), _d(dos_a), _d(dt),
                                              C.c_int32(n_t), C.c_int32(n_e), _d(sigma), _d(length)), "running_conductivity")
     return sigma, length
+
+
+def localization_length(length):
+    """oracle_localization_length: length [n_t][n_E] (Eq. 11) -> (xi [n_E] of Eq. 12 at the last time, growth [n_E])."""
+    length = np.ascontiguousarray(length, np.float64)
+    n_t, n_e = length.shape
+    xi, growth = np.empty(n_e), np.empty(n_e)
+    _check(lib().oracle_localization_length(_d(length), C.c_int32(n_t), C.c_int32(n_e), _d(xi), _d(growth)),
+           "localization_length")
+    return xi, growth

@@ -76,6 +76,7 @@ _SIGNATURES = {
                                              C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]),
     "gpuqt_get_info": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "gpuqt_running_conductivity": (C.c_int, [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int32, C.c_int32, _dp, _dp]),
+    "gpuqt_localization_length": (C.c_int, [C.c_void_p, _dp, C.c_int32, C.c_int32, _dp, _dp]),
     "gpuqt_get_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "gpuqt_get_table": (C.c_int, [C.c_void_p, _ip, _dp, _dp, _dp]),
     "gpuqt_bessel_coeffs": (C.c_int, [C.c_double, C.c_double, C.c_int32, _dp, _dp]),
@@ -354,6 +355,15 @@ class GpuQT:
                                                    C.c_int32(n_t), C.c_int32(n_e), _d(sigma), _d(length)),
                  "gpuqt_running_conductivity")
         return sigma, length
+
+    def localization_length(self, length):
+        """gpuqt_localization_length: length [n_t][n_E] (Eq. 11) -> (xi [n_E] of Eq. 12 at the last time, growth [n_E])."""
+        length = np.ascontiguousarray(length, np.float64)
+        n_t, n_e = length.shape
+        xi, growth = np.empty(n_e), np.empty(n_e)
+        self._ck(load().gpuqt_localization_length(self._h, _d(length), C.c_int32(n_t), C.c_int32(n_e), _d(xi), _d(growth)),
+                 "gpuqt_localization_length")
+        return xi, growth
 
     # ---- timing
     def kernel_stats(self, cls):

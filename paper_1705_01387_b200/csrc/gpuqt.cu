@@ -1147,6 +1147,26 @@ int gpuqt_running_conductivity(gpuqt_handle* h, int kind, const double* corr_hos
     return GPUQT_OK;
 }
 
+int gpuqt_localization_length(gpuqt_handle* h, const double* length_host, int32_t n_times, int32_t n_energies,
+                              double* xi_host, double* growth_host) {
+    if (!h || !length_host || !xi_host || n_times < 1 || n_energies < 1) return fail(h, GPUQT_ERR_ARG, "null or non-positive argument");
+    const size_t bl = (size_t)n_times * n_energies * sizeof(double), be = (size_t)n_energies * sizeof(double);
+    const size_t ol = 0, ox = align_up(bl), og = ox + align_up(be), tot = og + align_up(be);
+    CU(ensure_scratch(h, tot));
+    char* s = h->scratch;
+    cudaError_t e = cudaMemcpyAsync(s + ol, length_host, bl, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+        localization_kernel<<<(n_energies + 127) / 128, 128, 0, h->stream>>>(n_times, n_energies, (const double*)(s + ol),
+                                                                             (double*)(s + ox), growth_host ? (double*)(s + og) : nullptr);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(xi_host, s + ox, be, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && growth_host) e = cudaMemcpyAsync(growth_host, s + og, be, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "localization_length");
+    return GPUQT_OK;
+}
+
 int gpuqt_get_state(gpuqt_handle* h, int which, double* out_host) {
     if (!h || !out_host) return fail(h, GPUQT_ERR_ARG, "null argument");
     const double2* src = which == GPUQT_STATE_PSI ? h->psi : which == GPUQT_STATE_CHI ? h->chi

@@ -1422,6 +1422,17 @@ __global__ void conductivity_kernel(int kind, int n_t, int n_e, const double* __
     }
 }
 
+// Localization length (Eq. 12) from the propagating length of Eq. 11, the limit read as the last measured
+// time [A27]: xi[j] = L[n_t-1][j] / (2 pi); growth[j] = relative change of L over the last step (the saturation check).
+__global__ void localization_kernel(int n_t, int n_e, const double* __restrict__ length, double* __restrict__ xi,
+                                    double* __restrict__ growth) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_e) return;
+    const double last = length[(size_t)(n_t - 1) * n_e + j];
+    xi[j] = last / (2.0 * 3.14159265358979323846);
+    if (growth) growth[j] = last == 0.0 ? 0.0 : n_t == 1 ? 1.0 : (last - length[(size_t)(n_t - 2) * n_e + j]) / last;
+}
+
 // Decode the packed records back to canonical padded row-major arrays in the CALLER's site numbering (bit-exact
 // check).  new_of_old / old_of_new: the row permutation of a reordered lattice, or nullptr.
 __global__ void decode_table(const Mat m, int32_t* __restrict__ col, double* __restrict__ re,

@@ -48,6 +48,8 @@ def summary(ex, res):
         out["msd_at_0_over_time"] = (res["rho_msd"][:, j0] / res["dos"][j0]).tolist()
         out["sigma_msd_at_0"] = res["sigma_msd"][:, j0].tolist()
         out["length_at_0"] = res["length"][:, j0].tolist()
+        out["xi_at_0"] = float(res["xi"][j0])                      # Eq. 12 at the last time; meaningful once xi_growth ~ 0
+        out["xi_growth_at_0"] = float(res["xi_growth"][j0])
     return out
 
 

@@ -23,7 +23,8 @@ def run(engine, phi, dts, n_moments, energies, order_of, vac=True, msd=True, per
     Row conventions [A4]: VAC row k is measured at t_k BEFORE step k (N_t rows, the last evolution of
     the VAC branches is skipped only if MSD is off); MSD row k is measured at t_{k+1} AFTER step k.
     Returns a dict of arrays averaged over the B vectors: dos [n_E], rho_vac / rho_msd [N_t][n_E]
-    (= rho C_vv, rho dX^2), sigma_vac (at t_k), sigma_msd (at the middle of step k), length (Eq. 11).
+    (= rho C_vv, rho dX^2), sigma_vac (at t_k), sigma_msd (at the middle of step k), length (Eq. 11), xi (Eq. 12 read
+    at the last time) with xi_growth (relative change of the length over the last step: the saturation check).
     With per_vector=True nothing is averaged and no conductivity is formed: dos [B][n_E], rho_vac /
     rho_msd [N_t][B][n_E] -- the rows of the paper's dos.out / vac.out / msd.out.
     """
@@ -52,6 +53,7 @@ def run(engine, phi, dts, n_moments, energies, order_of, vac=True, msd=True, per
         out["sigma_vac"], _ = engine.running_conductivity("vac", out["rho_vac"], dos, dts[:len(dts) - 1])
     if msd:
         out["sigma_msd"], out["length"] = engine.running_conductivity("msd", out["rho_msd"], dos, dts)
+        out["xi"], out["xi_growth"] = engine.localization_length(out["length"])
     return out
 
 

@@ -47,6 +47,7 @@ def simulation_loop(oracle_mod, model, phi, dts, n_moments, energies, vac, msd):
     if msd:
         res["rho_msd"] = np.array(rows_m)
         res["sigma_msd"], res["length"] = oracle_mod.running_conductivity("msd", res["rho_msd"], res["dos"], np.asarray(dts, float))
+        res["xi"], res["xi_growth"] = oracle_mod.localization_length(res["length"])
     o.close()
     return res
 

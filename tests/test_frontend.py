@@ -81,6 +81,9 @@ class _OracleEngine:
     def running_conductivity(self, kind, corr, dos, dt):
         return self.mod.running_conductivity(kind, corr, dos, dt)
 
+    def localization_length(self, length):
+        return self.mod.localization_length(length)
+
 
 def test_run_folder_and_driver_file(tmp_path, oracle_mod, monkeypatch):
     """run_folder writes one dos row and N_t vac / msd rows per random vector, appends on a second run, and

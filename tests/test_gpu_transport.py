@@ -44,6 +44,11 @@ def test_running_conductivity_parity(gq, oracle_mod):
             if kind == "msd":
                 assert rel(l_got, l_ref) <= 1e-14
                 assert np.all(l_got[:, 0] == 0.0)
+                # Eq. 12 on top of it: xi at the last time and the saturation check, element by element
+                xi_ref, gr_ref = oracle_mod.localization_length(l_ref)
+                xi_got, gr_got = g.localization_length(l_ref)
+                assert np.array_equal(xi_got, xi_ref) and np.allclose(gr_got, gr_ref, rtol=1e-14, atol=0)
+                assert xi_got[0] == 0.0 and gr_got[0] == 0.0
     with pytest.raises(gq.GpuqtError):
         g.running_conductivity("msd", np.ones((2, 2)), None, np.array([0.1, -0.1]))
     g.close()
@@ -72,6 +77,8 @@ def test_paper_examples_reduced(gq, oracle_mod, key, scale):
         # rounding-level numbers, so it is compared where it is conditioned, rho > 1e-3 max rho
         ok = ref["dos"] > 1e-3 * np.max(ref["dos"])
         assert rel(got["length"][:, ok], ref["length"][:, ok]) <= TOL
+        assert rel(got["xi"][ok], ref["xi"][ok]) <= TOL                     # Eq. 12 at the last time [A27]
+        assert np.max(np.abs(got["xi_growth"][ok] - ref["xi_growth"][ok])) <= 1e-8      # a difference of two lengths / L
     # what the paper says about its figures, on quantities that are exact for any size:
     E = ex.energies()
     assert abs(np.trapezoid(got["dos"], E) - 2.0) < 0.02                    # int rho dE = 2 per site (spin factor, Eq. 4)

@@ -454,6 +454,30 @@ def test_running_conductivity_closed_forms(oracle_mod):
     assert np.max(np.abs(sig_v_mid - sig_m[:, 0])) <= 1e-4 * exact[-1]
 
 
+def test_localization_length_pins(oracle_mod):
+    """oracle_localization_length (Eq. 12, reading A27) against hand values, an exact plateau and a saturating series."""
+    # hand values: L_last = (2 pi, 8 pi), L_prev = (2 pi, 4 pi)  ->  xi = (1, 4), growth = (0, 1/2)
+    xi, gr = oracle_mod.localization_length(np.array([[2 * np.pi, 4 * np.pi], [2 * np.pi, 8 * np.pi]]))
+    assert np.allclose(xi, [1.0, 4.0], rtol=1e-15) and np.array_equal(gr, [0.0, 0.5])
+    # an exact plateau gives xi exactly and zero growth, whatever came before it
+    L0 = np.array([0.3, 17.0, 1e-9])
+    series = np.vstack([np.linspace(0, 1, 9)[:, None] * L0[None, :], L0[None, :], L0[None, :]])
+    xi, gr = oracle_mod.localization_length(series)
+    assert np.array_equal(xi, L0 / (2.0 * np.pi)) and np.array_equal(gr, np.zeros(3))
+    # a saturating length L(t) = Linf (1 - exp(-t/tau)): xi -> Linf / 2 pi from below, growth -> 0 as exp(-t/tau) dt/tau
+    t = np.arange(1, 41) * 0.5
+    Linf, tau = 12.0, 2.0
+    xi, gr = oracle_mod.localization_length((Linf * (1.0 - np.exp(-t / tau)))[:, None])
+    assert 0.0 < Linf / (2 * np.pi) - xi[0] < 1e-4 * Linf
+    assert 0.0 < gr[0] < 1.5e-5
+    # a length that still grows linearly (ballistic) is flagged by its growth = dt / t_last
+    xi, gr = oracle_mod.localization_length((2.0 * t)[:, None])
+    assert np.isclose(gr[0], 0.5 / t[-1], rtol=1e-12) and np.isclose(xi[0], 2.0 * t[-1] / (2 * np.pi), rtol=1e-15)
+    # degenerate rows: a single time (nothing known about saturation), a vanishing length
+    xi, gr = oracle_mod.localization_length(np.array([[5.0, 0.0]]))
+    assert np.allclose(xi, [5.0 / (2 * np.pi), 0.0]) and np.array_equal(gr, [1.0, 0.0])
+
+
 def test_running_conductivity_on_a_lattice(oracle_mod):
     """The two routes to sigma(E, t) agree on a clean periodic chain with a plane-wave state, where both
     correlation functions are known exactly: rho C_vv = rho v_k^2, rho dX^2 = rho v_k^2 t^2."""

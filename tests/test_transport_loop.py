@@ -22,6 +22,9 @@ class OracleEngine:
     def running_conductivity(self, kind, corr, dos, dt):
         return self.mod.running_conductivity(kind, corr, dos, dt)
 
+    def localization_length(self, length):
+        return self.mod.localization_length(length)
+
 
 def test_rows_are_at_the_times_of_reading_a4(oracle_mod):
     """phi = e^{ikx} on a clean ring: rho C_vv(t) = rho v_k^2 at every t, rho dX^2(t) = rho v_k^2 t^2.  With
