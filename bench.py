@@ -144,24 +144,41 @@ def load_traffic():
     return t, False
 
 
-def measure_l2_copy_gbs(torch, stream, mbytes=24, reps=200):
-    """L2-resident copy rate for the configs whose recurrence step lives in the L2: a device-to-device copy of
-    `mbytes` MB (source + destination = 2 x 24 MB, well inside the 126 MB L2) repeated back to back on the bench
-    stream, read + write bytes over the CUDA-event time of `reps` copies after 20 warm-up copies.  torch's copy
-    kernel serves as the yardstick only (as in MEASURED_PEAKS.json); it is not on the measured path."""
-    n = mbytes * 1000 * 1000 // 8
-    a = torch.ones(n, dtype=torch.float64, device="cuda")
-    b = torch.empty_like(a)
+def measure_l2_gbs(torch, stream, reps=100):
+    """L2-resident data rates for the configs whose recurrence step lives (partly) in the L2, measured in this run on
+    the bench stream with CUDA events over `reps` back-to-back launches after 10 warm-up launches.  Candidates:
+    device-to-device copies (read + write bytes) and read-only reductions (read bytes) over buffers that fit the 126 MB
+    L2 with room to spare.  torch's copy / sum kernels serve as yardsticks only (as in MEASURED_PEAKS.json); they are
+    not on the measured path.  Returns (best rate, {candidate: rate}): the best is the yardstick -- a LOWER bound of
+    what the L2 can deliver (short launches, generic kernels), not a hardware ceiling."""
+    out = {}
+
+    def rate(fn, nbytes):
+        with torch.cuda.stream(stream):
+            for _ in range(10):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream)
+            stream.synchronize()
+        return nbytes * reps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
+    for mb in (24, 40):
+        n = mb * 1000 * 1000 // 8
+        with torch.cuda.stream(stream):
+            a = torch.ones(n, dtype=torch.float64, device="cuda")
+            b = torch.empty_like(a)
+        out[f"copy_2x{mb}MB"] = rate(lambda: b.copy_(a), 2.0 * n * 8)
+        del b
+        out[f"sum_{mb}MB"] = rate(lambda: a.sum(), 1.0 * n * 8)
+        del a
     with torch.cuda.stream(stream):
-        for _ in range(20):
-            b.copy_(a)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(reps):
-            b.copy_(a)
-        e1.record(stream)
-        stream.synchronize()
-    return 2.0 * n * 8 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        a = torch.ones(80 * 1000 * 1000 // 8, dtype=torch.float64, device="cuda")
+    out["sum_80MB"] = rate(lambda: a.sum(), 80e6)
+    del a
+    return max(out.values()), out
 
 
 def residency(wset, stored, traffic):
@@ -374,10 +391,10 @@ def run_ours(args, w):
         names = {0: "kpm_doubling", 1: "kpm_left", 2: "evolve", 3: "evolve_msd"}
         peak, peak_src = load_peak()
         traffic_table, traffic_stale = load_traffic()
-        l2_peak = None
+        l2_peak, l2_candidates = None, None
 
         def entry(c):
-            nonlocal l2_peak
+            nonlocal l2_peak, l2_candidates
             kernel = names[c]
             c_ms, c_steps, c_launches = stats[c]
             step_s = c_ms * 1e-3 / max(c_steps, 1)                 # one recurrence step of that kernel
@@ -399,11 +416,17 @@ def run_ours(args, w):
                           "dram_frac_from_ncu_traffic": (traffic / step_s / 1e9 / peak) if traffic else None})
             else:           # the step is served (partly) from the L2: an HBM fraction would exceed 1 and say nothing
                 if l2_peak is None:
-                    l2_peak = measure_l2_copy_gbs(torch, stream)
-                e.update({"bound": "l2", "peak": l2_peak, "frac": achieved / l2_peak,
-                          "peak_source": "measured in this run: L2-resident device copy, 2 x 24 MB, read + write bytes, 200 "
-                                         "back-to-back copies (bench.py measure_l2_copy_gbs)",
-                          "hbm_peak": peak, "hbm_peak_source": peak_src})
+                    l2_peak, l2_candidates = measure_l2_gbs(torch, stream)
+                frac = achieved / l2_peak
+                e.update({"bound": "l2", "peak": l2_peak, "frac": frac if frac <= 1.0 else None,
+                          "peak_source": "measured in this run: the best of the L2-resident copy / read-only reduction rates "
+                                         "in l2_yardsticks_gbs (bench.py measure_l2_gbs; torch kernels as yardsticks, a lower "
+                                         "bound of the L2's rate, not a hardware ceiling)",
+                          "l2_yardsticks_gbs": l2_candidates, "hbm_peak": peak, "hbm_peak_source": peak_src,
+                          "dram_share_of_stored_bytes": (traffic / stored) if traffic else None})
+                if frac > 1.0:
+                    e["frac_note"] = ("the kernel moves its stored bytes %.2f x faster than the best L2 yardstick of this run: "
+                                      "no ceiling is known for this step, so no fraction is quoted" % frac)
             return e
 
         big = sorted((c for c in names if stats[c][0] >= 0.05 * ms), key=lambda c: -stats[c][0]) or [max(names, key=lambda c: stats[c][0])]
